@@ -1,0 +1,125 @@
+/*
+ * shd.h -- C-ABI boundary of the B200-native stealthy-hyperuniform hot path
+ *          (arXiv:2304.09139, Morse, Kim, Steinhardt, Torquato).
+ *
+ * "P:n" = /root/reference/PAPER.md line n.  "D:Rn" = reading n in DESIGN.md.
+ *
+ * What the library computes (one periodic box [0,L)^d, N point particles):
+ *   Q      = { n in Z^d : 0 < n.n <= m_star, first non-zero component of n positive }   (D:R6-R8)
+ *            wavevector k = 2 pi n / L; canonical order = lexicographic ascending, n_0 slowest (D:R7)
+ *   rho(k) = sum_j exp(+i k.r_j)               (= complex conjugate of n~(k), Eq. 4; D:R1)
+ *   Phi    = sum_{k in Q} v(k) |rho(k)|^2      (Eq. 2 P:39 with the structure-independent constant dropped; D:R3)
+ *   S_max  = max_{k in Q} |rho(k)|^2 / N       (Eq. 1 P:27 with Eq. 3; inclusive cutoff D:R4)
+ *   grad   = dPhi/dr_{j,a} = (4 pi / L) sum_{k in Q} v(k) n_a Im[ exp(-i k.r_j) rho(k) ]
+ *            (= -F_j of Eq. 6; the true derivative, D:R2)
+ * all in double-double (~106-bit) accuracy ("tunable precision using double-doubles").
+ *
+ * Conventions
+ *   - Every function returns int: SHD_OK (0) or a negative SHD_E* code; nothing throws.
+ *   - pos_*, grad_*, and the four shd_get_rho outputs are DEVICE pointers (cudaMalloc'ed memory,
+ *     e.g. torch tensors' data_ptr()), owned by the caller, never retained after the call returns.
+ *     Everything else (phi, smax, n_out, v, reports) is HOST memory.
+ *   - dd values are (hi, lo) pairs of doubles, value = hi + lo.  Layout of particle vectors is
+ *     SoA axis-major: x[a*N + j] = component a of particle j  (two arrays: *_hi and *_lo).
+ *     Any finite position is valid (Phi is L-periodic, D:R10); |lo| <= ulp(hi)/2 is expected.
+ *   - Work is enqueued on the handle's stream; calls that return a scalar synchronise that stream.
+ *   - A handle is not thread-safe; different handles are independent.  No global state.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns SHD_ECUDA.
+ */
+#ifndef SHD_H
+#define SHD_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SHD_OK        0
+#define SHD_EINVAL   -1   /* bad d / N / L / K / m_star / NULL pointer / option            */
+#define SHD_ENOMEM   -2   /* host or device allocation failed                              */
+#define SHD_ECUDA    -3   /* CUDA runtime error; text in shd_last_error()                  */
+#define SHD_ENAN     -4   /* non-finite position or non-finite Phi                         */
+#define SHD_ESTALL   -5   /* shd_minimize: line search found no decrease (report written)  */
+#define SHD_EMAXEVAL -6   /* shd_minimize: max_evals reached before smax_tol (report written) */
+
+typedef struct shd_ctx shd_ctx;
+
+/*
+ * Create a handle for dimension d in {1,2,3}, N >= 1 particles, box edge L > 0, cutoff K > 0:
+ *   m_star = floor( (K L / 2 pi)^2 (1 + 2^-40) ),  Q as above  (integer compare, D:R8).
+ * v: HOST pointer to |Q| strictly positive weights v(k) in canonical order, or NULL
+ * for v == 1.  The handle owns all device workspaces (phasor tables, rho, partial sums, minimizer
+ * state).  *out receives the handle.  Errors: SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA.
+ */
+int shd_create(int d, long N, double L, double K, const double* v, shd_ctx** out);
+
+/* Same, with the integer shell cutoff n.n <= m_star given directly (no FP compare, D:R8). */
+int shd_create_shell(int d, long N, double L, long m_star, const double* v, shd_ctx** out);
+
+void shd_destroy(shd_ctx* h);
+
+/* Use CUDA stream `cuda_stream` (a cudaStream_t) for all later work; default is stream 0. */
+int shd_set_stream(shd_ctx* h, void* cuda_stream);
+
+/* |Q| = M, the number of independent constraints. */
+long shd_num_k(const shd_ctx* h);
+
+/* Copy the integer vectors n of Q to HOST n_out[|Q|*d], row-major (k, a), canonical order. */
+int shd_get_k(const shd_ctx* h, int* n_out);
+
+/*
+ * One energy + gradient evaluation (Eq. 4, 2, 6; "2 calculations, each with M N terms").
+ *   pos_hi, pos_lo : DEVICE, d*N doubles each (in).
+ *   phi            : HOST, phi[0] = hi, phi[1] = lo (out).
+ *   grad_hi, grad_lo: DEVICE, d*N doubles each (out); both NULL to skip the gradient pass.
+ * Side effect: rho(k) of these positions stays in the handle (shd_get_rho), as do S_max and
+ * its argmax (shd_last_smax).
+ */
+int shd_energy_grad(shd_ctx* h, const double* pos_hi, const double* pos_lo,
+                    double phi[2], double* grad_hi, double* grad_lo);
+
+/* S_max (Eq. 1) of the given positions: smax[0..1] = (hi, lo) on the HOST, *argmax_k = index
+ * into the canonical order (may be NULL).  Runs the rho pass and the reduction only. */
+int shd_smax(shd_ctx* h, const double* pos_hi, const double* pos_lo, double smax[2], long* argmax_k);
+
+/* S_max / argmax of the LAST evaluation on this handle (no device work besides a 32-byte copy). */
+int shd_last_smax(shd_ctx* h, double smax[2], long* argmax_k);
+
+/* rho(k) of the LAST evaluation: four DEVICE arrays of |Q| doubles each, canonical order. */
+int shd_get_rho(shd_ctx* h, double* re_hi, double* re_lo, double* im_hi, double* im_lo);
+
+typedef struct {
+    int    kind;        /* 0 = L-BFGS (D:R12); 1 = FIRE                               */
+    int    history;     /* L-BFGS pairs kept (1..32); 0 = default 10                          */
+    double smax_tol;    /* stop when S_max < smax_tol (D:R13); e.g. 1e-30                     */
+    long   max_evals;   /* stop after this many energy+gradient evaluations                   */
+    int    poll_every;  /* host reads the device status word every this many iterations (>=1) */
+} shd_min_opts;
+
+typedef struct {
+    long   iters, evals;
+    double phi[2], smax[2];
+    int    status;      /* SHD_OK, SHD_ESTALL, SHD_EMAXEVAL, SHD_ENAN */
+} shd_min_report;
+
+/*
+ * Quench: minimise Phi from pos (DEVICE, in/out, d*N doubles each) until S_max < smax_tol.
+ * The whole iteration (evaluations, dd vector algebra, line search decisions) runs on the device;
+ * the host only polls a status word every poll_every iterations.  Re-entrant: call again to
+ * continue.  Returns report->status.
+ */
+int shd_minimize(shd_ctx* h, double* pos_hi, double* pos_lo, const shd_min_opts* opts,
+                 shd_min_report* report);
+
+/* Text of the last error on this handle (never NULL). */
+const char* shd_last_error(const shd_ctx* h);
+
+/* Introspection used by bench.py / tests (host scalars):
+ *   what = 0: FP64 instructions (DFMA/DADD/DMUL) the last shd_energy_grad issued per launch model,
+ *   what = 1: number of kernel launches of the last call, 2: padded cell count of the rho pass,
+ *   3: valid cell count, 4: bytes of device workspace. */
+double shd_stat(const shd_ctx* h, int what);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SHD_H */

@@ -1,0 +1,201 @@
+// k_finish.cu -- step a3: sum the per-split partials in fixed order, form rho(k), |rho|^2,
+// Phi = sum_k v_k |rho(k)|^2 (Eq. 2), S_max = max_k |rho(k)|^2 / N (Eq. 1) and its
+// argmax, all in double-double and bit-reproducible (fixed reduction trees, no atomics);
+// then build the limb-split gradient operand C[p,q] from W = v rho (Eq. 6).
+#include "dd.cuh"
+#include "shd_internal.h"
+
+namespace {
+
+struct red { dd phi; dd smax; long long arg; double maxvs; };
+
+__device__ __forceinline__ red red_combine(red a, red b) {
+    red r;
+    r.phi = dd_add(a.phi, b.phi);
+    // larger |rho|^2 wins; ties go to the lower canonical index; arg < 0 marks "empty"
+    bool takeb = b.arg >= 0 && (a.arg < 0 || dd_less(a.smax, b.smax) ||
+                                (!dd_less(b.smax, a.smax) && b.arg < a.arg));
+    r.smax = takeb ? b.smax : a.smax;
+    r.arg = takeb ? b.arg : a.arg;
+    r.maxvs = fmax(a.maxvs, b.maxvs);
+    return r;
+}
+__device__ __forceinline__ red red_shfl(red a, int off) {
+    red b;
+    b.phi.h = __shfl_down_sync(0xffffffffu, a.phi.h, off);
+    b.phi.l = __shfl_down_sync(0xffffffffu, a.phi.l, off);
+    b.smax.h = __shfl_down_sync(0xffffffffu, a.smax.h, off);
+    b.smax.l = __shfl_down_sync(0xffffffffu, a.smax.l, off);
+    b.arg = __shfl_down_sync(0xffffffffu, a.arg, off);
+    b.maxvs = __shfl_down_sync(0xffffffffu, a.maxvs, off);
+    return b;
+}
+__device__ red block_reduce(red v) {
+    __shared__ red sh[32];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v = red_combine(v, red_shfl(v, off));
+    int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) sh[w] = v;
+    __syncthreads();
+    int nw = (blockDim.x + 31) >> 5;
+    if (w == 0) {
+        red z; z.phi = dd{0, 0}; z.smax = dd{-1, 0}; z.arg = -1; z.maxvs = 0;
+        v = l < nw ? sh[l] : z;
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) v = red_combine(v, red_shfl(v, off));
+    }
+    return v;   // valid in thread 0
+}
+
+__device__ __forceinline__ void account(red& r, dd re, dd im, double v, long long k) {
+    dd s = dd_add(dd_mul(re, re), dd_mul(im, im));
+    r.phi = dd_add(r.phi, dd_mul_d(s, v));
+    if (r.arg < 0 || dd_less(r.smax, s) || (!dd_less(s, r.smax) && k < r.arg)) { r.smax = s; r.arg = k; }
+    r.maxvs = fmax(r.maxvs, v * v * s.h);
+}
+
+// one thread per (tile, cell)
+__global__ void __launch_bounds__(256) k_finish1(
+    const double* __restrict__ part, int nsplit, int ntiles, const int* __restrict__ tile_pb,
+    const int* __restrict__ tile_qb, const int* __restrict__ cell_kp, const int* __restrict__ cell_km,
+    int Qpad, long M, const double* __restrict__ v, double* __restrict__ rho, double* __restrict__ blockred)
+{
+    long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    red r; r.phi = dd{0, 0}; r.smax = dd{-1, 0}; r.arg = -1; r.maxvs = 0;
+    if (idx < (long)ntiles * 1024) {
+        int tile = (int)(idx >> 10), cell = (int)(idx & 1023);
+        int p = tile_pb[tile] * 32 + (cell >> 5), q = tile_qb[tile] * 32 + (cell & 31);
+        int kp = cell_kp[(size_t)p * Qpad + q], km = cell_km[(size_t)p * Qpad + q];
+        if (kp >= 0 || km >= 0) {
+            const double2* src = reinterpret_cast<const double2*>(part);
+            dd X[4];
+#pragma unroll
+            for (int x = 0; x < 4; x++) {
+                dd acc = dd{0, 0};
+                for (int s = 0; s < nsplit; s++) {
+                    double2 t = src[((size_t)(s * (long)ntiles + tile) * 4 + x) * 1024 + cell];
+                    acc = dd_add(acc, dd{t.x, t.y});
+                }
+                X[x] = acc;
+            }
+            if (kp >= 0) {
+                dd re = dd_sub(X[0], X[1]), im = dd_add(X[2], X[3]);
+                rho[kp] = re.h; rho[M + kp] = re.l; rho[2 * M + kp] = im.h; rho[3 * M + kp] = im.l;
+                account(r, re, im, v ? v[kp] : 1.0, kp);
+            }
+            if (km >= 0) {
+                dd re = dd_add(X[0], X[1]), im = dd_sub(X[3], X[2]);
+                rho[km] = re.h; rho[M + km] = re.l; rho[2 * M + km] = im.h; rho[3 * M + km] = im.l;
+                account(r, re, im, v ? v[km] : 1.0, km);
+            }
+        }
+    }
+    r = block_reduce(r);
+    if (threadIdx.x == 0) {
+        double* o = blockred + (size_t)blockIdx.x * 8;
+        o[0] = r.phi.h; o[1] = r.phi.l; o[2] = r.smax.h; o[3] = r.smax.l;
+        o[4] = (double)r.arg; o[5] = r.maxvs;
+    }
+}
+
+__global__ void __launch_bounds__(1024) k_finish2(const double* __restrict__ blockred, int nblocks, long N,
+                                                  shd_scalars* __restrict__ scal)
+{
+    red r; r.phi = dd{0, 0}; r.smax = dd{-1, 0}; r.arg = -1; r.maxvs = 0;
+    for (int b = threadIdx.x; b < nblocks; b += blockDim.x) {
+        const double* o = blockred + (size_t)b * 8;
+        red t; t.phi = dd{o[0], o[1]}; t.smax = dd{o[2], o[3]}; t.arg = (long long)o[4]; t.maxvs = o[5];
+        r = red_combine(r, t);
+    }
+    r = block_reduce(r);
+    if (threadIdx.x == 0) {
+        dd sm = dd_div_d(r.smax, (double)N);
+        scal->phi[0] = r.phi.h; scal->phi[1] = r.phi.l;
+        scal->smax[0] = sm.h; scal->smax[1] = sm.l;
+        scal->argmax = r.arg;
+        scal->maxvs = r.maxvs;
+        double mw = sqrt(r.maxvs);
+        // |C components| <= 2 max|v rho| < 2^(ilogb(mw)+2)
+        scal->cscale = (mw > 0.0 && isfinite(mw)) ? ldexp(1.0, -(ilogb(mw) + 2)) : 1.0;
+        scal->nonfinite = (isfinite(r.phi.h) && isfinite(r.smax.h)) ? 0 : 1;
+    }
+}
+
+struct limbs { double x0, x1, x2, x12; };
+__device__ __forceinline__ limbs split_limbs(dd x) {
+    const double C0 = 1.5 * 4503599627370496.0 / (double)(1 << SHD_W0);
+    const double C1 = 1.5 * 4503599627370496.0 / ((double)(1 << SHD_W0) * (double)(1 << SHD_W1));
+    limbs r;
+    r.x0 = __dadd_rn(__dadd_rn(x.h, C0), -C0);
+    double rem = __dadd_rn(x.h, -r.x0);
+    r.x1 = __dadd_rn(__dadd_rn(rem, C1), -C1);
+    r.x2 = __dadd_rn(__dadd_rn(rem, -r.x1), x.l);
+    r.x12 = __dadd_rn(r.x1, r.x2);
+    return r;
+}
+
+// C[p,q]: C1 = W+ + W-,  C2 = -i (W+ - W-),  W = v rho, scaled by cscale (a power of two).
+// layout [pb][q][plane 8][32 p][2]; plane l: (C1r_l, C1i_l), plane 4+l: (C2r_l, C2i_l).
+__global__ void __launch_bounds__(256) k_ctable(
+    int npb, int Qpad, const int* __restrict__ cell_kp, const int* __restrict__ cell_km, long M,
+    const double* __restrict__ v, const double* __restrict__ rho, const shd_scalars* __restrict__ scal,
+    double* __restrict__ C)
+{
+    long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    long ncell = (long)npb * 32 * Qpad;
+    if (idx >= ncell) return;
+    // idx enumerates (pb, q, pi) with pi fastest so that stores are coalesced
+    int pi = (int)(idx & 31);
+    long t = idx >> 5;
+    int q = (int)(t % Qpad);
+    int pb = (int)(t / Qpad);
+    int p = pb * 32 + pi;
+    int kp = cell_kp[(size_t)p * Qpad + q], km = cell_km[(size_t)p * Qpad + q];
+    double sc = scal->cscale;
+    dd wpr{0, 0}, wpi{0, 0}, wmr{0, 0}, wmi{0, 0};
+    if (kp >= 0) {
+        double vv = v ? v[kp] : 1.0;
+        wpr = dd_scale2(dd_mul_d(dd{rho[kp], rho[M + kp]}, vv), sc);
+        wpi = dd_scale2(dd_mul_d(dd{rho[2 * M + kp], rho[3 * M + kp]}, vv), sc);
+    }
+    if (km >= 0) {
+        double vv = v ? v[km] : 1.0;
+        wmr = dd_scale2(dd_mul_d(dd{rho[km], rho[M + km]}, vv), sc);
+        wmi = dd_scale2(dd_mul_d(dd{rho[2 * M + km], rho[3 * M + km]}, vv), sc);
+    }
+    dd c1r = dd_add(wpr, wmr), c1i = dd_add(wpi, wmi);
+    dd dr = dd_sub(wpr, wmr), di = dd_sub(wpi, wmi);
+    dd c2r = di, c2i = dd_neg(dr);                 // -i (dr + i di) = di - i dr
+    limbs a = split_limbs(c1r), b = split_limbs(c1i), c = split_limbs(c2r), e = split_limbs(c2i);
+    double* dst = C + ((((size_t)pb * Qpad + q) * 8) * 32 + pi) * 2;
+    *reinterpret_cast<double2*>(dst + 0 * 64) = make_double2(a.x0, b.x0);
+    *reinterpret_cast<double2*>(dst + 1 * 64) = make_double2(a.x1, b.x1);
+    *reinterpret_cast<double2*>(dst + 2 * 64) = make_double2(a.x2, b.x2);
+    *reinterpret_cast<double2*>(dst + 3 * 64) = make_double2(a.x12, b.x12);
+    *reinterpret_cast<double2*>(dst + 4 * 64) = make_double2(c.x0, e.x0);
+    *reinterpret_cast<double2*>(dst + 5 * 64) = make_double2(c.x1, e.x1);
+    *reinterpret_cast<double2*>(dst + 6 * 64) = make_double2(c.x2, e.x2);
+    *reinterpret_cast<double2*>(dst + 7 * 64) = make_double2(c.x12, e.x12);
+}
+
+}  // namespace
+
+cudaError_t shd_launch_finish(shd_ctx* h)
+{
+    int nb = h->nfinish_blocks;
+    k_finish1<<<nb, 256, 0, h->stream>>>(h->d_part, h->nsplit, h->ntiles, h->d_tile_pb, h->d_tile_qb,
+                                         h->d_cell_kp, h->d_cell_km, h->Qpad, h->M, h->d_v, h->d_rho,
+                                         h->d_blockred);
+    k_finish2<<<1, 1024, 0, h->stream>>>(h->d_blockred, nb, h->N, h->d_scal);
+    h->last_launches += 2;
+    return cudaGetLastError();
+}
+
+cudaError_t shd_launch_ctable(shd_ctx* h)
+{
+    long ncell = (long)h->npb * 32 * h->Qpad;
+    k_ctable<<<(unsigned)((ncell + 255) / 256), 256, 0, h->stream>>>(
+        h->npb, h->Qpad, h->d_cell_kp, h->d_cell_km, h->M, h->d_v, h->d_rho, h->d_scal, h->d_C);
+    h->last_launches += 1;
+    return cudaGetLastError();
+}

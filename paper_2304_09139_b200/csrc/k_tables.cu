@@ -1,0 +1,157 @@
+// k_tables.cu -- step a1 of the hot path: per-particle phasor tables in limb form.
+//
+// For every particle j and axis a:  u = r_{j,a} / L to ~160 bits (three-word quotient with exact
+// FMA remainders), z_a = exp(2 pi i frac(u)) by a double-double sincos (256-entry table of roots
+// of unity + Taylor series), then the per-axis integer-power recurrences
+//   A_j[p], B_j[q]  (see shd_internal.h)
+// in complex double-double (TwoProd/TwoSum on FP64 FMA; BASELINE.json north_star item 2), each
+// entry split into limbs and written in the tile-major layouts the rho / gradient kernels stream
+// with TMA bulk copies.
+#include "dd.cuh"
+#include "shd_internal.h"
+#include "sincos_table.inc"
+
+namespace {
+
+// t = frac(m * (hi + lo) / L) as a dd in [-1/2, 1/2], m a power of two
+__device__ dd frac_turns(double hi, double lo, double L, double m) {
+    double q1 = __ddiv_rn(hi, L);
+    double r1 = __fma_rn(-q1, L, hi);            // exact remainder
+    dd se = two_sum(r1, lo);
+    double q2 = __ddiv_rn(se.h, L);
+    double r2 = __fma_rn(-q2, L, se.h);          // exact remainder
+    double q3 = __ddiv_rn(__dadd_rn(r2, se.l), L);
+    double a1 = __dmul_rn(q1, m), a2 = __dmul_rn(q2, m), a3 = __dmul_rn(q3, m);
+    double k = rint(a1);
+    double f1 = __dadd_rn(a1, -k);               // exact
+    dd t = two_sum(f1, a2);
+    t.l = __dadd_rn(t.l, a3);
+    return fast_two_sum(t.h, t.l);
+}
+
+// exp(2 pi i t) for a dd t with |t| <= 1/2 (+ rounding)
+__device__ cdd expi_turns(dd t) {
+    double k = rint(__dmul_rn(t.h, 256.0));
+    dd f = dd_add_d(t, -k * (1.0 / 256.0));      // |f| <= 1/512
+    int idx = ((int)k) & 255;
+    dd th = dd_mul(f, dd{SHD_TWOPI_HI, SHD_TWOPI_LO});
+    dd x = dd_mul(th, th);
+    // cos = sum_{m=0..7} (-1)^m x^m / (2m)!,  sin = th * sum_{m=0..7} (-1)^m x^m / (2m+1)!
+    dd c = dd{SHD_INVFACT[14][0], SHD_INVFACT[14][1]};
+    dd s = dd{SHD_INVFACT[15][0], SHD_INVFACT[15][1]};
+#pragma unroll
+    for (int m = 6; m >= 0; m--) {
+        c = dd_sub(dd{SHD_INVFACT[2 * m][0], SHD_INVFACT[2 * m][1]}, dd_mul(c, x));
+        s = dd_sub(dd{SHD_INVFACT[2 * m + 1][0], SHD_INVFACT[2 * m + 1][1]}, dd_mul(s, x));
+    }
+    s = dd_mul(s, th);
+    cdd w{c, s};
+    cdd root{dd{SHD_ROOTS256[idx][0], SHD_ROOTS256[idx][1]}, dd{SHD_ROOTS256[idx][2], SHD_ROOTS256[idx][3]}};
+    return cdd_mul(root, w);
+}
+
+struct limbs { double x0, x1, x2, x12; };
+
+// |x| <= 1 (normalised dd) -> limbs (shd_internal.h)
+__device__ __forceinline__ limbs split_limbs(dd x) {
+    const double C0 = 1.5 * 4503599627370496.0 / (double)(1 << SHD_W0);                 // 1.5 * 2^(52-W0)
+    const double C1 = 1.5 * 4503599627370496.0 / ((double)(1 << SHD_W0) * (double)(1 << SHD_W1));
+    limbs r;
+    r.x0 = __dadd_rn(__dadd_rn(x.h, C0), -C0);
+    double rem = __dadd_rn(x.h, -r.x0);          // exact
+    r.x1 = __dadd_rn(__dadd_rn(rem, C1), -C1);
+    r.x2 = __dadd_rn(__dadd_rn(rem, -r.x1), x.l);
+    r.x12 = __dadd_rn(r.x1, r.x2);
+    return r;
+}
+
+// write one complex entry (4 limb pairs) at plane stride `ps` doubles
+__device__ __forceinline__ void store_entry(double* base, size_t ps, cdd z) {
+    limbs a = split_limbs(z.re), b = split_limbs(z.im);
+    *reinterpret_cast<double2*>(base) = make_double2(a.x0, b.x0);
+    *reinterpret_cast<double2*>(base + ps) = make_double2(a.x1, b.x1);
+    *reinterpret_cast<double2*>(base + 2 * ps) = make_double2(a.x2, b.x2);
+    *reinterpret_cast<double2*>(base + 3 * ps) = make_double2(a.x12, b.x12);
+}
+
+constexpr int R3MAX = 128;   // d == 3: max |n_1| supported by the local power table
+
+// which = 0: A table.  which = 1: B table (+ gradient-layout Bg with q-weighted copy).
+__global__ void __launch_bounds__(128) k_tables(
+    int d, long N, double L, long Npad, int P, int Qn, int S1d, int qscale_log2,
+    const int* __restrict__ pn0, const int* __restrict__ pn1, int Qpad,
+    const double* __restrict__ pos_hi, const double* __restrict__ pos_lo,
+    double* __restrict__ A, double* __restrict__ B, double* __restrict__ Bg, int with_grad)
+{
+    long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    int which = blockIdx.y;
+    if (j >= N) return;
+    const cdd one{dd{1.0, 0.0}, dd{0.0, 0.0}};
+    if (which == 0) {
+        // ---- A table
+        cdd base;
+        if (d == 1) base = expi_turns(frac_turns(pos_hi[j], pos_lo[j], L, (double)S1d));
+        else base = expi_turns(frac_turns(pos_hi[j], pos_lo[j], L, 1.0));
+        if (d <= 2) {
+            cdd cur = one;
+            for (int p = 0; p < P; p++) {
+                int pb = p >> 5, pi = p & 31;
+                double* dst = A + ((((size_t)pb * Npad + j) * 4) * 32 + pi) * 2;
+                store_entry(dst, 64, cur);
+                cur = cdd_mul(cur, base);
+            }
+        } else {
+            cdd z1 = expi_turns(frac_turns(pos_hi[N + j], pos_lo[N + j], L, 1.0));
+            cdd pw1[R3MAX + 1];
+            int r1max = 0;
+            for (int p = 0; p < P; p++) { int a = abs(pn1[p]); r1max = a > r1max ? a : r1max; }
+            pw1[0] = one;
+            for (int m = 1; m <= r1max; m++) pw1[m] = cdd_mul(pw1[m - 1], z1);
+            cdd cur0 = one;
+            int n0cur = 0;
+            for (int p = 0; p < P; p++) {
+                int n0 = pn0[p], n1 = pn1[p];
+                while (n0cur < n0) { cur0 = cdd_mul(cur0, base); n0cur++; }
+                cdd f = n1 >= 0 ? pw1[n1] : cdd_conj(pw1[-n1]);
+                cdd e = cdd_mul(cur0, f);
+                int pb = p >> 5, pi = p & 31;
+                double* dst = A + ((((size_t)pb * Npad + j) * 4) * 32 + pi) * 2;
+                store_entry(dst, 64, e);
+            }
+        }
+    } else {
+        // ---- B table: powers of the last axis' base phasor
+        int a = d - 1;
+        cdd base = expi_turns(frac_turns(pos_hi[(size_t)a * N + j], pos_lo[(size_t)a * N + j], L, 1.0));
+        cdd cur = one;
+        double qs = ldexp(1.0, -qscale_log2);
+        long jb = j >> 5;
+        int jj = (int)(j & 31);
+        for (int q = 0; q < Qn; q++) {
+            int qb = q >> 5, qi = q & 31;
+            double* dst = B + ((((size_t)qb * Npad + j) * 4) * 32 + qi) * 2;
+            store_entry(dst, 64, cur);
+            if (with_grad) {
+                double* g = Bg + ((((size_t)jb * Qpad + q) * 8) * 32 + jj) * 2;
+                store_entry(g, 64, cur);
+                cdd w;
+                w.re = dd_scale2(dd_mul_d(cur.re, (double)q), qs);
+                w.im = dd_scale2(dd_mul_d(cur.im, (double)q), qs);
+                store_entry(g + 4 * 64, 64, w);
+            }
+            cur = cdd_mul(cur, base);
+        }
+    }
+}
+
+}  // namespace
+
+cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool with_grad_tables)
+{
+    dim3 grid((unsigned)((h->N + 127) / 128), 2);
+    k_tables<<<grid, 128, 0, h->stream>>>(h->d, h->N, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2,
+                                         h->d_pn0, h->d_pn1, h->Qpad, pos_hi, pos_lo,
+                                         h->d_A, h->d_B, h->d_Bg, with_grad_tables ? 1 : 0);
+    h->last_launches += 1;
+    return cudaGetLastError();
+}

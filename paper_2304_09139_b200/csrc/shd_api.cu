@@ -1,0 +1,368 @@
+// shd_api.cu -- the C-ABI of include/shd.h: host-side setup (step a0: enumeration of Q, the
+// outer-product decomposition, tile lists) and the launch sequences of the hot path.
+#include "../../include/shd.h"
+#include "shd_internal.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+
+namespace {
+
+int fail(shd_ctx* h, int code, const std::string& msg) {
+    if (h) h->err = msg;
+    return code;
+}
+#define CU(call)                                                                         \
+    do {                                                                                 \
+        cudaError_t e_ = (call);                                                         \
+        if (e_ != cudaSuccess) {                                                         \
+            h->err = std::string(#call) + ": " + cudaGetErrorString(e_);                 \
+            return e_ == cudaErrorMemoryAllocation ? SHD_ENOMEM : SHD_ECUDA;             \
+        }                                                                                \
+    } while (0)
+
+long isqrt_floor(long m) {
+    long r = (long)std::floor(std::sqrt((double)m));
+    while ((r + 1) * (r + 1) <= m) r++;
+    while (r * r > m) r--;
+    return r;
+}
+
+// a0: canonical half-space set Q (D:R6-R8): lexicographic, first non-zero component > 0
+void enumerate_Q(int d, long m_star, std::vector<int>& out) {
+    long R = isqrt_floor(m_star);
+    out.clear();
+    if (d == 1) {
+        for (long n = 1; n <= R; n++) out.push_back((int)n);
+    } else if (d == 2) {
+        for (long a = 0; a <= R; a++) {
+            long r1 = isqrt_floor(m_star - a * a);
+            for (long b = (a == 0 ? 1 : -r1); b <= r1; b++) { out.push_back((int)a); out.push_back((int)b); }
+        }
+    } else {
+        for (long a = 0; a <= R; a++) {
+            long r1 = isqrt_floor(m_star - a * a);
+            for (long b = (a == 0 ? 0 : -r1); b <= r1; b++) {
+                long r2 = isqrt_floor(m_star - a * a - b * b);
+                long c0 = (a == 0 && b == 0) ? 1 : -r2;
+                for (long c = c0; c <= r2; c++) { out.push_back((int)a); out.push_back((int)b); out.push_back((int)c); }
+            }
+        }
+    }
+}
+
+template <class T>
+int upload(shd_ctx* h, T** dst, const std::vector<T>& src) {
+    size_t bytes = std::max<size_t>(src.size(), 1) * sizeof(T);
+    CU(cudaMalloc((void**)dst, bytes));
+    h->workspace_bytes += bytes;
+    if (!src.empty()) CU(cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return SHD_OK;
+}
+int dalloc_zero(shd_ctx* h, double** dst, size_t ndoubles) {
+    size_t bytes = std::max<size_t>(ndoubles, 1) * sizeof(double);
+    CU(cudaMalloc((void**)dst, bytes));
+    h->workspace_bytes += bytes;
+    CU(cudaMemset(*dst, 0, bytes));
+    return SHD_OK;
+}
+
+int build(shd_ctx* h, const double* v) {
+    const int d = h->d;
+    const long m_star = h->m_star;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+        return fail(h, SHD_ECUDA, "no CUDA device: libshd has no CPU fallback");
+    enumerate_Q(d, m_star, h->nvec);
+    h->M = (long)h->nvec.size() / d;
+    if (h->M < 1) return fail(h, SHD_EINVAL, "empty Q");
+    if (v) {
+        h->v.assign(v, v + h->M);
+        for (double x : h->v)
+            if (!(x > 0.0) || !std::isfinite(x)) return fail(h, SHD_EINVAL, "v(k) must be positive and finite");
+    }
+    const long R = isqrt_floor(m_star);
+    // ---- outer-product decomposition
+    std::map<std::vector<int>, int> index;
+    for (long k = 0; k < h->M; k++)
+        index[std::vector<int>(h->nvec.begin() + k * d, h->nvec.begin() + (k + 1) * d)] = (int)k;
+    std::vector<std::vector<int>> wT(3);
+    if (d == 1) {
+        int S = 2;
+        while ((double)S * S < 2.0 * (double)R) S *= 2;
+        h->S1d = S;
+        h->Qn = S / 2 + 1;
+        h->P = (int)((R + S / 2 - 1) / S) + 1;
+        for (int p = 0; p < h->P; p++) { h->pn0.push_back(p); h->pn1.push_back(0); }
+    } else if (d == 2) {
+        h->P = (int)R + 1;
+        h->Qn = (int)R + 1;
+        for (int p = 0; p < h->P; p++) { h->pn0.push_back(p); h->pn1.push_back(0); }
+    } else {
+        if (R > 128) return fail(h, SHD_EINVAL, "d = 3 supports |n_a| <= 128");
+        for (long a = 0; a <= R; a++) {
+            long r1 = isqrt_floor(m_star - a * a);
+            for (long b = (a == 0 ? 0 : -r1); b <= r1; b++) { h->pn0.push_back((int)a); h->pn1.push_back((int)b); }
+        }
+        h->P = (int)h->pn0.size();
+        h->Qn = (int)R + 1;
+    }
+    h->npb = (h->P + 31) / 32;
+    h->nqb = (h->Qn + 31) / 32;
+    h->Qpad = h->nqb * 32;
+    const int Ppad = h->npb * 32;
+    h->qscale_log2 = 0;
+    while ((1 << h->qscale_log2) < std::max(h->Qn - 1, 1)) h->qscale_log2++;
+    for (int a = 0; a < 3; a++) wT[a].assign(Ppad, 0);
+    for (int p = 0; p < h->P; p++) {
+        if (d == 1) wT[0][p] = h->S1d * p;
+        else if (d == 2) wT[0][p] = h->pn0[p];
+        else { wT[0][p] = h->pn0[p]; wT[1][p] = h->pn1[p]; }
+    }
+    std::vector<int> kp((size_t)Ppad * h->Qpad, -1), km((size_t)Ppad * h->Qpad, -1);
+    long found = 0;
+    for (int p = 0; p < h->P; p++)
+        for (int q = 0; q < h->Qn; q++)
+            for (int sg = 1; sg >= -1; sg -= 2) {
+                if (q == 0 && sg < 0) continue;
+                std::vector<int> n(d);
+                if (d == 1) n[0] = h->S1d * p + sg * q;
+                else if (d == 2) { n[0] = h->pn0[p]; n[1] = sg * q; }
+                else { n[0] = h->pn0[p]; n[1] = h->pn1[p]; n[2] = sg * q; }
+                if (d == 1 && q == h->S1d / 2 && sg < 0) continue;   // S p - S/2 is (p-1, +S/2)
+                auto it = index.find(n);
+                if (it == index.end()) continue;
+                int& slot = (sg > 0 ? kp : km)[(size_t)p * h->Qpad + q];
+                if (slot >= 0) return fail(h, SHD_EINVAL, "internal: duplicate cell");
+                slot = it->second;
+                found++;
+            }
+    if (found != h->M) return fail(h, SHD_EINVAL, "internal: decomposition does not cover Q");
+    // ---- tiles and q-chunk counts
+    std::vector<int> tile_pb, tile_qb, qchunks(h->npb, 0);
+    h->valid_cells = 0;
+    for (int pb = 0; pb < h->npb; pb++)
+        for (int qb = 0; qb < h->nqb; qb++) {
+            bool any = false;
+            for (int pi = 0; pi < 32; pi++)
+                for (int qi = 0; qi < 32; qi++) {
+                    size_t c = (size_t)(pb * 32 + pi) * h->Qpad + qb * 32 + qi;
+                    if (kp[c] >= 0 || km[c] >= 0) {
+                        any = true;
+                        h->valid_cells++;
+                        qchunks[pb] = std::max(qchunks[pb], (qb * 32 + qi) / SHD_QCH + 1);
+                    }
+                }
+            if (any) { tile_pb.push_back(pb); tile_qb.push_back(qb); }
+        }
+    h->ntiles = (int)tile_pb.size();
+    h->grad_qsteps = 0;
+    for (int pb = 0; pb < h->npb; pb++) h->grad_qsteps += (long)qchunks[pb] * SHD_QCH;
+    // ---- particle splits of the rho pass: minimise (waves of CTAs) x (chunks per CTA)
+    cudaDeviceProp prop;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return fail(h, SHD_ECUDA, "cudaGetDeviceProperties failed");
+    const long sms = prop.multiProcessorCount;
+    const long nchunks = (h->N + SHD_NPS - 1) / SHD_NPS;
+    long best_cost = -1;
+    for (long ns = 1; ns <= std::min<long>(256, nchunks); ns++) {
+        long cps = (nchunks + ns - 1) / ns;
+        long waves = ((long)h->ntiles * ns + sms - 1) / sms;
+        long cost = waves * (cps + 2);          // +2: per-CTA prologue/epilogue
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; h->nsplit = (int)ns; h->chunks_per_split = cps; }
+    }
+    h->Npad = (long)h->nsplit * h->chunks_per_split * SHD_NPS;
+    h->njb = (h->N + 31) / 32;
+    // ---- device memory
+    int rc;
+    if ((rc = upload(h, &h->d_pn0, h->pn0))) return rc;
+    if ((rc = upload(h, &h->d_pn1, h->pn1))) return rc;
+    std::vector<int> wflat;
+    for (int a = 0; a < 3; a++) wflat.insert(wflat.end(), wT[a].begin(), wT[a].end());
+    if ((rc = upload(h, &h->d_wT, wflat))) return rc;
+    if ((rc = upload(h, &h->d_cell_kp, kp))) return rc;
+    if ((rc = upload(h, &h->d_cell_km, km))) return rc;
+    if ((rc = upload(h, &h->d_tile_pb, tile_pb))) return rc;
+    if ((rc = upload(h, &h->d_tile_qb, tile_qb))) return rc;
+    if ((rc = upload(h, &h->d_qchunks, qchunks))) return rc;
+    if (!h->v.empty()) { if ((rc = upload(h, &h->d_v, h->v))) return rc; }
+    const size_t slab = SHD_TILE_ENTRY_DOUBLES;
+    if ((rc = dalloc_zero(h, &h->d_A, (size_t)h->npb * h->Npad * slab))) return rc;
+    if ((rc = dalloc_zero(h, &h->d_B, (size_t)h->nqb * h->Npad * slab))) return rc;
+    if ((rc = dalloc_zero(h, &h->d_Bg, (size_t)h->njb * h->Qpad * 2 * slab))) return rc;
+    if ((rc = dalloc_zero(h, &h->d_C, (size_t)h->npb * h->Qpad * 2 * slab))) return rc;
+    if ((rc = dalloc_zero(h, &h->d_part, (size_t)h->nsplit * h->ntiles * 4 * 1024 * 2))) return rc;
+    if ((rc = dalloc_zero(h, &h->d_rho, (size_t)4 * h->M))) return rc;
+    h->nfinish_blocks = (int)(((long)h->ntiles * 1024 + 255) / 256);
+    if ((rc = dalloc_zero(h, &h->d_blockred, (size_t)h->nfinish_blocks * 8))) return rc;
+    CU(cudaMalloc((void**)&h->d_scal, sizeof(shd_scalars)));
+    CU(cudaMemset(h->d_scal, 0, sizeof(shd_scalars)));
+    CU(cudaMallocHost((void**)&h->h_scal, sizeof(shd_scalars)));
+    std::memset(h->h_scal, 0, sizeof(shd_scalars));
+    CU(shd_rho_configure());
+    CU(shd_grad_configure());
+    return SHD_OK;
+}
+
+int create_common(int d, long N, double L, long m_star, const double* v, shd_ctx** out) {
+    if (!out) return SHD_EINVAL;
+    *out = nullptr;
+    if (d < 1 || d > 3 || N < 1 || !(L > 0.0) || !std::isfinite(L) || m_star < 1) return SHD_EINVAL;
+    if (d == 1 && m_star > (long)4e12) return SHD_EINVAL;
+    if (d >= 2 && m_star > (long)4e6) return SHD_EINVAL;
+    shd_ctx* h = new (std::nothrow) shd_ctx();
+    if (!h) return SHD_ENOMEM;
+    h->d = d; h->N = N; h->L = L; h->m_star = m_star;
+    int rc;
+    try {
+        rc = build(h, v);
+    } catch (const std::bad_alloc&) {
+        rc = SHD_ENOMEM;
+        h->err = "host allocation failed";
+    }
+    *out = h;            // returned even on error so that shd_last_error() can be read; caller destroys
+    return rc;
+}
+
+// rho pass + reduction (steps a1-a3); optionally the gradient tables too
+int run_rho(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool with_grad) {
+    h->last_launches = 0;
+    CU(shd_launch_tables(h, pos_hi, pos_lo, with_grad));
+    CU(shd_launch_rho(h));
+    CU(shd_launch_finish(h));
+    return SHD_OK;
+}
+int fetch_scalars(shd_ctx* h) {
+    CU(cudaMemcpyAsync(h->h_scal, h->d_scal, sizeof(shd_scalars), cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return SHD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int shd_create_shell(int d, long N, double L, long m_star, const double* v, shd_ctx** out) {
+    return create_common(d, N, L, m_star, v, out);
+}
+
+int shd_create(int d, long N, double L, double K, const double* v, shd_ctx** out) {
+    if (!(K > 0.0) || !std::isfinite(K) || !(L > 0.0) || !std::isfinite(L)) { if (out) *out = nullptr; return SHD_EINVAL; }
+    double x = K * L / (2.0 * 3.14159265358979323846);
+    double m = std::floor(x * x * (1.0 + std::ldexp(1.0, -40)));
+    if (!(m >= 1.0) || m > 4e12) { if (out) *out = nullptr; return SHD_EINVAL; }
+    return create_common(d, N, L, (long)m, v, out);
+}
+
+void shd_destroy(shd_ctx* h) {
+    if (!h) return;
+    shd_min_free(h);
+    cudaFree(h->d_pn0); cudaFree(h->d_pn1); cudaFree(h->d_wT); cudaFree(h->d_cell_kp); cudaFree(h->d_cell_km);
+    cudaFree(h->d_tile_pb); cudaFree(h->d_tile_qb); cudaFree(h->d_qchunks); cudaFree(h->d_v);
+    cudaFree(h->d_A); cudaFree(h->d_B); cudaFree(h->d_Bg); cudaFree(h->d_C); cudaFree(h->d_part);
+    cudaFree(h->d_rho); cudaFree(h->d_blockred); cudaFree(h->d_scal);
+    if (h->h_scal) cudaFreeHost(h->h_scal);
+    delete h;
+}
+
+int shd_set_stream(shd_ctx* h, void* cuda_stream) {
+    if (!h) return SHD_EINVAL;
+    h->stream = (cudaStream_t)cuda_stream;
+    return SHD_OK;
+}
+
+long shd_num_k(const shd_ctx* h) { return h ? h->M : 0; }
+
+int shd_get_k(const shd_ctx* h, int* n_out) {
+    if (!h || !n_out) return SHD_EINVAL;
+    std::memcpy(n_out, h->nvec.data(), h->nvec.size() * sizeof(int));
+    return SHD_OK;
+}
+
+int shd_energy_grad(shd_ctx* h, const double* pos_hi, const double* pos_lo, double phi[2],
+                    double* grad_hi, double* grad_lo) {
+    if (!h) return SHD_EINVAL;
+    if (!pos_hi || !pos_lo || !phi) return fail(h, SHD_EINVAL, "NULL pointer");
+    if ((grad_hi == nullptr) != (grad_lo == nullptr)) return fail(h, SHD_EINVAL, "grad_hi and grad_lo must both be given or both NULL");
+    const bool want_grad = grad_hi != nullptr;
+    int rc = run_rho(h, pos_hi, pos_lo, want_grad);
+    if (rc) return rc;
+    if (want_grad) {
+        CU(shd_launch_ctable(h));
+        CU(shd_launch_grad(h, grad_hi, grad_lo));
+    }
+    if ((rc = fetch_scalars(h))) return rc;
+    phi[0] = h->h_scal->phi[0];
+    phi[1] = h->h_scal->phi[1];
+    if (h->h_scal->nonfinite) return fail(h, SHD_ENAN, "non-finite Phi (non-finite positions?)");
+    return SHD_OK;
+}
+
+int shd_smax(shd_ctx* h, const double* pos_hi, const double* pos_lo, double smax[2], long* argmax_k) {
+    if (!h) return SHD_EINVAL;
+    if (!pos_hi || !pos_lo || !smax) return fail(h, SHD_EINVAL, "NULL pointer");
+    int rc = run_rho(h, pos_hi, pos_lo, false);
+    if (rc) return rc;
+    if ((rc = fetch_scalars(h))) return rc;
+    smax[0] = h->h_scal->smax[0];
+    smax[1] = h->h_scal->smax[1];
+    if (argmax_k) *argmax_k = (long)h->h_scal->argmax;
+    if (h->h_scal->nonfinite) return fail(h, SHD_ENAN, "non-finite S_max");
+    return SHD_OK;
+}
+
+int shd_last_smax(shd_ctx* h, double smax[2], long* argmax_k) {
+    if (!h || !smax) return SHD_EINVAL;
+    int rc = fetch_scalars(h);
+    if (rc) return rc;
+    smax[0] = h->h_scal->smax[0];
+    smax[1] = h->h_scal->smax[1];
+    if (argmax_k) *argmax_k = (long)h->h_scal->argmax;
+    return SHD_OK;
+}
+
+int shd_get_rho(shd_ctx* h, double* re_hi, double* re_lo, double* im_hi, double* im_lo) {
+    if (!h) return SHD_EINVAL;
+    if (!re_hi || !re_lo || !im_hi || !im_lo) return fail(h, SHD_EINVAL, "NULL pointer");
+    size_t b = (size_t)h->M * sizeof(double);
+    CU(cudaMemcpyAsync(re_hi, h->d_rho, b, cudaMemcpyDeviceToDevice, h->stream));
+    CU(cudaMemcpyAsync(re_lo, h->d_rho + h->M, b, cudaMemcpyDeviceToDevice, h->stream));
+    CU(cudaMemcpyAsync(im_hi, h->d_rho + 2 * h->M, b, cudaMemcpyDeviceToDevice, h->stream));
+    CU(cudaMemcpyAsync(im_lo, h->d_rho + 3 * h->M, b, cudaMemcpyDeviceToDevice, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return SHD_OK;
+}
+
+const char* shd_last_error(const shd_ctx* h) { return h ? h->err.c_str() : "NULL handle"; }
+
+double shd_stat(const shd_ctx* h, int what) {
+    if (!h) return 0.0;
+    const double cells_rho = (double)h->ntiles * 1024.0;
+    switch (what) {
+        case 0: {   // FP64 instructions of the two contractions as launched (padded cells)
+            double rho = cells_rho * (double)h->Npad * 24.0;
+            double qsteps = 0.0;
+            // gradient: per particle block, per p-block, qchunks*8 q-steps x 32x32 x 48
+            return rho + qsteps;
+        }
+        case 1: return (double)h->last_launches;
+        case 2: return cells_rho;
+        case 3: return (double)h->valid_cells;
+        case 4: return (double)h->workspace_bytes;
+        case 5: return (double)h->nsplit;
+        case 6: return (double)h->ntiles;
+        case 7: return (double)h->P;
+        case 8: return (double)h->Qn;
+        case 9: return (double)h->Npad;
+        case 10: return (double)h->njb;
+        case 11: return (double)h->grad_qsteps;
+        default: return 0.0;
+    }
+}
+
+}  // extern "C"

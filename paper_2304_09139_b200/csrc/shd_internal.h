@@ -1,0 +1,110 @@
+// shd_internal.h -- handle layout and device data layouts shared by the kernels of libshd.so.
+//
+// Decomposition: every k in Q is written once as
+//   exp(i k.r_j) = A_j[p] * B_j[q]^sigma ,  sigma = +1 (B) or -1 (conj B),
+// with per-particle tables A_j[0..P), B_j[0..Qn) of complex dd phasors built from per-axis
+// integer-power recurrences:
+//   d=1: n = S p + sigma q,          A[p] = (z^S)^p,          B[q] = z^q       (q <= S/2)
+//   d=2: n = (p, sigma q),           A[p] = z0^p,             B[q] = z1^q
+//   d=3: n = (n0(p), n1(p), sigma q) A[p] = z0^n0 z1^n1,      B[q] = z2^q
+// so that rho(+/-)[p,q] = sum_j A_j[p] B_j[q]^(+/-) is a contraction over particles (rho pass) and
+// the gradient is a contraction over q followed by one over p (gradient pass).
+//
+// Each real operand x (|x| <= 1) is stored as four "limbs" (x0, x1, x2, x12):
+//   x0  = x rounded to a multiple of 2^-W0,  x1 = (x - x0) rounded to a multiple of 2^-(W0+W1),
+//   x2  = x - x0 - x1 (a free double),       x12 = x1 + x2,
+// and a product-accumulate  acc += x*y  is the 6 FMAs
+//   L0 += x0 y0 ;  L1 += x0 y1 + x1 y0 ;  L2 += x0 y2 + x2 y0 + x12 y12
+// where L0 and L1 are EXACT (all partial sums representable) for bursts of <= 128 terms, and
+// L2 carries the terms below 2^-45 in plain FP64 (error ~2^-100 per term).  Bursts are folded
+// into ordinary double-double accumulators with TwoSum.
+#pragma once
+#include <cuda_runtime.h>
+#include <cstddef>
+#include <string>
+#include <vector>
+
+constexpr int SHD_PT = 32;          // A-entries (p) per tile
+constexpr int SHD_QT = 32;          // B-entries (q) per tile
+constexpr int SHD_NPS = 16;         // particles per rho-pass pipeline stage
+constexpr int SHD_RHO_STAGES = 3;   // TMA pipeline depth, rho pass
+constexpr int SHD_BURST = 128;      // products per exact burst (see header comment)
+constexpr int SHD_QCH = 8;          // q per gradient-pass pipeline stage
+constexpr int SHD_GRAD_STAGES = 2;  // TMA pipeline depth, gradient pass
+constexpr int SHD_JT = 32;          // particles per gradient-pass block
+constexpr int SHD_W0 = 23;          // limb widths (bits)
+constexpr int SHD_W1 = 22;
+constexpr int SHD_ENTRY_DOUBLES = 8;            // (re,im) x 4 limbs
+constexpr int SHD_TILE_ENTRY_DOUBLES = 32 * 8;  // one (block, particle) slab: 2 KB
+
+// device scalars (one small struct in device memory, mirrored in pinned host memory)
+struct shd_scalars {
+    double phi[2];
+    double smax[2];       // max |rho|^2 / N
+    double maxvs;         // max v^2 |rho|^2   (scale of the gradient operand)
+    double cscale;        // 2^-e applied to the C table
+    long long argmax;
+    int nonfinite;
+    int pad;
+};
+
+struct shd_minstate;      // minimizer workspace (shd_min.cu)
+
+struct shd_ctx {
+    int d = 0;
+    long N = 0;
+    double L = 0;
+    long m_star = 0;
+    long M = 0;
+    // decomposition
+    int P = 0, Qn = 0, npb = 0, nqb = 0;
+    int S1d = 0;               // d == 1: n = S1d * p + sigma q
+    int qscale_log2 = 0;       // q * B is stored as q * B * 2^-qscale_log2
+    long Npad = 0;             // particles padded to nsplit * chunks_per_split * NPS
+    int nsplit = 0;
+    long chunks_per_split = 0;
+    int ntiles = 0;
+    long njb = 0;              // ceil(N / 32)
+    int Qpad = 0;              // nqb * 32
+    long valid_cells = 0;
+    long grad_qsteps = 0;      // sum over p-blocks of q-steps walked by the gradient pass
+    // host copies
+    std::vector<int> nvec;     // M * d
+    std::vector<double> v;     // M (empty = all ones)
+    std::vector<int> pn0, pn1; // exponent of z0 (and z1 for d=3) of A entry p
+    // device: setup tables
+    int *d_pn0 = nullptr, *d_pn1 = nullptr;
+    int *d_wT = nullptr;       // [3][P padded]: integer weight of Im(conj(A) T) for axis a
+    int *d_cell_kp = nullptr, *d_cell_km = nullptr;   // [npb*32][Qpad] -> k or -1
+    int *d_tile_pb = nullptr, *d_tile_qb = nullptr;   // [ntiles]
+    int *d_qchunks = nullptr;  // [npb] number of q-chunks (of SHD_QCH) with any valid cell
+    double *d_v = nullptr;     // [M]
+    // device: per-evaluation data
+    double *d_A = nullptr;     // [npb][Npad][4][32][2]
+    double *d_B = nullptr;     // [nqb][Npad][4][32][2]
+    double *d_Bg = nullptr;    // [njb][Qpad][8][32][2]
+    double *d_C = nullptr;     // [npb][Qpad][8][32][2]
+    double *d_part = nullptr;  // [nsplit][ntiles][4][1024][2]
+    double *d_rho = nullptr;   // [4][M]: re_hi, re_lo, im_hi, im_lo
+    double *d_blockred = nullptr;   // per-block partials of the finish kernel
+    int nfinish_blocks = 0;
+    shd_scalars *d_scal = nullptr;
+    shd_scalars *h_scal = nullptr;  // pinned
+    size_t workspace_bytes = 0;
+    cudaStream_t stream = 0;
+    shd_minstate *min = nullptr;
+    std::string err;
+    int last_launches = 0;
+};
+
+// kernels / launchers (each returns the cudaError of its launches)
+cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool with_grad_tables);
+cudaError_t shd_launch_rho(shd_ctx* h);
+cudaError_t shd_launch_finish(shd_ctx* h);
+cudaError_t shd_launch_ctable(shd_ctx* h);
+cudaError_t shd_launch_grad(shd_ctx* h, double* grad_hi, double* grad_lo);
+cudaError_t shd_rho_configure();
+cudaError_t shd_grad_configure();
+
+// minimizer (shd_min.cu)
+void shd_min_free(shd_ctx* h);

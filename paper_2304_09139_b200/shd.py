@@ -1,0 +1,177 @@
+"""Thin ctypes binding over libshd.so (include/shd.h).  Argument marshalling only: every step of the
+hot path runs inside the library's CUDA kernels.  PyTorch is used for device buffers and streams.
+
+There is NO CPU fallback: importing this module without a built ``libshd.so`` raises, and every
+compute call needs a CUDA device.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+LIB_PATH = _HERE / "libshd.so"
+
+SHD_OK, SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA, SHD_ENAN, SHD_ESTALL, SHD_EMAXEVAL = 0, -1, -2, -3, -4, -5, -6
+EXPORTS = ["shd_create", "shd_create_shell", "shd_destroy", "shd_set_stream", "shd_num_k", "shd_get_k",
+           "shd_energy_grad", "shd_smax", "shd_last_smax", "shd_get_rho", "shd_minimize",
+           "shd_last_error", "shd_stat"]
+
+
+class ShdError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libshd error {code}: {msg}")
+        self.code = code
+
+
+class shd_min_opts(C.Structure):
+    _fields_ = [("kind", C.c_int), ("history", C.c_int), ("smax_tol", C.c_double),
+                ("max_evals", C.c_long), ("poll_every", C.c_int)]
+
+
+class shd_min_report(C.Structure):
+    _fields_ = [("iters", C.c_long), ("evals", C.c_long), ("phi", C.c_double * 2),
+                ("smax", C.c_double * 2), ("status", C.c_int)]
+
+
+def _load():
+    if not LIB_PATH.exists():
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2304_09139_b200.build` "
+                          "(libshd has no CPU fallback)")
+    lib = C.CDLL(str(LIB_PATH))
+    vp, dp = C.c_void_p, C.POINTER(C.c_double)
+    lib.shd_create.argtypes = [C.c_int, C.c_long, C.c_double, C.c_double, dp, C.POINTER(vp)]
+    lib.shd_create_shell.argtypes = [C.c_int, C.c_long, C.c_double, C.c_long, dp, C.POINTER(vp)]
+    lib.shd_destroy.argtypes = [vp]
+    lib.shd_destroy.restype = None
+    lib.shd_set_stream.argtypes = [vp, vp]
+    lib.shd_num_k.argtypes = [vp]
+    lib.shd_num_k.restype = C.c_long
+    lib.shd_get_k.argtypes = [vp, C.POINTER(C.c_int)]
+    lib.shd_energy_grad.argtypes = [vp, vp, vp, dp, vp, vp]
+    lib.shd_smax.argtypes = [vp, vp, vp, dp, C.POINTER(C.c_long)]
+    lib.shd_last_smax.argtypes = [vp, dp, C.POINTER(C.c_long)]
+    lib.shd_get_rho.argtypes = [vp, vp, vp, vp, vp]
+    lib.shd_minimize.argtypes = [vp, vp, vp, C.POINTER(shd_min_opts), C.POINTER(shd_min_report)]
+    lib.shd_last_error.argtypes = [vp]
+    lib.shd_last_error.restype = C.c_char_p
+    lib.shd_stat.argtypes = [vp, C.c_int]
+    lib.shd_stat.restype = C.c_double
+    return lib
+
+
+lib = _load()
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("libshd needs a CUDA device (no CPU fallback)")
+    return torch
+
+
+class Shd:
+    """One handle (shd_ctx).  Tensors are CUDA float64, axis-major ``x[a*N + j]``."""
+
+    def __init__(self, d, N, L, K=None, v=None, m_star=None):
+        self.d, self.N, self.L = int(d), int(N), float(L)
+        self._h = C.c_void_p()
+        pv = None
+        if v is not None:
+            self._v = np.ascontiguousarray(v, dtype=np.float64)
+            pv = self._v.ctypes.data_as(C.POINTER(C.c_double))
+        if m_star is not None:
+            rc = lib.shd_create_shell(self.d, self.N, self.L, int(m_star), pv, C.byref(self._h))
+        else:
+            rc = lib.shd_create(self.d, self.N, self.L, float(K), pv, C.byref(self._h))
+        if rc != SHD_OK:
+            msg = lib.shd_last_error(self._h).decode() if self._h else "invalid argument"
+            if self._h:
+                lib.shd_destroy(self._h)
+                self._h = C.c_void_p()
+            raise ShdError(rc, msg)
+        self.M = int(lib.shd_num_k(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib.shd_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc, ok=(SHD_OK,)):
+        if rc not in ok:
+            raise ShdError(rc, lib.shd_last_error(self._h).decode())
+        return rc
+
+    def set_stream(self, stream):
+        """stream: a torch.cuda.Stream (or None for the legacy default stream)."""
+        self._check(lib.shd_set_stream(self._h, C.c_void_p(stream.cuda_stream if stream is not None else 0)))
+
+    def k(self) -> np.ndarray:
+        n = np.zeros((self.M, self.d), dtype=np.int32)
+        self._check(lib.shd_get_k(self._h, n.ctypes.data_as(C.POINTER(C.c_int))))
+        return n
+
+    def _pos(self, pos_hi, pos_lo):
+        torch = _torch()
+        for t in (pos_hi, pos_lo):
+            assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == self.d * self.N
+        return C.c_void_p(pos_hi.data_ptr()), C.c_void_p(pos_lo.data_ptr())
+
+    def energy_grad(self, pos_hi, pos_lo, grad_hi=None, grad_lo=None, want_grad=True):
+        """shd_energy_grad: returns (phi_hi, phi_lo), grad_hi, grad_lo (device tensors or None)."""
+        torch = _torch()
+        ph, pl = self._pos(pos_hi, pos_lo)
+        if want_grad and grad_hi is None:
+            grad_hi = torch.empty_like(pos_hi)
+            grad_lo = torch.empty_like(pos_hi)
+        phi = (C.c_double * 2)()
+        gh = C.c_void_p(grad_hi.data_ptr()) if want_grad else None
+        gl = C.c_void_p(grad_lo.data_ptr()) if want_grad else None
+        self._check(lib.shd_energy_grad(self._h, ph, pl, phi, gh, gl))
+        return (phi[0], phi[1]), (grad_hi if want_grad else None), (grad_lo if want_grad else None)
+
+    def smax(self, pos_hi, pos_lo):
+        ph, pl = self._pos(pos_hi, pos_lo)
+        s = (C.c_double * 2)()
+        arg = C.c_long(-1)
+        self._check(lib.shd_smax(self._h, ph, pl, s, C.byref(arg)))
+        return (s[0], s[1]), int(arg.value)
+
+    def last_smax(self):
+        s = (C.c_double * 2)()
+        arg = C.c_long(-1)
+        self._check(lib.shd_last_smax(self._h, s, C.byref(arg)))
+        return (s[0], s[1]), int(arg.value)
+
+    def rho(self):
+        """rho(k) of the last evaluation: (re_hi, re_lo, im_hi, im_lo) device tensors."""
+        torch = _torch()
+        out = [torch.empty(self.M, dtype=torch.float64, device="cuda") for _ in range(4)]
+        self._check(lib.shd_get_rho(self._h, *[C.c_void_p(t.data_ptr()) for t in out]))
+        return tuple(out)
+
+    def minimize(self, pos_hi, pos_lo, kind=0, history=10, smax_tol=1e-30, max_evals=10000, poll_every=8):
+        ph, pl = self._pos(pos_hi, pos_lo)
+        opts = shd_min_opts(kind, history, smax_tol, max_evals, poll_every)
+        rep = shd_min_report()
+        rc = lib.shd_minimize(self._h, ph, pl, C.byref(opts), C.byref(rep))
+        self._check(rc, ok=(SHD_OK, SHD_ESTALL, SHD_EMAXEVAL))
+        return dict(status=rc, iters=int(rep.iters), evals=int(rep.evals),
+                    phi=(rep.phi[0], rep.phi[1]), smax=(rep.smax[0], rep.smax[1]))
+
+    def stat(self, what: int) -> float:
+        return float(lib.shd_stat(self._h, int(what)))
+
+
+def from_host(hi: np.ndarray, lo: np.ndarray):
+    """numpy (hi, lo) -> CUDA tensors."""
+    torch = _torch()
+    return (torch.from_numpy(np.ascontiguousarray(hi)).cuda(), torch.from_numpy(np.ascontiguousarray(lo)).cuda())
