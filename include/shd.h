@@ -77,6 +77,16 @@ int shd_get_k(const shd_ctx* h, int* n_out);
 int shd_energy_grad(shd_ctx* h, const double* pos_hi, const double* pos_lo,
                     double phi[2], double* grad_hi, double* grad_lo);
 
+/*
+ * The same evaluation for a caller whose data lives in HOST memory: pos_hi, pos_lo (in) and
+ * grad_hi, grad_lo (out, both NULL to skip the gradient) are HOST pointers to d*N doubles each
+ * (pinned memory makes the copies faster but is not required).  The library copies the positions
+ * to a device staging buffer it owns, runs shd_energy_grad, and copies the gradient back; the call
+ * returns when the results are in host memory.
+ */
+int shd_energy_grad_host(shd_ctx* h, const double* pos_hi, const double* pos_lo,
+                         double phi[2], double* grad_hi, double* grad_lo);
+
 /* S_max (Eq. 1) of the given positions: smax[0..1] = (hi, lo) on the HOST, *argmax_k = index
  * into the canonical order (may be NULL).  Runs the rho pass and the reduction only. */
 int shd_smax(shd_ctx* h, const double* pos_hi, const double* pos_lo, double smax[2], long* argmax_k);
@@ -113,11 +123,28 @@ int shd_minimize(shd_ctx* h, double* pos_hi, double* pos_lo, const shd_min_opts*
 /* Text of the last error on this handle (never NULL). */
 const char* shd_last_error(const shd_ctx* h);
 
+/* Per-kernel device timing: with on != 0 every later shd_energy_grad / shd_smax records CUDA events on
+ * the handle's stream around its launch groups; read the durations with shd_stat(h, 20..24). */
+int shd_set_timing(shd_ctx* h, int on);
+
 /* Introspection used by bench.py / tests (host scalars):
- *   what = 0: FP64 instructions (DFMA/DADD/DMUL) the last shd_energy_grad issued per launch model,
- *   what = 1: number of kernel launches of the last call, 2: padded cell count of the rho pass,
- *   3: valid cell count, 4: bytes of device workspace. */
+ *   what = 0 / 12: DFMAs the rho / gradient pass launches (padding included),
+ *   what = 1: kernel launches of the last call, 2: padded (p,q) cell count of the rho pass,
+ *   3: valid cell count, 4: bytes of device workspace, 5: particle splits of the rho pass,
+ *   6: (p,q) tiles, 7: P, 8: Qn, 9: padded particle count, 10: particle blocks of the gradient
+ *   pass, 11: q-steps walked by one gradient block,
+ *   20..24: milliseconds of the last call's launch groups (needs shd_set_timing):
+ *           20 phasor tables (a1), 21 rho pass (a2), 22 finish (a3), 23 gradient operand, 24 gradient pass (a4). */
 double shd_stat(const shd_ctx* h, int what);
+
+/*
+ * Measured FP64-pipe issue rate of the current device, the denominator of the "alu" roofline
+ * (DESIGN.md "roofline").  kind = 0: dependent-DFMA chains, 1: DADD chains (8 per
+ * thread, all SMs); runs for about `seconds` (0 < seconds <= 10).  HOST out: instr_per_s[0] = best
+ * launch, instr_per_s[1] = mean over the run (sustained), in thread-level FP64 instructions per
+ * second.  Errors: SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA.  Needs no handle.
+ */
+int shd_fp64_peak(int kind, double seconds, double instr_per_s[2]);
 
 #ifdef __cplusplus
 }

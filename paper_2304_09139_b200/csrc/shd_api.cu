@@ -229,12 +229,37 @@ int create_common(int d, long N, double L, long m_star, const double* v, shd_ctx
     return rc;
 }
 
+// event i is recorded BEFORE launch group i; event SHD_NKERN after the last group
+int mark(shd_ctx* h, int i) {
+    if (!h->timing) return SHD_OK;
+    CU(cudaEventRecord(h->ev[i], h->stream));
+    h->ev_used[i] = true;
+    return SHD_OK;
+}
+int collect_timing(shd_ctx* h) {      // after the stream has been synchronised
+    if (!h->timing) return SHD_OK;
+    for (int i = 0; i < SHD_NKERN; i++) {
+        h->kern_ms[i] = 0.f;
+        if (!h->ev_used[i]) continue;
+        int nxt = i + 1;
+        while (nxt <= SHD_NKERN && !h->ev_used[nxt]) nxt++;
+        if (nxt > SHD_NKERN) continue;
+        CU(cudaEventElapsedTime(&h->kern_ms[i], h->ev[i], h->ev[nxt]));
+    }
+    return SHD_OK;
+}
 // rho pass + reduction (steps a1-a3); optionally the gradient tables too
 int run_rho(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool with_grad) {
     h->last_launches = 0;
+    for (int i = 0; i <= SHD_NKERN; i++) h->ev_used[i] = false;
+    int rc;
+    if ((rc = mark(h, 0))) return rc;
     CU(shd_launch_tables(h, pos_hi, pos_lo, with_grad));
+    if ((rc = mark(h, 1))) return rc;
     CU(shd_launch_rho(h));
+    if ((rc = mark(h, 2))) return rc;
     CU(shd_launch_finish(h));
+    if ((rc = mark(h, 3))) return rc;
     return SHD_OK;
 }
 int fetch_scalars(shd_ctx* h) {
@@ -266,6 +291,8 @@ void shd_destroy(shd_ctx* h) {
     cudaFree(h->d_tile_pb); cudaFree(h->d_tile_qb); cudaFree(h->d_qchunks); cudaFree(h->d_v);
     cudaFree(h->d_A); cudaFree(h->d_B); cudaFree(h->d_Bg); cudaFree(h->d_C); cudaFree(h->d_part);
     cudaFree(h->d_rho); cudaFree(h->d_blockred); cudaFree(h->d_scal);
+    cudaFree(h->d_hpos); cudaFree(h->d_hgrad);
+    for (int i = 0; i <= SHD_NKERN; i++) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     if (h->h_scal) cudaFreeHost(h->h_scal);
     delete h;
 }
@@ -294,12 +321,48 @@ int shd_energy_grad(shd_ctx* h, const double* pos_hi, const double* pos_lo, doub
     if (rc) return rc;
     if (want_grad) {
         CU(shd_launch_ctable(h));
+        if ((rc = mark(h, 4))) return rc;
         CU(shd_launch_grad(h, grad_hi, grad_lo));
+        if ((rc = mark(h, 5))) return rc;
     }
     if ((rc = fetch_scalars(h))) return rc;
+    if ((rc = collect_timing(h))) return rc;
     phi[0] = h->h_scal->phi[0];
     phi[1] = h->h_scal->phi[1];
     if (h->h_scal->nonfinite) return fail(h, SHD_ENAN, "non-finite Phi (non-finite positions?)");
+    return SHD_OK;
+}
+
+int shd_energy_grad_host(shd_ctx* h, const double* pos_hi, const double* pos_lo, double phi[2],
+                         double* grad_hi, double* grad_lo) {
+    if (!h) return SHD_EINVAL;
+    if (!pos_hi || !pos_lo || !phi) return fail(h, SHD_EINVAL, "NULL pointer");
+    if ((grad_hi == nullptr) != (grad_lo == nullptr)) return fail(h, SHD_EINVAL, "grad_hi and grad_lo must both be given or both NULL");
+    const size_t n = (size_t)h->d * h->N, b = n * sizeof(double);
+    if (!h->d_hpos) {
+        CU(cudaMalloc((void**)&h->d_hpos, 2 * b));
+        CU(cudaMalloc((void**)&h->d_hgrad, 2 * b));
+        h->workspace_bytes += 4 * b;
+    }
+    CU(cudaMemcpyAsync(h->d_hpos, pos_hi, b, cudaMemcpyHostToDevice, h->stream));
+    CU(cudaMemcpyAsync(h->d_hpos + n, pos_lo, b, cudaMemcpyHostToDevice, h->stream));
+    const bool want_grad = grad_hi != nullptr;
+    int rc = shd_energy_grad(h, h->d_hpos, h->d_hpos + n, phi, want_grad ? h->d_hgrad : nullptr,
+                             want_grad ? h->d_hgrad + n : nullptr);
+    if (rc) return rc;
+    if (want_grad) {
+        CU(cudaMemcpyAsync(grad_hi, h->d_hgrad, b, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaMemcpyAsync(grad_lo, h->d_hgrad + n, b, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaStreamSynchronize(h->stream));
+    }
+    return SHD_OK;
+}
+
+int shd_set_timing(shd_ctx* h, int on) {
+    if (!h) return SHD_EINVAL;
+    if (on && !h->ev[0])
+        for (int i = 0; i <= SHD_NKERN; i++) CU(cudaEventCreate(&h->ev[i]));
+    h->timing = on != 0;
     return SHD_OK;
 }
 
@@ -309,6 +372,7 @@ int shd_smax(shd_ctx* h, const double* pos_hi, const double* pos_lo, double smax
     int rc = run_rho(h, pos_hi, pos_lo, false);
     if (rc) return rc;
     if ((rc = fetch_scalars(h))) return rc;
+    if ((rc = collect_timing(h))) return rc;
     smax[0] = h->h_scal->smax[0];
     smax[1] = h->h_scal->smax[1];
     if (argmax_k) *argmax_k = (long)h->h_scal->argmax;
@@ -344,12 +408,8 @@ double shd_stat(const shd_ctx* h, int what) {
     if (!h) return 0.0;
     const double cells_rho = (double)h->ntiles * 1024.0;
     switch (what) {
-        case 0: {   // FP64 instructions of the two contractions as launched (padded cells)
-            double rho = cells_rho * (double)h->Npad * 24.0;
-            double qsteps = 0.0;
-            // gradient: per particle block, per p-block, qchunks*8 q-steps x 32x32 x 48
-            return rho + qsteps;
-        }
+        case 0: return cells_rho * (double)h->Npad * 24.0;     // DFMAs launched by the rho pass (padded)
+        case 12: return (double)h->njb * (double)h->grad_qsteps * 1024.0 * 48.0;   // ... by the gradient pass
         case 1: return (double)h->last_launches;
         case 2: return cells_rho;
         case 3: return (double)h->valid_cells;
@@ -361,6 +421,7 @@ double shd_stat(const shd_ctx* h, int what) {
         case 9: return (double)h->Npad;
         case 10: return (double)h->njb;
         case 11: return (double)h->grad_qsteps;
+        case 20: case 21: case 22: case 23: case 24: return (double)h->kern_ms[what - 20];
         default: return 0.0;
     }
 }

@@ -37,6 +37,9 @@ constexpr int SHD_W1 = 22;
 constexpr int SHD_ENTRY_DOUBLES = 8;            // (re,im) x 4 limbs
 constexpr int SHD_TILE_ENTRY_DOUBLES = 32 * 8;  // one (block, particle) slab: 2 KB
 
+// launch groups timed by shd_set_timing: tables (a1), rho (a2), finish (a3), ctable, grad (a4)
+constexpr int SHD_NKERN = 5;
+
 // device scalars (one small struct in device memory, mirrored in pinned host memory)
 struct shd_scalars {
     double phi[2];
@@ -95,6 +98,13 @@ struct shd_ctx {
     shd_minstate *min = nullptr;
     std::string err;
     int last_launches = 0;
+    // optional per-kernel device timing (shd_set_timing): events around each launch group
+    bool timing = false;
+    cudaEvent_t ev[SHD_NKERN + 1] = {};
+    bool ev_used[SHD_NKERN + 1] = {};
+    float kern_ms[SHD_NKERN] = {};
+    // staging buffers of shd_energy_grad_host (device)
+    double *d_hpos = nullptr, *d_hgrad = nullptr;
 };
 
 // kernels / launchers (each returns the cudaError of its launches)

@@ -16,8 +16,8 @@ LIB_PATH = _HERE / "libshd.so"
 
 SHD_OK, SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA, SHD_ENAN, SHD_ESTALL, SHD_EMAXEVAL = 0, -1, -2, -3, -4, -5, -6
 EXPORTS = ["shd_create", "shd_create_shell", "shd_destroy", "shd_set_stream", "shd_num_k", "shd_get_k",
-           "shd_energy_grad", "shd_smax", "shd_last_smax", "shd_get_rho", "shd_minimize",
-           "shd_last_error", "shd_stat"]
+           "shd_energy_grad", "shd_energy_grad_host", "shd_set_timing", "shd_smax", "shd_last_smax", "shd_get_rho", "shd_minimize",
+           "shd_last_error", "shd_stat", "shd_fp64_peak"]
 
 
 class ShdError(RuntimeError):
@@ -51,6 +51,8 @@ def _load():
     lib.shd_num_k.restype = C.c_long
     lib.shd_get_k.argtypes = [vp, C.POINTER(C.c_int)]
     lib.shd_energy_grad.argtypes = [vp, vp, vp, dp, vp, vp]
+    lib.shd_energy_grad_host.argtypes = [vp, dp, dp, dp, dp, dp]
+    lib.shd_set_timing.argtypes = [vp, C.c_int]
     lib.shd_smax.argtypes = [vp, vp, vp, dp, C.POINTER(C.c_long)]
     lib.shd_last_smax.argtypes = [vp, dp, C.POINTER(C.c_long)]
     lib.shd_get_rho.argtypes = [vp, vp, vp, vp, vp]
@@ -59,6 +61,7 @@ def _load():
     lib.shd_last_error.restype = C.c_char_p
     lib.shd_stat.argtypes = [vp, C.c_int]
     lib.shd_stat.restype = C.c_double
+    lib.shd_fp64_peak.argtypes = [C.c_int, C.c_double, dp]
     return lib
 
 
@@ -138,6 +141,26 @@ class Shd:
         self._check(lib.shd_energy_grad(self._h, ph, pl, phi, gh, gl))
         return (phi[0], phi[1]), (grad_hi if want_grad else None), (grad_lo if want_grad else None)
 
+    def energy_grad_host(self, pos_hi, pos_lo, grad_hi=None, grad_lo=None):
+        """shd_energy_grad_host: numpy float64 arrays in HOST memory (e.g. views of pinned tensors);
+        grad arrays are filled in place.  Returns (phi_hi, phi_lo)."""
+        dp = C.POINTER(C.c_double)
+        for a in (pos_hi, pos_lo, grad_hi, grad_lo):
+            assert a is None or (a.dtype == np.float64 and a.flags.c_contiguous and a.size == self.d * self.N)
+        phi = (C.c_double * 2)()
+        g = [a.ctypes.data_as(dp) if a is not None else None for a in (grad_hi, grad_lo)]
+        self._check(lib.shd_energy_grad_host(self._h, pos_hi.ctypes.data_as(dp), pos_lo.ctypes.data_as(dp),
+                                             phi, g[0], g[1]))
+        return phi[0], phi[1]
+
+    def set_timing(self, on: bool):
+        self._check(lib.shd_set_timing(self._h, 1 if on else 0))
+
+    def kernel_ms(self):
+        """milliseconds of the last call's launch groups (after set_timing(True))."""
+        names = ["tables", "rho", "finish", "ctable", "grad"]
+        return {n: self.stat(20 + i) for i, n in enumerate(names)}
+
     def smax(self, pos_hi, pos_lo):
         ph, pl = self._pos(pos_hi, pos_lo)
         s = (C.c_double * 2)()
@@ -169,6 +192,16 @@ class Shd:
 
     def stat(self, what: int) -> float:
         return float(lib.shd_stat(self._h, int(what)))
+
+
+def fp64_peak(kind: int = 0, seconds: float = 1.0):
+    """shd_fp64_peak: (best, sustained) thread-level FP64 instructions per second."""
+    _torch()
+    out = (C.c_double * 2)()
+    rc = lib.shd_fp64_peak(int(kind), float(seconds), out)
+    if rc != SHD_OK:
+        raise ShdError(rc, "shd_fp64_peak failed")
+    return out[0], out[1]
 
 
 def from_host(hi: np.ndarray, lo: np.ndarray):
