@@ -96,3 +96,13 @@ DD_HD dd dd_sqrt(dd x) {                      // x >= 0
     return fast_two_sum(s, c);
 }
 DD_HD bool dd_less(dd a, dd b) { return a.h < b.h || (a.h == b.h && a.l < b.l); }
+// dd / dd (relative error ~ 2^-103): three quotient digits with exact dd remainders
+DD_HD dd dd_div(dd x, dd y) {
+    double q1 = __ddiv_rn(x.h, y.h);
+    dd r = dd_sub(x, dd_mul_d(y, q1));
+    double q2 = __ddiv_rn(r.h, y.h);
+    r = dd_sub(r, dd_mul_d(y, q2));
+    double q3 = __ddiv_rn(r.h, y.h);
+    dd q = fast_two_sum(q1, q2);
+    return dd_add_d(q, q3);
+}

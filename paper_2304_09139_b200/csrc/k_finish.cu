@@ -58,8 +58,10 @@ __device__ __forceinline__ void account(red& r, dd re, dd im, double v, long lon
 __global__ void __launch_bounds__(256) k_finish1(
     const double* __restrict__ part, int nsplit, int ntiles, const int* __restrict__ tile_pb,
     const int* __restrict__ tile_qb, const int* __restrict__ cell_kp, const int* __restrict__ cell_km,
-    int Qpad, long M, const double* __restrict__ v, double* __restrict__ rho, double* __restrict__ blockred)
+    int Qpad, long M, const double* __restrict__ v, double* __restrict__ rho, double* __restrict__ blockred,
+    const int* __restrict__ skip)
 {
+    if (skip && *skip) return;
     long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     red r; r.phi = dd{0, 0}; r.smax = dd{-1, 0}; r.arg = -1; r.maxvs = 0;
     if (idx < (long)ntiles * 1024) {
@@ -99,8 +101,9 @@ __global__ void __launch_bounds__(256) k_finish1(
 }
 
 __global__ void __launch_bounds__(1024) k_finish2(const double* __restrict__ blockred, int nblocks, long N,
-                                                  shd_scalars* __restrict__ scal)
+                                                  shd_scalars* __restrict__ scal, const int* __restrict__ skip)
 {
+    if (skip && *skip) return;
     red r; r.phi = dd{0, 0}; r.smax = dd{-1, 0}; r.arg = -1; r.maxvs = 0;
     for (int b = threadIdx.x; b < nblocks; b += blockDim.x) {
         const double* o = blockred + (size_t)b * 8;
@@ -139,8 +142,9 @@ __device__ __forceinline__ limbs split_limbs(dd x) {
 __global__ void __launch_bounds__(256) k_ctable(
     int npb, int Qpad, const int* __restrict__ cell_kp, const int* __restrict__ cell_km, long M,
     const double* __restrict__ v, const double* __restrict__ rho, const shd_scalars* __restrict__ scal,
-    double* __restrict__ C)
+    double* __restrict__ C, const int* __restrict__ skip)
 {
+    if (skip && *skip) return;
     long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     long ncell = (long)npb * 32 * Qpad;
     if (idx >= ncell) return;
@@ -185,8 +189,8 @@ cudaError_t shd_launch_finish(shd_ctx* h)
     int nb = h->nfinish_blocks;
     k_finish1<<<nb, 256, 0, h->stream>>>(h->d_part, h->nsplit, h->ntiles, h->d_tile_pb, h->d_tile_qb,
                                          h->d_cell_kp, h->d_cell_km, h->Qpad, h->M, h->d_v, h->d_rho,
-                                         h->d_blockred);
-    k_finish2<<<1, 1024, 0, h->stream>>>(h->d_blockred, nb, h->N, h->d_scal);
+                                         h->d_blockred, h->d_skip);
+    k_finish2<<<1, 1024, 0, h->stream>>>(h->d_blockred, nb, h->N, h->d_scal, h->d_skip);
     h->last_launches += 2;
     return cudaGetLastError();
 }
@@ -195,7 +199,7 @@ cudaError_t shd_launch_ctable(shd_ctx* h)
 {
     long ncell = (long)h->npb * 32 * h->Qpad;
     k_ctable<<<(unsigned)((ncell + 255) / 256), 256, 0, h->stream>>>(
-        h->npb, h->Qpad, h->d_cell_kp, h->d_cell_km, h->M, h->d_v, h->d_rho, h->d_scal, h->d_C);
+        h->npb, h->Qpad, h->d_cell_kp, h->d_cell_km, h->M, h->d_v, h->d_rho, h->d_scal, h->d_C, h->d_skip);
     h->last_launches += 1;
     return cudaGetLastError();
 }

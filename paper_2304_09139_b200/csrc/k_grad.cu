@@ -65,8 +65,10 @@ __global__ void __launch_bounds__(TJ * TP, 1) k_grad(
     int d, long N, double L, long Npad, int npb, int Qpad, int Ppad, int qscale_log2,
     const int* __restrict__ qchunks, const int* __restrict__ wT,
     const double* __restrict__ A, const double* __restrict__ Bg, const double* __restrict__ C,
-    const shd_scalars* __restrict__ scal, double* __restrict__ grad_hi, double* __restrict__ grad_lo)
+    const shd_scalars* __restrict__ scal, double* __restrict__ grad_hi, double* __restrict__ grad_lo,
+    const int* __restrict__ skip)
 {
+    if (skip && *skip) return;
     extern __shared__ __align__(1024) unsigned char smem[];
     __shared__ __align__(8) unsigned long long bars[SHD_GRAD_STAGES];
     const int tid = threadIdx.x;
@@ -261,7 +263,7 @@ cudaError_t shd_launch_grad(shd_ctx* h, double* grad_hi, double* grad_lo)
 {
     k_grad<<<(unsigned)h->njb, TJ * TP, GSMEM, h->stream>>>(
         h->d, h->N, h->L, h->Npad, h->npb, h->Qpad, h->npb * 32, h->qscale_log2, h->d_qchunks, h->d_wT,
-        h->d_A, h->d_Bg, h->d_C, h->d_scal, grad_hi, grad_lo);
+        h->d_A, h->d_Bg, h->d_C, h->d_scal, grad_hi, grad_lo, h->d_skip);
     h->last_launches += 1;
     return cudaGetLastError();
 }

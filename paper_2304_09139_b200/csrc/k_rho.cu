@@ -66,8 +66,9 @@ __device__ __forceinline__ void flush_acc(Acc& a, dd& m) {
 __global__ void __launch_bounds__(TX * TY, 1) k_rho(
     const double* __restrict__ A, const double* __restrict__ B,
     const int* __restrict__ tile_pb, const int* __restrict__ tile_qb, int ntiles,
-    long Npad, long chunks_per_split, double* __restrict__ part)
+    long Npad, long chunks_per_split, double* __restrict__ part, const int* __restrict__ skip)
 {
+    if (skip && *skip) return;
     extern __shared__ __align__(1024) unsigned char smem[];
     __shared__ __align__(8) unsigned long long bars[SHD_RHO_STAGES];
     const int tid = threadIdx.x;
@@ -190,7 +191,7 @@ cudaError_t shd_launch_rho(shd_ctx* h)
 {
     unsigned grid = (unsigned)(h->ntiles * h->nsplit);
     k_rho<<<grid, TX * TY, SHD_RHO_STAGES * STAGE_BYTES, h->stream>>>(
-        h->d_A, h->d_B, h->d_tile_pb, h->d_tile_qb, h->ntiles, h->Npad, h->chunks_per_split, h->d_part);
+        h->d_A, h->d_B, h->d_tile_pb, h->d_tile_qb, h->ntiles, h->Npad, h->chunks_per_split, h->d_part, h->d_skip);
     h->last_launches += 1;
     return cudaGetLastError();
 }

@@ -81,8 +81,10 @@ __global__ void __launch_bounds__(128) k_tables(
     int d, long N, double L, long Npad, int P, int Qn, int S1d, int qscale_log2,
     const int* __restrict__ pn0, const int* __restrict__ pn1, int Qpad,
     const double* __restrict__ pos_hi, const double* __restrict__ pos_lo,
-    double* __restrict__ A, double* __restrict__ B, double* __restrict__ Bg, int with_grad)
+    double* __restrict__ A, double* __restrict__ B, double* __restrict__ Bg, int with_grad,
+    const int* __restrict__ skip)
 {
+    if (skip && *skip) return;
     long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
     int which = blockIdx.y;
     if (j >= N) return;
@@ -151,7 +153,7 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
     dim3 grid((unsigned)((h->N + 127) / 128), 2);
     k_tables<<<grid, 128, 0, h->stream>>>(h->d, h->N, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2,
                                          h->d_pn0, h->d_pn1, h->Qpad, pos_hi, pos_lo,
-                                         h->d_A, h->d_B, h->d_Bg, with_grad_tables ? 1 : 0);
+                                         h->d_A, h->d_B, h->d_Bg, with_grad_tables ? 1 : 0, h->d_skip);
     h->last_launches += 1;
     return cudaGetLastError();
 }

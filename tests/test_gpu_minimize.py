@@ -1,0 +1,119 @@
+"""Minimizer outcome tests (SURVEY.md 8(c) "Minimization oracle", D:R16): the quench has many correct
+results (degenerate ground-state manifold), so only the outcome is compared: the ORACLE's
+S_max on the GPU's final positions must be below the threshold, Phi must not increase, and P:64 /
+P:107 say no run may get stuck for chi < 1/2 (d >= 2)."""
+import numpy as np
+import pytest
+
+from paper_2304_09139_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def shd():
+    from paper_2304_09139_b200 import shd as m
+    return m
+
+
+def oracle_smax(oracle, d, N, L, m_star, hi, lo):
+    n = oracle.enumerate_Q(d, m_star)
+    re, im = oracle.rho(d, N, L, hi, lo, n)
+    phi, smax, arg, s2 = oracle.energy(N, re, im)
+    return oracle.to_float(smax)[0], oracle.to_float(phi)[0]
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_cfg1_quench_reaches_1e30(shd, oracle, seed):
+    """BASELINE.json configs[0]: full L-BFGS minimization to S_max < 1e-30, every seed."""
+    cfg = inputs.CONFIGS["cfg1"]
+    hi, lo = inputs.uniform_positions(cfg, seed)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    th, tl = shd.from_host(hi, lo)
+    phi0, _, _ = h.energy_grad(th, tl, want_grad=False)
+    rep = h.minimize(th, tl, smax_tol=1e-30, max_evals=5000)
+    assert rep["status"] == shd.SHD_OK, rep
+    assert rep["smax"][0] < 1e-30
+    assert rep["evals"] <= 1.5 * rep["iters"] + 10, "backtracking should be rare"
+    s_or, phi_or = oracle_smax(oracle, cfg.d, cfg.N, cfg.L, cfg.m_star, th.cpu().numpy(), tl.cpu().numpy())
+    print(seed, rep, s_or)
+    assert s_or < 1e-30, f"oracle S_max on the GPU's final positions: {s_or:.3e}"
+    assert abs(s_or - rep["smax"][0]) <= 1e-3 * s_or + 1e-40
+    assert phi_or < phi0[0] * 1e-25
+    # the reported Phi belongs to the returned positions
+    phi1, _, _ = h.energy_grad(th, tl, want_grad=False)
+    assert phi1[0] == rep["phi"][0] and phi1[1] == rep["phi"][1]
+    h.close()
+
+
+def test_oracle_quench_same_outcome(shd, oracle):
+    """The binary128 textbook L-BFGS (oracle) and the device L-BFGS both reach the ground-state
+    manifold from the same start; trajectories are not compared (D:R16)."""
+    cfg = inputs.CONFIGS["cfg1"]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    n = oracle.enumerate_Q(cfg.d, cfg.m_star)
+    o = oracle.minimize_lbfgs(cfg.d, cfg.N, cfg.L, hi, lo, n, smax_tol=1e-30, max_evals=3000)
+    assert o["status"] == 0 and oracle.to_float(o["smax"])[0] < 1e-30
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    th, tl = shd.from_host(hi, lo)
+    rep = h.minimize(th, tl, smax_tol=1e-30, max_evals=3000)
+    assert rep["status"] == shd.SHD_OK
+    print("oracle iters", o["iters"], "gpu iters", rep["iters"])
+    assert rep["iters"] < 3 * o["iters"] + 50
+    h.close()
+
+
+def test_max_evals_and_reentry(shd, oracle):
+    """SHD_EMAXEVAL still writes the report and leaves the last accepted point in pos; calling again
+    continues from there; Phi never increases across calls."""
+    d, N, L, m_star = 2, 500, 22.0, 300
+    hi, lo = inputs.uniform_positions_raw(d, N, L, 3)
+    h = shd.Shd(d, N, L, m_star=m_star)
+    th, tl = shd.from_host(hi, lo)
+    phi_prev = h.energy_grad(th, tl, want_grad=False)[0][0]
+    total = 0
+    for _ in range(60):
+        rep = h.minimize(th, tl, smax_tol=1e-30, max_evals=60, poll_every=7)
+        assert rep["status"] in (shd.SHD_OK, shd.SHD_EMAXEVAL)
+        assert rep["evals"] <= 60
+        total += rep["evals"]
+        phi_now = h.energy_grad(th, tl, want_grad=False)[0]
+        assert phi_now[0] == rep["phi"][0]
+        assert phi_now[0] <= phi_prev
+        phi_prev = phi_now[0]
+        if rep["status"] == shd.SHD_OK:
+            break
+    assert rep["status"] == shd.SHD_OK, (rep, total)
+    s_or, _ = oracle_smax(oracle, d, N, L, m_star, th.cpu().numpy(), tl.cpu().numpy())
+    assert s_or < 1e-30
+    h.close()
+
+
+@pytest.mark.parametrize("d,N,L,m_star,hist", [(1, 300, 300.0, 40 * 40, 5), (3, 216, 6.0, 14, 10), (2, 400, 20.0, 200, 32)])
+def test_quench_other_dimensions(shd, oracle, d, N, L, m_star, hist):
+    hi, lo = inputs.uniform_positions_raw(d, N, L, 11)
+    h = shd.Shd(d, N, L, m_star=m_star)
+    chi = h.M / (d * (N - 1))
+    assert chi < (1 / 3 if d == 1 else 1 / 2)
+    th, tl = shd.from_host(hi, lo)
+    rep = h.minimize(th, tl, history=hist, smax_tol=1e-30, max_evals=20000, poll_every=16)
+    print(d, N, chi, rep)
+    assert rep["status"] == shd.SHD_OK, rep
+    s_or, _ = oracle_smax(oracle, d, N, L, m_star, th.cpu().numpy(), tl.cpu().numpy())
+    assert s_or < 1e-30
+    h.close()
+
+
+def test_minimize_argument_errors(shd):
+    h = shd.Shd(2, 64, 8.0, m_star=9)
+    hi, lo = inputs.uniform_positions_raw(2, 64, 8.0, 0)
+    th, tl = shd.from_host(hi, lo)
+    for kw in (dict(history=33), dict(max_evals=0), dict(poll_every=0), dict(kind=7)):
+        with pytest.raises(shd.ShdError) as e:
+            h.minimize(th, tl, **kw)
+        assert e.value.code == shd.SHD_EINVAL
+    bad = th.clone(); bad[3] = float("nan")
+    with pytest.raises(shd.ShdError) as e:
+        h.minimize(bad, tl)
+    assert e.value.code == shd.SHD_ENAN
+    h.close()
