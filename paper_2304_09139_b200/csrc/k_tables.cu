@@ -75,9 +75,45 @@ __device__ __forceinline__ void store_entry(double* base, size_t ps, cdd z) {
 }
 
 constexpr int R3MAX = 128;   // d == 3: max |n_1| supported by the local power table
+constexpr int TB = 64;       // particles (threads) per block
+constexpr int TG = 8;        // table entries staged per flush: 8 x 16 B = one 128-byte line per limb plane
+
+// Staging tile for the rho-layout tables  T[block][Npad][limb 4][32 entries][re,im]:
+// a thread owns one particle, so its 16-byte stores would land 2 KB apart in global memory.  They go to
+// shared memory instead (tile[particle][limb][TG entries], 16-byte chunks XOR-swizzled by the particle
+// index against bank conflicts) and the block then writes full 128-byte lines.
+struct Stager {
+    double2* tile;        // [TB][4][TG]
+    double* table;        // A or B
+    long Npad, j0, N;
+    __device__ __forceinline__ void put(int slot, cdd z) {
+        limbs a = split_limbs(z.re), b = split_limbs(z.im);
+        const int t = threadIdx.x, c = slot ^ (t & 7);
+        double2* row = tile + t * (4 * TG);
+        row[0 * TG + c] = make_double2(a.x0, b.x0);
+        row[1 * TG + c] = make_double2(a.x1, b.x1);
+        row[2 * TG + c] = make_double2(a.x2, b.x2);
+        row[3 * TG + c] = make_double2(a.x12, b.x12);
+    }
+    // entries e0 .. e0+count-1 (e0 a multiple of TG) of every particle of the block
+    __device__ __forceinline__ void flush(int e0, int count) {
+        __syncthreads();
+        const int blk = e0 >> 5, off = e0 & 31;
+        for (int piece = threadIdx.x; piece < TB * 4 * TG; piece += TB) {
+            const int c = piece & 7, l = (piece >> 3) & 3, jj = piece >> 5;
+            const long j = j0 + jj;
+            if (c < count && j < N) {
+                double2 v = tile[jj * (4 * TG) + l * TG + (c ^ (jj & 7))];
+                double2* dst = reinterpret_cast<double2*>(table) + (((size_t)blk * Npad + j) * 4 + l) * 32 + off + c;
+                *dst = v;
+            }
+        }
+        __syncthreads();
+    }
+};
 
 // which = 0: A table.  which = 1: B table (+ gradient-layout Bg with q-weighted copy).
-__global__ void __launch_bounds__(128) k_tables(
+__global__ void __launch_bounds__(TB) k_tables(
     int d, long N, double L, long Npad, int P, int Qn, int S1d, int qscale_log2,
     const int* __restrict__ pn0, const int* __restrict__ pn1, int Qpad,
     const double* __restrict__ pos_hi, const double* __restrict__ pos_lo,
@@ -85,25 +121,31 @@ __global__ void __launch_bounds__(128) k_tables(
     const int* __restrict__ skip)
 {
     if (skip && *skip) return;
-    long j = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    int which = blockIdx.y;
-    if (j >= N) return;
+    __shared__ __align__(16) double2 tile[TB * 4 * TG];
+    const int which = blockIdx.y;
+    const long j0 = (long)blockIdx.x * TB;
+    const long j = j0 + threadIdx.x;
+    const bool live = j < N;
+    const long jc = live ? j : N - 1;            // dead threads shadow the last particle (keeps barriers uniform)
     const cdd one{dd{1.0, 0.0}, dd{0.0, 0.0}};
+    Stager st{tile, which == 0 ? A : B, Npad, j0, N};
     if (which == 0) {
         // ---- A table
         cdd base;
-        if (d == 1) base = expi_turns(frac_turns(pos_hi[j], pos_lo[j], L, (double)S1d));
-        else base = expi_turns(frac_turns(pos_hi[j], pos_lo[j], L, 1.0));
+        if (d == 1) base = expi_turns(frac_turns(pos_hi[jc], pos_lo[jc], L, (double)S1d));
+        else base = expi_turns(frac_turns(pos_hi[jc], pos_lo[jc], L, 1.0));
         if (d <= 2) {
             cdd cur = one;
-            for (int p = 0; p < P; p++) {
-                int pb = p >> 5, pi = p & 31;
-                double* dst = A + ((((size_t)pb * Npad + j) * 4) * 32 + pi) * 2;
-                store_entry(dst, 64, cur);
-                cur = cdd_mul(cur, base);
+            for (int p0 = 0; p0 < P; p0 += TG) {
+                const int cnt = min(TG, P - p0);
+                for (int s = 0; s < cnt; s++) {
+                    st.put(s, cur);
+                    cur = cdd_mul(cur, base);
+                }
+                st.flush(p0, cnt);
             }
         } else {
-            cdd z1 = expi_turns(frac_turns(pos_hi[N + j], pos_lo[N + j], L, 1.0));
+            cdd z1 = expi_turns(frac_turns(pos_hi[N + jc], pos_lo[N + jc], L, 1.0));
             cdd pw1[R3MAX + 1];
             int r1max = 0;
             for (int p = 0; p < P; p++) { int a = abs(pn1[p]); r1max = a > r1max ? a : r1max; }
@@ -111,37 +153,41 @@ __global__ void __launch_bounds__(128) k_tables(
             for (int m = 1; m <= r1max; m++) pw1[m] = cdd_mul(pw1[m - 1], z1);
             cdd cur0 = one;
             int n0cur = 0;
-            for (int p = 0; p < P; p++) {
-                int n0 = pn0[p], n1 = pn1[p];
-                while (n0cur < n0) { cur0 = cdd_mul(cur0, base); n0cur++; }
-                cdd f = n1 >= 0 ? pw1[n1] : cdd_conj(pw1[-n1]);
-                cdd e = cdd_mul(cur0, f);
-                int pb = p >> 5, pi = p & 31;
-                double* dst = A + ((((size_t)pb * Npad + j) * 4) * 32 + pi) * 2;
-                store_entry(dst, 64, e);
+            for (int p0 = 0; p0 < P; p0 += TG) {
+                const int cnt = min(TG, P - p0);
+                for (int s = 0; s < cnt; s++) {
+                    const int n0 = pn0[p0 + s], n1 = pn1[p0 + s];
+                    while (n0cur < n0) { cur0 = cdd_mul(cur0, base); n0cur++; }
+                    cdd f = n1 >= 0 ? pw1[n1] : cdd_conj(pw1[-n1]);
+                    st.put(s, cdd_mul(cur0, f));
+                }
+                st.flush(p0, cnt);
             }
         }
     } else {
         // ---- B table: powers of the last axis' base phasor
-        int a = d - 1;
-        cdd base = expi_turns(frac_turns(pos_hi[(size_t)a * N + j], pos_lo[(size_t)a * N + j], L, 1.0));
+        const int a = d - 1;
+        cdd base = expi_turns(frac_turns(pos_hi[(size_t)a * N + jc], pos_lo[(size_t)a * N + jc], L, 1.0));
         cdd cur = one;
-        double qs = ldexp(1.0, -qscale_log2);
-        long jb = j >> 5;
-        int jj = (int)(j & 31);
-        for (int q = 0; q < Qn; q++) {
-            int qb = q >> 5, qi = q & 31;
-            double* dst = B + ((((size_t)qb * Npad + j) * 4) * 32 + qi) * 2;
-            store_entry(dst, 64, cur);
-            if (with_grad) {
-                double* g = Bg + ((((size_t)jb * Qpad + q) * 8) * 32 + jj) * 2;
-                store_entry(g, 64, cur);
-                cdd w;
-                w.re = dd_scale2(dd_mul_d(cur.re, (double)q), qs);
-                w.im = dd_scale2(dd_mul_d(cur.im, (double)q), qs);
-                store_entry(g + 4 * 64, 64, w);
+        const double qs = ldexp(1.0, -qscale_log2);
+        const long jb = j >> 5;
+        const int jj = (int)(j & 31);
+        for (int q0 = 0; q0 < Qn; q0 += TG) {
+            const int cnt = min(TG, Qn - q0);
+            for (int s = 0; s < cnt; s++) {
+                const int q = q0 + s;
+                st.put(s, cur);
+                if (with_grad && live) {   // gradient layout: consecutive threads write consecutive 16 B
+                    double* g = Bg + ((((size_t)jb * Qpad + q) * 8) * 32 + jj) * 2;
+                    store_entry(g, 64, cur);
+                    cdd w;
+                    w.re = dd_scale2(dd_mul_d(cur.re, (double)q), qs);
+                    w.im = dd_scale2(dd_mul_d(cur.im, (double)q), qs);
+                    store_entry(g + 4 * 64, 64, w);
+                }
+                cur = cdd_mul(cur, base);
             }
-            cur = cdd_mul(cur, base);
+            st.flush(q0, cnt);
         }
     }
 }
@@ -150,8 +196,8 @@ __global__ void __launch_bounds__(128) k_tables(
 
 cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool with_grad_tables)
 {
-    dim3 grid((unsigned)((h->N + 127) / 128), 2);
-    k_tables<<<grid, 128, 0, h->stream>>>(h->d, h->N, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2,
+    dim3 grid((unsigned)((h->N + TB - 1) / TB), 2);
+    k_tables<<<grid, TB, 0, h->stream>>>(h->d, h->N, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2,
                                          h->d_pn0, h->d_pn1, h->Qpad, pos_hi, pos_lo,
                                          h->d_A, h->d_B, h->d_Bg, with_grad_tables ? 1 : 0, h->d_skip);
     h->last_launches += 1;
