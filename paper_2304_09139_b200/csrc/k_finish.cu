@@ -124,7 +124,7 @@ __global__ void __launch_bounds__(1024) k_finish2(const double* __restrict__ blo
     }
 }
 
-struct limbs { double x0, x1, x2, x12; };
+struct limbs { double x0, x1, x2; };
 __device__ __forceinline__ limbs split_limbs(dd x) {
     const double C0 = 1.5 * 4503599627370496.0 / (double)(1 << SHD_W0);
     const double C1 = 1.5 * 4503599627370496.0 / ((double)(1 << SHD_W0) * (double)(1 << SHD_W1));
@@ -133,12 +133,12 @@ __device__ __forceinline__ limbs split_limbs(dd x) {
     double rem = __dadd_rn(x.h, -r.x0);
     r.x1 = __dadd_rn(__dadd_rn(rem, C1), -C1);
     r.x2 = __dadd_rn(__dadd_rn(rem, -r.x1), x.l);
-    r.x12 = __dadd_rn(r.x1, r.x2);
     return r;
 }
 
 // C[p,q]: C1 = W+ + W-,  C2 = -i (W+ - W-),  W = v rho, scaled by cscale (a power of two).
-// layout [pb][q][plane 8][32 p][2]; plane l: (C1r_l, C1i_l), plane 4+l: (C2r_l, C2i_l).
+// layout [pb][q/4][plane 6][32 p][q%4][re,im]; plane l: (C1r_l, C1i_l), plane 3+l: (C2r_l, C2i_l)
+// (fragment-major for the gradient pass, shd_internal.h).
 __global__ void __launch_bounds__(256) k_ctable(
     int npb, int Qpad, const int* __restrict__ cell_kp, const int* __restrict__ cell_km, long M,
     const double* __restrict__ v, const double* __restrict__ rho, const shd_scalars* __restrict__ scal,
@@ -148,12 +148,12 @@ __global__ void __launch_bounds__(256) k_ctable(
     long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
     long ncell = (long)npb * 32 * Qpad;
     if (idx >= ncell) return;
-    // idx enumerates (pb, q, pi) with pi fastest so that stores are coalesced
-    int pi = (int)(idx & 31);
-    long t = idx >> 5;
-    int q = (int)(t % Qpad);
-    int pb = (int)(t / Qpad);
-    int p = pb * 32 + pi;
+    // idx enumerates (pb, q/4, p%32, q%4) with q%4 fastest so that stores are coalesced
+    const int q4 = (int)(idx & 3), pi = (int)((idx >> 2) & 31);
+    long t = idx >> 7;
+    const int qg = (int)(t % (Qpad / 4));
+    const int pb = (int)(t / (Qpad / 4));
+    const int p = pb * 32 + pi, q = qg * 4 + q4;
     int kp = cell_kp[(size_t)p * Qpad + q], km = cell_km[(size_t)p * Qpad + q];
     double sc = scal->cscale;
     dd wpr{0, 0}, wpi{0, 0}, wmr{0, 0}, wmi{0, 0};
@@ -171,15 +171,13 @@ __global__ void __launch_bounds__(256) k_ctable(
     dd dr = dd_sub(wpr, wmr), di = dd_sub(wpi, wmi);
     dd c2r = di, c2i = dd_neg(dr);                 // -i (dr + i di) = di - i dr
     limbs a = split_limbs(c1r), b = split_limbs(c1i), c = split_limbs(c2r), e = split_limbs(c2i);
-    double* dst = C + ((((size_t)pb * Qpad + q) * 8) * 32 + pi) * 2;
-    *reinterpret_cast<double2*>(dst + 0 * 64) = make_double2(a.x0, b.x0);
-    *reinterpret_cast<double2*>(dst + 1 * 64) = make_double2(a.x1, b.x1);
-    *reinterpret_cast<double2*>(dst + 2 * 64) = make_double2(a.x2, b.x2);
-    *reinterpret_cast<double2*>(dst + 3 * 64) = make_double2(a.x12, b.x12);
-    *reinterpret_cast<double2*>(dst + 4 * 64) = make_double2(c.x0, e.x0);
-    *reinterpret_cast<double2*>(dst + 5 * 64) = make_double2(c.x1, e.x1);
-    *reinterpret_cast<double2*>(dst + 6 * 64) = make_double2(c.x2, e.x2);
-    *reinterpret_cast<double2*>(dst + 7 * 64) = make_double2(c.x12, e.x12);
+    double2* dst = reinterpret_cast<double2*>(C) + ((((size_t)pb * (Qpad / 4) + qg) * 6) * 32 + pi) * 4 + q4;
+    dst[0 * 128] = make_double2(a.x0, b.x0);
+    dst[1 * 128] = make_double2(a.x1, b.x1);
+    dst[2 * 128] = make_double2(a.x2, b.x2);
+    dst[3 * 128] = make_double2(c.x0, e.x0);
+    dst[4 * 128] = make_double2(c.x1, e.x1);
+    dst[5 * 128] = make_double2(c.x2, e.x2);
 }
 
 }  // namespace

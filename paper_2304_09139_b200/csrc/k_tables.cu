@@ -50,7 +50,7 @@ __device__ cdd expi_turns(dd t) {
     return cdd_mul(root, w);
 }
 
-struct limbs { double x0, x1, x2, x12; };
+struct limbs { double x0, x1, x2; };
 
 // |x| <= 1 (normalised dd) -> limbs (shd_internal.h)
 __device__ __forceinline__ limbs split_limbs(dd x) {
@@ -61,51 +61,67 @@ __device__ __forceinline__ limbs split_limbs(dd x) {
     double rem = __dadd_rn(x.h, -r.x0);          // exact
     r.x1 = __dadd_rn(__dadd_rn(rem, C1), -C1);
     r.x2 = __dadd_rn(__dadd_rn(rem, -r.x1), x.l);
-    r.x12 = __dadd_rn(r.x1, r.x2);
     return r;
-}
-
-// write one complex entry (4 limb pairs) at plane stride `ps` doubles
-__device__ __forceinline__ void store_entry(double* base, size_t ps, cdd z) {
-    limbs a = split_limbs(z.re), b = split_limbs(z.im);
-    *reinterpret_cast<double2*>(base) = make_double2(a.x0, b.x0);
-    *reinterpret_cast<double2*>(base + ps) = make_double2(a.x1, b.x1);
-    *reinterpret_cast<double2*>(base + 2 * ps) = make_double2(a.x2, b.x2);
-    *reinterpret_cast<double2*>(base + 3 * ps) = make_double2(a.x12, b.x12);
 }
 
 constexpr int R3MAX = 128;   // d == 3: max |n_1| supported by the local power table
 constexpr int TB = 64;       // particles (threads) per block
-constexpr int TG = 8;        // table entries staged per flush: 8 x 16 B = one 128-byte line per limb plane
+constexpr int TG = 8;        // table entries staged per flush: 8 x 16 B = one 128-byte row per limb plane
+constexpr int TABLES_SMEM = TB * 6 * TG * 16;
 
-// Staging tile for the rho-layout tables  T[block][Npad][limb 4][32 entries][re,im]:
-// a thread owns one particle, so its 16-byte stores would land 2 KB apart in global memory.  They go to
-// shared memory instead (tile[particle][limb][TG entries], 16-byte chunks XOR-swizzled by the particle
-// index against bank conflicts) and the block then writes full 128-byte lines.
+// Staging tile: a thread owns one particle, so its 16-byte stores would land far apart in global
+// memory.  They go to shared memory instead (tile[particle][plane][TG entries], 16-byte chunks
+// XOR-swizzled by the bit-reversed particle index: conflict-free for the writes and for both read
+// patterns below) and the block then writes runs of 512 contiguous bytes:
+//   rho layout       T[block][j/4][limb 3][32 entries][j%4][re,im]            (A and B)
+//   gradient layout  Bg[j/32][q/4][plane 6: b limbs, (q b) limbs][j%32][q%4][re,im]
 struct Stager {
-    double2* tile;        // [TB][4][TG]
+    double2* tile;        // [TB][planes][TG]
+    int planes;           // 3 (A, B) or 6 (B with the q-weighted copy for the gradient pass)
     double* table;        // A or B
+    double* Bg;           // gradient layout (or nullptr)
     long Npad, j0, N;
-    __device__ __forceinline__ void put(int slot, cdd z) {
+    int Qpad;
+    __device__ __forceinline__ static int swz(int r) { return ((r & 1) << 2) | (r & 2) | ((r >> 2) & 1); }
+    __device__ __forceinline__ void put(int plane0, int slot, cdd z) {
         limbs a = split_limbs(z.re), b = split_limbs(z.im);
-        const int t = threadIdx.x, c = slot ^ (t & 7);
-        double2* row = tile + t * (4 * TG);
+        const int t = threadIdx.x, c = slot ^ swz(t);
+        double2* row = tile + (t * planes + plane0) * TG;
         row[0 * TG + c] = make_double2(a.x0, b.x0);
         row[1 * TG + c] = make_double2(a.x1, b.x1);
         row[2 * TG + c] = make_double2(a.x2, b.x2);
-        row[3 * TG + c] = make_double2(a.x12, b.x12);
     }
     // entries e0 .. e0+count-1 (e0 a multiple of TG) of every particle of the block
     __device__ __forceinline__ void flush(int e0, int count) {
         __syncthreads();
         const int blk = e0 >> 5, off = e0 & 31;
-        for (int piece = threadIdx.x; piece < TB * 4 * TG; piece += TB) {
-            const int c = piece & 7, l = (piece >> 3) & 3, jj = piece >> 5;
-            const long j = j0 + jj;
+        // rho layout: piece -> (group, limb, entry, j%4), j%4 fastest
+        for (int piece = threadIdx.x; piece < (TB / 4) * 3 * TG * 4; piece += TB) {
+            const int jj = piece & 3, c = (piece >> 2) & 7, l = (piece >> 5) % 3, jg = piece / 96;
+            const int row = jg * 4 + jj;
+            const long j = j0 + row;
             if (c < count && j < N) {
-                double2 v = tile[jj * (4 * TG) + l * TG + (c ^ (jj & 7))];
-                double2* dst = reinterpret_cast<double2*>(table) + (((size_t)blk * Npad + j) * 4 + l) * 32 + off + c;
+                double2 v = tile[(row * planes + l) * TG + (c ^ swz(row))];
+                double2* dst = reinterpret_cast<double2*>(table) +
+                               ((((size_t)blk * (Npad / 4) + (j >> 2)) * 3 + l) * 32 + off + c) * 4 + jj;
                 *dst = v;
+            }
+        }
+        if (Bg != nullptr) {
+            // gradient layout: piece -> (j/32, q-group, plane, j%32, q%4), q%4 fastest
+            for (int piece = threadIdx.x; piece < TB * 6 * TG; piece += TB) {
+                const int q4 = piece & 3, jl = (piece >> 2) & 31;
+                int rest = piece >> 7;
+                const int pl = rest % 6; rest /= 6;
+                const int qg = rest & 1, jbl = rest >> 1;
+                const int row = jbl * 32 + jl, c = qg * 4 + q4;
+                const long j = j0 + row;
+                if (c < count && j < N) {
+                    double2 v = tile[(row * planes + pl) * TG + (c ^ swz(row))];
+                    double2* dst = reinterpret_cast<double2*>(Bg) +
+                                   ((((size_t)(j >> 5) * (Qpad / 4) + ((e0 + c) >> 2)) * 6 + pl) * 32 + jl) * 4 + q4;
+                    *dst = v;
+                }
             }
         }
         __syncthreads();
@@ -121,14 +137,16 @@ __global__ void __launch_bounds__(TB) k_tables(
     const int* __restrict__ skip)
 {
     if (skip && *skip) return;
-    __shared__ __align__(16) double2 tile[TB * 4 * TG];
+    extern __shared__ __align__(16) unsigned char tables_smem[];
+    double2* tile = reinterpret_cast<double2*>(tables_smem);
     const int which = blockIdx.y;
     const long j0 = (long)blockIdx.x * TB;
     const long j = j0 + threadIdx.x;
     const bool live = j < N;
     const long jc = live ? j : N - 1;            // dead threads shadow the last particle (keeps barriers uniform)
     const cdd one{dd{1.0, 0.0}, dd{0.0, 0.0}};
-    Stager st{tile, which == 0 ? A : B, Npad, j0, N};
+    const bool gradB = which == 1 && with_grad != 0;
+    Stager st{tile, gradB ? 6 : 3, which == 0 ? A : B, gradB ? Bg : nullptr, Npad, j0, N, Qpad};
     if (which == 0) {
         // ---- A table
         cdd base;
@@ -139,7 +157,7 @@ __global__ void __launch_bounds__(TB) k_tables(
             for (int p0 = 0; p0 < P; p0 += TG) {
                 const int cnt = min(TG, P - p0);
                 for (int s = 0; s < cnt; s++) {
-                    st.put(s, cur);
+                    st.put(0, s, cur);
                     cur = cdd_mul(cur, base);
                 }
                 st.flush(p0, cnt);
@@ -159,7 +177,7 @@ __global__ void __launch_bounds__(TB) k_tables(
                     const int n0 = pn0[p0 + s], n1 = pn1[p0 + s];
                     while (n0cur < n0) { cur0 = cdd_mul(cur0, base); n0cur++; }
                     cdd f = n1 >= 0 ? pw1[n1] : cdd_conj(pw1[-n1]);
-                    st.put(s, cdd_mul(cur0, f));
+                    st.put(0, s, cdd_mul(cur0, f));
                 }
                 st.flush(p0, cnt);
             }
@@ -170,20 +188,16 @@ __global__ void __launch_bounds__(TB) k_tables(
         cdd base = expi_turns(frac_turns(pos_hi[(size_t)a * N + jc], pos_lo[(size_t)a * N + jc], L, 1.0));
         cdd cur = one;
         const double qs = ldexp(1.0, -qscale_log2);
-        const long jb = j >> 5;
-        const int jj = (int)(j & 31);
         for (int q0 = 0; q0 < Qn; q0 += TG) {
             const int cnt = min(TG, Qn - q0);
             for (int s = 0; s < cnt; s++) {
                 const int q = q0 + s;
-                st.put(s, cur);
-                if (with_grad && live) {   // gradient layout: consecutive threads write consecutive 16 B
-                    double* g = Bg + ((((size_t)jb * Qpad + q) * 8) * 32 + jj) * 2;
-                    store_entry(g, 64, cur);
+                st.put(0, s, cur);
+                if (gradB) {
                     cdd w;
                     w.re = dd_scale2(dd_mul_d(cur.re, (double)q), qs);
                     w.im = dd_scale2(dd_mul_d(cur.im, (double)q), qs);
-                    store_entry(g + 4 * 64, 64, w);
+                    st.put(3, s, w);
                 }
                 cur = cdd_mul(cur, base);
             }
@@ -194,10 +208,15 @@ __global__ void __launch_bounds__(TB) k_tables(
 
 }  // namespace
 
+cudaError_t shd_tables_configure()
+{
+    return cudaFuncSetAttribute(k_tables, cudaFuncAttributeMaxDynamicSharedMemorySize, TABLES_SMEM);
+}
+
 cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool with_grad_tables)
 {
     dim3 grid((unsigned)((h->N + TB - 1) / TB), 2);
-    k_tables<<<grid, TB, 0, h->stream>>>(h->d, h->N, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2,
+    k_tables<<<grid, TB, TABLES_SMEM, h->stream>>>(h->d, h->N, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2,
                                          h->d_pn0, h->d_pn1, h->Qpad, pos_hi, pos_lo,
                                          h->d_A, h->d_B, h->d_Bg, with_grad_tables ? 1 : 0, h->d_skip);
     h->last_launches += 1;

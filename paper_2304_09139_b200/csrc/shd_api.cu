@@ -191,11 +191,10 @@ int build(shd_ctx* h, const double* v) {
     if ((rc = upload(h, &h->d_tile_qb, tile_qb))) return rc;
     if ((rc = upload(h, &h->d_qchunks, qchunks))) return rc;
     if (!h->v.empty()) { if ((rc = upload(h, &h->d_v, h->v))) return rc; }
-    const size_t slab = SHD_TILE_ENTRY_DOUBLES;
-    if ((rc = dalloc_zero(h, &h->d_A, (size_t)h->npb * h->Npad * slab))) return rc;
-    if ((rc = dalloc_zero(h, &h->d_B, (size_t)h->nqb * h->Npad * slab))) return rc;
-    if ((rc = dalloc_zero(h, &h->d_Bg, (size_t)h->njb * h->Qpad * 2 * slab))) return rc;
-    if ((rc = dalloc_zero(h, &h->d_C, (size_t)h->npb * h->Qpad * 2 * slab))) return rc;
+    if ((rc = dalloc_zero(h, &h->d_A, (size_t)h->npb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
+    if ((rc = dalloc_zero(h, &h->d_B, (size_t)h->nqb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
+    if ((rc = dalloc_zero(h, &h->d_Bg, (size_t)h->njb * (h->Qpad / 4) * SHD_GGROUP_DOUBLES))) return rc;
+    if ((rc = dalloc_zero(h, &h->d_C, (size_t)h->npb * (h->Qpad / 4) * SHD_GGROUP_DOUBLES))) return rc;
     if ((rc = dalloc_zero(h, &h->d_part, (size_t)h->nsplit * h->ntiles * 4 * 1024 * 2))) return rc;
     if ((rc = dalloc_zero(h, &h->d_rho, (size_t)4 * h->M))) return rc;
     h->nfinish_blocks = (int)(((long)h->ntiles * 1024 + 255) / 256);
@@ -204,6 +203,7 @@ int build(shd_ctx* h, const double* v) {
     CU(cudaMemset(h->d_scal, 0, sizeof(shd_scalars)));
     CU(cudaMallocHost((void**)&h->h_scal, sizeof(shd_scalars)));
     std::memset(h->h_scal, 0, sizeof(shd_scalars));
+    CU(shd_tables_configure());
     CU(shd_rho_configure());
     CU(shd_grad_configure());
     return SHD_OK;

@@ -10,14 +10,21 @@
 // so that rho(+/-)[p,q] = sum_j A_j[p] B_j[q]^(+/-) is a contraction over particles (rho pass) and
 // the gradient is a contraction over q followed by one over p (gradient pass).
 //
-// Each real operand x (|x| <= 1) is stored as four "limbs" (x0, x1, x2, x12):
+// Each real operand x (|x| <= 1) is stored as three "limbs" (x0, x1, x2):
 //   x0  = x rounded to a multiple of 2^-W0,  x1 = (x - x0) rounded to a multiple of 2^-(W0+W1),
-//   x2  = x - x0 - x1 (a free double),       x12 = x1 + x2,
+//   x2  = x - x0 - x1 (a free double);   x12 = x1 + x2 is formed in registers,
 // and a product-accumulate  acc += x*y  is the 6 FMAs
 //   L0 += x0 y0 ;  L1 += x0 y1 + x1 y0 ;  L2 += x0 y2 + x2 y0 + x12 y12
 // where L0 and L1 are EXACT (all partial sums representable) for bursts of <= 128 terms, and
 // L2 carries the terms below 2^-45 in plain FP64 (error ~2^-100 per term).  Bursts are folded
 // into ordinary double-double accumulators with TwoSum.
+//
+// The FMAs are issued as FP64 matrix instructions (mma.sync m8n8k4, SASS DMMA.8x8x4: 256 FMAs per
+// warp instruction on the same FP64 pipe and at the same peak rate as DFMA, measured), with the
+// contraction index (particles in the rho pass, q in the gradient pass) as the k dimension.  The
+// tables are therefore stored "fragment-major": groups of 4 consecutive contraction indices, and
+// inside a group  [limb 3][entry 32][index-in-group 4][re,im]  so that the 32 lanes of a warp
+// (entry = lane/4, index = lane%4) read one contiguous 512-byte run with LDS.128.
 #pragma once
 #include <cuda_runtime.h>
 #include <cstddef>
@@ -26,16 +33,17 @@
 
 constexpr int SHD_PT = 32;          // A-entries (p) per tile
 constexpr int SHD_QT = 32;          // B-entries (q) per tile
-constexpr int SHD_NPS = 16;         // particles per rho-pass pipeline stage
-constexpr int SHD_RHO_STAGES = 3;   // TMA pipeline depth, rho pass
+constexpr int SHD_NPS = 8;          // particles per rho-pass pipeline stage (2 groups of 4)
+constexpr int SHD_RHO_STAGES = 6;   // TMA pipeline depth, rho pass
 constexpr int SHD_BURST = 128;      // products per exact burst (see header comment)
-constexpr int SHD_QCH = 8;          // q per gradient-pass pipeline stage
-constexpr int SHD_GRAD_STAGES = 2;  // TMA pipeline depth, gradient pass
+constexpr int SHD_QCH = 4;          // q per gradient-pass pipeline stage (1 group of 4)
+constexpr int SHD_GRAD_STAGES = 6;  // TMA pipeline depth, gradient pass
 constexpr int SHD_JT = 32;          // particles per gradient-pass block
 constexpr int SHD_W0 = 23;          // limb widths (bits)
 constexpr int SHD_W1 = 22;
-constexpr int SHD_ENTRY_DOUBLES = 8;            // (re,im) x 4 limbs
-constexpr int SHD_TILE_ENTRY_DOUBLES = 32 * 8;  // one (block, particle) slab: 2 KB
+constexpr int SHD_NLIMB = 3;
+constexpr int SHD_GROUP_DOUBLES = SHD_NLIMB * 32 * 4 * 2;   // one (block, group of 4) slab of A / B: 6 KB
+constexpr int SHD_GGROUP_DOUBLES = 2 * SHD_GROUP_DOUBLES;   // gradient operands: 6 planes (Bg: b, q b; C: C1, C2)
 
 // launch groups timed by shd_set_timing: tables (a1), rho (a2), finish (a3), ctable, grad (a4)
 constexpr int SHD_NKERN = 5;
@@ -83,10 +91,10 @@ struct shd_ctx {
     int *d_qchunks = nullptr;  // [npb] number of q-chunks (of SHD_QCH) with any valid cell
     double *d_v = nullptr;     // [M]
     // device: per-evaluation data
-    double *d_A = nullptr;     // [npb][Npad][4][32][2]
-    double *d_B = nullptr;     // [nqb][Npad][4][32][2]
-    double *d_Bg = nullptr;    // [njb][Qpad][8][32][2]
-    double *d_C = nullptr;     // [npb][Qpad][8][32][2]
+    double *d_A = nullptr;     // [npb][Npad/4][3 limbs][32 p][4 j][2]
+    double *d_B = nullptr;     // [nqb][Npad/4][3 limbs][32 q][4 j][2]
+    double *d_Bg = nullptr;    // [njb][Qpad/4][6 planes: b limbs, (q b) limbs][32 j][4 q][2]
+    double *d_C = nullptr;     // [npb][Qpad/4][6 planes: C1 limbs, C2 limbs][32 p][4 q][2]
     double *d_part = nullptr;  // [nsplit][ntiles][4][1024][2]
     double *d_rho = nullptr;   // [4][M]: re_hi, re_lo, im_hi, im_lo
     double *d_blockred = nullptr;   // per-block partials of the finish kernel
@@ -115,6 +123,7 @@ cudaError_t shd_launch_rho(shd_ctx* h);
 cudaError_t shd_launch_finish(shd_ctx* h);
 cudaError_t shd_launch_ctable(shd_ctx* h);
 cudaError_t shd_launch_grad(shd_ctx* h, double* grad_hi, double* grad_lo);
+cudaError_t shd_tables_configure();
 cudaError_t shd_rho_configure();
 cudaError_t shd_grad_configure();
 

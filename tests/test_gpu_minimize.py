@@ -73,9 +73,11 @@ def test_max_evals_and_reentry(shd, oracle):
     phi_prev = h.energy_grad(th, tl, want_grad=False)[0][0]
     total = 0
     for _ in range(60):
-        rep = h.minimize(th, tl, smax_tol=1e-30, max_evals=60, poll_every=7)
+        # every re-entry restarts the L-BFGS history, so short calls converge more slowly than one long
+        # call (2203 evaluations in one call); 150 per call leaves a wide margin
+        rep = h.minimize(th, tl, smax_tol=1e-30, max_evals=150, poll_every=7)
         assert rep["status"] in (shd.SHD_OK, shd.SHD_EMAXEVAL)
-        assert rep["evals"] <= 60
+        assert rep["evals"] <= 150
         total += rep["evals"]
         phi_now = h.energy_grad(th, tl, want_grad=False)[0]
         assert phi_now[0] == rep["phi"][0]
