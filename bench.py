@@ -32,8 +32,9 @@ from paper_2304_09139_b200 import inputs  # noqa: E402  (pure numpy workload rec
 
 METRIC = "dd energy+grad pair-terms/s"
 UNIT = "pair-terms/s"
-# DFMAs the formulation itself needs per particle-wavevector pair:
-# rho pass 24 per (p,q) cell = 2 wavevectors -> 12; gradient pass 48 per cell -> 24.
+# FP64 FMAs the formulation itself needs per particle-wavevector pair:
+# rho pass 24 per (p,q) cell = 2 wavevectors -> 12; gradient pass 48 per cell -> 24 (issued as
+# DMMA.8x8x4, 256 FMAs per warp instruction).
 ALG_DFMA_RHO, ALG_DFMA_GRAD = 12.0, 24.0
 
 
@@ -234,25 +235,29 @@ def run_gpu(args, cfg):
     nbytes = 2 * cfg.d * cfg.N * 8
 
     # ---- roofline of the dominant kernel (ALU-bound on the FP64 pipe)
-    dfma_best, dfma_sus = shd.fp64_peak(0, 1.0)
+    dfma_best, dfma_sus = shd.fp64_peak(0, 0.5)
     dadd_best, dadd_sus = shd.fp64_peak(1, 0.5)
+    dmma_best, dmma_sus = shd.fp64_peak(2, 1.0)      # the instruction k_rho / k_grad issue (same FP64 pipe)
+    pipe_sus = max(dfma_sus, dmma_sus)
     grad_ms, rho_ms = kms["grad"] / args.steps, kms["rho"] / args.steps
     dom = "k_grad" if grad_ms >= rho_ms else "k_rho"
     dom_ms = max(grad_ms, rho_ms)
     alg = ALG_DFMA_GRAD if dom == "k_grad" else ALG_DFMA_RHO
     achieved = pairs * alg * 2.0 / (dom_ms * 1e-3) / 1e12             # TFLOP/s, DFMA = 2 FLOP
-    peak = dfma_sus * 2.0 / 1e12
+    peak = pipe_sus * 2.0 / 1e12
     launched = h.stat(12) if dom == "k_grad" else h.stat(0)
     roofline = {
         "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
         "frac": achieved / peak, "traffic": None,
-        "peak_source": "measured live: shd_fp64_peak dependent-DFMA chains, sustained over 1 s (of measured)",
-        "peak_burst": dfma_best * 2.0 / 1e12, "dadd_peak_tinstr": dadd_sus / 1e12,
+        "peak_source": "measured live: shd_fp64_peak, max of dependent-DFMA chains and DMMA.8x8x4 chains "
+                       "(one FP64 pipe), sustained over 1 s (of measured)",
+        "peak_burst": max(dfma_best, dmma_best) * 2.0 / 1e12, "dfma_peak_tfma": dfma_sus / 1e12,
+        "dmma_peak_tfma": dmma_sus / 1e12, "dadd_peak_tinstr": dadd_sus / 1e12,
         "nominal_peak": 148 * 64 * 2 * 1.965e9 / 1e12,
         "kernel_ms": dom_ms, "algorithmic_dfma_per_pair": alg,
         "launched_dfma_per_pair": launched / pairs,
-        "issue_frac_launched": launched / (dom_ms * 1e-3) / dfma_sus,
-        "whole_eval_frac": pairs * (ALG_DFMA_RHO + ALG_DFMA_GRAD) / (total_ms / args.steps * 1e-3) / dfma_sus,
+        "issue_frac_launched": launched / (dom_ms * 1e-3) / pipe_sus,
+        "whole_eval_frac": pairs * (ALG_DFMA_RHO + ALG_DFMA_GRAD) / (total_ms / args.steps * 1e-3) / pipe_sus,
         "kernel_ms_all": {k: v / args.steps for k, v in kms.items()},
     }
 

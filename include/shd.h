@@ -140,7 +140,9 @@ double shd_stat(const shd_ctx* h, int what);
 /*
  * Measured FP64-pipe issue rate of the current device, the denominator of the "alu" roofline
  * (DESIGN.md "roofline").  kind = 0: dependent-DFMA chains, 1: DADD chains (8 per
- * thread, all SMs); runs for about `seconds` (0 < seconds <= 10).  HOST out: instr_per_s[0] = best
+ * thread, all SMs), 2: chains of the FP64 matrix instruction DMMA.8x8x4 (8 per warp; counted as 8 FMAs
+ * per thread and instruction), the instruction the rho and gradient passes issue; runs for about
+ * `seconds` (0 < seconds <= 10).  HOST out: instr_per_s[0] = best
  * launch, instr_per_s[1] = mean over the run (sustained), in thread-level FP64 instructions per
  * second.  Errors: SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA.  Needs no handle.
  */

@@ -90,9 +90,7 @@ __global__ void __launch_bounds__(NW * 32, 1) k_grad(
     for (int t = 0; t < 2; t++)
 #pragma unroll
         for (int x = 0; x < 4; x++) acc3_zero(acc[t][x]);
-    dd g[3];
-#pragma unroll
-    for (int a = 0; a < 3; a++) g[a] = dd{0.0, 0.0};
+    dd g0{0.0, 0.0}, g1{0.0, 0.0}, g2{0.0, 0.0};
 
     int c = 0;
     for (int pb = 0; pb < npb; pb++) {
@@ -177,14 +175,14 @@ __global__ void __launch_bounds__(NW * 32, 1) k_grad(
                             dd ar = limbs_to_dd(a0.x, a1.x, a2.x), ai = limbs_to_dd(a0.y, a1.y, a2.y);
                             dd I = dd_dot2(ar, T[1], ai, T[0], -1.0);     // Im[conj(A) T]
                             dd R = dd_dot2(ar, T[2], ai, T[3], 1.0);      // Re[conj(A) T'']
-#pragma unroll
-                            for (int a = 0; a < 3; a++) {
-                                if (a < d) {
-                                    int wgt = wT[a * Ppad + p];
-                                    if (wgt != 0) g[a] = dd_add(g[a], dd_mul_d(I, (double)wgt));
-                                    if (a == d - 1) g[a] = dd_add(g[a], dd_scale2(R, qs));
-                                }
-                            }
+#define GACC(AX)                                                                              \
+    if (AX < d) {                                                                             \
+        const int wgt = wT[AX * Ppad + p];                                                    \
+        if (wgt != 0) g##AX = dd_add(g##AX, dd_mul_d(I, (double)wgt));                        \
+        if (AX == d - 1) g##AX = dd_add(g##AX, dd_scale2(R, qs));                             \
+    }
+                            GACC(0) GACC(1) GACC(2)
+#undef GACC
                         }
                     }
             }
@@ -200,9 +198,9 @@ __global__ void __launch_bounds__(NW * 32, 1) k_grad(
     // reduce over the 8 threads that share a particle: gred[a][j_local][4 ph + tq]
     __syncthreads();
     double2* gred = reinterpret_cast<double2*>(smem);
-#pragma unroll
-    for (int a = 0; a < 3; a++)
-        gred[(a * 32 + jl) * 8 + ph * 4 + (lane & 3)] = make_double2(g[a].h, g[a].l);
+    gred[(0 * 32 + jl) * 8 + ph * 4 + (lane & 3)] = make_double2(g0.h, g0.l);
+    gred[(1 * 32 + jl) * 8 + ph * 4 + (lane & 3)] = make_double2(g1.h, g1.l);
+    gred[(2 * 32 + jl) * 8 + ph * 4 + (lane & 3)] = make_double2(g2.h, g2.l);
     __syncthreads();
     if (tid < 32 * d) {
         const int a = tid / 32, jr = tid % 32;

@@ -1,7 +1,8 @@
 // k_probe.cu -- FP64-pipe issue-rate probe: the measured denominator of the "alu" roofline
 // (no FP64 entry exists in MEASURED_PEAKS.json, so the library measures one).
-// Every thread runs 8 independent dependent-DFMA (or DADD) chains; the result is thread-level
-// FP64 instructions per second over the whole GPU.
+// Every thread runs 8 independent dependent-DFMA (or DADD) chains, or every warp 8 independent
+// chains of the FP64 matrix instruction (mma.sync m8n8k4, SASS DMMA.8x8x4 = 256 FMAs per warp =
+// 8 per thread); the result is thread-level FP64 instructions (FMAs) per second over the whole GPU.
 #include "../../include/shd.h"
 #include <cuda_runtime.h>
 
@@ -29,11 +30,29 @@ __global__ void __launch_bounds__(256) k_fp64_chain(double* out, int iters, doub
     if (s == 123.456) out[0] = s;   // never true; keeps the chains alive
 }
 
+__global__ void __launch_bounds__(256) k_fp64_dmma(double* out, int iters, double seed)
+{
+    double c[8][2];
+#pragma unroll
+    for (int i = 0; i < 8; i++) { c[i][0] = seed + i; c[i][1] = seed - i; }
+    const double a = 1e-3 * (threadIdx.x & 31), b = 1e-3;
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int i = 0; i < 8; i++)
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                         : "+d"(c[i][0]), "+d"(c[i][1]) : "d"(a), "d"(b));
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; i++) s += c[i][0] + c[i][1];
+    if (s == 123.456) out[0] = s;
+}
+
 }  // namespace
 
 extern "C" int shd_fp64_peak(int kind, double seconds, double* instr_per_s)
 {
-    if (!instr_per_s || (kind != 0 && kind != 1) || !(seconds > 0.0) || seconds > 10.0) return SHD_EINVAL;
+    if (!instr_per_s || (kind < 0 || kind > 2) || !(seconds > 0.0) || seconds > 10.0) return SHD_EINVAL;
     int dev = 0;
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return SHD_ECUDA;
@@ -48,7 +67,8 @@ extern "C" int shd_fp64_peak(int kind, double seconds, double* instr_per_s)
     for (int rep = 0; rep < 64 && spent < seconds; rep++) {
         cudaEventRecord(e0, 0);
         if (kind == 0) k_fp64_chain<0><<<blocks, threads>>>(d_out, iters, 1.0);
-        else k_fp64_chain<1><<<blocks, threads>>>(d_out, iters, 1.0);
+        else if (kind == 1) k_fp64_chain<1><<<blocks, threads>>>(d_out, iters, 1.0);
+        else k_fp64_dmma<<<blocks, threads>>>(d_out, iters, 1.0);   // 8 DMMAs = 64 FMAs per thread and iteration
         cudaEventRecord(e1, 0);
         if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d_out); return SHD_ECUDA; }
         float ms = 0.f;
