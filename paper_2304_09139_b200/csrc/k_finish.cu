@@ -137,23 +137,23 @@ __device__ __forceinline__ limbs split_limbs(dd x) {
 }
 
 // C[p,q]: C1 = W+ + W-,  C2 = -i (W+ - W-),  W = v rho, scaled by cscale (a power of two).
-// layout [pb][q/4][plane 6][32 p][q%4][re,im]; plane l: (C1r_l, C1i_l), plane 3+l: (C2r_l, C2i_l)
+// layout [pb16][q/4][plane 6][16 p][q%4][re,im]; plane l: (C1r_l, C1i_l), plane 3+l: (C2r_l, C2i_l)
 // (fragment-major for the gradient pass, shd_internal.h).
 __global__ void __launch_bounds__(256) k_ctable(
-    int npb, int Qpad, const int* __restrict__ cell_kp, const int* __restrict__ cell_km, long M,
+    int npb16, int Qpad, const int* __restrict__ cell_kp, const int* __restrict__ cell_km, long M,
     const double* __restrict__ v, const double* __restrict__ rho, const shd_scalars* __restrict__ scal,
     double* __restrict__ C, const int* __restrict__ skip)
 {
     if (skip && *skip) return;
     long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    long ncell = (long)npb * 32 * Qpad;
+    long ncell = (long)npb16 * 16 * Qpad;
     if (idx >= ncell) return;
-    // idx enumerates (pb, q/4, p%32, q%4) with q%4 fastest so that stores are coalesced
-    const int q4 = (int)(idx & 3), pi = (int)((idx >> 2) & 31);
-    long t = idx >> 7;
+    // idx enumerates (pb16, q/4, p%16, q%4) with q%4 fastest so that stores are coalesced
+    const int q4 = (int)(idx & 3), pi = (int)((idx >> 2) & 15);
+    long t = idx >> 6;
     const int qg = (int)(t % (Qpad / 4));
     const int pb = (int)(t / (Qpad / 4));
-    const int p = pb * 32 + pi, q = qg * 4 + q4;
+    const int p = pb * 16 + pi, q = qg * 4 + q4;
     int kp = cell_kp[(size_t)p * Qpad + q], km = cell_km[(size_t)p * Qpad + q];
     double sc = scal->cscale;
     dd wpr{0, 0}, wpi{0, 0}, wmr{0, 0}, wmi{0, 0};
@@ -171,13 +171,13 @@ __global__ void __launch_bounds__(256) k_ctable(
     dd dr = dd_sub(wpr, wmr), di = dd_sub(wpi, wmi);
     dd c2r = di, c2i = dd_neg(dr);                 // -i (dr + i di) = di - i dr
     limbs a = split_limbs(c1r), b = split_limbs(c1i), c = split_limbs(c2r), e = split_limbs(c2i);
-    double2* dst = reinterpret_cast<double2*>(C) + ((((size_t)pb * (Qpad / 4) + qg) * 6) * 32 + pi) * 4 + q4;
-    dst[0 * 128] = make_double2(a.x0, b.x0);
-    dst[1 * 128] = make_double2(a.x1, b.x1);
-    dst[2 * 128] = make_double2(a.x2, b.x2);
-    dst[3 * 128] = make_double2(c.x0, e.x0);
-    dst[4 * 128] = make_double2(c.x1, e.x1);
-    dst[5 * 128] = make_double2(c.x2, e.x2);
+    double2* dst = reinterpret_cast<double2*>(C) + ((((size_t)pb * (Qpad / 4) + qg) * 6) * 16 + pi) * 4 + q4;
+    dst[0 * 64] = make_double2(a.x0, b.x0);
+    dst[1 * 64] = make_double2(a.x1, b.x1);
+    dst[2 * 64] = make_double2(a.x2, b.x2);
+    dst[3 * 64] = make_double2(c.x0, e.x0);
+    dst[4 * 64] = make_double2(c.x1, e.x1);
+    dst[5 * 64] = make_double2(c.x2, e.x2);
 }
 
 }  // namespace
@@ -195,9 +195,9 @@ cudaError_t shd_launch_finish(shd_ctx* h)
 
 cudaError_t shd_launch_ctable(shd_ctx* h)
 {
-    long ncell = (long)h->npb * 32 * h->Qpad;
+    long ncell = (long)h->npb16 * 16 * h->Qpad;
     k_ctable<<<(unsigned)((ncell + 255) / 256), 256, 0, h->stream>>>(
-        h->npb, h->Qpad, h->d_cell_kp, h->d_cell_km, h->M, h->d_v, h->d_rho, h->d_scal, h->d_C, h->d_skip);
+        h->npb16, h->Qpad, h->d_cell_kp, h->d_cell_km, h->M, h->d_v, h->d_rho, h->d_scal, h->d_C, h->d_skip);
     h->last_launches += 1;
     return cudaGetLastError();
 }

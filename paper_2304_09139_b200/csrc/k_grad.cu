@@ -5,52 +5,89 @@
 //   grad_a   = (4 pi/L) sum_p ( w_a(p) Im[conj(A_j[p]) T_j[p]] + [a = last axis] Re[conj(A_j[p]) T''_j[p]] )
 // with C1 = W+ + W-, C2 = -i (W+ - W-), W = v rho (built by k_ctable), so both signs of the last
 // axis share the same products: 24 FP64 FMAs per particle-wavevector pair.
-// One CTA owns 32 particles and walks all p-blocks; per p-block it streams the q-groups (4 q) of the
-// rho.v operand C (k_ctable output, shared by every CTA, L2 resident) and of the particles' own
-// B-table into shared memory with TMA bulk copies (cp.async.bulk + full/empty mbarriers, 6-stage ring,
-// no block-wide barrier in the main loop).  Each warp owns 8 particles x 16 p (two 8x8 blocks) and
-// issues the FMAs as FP64 matrix instructions (DMMA.8x8x4, k = 4 q) on the limb planes: 96 per warp and
-// k-step.  Exact limb bursts (64 q) are folded into double-double sums kept in thread-private
-// shared-memory slots; the p-contraction and the reduction over the 8 threads that share a particle
-// run in double-double in a fixed order (deterministic, no atomics).
+//
+// Work unit (one CTA) = 64 particles x one segment of the step list.  A step is one group of 4 q of
+// one block of 16 p (host-built list, shd_api.cu); a block's q-range ends at the circle boundary of
+// its smallest p, so 16-wide blocks waste 4 % of the cells where 32-wide ones wasted 9 %.  Segments
+// have equal length and may cut a block anywhere: the p-contraction is linear in T, so a partial T
+// gives a partial gradient; partial gradients are summed in fixed order by k_gradsum.
+// Each warp owns 8 particles x 16 p (two 8x8 blocks) and issues the FMAs as FP64 matrix
+// instructions (DMMA.8x8x4, k = 4 q) on the limb planes: 96 per warp and step.  Operand slabs (the
+// particles' own Bg table, 2 x 12 KB, and the 16-p slab of C, 6 KB, L2 resident) arrive by TMA bulk
+// copies through a 5-stage full/empty mbarrier ring.  The operand fragment loads are software
+// pipelined: every LDS is issued one round of 16 DMMAs (or more) ahead of its first use and the
+// first fragments of the next step are loaded under the last round, so the two warps of a
+// scheduler never stall on shared memory at the same time (they wait on the same stage).
+// Exact limb bursts (<= 256 q) are folded into double-double sums kept in thread-private
+// shared-memory slots; the p-contraction runs in double-double (deterministic, no atomics).
 #include "pipe.cuh"
 #include "shd_internal.h"
 
 namespace {
 
 constexpr int NW = 8;
-constexpr int PLANE_BYTES = 32 * 4 * 16;                     // 2048
-constexpr int GSLAB = (SHD_QCH / 4) * SHD_GGROUP_DOUBLES * 8;  // 12288: 6 planes of one q-group
-constexpr int GSTAGE = 2 * GSLAB;                            // Bg slab + C slab
-constexpr int RING_BYTES = SHD_GRAD_STAGES * GSTAGE;
+constexpr int NST = SHD_GRAD_STAGES;
+constexpr int PLANE_B = 32 * 4 * 16;                         // 2048: one limb plane of a 32-particle Bg slab
+constexpr int PLANE_C = 16 * 4 * 16;                         // 1024: one limb plane of a 16-p C slab
+constexpr int BSLAB = 6 * PLANE_B;                           // 12288
+constexpr int CSLAB = 6 * PLANE_C;                           // 6144
+constexpr int GSTAGE = 2 * BSLAB + CSLAB;                    // 30720
+constexpr int RING_BYTES = NST * GSTAGE;
 constexpr int MAIN_BYTES = 16 * 256 * 16;                    // 16 dd accumulators per thread
 constexpr int GSMEM = RING_BYTES + MAIN_BYTES;
-constexpr int KSTEPS_PER_BURST = SHD_BURST / 8;              // two products per q and accumulator
 
 __device__ __forceinline__ dd limbs_to_dd(double x0, double x1, double x2) {
-    return fast_two_sum(__dadd_rn(x0, x1), x2);    // x0 + x1 is exact (46 bits)
+    return fast_two_sum(__dadd_rn(x0, x1), x2);    // x0 + x1 is exact (44 bits)
 }
 
+struct F2 { double r, i; };                                  // one limb of one complex operand
+__device__ __forceinline__ F2 lds2(uint32_t addr) {
+    F2 f;
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(f.r), "=d"(f.i) : "r"(addr));
+    return f;
+}
+__device__ __forceinline__ F2 add2(F2 a, F2 b) { return F2{__dadd_rn(a.r, b.r), __dadd_rn(a.i, b.i)}; }
+// volatile: the DMMAs and the LDS keep the program order written below (that order IS the pipeline)
+__device__ __forceinline__ void dmma_v(Frag2& c, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c.c0), "+d"(c.c1) : "d"(a), "d"(b));
+}
+
+// one round: 16 DMMAs on limb level LV; particle-side limbs (b, w), C-side limbs (c1[t], c2[t]).
+// w holds (q br, -q bi) (k_tables stores the sign), so T'' = C2 (q br) - C1 (q bi) is all additions.
+#define GROUND(LV, Bx, Wx, C1x, C2x)                                        \
+    _Pragma("unroll") for (int t = 0; t < 2; t++) {                         \
+        dmma_v(acc[t][0].LV, Bx.r, C1x[t].r);                               \
+        dmma_v(acc[t][1].LV, Bx.r, C1x[t].i);                               \
+        dmma_v(acc[t][2].LV, Wx.r, C2x[t].r);                               \
+        dmma_v(acc[t][3].LV, Wx.r, C2x[t].i);                               \
+    }                                                                       \
+    _Pragma("unroll") for (int t = 0; t < 2; t++) {                         \
+        dmma_v(acc[t][0].LV, Bx.i, C2x[t].r);                               \
+        dmma_v(acc[t][1].LV, Bx.i, C2x[t].i);                               \
+        dmma_v(acc[t][2].LV, Wx.i, C1x[t].r);                               \
+        dmma_v(acc[t][3].LV, Wx.i, C1x[t].i);                               \
+    }
+
 __global__ void __launch_bounds__(NW * 32, 1) k_grad(
-    int d, long N, double L, long Npad, int npb, int Qpad, int Ppad, int qscale_log2,
-    const int* __restrict__ qchunks, const int* __restrict__ wT,
+    int d, long N, long Npad, long njb64, int Qpad, int Ppad, int qscale_log2,
+    const int2* __restrict__ steps, int nsteps, int nseg, const int* __restrict__ wT,
     const double* __restrict__ A, const double* __restrict__ Bg, const double* __restrict__ C,
-    const shd_scalars* __restrict__ scal, double* __restrict__ grad_hi, double* __restrict__ grad_lo,
-    const int* __restrict__ skip)
+    double* __restrict__ gpart, const int* __restrict__ skip)
 {
     if (skip && *skip) return;
     extern __shared__ __align__(1024) unsigned char smem[];
-    __shared__ __align__(8) unsigned long long full_bar[SHD_GRAD_STAGES], empty_bar[SHD_GRAD_STAGES];
+    __shared__ __align__(8) unsigned long long full_bar[NST], empty_bar[NST];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const long jb = blockIdx.x;
+    const long jb = blockIdx.x % njb64;
+    const int seg = (int)(blockIdx.x / njb64);
+    const int c_begin = (int)((long)nsteps * seg / nseg), c_end = (int)((long)nsteps * (seg + 1) / nseg);
+    const int total = c_end - c_begin;
     const uint32_t s0 = smem_u32(smem);
     double2* mainacc = reinterpret_cast<double2*>(smem + RING_BYTES);   // [16][256]
 
-    int total = 0;
-    for (int pb = 0; pb < npb; pb++) total += qchunks[pb];
-
     if (tid == 0) {
-        for (int s = 0; s < SHD_GRAD_STAGES; s++) {
+        for (int s = 0; s < NST; s++) {
             mbar_init(smem_u32(&full_bar[s]), 1);
             mbar_init(smem_u32(&empty_bar[s]), NW);
         }
@@ -60,30 +97,30 @@ __global__ void __launch_bounds__(NW * 32, 1) k_grad(
     for (int a = 0; a < 16; a++) mainacc[a * 256 + tid] = make_double2(0.0, 0.0);
     __syncthreads();
 
-    // producer cursor (thread 0 only)
-    int lpb = 0, lqc = 0, issued = 0;
+    // producer (thread 0): stage of step c <- Bg slabs of the two 32-particle halves + C slab
+    const double* gB = Bg + (size_t)(2 * jb) * (Qpad / 4) * SHD_GGROUP_DOUBLES;
+    const size_t halfB = (size_t)(Qpad / 4) * SHD_GGROUP_DOUBLES;
+    int issued = 0;
     auto issue = [&]() {
-        const int stage = issued % SHD_GRAD_STAGES;
+        const int stage = issued % NST;
         const uint32_t bar = smem_u32(&full_bar[stage]);
+        const int2 st = steps[c_begin + issued];
+        const int qg = st.y & 0xffff;
         mbar_expect_tx(bar, GSTAGE);
-        const double* srcB = Bg + ((size_t)jb * (Qpad / 4) + (size_t)lqc * (SHD_QCH / 4)) * SHD_GGROUP_DOUBLES;
-        const double* srcC = C + ((size_t)lpb * (Qpad / 4) + (size_t)lqc * (SHD_QCH / 4)) * SHD_GGROUP_DOUBLES;
-        tma_load_1d(s0 + stage * GSTAGE, srcB, GSLAB, bar);
-        tma_load_1d(s0 + stage * GSTAGE + GSLAB, srcC, GSLAB, bar);
+        tma_load_1d(s0 + stage * GSTAGE, gB + (size_t)qg * SHD_GGROUP_DOUBLES, BSLAB, bar);
+        tma_load_1d(s0 + stage * GSTAGE + BSLAB, gB + halfB + (size_t)qg * SHD_GGROUP_DOUBLES, BSLAB, bar);
+        tma_load_1d(s0 + stage * GSTAGE + 2 * BSLAB, C + (size_t)st.x * (CSLAB / 8), CSLAB, bar);
         issued++;
-        if (++lqc == qchunks[lpb]) { lqc = 0; lpb++; }
     };
     if (tid == 0)
-        while (issued < SHD_GRAD_STAGES && issued < total) issue();
+        while (issued < NST && issued < total) issue();
 
-    // warp tile: j_local = 8 (warp % 4) + g,  p_local = 16 (warp / 4) + 8 t + {2 tq, 2 tq + 1}
-    const int jb8 = warp & 3, ph = warp >> 2;
+    // warp tile: j_local = 8 warp + g,  p_local = 8 t + {2 tq, 2 tq + 1}
     const uint32_t fragoff = (uint32_t)(lane >> 2) * 64 + (uint32_t)(lane & 3) * 16;
-    const uint32_t offB = (uint32_t)jb8 * 8 * 64 + fragoff;
-    const uint32_t offC = GSLAB + (uint32_t)ph * 16 * 64 + fragoff;
+    const uint32_t offB = (uint32_t)(warp >> 2) * BSLAB + (uint32_t)(warp & 3) * 8 * 64 + fragoff;
+    const uint32_t offC = 2 * BSLAB + fragoff;
     const double qs = ldexp(1.0, qscale_log2);
-    const int jl = jb8 * 8 + (lane >> 2);
-    const long j = jb * 32 + jl;
+    const long j = jb * 64 + warp * 8 + (lane >> 2);
 
     Acc3 acc[2][4];
 #pragma unroll
@@ -92,133 +129,160 @@ __global__ void __launch_bounds__(NW * 32, 1) k_grad(
         for (int x = 0; x < 4; x++) acc3_zero(acc[t][x]);
     dd g0{0.0, 0.0}, g1{0.0, 0.0}, g2{0.0, 0.0};
 
-    int c = 0;
-    for (int pb = 0; pb < npb; pb++) {
-        const int nqc = qchunks[pb];
-        for (int qc = 0; qc < nqc; qc++, c++) {
-            const int s = c % SHD_GRAD_STAGES;
-            mbar_wait(smem_u32(&full_bar[s]), (uint32_t)((c / SHD_GRAD_STAGES) & 1));
-            const uint32_t sb = s0 + s * GSTAGE;
+    F2 b0, w0, c10[2], c20[2];
+    if (total > 0) {
+        mbar_wait(smem_u32(&full_bar[0]), 0u);
+        b0 = lds2(s0 + offB);
+        w0 = lds2(s0 + offB + 3 * PLANE_B);
 #pragma unroll
-            for (int gq = 0; gq < SHD_QCH / 4; gq++) {
-                const uint32_t gb = sb + gq * (SHD_GGROUP_DOUBLES * 8);
-                const LimbFrag b = lds_frag(gb + offB, PLANE_BYTES);                    // (br, bi)
-                LimbFrag w = lds_frag(gb + offB + 3 * PLANE_BYTES, PLANE_BYTES);        // (q br, q bi)
-                w.i0 = -w.i0; w.i1 = -w.i1; w.i2 = -w.i2; w.i12 = -w.i12;               // T'' -= C1 (q bi)
-                LimbFrag c1[2], c2[2];
-#pragma unroll
-                for (int t = 0; t < 2; t++) {
-                    c1[t] = lds_frag(gb + offC + t * 8 * 64, PLANE_BYTES);
-                    c2[t] = lds_frag(gb + offC + t * 8 * 64 + 3 * PLANE_BYTES, PLANE_BYTES);
-                }
-                // six rounds of 16 DMMAs; the two products of one accumulator are 8 DMMAs apart
-#define GROUND(LV, AL, BL)                                                  \
-    _Pragma("unroll") for (int t = 0; t < 2; t++) {                         \
-        dmma(acc[t][0].LV, b.r##AL, c1[t].r##BL);                           \
-        dmma(acc[t][1].LV, b.r##AL, c1[t].i##BL);                           \
-        dmma(acc[t][2].LV, w.r##AL, c2[t].r##BL);                           \
-        dmma(acc[t][3].LV, w.r##AL, c2[t].i##BL);                           \
-    }                                                                       \
-    _Pragma("unroll") for (int t = 0; t < 2; t++) {                         \
-        dmma(acc[t][0].LV, b.i##AL, c2[t].r##BL);                           \
-        dmma(acc[t][1].LV, b.i##AL, c2[t].i##BL);                           \
-        dmma(acc[t][2].LV, w.i##AL, c1[t].r##BL);                           \
-        dmma(acc[t][3].LV, w.i##AL, c1[t].i##BL);                           \
+        for (int t = 0; t < 2; t++) {
+            c10[t] = lds2(s0 + offC + t * 512);
+            c20[t] = lds2(s0 + offC + t * 512 + 3 * PLANE_C);
+        }
     }
-                GROUND(l0, 0, 0)
-                GROUND(l2, 0, 2)
-                GROUND(l1, 0, 1)
-                GROUND(l2, 2, 0)
-                GROUND(l1, 1, 0)
-                GROUND(l2, 12, 12)
-#undef GROUND
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(smem_u32(&empty_bar[s]));
-            const bool last = (qc == nqc - 1);
-            if (((qc + 1) * (SHD_QCH / 4)) % KSTEPS_PER_BURST == 0 || last) {
-                // fold the exact burst into the dd sums (shared memory, thread-private slots)
+    for (int c = 0; c < total; c++) {
+        const int s = c % NST;
+        const uint32_t pB = s0 + s * GSTAGE + offB, pC = s0 + s * GSTAGE + offC;
+        const int2 st = steps[c_begin + c];
+        const F2 b1 = lds2(pB + 1 * PLANE_B), w1 = lds2(pB + 4 * PLANE_B);
+        const F2 b2 = lds2(pB + 2 * PLANE_B), w2 = lds2(pB + 5 * PLANE_B);
+        GROUND(l0, b0, w0, c10, c20)
+        F2 c11[2], c21[2];
 #pragma unroll
-                for (int t = 0; t < 2; t++)
+        for (int t = 0; t < 2; t++) {
+            c11[t] = lds2(pC + t * 512 + 1 * PLANE_C);
+            c21[t] = lds2(pC + t * 512 + 4 * PLANE_C);
+        }
+        GROUND(l1, b1, w1, c10, c20)
+        F2 c12[2], c22[2];
+#pragma unroll
+        for (int t = 0; t < 2; t++) {
+            c12[t] = lds2(pC + t * 512 + 2 * PLANE_C);
+            c22[t] = lds2(pC + t * 512 + 5 * PLANE_C);
+        }
+        GROUND(l2, b2, w2, c10, c20)
+        const F2 b12 = add2(b1, b2), w12 = add2(w1, w2);
+        GROUND(l1, b0, w0, c11, c21)
+        GROUND(l2, b0, w0, c12, c22)
+        // every LDS of stage s has been consumed by an issued DMMA: release the stage
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&empty_bar[s]));
+        F2 c1s[2], c2s[2];
+#pragma unroll
+        for (int t = 0; t < 2; t++) { c1s[t] = add2(c11[t], c12[t]); c2s[t] = add2(c21[t], c22[t]); }
+        if (c + 1 < total) {
+            const int sn = (c + 1) % NST;
+            mbar_wait(smem_u32(&full_bar[sn]), (uint32_t)(((c + 1) / NST) & 1));
+            const uint32_t nB = s0 + sn * GSTAGE + offB, nC = s0 + sn * GSTAGE + offC;
+            b0 = lds2(nB);
+            w0 = lds2(nB + 3 * PLANE_B);
+#pragma unroll
+            for (int t = 0; t < 2; t++) {
+                c10[t] = lds2(nC + t * 512);
+                c20[t] = lds2(nC + t * 512 + 3 * PLANE_C);
+            }
+        }
+        GROUND(l2, b12, w12, c1s, c2s)
+        // refill, one stage behind: the stage of step c-1 has been released by (nearly) every warp
+        if (tid == 0 && c >= 1 && issued < total) {
+            const int sp = (c - 1) % NST;
+            mbar_wait(smem_u32(&empty_bar[sp]), (uint32_t)(((c - 1) / NST) & 1));
+            issue();
+        }
+        const int flags = st.y >> 16;
+        const bool last = (c == total - 1);
+        if ((flags & 1) || last) {
+            // fold the exact burst into the dd sums (shared memory, thread-private slots)
+#pragma unroll
+            for (int t = 0; t < 2; t++)
+#pragma unroll
+                for (int x = 0; x < 4; x++) {
+                    Acc3& r = acc[t][x];
+                    double2* p0 = &mainacc[((t * 4 + x) * 2 + 0) * 256 + tid];
+                    double2* p1 = &mainacc[((t * 4 + x) * 2 + 1) * 256 + tid];
+                    double2 m0 = *p0, m1 = *p1;
+                    fold_burst(r.l0.c0, r.l1.c0, r.l2.c0, m0);
+                    fold_burst(r.l0.c1, r.l1.c1, r.l2.c1, m1);
+                    *p0 = m0; *p1 = m1;
+                    acc3_zero(r);
+                }
+        }
+        if ((flags & 2) || last) {
+            // p-contraction of the (possibly partial) T, T'' of this block of 16 p
+            const int pb16 = st.x / (Qpad / 4);
+#pragma unroll
+            for (int t = 0; t < 2; t++)
+#pragma unroll
+                for (int e = 0; e < 2; e++) {
+                    const int p = pb16 * 16 + t * 8 + (lane & 3) * 2 + e;
+                    dd T[4];
 #pragma unroll
                     for (int x = 0; x < 4; x++) {
-                        Acc3& r = acc[t][x];
-                        double2* p0 = &mainacc[((t * 4 + x) * 2 + 0) * 256 + tid];
-                        double2* p1 = &mainacc[((t * 4 + x) * 2 + 1) * 256 + tid];
-                        double2 m0 = *p0, m1 = *p1;
-                        fold_burst(r.l0.c0, r.l1.c0, r.l2.c0, m0);
-                        fold_burst(r.l0.c1, r.l1.c1, r.l2.c1, m1);
-                        *p0 = m0; *p1 = m1;
-                        acc3_zero(r);
+                        double2* slot = &mainacc[((t * 4 + x) * 2 + e) * 256 + tid];
+                        double2 m = *slot;
+                        T[x] = fast_two_sum(m.x, m.y);
+                        *slot = make_double2(0.0, 0.0);
                     }
-            }
-            if (last) {
-                // p-contraction for this p-block
-#pragma unroll
-                for (int t = 0; t < 2; t++)
-#pragma unroll
-                    for (int e = 0; e < 2; e++) {
-                        const int pl = ph * 16 + t * 8 + (lane & 3) * 2 + e;
-                        const int p = pb * 32 + pl;
-                        dd T[4];
-#pragma unroll
-                        for (int x = 0; x < 4; x++) {
-                            double2* slot = &mainacc[((t * 4 + x) * 2 + e) * 256 + tid];
-                            double2 m = *slot;
-                            T[x] = fast_two_sum(m.x, m.y);
-                            *slot = make_double2(0.0, 0.0);
-                        }
-                        if (j < N) {
-                            const double2* ap = reinterpret_cast<const double2*>(A) +
-                                                ((((size_t)pb * (Npad / 4) + (j >> 2)) * 3) * 32 + pl) * 4 + (j & 3);
-                            double2 a0 = ap[0], a1 = ap[128], a2 = ap[256];
-                            dd ar = limbs_to_dd(a0.x, a1.x, a2.x), ai = limbs_to_dd(a0.y, a1.y, a2.y);
-                            dd I = dd_dot2(ar, T[1], ai, T[0], -1.0);     // Im[conj(A) T]
-                            dd R = dd_dot2(ar, T[2], ai, T[3], 1.0);      // Re[conj(A) T'']
+                    if (j < N) {
+                        const double2* ap = reinterpret_cast<const double2*>(A) +
+                                            ((((size_t)(p >> 5) * (Npad / 4) + (j >> 2)) * 3) * 32 + (p & 31)) * 4 + (j & 3);
+                        double2 a0 = ap[0], a1 = ap[128], a2 = ap[256];
+                        dd ar = limbs_to_dd(a0.x, a1.x, a2.x), ai = limbs_to_dd(a0.y, a1.y, a2.y);
+                        dd I = dd_dot2(ar, T[1], ai, T[0], -1.0);     // Im[conj(A) T]
+                        dd R = dd_dot2(ar, T[2], ai, T[3], 1.0);      // Re[conj(A) T'']
 #define GACC(AX)                                                                              \
     if (AX < d) {                                                                             \
         const int wgt = wT[AX * Ppad + p];                                                    \
         if (wgt != 0) g##AX = dd_add(g##AX, dd_mul_d(I, (double)wgt));                        \
         if (AX == d - 1) g##AX = dd_add(g##AX, dd_scale2(R, qs));                             \
     }
-                            GACC(0) GACC(1) GACC(2)
+                        GACC(0) GACC(1) GACC(2)
 #undef GACC
-                        }
                     }
-            }
-            // refill, one stage behind: the stage of chunk c-1 has been released by (nearly) every warp
-            if (tid == 0 && c >= 1 && issued < total) {
-                const int sp = (c - 1) % SHD_GRAD_STAGES;
-                mbar_wait(smem_u32(&empty_bar[sp]), (uint32_t)(((c - 1) / SHD_GRAD_STAGES) & 1));
-                issue();
-            }
+                }
         }
     }
 
-    // reduce over the 8 threads that share a particle: gred[a][j_local][4 ph + tq]
+    // reduce over the 4 threads that share a particle: gred[a][j_local 64][tq 4]
     __syncthreads();
     double2* gred = reinterpret_cast<double2*>(smem);
-    gred[(0 * 32 + jl) * 8 + ph * 4 + (lane & 3)] = make_double2(g0.h, g0.l);
-    gred[(1 * 32 + jl) * 8 + ph * 4 + (lane & 3)] = make_double2(g1.h, g1.l);
-    gred[(2 * 32 + jl) * 8 + ph * 4 + (lane & 3)] = make_double2(g2.h, g2.l);
+    const int jl = warp * 8 + (lane >> 2);
+    gred[(0 * 64 + jl) * 4 + (lane & 3)] = make_double2(g0.h, g0.l);
+    gred[(1 * 64 + jl) * 4 + (lane & 3)] = make_double2(g1.h, g1.l);
+    gred[(2 * 64 + jl) * 4 + (lane & 3)] = make_double2(g2.h, g2.l);
     __syncthreads();
-    if (tid < 32 * d) {
-        const int a = tid / 32, jr = tid % 32;
-        const long jo = jb * 32 + jr;
+    if (tid < 64 * d) {
+        const int a = tid / 64, jr = tid % 64;
+        const long jo = jb * 64 + jr;
         if (jo < N) {
             dd sum{0.0, 0.0};
-            for (int t = 0; t < 8; t++) {
-                double2 v = gred[(a * 32 + jr) * 8 + t];
+            for (int t = 0; t < 4; t++) {
+                double2 v = gred[(a * 64 + jr) * 4 + t];
                 sum = dd_add(sum, dd{v.x, v.y});
             }
-            // (4 pi / L) / cscale
-            dd pref = dd_div_d(dd_mul_d(dd{0x1.921fb54442d18p+2, 0x1.1a62633145c07p-52}, 2.0), L);
-            sum = dd_mul(sum, pref);
-            sum = dd_scale2(sum, 1.0 / scal->cscale);
-            grad_hi[(size_t)a * N + jo] = sum.h;
-            grad_lo[(size_t)a * N + jo] = sum.l;
+            reinterpret_cast<double2*>(gpart)[((size_t)seg * d + a) * N + jo] = make_double2(sum.h, sum.l);
         }
     }
+}
+
+// grad = (4 pi / L) / cscale * sum_seg gpart[seg], fixed order
+__global__ void __launch_bounds__(256) k_gradsum(
+    long n, int nseg, double L, const double* __restrict__ gpart, const shd_scalars* __restrict__ scal,
+    double* __restrict__ grad_hi, double* __restrict__ grad_lo, const int* __restrict__ skip)
+{
+    if (skip && *skip) return;
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    dd sum{0.0, 0.0};
+    for (int s = 0; s < nseg; s++) {
+        double2 v = reinterpret_cast<const double2*>(gpart)[(size_t)s * n + i];
+        sum = dd_add(sum, dd{v.x, v.y});
+    }
+    dd pref = dd_div_d(dd_mul_d(dd{0x1.921fb54442d18p+2, 0x1.1a62633145c07p-52}, 2.0), L);   // 4 pi / L
+    sum = dd_mul(sum, pref);
+    sum = dd_scale2(sum, 1.0 / scal->cscale);
+    grad_hi[i] = sum.h;
+    grad_lo[i] = sum.l;
 }
 
 }  // namespace
@@ -230,9 +294,13 @@ cudaError_t shd_grad_configure()
 
 cudaError_t shd_launch_grad(shd_ctx* h, double* grad_hi, double* grad_lo)
 {
-    k_grad<<<(unsigned)h->njb, NW * 32, GSMEM, h->stream>>>(
-        h->d, h->N, h->L, h->Npad, h->npb, h->Qpad, h->npb * 32, h->qscale_log2, h->d_qchunks, h->d_wT,
-        h->d_A, h->d_Bg, h->d_C, h->d_scal, grad_hi, grad_lo, h->d_skip);
-    h->last_launches += 1;
+    k_grad<<<(unsigned)(h->njb64 * h->nseg), NW * 32, GSMEM, h->stream>>>(
+        h->d, h->N, h->Npad, h->njb64, h->Qpad, h->npb * 32, h->qscale_log2,
+        reinterpret_cast<const int2*>(h->d_steps), h->nsteps, h->nseg, h->d_wT,
+        h->d_A, h->d_Bg, h->d_C, h->d_gpart, h->d_skip);
+    const long n = (long)h->d * h->N;
+    k_gradsum<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(
+        n, h->nseg, h->L, h->d_gpart, h->d_scal, grad_hi, grad_lo, h->d_skip);
+    h->last_launches += 2;
     return cudaGetLastError();
 }

@@ -74,7 +74,7 @@ constexpr int TABLES_SMEM = TB * 6 * TG * 16;
 // XOR-swizzled by the bit-reversed particle index: conflict-free for the writes and for both read
 // patterns below) and the block then writes runs of 512 contiguous bytes:
 //   rho layout       T[block][j/4][limb 3][32 entries][j%4][re,im]            (A and B)
-//   gradient layout  Bg[j/32][q/4][plane 6: b limbs, (q b) limbs][j%32][q%4][re,im]
+//   gradient layout  Bg[j/32][q/4][plane 6: b limbs, (q br, -q bi) limbs][j%32][q%4][re,im]
 struct Stager {
     double2* tile;        // [TB][planes][TG]
     int planes;           // 3 (A, B) or 6 (B with the q-weighted copy for the gradient pass)
@@ -196,7 +196,7 @@ __global__ void __launch_bounds__(TB) k_tables(
                 if (gradB) {
                     cdd w;
                     w.re = dd_scale2(dd_mul_d(cur.re, (double)q), qs);
-                    w.im = dd_scale2(dd_mul_d(cur.im, (double)q), qs);
+                    w.im = dd_neg(dd_scale2(dd_mul_d(cur.im, (double)q), qs));   // k_grad adds C1 * (-q bi)
                     st.put(3, s, w);
                 }
                 cur = cdd_mul(cur, base);

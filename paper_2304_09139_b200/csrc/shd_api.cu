@@ -143,7 +143,7 @@ int build(shd_ctx* h, const double* v) {
             }
     if (found != h->M) return fail(h, SHD_EINVAL, "internal: decomposition does not cover Q");
     // ---- tiles and q-chunk counts
-    std::vector<int> tile_pb, tile_qb, qchunks(h->npb, 0);
+    std::vector<int> tile_pb, tile_qb;
     h->valid_cells = 0;
     for (int pb = 0; pb < h->npb; pb++)
         for (int qb = 0; qb < h->nqb; qb++) {
@@ -154,14 +154,32 @@ int build(shd_ctx* h, const double* v) {
                     if (kp[c] >= 0 || km[c] >= 0) {
                         any = true;
                         h->valid_cells++;
-                        qchunks[pb] = std::max(qchunks[pb], (qb * 32 + qi) / SHD_QCH + 1);
                     }
                 }
             if (any) { tile_pb.push_back(pb); tile_qb.push_back(qb); }
         }
     h->ntiles = (int)tile_pb.size();
-    h->grad_qsteps = 0;
-    for (int pb = 0; pb < h->npb; pb++) h->grad_qsteps += (long)qchunks[pb] * SHD_QCH;
+    // ---- gradient pass: step list over blocks of 16 p (q-groups up to the last valid cell of the block)
+    h->npb16 = (h->P + SHD_PG - 1) / SHD_PG;
+    std::vector<int> steps;
+    const int fold_every = SHD_BURST / 8;        // 2 products per q and L0 accumulator, 4 q per step
+    for (int pb = 0; pb < h->npb16; pb++) {
+        int nq = 0;
+        for (int pi = 0; pi < SHD_PG; pi++)
+            for (int q = 0; q < h->Qpad; q++) {
+                size_t c = (size_t)(pb * SHD_PG + pi) * h->Qpad + q;
+                if (kp[c] >= 0 || km[c] >= 0) nq = std::max(nq, q / SHD_QCH + 1);
+            }
+        for (int qg = 0; qg < nq; qg++) {
+            int flags = 0;
+            if ((qg + 1) % fold_every == 0 || qg == nq - 1) flags |= 1;
+            if (qg == nq - 1) flags |= 3;
+            steps.push_back(pb * (h->Qpad / 4) + qg);
+            steps.push_back(qg | (flags << 16));
+        }
+    }
+    h->nsteps = (int)steps.size() / 2;
+    h->grad_qsteps = (long)h->nsteps * SHD_QCH;
     // ---- particle splits of the rho pass: minimise (waves of CTAs) x (chunks per CTA)
     cudaDeviceProp prop;
     int dev = 0;
@@ -178,6 +196,17 @@ int build(shd_ctx* h, const double* v) {
     }
     h->Npad = (long)h->nsplit * h->chunks_per_split * SHD_NPS;
     h->njb = (h->N + 31) / 32;
+    h->njb64 = (h->N + SHD_JT - 1) / SHD_JT;
+    // ---- segments of the gradient pass: minimise (waves of CTAs) x (steps per CTA)
+    {
+        double best = -1.0;
+        h->nseg = 1;
+        for (int ns = 1; ns <= std::min(16, h->nsteps); ns++) {
+            long waves = (h->njb64 * ns + sms - 1) / sms;
+            double cost = (double)waves * ((double)((h->nsteps + ns - 1) / ns) + 4.0);   // +4: prologue, epilogue, partial write
+            if (best < 0.0 || cost < best) { best = cost; h->nseg = ns; }
+        }
+    }
     // ---- device memory
     int rc;
     if ((rc = upload(h, &h->d_pn0, h->pn0))) return rc;
@@ -189,12 +218,13 @@ int build(shd_ctx* h, const double* v) {
     if ((rc = upload(h, &h->d_cell_km, km))) return rc;
     if ((rc = upload(h, &h->d_tile_pb, tile_pb))) return rc;
     if ((rc = upload(h, &h->d_tile_qb, tile_qb))) return rc;
-    if ((rc = upload(h, &h->d_qchunks, qchunks))) return rc;
+    if ((rc = upload(h, &h->d_steps, steps))) return rc;
     if (!h->v.empty()) { if ((rc = upload(h, &h->d_v, h->v))) return rc; }
     if ((rc = dalloc_zero(h, &h->d_A, (size_t)h->npb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
     if ((rc = dalloc_zero(h, &h->d_B, (size_t)h->nqb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
-    if ((rc = dalloc_zero(h, &h->d_Bg, (size_t)h->njb * (h->Qpad / 4) * SHD_GGROUP_DOUBLES))) return rc;
-    if ((rc = dalloc_zero(h, &h->d_C, (size_t)h->npb * (h->Qpad / 4) * SHD_GGROUP_DOUBLES))) return rc;
+    if ((rc = dalloc_zero(h, &h->d_Bg, (size_t)(2 * h->njb64) * (h->Qpad / 4) * SHD_GGROUP_DOUBLES))) return rc;
+    if ((rc = dalloc_zero(h, &h->d_C, (size_t)h->npb16 * (h->Qpad / 4) * (6 * SHD_PG * 4 * 2)))) return rc;
+    if ((rc = dalloc_zero(h, &h->d_gpart, (size_t)h->nseg * h->d * h->N * 2))) return rc;
     if ((rc = dalloc_zero(h, &h->d_part, (size_t)h->nsplit * h->ntiles * 4 * 1024 * 2))) return rc;
     if ((rc = dalloc_zero(h, &h->d_rho, (size_t)4 * h->M))) return rc;
     h->nfinish_blocks = (int)(((long)h->ntiles * 1024 + 255) / 256);
@@ -288,7 +318,7 @@ void shd_destroy(shd_ctx* h) {
     if (!h) return;
     shd_min_free(h);
     cudaFree(h->d_pn0); cudaFree(h->d_pn1); cudaFree(h->d_wT); cudaFree(h->d_cell_kp); cudaFree(h->d_cell_km);
-    cudaFree(h->d_tile_pb); cudaFree(h->d_tile_qb); cudaFree(h->d_qchunks); cudaFree(h->d_v);
+    cudaFree(h->d_tile_pb); cudaFree(h->d_tile_qb); cudaFree(h->d_steps); cudaFree(h->d_v); cudaFree(h->d_gpart);
     cudaFree(h->d_A); cudaFree(h->d_B); cudaFree(h->d_Bg); cudaFree(h->d_C); cudaFree(h->d_part);
     cudaFree(h->d_rho); cudaFree(h->d_blockred); cudaFree(h->d_scal);
     cudaFree(h->d_hpos); cudaFree(h->d_hgrad);
@@ -409,7 +439,7 @@ double shd_stat(const shd_ctx* h, int what) {
     const double cells_rho = (double)h->ntiles * 1024.0;
     switch (what) {
         case 0: return cells_rho * (double)h->Npad * 24.0;     // DFMAs launched by the rho pass (padded)
-        case 12: return (double)h->njb * (double)h->grad_qsteps * 1024.0 * 48.0;   // ... by the gradient pass
+        case 12: return (double)h->njb64 * SHD_JT * (double)h->grad_qsteps * SHD_PG * 48.0;   // ... by the gradient pass
         case 1: return (double)h->last_launches;
         case 2: return cells_rho;
         case 3: return (double)h->valid_cells;
@@ -421,6 +451,7 @@ double shd_stat(const shd_ctx* h, int what) {
         case 9: return (double)h->Npad;
         case 10: return (double)h->njb;
         case 11: return (double)h->grad_qsteps;
+        case 13: return (double)h->nseg;
         case 20: case 21: case 22: case 23: case 24: return (double)h->kern_ms[what - 20];
         default: return 0.0;
     }

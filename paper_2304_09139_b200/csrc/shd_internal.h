@@ -11,12 +11,13 @@
 // the gradient is a contraction over q followed by one over p (gradient pass).
 //
 // Each real operand x (|x| <= 1) is stored as three "limbs" (x0, x1, x2):
-//   x0  = x rounded to a multiple of 2^-W0,  x1 = (x - x0) rounded to a multiple of 2^-(W0+W1),
+//   x0  = x rounded to a multiple of 2^-W0,  x1 = (x - x0) rounded to a multiple of 2^-(W0+W1),  W0 = W1 = 22,
 //   x2  = x - x0 - x1 (a free double);   x12 = x1 + x2 is formed in registers,
 // and a product-accumulate  acc += x*y  is the 6 FMAs
 //   L0 += x0 y0 ;  L1 += x0 y1 + x1 y0 ;  L2 += x0 y2 + x2 y0 + x12 y12
-// where L0 and L1 are EXACT (all partial sums representable) for bursts of <= 128 terms, and
-// L2 carries the terms below 2^-45 in plain FP64 (error ~2^-100 per term).  Bursts are folded
+// where L0 and L1 are EXACT (all partial sums representable: L0 in units of 2^-44 below 2^9, L1 in
+// units of 2^-66 below 2^-13) for bursts of <= 512 products, and L2 carries the terms below 2^-44 in
+// plain FP64 (error ~2^-98 per term).  Bursts are folded
 // into ordinary double-double accumulators with TwoSum.
 //
 // The FMAs are issued as FP64 matrix instructions (mma.sync m8n8k4, SASS DMMA.8x8x4: 256 FMAs per
@@ -35,11 +36,12 @@ constexpr int SHD_PT = 32;          // A-entries (p) per tile
 constexpr int SHD_QT = 32;          // B-entries (q) per tile
 constexpr int SHD_NPS = 8;          // particles per rho-pass pipeline stage (2 groups of 4)
 constexpr int SHD_RHO_STAGES = 6;   // TMA pipeline depth, rho pass
-constexpr int SHD_BURST = 128;      // products per exact burst (see header comment)
+constexpr int SHD_BURST = 512;      // products per exact burst (see header comment)
 constexpr int SHD_QCH = 4;          // q per gradient-pass pipeline stage (1 group of 4)
-constexpr int SHD_GRAD_STAGES = 6;  // TMA pipeline depth, gradient pass
-constexpr int SHD_JT = 32;          // particles per gradient-pass block
-constexpr int SHD_W0 = 23;          // limb widths (bits)
+constexpr int SHD_GRAD_STAGES = 5;  // TMA pipeline depth, gradient pass
+constexpr int SHD_JT = 64;          // particles per gradient-pass block
+constexpr int SHD_PG = 16;          // p per gradient-pass block
+constexpr int SHD_W0 = 22;          // limb widths (bits)
 constexpr int SHD_W1 = 22;
 constexpr int SHD_NLIMB = 3;
 constexpr int SHD_GROUP_DOUBLES = SHD_NLIMB * 32 * 4 * 2;   // one (block, group of 4) slab of A / B: 6 KB
@@ -76,9 +78,13 @@ struct shd_ctx {
     long chunks_per_split = 0;
     int ntiles = 0;
     long njb = 0;              // ceil(N / 32)
+    long njb64 = 0;            // ceil(N / 64): particle blocks of the gradient pass
+    int npb16 = 0;             // ceil(P / 16): p-blocks of the gradient pass
+    int nsteps = 0;            // gradient pass: steps (16 p x 4 q) in the step list
+    int nseg = 0;              // gradient pass: equal segments of the step list (work units per particle block)
     int Qpad = 0;              // nqb * 32
     long valid_cells = 0;
-    long grad_qsteps = 0;      // sum over p-blocks of q-steps walked by the gradient pass
+    long grad_qsteps = 0;      // 4 * nsteps: q-steps walked by the gradient pass over all 16-p blocks
     // host copies
     std::vector<int> nvec;     // M * d
     std::vector<double> v;     // M (empty = all ones)
@@ -88,13 +94,15 @@ struct shd_ctx {
     int *d_wT = nullptr;       // [3][P padded]: integer weight of Im(conj(A) T) for axis a
     int *d_cell_kp = nullptr, *d_cell_km = nullptr;   // [npb*32][Qpad] -> k or -1
     int *d_tile_pb = nullptr, *d_tile_qb = nullptr;   // [ntiles]
-    int *d_qchunks = nullptr;  // [npb] number of q-chunks (of SHD_QCH) with any valid cell
+    int *d_steps = nullptr;    // [nsteps] int2: x = C slab index pb16 * (Qpad/4) + qg, y = qg | flags << 16
+                               //   (flag 1: fold the limb burst after this step, 2: last step of its p-block)
     double *d_v = nullptr;     // [M]
     // device: per-evaluation data
     double *d_A = nullptr;     // [npb][Npad/4][3 limbs][32 p][4 j][2]
     double *d_B = nullptr;     // [nqb][Npad/4][3 limbs][32 q][4 j][2]
-    double *d_Bg = nullptr;    // [njb][Qpad/4][6 planes: b limbs, (q b) limbs][32 j][4 q][2]
-    double *d_C = nullptr;     // [npb][Qpad/4][6 planes: C1 limbs, C2 limbs][32 p][4 q][2]
+    double *d_Bg = nullptr;    // [2 njb64][Qpad/4][6 planes: b limbs, (q br, -q bi) limbs][32 j][4 q][2]
+    double *d_C = nullptr;     // [npb16][Qpad/4][6 planes: C1 limbs, C2 limbs][16 p][4 q][2]
+    double *d_gpart = nullptr; // [nseg][d][N] (hi, lo): partial gradients of the segments
     double *d_part = nullptr;  // [nsplit][ntiles][4][1024][2]
     double *d_rho = nullptr;   // [4][M]: re_hi, re_lo, im_hi, im_lo
     double *d_blockred = nullptr;   // per-block partials of the finish kernel
