@@ -14,12 +14,14 @@
 // Each warp owns 8 particles x 16 p (two 8x8 blocks) and issues the FMAs as FP64 matrix
 // instructions (DMMA.8x8x4, k = 4 q) on the limb planes: 96 per warp and step.  Operand slabs (the
 // particles' own Bg table, 2 x 12 KB, and the 16-p slab of C, 6 KB, L2 resident) arrive by TMA bulk
-// copies through a 5-stage full/empty mbarrier ring.  The operand fragment loads are software
+// copies, issued by a ninth (producer) warp, through a 5-stage full/empty mbarrier ring.  The operand fragment loads are software
 // pipelined: every LDS is issued one round of 16 DMMAs (or more) ahead of its first use and the
 // first fragments of the next step are loaded under the last round, so the two warps of a
 // scheduler never stall on shared memory at the same time (they wait on the same stage).
-// Exact limb bursts (<= 256 q) are folded into double-double sums kept in thread-private
-// shared-memory slots; the p-contraction runs in double-double (deterministic, no atomics).
+// A block ends after <= 64 steps (one exact limb burst, 256 q): the limbs are folded into double-double
+// T, T'' and parked in thread-private shared-memory slots; their p-contraction with A (double-double,
+// deterministic, no atomics) is deferred and spread over the next four steps, A loaded a step ahead,
+// so that no warp waits on global memory or on a long dependent chain while the FP64 pipe idles.
 #include "pipe.cuh"
 #include "shd_internal.h"
 
@@ -40,19 +42,6 @@ __device__ __forceinline__ dd limbs_to_dd(double x0, double x1, double x2) {
     return fast_two_sum(__dadd_rn(x0, x1), x2);    // x0 + x1 is exact (44 bits)
 }
 
-struct F2 { double r, i; };                                  // one limb of one complex operand
-__device__ __forceinline__ F2 lds2(uint32_t addr) {
-    F2 f;
-    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(f.r), "=d"(f.i) : "r"(addr));
-    return f;
-}
-__device__ __forceinline__ F2 add2(F2 a, F2 b) { return F2{__dadd_rn(a.r, b.r), __dadd_rn(a.i, b.i)}; }
-// volatile: the DMMAs and the LDS keep the program order written below (that order IS the pipeline)
-__device__ __forceinline__ void dmma_v(Frag2& c, double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-                 : "+d"(c.c0), "+d"(c.c1) : "d"(a), "d"(b));
-}
-
 // one round: 16 DMMAs on limb level LV; particle-side limbs (b, w), C-side limbs (c1[t], c2[t]).
 // w holds (q br, -q bi) (k_tables stores the sign), so T'' = C2 (q br) - C1 (q bi) is all additions.
 #define GROUND(LV, Bx, Wx, C1x, C2x)                                        \
@@ -69,7 +58,7 @@ __device__ __forceinline__ void dmma_v(Frag2& c, double a, double b) {
         dmma_v(acc[t][3].LV, Wx.i, C1x[t].i);                               \
     }
 
-__global__ void __launch_bounds__(NW * 32, 1) k_grad(
+__global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
     int d, long N, long Npad, long njb64, int Qpad, int Ppad, int qscale_log2,
     const int2* __restrict__ steps, int nsteps, int nseg, const int* __restrict__ wT,
     const double* __restrict__ A, const double* __restrict__ Bg, const double* __restrict__ C,
@@ -93,27 +82,37 @@ __global__ void __launch_bounds__(NW * 32, 1) k_grad(
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    if (warp < NW) {
 #pragma unroll
-    for (int a = 0; a < 16; a++) mainacc[a * 256 + tid] = make_double2(0.0, 0.0);
+        for (int a = 0; a < 16; a++) mainacc[a * 256 + tid] = make_double2(0.0, 0.0);
+    }
     __syncthreads();
 
-    // producer (thread 0): stage of step c <- Bg slabs of the two 32-particle halves + C slab
-    const double* gB = Bg + (size_t)(2 * jb) * (Qpad / 4) * SHD_GGROUP_DOUBLES;
-    const size_t halfB = (size_t)(Qpad / 4) * SHD_GGROUP_DOUBLES;
-    int issued = 0;
-    auto issue = [&]() {
-        const int stage = issued % NST;
-        const uint32_t bar = smem_u32(&full_bar[stage]);
-        const int2 st = steps[c_begin + issued];
-        const int qg = st.y & 0xffff;
-        mbar_expect_tx(bar, GSTAGE);
-        tma_load_1d(s0 + stage * GSTAGE, gB + (size_t)qg * SHD_GGROUP_DOUBLES, BSLAB, bar);
-        tma_load_1d(s0 + stage * GSTAGE + BSLAB, gB + halfB + (size_t)qg * SHD_GGROUP_DOUBLES, BSLAB, bar);
-        tma_load_1d(s0 + stage * GSTAGE + 2 * BSLAB, C + (size_t)st.x * (CSLAB / 8), CSLAB, bar);
-        issued++;
-    };
-    if (tid == 0)
-        while (issued < NST && issued < total) issue();
+    if (warp >= NW) {
+        // producer warpgroup: hands its registers to the consumers (setmaxnreg), then one lane streams.
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+        // producer warp (one lane): stage of step i <- Bg slabs of the two 32-particle halves + C slab;
+        // it does nothing else, so a refill is issued the moment the last consumer warp releases a stage
+        if (warp == NW && lane == 0) {
+            const double* gB = Bg + (size_t)(2 * jb) * (Qpad / 4) * SHD_GGROUP_DOUBLES;
+            const size_t halfB = (size_t)(Qpad / 4) * SHD_GGROUP_DOUBLES;
+            for (int i = 0; i < total; i++) {
+                const int stage = i % NST;
+                if (i >= NST) mbar_wait(smem_u32(&empty_bar[stage]), (uint32_t)((i / NST - 1) & 1));
+                const uint32_t bar = smem_u32(&full_bar[stage]);
+                const int2 st = steps[c_begin + i];
+                const int qg = st.y & 0xffff;
+                mbar_expect_tx(bar, GSTAGE);
+                tma_load_1d(s0 + stage * GSTAGE, gB + (size_t)qg * SHD_GGROUP_DOUBLES, BSLAB, bar);
+                tma_load_1d(s0 + stage * GSTAGE + BSLAB, gB + halfB + (size_t)qg * SHD_GGROUP_DOUBLES, BSLAB, bar);
+                tma_load_1d(s0 + stage * GSTAGE + 2 * BSLAB, C + (size_t)st.x * (CSLAB / 8), CSLAB, bar);
+            }
+        }
+        __syncthreads();        // the two block-wide barriers of the consumers' epilogue
+        __syncthreads();
+        return;
+    }
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
 
     // warp tile: j_local = 8 warp + g,  p_local = 8 t + {2 tq, 2 tq + 1}
     const uint32_t fragoff = (uint32_t)(lane >> 2) * 64 + (uint32_t)(lane & 3) * 16;
@@ -128,6 +127,44 @@ __global__ void __launch_bounds__(NW * 32, 1) k_grad(
 #pragma unroll
         for (int x = 0; x < 4; x++) acc3_zero(acc[t][x]);
     dd g0{0.0, 0.0}, g1{0.0, 0.0}, g2{0.0, 0.0};
+
+    // deferred p-contraction state (warp-uniform): quarter pk = (t, e) of block ppb is pending
+    bool pend = false;
+    int pk = 0, ppb = 0;
+    double2 pa0 = make_double2(0.0, 0.0), pa1 = pa0, pa2 = pa0;
+    const double2* Aj = reinterpret_cast<const double2*>(A) + (size_t)(j >> 2) * 3 * 32 * 4 + (j & 3);
+    auto load_quarter = [&](int k, int pb16, double2& a0, double2& a1, double2& a2) {
+        const int p = pb16 * 16 + (k >> 1) * 8 + (lane & 3) * 2 + (k & 1);
+        if (j < N) {
+            const double2* ap = Aj + ((size_t)(p >> 5) * (Npad / 4) * 3 * 32 + (p & 31)) * 4;
+            asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(a0.x), "=d"(a0.y) : "l"(ap));
+            asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(a1.x), "=d"(a1.y) : "l"(ap + 128));
+            asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(a2.x), "=d"(a2.y) : "l"(ap + 256));
+        }
+    };
+    auto contract_quarter = [&](int k, int pb16, double2 a0, double2 a1, double2 a2) {
+        const int t = k >> 1, e = k & 1;
+        const int p = pb16 * 16 + t * 8 + (lane & 3) * 2 + e;
+        dd T[4];
+#pragma unroll
+        for (int x = 0; x < 4; x++) {
+            double2 m = mainacc[((t * 4 + x) * 2 + e) * 256 + tid];
+            T[x] = dd{m.x, m.y};
+        }
+        if (j < N) {
+            dd ar = limbs_to_dd(a0.x, a1.x, a2.x), ai = limbs_to_dd(a0.y, a1.y, a2.y);
+            dd I = dd_dot2(ar, T[1], ai, T[0], -1.0);     // Im[conj(A) T]
+            dd R = dd_dot2(ar, T[2], ai, T[3], 1.0);      // Re[conj(A) T'']
+#define GACC(AX)                                                                              \
+    if (AX < d) {                                                                             \
+        const int wgt = wT[AX * Ppad + p];                                                    \
+        if (wgt != 0) g##AX = dd_add(g##AX, dd_mul_d(I, (double)wgt));                        \
+        if (AX == d - 1) g##AX = dd_add(g##AX, dd_scale2(R, qs));                             \
+    }
+            GACC(0) GACC(1) GACC(2)
+#undef GACC
+        }
+    };
 
     F2 b0, w0, c10[2], c20[2];
     if (total > 0) {
@@ -144,6 +181,7 @@ __global__ void __launch_bounds__(NW * 32, 1) k_grad(
         const int s = c % NST;
         const uint32_t pB = s0 + s * GSTAGE + offB, pC = s0 + s * GSTAGE + offC;
         const int2 st = steps[c_begin + c];
+        if (pend) load_quarter(pk, ppb, pa0, pa1, pa2);
         const F2 b1 = lds2(pB + 1 * PLANE_B), w1 = lds2(pB + 4 * PLANE_B);
         const F2 b2 = lds2(pB + 2 * PLANE_B), w2 = lds2(pB + 5 * PLANE_B);
         GROUND(l0, b0, w0, c10, c20)
@@ -183,64 +221,40 @@ __global__ void __launch_bounds__(NW * 32, 1) k_grad(
             }
         }
         GROUND(l2, b12, w12, c1s, c2s)
-        // refill, one stage behind: the stage of step c-1 has been released by (nearly) every warp
-        if (tid == 0 && c >= 1 && issued < total) {
-            const int sp = (c - 1) % NST;
-            mbar_wait(smem_u32(&empty_bar[sp]), (uint32_t)(((c - 1) / NST) & 1));
-            issue();
+        // deferred p-contraction: one quarter of the previous block per step, its A limbs loaded at the
+        // top of this step (global-memory latency hidden under the 96 DMMAs above)
+        if (pend) {
+            contract_quarter(pk, ppb, pa0, pa1, pa2);
+            if (++pk == 4) pend = false;
         }
         const int flags = st.y >> 16;
-        const bool last = (c == total - 1);
-        if ((flags & 1) || last) {
-            // fold the exact burst into the dd sums (shared memory, thread-private slots)
+        if ((flags & 1) || c == total - 1) {
+            // end of a block of <= 64 steps (one exact burst) or of the segment: limbs -> dd T, T'' parked
+            // in the thread-private shared-memory slots until the next steps contract them with A
+            while (pend) {                         // blocks shorter than 4 steps: finish the previous one now
+                load_quarter(pk, ppb, pa0, pa1, pa2);
+                contract_quarter(pk, ppb, pa0, pa1, pa2);
+                if (++pk == 4) pend = false;
+            }
 #pragma unroll
             for (int t = 0; t < 2; t++)
 #pragma unroll
                 for (int x = 0; x < 4; x++) {
                     Acc3& r = acc[t][x];
-                    double2* p0 = &mainacc[((t * 4 + x) * 2 + 0) * 256 + tid];
-                    double2* p1 = &mainacc[((t * 4 + x) * 2 + 1) * 256 + tid];
-                    double2 m0 = *p0, m1 = *p1;
+                    double2 m0 = make_double2(0.0, 0.0), m1 = make_double2(0.0, 0.0);
                     fold_burst(r.l0.c0, r.l1.c0, r.l2.c0, m0);
                     fold_burst(r.l0.c1, r.l1.c1, r.l2.c1, m1);
-                    *p0 = m0; *p1 = m1;
+                    mainacc[((t * 4 + x) * 2 + 0) * 256 + tid] = m0;
+                    mainacc[((t * 4 + x) * 2 + 1) * 256 + tid] = m1;
                     acc3_zero(r);
                 }
+            pend = true; pk = 0; ppb = st.x / (Qpad / 4);
         }
-        if ((flags & 2) || last) {
-            // p-contraction of the (possibly partial) T, T'' of this block of 16 p
-            const int pb16 = st.x / (Qpad / 4);
-#pragma unroll
-            for (int t = 0; t < 2; t++)
-#pragma unroll
-                for (int e = 0; e < 2; e++) {
-                    const int p = pb16 * 16 + t * 8 + (lane & 3) * 2 + e;
-                    dd T[4];
-#pragma unroll
-                    for (int x = 0; x < 4; x++) {
-                        double2* slot = &mainacc[((t * 4 + x) * 2 + e) * 256 + tid];
-                        double2 m = *slot;
-                        T[x] = fast_two_sum(m.x, m.y);
-                        *slot = make_double2(0.0, 0.0);
-                    }
-                    if (j < N) {
-                        const double2* ap = reinterpret_cast<const double2*>(A) +
-                                            ((((size_t)(p >> 5) * (Npad / 4) + (j >> 2)) * 3) * 32 + (p & 31)) * 4 + (j & 3);
-                        double2 a0 = ap[0], a1 = ap[128], a2 = ap[256];
-                        dd ar = limbs_to_dd(a0.x, a1.x, a2.x), ai = limbs_to_dd(a0.y, a1.y, a2.y);
-                        dd I = dd_dot2(ar, T[1], ai, T[0], -1.0);     // Im[conj(A) T]
-                        dd R = dd_dot2(ar, T[2], ai, T[3], 1.0);      // Re[conj(A) T'']
-#define GACC(AX)                                                                              \
-    if (AX < d) {                                                                             \
-        const int wgt = wT[AX * Ppad + p];                                                    \
-        if (wgt != 0) g##AX = dd_add(g##AX, dd_mul_d(I, (double)wgt));                        \
-        if (AX == d - 1) g##AX = dd_add(g##AX, dd_scale2(R, qs));                             \
     }
-                        GACC(0) GACC(1) GACC(2)
-#undef GACC
-                    }
-                }
-        }
+    while (pend) {
+        load_quarter(pk, ppb, pa0, pa1, pa2);
+        contract_quarter(pk, ppb, pa0, pa1, pa2);
+        if (++pk == 4) pend = false;
     }
 
     // reduce over the 4 threads that share a particle: gred[a][j_local 64][tq 4]
@@ -294,7 +308,7 @@ cudaError_t shd_grad_configure()
 
 cudaError_t shd_launch_grad(shd_ctx* h, double* grad_hi, double* grad_lo)
 {
-    k_grad<<<(unsigned)(h->njb64 * h->nseg), NW * 32, GSMEM, h->stream>>>(
+    k_grad<<<(unsigned)(h->njb64 * h->nseg), NW * 32 + 128, GSMEM, h->stream>>>(
         h->d, h->N, h->Npad, h->njb64, h->Qpad, h->npb * 32, h->qscale_log2,
         reinterpret_cast<const int2*>(h->d_steps), h->nsteps, h->nseg, h->d_wT,
         h->d_A, h->d_Bg, h->d_C, h->d_gpart, h->d_skip);

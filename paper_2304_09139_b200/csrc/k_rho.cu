@@ -8,8 +8,8 @@
 // The FMAs are FP64 matrix instructions (DMMA.8x8x4, k = 4 particles) on the limb planes of the
 // operands (shd_internal.h): 6 per real sum, 48 per warp and k-step.
 // Operand slabs (8 particles x 32 entries x 48 B for A and for B) are streamed from the
-// fragment-major tables by TMA bulk copies (cp.async.bulk + full/empty mbarriers) through a 6-stage
-// ring; no block-wide barrier in the main loop.
+// fragment-major tables by TMA bulk copies (cp.async.bulk + full/empty mbarriers), issued by a ninth
+// (producer) warp, through a 6-stage ring; no block-wide barrier in the main loop.
 // Every 128 particles the exact limb accumulators are folded into double-double sums (TwoSum) kept
 // in thread-private shared-memory slots.
 // No atomics: each (tile, split) writes its own partial, summed in fixed order by k_finish.
@@ -28,7 +28,7 @@ constexpr int MAIN_BYTES = 16 * 256 * 16;                    // 16 dd sums per t
 constexpr int RHO_SMEM = RING_BYTES + MAIN_BYTES;
 constexpr int KSTEPS_PER_BURST = SHD_BURST / 4;
 
-__global__ void __launch_bounds__(NW * 32, 1) k_rho(
+__global__ void __launch_bounds__(NW * 32 + 128, 1) k_rho(
     const double* __restrict__ A, const double* __restrict__ B,
     const int* __restrict__ tile_pb, const int* __restrict__ tile_qb, int ntiles,
     long Npad, long chunks_per_split, double* __restrict__ part, const int* __restrict__ skip)
@@ -54,19 +54,30 @@ __global__ void __launch_bounds__(NW * 32, 1) k_rho(
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    if (warp < NW) {
 #pragma unroll
-    for (int a = 0; a < 16; a++) mainacc[a * 256 + tid] = make_double2(0.0, 0.0);
+        for (int a = 0; a < 16; a++) mainacc[a * 256 + tid] = make_double2(0.0, 0.0);
+    }
     __syncthreads();
-    auto issue = [&](int chunk) {           // one elected thread
-        const int s = chunk % SHD_RHO_STAGES;
-        const uint32_t bar = smem_u32(&full_bar[s]);
-        const size_t off = (size_t)chunk * (SHD_NPS / 4) * SHD_GROUP_DOUBLES;
-        mbar_expect_tx(bar, STAGE_BYTES);
-        tma_load_1d(s0 + s * STAGE_BYTES, gA + off, SLAB_BYTES, bar);
-        tma_load_1d(s0 + s * STAGE_BYTES + SLAB_BYTES, gB + off, SLAB_BYTES, bar);
-    };
-    if (tid == 0)
-        for (int c = 0; c < SHD_RHO_STAGES && c < nchunks; c++) issue(c);
+    if (warp >= NW) {
+        // producer warpgroup: hands its registers to the consumers (setmaxnreg), then one lane streams.
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+        // producer warp (one lane): it does nothing else, so a stage is refilled the moment the last
+        // consumer warp releases it
+        if (warp == NW && lane == 0)
+            for (int chunk = 0; chunk < nchunks; chunk++) {
+                const int s = chunk % SHD_RHO_STAGES;
+                if (chunk >= SHD_RHO_STAGES)
+                    mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((chunk / SHD_RHO_STAGES - 1) & 1));
+                const uint32_t bar = smem_u32(&full_bar[s]);
+                const size_t off = (size_t)chunk * (SHD_NPS / 4) * SHD_GROUP_DOUBLES;
+                mbar_expect_tx(bar, STAGE_BYTES);
+                tma_load_1d(s0 + s * STAGE_BYTES, gA + off, SLAB_BYTES, bar);
+                tma_load_1d(s0 + s * STAGE_BYTES + SLAB_BYTES, gB + off, SLAB_BYTES, bar);
+            }
+        return;
+    }
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
 
     // warp tile: p_local = 8 (warp / 2) + g, q_local = 16 (warp % 2) + 8 t + {2 tq, 2 tq + 1}
     const uint32_t fragoff = (uint32_t)(lane >> 2) * 64 + (uint32_t)(lane & 3) * 16;
@@ -79,39 +90,59 @@ __global__ void __launch_bounds__(NW * 32, 1) k_rho(
 #pragma unroll
         for (int x = 0; x < 4; x++) acc3_zero(acc[t][x]);
 
-    int ksteps = 0;
-    for (int c = 0; c < nchunks; c++) {
-        const int s = c % SHD_RHO_STAGES;
-        mbar_wait(smem_u32(&full_bar[s]), (uint32_t)((c / SHD_RHO_STAGES) & 1));
-        const uint32_t sb = s0 + s * STAGE_BYTES;
-#pragma unroll
-        for (int g = 0; g < SHD_NPS / 4; g++) {
-            const LimbFrag a = lds_frag(sb + g * GROUP_BYTES + offA, PLANE_BYTES);
-            LimbFrag b[2];
-#pragma unroll
-            for (int t = 0; t < 2; t++) b[t] = lds_frag(sb + g * GROUP_BYTES + offB + t * 8 * 64, PLANE_BYTES);
-            // six rounds of 8 independent DMMAs; the three updates of each L2 (two of each L1) are
-            // two rounds apart
-#define ROUND(LV, AL, BL)                                                   \
+    // k-steps (groups of 4 particles) run through a software pipeline: every LDS is issued at least one
+    // round of 8 DMMAs ahead of its first use and the limb-0 fragments of the next k-step are loaded
+    // under the last round (the DMMAs and the LDS are volatile: the order below is the schedule).
+#define ROUND(LV, Ax, Bx)                                                   \
     _Pragma("unroll") for (int t = 0; t < 2; t++) {                         \
-        dmma(acc[t][0].LV, a.r##AL, b[t].r##BL);                            \
-        dmma(acc[t][1].LV, a.i##AL, b[t].i##BL);                            \
-        dmma(acc[t][2].LV, a.r##AL, b[t].i##BL);                            \
-        dmma(acc[t][3].LV, a.i##AL, b[t].r##BL);                            \
+        dmma_v(acc[t][0].LV, Ax.r, Bx[t].r);                                \
+        dmma_v(acc[t][1].LV, Ax.i, Bx[t].i);                                \
+        dmma_v(acc[t][2].LV, Ax.r, Bx[t].i);                                \
+        dmma_v(acc[t][3].LV, Ax.i, Bx[t].r);                                \
     }
-            ROUND(l0, 0, 0)
-            ROUND(l2, 0, 2)
-            ROUND(l1, 0, 1)
-            ROUND(l2, 2, 0)
-            ROUND(l1, 1, 0)
-            ROUND(l2, 12, 12)
-#undef ROUND
-            ksteps++;
+    constexpr int GPS = SHD_NPS / 4;                 // groups (k-steps) per stage
+    const int nk = nchunks * GPS;
+    F2 a0, b0[2];
+    if (nk > 0) {
+        mbar_wait(smem_u32(&full_bar[0]), 0u);
+        a0 = lds2(s0 + offA);
+#pragma unroll
+        for (int t = 0; t < 2; t++) b0[t] = lds2(s0 + offB + t * 8 * 64);
+    }
+    for (int k = 0; k < nk; k++) {
+        const int c = k / GPS, g = k % GPS, s = c % SHD_RHO_STAGES;
+        const uint32_t pA = s0 + s * STAGE_BYTES + g * GROUP_BYTES + offA;
+        const uint32_t pB = s0 + s * STAGE_BYTES + g * GROUP_BYTES + offB;
+        const F2 a1 = lds2(pA + PLANE_BYTES), a2 = lds2(pA + 2 * PLANE_BYTES);
+        ROUND(l0, a0, b0)
+        F2 b1[2], b2[2];
+#pragma unroll
+        for (int t = 0; t < 2; t++) b1[t] = lds2(pB + t * 8 * 64 + PLANE_BYTES);
+        ROUND(l1, a1, b0)
+#pragma unroll
+        for (int t = 0; t < 2; t++) b2[t] = lds2(pB + t * 8 * 64 + 2 * PLANE_BYTES);
+        ROUND(l2, a2, b0)
+        const F2 a12 = add2(a1, a2);
+        ROUND(l1, a0, b1)
+        ROUND(l2, a0, b2)
+        if (g == GPS - 1) {
+            // every LDS of stage s has been consumed by an issued DMMA: release the stage
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&empty_bar[s]));
         }
-        // this warp is done reading stage s
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&empty_bar[s]));
-        if (ksteps % KSTEPS_PER_BURST == 0 || c == nchunks - 1) {
+        F2 bs[2];
+#pragma unroll
+        for (int t = 0; t < 2; t++) bs[t] = add2(b1[t], b2[t]);
+        if (k + 1 < nk) {
+            const int cn = (k + 1) / GPS, gn = (k + 1) % GPS, sn = cn % SHD_RHO_STAGES;
+            if (gn == 0) mbar_wait(smem_u32(&full_bar[sn]), (uint32_t)((cn / SHD_RHO_STAGES) & 1));
+            const uint32_t nb = s0 + sn * STAGE_BYTES + gn * GROUP_BYTES;
+            a0 = lds2(nb + offA);
+#pragma unroll
+            for (int t = 0; t < 2; t++) b0[t] = lds2(nb + offB + t * 8 * 64);
+        }
+        ROUND(l2, a12, bs)
+        if ((k + 1) % KSTEPS_PER_BURST == 0 || k == nk - 1) {
 #pragma unroll
             for (int t = 0; t < 2; t++)
 #pragma unroll
@@ -126,13 +157,8 @@ __global__ void __launch_bounds__(NW * 32, 1) k_rho(
                     acc3_zero(r);
                 }
         }
-        // refill, one stage behind: the stage of chunk c-1 has been released by (nearly) every warp
-        if (tid == 0 && c >= 1 && c - 1 + SHD_RHO_STAGES < nchunks) {
-            const int sp = (c - 1) % SHD_RHO_STAGES;
-            mbar_wait(smem_u32(&empty_bar[sp]), (uint32_t)(((c - 1) / SHD_RHO_STAGES) & 1));
-            issue(c - 1 + SHD_RHO_STAGES);
-        }
     }
+#undef ROUND
 
     // partial sums: part[((split*ntiles + tile)*4 + x)*1024 + cell] as (hi, lo)
     double2* out = reinterpret_cast<double2*>(part) + ((size_t)(split * ntiles + tile) * 4) * 1024;
@@ -160,7 +186,7 @@ cudaError_t shd_rho_configure()
 cudaError_t shd_launch_rho(shd_ctx* h)
 {
     unsigned grid = (unsigned)(h->ntiles * h->nsplit);
-    k_rho<<<grid, NW * 32, RHO_SMEM, h->stream>>>(
+    k_rho<<<grid, NW * 32 + 128, RHO_SMEM, h->stream>>>(
         h->d_A, h->d_B, h->d_tile_pb, h->d_tile_qb, h->ntiles, h->Npad, h->chunks_per_split, h->d_part, h->d_skip);
     h->last_launches += 1;
     return cudaGetLastError();

@@ -39,6 +39,20 @@ __device__ __forceinline__ void dmma(Frag2& c, double a, double b) {
         : "+d"(c.c0), "+d"(c.c1) : "d"(a), "d"(b));
 }
 
+// one limb of one complex operand fragment, loaded / used in program order (volatile): the rho and
+// gradient kernels write their LDS -> DMMA software pipeline as straight-line code
+struct F2 { double r, i; };
+__device__ __forceinline__ F2 lds2(uint32_t addr) {
+    F2 f;
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(f.r), "=d"(f.i) : "r"(addr));
+    return f;
+}
+__device__ __forceinline__ F2 add2(F2 a, F2 b) { return F2{__dadd_rn(a.r, b.r), __dadd_rn(a.i, b.i)}; }
+__device__ __forceinline__ void dmma_v(Frag2& c, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c.c0), "+d"(c.c1) : "d"(a), "d"(b));
+}
+
 // one complex operand fragment: limbs 0..2 of (re, im) plus x12 = x1 + x2
 struct LimbFrag { double r0, i0, r1, i1, r2, i2, r12, i12; };
 // three LDS.128 at plane stride `ps` bytes (shared-memory byte address)

@@ -171,9 +171,9 @@ int build(shd_ctx* h, const double* v) {
                 if (kp[c] >= 0 || km[c] >= 0) nq = std::max(nq, q / SHD_QCH + 1);
             }
         for (int qg = 0; qg < nq; qg++) {
-            int flags = 0;
-            if ((qg + 1) % fold_every == 0 || qg == nq - 1) flags |= 1;
-            if (qg == nq - 1) flags |= 3;
+            // flag 1: end of a block: after <= 64 steps (one exact burst) or at the block's last q-group
+            // (the p-contraction is linear in T, so a long q-range may be contracted in pieces)
+            int flags = ((qg + 1) % fold_every == 0 || qg == nq - 1) ? 1 : 0;
             steps.push_back(pb * (h->Qpad / 4) + qg);
             steps.push_back(qg | (flags << 16));
         }

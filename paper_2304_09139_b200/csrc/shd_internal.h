@@ -95,7 +95,7 @@ struct shd_ctx {
     int *d_cell_kp = nullptr, *d_cell_km = nullptr;   // [npb*32][Qpad] -> k or -1
     int *d_tile_pb = nullptr, *d_tile_qb = nullptr;   // [ntiles]
     int *d_steps = nullptr;    // [nsteps] int2: x = C slab index pb16 * (Qpad/4) + qg, y = qg | flags << 16
-                               //   (flag 1: fold the limb burst after this step, 2: last step of its p-block)
+                               //   (flag 1: last step of a block: fold the limb burst, contract with A)
     double *d_v = nullptr;     // [M]
     // device: per-evaluation data
     double *d_A = nullptr;     // [npb][Npad/4][3 limbs][32 p][4 j][2]
