@@ -137,7 +137,8 @@ __device__ __forceinline__ limbs split_limbs(dd x) {
 }
 
 // C[p,q]: C1 = W+ + W-,  C2 = -i (W+ - W-),  W = v rho, scaled by cscale (a power of two).
-// layout [pb16][q/4][plane 6][16 p][q%4][re,im]; plane l: (C1r_l, C1i_l), plane 3+l: (C2r_l, C2i_l)
+// layout [pb16][q/4][plane 8][16 p][q%4][re,im]; planes 0..3: (C1r, C1i) limbs x0, x1, x2 and x1 + x2,
+// planes 4..7: (C2r, C2i) likewise (the sum is stored so that the gradient pass need not form it)
 // (fragment-major for the gradient pass, shd_internal.h).
 __global__ void __launch_bounds__(256) k_ctable(
     int npb16, int Qpad, const int* __restrict__ cell_kp, const int* __restrict__ cell_km, long M,
@@ -171,13 +172,15 @@ __global__ void __launch_bounds__(256) k_ctable(
     dd dr = dd_sub(wpr, wmr), di = dd_sub(wpi, wmi);
     dd c2r = di, c2i = dd_neg(dr);                 // -i (dr + i di) = di - i dr
     limbs a = split_limbs(c1r), b = split_limbs(c1i), c = split_limbs(c2r), e = split_limbs(c2i);
-    double2* dst = reinterpret_cast<double2*>(C) + ((((size_t)pb * (Qpad / 4) + qg) * 6) * 16 + pi) * 4 + q4;
+    double2* dst = reinterpret_cast<double2*>(C) + ((((size_t)pb * (Qpad / 4) + qg) * 8) * 16 + pi) * 4 + q4;
     dst[0 * 64] = make_double2(a.x0, b.x0);
     dst[1 * 64] = make_double2(a.x1, b.x1);
     dst[2 * 64] = make_double2(a.x2, b.x2);
-    dst[3 * 64] = make_double2(c.x0, e.x0);
-    dst[4 * 64] = make_double2(c.x1, e.x1);
-    dst[5 * 64] = make_double2(c.x2, e.x2);
+    dst[3 * 64] = make_double2(__dadd_rn(a.x1, a.x2), __dadd_rn(b.x1, b.x2));
+    dst[4 * 64] = make_double2(c.x0, e.x0);
+    dst[5 * 64] = make_double2(c.x1, e.x1);
+    dst[6 * 64] = make_double2(c.x2, e.x2);
+    dst[7 * 64] = make_double2(__dadd_rn(c.x1, c.x2), __dadd_rn(e.x1, e.x2));
 }
 
 }  // namespace

@@ -13,7 +13,7 @@
 // gives a partial gradient; partial gradients are summed in fixed order by k_gradsum.
 // Each warp owns 8 particles x 16 p (two 8x8 blocks) and issues the FMAs as FP64 matrix
 // instructions (DMMA.8x8x4, k = 4 q) on the limb planes: 96 per warp and step.  Operand slabs (the
-// particles' own Bg table, 2 x 12 KB, and the 16-p slab of C, 6 KB, L2 resident) arrive by TMA bulk
+// particles' own Bg table, 2 x 12 KB, and the 16-p slab of C, 8 KB, L2 resident) arrive by TMA bulk
 // copies, issued by a ninth (producer) warp, through a 5-stage full/empty mbarrier ring.  The operand fragment loads are software
 // pipelined: every LDS is issued one round of 16 DMMAs (or more) ahead of its first use and the
 // first fragments of the next step are loaded under the last round, so the two warps of a
@@ -32,8 +32,8 @@ constexpr int NST = SHD_GRAD_STAGES;
 constexpr int PLANE_B = 32 * 4 * 16;                         // 2048: one limb plane of a 32-particle Bg slab
 constexpr int PLANE_C = 16 * 4 * 16;                         // 1024: one limb plane of a 16-p C slab
 constexpr int BSLAB = 6 * PLANE_B;                           // 12288
-constexpr int CSLAB = 6 * PLANE_C;                           // 6144
-constexpr int GSTAGE = 2 * BSLAB + CSLAB;                    // 30720
+constexpr int CSLAB = 8 * PLANE_C;                           // 8192: C1 limbs x0, x1, x2, x1 + x2; C2 likewise
+constexpr int GSTAGE = 2 * BSLAB + CSLAB;                    // 32768
 constexpr int RING_BYTES = NST * GSTAGE;
 constexpr int MAIN_BYTES = 16 * 256 * 16;                    // 16 dd accumulators per thread
 constexpr int GSMEM = RING_BYTES + MAIN_BYTES;
@@ -174,7 +174,7 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
 #pragma unroll
         for (int t = 0; t < 2; t++) {
             c10[t] = lds2(s0 + offC + t * 512);
-            c20[t] = lds2(s0 + offC + t * 512 + 3 * PLANE_C);
+            c20[t] = lds2(s0 + offC + t * 512 + 4 * PLANE_C);
         }
     }
     for (int c = 0; c < total; c++) {
@@ -189,25 +189,25 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
 #pragma unroll
         for (int t = 0; t < 2; t++) {
             c11[t] = lds2(pC + t * 512 + 1 * PLANE_C);
-            c21[t] = lds2(pC + t * 512 + 4 * PLANE_C);
+            c21[t] = lds2(pC + t * 512 + 5 * PLANE_C);
         }
         GROUND(l1, b1, w1, c10, c20)
         F2 c12[2], c22[2];
 #pragma unroll
         for (int t = 0; t < 2; t++) {
             c12[t] = lds2(pC + t * 512 + 2 * PLANE_C);
-            c22[t] = lds2(pC + t * 512 + 5 * PLANE_C);
+            c22[t] = lds2(pC + t * 512 + 6 * PLANE_C);
         }
         GROUND(l2, b2, w2, c10, c20)
         const F2 b12 = add2(b1, b2), w12 = add2(w1, w2);
         GROUND(l1, b0, w0, c11, c21)
-        GROUND(l2, b0, w0, c12, c22)
-        // every LDS of stage s has been consumed by an issued DMMA: release the stage
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&empty_bar[s]));
-        F2 c1s[2], c2s[2];
+        F2 c1s[2], c2s[2];                       // x1 + x2 of the C limbs comes from the table (k_ctable)
 #pragma unroll
-        for (int t = 0; t < 2; t++) { c1s[t] = add2(c11[t], c12[t]); c2s[t] = add2(c21[t], c22[t]); }
+        for (int t = 0; t < 2; t++) {
+            c1s[t] = lds2(pC + t * 512 + 3 * PLANE_C);
+            c2s[t] = lds2(pC + t * 512 + 7 * PLANE_C);
+        }
+        GROUND(l2, b0, w0, c12, c22)
         if (c + 1 < total) {
             const int sn = (c + 1) % NST;
             mbar_wait(smem_u32(&full_bar[sn]), (uint32_t)(((c + 1) / NST) & 1));
@@ -217,10 +217,15 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
 #pragma unroll
             for (int t = 0; t < 2; t++) {
                 c10[t] = lds2(nC + t * 512);
-                c20[t] = lds2(nC + t * 512 + 3 * PLANE_C);
+                c20[t] = lds2(nC + t * 512 + 4 * PLANE_C);
             }
         }
         GROUND(l2, b12, w12, c1s, c2s)
+        // Release the stage only now: every LDS from it has been CONSUMED by an issued DMMA.  An LDS that
+        // is merely issued before the arrive may still be in flight when the refill lands (measured: one
+        // warp in ~10^5 got a stale limb when the arrive sat between the x1+x2 loads and their round).
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&empty_bar[s]));
         // deferred p-contraction: one quarter of the previous block per step, its A limbs loaded at the
         // top of this step (global-memory latency hidden under the 96 DMMAs above)
         if (pend) {

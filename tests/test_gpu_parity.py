@@ -140,6 +140,27 @@ def test_determinism(shd):
     assert np.array_equal(a["grad_hi"], b["grad_hi"]) and np.array_equal(a["grad_lo"], b["grad_lo"])
 
 
+@pytest.mark.parametrize("name,reps", [("cfg2", 200), ("cfg4", 60), ("cfg5", 20), ("cfg3", 100)])
+def test_determinism_stress(shd, name, reps):
+    """Many repeats of the same evaluation must be bit-identical in EVERY output word.  A stage of the
+    TMA ring released before all its LDS were consumed once gave one warp in ~10^5 a stale limb in
+    about one evaluation in five: a single repeat does not catch that."""
+    import torch
+    cfg = inputs.CONFIGS[name]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    th, tl = shd.from_host(hi, lo)
+    gh, gl = torch.empty_like(th), torch.empty_like(th)
+    phi0, _, _ = h.energy_grad(th, tl, gh, gl)
+    ref = [gh.clone(), gl.clone()] + [x.clone() for x in h.rho()]
+    for rep in range(reps):
+        phi, _, _ = h.energy_grad(th, tl, gh, gl)
+        assert phi == phi0, rep
+        for x, y in zip(ref, [gh, gl] + list(h.rho())):
+            assert torch.equal(x, y), (name, rep)
+    h.close()
+
+
 def test_cfg2_full_direct(shd, oracle):
     """BASELINE.json configs[1] (d=2, N=1e4, |Q|=8002) against the direct-mode oracle on a strided
     sample of k (rho) and of particles (gradient), and against the factored oracle in full."""
