@@ -14,7 +14,7 @@
 // Each warp owns 8 particles x 16 p (two 8x8 blocks) and issues the FMAs as FP64 matrix
 // instructions (DMMA.8x8x4, k = 4 q) on the limb planes: 96 per warp and step.  Operand slabs (the
 // particles' own Bg table, 2 x 12 KB, and the 16-p slab of C, 8 KB, L2 resident) arrive by TMA bulk
-// copies, issued by a ninth (producer) warp, through a 5-stage full/empty mbarrier ring.  The operand fragment loads are software
+// copies, issued by a ninth (producer) warp, through a 4-stage full/empty mbarrier ring.  The operand fragment loads are software
 // pipelined: every LDS is issued one round of 16 DMMAs (or more) ahead of its first use and the
 // first fragments of the next step are loaded under the last round, so the two warps of a
 // scheduler never stall on shared memory at the same time (they wait on the same stage).
@@ -220,12 +220,24 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
                 c20[t] = lds2(nC + t * 512 + 4 * PLANE_C);
             }
         }
-        GROUND(l2, b12, w12, c1s, c2s)
-        // Release the stage only now: every LDS from it has been CONSUMED by an issued DMMA.  An LDS that
-        // is merely issued before the arrive may still be in flight when the refill lands (measured: one
-        // warp in ~10^5 got a stale limb when the arrive sat between the x1+x2 loads and their round).
+        _Pragma("unroll") for (int t = 0; t < 2; t++) {
+            dmma_v(acc[t][0].l2, b12.r, c1s[t].r);
+            dmma_v(acc[t][1].l2, b12.r, c1s[t].i);
+            dmma_v(acc[t][2].l2, w12.r, c2s[t].r);
+            dmma_v(acc[t][3].l2, w12.r, c2s[t].i);
+        }
+        // Release the stage here: every LDS from it has been CONSUMED by an issued DMMA (the eight above
+        // read all four x1+x2 fragments).  An LDS that is merely issued before the arrive may still be in
+        // flight when the refill lands (measured: one warp in ~10^5 got a stale limb when the arrive sat
+        // between the x1+x2 loads and their round).
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(&empty_bar[s]));
+        _Pragma("unroll") for (int t = 0; t < 2; t++) {
+            dmma_v(acc[t][0].l2, b12.i, c2s[t].r);
+            dmma_v(acc[t][1].l2, b12.i, c2s[t].i);
+            dmma_v(acc[t][2].l2, w12.i, c1s[t].r);
+            dmma_v(acc[t][3].l2, w12.i, c1s[t].i);
+        }
         // deferred p-contraction: one quarter of the previous block per step, its A limbs loaded at the
         // top of this step (global-memory latency hidden under the 96 DMMAs above)
         if (pend) {

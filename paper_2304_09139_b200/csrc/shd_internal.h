@@ -38,7 +38,7 @@ constexpr int SHD_NPS = 8;          // particles per rho-pass pipeline stage (2 
 constexpr int SHD_RHO_STAGES = 6;   // TMA pipeline depth, rho pass
 constexpr int SHD_BURST = 512;      // products per exact burst (see header comment)
 constexpr int SHD_QCH = 4;          // q per gradient-pass pipeline stage (1 group of 4)
-constexpr int SHD_GRAD_STAGES = 5;  // TMA pipeline depth, gradient pass
+constexpr int SHD_GRAD_STAGES = 4;  // TMA pipeline depth, gradient pass
 constexpr int SHD_JT = 64;          // particles per gradient-pass block
 constexpr int SHD_PG = 16;          // p per gradient-pass block
 constexpr int SHD_W0 = 22;          // limb widths (bits)
