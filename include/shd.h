@@ -103,6 +103,10 @@ typedef struct {
     double smax_tol;    /* stop when S_max < smax_tol (D:R13); e.g. 1e-30                     */
     long   max_evals;   /* stop after this many energy+gradient evaluations                   */
     int    poll_every;  /* host reads the device status word every this many iterations (>=1) */
+    double fire_dt0;    /* FIRE only: initial time step (dt_max = 10 dt0); 0 = default
+                           0.05 / (k_max sqrt(2 N max v)), a quarter of the explicit stability bound */
+    int    resume;      /* FIRE only: 1 = continue the previous call on this handle (same positions
+                           buffer content as it left): keep velocities, dt, alpha; 0 = fresh start    */
 } shd_min_opts;
 
 typedef struct {
@@ -115,7 +119,11 @@ typedef struct {
  * Quench: minimise Phi from pos (DEVICE, in/out, d*N doubles each) until S_max < smax_tol.
  * The whole iteration (evaluations, dd vector algebra, line search decisions) runs on the device;
  * the host only polls a status word every poll_every iterations.  Re-entrant: call again to
- * continue.  Returns report->status.
+ * continue (L-BFGS restarts its history; FIRE keeps velocities, dt and alpha when opts->resume = 1).
+ * kind 0: L-BFGS with Armijo backtracking (D:R12); the caller's buffer ends at the last accepted point.
+ * kind 1: FIRE (ref.[37]) with the published default parameters, unit masses, semi-implicit Euler;
+ *         report->iters counts MD steps; there is no step rejection, the buffer ends at the last point
+ *         evaluated.  Returns report->status.
  */
 int shd_minimize(shd_ctx* h, double* pos_hi, double* pos_lo, const shd_min_opts* opts,
                  shd_min_report* report);

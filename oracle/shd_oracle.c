@@ -531,3 +531,62 @@ int shdo_minimize_lbfgs(int d, long N, double L, q128 *x, long M, const int *n, 
     free(g); free(gn); free(xn); free(p); free(S); free(Y); free(rho_h); free(alpha);
     return status;
 }
+
+/* ---------------------------------------------------------- a5: FIRE oracle */
+
+/*
+ * FIRE ("fast inertial relaxation engine", the minimizer the paper uses: P:75, ref.[37] P:152)
+ * in binary128.  The paper restates none of its parameters (D:R12), so this is the published
+ * algorithm with its published defaults, written out step by step; unit masses, force
+ * F = -grad Phi, semi-implicit Euler as the MD integrator:
+ *     evaluate F(x)
+ *     P = F.v
+ *     if P > 0:  v <- (1-alpha) v + alpha |v| F/|F|;
+ *                if more than N_min = 5 steps since the last P <= 0:
+ *                    dt <- min(dt f_inc, dt_max), alpha <- alpha f_alpha      (f_inc 1.1, f_alpha 0.99)
+ *     else:      v <- 0, dt <- dt f_dec, alpha <- alpha_start                 (f_dec 0.5, alpha_start 0.1)
+ *     v <- v + dt F;  x <- x + dt v
+ * dt starts at dt0, dt_max = 10 dt0.  Stops when S_max < smax_tol (checked on every
+ * evaluation, before the move) or after max_evals evaluations.  Like the L-BFGS oracle it is
+ * compared by OUTCOME only.  Returns 0 converged, 1 max_evals, 3 non-finite Phi.
+ * report = {steps, evals}.
+ */
+int shdo_minimize_fire(int d, long N, double L, q128 *x, long M, const int *n, const double *v,
+                       int mode, double dt0, double smax_tol, long max_evals, long *report,
+                       q128 *phi_out, q128 *smax_out)
+{
+    const long nd = N * d;
+    /* the parameters are the DOUBLES nearest to 1.1, 0.5, 0.1, 0.99 (what a caller can pass) */
+    const q128 f_inc = (q128)1.1, f_dec = (q128)0.5, alpha_start = (q128)0.1, f_alpha = (q128)0.99;
+    const int n_min = 5;
+    q128 *g = (q128 *)malloc(sizeof(q128) * nd), *vel = (q128 *)calloc(nd, sizeof(q128));
+    q128 phi = 0, smax = 0, dt = dt0, dt_max = (q128)(10.0 * dt0), alpha = alpha_start;
+    long arg, evals = 0, steps = 0, since = 0;
+    int status = 1;
+    while (1) {
+        shdo_eval_q(d, N, L, x, M, n, v, mode, &phi, &smax, &arg, g); evals++;
+        if (!finiteq(phi)) { status = 3; break; }
+        if ((double)smax < smax_tol) { status = 0; break; }
+        if (evals >= max_evals) { status = 1; break; }
+        q128 P = 0, vv = 0, ff = 0;
+        for (long i = 0; i < nd; i++) { P -= g[i] * vel[i]; vv += vel[i] * vel[i]; ff += g[i] * g[i]; }
+        if (P > 0) {
+            q128 c = (ff > 0) ? alpha * sqrtq(vv / ff) : 0;
+            for (long i = 0; i < nd; i++) vel[i] = (1 - alpha) * vel[i] - c * g[i];
+            if (since > n_min) {
+                dt = dt * f_inc; if (dt > dt_max) dt = dt_max;
+                alpha *= f_alpha;
+            }
+            since++;
+        } else {
+            for (long i = 0; i < nd; i++) vel[i] = 0;
+            dt *= f_dec; alpha = alpha_start; since = 0;
+        }
+        for (long i = 0; i < nd; i++) { vel[i] -= dt * g[i]; x[i] += dt * vel[i]; }
+        steps++;
+    }
+    report[0] = steps; report[1] = evals;
+    *phi_out = phi; *smax_out = smax;
+    free(g); free(vel);
+    return status;
+}

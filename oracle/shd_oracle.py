@@ -62,6 +62,9 @@ def lib():
         L.shdo_minimize_lbfgs.argtypes = [C.c_int, C.c_long, C.c_double, vp, C.c_long, ip, dp,
                                           C.c_int, C.c_int, C.c_double, C.c_long, lp, vp, vp]
         L.shdo_minimize_lbfgs.restype = C.c_int
+        L.shdo_minimize_fire.argtypes = [C.c_int, C.c_long, C.c_double, vp, C.c_long, ip, dp,
+                                         C.c_int, C.c_double, C.c_double, C.c_long, lp, vp, vp]
+        L.shdo_minimize_fire.restype = C.c_int
         _lib = L
     return _lib
 
@@ -249,3 +252,32 @@ def minimize_lbfgs(d, N, L, pos_hi, pos_lo, n, v=None, mode="direct", history=10
     hi, lo = to_dd(x)
     return dict(status=st, iters=int(rep[0]), evals=int(rep[1]), phi=phi, smax=smax,
                 pos_hi=hi, pos_lo=lo)
+
+
+def fire_dt0(d, N, L, n) -> float:
+    """Default FIRE time step: the stiffest collective mode of Phi = sum |rho|^2 has
+    curvature ~ 2 N k_max^2 (unit masses), so explicit integration is stable for dt < 2 / (k_max sqrt(2N));
+    dt_max = 10 dt0 is put at a quarter of that bound."""
+    n = np.asarray(n).reshape(-1, d)
+    kmax = 2.0 * np.pi * np.sqrt(float((n.astype(np.int64) ** 2).sum(axis=1).max())) / float(L)
+    return 0.05 / (kmax * np.sqrt(2.0 * N))
+
+
+def minimize_fire(d, N, L, pos_hi, pos_lo, n, v=None, mode="direct", dt0=None,
+                  smax_tol=1e-30, max_evals=20000):
+    """Binary128 FIRE (ref.[37]).  Returns dict with final dd positions and report."""
+    if dt0 is None:
+        dt0 = fire_dt0(d, N, L, n)
+    n, pn = _i(n)
+    M = n.size // d
+    pv = None
+    if v is not None:
+        v, pv = _d(v)
+    x = from_dd(pos_hi, pos_lo)
+    rep = (C.c_long * 2)()
+    phi, smax = qzeros(1), qzeros(1)
+    st = lib().shdo_minimize_fire(d, N, float(L), _q(x), M, pn, pv, 0 if mode == "direct" else 1,
+                                  float(dt0), float(smax_tol), int(max_evals), rep, _q(phi), _q(smax))
+    hi, lo = to_dd(x)
+    return dict(status=st, steps=int(rep[0]), evals=int(rep[1]), phi=phi, smax=smax,
+                pos_hi=hi, pos_lo=lo, dt0=float(dt0))

@@ -317,6 +317,7 @@ int shd_create(int d, long N, double L, double K, const double* v, shd_ctx** out
 void shd_destroy(shd_ctx* h) {
     if (!h) return;
     shd_min_free(h);
+    shd_fire_free(h);
     cudaFree(h->d_pn0); cudaFree(h->d_pn1); cudaFree(h->d_wT); cudaFree(h->d_cell_kp); cudaFree(h->d_cell_km);
     cudaFree(h->d_tile_pb); cudaFree(h->d_tile_qb); cudaFree(h->d_steps); cudaFree(h->d_v); cudaFree(h->d_gpart);
     cudaFree(h->d_A); cudaFree(h->d_B); cudaFree(h->d_Bg); cudaFree(h->d_C); cudaFree(h->d_part);

@@ -61,7 +61,8 @@ struct shd_scalars {
     int pad;
 };
 
-struct shd_minstate;      // minimizer workspace (shd_min.cu)
+struct shd_minstate;      // L-BFGS workspace (shd_min.cu)
+struct shd_firestate;     // FIRE workspace (shd_fire.cu)
 
 struct shd_ctx {
     int d = 0;
@@ -114,6 +115,7 @@ struct shd_ctx {
     const int* d_skip = nullptr;    // device flag: when non-NULL and *d_skip != 0 every kernel of the
                                     // evaluation path returns at once (set by the minimizer when done)
     shd_minstate *min = nullptr;
+    shd_firestate *fire = nullptr;
     std::string err;
     int last_launches = 0;
     // optional per-kernel device timing (shd_set_timing): events around each launch group
@@ -135,5 +137,6 @@ cudaError_t shd_tables_configure();
 cudaError_t shd_rho_configure();
 cudaError_t shd_grad_configure();
 
-// minimizer (shd_min.cu)
+// minimizers (shd_min.cu, shd_fire.cu)
 void shd_min_free(shd_ctx* h);
+void shd_fire_free(shd_ctx* h);

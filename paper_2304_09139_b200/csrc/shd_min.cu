@@ -17,6 +17,8 @@
 
 #include <cstring>
 
+int shd_fire_run(shd_ctx* h, double* pos_hi, double* pos_lo, const shd_min_opts* opts, shd_min_report* report);
+
 constexpr int MIN_MAXHIST = 32;
 constexpr int MIN_NBS = 2 * (MIN_MAXHIST + 1) + 1;   // basis stride of the Gram matrix
 constexpr int MIN_EPT = 4;                           // elements per thread in k_min_dots
@@ -381,7 +383,8 @@ extern "C" int shd_minimize(shd_ctx* h, double* pos_hi, double* pos_lo, const sh
                             shd_min_report* report) {
     if (!h) return SHD_EINVAL;
     if (!pos_hi || !pos_lo || !opts || !report) return min_fail(h, SHD_EINVAL, "NULL pointer");
-    if (opts->kind != 0) return min_fail(h, SHD_EINVAL, "shd_minimize: kind must be 0 (L-BFGS) in this build");
+    if (opts->kind == 1) return shd_fire_run(h, pos_hi, pos_lo, opts, report);
+    if (opts->kind != 0) return min_fail(h, SHD_EINVAL, "shd_minimize: kind must be 0 (L-BFGS) or 1 (FIRE)");
     const int m = opts->history == 0 ? 10 : opts->history;
     if (m < 1 || m > MIN_MAXHIST) return min_fail(h, SHD_EINVAL, "history must be in 1..32");
     if (!(opts->smax_tol >= 0.0) || opts->max_evals < 1 || opts->poll_every < 1)

@@ -50,7 +50,8 @@ def main(argv=None):
     t0 = time.perf_counter()
     while evals < args.max_evals:
         rep = h.minimize(pos_hi, pos_lo, kind=args.kind, history=args.history, smax_tol=args.tol,
-                         max_evals=min(args.chunk, args.max_evals - evals), poll_every=args.poll_every)
+                         max_evals=min(args.chunk, args.max_evals - evals), poll_every=args.poll_every,
+                         resume=evals > 0)
         evals += rep["evals"]
         iters += rep["iters"]
         status = rep["status"]

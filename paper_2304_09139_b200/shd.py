@@ -28,7 +28,8 @@ class ShdError(RuntimeError):
 
 class shd_min_opts(C.Structure):
     _fields_ = [("kind", C.c_int), ("history", C.c_int), ("smax_tol", C.c_double),
-                ("max_evals", C.c_long), ("poll_every", C.c_int)]
+                ("max_evals", C.c_long), ("poll_every", C.c_int), ("fire_dt0", C.c_double),
+                ("resume", C.c_int)]
 
 
 class shd_min_report(C.Structure):
@@ -181,9 +182,11 @@ class Shd:
         self._check(lib.shd_get_rho(self._h, *[C.c_void_p(t.data_ptr()) for t in out]))
         return tuple(out)
 
-    def minimize(self, pos_hi, pos_lo, kind=0, history=10, smax_tol=1e-30, max_evals=10000, poll_every=8):
+    def minimize(self, pos_hi, pos_lo, kind=0, history=10, smax_tol=1e-30, max_evals=10000, poll_every=8,
+                 fire_dt0=0.0, resume=False):
+        """shd_minimize: kind 0 = L-BFGS, 1 = FIRE (fire_dt0 = 0: the library's default time step)."""
         ph, pl = self._pos(pos_hi, pos_lo)
-        opts = shd_min_opts(kind, history, smax_tol, max_evals, poll_every)
+        opts = shd_min_opts(kind, history, smax_tol, max_evals, poll_every, fire_dt0, 1 if resume else 0)
         rep = shd_min_report()
         rc = lib.shd_minimize(self._h, ph, pl, C.byref(opts), C.byref(rep))
         self._check(rc, ok=(SHD_OK, SHD_ESTALL, SHD_EMAXEVAL))

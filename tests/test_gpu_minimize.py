@@ -110,7 +110,7 @@ def test_minimize_argument_errors(shd):
     h = shd.Shd(2, 64, 8.0, m_star=9)
     hi, lo = inputs.uniform_positions_raw(2, 64, 8.0, 0)
     th, tl = shd.from_host(hi, lo)
-    for kw in (dict(history=33), dict(max_evals=0), dict(poll_every=0), dict(kind=7)):
+    for kw in (dict(history=33), dict(max_evals=0), dict(poll_every=0), dict(kind=7), dict(kind=1, fire_dt0=-1.0)):
         with pytest.raises(shd.ShdError) as e:
             h.minimize(th, tl, **kw)
         assert e.value.code == shd.SHD_EINVAL
@@ -118,4 +118,68 @@ def test_minimize_argument_errors(shd):
     with pytest.raises(shd.ShdError) as e:
         h.minimize(bad, tl)
     assert e.value.code == shd.SHD_ENAN
+    h.close()
+
+
+# --------------------------------------------------------------------------- FIRE (kind = 1)
+def test_fire_trajectory_matches_oracle(shd, oracle):
+    """FIRE has no line search, only the sign test P > 0: the device FIRE (dd) and the binary128 FIRE
+    follow the same trajectory, so here the STEP itself is compared, not just the outcome: positions
+    after 1, 10, 40 and 200 moves from BASELINE.json configs[0]'s seeded start."""
+    cfg = inputs.CONFIGS["cfg1"]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    n = h.k()
+    for K, tol in ((2, 1e-30), (11, 1e-29), (41, 1e-27), (201, 1e-26)):
+        th, tl = shd.from_host(hi, lo)
+        with_status = h.minimize(th, tl, kind=1, smax_tol=1e-30, max_evals=K, poll_every=8)
+        o = oracle.minimize_fire(cfg.d, cfg.N, cfg.L, hi, lo, n, smax_tol=1e-30, max_evals=K)
+        assert with_status["status"] == shd.SHD_EMAXEVAL and o["status"] == 1
+        assert with_status["evals"] == o["evals"] == K and with_status["iters"] == o["steps"] == K - 1
+        e = oracle.absdiff_dd(oracle.from_dd(o["pos_hi"], o["pos_lo"]), th.cpu().numpy(), tl.cpu().numpy())
+        print(K, e.max())
+        assert e.max() <= tol, (K, e.max())
+        assert abs(with_status["phi"][0] - oracle.to_float(o["phi"])[0]) <= 1e-13 * abs(with_status["phi"][0])
+    h.close()
+
+
+@pytest.mark.parametrize("name,seed,budget", [("cfg1", 0, 5000), ("cfg1", 1, 5000), ("cfg1", 2, 5000),
+                                               ("cfg2", 0, 30000), ("cfg3", 0, 20000)])
+def test_fire_quench_reaches_1e30(shd, oracle, name, seed, budget):
+    """The paper's minimizer (FIRE) on the device reaches S_max < 1e-30 from the seeded random start
+    (no run may get stuck); the ORACLE evaluates S_max on the final positions."""
+    cfg = inputs.CONFIGS[name]
+    hi, lo = inputs.uniform_positions(cfg, seed)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    th, tl = shd.from_host(hi, lo)
+    rep = h.minimize(th, tl, kind=1, smax_tol=1e-30, max_evals=budget, poll_every=32)
+    print(name, seed, rep)
+    assert rep["status"] == shd.SHD_OK, rep
+    n = oracle.enumerate_Q(cfg.d, cfg.m_star)
+    re, im = oracle.rho(cfg.d, cfg.N, cfg.L, th.cpu().numpy(), tl.cpu().numpy(), n, mode="factored")
+    _, smax, _, _ = oracle.energy(cfg.N, re, im)
+    assert oracle.to_float(smax)[0] < 1e-30
+    # the reported values belong to the returned positions (FIRE never moves after the stop test)
+    phi1, _, _ = h.energy_grad(th, tl, want_grad=False)
+    assert phi1[0] == rep["phi"][0] and phi1[1] == rep["phi"][1]
+    h.close()
+
+
+def test_fire_resume_is_a_continuation(shd):
+    """resume=1 keeps velocities, dt and alpha: two calls of K moves each equal one call of 2K moves,
+    bit for bit; resume=0 restarts from rest and does not."""
+    cfg = inputs.CONFIGS["cfg1"]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    a_hi, a_lo = shd.from_host(hi, lo)
+    h.minimize(a_hi, a_lo, kind=1, max_evals=61, poll_every=4)            # 60 moves
+    b_hi, b_lo = shd.from_host(hi, lo)
+    h.minimize(b_hi, b_lo, kind=1, max_evals=31, poll_every=4)            # 30 moves, stops at an evaluated point
+    h.minimize(b_hi, b_lo, kind=1, max_evals=31, poll_every=4, resume=True)
+    import torch
+    assert torch.equal(a_hi, b_hi) and torch.equal(a_lo, b_lo)
+    c_hi, c_lo = shd.from_host(hi, lo)
+    h.minimize(c_hi, c_lo, kind=1, max_evals=31, poll_every=4)
+    h.minimize(c_hi, c_lo, kind=1, max_evals=31, poll_every=4)            # fresh start from rest
+    assert not torch.equal(a_hi, c_hi)
     h.close()

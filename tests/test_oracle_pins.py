@@ -357,3 +357,46 @@ def test_lbfgs_oracle_reaches_ground_state_cfg1(oracle):
     assert oracle.to_float(r["smax"])[0] < 1e-30
     assert oracle.to_float(r["phi"])[0] >= 0
     assert out["evals"] < 1.2 * out["iters"] + 20
+
+
+# --------------------------------------------------------------------------- FIRE (ref.[37])
+def test_fire_oracle_first_steps_closed_form(oracle):
+    """From rest the first FIRE evaluation has P = F.v = 0, so the step is: v <- 0, dt <- dt0 / 2,
+    v <- -dt g, x <- x - dt^2 g (closed form, using the gradient pinned by finite differences above).
+    One further evaluation has P > 0 and 'since' = 0 (no dt growth):
+    v <- (1-a) v + a |v| F/|F| with v parallel to F is v itself, then v <- v + dt F2, x <- x + dt v."""
+    d, N, L, m_star = 2, 12, 4.0, 5
+    hi, lo = inputs.uniform_positions_raw(d, N, L, 5)
+    n = oracle.enumerate_Q(d, m_star)
+    dt0 = 1e-3
+    g1 = oracle.to_float(oracle.energy_grad(d, N, L, hi, lo, n)["grad"])
+    out = oracle.minimize_fire(d, N, L, hi, lo, n, dt0=dt0, smax_tol=0.0, max_evals=2)
+    assert out["status"] == 1 and out["steps"] == 1 and out["evals"] == 2
+    dt = dt0 / 2
+    x1 = hi - dt * dt * g1
+    assert np.abs(out["pos_hi"] - x1).max() < 1e-15
+    # the second move: v1 = -dt g1 is parallel to F1 but F2 != F1, so the mixing changes v slightly:
+    # v' = (1-a) v1 + a |v1| F2/|F2|, then v'' = v' - dt g2, x2 = x1 + dt v''
+    out2 = oracle.minimize_fire(d, N, L, hi, lo, n, dt0=dt0, smax_tol=0.0, max_evals=3)
+    g2 = oracle.to_float(oracle.energy_grad(d, N, L, out["pos_hi"], out["pos_lo"], n)["grad"])
+    v1 = -dt * g1
+    assert np.dot(-g2, v1) > 0
+    vm = 0.9 * v1 - 0.1 * np.linalg.norm(v1) * g2 / np.linalg.norm(g2)
+    x2 = out["pos_hi"] + dt * (vm - dt * g2)
+    assert np.abs(out2["pos_hi"] - x2).max() < 1e-14
+
+
+@pytest.mark.parametrize("d,N,L,m_star", [(2, 32, 32 ** 0.5, 12), (1, 40, 40.0, 36), (3, 27, 3.0, 3)])
+def test_fire_oracle_reaches_ground_state(oracle, d, N, L, m_star):
+    """every quench below the chi threshold reaches a ground state -- with the paper's own
+    minimizer.  Outcome only: direct-mode S_max at the final positions < 1e-30, Phi -> 0."""
+    hi, lo = inputs.uniform_positions_raw(d, N, L, 1)
+    n = oracle.enumerate_Q(d, m_star)
+    chi = len(n) / (d * (N - 1))
+    assert chi < (1 / 3 if d == 1 else 1 / 2)
+    out = oracle.minimize_fire(d, N, L, hi, lo, n, mode="factored", smax_tol=1e-30, max_evals=40000)
+    assert out["status"] == 0, out
+    r = oracle.energy_grad(d, N, L, out["pos_hi"], out["pos_lo"], n, want_grad=False)
+    assert oracle.to_float(r["smax"])[0] < 1e-30
+    r0 = oracle.energy_grad(d, N, L, hi, lo, n, want_grad=False)
+    assert oracle.to_float(r["phi"])[0] < 1e-25 * oracle.to_float(r0["phi"])[0]
