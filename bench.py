@@ -42,6 +42,24 @@ def dist_env():
     return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
 
 
+def max_over_ranks(values, device):
+    """Element-wise MAX over all ranks of a short list of floats (timings): the contract's "time on the
+    device, max over ranks".  Works on whatever backend the process group has (nccl on the GPU box,
+    gloo in the CPU tests); with no process group it is the identity."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t.cpu()]
+
+
+def whole_job_value(pairs_per_rank, steps, world, total_ms):
+    """Whole-job throughput of N independent replicas (replicas only, weak
+    scaling): every rank processes pairs_per_rank * steps pair-terms in the max-over-ranks time."""
+    return world * float(pairs_per_rank) * steps / (total_ms * 1e-3)
+
+
 # ------------------------------------------------------------------------------ oracle legs
 def oracle_sample(cfg, hi, lo, budget_pairs, rho_dd=None):
     """Time the binary128 oracle (direct mode, as it stands) on a bounded sample of the workload:
@@ -221,17 +239,14 @@ def run_gpu(args, cfg):
     e2e_s = time.perf_counter() - t0
     barrier()
 
-    t = torch.tensor([total_ms, e2e_s * 1e3], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms, e2e_ms = float(t[0]), float(t[1])
+    total_ms, e2e_ms = max_over_ranks([total_ms, e2e_s * 1e3], "cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
     pairs = float(cfg.pairs)
-    value = world * pairs * args.steps / (total_ms * 1e-3)
-    e2e_value = world * pairs * args.steps / (e2e_ms * 1e-3)
+    value = whole_job_value(pairs, args.steps, world, total_ms)
+    e2e_value = whole_job_value(pairs, args.steps, world, e2e_ms)
     nbytes = 2 * cfg.d * cfg.N * 8
 
     # ---- roofline of the dominant kernel (ALU-bound on the FP64 pipe)
