@@ -97,6 +97,17 @@ int shd_last_smax(shd_ctx* h, double smax[2], long* argmax_k);
 /* rho(k) of the LAST evaluation: four DEVICE arrays of |Q| doubles each, canonical order. */
 int shd_get_rho(shd_ctx* h, double* re_hi, double* re_lo, double* im_hi, double* im_lo);
 
+/*
+ * Structure factor of the LAST evaluation on this handle (Eq. 3): S(k) = |rho(k)|^2 / N for every k
+ * of the handle's Q, canonical order, into S_out (DEVICE, |Q| doubles; may be NULL), and
+ * dev2 (HOST, (hi, lo)) = sum_{k in Q} (S(k) - 1)^2 in double-double, the lattice sum behind the order
+ * metric tau of Eq. 7:  tau = K^d V / N^2 * 2 * dev2  for a handle whose Q reaches far enough
+ * beyond K that S has decayed to 1 (the factor 2 counts -k; V = L^d; D = 1/K).  Create a second handle
+ * with a larger cutoff for this (S(k > K) and tau are SURVEY.md 8(f) NEXT-3; FP64 would suffice there,
+ * the dd kernels are simply reused).  Synchronises the stream.
+ */
+int shd_structure_factor(shd_ctx* h, double* S_out, double dev2[2]);
+
 typedef struct {
     int    kind;        /* 0 = L-BFGS (D:R12); 1 = FIRE                               */
     int    history;     /* L-BFGS pairs kept (1..32); 0 = default 10                          */

@@ -590,3 +590,22 @@ int shdo_minimize_fire(int d, long N, double L, q128 *x, long M, const int *n, c
     free(g); free(vel);
     return status;
 }
+
+/* ------------------------------------------------ NEXT-3: S(k) and the tau lattice sum */
+
+/*
+ * Structure factor S(k) = |rho(k)|^2 / N (Eq. 3) for the M given wavevectors and
+ * dev2 = sum_k (S(k) - 1)^2, the lattice sum behind the order metric of Eq. 7:
+ * with int dk -> (2 pi)^d / V sum over all non-zero k (= twice the half-space sum) and
+ * rho = N / V, D = 1/K:  tau = K^d V / N^2 * 2 * dev2.
+ */
+void shdo_structure_factor(long N, long M, const q128 *rho_re, const q128 *rho_im, q128 *S, q128 *dev2)
+{
+    q128 *t = (q128 *)malloc(sizeof(q128) * (size_t)M);
+    for (long k = 0; k < M; k++) {
+        S[k] = (rho_re[k] * rho_re[k] + rho_im[k] * rho_im[k]) / (q128)N;
+        t[k] = (S[k] - 1) * (S[k] - 1);
+    }
+    *dev2 = pairwise_sum(t, M);
+    free(t);
+}

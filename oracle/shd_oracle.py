@@ -65,6 +65,7 @@ def lib():
         L.shdo_minimize_fire.argtypes = [C.c_int, C.c_long, C.c_double, vp, C.c_long, ip, dp,
                                          C.c_int, C.c_double, C.c_double, C.c_long, lp, vp, vp]
         L.shdo_minimize_fire.restype = C.c_int
+        L.shdo_structure_factor.argtypes = [C.c_long, C.c_long, vp, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -281,3 +282,16 @@ def minimize_fire(d, N, L, pos_hi, pos_lo, n, v=None, mode="direct", dt0=None,
     hi, lo = to_dd(x)
     return dict(status=st, steps=int(rep[0]), evals=int(rep[1]), phi=phi, smax=smax,
                 pos_hi=hi, pos_lo=lo, dt0=float(dt0))
+
+
+def structure_factor(N, rho_re, rho_im):
+    """S(k) = |rho|^2 / N (binary128 array) and sum_k (S - 1)^2 (Eq. 3, Eq. 7)."""
+    M = len(rho_re)
+    S, dev2 = qzeros(M), qzeros(1)
+    lib().shdo_structure_factor(int(N), M, _q(rho_re), _q(rho_im), _q(S), _q(dev2))
+    return S, dev2
+
+
+def tau(d, N, L, K, dev2) -> float:
+    """tau = K^d V / N^2 * 2 * sum_{k in half space} (S(k) - 1)^2   (Eq. 7, D = 1/K)."""
+    return float(K) ** d * float(L) ** d / float(N) ** 2 * 2.0 * float(to_float(dev2)[0])

@@ -183,7 +183,44 @@ __global__ void __launch_bounds__(256) k_ctable(
     dst[7 * 64] = make_double2(__dadd_rn(c.x1, c.x2), __dadd_rn(e.x1, e.x2));
 }
 
+// NEXT-3 (Eq. 7, Eq. 3): S(k) = |rho(k)|^2 / N for every k of the handle's Q, and the
+// sum over Q of (S(k) - 1)^2 that the order metric tau integrates, in double-double, fixed tree.
+__global__ void __launch_bounds__(256) k_sfactor1(long M, long N, const double* __restrict__ rho,
+                                                  double* __restrict__ S_out, double* __restrict__ blockred)
+{
+    const long k = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    red r; r.phi = dd{0, 0}; r.smax = dd{-1, 0}; r.arg = -1; r.maxvs = 0;
+    if (k < M) {
+        dd re{rho[k], rho[M + k]}, im{rho[2 * M + k], rho[3 * M + k]};
+        dd s = dd_div_d(dd_add(dd_mul(re, re), dd_mul(im, im)), (double)N);
+        if (S_out) S_out[k] = s.h;
+        dd e = dd_add_d(s, -1.0);
+        r.phi = dd_mul(e, e);
+    }
+    r = block_reduce(r);
+    if (threadIdx.x == 0) { blockred[2 * blockIdx.x] = r.phi.h; blockred[2 * blockIdx.x + 1] = r.phi.l; }
+}
+__global__ void __launch_bounds__(1024) k_sfactor2(const double* __restrict__ blockred, int nblocks,
+                                                   double* __restrict__ out)
+{
+    red r; r.phi = dd{0, 0}; r.smax = dd{-1, 0}; r.arg = -1; r.maxvs = 0;
+    for (int b = threadIdx.x; b < nblocks; b += blockDim.x)
+        r.phi = dd_add(r.phi, dd{blockred[2 * b], blockred[2 * b + 1]});
+    r = block_reduce(r);
+    if (threadIdx.x == 0) { out[0] = r.phi.h; out[1] = r.phi.l; }
+}
+
 }  // namespace
+
+// S_out (device, M doubles) may be NULL; tau2 (device, 2 doubles) receives sum_k (S(k)-1)^2 as (hi, lo)
+cudaError_t shd_launch_sfactor(shd_ctx* h, double* S_out, double* scratch, double* tau2)
+{
+    const int nb = (int)((h->M + 255) / 256);
+    k_sfactor1<<<nb, 256, 0, h->stream>>>(h->M, h->N, h->d_rho, S_out, scratch);
+    k_sfactor2<<<1, 1024, 0, h->stream>>>(scratch, nb, tau2);
+    h->last_launches += 2;
+    return cudaGetLastError();
+}
 
 cudaError_t shd_launch_finish(shd_ctx* h)
 {

@@ -433,6 +433,20 @@ int shd_get_rho(shd_ctx* h, double* re_hi, double* re_lo, double* im_hi, double*
     return SHD_OK;
 }
 
+int shd_structure_factor(shd_ctx* h, double* S_out, double dev2[2]) {
+    if (!h) return SHD_EINVAL;
+    if (!dev2) return fail(h, SHD_EINVAL, "NULL pointer");
+    const size_t nb = (size_t)((h->M + 255) / 256);
+    double* scratch = nullptr;
+    CU(cudaMalloc((void**)&scratch, (2 * nb + 2) * sizeof(double)));
+    cudaError_t e = shd_launch_sfactor(h, S_out, scratch, scratch + 2 * nb);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dev2, scratch + 2 * nb, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    cudaFree(scratch);
+    CU(e);
+    return SHD_OK;
+}
+
 const char* shd_last_error(const shd_ctx* h) { return h ? h->err.c_str() : "NULL handle"; }
 
 double shd_stat(const shd_ctx* h, int what) {

@@ -132,6 +132,7 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
 cudaError_t shd_launch_rho(shd_ctx* h);
 cudaError_t shd_launch_finish(shd_ctx* h);
 cudaError_t shd_launch_ctable(shd_ctx* h);
+cudaError_t shd_launch_sfactor(shd_ctx* h, double* S_out, double* scratch, double* tau2);
 cudaError_t shd_launch_grad(shd_ctx* h, double* grad_hi, double* grad_lo);
 cudaError_t shd_tables_configure();
 cudaError_t shd_rho_configure();

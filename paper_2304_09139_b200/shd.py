@@ -17,7 +17,7 @@ LIB_PATH = _HERE / "libshd.so"
 SHD_OK, SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA, SHD_ENAN, SHD_ESTALL, SHD_EMAXEVAL = 0, -1, -2, -3, -4, -5, -6
 EXPORTS = ["shd_create", "shd_create_shell", "shd_destroy", "shd_set_stream", "shd_num_k", "shd_get_k",
            "shd_energy_grad", "shd_energy_grad_host", "shd_set_timing", "shd_smax", "shd_last_smax", "shd_get_rho", "shd_minimize",
-           "shd_last_error", "shd_stat", "shd_fp64_peak"]
+           "shd_last_error", "shd_stat", "shd_fp64_peak", "shd_structure_factor"]
 
 
 class ShdError(RuntimeError):
@@ -63,6 +63,7 @@ def _load():
     lib.shd_stat.argtypes = [vp, C.c_int]
     lib.shd_stat.restype = C.c_double
     lib.shd_fp64_peak.argtypes = [C.c_int, C.c_double, dp]
+    lib.shd_structure_factor.argtypes = [vp, vp, dp]
     return lib
 
 
@@ -181,6 +182,22 @@ class Shd:
         out = [torch.empty(self.M, dtype=torch.float64, device="cuda") for _ in range(4)]
         self._check(lib.shd_get_rho(self._h, *[C.c_void_p(t.data_ptr()) for t in out]))
         return tuple(out)
+
+    def structure_factor(self, want_S=True):
+        """shd_structure_factor on the last evaluation: (S device tensor or None, (hi, lo) of
+        sum_{k in Q} (S(k) - 1)^2)."""
+        torch = _torch()
+        S = torch.empty(self.M, dtype=torch.float64, device="cuda") if want_S else None
+        dev2 = (C.c_double * 2)()
+        self._check(lib.shd_structure_factor(self._h, C.c_void_p(S.data_ptr()) if want_S else None, dev2))
+        return S, (dev2[0], dev2[1])
+
+    def tau(self, K):
+        """Order metric tau of Eq. 7 from the last evaluation on this handle, D = 1/K, as the
+        lattice sum over +-Q:  tau = K^d V / N^2 * 2 sum_{k in Q} (S(k) - 1)^2  (V = L^d).  The handle's
+        own cutoff must reach far enough beyond K that S(k) has decayed to 1."""
+        _, (hi, lo) = self.structure_factor(want_S=False)
+        return float(K) ** self.d * self.L ** self.d / float(self.N) ** 2 * 2.0 * (hi + lo)
 
     def minimize(self, pos_hi, pos_lo, kind=0, history=10, smax_tol=1e-30, max_evals=10000, poll_every=8,
                  fire_dt0=0.0, resume=False):

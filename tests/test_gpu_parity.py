@@ -182,3 +182,30 @@ def test_cfg2_full_direct(shd, oracle):
     eg = oracle.absdiff_dd(og, g["grad_hi"][sel], g["grad_lo"][sel])
     assert eg.max() <= 1e-27 * cfg.N * cfg.M * cfg.K
     print("cfg2 direct sample", e.max(), eg.max())
+
+
+def test_structure_factor_and_tau(shd, oracle):
+    """NEXT-3 (Eq. 3, Eq. 7): S(k) on a handle whose cutoff reaches beyond K, and the lattice sum
+    behind tau, against the oracle; closed forms: a lattice has S = 0 on Q, so sum (S-1)^2 = |Q| exactly."""
+    cfg = inputs.CONFIGS["cfg1"]
+    m_big = 4 * cfg.m_star                       # |k| up to 2 K
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=m_big)
+    th, tl = shd.from_host(hi, lo)
+    h.energy_grad(th, tl, want_grad=False)
+    S, dev2 = h.structure_factor()
+    n = oracle.enumerate_Q(cfg.d, m_big)
+    assert np.array_equal(h.k(), n)
+    re, im = oracle.rho(cfg.d, cfg.N, cfg.L, hi, lo, n)
+    So, dev2o = oracle.structure_factor(cfg.N, re, im)
+    assert np.abs(S.cpu().numpy() - oracle.to_float(So)).max() <= 1e-14 * cfg.N      # S is returned as one double
+    assert oracle.absdiff_dd(dev2o, [dev2[0]], [dev2[1]])[0] <= 1e-28 * cfg.N ** 2 * len(n)
+    assert h.tau(cfg.K) == pytest.approx(oracle.tau(cfg.d, cfg.N, cfg.L, cfg.K, dev2o), rel=1e-14)
+    h.close()
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    hi, lo = inputs.lattice((16, 8), cfg.L)
+    th, tl = shd.from_host(hi, lo)
+    h.energy_grad(th, tl, want_grad=False)
+    S, dev2 = h.structure_factor()
+    assert float(S.abs().max()) < 1e-25 and abs(dev2[0] - h.M) < 1e-12
+    h.close()

@@ -400,3 +400,34 @@ def test_fire_oracle_reaches_ground_state(oracle, d, N, L, m_star):
     assert oracle.to_float(r["smax"])[0] < 1e-30
     r0 = oracle.energy_grad(d, N, L, hi, lo, n, want_grad=False)
     assert oracle.to_float(r["phi"])[0] < 1e-25 * oracle.to_float(r0["phi"])[0]
+
+
+# --------------------------------------------------------------------------- S(k), tau (Eq. 3, Eq. 7)
+def test_structure_factor_closed_forms(oracle):
+    """S(k) = |rho|^2 / N and sum_k (S-1)^2: single site => S = N for every k, sum = M (N-1)^2;
+    perfect lattice with its first reciprocal shell beyond the cutoff => S = 0 on Q, sum = M
+    (a stealthy state contributes exactly 2M K^d V / N^2 to tau from inside the exclusion region);
+    ideal gas (tau = 0 in the thermodynamic limit) => S(k) is exponentially distributed with
+    mean 1 at finite N, so the sample mean of (S-1)^2 is 1 within statistics."""
+    d, N, L, m_star = 2, 128, 128 ** 0.5, 49
+    n = oracle.enumerate_Q(d, m_star)
+    M = len(n)
+    hi, lo = inputs.single_site(d, N, [1.234, 5.678])
+    re, im = oracle.rho(d, N, L, hi, lo, n)
+    S, dev2 = oracle.structure_factor(N, re, im)
+    assert np.abs(oracle.to_float(S) - N).max() < 1e-10
+    assert abs(oracle.to_float(dev2)[0] - M * (N - 1) ** 2) < 1e-6
+    hi, lo = inputs.lattice((16, 8), L)
+    re, im = oracle.rho(d, N, L, hi, lo, n)
+    S, dev2 = oracle.structure_factor(N, re, im)
+    assert np.abs(oracle.to_float(S)).max() < 1e-25      # lattice sites are rounded to double (lo = 0)
+    assert abs(oracle.to_float(dev2)[0] - M) < 1e-20
+    K = 2 * np.pi / L * np.sqrt(m_star + 0.5)
+    assert oracle.tau(d, N, L, K, dev2) == pytest.approx(2 * M * K ** d * L ** d / N ** 2, rel=1e-14)
+    vals = []
+    for seed in range(8):
+        hi, lo = inputs.uniform_positions_raw(d, N, L, 100 + seed)
+        re, im = oracle.rho(d, N, L, hi, lo, n, mode="factored")
+        S, dev2 = oracle.structure_factor(N, re, im)
+        vals.append(oracle.to_float(dev2)[0] / M)
+    assert 0.8 < np.mean(vals) < 1.2, vals
