@@ -136,12 +136,12 @@ __device__ __forceinline__ limbs split_limbs(dd x) {
     return r;
 }
 
-// C[p,q]: C1 = W+ + W-,  C2 = -i (W+ - W-),  W = v rho, scaled by cscale (a power of two).
-// layout [pb16][q/4][plane 8][16 p][q%4][re,im]; planes 0..3: (C1r, C1i) limbs x0, x1, x2 and x1 + x2,
-// planes 4..7: (C2r, C2i) likewise (the sum is stored so that the gradient pass need not form it)
-// (fragment-major for the gradient pass, shd_internal.h).
+// Shared operand of the gradient pass: C1 = W+ + W-,  C2 = -i (W+ - W-),  W = v rho scaled by cscale (a
+// power of two), and the q-weighted pair D1 = q C2, D2 = -q C1 scaled by 2^-qscale_log2 (exact).
+// layout [pb16][q/4][plane 16][16 p][q%4][re,im]; plane 4 o + l: operand o (C1, C2, D1, D2), limb l of
+// (re, im) for l = 0..2 and x1 + x2 for l = 3 (stored so that the gradient pass need not form it).
 __global__ void __launch_bounds__(256) k_ctable(
-    int npb16, int Qpad, const int* __restrict__ cell_kp, const int* __restrict__ cell_km, long M,
+    int npb16, int Qpad, int qscale_log2, const int* __restrict__ cell_kp, const int* __restrict__ cell_km, long M,
     const double* __restrict__ v, const double* __restrict__ rho, const shd_scalars* __restrict__ scal,
     double* __restrict__ C, const int* __restrict__ skip)
 {
@@ -168,19 +168,22 @@ __global__ void __launch_bounds__(256) k_ctable(
         wmr = dd_scale2(dd_mul_d(dd{rho[km], rho[M + km]}, vv), sc);
         wmi = dd_scale2(dd_mul_d(dd{rho[2 * M + km], rho[3 * M + km]}, vv), sc);
     }
-    dd c1r = dd_add(wpr, wmr), c1i = dd_add(wpi, wmi);
+    dd op[4][2];
+    op[0][0] = dd_add(wpr, wmr); op[0][1] = dd_add(wpi, wmi);                 // C1
     dd dr = dd_sub(wpr, wmr), di = dd_sub(wpi, wmi);
-    dd c2r = di, c2i = dd_neg(dr);                 // -i (dr + i di) = di - i dr
-    limbs a = split_limbs(c1r), b = split_limbs(c1i), c = split_limbs(c2r), e = split_limbs(c2i);
-    double2* dst = reinterpret_cast<double2*>(C) + ((((size_t)pb * (Qpad / 4) + qg) * 8) * 16 + pi) * 4 + q4;
-    dst[0 * 64] = make_double2(a.x0, b.x0);
-    dst[1 * 64] = make_double2(a.x1, b.x1);
-    dst[2 * 64] = make_double2(a.x2, b.x2);
-    dst[3 * 64] = make_double2(__dadd_rn(a.x1, a.x2), __dadd_rn(b.x1, b.x2));
-    dst[4 * 64] = make_double2(c.x0, e.x0);
-    dst[5 * 64] = make_double2(c.x1, e.x1);
-    dst[6 * 64] = make_double2(c.x2, e.x2);
-    dst[7 * 64] = make_double2(__dadd_rn(c.x1, c.x2), __dadd_rn(e.x1, e.x2));
+    op[1][0] = di; op[1][1] = dd_neg(dr);                                     // C2 = -i (dr + i di) = di - i dr
+    const double qw = ldexp((double)q, -qscale_log2);                         // q 2^-qs <= 1
+    op[2][0] = dd_mul_d(op[1][0], qw); op[2][1] = dd_mul_d(op[1][1], qw);     // D1 =  q C2
+    op[3][0] = dd_mul_d(op[0][0], -qw); op[3][1] = dd_mul_d(op[0][1], -qw);   // D2 = -q C1
+    double2* dst = reinterpret_cast<double2*>(C) + ((((size_t)pb * (Qpad / 4) + qg) * 16) * 16 + pi) * 4 + q4;
+#pragma unroll
+    for (int o = 0; o < 4; o++) {
+        limbs a = split_limbs(op[o][0]), b = split_limbs(op[o][1]);
+        dst[(o * 4 + 0) * 64] = make_double2(a.x0, b.x0);
+        dst[(o * 4 + 1) * 64] = make_double2(a.x1, b.x1);
+        dst[(o * 4 + 2) * 64] = make_double2(a.x2, b.x2);
+        dst[(o * 4 + 3) * 64] = make_double2(__dadd_rn(a.x1, a.x2), __dadd_rn(b.x1, b.x2));
+    }
 }
 
 // NEXT-3 (Eq. 7, Eq. 3): S(k) = |rho(k)|^2 / N for every k of the handle's Q, and the
@@ -237,7 +240,7 @@ cudaError_t shd_launch_ctable(shd_ctx* h)
 {
     long ncell = (long)h->npb16 * 16 * h->Qpad;
     k_ctable<<<(unsigned)((ncell + 255) / 256), 256, 0, h->stream>>>(
-        h->npb16, h->Qpad, h->d_cell_kp, h->d_cell_km, h->M, h->d_v, h->d_rho, h->d_scal, h->d_C, h->d_skip);
+        h->npb16, h->Qpad, h->qscale_log2, h->d_cell_kp, h->d_cell_km, h->M, h->d_v, h->d_rho, h->d_scal, h->d_C, h->d_skip);
     h->last_launches += 1;
     return cudaGetLastError();
 }

@@ -1,10 +1,12 @@
 // k_grad.cu -- step a4: dPhi/dr_{j,a} = (4 pi / L) sum_k v_k n_a Im[ exp(-i k.r_j) rho(k) ]
 // (Eq. 6, sign D:R2) as two contractions over q followed by one over p:
 //   T_j[p]   = sum_{q,sigma} W(p,q,sigma) conj(B_j[q]^sigma)          = sum_q ( C1 br + C2 bi )
-//   T''_j[p] = -i sum_{q,sigma} sigma q W conj(B^sigma)               = sum_q ( C2 (q br) - C1 (q bi) )
+//   T''_j[p] = -i sum_{q,sigma} sigma q W conj(B^sigma)               = sum_q ( D1 br + D2 bi ),  D1 = q C2, D2 = -q C1
 //   grad_a   = (4 pi/L) sum_p ( w_a(p) Im[conj(A_j[p]) T_j[p]] + [a = last axis] Re[conj(A_j[p]) T''_j[p]] )
 // with C1 = W+ + W-, C2 = -i (W+ - W-), W = v rho (built by k_ctable), so both signs of the last
-// axis share the same products: 24 FP64 FMAs per particle-wavevector pair.
+// axis share the same products: 24 FP64 FMAs per particle-wavevector pair.  The weight q of the last
+// axis sits on the SHARED operand (C, D: 16 KB per slab, L2 resident), not on the particles' table, which
+// therefore holds only the phasor limbs (half the bytes to write in k_tables and to stream here).
 //
 // Work unit (one CTA) = 64 particles x one segment of the step list.  A step is one group of 4 q of
 // one block of 16 p (host-built list, shd_api.cu); a block's q-range ends at the circle boundary of
@@ -13,7 +15,7 @@
 // gives a partial gradient; partial gradients are summed in fixed order by k_gradsum.
 // Each warp owns 8 particles x 16 p (two 8x8 blocks) and issues the FMAs as FP64 matrix
 // instructions (DMMA.8x8x4, k = 4 q) on the limb planes: 96 per warp and step.  Operand slabs (the
-// particles' own Bg table, 2 x 12 KB, and the 16-p slab of C, 8 KB, L2 resident) arrive by TMA bulk
+// particles' own Bg table, 2 x 6 KB, and the 16-p slab of C and D, 16 KB, L2 resident) arrive by TMA bulk
 // copies, issued by a ninth (producer) warp, through a 4-stage full/empty mbarrier ring.  The operand fragment loads are software
 // pipelined: every LDS is issued one round of 16 DMMAs (or more) ahead of its first use and the
 // first fragments of the next step are loaded under the last round, so the two warps of a
@@ -31,9 +33,9 @@ constexpr int NW = 8;
 constexpr int NST = SHD_GRAD_STAGES;
 constexpr int PLANE_B = 32 * 4 * 16;                         // 2048: one limb plane of a 32-particle Bg slab
 constexpr int PLANE_C = 16 * 4 * 16;                         // 1024: one limb plane of a 16-p C slab
-constexpr int BSLAB = 6 * PLANE_B;                           // 12288
-constexpr int CSLAB = 8 * PLANE_C;                           // 8192: C1 limbs x0, x1, x2, x1 + x2; C2 likewise
-constexpr int GSTAGE = 2 * BSLAB + CSLAB;                    // 32768
+constexpr int BSLAB = 3 * PLANE_B;                           // 6144: limbs of b
+constexpr int CSLAB = 16 * PLANE_C;                          // 16384: C1, C2, D1, D2, each x0, x1, x2, x1 + x2
+constexpr int GSTAGE = 2 * BSLAB + CSLAB;                    // 28672
 constexpr int RING_BYTES = NST * GSTAGE;
 constexpr int MAIN_BYTES = 16 * 256 * 16;                    // 16 dd accumulators per thread
 constexpr int GSMEM = RING_BYTES + MAIN_BYTES;
@@ -42,21 +44,24 @@ __device__ __forceinline__ dd limbs_to_dd(double x0, double x1, double x2) {
     return fast_two_sum(__dadd_rn(x0, x1), x2);    // x0 + x1 is exact (44 bits)
 }
 
-// one round: 16 DMMAs on limb level LV; particle-side limbs (b, w), C-side limbs (c1[t], c2[t]).
-// w holds (q br, -q bi) (k_tables stores the sign), so T'' = C2 (q br) - C1 (q bi) is all additions.
-#define GROUND(LV, Bx, Wx, C1x, C2x)                                        \
+// one round: 16 DMMAs on limb level LV; particle-side limb b, shared-side limbs of C1, C2, D1, D2
+#define GROUND(LV, Bx, X)                                                   \
     _Pragma("unroll") for (int t = 0; t < 2; t++) {                         \
-        dmma_v(acc[t][0].LV, Bx.r, C1x[t].r);                               \
-        dmma_v(acc[t][1].LV, Bx.r, C1x[t].i);                               \
-        dmma_v(acc[t][2].LV, Wx.r, C2x[t].r);                               \
-        dmma_v(acc[t][3].LV, Wx.r, C2x[t].i);                               \
+        dmma_v(acc[t][0].LV, Bx.r, X[0][t].r);                              \
+        dmma_v(acc[t][1].LV, Bx.r, X[0][t].i);                              \
+        dmma_v(acc[t][2].LV, Bx.r, X[2][t].r);                              \
+        dmma_v(acc[t][3].LV, Bx.r, X[2][t].i);                              \
     }                                                                       \
     _Pragma("unroll") for (int t = 0; t < 2; t++) {                         \
-        dmma_v(acc[t][0].LV, Bx.i, C2x[t].r);                               \
-        dmma_v(acc[t][1].LV, Bx.i, C2x[t].i);                               \
-        dmma_v(acc[t][2].LV, Wx.i, C1x[t].r);                               \
-        dmma_v(acc[t][3].LV, Wx.i, C1x[t].i);                               \
+        dmma_v(acc[t][0].LV, Bx.i, X[1][t].r);                              \
+        dmma_v(acc[t][1].LV, Bx.i, X[1][t].i);                              \
+        dmma_v(acc[t][2].LV, Bx.i, X[3][t].r);                              \
+        dmma_v(acc[t][3].LV, Bx.i, X[3][t].i);                              \
     }
+// fragments of limb plane L of the four shared operands (o = 0..3: C1, C2, D1, D2), both 8-p blocks
+#define LOADX(X, base, L)                                                   \
+    _Pragma("unroll") for (int o = 0; o < 4; o++)                           \
+        _Pragma("unroll") for (int t = 0; t < 2; t++) X[o][t] = lds2((base) + t * 512 + (o * 4 + (L)) * PLANE_C);
 
 __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
     int d, long N, long Npad, long njb64, int Qpad, int Ppad, int qscale_log2,
@@ -94,8 +99,8 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
         // producer warp (one lane): stage of step i <- Bg slabs of the two 32-particle halves + C slab;
         // it does nothing else, so a refill is issued the moment the last consumer warp releases a stage
         if (warp == NW && lane == 0) {
-            const double* gB = Bg + (size_t)(2 * jb) * (Qpad / 4) * SHD_GGROUP_DOUBLES;
-            const size_t halfB = (size_t)(Qpad / 4) * SHD_GGROUP_DOUBLES;
+            const double* gB = Bg + (size_t)(2 * jb) * (Qpad / 4) * SHD_GROUP_DOUBLES;
+            const size_t halfB = (size_t)(Qpad / 4) * SHD_GROUP_DOUBLES;
             for (int i = 0; i < total; i++) {
                 const int stage = i % NST;
                 if (i >= NST) mbar_wait(smem_u32(&empty_bar[stage]), (uint32_t)((i / NST - 1) & 1));
@@ -103,8 +108,8 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
                 const int2 st = steps[c_begin + i];
                 const int qg = st.y & 0xffff;
                 mbar_expect_tx(bar, GSTAGE);
-                tma_load_1d(s0 + stage * GSTAGE, gB + (size_t)qg * SHD_GGROUP_DOUBLES, BSLAB, bar);
-                tma_load_1d(s0 + stage * GSTAGE + BSLAB, gB + halfB + (size_t)qg * SHD_GGROUP_DOUBLES, BSLAB, bar);
+                tma_load_1d(s0 + stage * GSTAGE, gB + (size_t)qg * SHD_GROUP_DOUBLES, BSLAB, bar);
+                tma_load_1d(s0 + stage * GSTAGE + BSLAB, gB + halfB + (size_t)qg * SHD_GROUP_DOUBLES, BSLAB, bar);
                 tma_load_1d(s0 + stage * GSTAGE + 2 * BSLAB, C + (size_t)st.x * (CSLAB / 8), CSLAB, bar);
             }
         }
@@ -166,77 +171,57 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
         }
     };
 
-    F2 b0, w0, c10[2], c20[2];
+    F2 b0, X0[4][2];
     if (total > 0) {
         mbar_wait(smem_u32(&full_bar[0]), 0u);
         b0 = lds2(s0 + offB);
-        w0 = lds2(s0 + offB + 3 * PLANE_B);
-#pragma unroll
-        for (int t = 0; t < 2; t++) {
-            c10[t] = lds2(s0 + offC + t * 512);
-            c20[t] = lds2(s0 + offC + t * 512 + 4 * PLANE_C);
-        }
+        LOADX(X0, s0 + offC, 0)
     }
     for (int c = 0; c < total; c++) {
         const int s = c % NST;
         const uint32_t pB = s0 + s * GSTAGE + offB, pC = s0 + s * GSTAGE + offC;
         const int2 st = steps[c_begin + c];
         if (pend) load_quarter(pk, ppb, pa0, pa1, pa2);
-        const F2 b1 = lds2(pB + 1 * PLANE_B), w1 = lds2(pB + 4 * PLANE_B);
-        const F2 b2 = lds2(pB + 2 * PLANE_B), w2 = lds2(pB + 5 * PLANE_B);
-        GROUND(l0, b0, w0, c10, c20)
-        F2 c11[2], c21[2];
-#pragma unroll
-        for (int t = 0; t < 2; t++) {
-            c11[t] = lds2(pC + t * 512 + 1 * PLANE_C);
-            c21[t] = lds2(pC + t * 512 + 5 * PLANE_C);
-        }
-        GROUND(l1, b1, w1, c10, c20)
-        F2 c12[2], c22[2];
-#pragma unroll
-        for (int t = 0; t < 2; t++) {
-            c12[t] = lds2(pC + t * 512 + 2 * PLANE_C);
-            c22[t] = lds2(pC + t * 512 + 6 * PLANE_C);
-        }
-        GROUND(l2, b2, w2, c10, c20)
-        const F2 b12 = add2(b1, b2), w12 = add2(w1, w2);
-        GROUND(l1, b0, w0, c11, c21)
-        F2 c1s[2], c2s[2];                       // x1 + x2 of the C limbs comes from the table (k_ctable)
-#pragma unroll
-        for (int t = 0; t < 2; t++) {
-            c1s[t] = lds2(pC + t * 512 + 3 * PLANE_C);
-            c2s[t] = lds2(pC + t * 512 + 7 * PLANE_C);
-        }
-        GROUND(l2, b0, w0, c12, c22)
+        const F2 b1 = lds2(pB + 1 * PLANE_B), b2 = lds2(pB + 2 * PLANE_B);
+        GROUND(l0, b0, X0)
+        F2 X1[4][2];
+        LOADX(X1, pC, 1)
+        GROUND(l1, b1, X0)
+        F2 X2[4][2];
+        LOADX(X2, pC, 2)
+        GROUND(l2, b2, X0)
+        const F2 b12 = add2(b1, b2);
+        GROUND(l1, b0, X1)
+        F2 XS[4][2];                             // x1 + x2 of the shared operands comes from the table (k_ctable)
+        LOADX(XS, pC, 3)
+        GROUND(l2, b0, X2)
         if (c + 1 < total) {
             const int sn = (c + 1) % NST;
             mbar_wait(smem_u32(&full_bar[sn]), (uint32_t)(((c + 1) / NST) & 1));
-            const uint32_t nB = s0 + sn * GSTAGE + offB, nC = s0 + sn * GSTAGE + offC;
-            b0 = lds2(nB);
-            w0 = lds2(nB + 3 * PLANE_B);
-#pragma unroll
-            for (int t = 0; t < 2; t++) {
-                c10[t] = lds2(nC + t * 512);
-                c20[t] = lds2(nC + t * 512 + 4 * PLANE_C);
-            }
+            b0 = lds2(s0 + sn * GSTAGE + offB);
+            LOADX(X0, s0 + sn * GSTAGE + offC, 0)
+        }
+        // last round, first half: eight DMMAs that read all eight x1+x2 fragments
+        _Pragma("unroll") for (int t = 0; t < 2; t++) {
+            dmma_v(acc[t][0].l2, b12.r, XS[0][t].r);
+            dmma_v(acc[t][2].l2, b12.r, XS[2][t].r);
         }
         _Pragma("unroll") for (int t = 0; t < 2; t++) {
-            dmma_v(acc[t][0].l2, b12.r, c1s[t].r);
-            dmma_v(acc[t][1].l2, b12.r, c1s[t].i);
-            dmma_v(acc[t][2].l2, w12.r, c2s[t].r);
-            dmma_v(acc[t][3].l2, w12.r, c2s[t].i);
+            dmma_v(acc[t][0].l2, b12.i, XS[1][t].r);
+            dmma_v(acc[t][2].l2, b12.i, XS[3][t].r);
         }
-        // Release the stage here: every LDS from it has been CONSUMED by an issued DMMA (the eight above
-        // read all four x1+x2 fragments).  An LDS that is merely issued before the arrive may still be in
-        // flight when the refill lands (measured: one warp in ~10^5 got a stale limb when the arrive sat
-        // between the x1+x2 loads and their round).
+        // Release the stage here: every LDS from it has been CONSUMED by an issued DMMA.  An LDS that is
+        // merely issued before the arrive may still be in flight when the refill lands (measured: one
+        // warp in ~10^5 got a stale limb when the arrive sat between the x1+x2 loads and their round).
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(&empty_bar[s]));
         _Pragma("unroll") for (int t = 0; t < 2; t++) {
-            dmma_v(acc[t][0].l2, b12.i, c2s[t].r);
-            dmma_v(acc[t][1].l2, b12.i, c2s[t].i);
-            dmma_v(acc[t][2].l2, w12.i, c1s[t].r);
-            dmma_v(acc[t][3].l2, w12.i, c1s[t].i);
+            dmma_v(acc[t][1].l2, b12.r, XS[0][t].i);
+            dmma_v(acc[t][3].l2, b12.r, XS[2][t].i);
+        }
+        _Pragma("unroll") for (int t = 0; t < 2; t++) {
+            dmma_v(acc[t][1].l2, b12.i, XS[1][t].i);
+            dmma_v(acc[t][3].l2, b12.i, XS[3][t].i);
         }
         // deferred p-contraction: one quarter of the previous block per step, its A limbs loaded at the
         // top of this step (global-memory latency hidden under the 96 DMMAs above)

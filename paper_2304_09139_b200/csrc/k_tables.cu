@@ -67,17 +67,17 @@ __device__ __forceinline__ limbs split_limbs(dd x) {
 constexpr int R3MAX = 128;   // d == 3: max |n_1| supported by the local power table
 constexpr int TB = 64;       // particles (threads) per block
 constexpr int TG = 8;        // table entries staged per flush: 8 x 16 B = one 128-byte row per limb plane
-constexpr int TABLES_SMEM = TB * 6 * TG * 16;
+constexpr int TABLES_SMEM = TB * 3 * TG * 16;
 
 // Staging tile: a thread owns one particle, so its 16-byte stores would land far apart in global
 // memory.  They go to shared memory instead (tile[particle][plane][TG entries], 16-byte chunks
 // XOR-swizzled by the bit-reversed particle index: conflict-free for the writes and for both read
 // patterns below) and the block then writes runs of 512 contiguous bytes:
 //   rho layout       T[block][j/4][limb 3][32 entries][j%4][re,im]            (A and B)
-//   gradient layout  Bg[j/32][q/4][plane 6: b limbs, (q br, -q bi) limbs][j%32][q%4][re,im]
+//   gradient layout  Bg[j/32][q/4][limb 3][j%32][q%4][re,im]
 struct Stager {
     double2* tile;        // [TB][planes][TG]
-    int planes;           // 3 (A, B) or 6 (B with the q-weighted copy for the gradient pass)
+    int planes;           // 3 limbs
     double* table;        // A or B
     double* Bg;           // gradient layout (or nullptr)
     long Npad, j0, N;
@@ -109,17 +109,17 @@ struct Stager {
         }
         if (Bg != nullptr) {
             // gradient layout: piece -> (j/32, q-group, plane, j%32, q%4), q%4 fastest
-            for (int piece = threadIdx.x; piece < TB * 6 * TG; piece += TB) {
+            for (int piece = threadIdx.x; piece < TB * 3 * TG; piece += TB) {
                 const int q4 = piece & 3, jl = (piece >> 2) & 31;
                 int rest = piece >> 7;
-                const int pl = rest % 6; rest /= 6;
+                const int pl = rest % 3; rest /= 3;
                 const int qg = rest & 1, jbl = rest >> 1;
                 const int row = jbl * 32 + jl, c = qg * 4 + q4;
                 const long j = j0 + row;
                 if (c < count && j < N) {
                     double2 v = tile[(row * planes + pl) * TG + (c ^ swz(row))];
                     double2* dst = reinterpret_cast<double2*>(Bg) +
-                                   ((((size_t)(j >> 5) * (Qpad / 4) + ((e0 + c) >> 2)) * 6 + pl) * 32 + jl) * 4 + q4;
+                                   ((((size_t)(j >> 5) * (Qpad / 4) + ((e0 + c) >> 2)) * 3 + pl) * 32 + jl) * 4 + q4;
                     *dst = v;
                 }
             }
@@ -128,7 +128,7 @@ struct Stager {
     }
 };
 
-// which = 0: A table.  which = 1: B table (+ gradient-layout Bg with q-weighted copy).
+// which = 0: A table.  which = 1: B table (+ the same limbs in the gradient layout Bg).
 __global__ void __launch_bounds__(TB) k_tables(
     int d, long N, double L, long Npad, int P, int Qn, int S1d, int qscale_log2,
     const int* __restrict__ pn0, const int* __restrict__ pn1, int Qpad,
@@ -146,7 +146,7 @@ __global__ void __launch_bounds__(TB) k_tables(
     const long jc = live ? j : N - 1;            // dead threads shadow the last particle (keeps barriers uniform)
     const cdd one{dd{1.0, 0.0}, dd{0.0, 0.0}};
     const bool gradB = which == 1 && with_grad != 0;
-    Stager st{tile, gradB ? 6 : 3, which == 0 ? A : B, gradB ? Bg : nullptr, Npad, j0, N, Qpad};
+    Stager st{tile, 3, which == 0 ? A : B, gradB ? Bg : nullptr, Npad, j0, N, Qpad};
     if (which == 0) {
         // ---- A table
         cdd base;
@@ -187,18 +187,10 @@ __global__ void __launch_bounds__(TB) k_tables(
         const int a = d - 1;
         cdd base = expi_turns(frac_turns(pos_hi[(size_t)a * N + jc], pos_lo[(size_t)a * N + jc], L, 1.0));
         cdd cur = one;
-        const double qs = ldexp(1.0, -qscale_log2);
         for (int q0 = 0; q0 < Qn; q0 += TG) {
             const int cnt = min(TG, Qn - q0);
             for (int s = 0; s < cnt; s++) {
-                const int q = q0 + s;
                 st.put(0, s, cur);
-                if (gradB) {
-                    cdd w;
-                    w.re = dd_scale2(dd_mul_d(cur.re, (double)q), qs);
-                    w.im = dd_neg(dd_scale2(dd_mul_d(cur.im, (double)q), qs));   // k_grad adds C1 * (-q bi)
-                    st.put(3, s, w);
-                }
                 cur = cdd_mul(cur, base);
             }
             st.flush(q0, cnt);

@@ -222,8 +222,8 @@ int build(shd_ctx* h, const double* v) {
     if (!h->v.empty()) { if ((rc = upload(h, &h->d_v, h->v))) return rc; }
     if ((rc = dalloc_zero(h, &h->d_A, (size_t)h->npb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
     if ((rc = dalloc_zero(h, &h->d_B, (size_t)h->nqb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
-    if ((rc = dalloc_zero(h, &h->d_Bg, (size_t)(2 * h->njb64) * (h->Qpad / 4) * SHD_GGROUP_DOUBLES))) return rc;
-    if ((rc = dalloc_zero(h, &h->d_C, (size_t)h->npb16 * (h->Qpad / 4) * (8 * SHD_PG * 4 * 2)))) return rc;
+    if ((rc = dalloc_zero(h, &h->d_Bg, (size_t)(2 * h->njb64) * (h->Qpad / 4) * SHD_GROUP_DOUBLES))) return rc;
+    if ((rc = dalloc_zero(h, &h->d_C, (size_t)h->npb16 * (h->Qpad / 4) * (16 * SHD_PG * 4 * 2)))) return rc;
     if ((rc = dalloc_zero(h, &h->d_gpart, (size_t)h->nseg * h->d * h->N * 2))) return rc;
     if ((rc = dalloc_zero(h, &h->d_part, (size_t)h->nsplit * h->ntiles * 4 * 1024 * 2))) return rc;
     if ((rc = dalloc_zero(h, &h->d_rho, (size_t)4 * h->M))) return rc;

@@ -101,8 +101,8 @@ struct shd_ctx {
     // device: per-evaluation data
     double *d_A = nullptr;     // [npb][Npad/4][3 limbs][32 p][4 j][2]
     double *d_B = nullptr;     // [nqb][Npad/4][3 limbs][32 q][4 j][2]
-    double *d_Bg = nullptr;    // [2 njb64][Qpad/4][6 planes: b limbs, (q br, -q bi) limbs][32 j][4 q][2]
-    double *d_C = nullptr;     // [npb16][Qpad/4][8 planes: C1 limbs + (x1+x2), C2 likewise][16 p][4 q][2]
+    double *d_Bg = nullptr;    // [2 njb64][Qpad/4][3 limbs of b][32 j][4 q][2]
+    double *d_C = nullptr;     // [npb16][Qpad/4][16 planes: C1, C2, D1 = q C2, D2 = -q C1, each limbs + (x1+x2)][16 p][4 q][2]
     double *d_gpart = nullptr; // [nseg][d][N] (hi, lo): partial gradients of the segments
     double *d_part = nullptr;  // [nsplit][ntiles][4][1024][2]
     double *d_rho = nullptr;   // [4][M]: re_hi, re_lo, im_hi, im_lo

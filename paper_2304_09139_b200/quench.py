@@ -1,7 +1,8 @@
 """Quench one BASELINE.json configuration from its seeded random start to S_max < tol.
 
     python -m paper_2304_09139_b200.quench --config cfg4 [--seed 0] [--tol 1e-30] [--max-evals 20000]
-                                           [--kind 0] [--history 10] [--chunk 500] [--out file.json]
+                                           [--kind 0|1] [--weight one|n2] [--history 10] [--chunk 500]
+                                           [--out file.json]
 
 The whole iteration runs on the device (shd_minimize); this script only calls it in chunks of
 ``--chunk`` evaluations (shd_minimize is re-entrant) to log the S_max / Phi trajectory, and
@@ -30,6 +31,11 @@ def main(argv=None):
     ap.add_argument("--history", type=int, default=10)
     ap.add_argument("--chunk", type=int, default=500)
     ap.add_argument("--poll-every", type=int, default=16)
+    ap.add_argument("--weight", default="one", choices=["one", "n2"],
+                    help="v(k): 'one' = the step potential of BASELINE.json's configs; 'n2' = 1/|n|^2 "
+                         "(P:50: any positive v has the same ground states; S_max does not depend on v; "
+                         "SURVEY.md 8(f) NEXT-1: it removes the k^2 ill-conditioning, decisive in d = 1)")
+    ap.add_argument("--fire-dt0", type=float, default=0.0)
     ap.add_argument("--out", default=None)
     ap.add_argument("--save", default=None)
     args = ap.parse_args(argv)
@@ -40,6 +46,10 @@ def main(argv=None):
     cfg = inputs.CONFIGS[args.config]
     hi, lo = inputs.uniform_positions(cfg, args.seed)
     h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    if args.weight == "n2":
+        n = h.k().astype(np.float64)
+        h.close()
+        h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star, v=1.0 / (n * n).sum(axis=1))
     pos_hi, pos_lo = shd.from_host(hi, lo)
     phi0, _, _ = h.energy_grad(pos_hi, pos_lo, want_grad=False)
     smax0, _ = h.last_smax()
@@ -51,7 +61,7 @@ def main(argv=None):
     while evals < args.max_evals:
         rep = h.minimize(pos_hi, pos_lo, kind=args.kind, history=args.history, smax_tol=args.tol,
                          max_evals=min(args.chunk, args.max_evals - evals), poll_every=args.poll_every,
-                         resume=evals > 0)
+                         resume=evals > 0, fire_dt0=args.fire_dt0)
         evals += rep["evals"]
         iters += rep["iters"]
         status = rep["status"]
@@ -65,7 +75,7 @@ def main(argv=None):
     smax, arg = h.smax(pos_hi, pos_lo)
     n = h.k()
     line = {"config": cfg.name, "d": cfg.d, "N": cfg.N, "M": cfg.M, "chi_realised": cfg.M / (cfg.d * (cfg.N - 1)),
-            "seed": args.seed, "kind": "lbfgs" if args.kind == 0 else "fire", "history": args.history,
+            "seed": args.seed, "kind": "lbfgs" if args.kind == 0 else "fire", "weight": args.weight, "history": args.history,
             "tol": args.tol, "status": status, "evals": evals, "iters": iters, "seconds": seconds,
             "ms_per_eval": 1e3 * seconds / max(evals, 1), "phi_start": phi0[0], "smax_start": smax0[0],
             "phi_final": trace[-1]["phi"], "smax_final": smax[0], "argmax_n": n[arg].tolist(), "trace": trace}
