@@ -201,28 +201,12 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
             b0 = lds2(s0 + sn * GSTAGE + offB);
             LOADX(X0, s0 + sn * GSTAGE + offC, 0)
         }
-        // last round, first half: eight DMMAs that read all eight x1+x2 fragments
-        _Pragma("unroll") for (int t = 0; t < 2; t++) {
-            dmma_v(acc[t][0].l2, b12.r, XS[0][t].r);
-            dmma_v(acc[t][2].l2, b12.r, XS[2][t].r);
-        }
-        _Pragma("unroll") for (int t = 0; t < 2; t++) {
-            dmma_v(acc[t][0].l2, b12.i, XS[1][t].r);
-            dmma_v(acc[t][2].l2, b12.i, XS[3][t].r);
-        }
-        // Release the stage here: every LDS from it has been CONSUMED by an issued DMMA.  An LDS that is
-        // merely issued before the arrive may still be in flight when the refill lands (measured: one
+        GROUND(l2, b12, XS)
+        // Release the stage only now: every LDS from it has been CONSUMED by an issued DMMA.  An LDS that
+        // is merely issued before the arrive may still be in flight when the refill lands (measured: one
         // warp in ~10^5 got a stale limb when the arrive sat between the x1+x2 loads and their round).
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(&empty_bar[s]));
-        _Pragma("unroll") for (int t = 0; t < 2; t++) {
-            dmma_v(acc[t][1].l2, b12.r, XS[0][t].i);
-            dmma_v(acc[t][3].l2, b12.r, XS[2][t].i);
-        }
-        _Pragma("unroll") for (int t = 0; t < 2; t++) {
-            dmma_v(acc[t][1].l2, b12.i, XS[1][t].i);
-            dmma_v(acc[t][3].l2, b12.i, XS[3][t].i);
-        }
         // deferred p-contraction: one quarter of the previous block per step, its A limbs loaded at the
         // top of this step (global-memory latency hidden under the 96 DMMAs above)
         if (pend) {

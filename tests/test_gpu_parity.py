@@ -13,10 +13,12 @@ from paper_2304_09139_b200 import inputs
 
 pytestmark = pytest.mark.gpu
 
-# what the arithmetic delivers: the L2 limb accumulator rounds at
-# ~1.25 n^2 2^-106 per exact burst of n = 128 products, i.e. ~2e-29 sqrt(N) per rho(k)
-RHO_TIGHT = 1.5e-28
-GRAD_TIGHT = 1e-28
+# what the arithmetic delivers: with limb widths 22/22 the third limb carries
+# everything below 2^-44 in plain FP64 and is rounded once per product and once per accumulation over a
+# burst of 512 products: ~1e-28 sqrt(N) per rho(k) measured (4x the 23/22-limb, 128-product figures the
+# first version of these bounds was set for; BASELINE.json's own tolerances are 10^2..10^5 times looser)
+RHO_TIGHT = 6e-28
+GRAD_TIGHT = 4e-28
 
 
 @pytest.fixture(scope="module")
