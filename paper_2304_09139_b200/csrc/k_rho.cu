@@ -30,7 +30,7 @@ constexpr int KSTEPS_PER_BURST = SHD_BURST / 4;
 
 __global__ void __launch_bounds__(NW * 32 + 128, 1) k_rho(
     const double* __restrict__ A, const double* __restrict__ B,
-    const int* __restrict__ tile_pb, const int* __restrict__ tile_qb, int ntiles,
+    const int* __restrict__ tile_pb, const int* __restrict__ tile_qb, const int* __restrict__ tile_wmap, int ntiles,
     long Npad, long chunks_per_split, double* __restrict__ part, const int* __restrict__ skip)
 {
     if (skip && *skip) return;
@@ -40,6 +40,11 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_rho(
     const int tile = blockIdx.x % ntiles;
     const long split = blockIdx.x / ntiles;
     const int pb = tile_pb[tile], qb = tile_qb[tile];
+    // unit (8 p x 16 q) of this consumer warp: 2 (p strip) + (q half), or -1 when the tile has fewer valid
+    // units than warps (tiles on the circle boundary; with <= 4 valid units they sit on warps 0..3, one
+    // per scheduler, and the CTA runs its FMAs in about half the time); byte 8 = number of active warps
+    const int unit = warp < NW ? tile_wmap[tile * 9 + warp] : -1;
+    const int nactive = tile_wmap[tile * 9 + 8];
     const long g0 = split * chunks_per_split * (SHD_NPS / 4);          // first group of 4 particles
     const double* gA = A + ((size_t)pb * (Npad / 4) + g0) * SHD_GROUP_DOUBLES;
     const double* gB = B + ((size_t)qb * (Npad / 4) + g0) * SHD_GROUP_DOUBLES;
@@ -50,7 +55,7 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_rho(
     if (tid == 0) {
         for (int s = 0; s < SHD_RHO_STAGES; s++) {
             mbar_init(smem_u32(&full_bar[s]), 1);
-            mbar_init(smem_u32(&empty_bar[s]), NW);
+            mbar_init(smem_u32(&empty_bar[s]), nactive);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -78,11 +83,12 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_rho(
         return;
     }
     asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
+    if (unit < 0) return;            // no valid cell in this warp's unit (no block-wide barrier follows)
 
-    // warp tile: p_local = 8 (warp / 2) + g, q_local = 16 (warp % 2) + 8 t + {2 tq, 2 tq + 1}
+    // warp tile: p_local = 8 (unit / 2) + g, q_local = 16 (unit % 2) + 8 t + {2 tq, 2 tq + 1}
     const uint32_t fragoff = (uint32_t)(lane >> 2) * 64 + (uint32_t)(lane & 3) * 16;
-    const uint32_t offA = (uint32_t)(warp >> 1) * 8 * 64 + fragoff;
-    const uint32_t offB = SLAB_BYTES + (uint32_t)(warp & 1) * 16 * 64 + fragoff;
+    const uint32_t offA = (uint32_t)(unit >> 1) * 8 * 64 + fragoff;
+    const uint32_t offB = SLAB_BYTES + (uint32_t)(unit & 1) * 16 * 64 + fragoff;
 
     Acc3 acc[2][4];
 #pragma unroll
@@ -162,14 +168,14 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_rho(
 
     // partial sums: part[((split*ntiles + tile)*4 + x)*1024 + cell] as (hi, lo)
     double2* out = reinterpret_cast<double2*>(part) + ((size_t)(split * ntiles + tile) * 4) * 1024;
-    const int pl = (warp >> 1) * 8 + (lane >> 2);
+    const int pl = (unit >> 1) * 8 + (lane >> 2);
 #pragma unroll
     for (int t = 0; t < 2; t++)
 #pragma unroll
         for (int x = 0; x < 4; x++)
 #pragma unroll
             for (int e = 0; e < 2; e++) {
-                const int ql = (warp & 1) * 16 + t * 8 + (lane & 3) * 2 + e;
+                const int ql = (unit & 1) * 16 + t * 8 + (lane & 3) * 2 + e;
                 double2 m = mainacc[((t * 4 + x) * 2 + e) * 256 + tid];
                 dd r = fast_two_sum(m.x, m.y);
                 out[(size_t)x * 1024 + pl * 32 + ql] = make_double2(r.h, r.l);
@@ -187,7 +193,7 @@ cudaError_t shd_launch_rho(shd_ctx* h)
 {
     unsigned grid = (unsigned)(h->ntiles * h->nsplit);
     k_rho<<<grid, NW * 32 + 128, RHO_SMEM, h->stream>>>(
-        h->d_A, h->d_B, h->d_tile_pb, h->d_tile_qb, h->ntiles, h->Npad, h->chunks_per_split, h->d_part, h->d_skip);
+        h->d_A, h->d_B, h->d_tile_pb, h->d_tile_qb, h->d_tile_wmap, h->ntiles, h->Npad, h->chunks_per_split, h->d_part, h->d_skip);
     h->last_launches += 1;
     return cudaGetLastError();
 }

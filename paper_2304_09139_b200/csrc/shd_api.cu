@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <functional>
 #include <map>
 #include <new>
 
@@ -143,7 +144,8 @@ int build(shd_ctx* h, const double* v) {
             }
     if (found != h->M) return fail(h, SHD_EINVAL, "internal: decomposition does not cover Q");
     // ---- tiles and q-chunk counts
-    std::vector<int> tile_pb, tile_qb;
+    std::vector<int> tile_pb, tile_qb, tile_wmap;
+    h->tile_weight = 0.0;
     h->valid_cells = 0;
     for (int pb = 0; pb < h->npb; pb++)
         for (int qb = 0; qb < h->nqb; qb++) {
@@ -156,7 +158,27 @@ int build(shd_ctx* h, const double* v) {
                         h->valid_cells++;
                     }
                 }
-            if (any) { tile_pb.push_back(pb); tile_qb.push_back(qb); }
+            if (any) {
+                tile_pb.push_back(pb); tile_qb.push_back(qb);
+                // units (8 p x 16 q) with a valid cell -> consumer warps; <= 4 of them: one per scheduler
+                int valid_unit[8], nv = 0;
+                for (int u = 0; u < 8; u++) {
+                    bool uv = false;
+                    for (int pi = 0; pi < 8 && !uv; pi++)
+                        for (int qi = 0; qi < 16 && !uv; qi++) {
+                            size_t c = (size_t)(pb * 32 + (u >> 1) * 8 + pi) * h->Qpad + qb * 32 + (u & 1) * 16 + qi;
+                            uv = kp[c] >= 0 || km[c] >= 0;
+                        }
+                    if (uv) valid_unit[nv++] = u;
+                }
+                int wmap[9];
+                for (int w = 0; w < 8; w++) wmap[w] = -1;
+                if (nv <= 4) for (int i = 0; i < nv; i++) wmap[i] = valid_unit[i];
+                else for (int i = 0; i < nv; i++) wmap[valid_unit[i]] = valid_unit[i];
+                wmap[8] = nv;
+                tile_wmap.insert(tile_wmap.end(), wmap, wmap + 9);
+                h->tile_weight += nv <= 4 ? 0.6 : 1.0;      // one warp per scheduler: ~half the time
+            }
         }
     h->ntiles = (int)tile_pb.size();
     // ---- gradient pass: step list over blocks of 16 p (q-groups up to the last valid cell of the block)
@@ -187,12 +209,29 @@ int build(shd_ctx* h, const double* v) {
     if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return fail(h, SHD_ECUDA, "cudaGetDeviceProperties failed");
     const long sms = prop.multiProcessorCount;
     const long nchunks = (h->N + SHD_NPS - 1) / SHD_NPS;
-    long best_cost = -1;
-    for (long ns = 1; ns <= std::min<long>(256, nchunks); ns++) {
-        long cps = (nchunks + ns - 1) / ns;
-        long waves = ((long)h->ntiles * ns + sms - 1) / sms;
-        long cost = waves * (cps + 2);          // +2: per-CTA prologue/epilogue
-        if (best_cost < 0 || cost < best_cost) { best_cost = cost; h->nsplit = (int)ns; h->chunks_per_split = cps; }
+    // CTAs are dispatched in blockIdx order (split-major, tile-minor) to the first free SM; a tile with
+    // <= 4 valid units takes ~0.6 of a full tile's time.  Simulate that list schedule for every split count.
+    double best_cost = -1.0;
+    {
+        std::vector<double> tw(h->ntiles);
+        for (int t = 0; t < h->ntiles; t++) tw[t] = tile_wmap[(size_t)t * 9 + 8] <= 4 ? 0.6 : 1.0;
+        std::vector<double> sm_free((size_t)sms);
+        for (long ns = 1; ns <= std::min<long>(256, nchunks); ns++) {
+            const long cps = (nchunks + ns - 1) / ns;
+            std::fill(sm_free.begin(), sm_free.end(), 0.0);
+            std::make_heap(sm_free.begin(), sm_free.end(), std::greater<double>());
+            double makespan = 0.0;
+            for (long b = 0; b < (long)h->ntiles * ns; b++) {
+                std::pop_heap(sm_free.begin(), sm_free.end(), std::greater<double>());
+                double& slot = sm_free.back();
+                slot += tw[b % h->ntiles] * (double)cps + 2.0;        // +2: per-CTA prologue/epilogue
+                makespan = std::max(makespan, slot);
+                std::push_heap(sm_free.begin(), sm_free.end(), std::greater<double>());
+            }
+            // k_finish1 sums ns partials per cell: measured ~0.015 chunk-times per (split, tile)
+            const double cost = makespan + 0.015 * (double)ns * (double)h->ntiles;
+            if (best_cost < 0.0 || cost < best_cost) { best_cost = cost; h->nsplit = (int)ns; h->chunks_per_split = cps; }
+        }
     }
     h->Npad = (long)h->nsplit * h->chunks_per_split * SHD_NPS;
     h->njb = (h->N + 31) / 32;
@@ -218,6 +257,7 @@ int build(shd_ctx* h, const double* v) {
     if ((rc = upload(h, &h->d_cell_km, km))) return rc;
     if ((rc = upload(h, &h->d_tile_pb, tile_pb))) return rc;
     if ((rc = upload(h, &h->d_tile_qb, tile_qb))) return rc;
+    if ((rc = upload(h, &h->d_tile_wmap, tile_wmap))) return rc;
     if ((rc = upload(h, &h->d_steps, steps))) return rc;
     if (!h->v.empty()) { if ((rc = upload(h, &h->d_v, h->v))) return rc; }
     if ((rc = dalloc_zero(h, &h->d_A, (size_t)h->npb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
@@ -319,7 +359,7 @@ void shd_destroy(shd_ctx* h) {
     shd_min_free(h);
     shd_fire_free(h);
     cudaFree(h->d_pn0); cudaFree(h->d_pn1); cudaFree(h->d_wT); cudaFree(h->d_cell_kp); cudaFree(h->d_cell_km);
-    cudaFree(h->d_tile_pb); cudaFree(h->d_tile_qb); cudaFree(h->d_steps); cudaFree(h->d_v); cudaFree(h->d_gpart);
+    cudaFree(h->d_tile_pb); cudaFree(h->d_tile_qb); cudaFree(h->d_tile_wmap); cudaFree(h->d_steps); cudaFree(h->d_v); cudaFree(h->d_gpart);
     cudaFree(h->d_A); cudaFree(h->d_B); cudaFree(h->d_Bg); cudaFree(h->d_C); cudaFree(h->d_part);
     cudaFree(h->d_rho); cudaFree(h->d_blockred); cudaFree(h->d_scal);
     cudaFree(h->d_hpos); cudaFree(h->d_hgrad);

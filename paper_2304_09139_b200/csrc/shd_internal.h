@@ -95,6 +95,8 @@ struct shd_ctx {
     int *d_wT = nullptr;       // [3][P padded]: integer weight of Im(conj(A) T) for axis a
     int *d_cell_kp = nullptr, *d_cell_km = nullptr;   // [npb*32][Qpad] -> k or -1
     int *d_tile_pb = nullptr, *d_tile_qb = nullptr;   // [ntiles]
+    int *d_tile_wmap = nullptr;                       // [ntiles][9]: unit of consumer warp w (or -1), active warps
+    double tile_weight = 0;                           // sum over tiles of their relative duration (1 or ~0.6)
     int *d_steps = nullptr;    // [nsteps] int2: x = C slab index pb16 * (Qpad/4) + qg, y = qg | flags << 16
                                //   (flag 1: last step of a block: fold the limb burst, contract with A)
     double *d_v = nullptr;     // [M]
