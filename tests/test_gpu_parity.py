@@ -88,6 +88,9 @@ def test_cfg1_full(shd, oracle):
     (1, 37, 37.0, 20 * 20, 3), (1, 300, 300.0, 700 * 700, 4),         # d = 1, several p-blocks
     (2, 33, 5.7, 2, 5), (2, 500, 22.0, 1300, 6),                      # ragged N, 2x2 tiles
     (3, 130, 5.1, 50, 7), (3, 64, 4.0, 321, 8),                       # d = 3
+    (2, 63, 8.0, 15 * 15, 9), (2, 65, 8.0, 16 * 16, 10), (2, 129, 11.0, 17 * 17, 11),   # ragged 64-particle blocks, P = 16, 17, 18
+    (2, 96, 300.0, 265 * 265, 12),                                    # q-range > 256: gradient blocks cut after 64 steps
+    (1, 50, 50.0, 1100 * 1100, 13),                                   # d = 1, Qn > 256 as well
 ])
 def test_small_cases(shd, oracle, d, N, L, m_star, seed):
     hi, lo = inputs.uniform_positions_raw(d, N, L, seed)
