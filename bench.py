@@ -125,7 +125,9 @@ def run_reference(args, cfg):
 
 
 def workload_config(cfg, world):
-    return {"workload": f"BASELINE.json configs[{int(cfg.name[3:]) - 1}]: d={cfg.d}, N={cfg.N}, unit density, "
+    src = f"BASELINE.json configs[{int(cfg.name[3:]) - 1}]" if cfg.name.startswith("cfg") else \
+        "the paper's system size (P:33, P:89; not a BASELINE.json config)"
+    return {"workload": f"{src}: d={cfg.d}, N={cfg.N}, unit density, "
                         f"chi={cfg.chi} (m*={cfg.m_star}, |Q|={cfg.M}), v=1, uniform seeded positions",
             "d": cfg.d, "N": cfg.N, "M": cfg.M, "pair_terms_per_eval": cfg.pairs,
             "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (seed = rank)",

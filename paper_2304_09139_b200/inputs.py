@@ -46,6 +46,9 @@ CONFIGS = {
     "cfg3": Config("cfg3", 3, 10_000, float.fromhex("0x1.58b5a51868c62p+4"), 0.40, 321, 12055),
     "cfg4": Config("cfg4", 2, 100_000, float.fromhex("0x1.3c3a4edfa9759p+8"), 0.45, 57290, 90000),
     "cfg5": Config("cfg5", 1, 200_000, 200000.0, 0.30, 60000 * 60000, 60000),
+    # the paper's own system size (d = 2, N = 2 x 10^6) at its smallest chi; context, not a
+    # BASELINE.json config: one evaluation is 8 x 10^11 pair-terms and needs ~150 GB of phasor tables
+    "paper01": Config("paper01", 2, 2_000_000, float.fromhex("0x1.618dab0184066p+10"), 0.10, 254626, 399996),
 }
 
 
