@@ -183,3 +183,25 @@ def test_fire_resume_is_a_continuation(shd):
     h.minimize(c_hi, c_lo, kind=1, max_evals=31, poll_every=4)            # fresh start from rest
     assert not torch.equal(a_hi, c_hi)
     h.close()
+
+
+@pytest.mark.parametrize("name,floor", [("cfg1", 1e-50), ("cfg2", 1e-48)])
+def test_quench_to_the_precision_floor(shd, oracle, name, floor):
+    """the paper quenches "until Phi is at the minimum value attainable within machine precision" and
+    reports S_max ~ 1e-51 (Fig. 2a).  With smax_tol = 0 the device L-BFGS runs until its line search
+    finds no further decrease (SHD_ESTALL); the ORACLE's S_max on the final positions must then be at the
+    double-double floor, twenty orders of magnitude below BASELINE.json's 1e-30 target."""
+    cfg = inputs.CONFIGS[name]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    th, tl = shd.from_host(hi, lo)
+    rep = h.minimize(th, tl, smax_tol=0.0, max_evals=20000, poll_every=32)
+    assert rep["status"] == shd.SHD_ESTALL, rep
+    n = oracle.enumerate_Q(cfg.d, cfg.m_star)
+    re, im = oracle.rho(cfg.d, cfg.N, cfg.L, th.cpu().numpy(), tl.cpu().numpy(), n, mode="factored")
+    _, smax, _, _ = oracle.energy(cfg.N, re, im)
+    s_or = oracle.to_float(smax)[0]
+    print(name, rep, "oracle S_max", s_or)
+    assert s_or < floor
+    assert rep["smax"][0] < floor
+    h.close()
