@@ -98,6 +98,16 @@ int shd_last_smax(shd_ctx* h, double smax[2], long* argmax_k);
 int shd_get_rho(shd_ctx* h, double* re_hi, double* re_lo, double* im_hi, double* im_lo);
 
 /*
+ * "Tunable precision".  limbs = 3 (default): the products of the two O(N M) sums carry ~98 bits
+ * (double-double results; BASELINE.json's tolerances).  limbs = 2: "fast" evaluations for the early part of a
+ * quench (precision ladder): the phasor and rho operands are used at 44 bits
+ * (two exact limbs), half the FMAs; per-term error ~2^-45, i.e. |rho| to ~3e-14 sqrt(N), enough to drive
+ * S_max to ~1e-22; everything else (phasor tables, reductions, minimizer algebra) stays double-double.
+ * Applies to every later call on the handle.  Errors: SHD_EINVAL (limbs not 2 or 3).
+ */
+int shd_set_precision(shd_ctx* h, int limbs);
+
+/*
  * Structure factor of the LAST evaluation on this handle (Eq. 3): S(k) = |rho(k)|^2 / N for every k
  * of the handle's Q, canonical order, into S_out (DEVICE, |Q| doubles; may be NULL), and
  * dev2 (HOST, (hi, lo)) = sum_{k in Q} (S(k) - 1)^2 in double-double, the lattice sum behind the order
@@ -115,7 +125,7 @@ typedef struct {
     long   max_evals;   /* stop after this many energy+gradient evaluations                   */
     int    poll_every;  /* host reads the device status word every this many iterations (>=1) */
     double fire_dt0;    /* FIRE only: initial time step (dt_max = 10 dt0); 0 = default
-                           0.05 / (k_max sqrt(2 N max v)), a quarter of the explicit stability bound */
+                           0.1 / (k_max sqrt(2 N max v)): dt_max is half the explicit stability bound */
     int    resume;      /* FIRE only: 1 = continue the previous call on this handle (same positions
                            buffer content as it left): keep velocities, dt, alpha; 0 = fresh start    */
 } shd_min_opts;

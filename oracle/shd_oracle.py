@@ -258,10 +258,10 @@ def minimize_lbfgs(d, N, L, pos_hi, pos_lo, n, v=None, mode="direct", history=10
 def fire_dt0(d, N, L, n) -> float:
     """Default FIRE time step: the stiffest collective mode of Phi = sum |rho|^2 has
     curvature ~ 2 N k_max^2 (unit masses), so explicit integration is stable for dt < 2 / (k_max sqrt(2N));
-    dt_max = 10 dt0 is put at a quarter of that bound."""
+    dt_max = 10 dt0 is put at half of that bound."""
     n = np.asarray(n).reshape(-1, d)
     kmax = 2.0 * np.pi * np.sqrt(float((n.astype(np.int64) ** 2).sum(axis=1).max())) / float(L)
-    return 0.05 / (kmax * np.sqrt(2.0 * N))
+    return 0.1 / (kmax * np.sqrt(2.0 * N))
 
 
 def minimize_fire(d, N, L, pos_hi, pos_lo, n, v=None, mode="direct", dt0=None,

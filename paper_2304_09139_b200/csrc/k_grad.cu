@@ -63,6 +63,8 @@ __device__ __forceinline__ dd limbs_to_dd(double x0, double x1, double x2) {
     _Pragma("unroll") for (int o = 0; o < 4; o++)                           \
         _Pragma("unroll") for (int t = 0; t < 2; t++) X[o][t] = lds2((base) + t * 512 + (o * 4 + (L)) * PLANE_C);
 
+// FULL = false: the two-limb "fast" precision of shd_set_precision(h, 2) (see k_rho.cu)
+template <bool FULL>
 __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
     int d, long N, long Npad, long njb64, int Qpad, int Ppad, int qscale_log2,
     const int2* __restrict__ steps, int nsteps, int nseg, const int* __restrict__ wT,
@@ -87,11 +89,7 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp < NW) {
-#pragma unroll
-        for (int a = 0; a < 16; a++) mainacc[a * 256 + tid] = make_double2(0.0, 0.0);
-    }
-    __syncthreads();
+    __syncthreads();        // (the T slots behind the ring need no initialisation: written before read)
 
     if (warp >= NW) {
         // producer warpgroup: hands its registers to the consumers (setmaxnreg), then one lane streams.
@@ -182,26 +180,46 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
         const uint32_t pB = s0 + s * GSTAGE + offB, pC = s0 + s * GSTAGE + offC;
         const int2 st = steps[c_begin + c];
         if (pend) load_quarter(pk, ppb, pa0, pa1, pa2);
-        const F2 b1 = lds2(pB + 1 * PLANE_B), b2 = lds2(pB + 2 * PLANE_B);
+        const F2 b1 = lds2(pB + 1 * PLANE_B);
+        F2 b2{0.0, 0.0}, b12{0.0, 0.0};
+        if (FULL) b2 = lds2(pB + 2 * PLANE_B);
         GROUND(l0, b0, X0)
         F2 X1[4][2];
         LOADX(X1, pC, 1)
         GROUND(l1, b1, X0)
-        F2 X2[4][2];
-        LOADX(X2, pC, 2)
-        GROUND(l2, b2, X0)
-        const F2 b12 = add2(b1, b2);
-        GROUND(l1, b0, X1)
-        F2 XS[4][2];                             // x1 + x2 of the shared operands comes from the table (k_ctable)
-        LOADX(XS, pC, 3)
-        GROUND(l2, b0, X2)
-        if (c + 1 < total) {
-            const int sn = (c + 1) % NST;
-            mbar_wait(smem_u32(&full_bar[sn]), (uint32_t)(((c + 1) / NST) & 1));
-            b0 = lds2(s0 + sn * GSTAGE + offB);
-            LOADX(X0, s0 + sn * GSTAGE + offC, 0)
+        if (FULL) {
+            F2 X2[4][2];
+            LOADX(X2, pC, 2)
+            GROUND(l2, b2, X0)
+            b12 = add2(b1, b2);
+            GROUND(l1, b0, X1)
+            F2 XS[4][2];                         // x1 + x2 of the shared operands comes from the table (k_ctable)
+            LOADX(XS, pC, 3)
+            GROUND(l2, b0, X2)
+            if (c + 1 < total) {
+                const int sn = (c + 1) % NST;
+                mbar_wait(smem_u32(&full_bar[sn]), (uint32_t)(((c + 1) / NST) & 1));
+                b0 = lds2(s0 + sn * GSTAGE + offB);
+                LOADX(X0, s0 + sn * GSTAGE + offC, 0)
+            }
+            GROUND(l2, b12, XS)
+        } else {
+            F2 b0n = b0, X0n[4][2];
+            if (c + 1 < total) {
+                const int sn = (c + 1) % NST;
+                mbar_wait(smem_u32(&full_bar[sn]), (uint32_t)(((c + 1) / NST) & 1));
+                b0n = lds2(s0 + sn * GSTAGE + offB);
+                LOADX(X0n, s0 + sn * GSTAGE + offC, 0)
+            }
+            GROUND(l1, b0, X1)
+            b0 = b0n;
+            if (c + 1 < total) {
+#pragma unroll
+                for (int o = 0; o < 4; o++)
+#pragma unroll
+                    for (int t = 0; t < 2; t++) X0[o][t] = X0n[o][t];
+            }
         }
-        GROUND(l2, b12, XS)
         // Release the stage only now: every LDS from it has been CONSUMED by an issued DMMA.  An LDS that
         // is merely issued before the arrive may still be in flight when the refill lands (measured: one
         // warp in ~10^5 got a stale limb when the arrive sat between the x1+x2 loads and their round).
@@ -237,10 +255,16 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
             pend = true; pk = 0; ppb = st.x / (Qpad / 4);
         }
     }
-    while (pend) {
-        load_quarter(pk, ppb, pa0, pa1, pa2);
-        contract_quarter(pk, ppb, pa0, pa1, pa2);
-        if (++pk == 4) pend = false;
+    if (pend) {
+        // the last block of the segment: all remaining quarters' A limbs in flight at once
+        double2 qa[4][3];
+#pragma unroll
+        for (int k = 0; k < 4; k++)
+            if (k >= pk) load_quarter(k, ppb, qa[k][0], qa[k][1], qa[k][2]);
+#pragma unroll
+        for (int k = 0; k < 4; k++)
+            if (k >= pk) contract_quarter(k, ppb, qa[k][0], qa[k][1], qa[k][2]);
+        pend = false;
     }
 
     // reduce over the 4 threads that share a particle: gred[a][j_local 64][tq 4]
@@ -289,15 +313,23 @@ __global__ void __launch_bounds__(256) k_gradsum(
 
 cudaError_t shd_grad_configure()
 {
-    return cudaFuncSetAttribute(k_grad, cudaFuncAttributeMaxDynamicSharedMemorySize, GSMEM);
+    cudaError_t e = cudaFuncSetAttribute(k_grad<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GSMEM);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_grad<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GSMEM);
 }
 
 cudaError_t shd_launch_grad(shd_ctx* h, double* grad_hi, double* grad_lo)
 {
-    k_grad<<<(unsigned)(h->njb64 * h->nseg), NW * 32 + 128, GSMEM, h->stream>>>(
-        h->d, h->N, h->Npad, h->njb64, h->Qpad, h->npb * 32, h->qscale_log2,
-        reinterpret_cast<const int2*>(h->d_steps), h->nsteps, h->nseg, h->d_wT,
-        h->d_A, h->d_Bg, h->d_C, h->d_gpart, h->d_skip);
+    if (h->nlimb >= 3)
+        k_grad<true><<<(unsigned)(h->njb64 * h->nseg), NW * 32 + 128, GSMEM, h->stream>>>(
+            h->d, h->N, h->Npad, h->njb64, h->Qpad, h->npb * 32, h->qscale_log2,
+            reinterpret_cast<const int2*>(h->d_steps), h->nsteps, h->nseg, h->d_wT,
+            h->d_A, h->d_Bg, h->d_C, h->d_gpart, h->d_skip);
+    else
+        k_grad<false><<<(unsigned)(h->njb64 * h->nseg), NW * 32 + 128, GSMEM, h->stream>>>(
+            h->d, h->N, h->Npad, h->njb64, h->Qpad, h->npb * 32, h->qscale_log2,
+            reinterpret_cast<const int2*>(h->d_steps), h->nsteps, h->nseg, h->d_wT,
+            h->d_A, h->d_Bg, h->d_C, h->d_gpart, h->d_skip);
     const long n = (long)h->d * h->N;
     k_gradsum<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(
         n, h->nseg, h->L, h->d_gpart, h->d_scal, grad_hi, grad_lo, h->d_skip);

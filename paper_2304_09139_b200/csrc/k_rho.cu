@@ -28,6 +28,10 @@ constexpr int MAIN_BYTES = 16 * 256 * 16;                    // 16 dd sums per t
 constexpr int RHO_SMEM = RING_BYTES + MAIN_BYTES;
 constexpr int KSTEPS_PER_BURST = SHD_BURST / 4;
 
+// FULL = true: three limbs (double-double accuracy).  FULL = false: the "fast" precision of
+// shd_set_precision(h, 2): limbs x0, x1 only (L0 and L1, both exact), i.e. operands rounded to 44 bits,
+// half the FMAs; error ~2^-45 per term instead of ~2^-98 ("tunable precision").
+template <bool FULL>
 __global__ void __launch_bounds__(NW * 32 + 128, 1) k_rho(
     const double* __restrict__ A, const double* __restrict__ B,
     const int* __restrict__ tile_pb, const int* __restrict__ tile_qb, const int* __restrict__ tile_wmap, int ntiles,
@@ -119,26 +123,32 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_rho(
         const int c = k / GPS, g = k % GPS, s = c % SHD_RHO_STAGES;
         const uint32_t pA = s0 + s * STAGE_BYTES + g * GROUP_BYTES + offA;
         const uint32_t pB = s0 + s * STAGE_BYTES + g * GROUP_BYTES + offB;
-        const F2 a1 = lds2(pA + PLANE_BYTES), a2 = lds2(pA + 2 * PLANE_BYTES);
+        const F2 a1 = lds2(pA + PLANE_BYTES);
+        F2 a2{0.0, 0.0}, a12{0.0, 0.0};
+        if (FULL) a2 = lds2(pA + 2 * PLANE_BYTES);
         ROUND(l0, a0, b0)
-        F2 b1[2], b2[2];
+        F2 b1[2], b2[2] = {{0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll
         for (int t = 0; t < 2; t++) b1[t] = lds2(pB + t * 8 * 64 + PLANE_BYTES);
         ROUND(l1, a1, b0)
+        if (FULL) {
 #pragma unroll
-        for (int t = 0; t < 2; t++) b2[t] = lds2(pB + t * 8 * 64 + 2 * PLANE_BYTES);
-        ROUND(l2, a2, b0)
-        const F2 a12 = add2(a1, a2);
+            for (int t = 0; t < 2; t++) b2[t] = lds2(pB + t * 8 * 64 + 2 * PLANE_BYTES);
+            ROUND(l2, a2, b0)
+            a12 = add2(a1, a2);
+        }
         ROUND(l1, a0, b1)
-        ROUND(l2, a0, b2)
+        if (FULL) { ROUND(l2, a0, b2) }
         if (g == GPS - 1) {
             // every LDS of stage s has been consumed by an issued DMMA: release the stage
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(&empty_bar[s]));
         }
-        F2 bs[2];
+        F2 bs[2] = {{0.0, 0.0}, {0.0, 0.0}};
+        if (FULL) {
 #pragma unroll
-        for (int t = 0; t < 2; t++) bs[t] = add2(b1[t], b2[t]);
+            for (int t = 0; t < 2; t++) bs[t] = add2(b1[t], b2[t]);
+        }
         if (k + 1 < nk) {
             const int cn = (k + 1) / GPS, gn = (k + 1) % GPS, sn = cn % SHD_RHO_STAGES;
             if (gn == 0) mbar_wait(smem_u32(&full_bar[sn]), (uint32_t)((cn / SHD_RHO_STAGES) & 1));
@@ -147,7 +157,7 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_rho(
 #pragma unroll
             for (int t = 0; t < 2; t++) b0[t] = lds2(nb + offB + t * 8 * 64);
         }
-        ROUND(l2, a12, bs)
+        if (FULL) { ROUND(l2, a12, bs) }
         if ((k + 1) % KSTEPS_PER_BURST == 0 || k == nk - 1) {
 #pragma unroll
             for (int t = 0; t < 2; t++)
@@ -186,14 +196,20 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_rho(
 
 cudaError_t shd_rho_configure()
 {
-    return cudaFuncSetAttribute(k_rho, cudaFuncAttributeMaxDynamicSharedMemorySize, RHO_SMEM);
+    cudaError_t e = cudaFuncSetAttribute(k_rho<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHO_SMEM);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_rho<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHO_SMEM);
 }
 
 cudaError_t shd_launch_rho(shd_ctx* h)
 {
     unsigned grid = (unsigned)(h->ntiles * h->nsplit);
-    k_rho<<<grid, NW * 32 + 128, RHO_SMEM, h->stream>>>(
-        h->d_A, h->d_B, h->d_tile_pb, h->d_tile_qb, h->d_tile_wmap, h->ntiles, h->Npad, h->chunks_per_split, h->d_part, h->d_skip);
+    if (h->nlimb >= 3)
+        k_rho<true><<<grid, NW * 32 + 128, RHO_SMEM, h->stream>>>(
+            h->d_A, h->d_B, h->d_tile_pb, h->d_tile_qb, h->d_tile_wmap, h->ntiles, h->Npad, h->chunks_per_split, h->d_part, h->d_skip);
+    else
+        k_rho<false><<<grid, NW * 32 + 128, RHO_SMEM, h->stream>>>(
+            h->d_A, h->d_B, h->d_tile_pb, h->d_tile_qb, h->d_tile_wmap, h->ntiles, h->Npad, h->chunks_per_split, h->d_part, h->d_skip);
     h->last_launches += 1;
     return cudaGetLastError();
 }

@@ -473,6 +473,13 @@ int shd_get_rho(shd_ctx* h, double* re_hi, double* re_lo, double* im_hi, double*
     return SHD_OK;
 }
 
+int shd_set_precision(shd_ctx* h, int limbs) {
+    if (!h) return SHD_EINVAL;
+    if (limbs != 2 && limbs != 3) return fail(h, SHD_EINVAL, "shd_set_precision: limbs must be 2 or 3");
+    h->nlimb = limbs;
+    return SHD_OK;
+}
+
 int shd_structure_factor(shd_ctx* h, double* S_out, double dev2[2]) {
     if (!h) return SHD_EINVAL;
     if (!dev2) return fail(h, SHD_EINVAL, "NULL pointer");
@@ -493,7 +500,7 @@ double shd_stat(const shd_ctx* h, int what) {
     if (!h) return 0.0;
     const double cells_rho = (double)h->ntiles * 1024.0;
     switch (what) {
-        case 0: return cells_rho * (double)h->Npad * 24.0;     // DFMAs launched by the rho pass (padded)
+        case 0: return cells_rho * (double)h->Npad * 24.0;     // DFMAs launched by the rho pass (padded, 3 limbs)
         case 12: return (double)h->njb64 * SHD_JT * (double)h->grad_qsteps * SHD_PG * 48.0;   // ... by the gradient pass
         case 1: return (double)h->last_launches;
         case 2: return cells_rho;

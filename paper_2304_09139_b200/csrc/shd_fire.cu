@@ -208,11 +208,11 @@ int shd_fire_run(shd_ctx* h, double* pos_hi, double* pos_lo, const shd_min_opts*
     const long n = s->n;
     cudaStream_t st = h->stream;
     // default time step: the stiffest collective mode of Phi = sum v |rho|^2 has curvature ~ 2 N v k_max^2,
-    // explicit integration is stable for dt < 2 / (k_max sqrt(2 N v)); dt_max = 10 dt0 sits at a quarter of it
+    // explicit integration is stable for dt < 2 / (k_max sqrt(2 N v)); dt_max = 10 dt0 sits at half of it
     double vmax = 1.0;
     for (double x : h->v) vmax = x > vmax ? x : vmax;
     const double kmax = 2.0 * 3.14159265358979323846 * std::sqrt((double)h->m_star) / h->L;
-    const double dt0 = opts->fire_dt0 > 0.0 ? opts->fire_dt0 : 0.05 / (kmax * std::sqrt(2.0 * (double)h->N * vmax));
+    const double dt0 = opts->fire_dt0 > 0.0 ? opts->fire_dt0 : 0.1 / (kmax * std::sqrt(2.0 * (double)h->N * vmax));
     shd_firectrl* c = s->h_ctrl;
     if (cont) {                        // explicit re-entry: keep velocities, dt, alpha, counters
         const shd_firectrl keep = *c;

@@ -70,6 +70,7 @@ struct shd_ctx {
     double L = 0;
     long m_star = 0;
     long M = 0;
+    int nlimb = 3;             // 3: double-double products; 2: "fast" 44-bit operands (shd_set_precision)
     // decomposition
     int P = 0, Qn = 0, npb = 0, nqb = 0;
     int S1d = 0;               // d == 1: n = S1d * p + sigma q

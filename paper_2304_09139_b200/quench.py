@@ -36,6 +36,9 @@ def main(argv=None):
                          "(P:50: any positive v has the same ground states; S_max does not depend on v; "
                          "SURVEY.md 8(f) NEXT-1: it removes the k^2 ill-conditioning, decisive in d = 1)")
     ap.add_argument("--fire-dt0", type=float, default=0.0)
+    ap.add_argument("--ladder", type=float, default=0.0,
+                    help="precision ladder (P:77 'tunable precision'; SURVEY.md 8(f) NEXT-1): evaluate with two "
+                         "limbs (shd_set_precision 2) until S_max < this value, e.g. 1e-18, then with three")
     ap.add_argument("--out", default=None)
     ap.add_argument("--save", default=None)
     args = ap.parse_args(argv)
@@ -58,8 +61,12 @@ def main(argv=None):
     status = shd.SHD_EMAXEVAL
     torch.cuda.synchronize()
     t0 = time.perf_counter()
+    fast = args.ladder > args.tol
+    if fast:
+        h.set_precision(2)
     while evals < args.max_evals:
-        rep = h.minimize(pos_hi, pos_lo, kind=args.kind, history=args.history, smax_tol=args.tol,
+        rep = h.minimize(pos_hi, pos_lo, kind=args.kind, history=args.history,
+                         smax_tol=args.ladder if fast else args.tol,
                          max_evals=min(args.chunk, args.max_evals - evals), poll_every=args.poll_every,
                          resume=evals > 0, fire_dt0=args.fire_dt0)
         evals += rep["evals"]
@@ -69,6 +76,12 @@ def main(argv=None):
                       "seconds": time.perf_counter() - t0})
         print(f"[quench {cfg.name}] evals={evals} iters={iters} Phi={rep['phi'][0]:.6e} "
               f"S_max={rep['smax'][0]:.6e} t={trace[-1]['seconds']:.1f}s", file=sys.stderr, flush=True)
+        if fast and status in (shd.SHD_OK, shd.SHD_ESTALL):
+            fast = False                      # second rung: double-double evaluations from here on
+            h.set_precision(3)
+            trace[-1]["switched_to_3_limbs"] = True
+            status = shd.SHD_EMAXEVAL
+            continue
         if status != shd.SHD_EMAXEVAL:
             break
     seconds = time.perf_counter() - t0
@@ -76,7 +89,7 @@ def main(argv=None):
     n = h.k()
     line = {"config": cfg.name, "d": cfg.d, "N": cfg.N, "M": cfg.M, "chi_realised": cfg.M / (cfg.d * (cfg.N - 1)),
             "seed": args.seed, "kind": "lbfgs" if args.kind == 0 else "fire", "weight": args.weight, "history": args.history,
-            "tol": args.tol, "status": status, "evals": evals, "iters": iters, "seconds": seconds,
+            "tol": args.tol, "ladder": args.ladder, "status": status, "evals": evals, "iters": iters, "seconds": seconds,
             "ms_per_eval": 1e3 * seconds / max(evals, 1), "phi_start": phi0[0], "smax_start": smax0[0],
             "phi_final": trace[-1]["phi"], "smax_final": smax[0], "argmax_n": n[arg].tolist(), "trace": trace}
     if args.save:

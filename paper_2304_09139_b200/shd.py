@@ -17,7 +17,7 @@ LIB_PATH = _HERE / "libshd.so"
 SHD_OK, SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA, SHD_ENAN, SHD_ESTALL, SHD_EMAXEVAL = 0, -1, -2, -3, -4, -5, -6
 EXPORTS = ["shd_create", "shd_create_shell", "shd_destroy", "shd_set_stream", "shd_num_k", "shd_get_k",
            "shd_energy_grad", "shd_energy_grad_host", "shd_set_timing", "shd_smax", "shd_last_smax", "shd_get_rho", "shd_minimize",
-           "shd_last_error", "shd_stat", "shd_fp64_peak", "shd_structure_factor"]
+           "shd_last_error", "shd_stat", "shd_fp64_peak", "shd_structure_factor", "shd_set_precision"]
 
 
 class ShdError(RuntimeError):
@@ -64,6 +64,7 @@ def _load():
     lib.shd_stat.restype = C.c_double
     lib.shd_fp64_peak.argtypes = [C.c_int, C.c_double, dp]
     lib.shd_structure_factor.argtypes = [vp, vp, dp]
+    lib.shd_set_precision.argtypes = [vp, C.c_int]
     return lib
 
 
@@ -182,6 +183,10 @@ class Shd:
         out = [torch.empty(self.M, dtype=torch.float64, device="cuda") for _ in range(4)]
         self._check(lib.shd_get_rho(self._h, *[C.c_void_p(t.data_ptr()) for t in out]))
         return tuple(out)
+
+    def set_precision(self, limbs: int):
+        """shd_set_precision: 3 = double-double products (default), 2 = fast 44-bit operands."""
+        self._check(lib.shd_set_precision(self._h, int(limbs)))
 
     def structure_factor(self, want_S=True):
         """shd_structure_factor on the last evaluation: (S device tensor or None, (hi, lo) of

@@ -205,3 +205,26 @@ def test_quench_to_the_precision_floor(shd, oracle, name, floor):
     assert s_or < floor
     assert rep["smax"][0] < floor
     h.close()
+
+
+def test_precision_ladder_quench(shd, oracle):
+    """Two rungs: 2-limb evaluations down to S_max < 1e-18, then double-double
+    to S_max < 1e-30; the oracle evaluates the final positions.  The first rung must carry most of the
+    evaluations (that is the point of the ladder)."""
+    cfg = inputs.CONFIGS["cfg2"]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    th, tl = shd.from_host(hi, lo)
+    h.set_precision(2)
+    r1 = h.minimize(th, tl, smax_tol=1e-18, max_evals=20000, poll_every=32)
+    assert r1["status"] == shd.SHD_OK, r1
+    h.set_precision(3)
+    r2 = h.minimize(th, tl, smax_tol=1e-30, max_evals=20000, poll_every=32)
+    print("ladder", r1, r2)
+    assert r2["status"] == shd.SHD_OK, r2
+    assert r1["evals"] > r2["evals"]
+    n = oracle.enumerate_Q(cfg.d, cfg.m_star)
+    re, im = oracle.rho(cfg.d, cfg.N, cfg.L, th.cpu().numpy(), tl.cpu().numpy(), n, mode="factored")
+    _, smax, _, _ = oracle.energy(cfg.N, re, im)
+    assert oracle.to_float(smax)[0] < 1e-30
+    h.close()

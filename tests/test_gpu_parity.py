@@ -214,3 +214,33 @@ def test_structure_factor_and_tau(shd, oracle):
     S, dev2 = h.structure_factor()
     assert float(S.abs().max()) < 1e-25 and abs(dev2[0] - h.M) < 1e-12
     h.close()
+
+
+def test_fast_precision_two_limbs(shd, oracle):
+    """shd_set_precision(h, 2) ("tunable precision"): operands at 44 bits,
+    per-term error <= 3 * 2^-45; the mode must really be active (error far above the dd level) and
+    switching back to 3 limbs must restore the dd result bit for bit."""
+    cfg = inputs.CONFIGS["cfg2"]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    th, tl = shd.from_host(hi, lo)
+    phi3, gh3, gl3 = h.energy_grad(th, tl)
+    rho3 = [x.cpu().numpy() for x in h.rho()]
+    h.set_precision(2)
+    phi2, gh2, gl2 = h.energy_grad(th, tl)
+    rho2 = [x.cpu().numpy() for x in h.rho()]
+    N, M, K = cfg.N, cfg.M, cfg.K
+    e_rho = oracle.cabsdiff_dd(oracle.from_dd(rho3[0], rho3[1]), oracle.from_dd(rho3[2], rho3[3]), *rho2)
+    e_g = oracle.absdiff_dd(oracle.from_dd(gh3.cpu().numpy(), gl3.cpu().numpy()), gh2.cpu().numpy(), gl2.cpu().numpy())
+    print("fast mode: max |drho|", e_rho.max(), "max |dgrad|", e_g.max(), "dPhi", phi2[0] - phi3[0])
+    assert 1e-20 < e_rho.max() <= 1e-13 * N               # worst case N * 3 * 2^-45; typically ~ sqrt(N)
+    assert e_rho.max() <= 2e-13 * np.sqrt(N) * 10
+    assert 1e-18 < e_g.max() <= 1e-13 * N * M * K
+    assert abs(phi2[0] - phi3[0]) <= 1e-11 * abs(phi3[0])
+    h.set_precision(3)
+    phi3b, gh3b, gl3b = h.energy_grad(th, tl)
+    import torch
+    assert phi3b == phi3 and torch.equal(gh3b, gh3) and torch.equal(gl3b, gl3)
+    with pytest.raises(shd.ShdError):
+        h.set_precision(4)
+    h.close()
