@@ -102,8 +102,10 @@ int shd_get_rho(shd_ctx* h, double* re_hi, double* re_lo, double* im_hi, double*
  * (double-double results; BASELINE.json's tolerances).  limbs = 2: "fast" evaluations for the early part of a
  * quench (precision ladder): the phasor and rho operands are used at 44 bits
  * (two exact limbs), half the FMAs; per-term error ~2^-45, i.e. |rho| to ~3e-14 sqrt(N), enough to drive
- * S_max to ~1e-22; everything else (phasor tables, reductions, minimizer algebra) stays double-double.
- * Applies to every later call on the handle.  Errors: SHD_EINVAL (limbs not 2 or 3).
+ * S_max to ~1e-22.  limbs = 1: operands at 22 bits (one exact limb), one sixth of the FMAs, per-term error
+ * ~2^-23: the first decades of a quench (S_max down to ~1e-10).  Everything else (phasor tables, reductions,
+ * minimizer algebra) stays double-double.  Applies to every later call on the handle.
+ * Errors: SHD_EINVAL (limbs not 1, 2 or 3).
  */
 int shd_set_precision(shd_ctx* h, int limbs);
 

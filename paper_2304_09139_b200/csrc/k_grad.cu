@@ -63,8 +63,8 @@ __device__ __forceinline__ dd limbs_to_dd(double x0, double x1, double x2) {
     _Pragma("unroll") for (int o = 0; o < 4; o++)                           \
         _Pragma("unroll") for (int t = 0; t < 2; t++) X[o][t] = lds2((base) + t * 512 + (o * 4 + (L)) * PLANE_C);
 
-// FULL = false: the two-limb "fast" precision of shd_set_precision(h, 2) (see k_rho.cu)
-template <bool FULL>
+// NL = 2 / 1: the two-limb / one-limb "fast" precisions of shd_set_precision (see k_rho.cu)
+template <int NL>
 __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
     int d, long N, long Npad, long njb64, int Qpad, int Ppad, int qscale_log2,
     const int2* __restrict__ steps, int nsteps, int nseg, const int* __restrict__ wT,
@@ -175,18 +175,21 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
         b0 = lds2(s0 + offB);
         LOADX(X0, s0 + offC, 0)
     }
+    constexpr bool FULL = NL >= 3, TWO = NL >= 2;
     for (int c = 0; c < total; c++) {
         const int s = c % NST;
         const uint32_t pB = s0 + s * GSTAGE + offB, pC = s0 + s * GSTAGE + offC;
         const int2 st = steps[c_begin + c];
         if (pend) load_quarter(pk, ppb, pa0, pa1, pa2);
-        const F2 b1 = lds2(pB + 1 * PLANE_B);
-        F2 b2{0.0, 0.0}, b12{0.0, 0.0};
+        F2 b1{0.0, 0.0}, b2{0.0, 0.0}, b12{0.0, 0.0};
+        if (TWO) b1 = lds2(pB + 1 * PLANE_B);
         if (FULL) b2 = lds2(pB + 2 * PLANE_B);
-        GROUND(l0, b0, X0)
         F2 X1[4][2];
-        LOADX(X1, pC, 1)
-        GROUND(l1, b1, X0)
+        if (TWO) {
+            GROUND(l0, b0, X0)
+            LOADX(X1, pC, 1)
+            GROUND(l1, b1, X0)
+        }
         if (FULL) {
             F2 X2[4][2];
             LOADX(X2, pC, 2)
@@ -211,7 +214,7 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
                 b0n = lds2(s0 + sn * GSTAGE + offB);
                 LOADX(X0n, s0 + sn * GSTAGE + offC, 0)
             }
-            GROUND(l1, b0, X1)
+            if (TWO) { GROUND(l1, b0, X1) } else { GROUND(l0, b0, X0) }
             b0 = b0n;
             if (c + 1 < total) {
 #pragma unroll
@@ -313,23 +316,23 @@ __global__ void __launch_bounds__(256) k_gradsum(
 
 cudaError_t shd_grad_configure()
 {
-    cudaError_t e = cudaFuncSetAttribute(k_grad<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, GSMEM);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_grad<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, GSMEM);
+    cudaError_t e = cudaFuncSetAttribute(k_grad<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, GSMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, GSMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, GSMEM);
+    return e;
 }
 
 cudaError_t shd_launch_grad(shd_ctx* h, double* grad_hi, double* grad_lo)
 {
-    if (h->nlimb >= 3)
-        k_grad<true><<<(unsigned)(h->njb64 * h->nseg), NW * 32 + 128, GSMEM, h->stream>>>(
-            h->d, h->N, h->Npad, h->njb64, h->Qpad, h->npb * 32, h->qscale_log2,
-            reinterpret_cast<const int2*>(h->d_steps), h->nsteps, h->nseg, h->d_wT,
-            h->d_A, h->d_Bg, h->d_C, h->d_gpart, h->d_skip);
-    else
-        k_grad<false><<<(unsigned)(h->njb64 * h->nseg), NW * 32 + 128, GSMEM, h->stream>>>(
-            h->d, h->N, h->Npad, h->njb64, h->Qpad, h->npb * 32, h->qscale_log2,
-            reinterpret_cast<const int2*>(h->d_steps), h->nsteps, h->nseg, h->d_wT,
-            h->d_A, h->d_Bg, h->d_C, h->d_gpart, h->d_skip);
+#define LAUNCH_GRAD(NLV)                                                                                 \
+    k_grad<NLV><<<(unsigned)(h->njb64 * h->nseg), NW * 32 + 128, GSMEM, h->stream>>>(                      \
+        h->d, h->N, h->Npad, h->njb64, h->Qpad, h->npb * 32, h->qscale_log2,                               \
+        reinterpret_cast<const int2*>(h->d_steps), h->nsteps, h->nseg, h->d_wT,                            \
+        h->d_A, h->d_Bg, h->d_C, h->d_gpart, h->d_skip)
+    if (h->nlimb >= 3) LAUNCH_GRAD(3);
+    else if (h->nlimb == 2) LAUNCH_GRAD(2);
+    else LAUNCH_GRAD(1);
+#undef LAUNCH_GRAD
     const long n = (long)h->d * h->N;
     k_gradsum<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(
         n, h->nseg, h->L, h->d_gpart, h->d_scal, grad_hi, grad_lo, h->d_skip);

@@ -28,10 +28,11 @@ constexpr int MAIN_BYTES = 16 * 256 * 16;                    // 16 dd sums per t
 constexpr int RHO_SMEM = RING_BYTES + MAIN_BYTES;
 constexpr int KSTEPS_PER_BURST = SHD_BURST / 4;
 
-// FULL = true: three limbs (double-double accuracy).  FULL = false: the "fast" precision of
-// shd_set_precision(h, 2): limbs x0, x1 only (L0 and L1, both exact), i.e. operands rounded to 44 bits,
-// half the FMAs; error ~2^-45 per term instead of ~2^-98 ("tunable precision").
-template <bool FULL>
+// NL = 3: three limbs (double-double accuracy).  NL = 2: the "fast" precision of shd_set_precision(h, 2):
+// limbs x0, x1 only (L0 and L1, both exact), i.e. operands rounded to 44 bits, half the FMAs; error ~2^-45
+// per term instead of ~2^-98.  NL = 1: limb x0 only (22-bit operands, one sixth of the FMAs, error ~2^-23
+// per term) for the first decades of a quench ("tunable precision").
+template <int NL>
 __global__ void __launch_bounds__(NW * 32 + 128, 1) k_rho(
     const double* __restrict__ A, const double* __restrict__ B,
     const int* __restrict__ tile_pb, const int* __restrict__ tile_qb, const int* __restrict__ tile_wmap, int ntiles,
@@ -119,25 +120,28 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_rho(
 #pragma unroll
         for (int t = 0; t < 2; t++) b0[t] = lds2(s0 + offB + t * 8 * 64);
     }
+    constexpr bool FULL = NL >= 3, TWO = NL >= 2;
     for (int k = 0; k < nk; k++) {
         const int c = k / GPS, g = k % GPS, s = c % SHD_RHO_STAGES;
         const uint32_t pA = s0 + s * STAGE_BYTES + g * GROUP_BYTES + offA;
         const uint32_t pB = s0 + s * STAGE_BYTES + g * GROUP_BYTES + offB;
-        const F2 a1 = lds2(pA + PLANE_BYTES);
-        F2 a2{0.0, 0.0}, a12{0.0, 0.0};
+        F2 a1{0.0, 0.0}, a2{0.0, 0.0}, a12{0.0, 0.0};
+        if (TWO) a1 = lds2(pA + PLANE_BYTES);
         if (FULL) a2 = lds2(pA + 2 * PLANE_BYTES);
         ROUND(l0, a0, b0)
-        F2 b1[2], b2[2] = {{0.0, 0.0}, {0.0, 0.0}};
+        F2 b1[2] = {{0.0, 0.0}, {0.0, 0.0}}, b2[2] = {{0.0, 0.0}, {0.0, 0.0}};
+        if (TWO) {
 #pragma unroll
-        for (int t = 0; t < 2; t++) b1[t] = lds2(pB + t * 8 * 64 + PLANE_BYTES);
-        ROUND(l1, a1, b0)
+            for (int t = 0; t < 2; t++) b1[t] = lds2(pB + t * 8 * 64 + PLANE_BYTES);
+            ROUND(l1, a1, b0)
+        }
         if (FULL) {
 #pragma unroll
             for (int t = 0; t < 2; t++) b2[t] = lds2(pB + t * 8 * 64 + 2 * PLANE_BYTES);
             ROUND(l2, a2, b0)
             a12 = add2(a1, a2);
         }
-        ROUND(l1, a0, b1)
+        if (TWO) { ROUND(l1, a0, b1) }
         if (FULL) { ROUND(l2, a0, b2) }
         if (g == GPS - 1) {
             // every LDS of stage s has been consumed by an issued DMMA: release the stage
@@ -196,20 +200,22 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_rho(
 
 cudaError_t shd_rho_configure()
 {
-    cudaError_t e = cudaFuncSetAttribute(k_rho<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHO_SMEM);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_rho<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHO_SMEM);
+    cudaError_t e = cudaFuncSetAttribute(k_rho<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHO_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rho<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHO_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rho<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, RHO_SMEM);
+    return e;
 }
 
 cudaError_t shd_launch_rho(shd_ctx* h)
 {
     unsigned grid = (unsigned)(h->ntiles * h->nsplit);
-    if (h->nlimb >= 3)
-        k_rho<true><<<grid, NW * 32 + 128, RHO_SMEM, h->stream>>>(
-            h->d_A, h->d_B, h->d_tile_pb, h->d_tile_qb, h->d_tile_wmap, h->ntiles, h->Npad, h->chunks_per_split, h->d_part, h->d_skip);
-    else
-        k_rho<false><<<grid, NW * 32 + 128, RHO_SMEM, h->stream>>>(
-            h->d_A, h->d_B, h->d_tile_pb, h->d_tile_qb, h->d_tile_wmap, h->ntiles, h->Npad, h->chunks_per_split, h->d_part, h->d_skip);
+#define LAUNCH_RHO(NLV)                                                                                   \
+    k_rho<NLV><<<grid, NW * 32 + 128, RHO_SMEM, h->stream>>>(h->d_A, h->d_B, h->d_tile_pb, h->d_tile_qb,    \
+        h->d_tile_wmap, h->ntiles, h->Npad, h->chunks_per_split, h->d_part, h->d_skip)
+    if (h->nlimb >= 3) LAUNCH_RHO(3);
+    else if (h->nlimb == 2) LAUNCH_RHO(2);
+    else LAUNCH_RHO(1);
+#undef LAUNCH_RHO
     h->last_launches += 1;
     return cudaGetLastError();
 }

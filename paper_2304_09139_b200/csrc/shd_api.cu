@@ -475,7 +475,7 @@ int shd_get_rho(shd_ctx* h, double* re_hi, double* re_lo, double* im_hi, double*
 
 int shd_set_precision(shd_ctx* h, int limbs) {
     if (!h) return SHD_EINVAL;
-    if (limbs != 2 && limbs != 3) return fail(h, SHD_EINVAL, "shd_set_precision: limbs must be 2 or 3");
+    if (limbs < 1 || limbs > 3) return fail(h, SHD_EINVAL, "shd_set_precision: limbs must be 1, 2 or 3");
     h->nlimb = limbs;
     return SHD_OK;
 }

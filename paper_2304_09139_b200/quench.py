@@ -39,6 +39,9 @@ def main(argv=None):
     ap.add_argument("--ladder", type=float, default=0.0,
                     help="precision ladder (P:77 'tunable precision'; SURVEY.md 8(f) NEXT-1): evaluate with two "
                          "limbs (shd_set_precision 2) until S_max < this value, e.g. 1e-18, then with three")
+    ap.add_argument("--ladder1", type=float, default=0.0,
+                    help="optional first rung below that: ONE limb (22-bit operands) until S_max < this value, "
+                         "e.g. 1e-8")
     ap.add_argument("--out", default=None)
     ap.add_argument("--save", default=None)
     args = ap.parse_args(argv)
@@ -61,12 +64,17 @@ def main(argv=None):
     status = shd.SHD_EMAXEVAL
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    fast = args.ladder > args.tol
-    if fast:
-        h.set_precision(2)
+    # rungs: (limbs, stop below this S_max); the last rung is always 3 limbs down to --tol
+    rungs = [(1, args.ladder1)] if args.ladder1 > max(args.ladder, args.tol) else []
+    if args.ladder > args.tol:
+        rungs.append((2, args.ladder))
+    rungs.append((3, args.tol))
+    rung = 0
+    h.set_precision(rungs[0][0])
     while evals < args.max_evals:
+        fast = rung < len(rungs) - 1
         rep = h.minimize(pos_hi, pos_lo, kind=args.kind, history=args.history,
-                         smax_tol=args.ladder if fast else args.tol,
+                         smax_tol=rungs[rung][1],
                          max_evals=min(args.chunk, args.max_evals - evals), poll_every=args.poll_every,
                          resume=evals > 0, fire_dt0=args.fire_dt0)
         evals += rep["evals"]
@@ -77,9 +85,9 @@ def main(argv=None):
         print(f"[quench {cfg.name}] evals={evals} iters={iters} Phi={rep['phi'][0]:.6e} "
               f"S_max={rep['smax'][0]:.6e} t={trace[-1]['seconds']:.1f}s", file=sys.stderr, flush=True)
         if fast and status in (shd.SHD_OK, shd.SHD_ESTALL):
-            fast = False                      # second rung: double-double evaluations from here on
-            h.set_precision(3)
-            trace[-1]["switched_to_3_limbs"] = True
+            rung += 1                         # next rung: more limbs from here on
+            h.set_precision(rungs[rung][0])
+            trace[-1]["switched_to_limbs"] = rungs[rung][0]
             status = shd.SHD_EMAXEVAL
             continue
         if status != shd.SHD_EMAXEVAL:
@@ -89,7 +97,7 @@ def main(argv=None):
     n = h.k()
     line = {"config": cfg.name, "d": cfg.d, "N": cfg.N, "M": cfg.M, "chi_realised": cfg.M / (cfg.d * (cfg.N - 1)),
             "seed": args.seed, "kind": "lbfgs" if args.kind == 0 else "fire", "weight": args.weight, "history": args.history,
-            "tol": args.tol, "ladder": args.ladder, "status": status, "evals": evals, "iters": iters, "seconds": seconds,
+            "tol": args.tol, "ladder": args.ladder, "ladder1": args.ladder1, "status": status, "evals": evals, "iters": iters, "seconds": seconds,
             "ms_per_eval": 1e3 * seconds / max(evals, 1), "phi_start": phi0[0], "smax_start": smax0[0],
             "phi_final": trace[-1]["phi"], "smax_final": smax[0], "argmax_n": n[arg].tolist(), "trace": trace}
     if args.save:

@@ -185,7 +185,7 @@ class Shd:
         return tuple(out)
 
     def set_precision(self, limbs: int):
-        """shd_set_precision: 3 = double-double products (default), 2 = fast 44-bit operands."""
+        """shd_set_precision: 3 = double-double products (default), 2 = 44-bit operands, 1 = 22-bit operands."""
         self._check(lib.shd_set_precision(self._h, int(limbs)))
 
     def structure_factor(self, want_S=True):

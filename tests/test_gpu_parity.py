@@ -237,10 +237,21 @@ def test_fast_precision_two_limbs(shd, oracle):
     assert e_rho.max() <= 2e-13 * np.sqrt(N) * 10
     assert 1e-18 < e_g.max() <= 1e-13 * N * M * K
     assert abs(phi2[0] - phi3[0]) <= 1e-11 * abs(phi3[0])
+    # one limb: 22-bit operands, per-term error <= 2^-22
+    h.set_precision(1)
+    phi1, gh1, gl1 = h.energy_grad(th, tl)
+    rho1 = [x.cpu().numpy() for x in h.rho()]
+    e_rho1 = oracle.cabsdiff_dd(oracle.from_dd(rho3[0], rho3[1]), oracle.from_dd(rho3[2], rho3[3]), *rho1)
+    e_g1 = oracle.absdiff_dd(oracle.from_dd(gh3.cpu().numpy(), gl3.cpu().numpy()), gh1.cpu().numpy(), gl1.cpu().numpy())
+    print("one limb: max |drho|", e_rho1.max(), "max |dgrad|", e_g1.max(), "dPhi", phi1[0] - phi3[0])
+    assert 1e-9 < e_rho1.max() <= 2.0 ** -21 * N
+    assert e_rho1.max() <= 2.0 ** -21 * np.sqrt(N) * 10
+    assert e_g1.max() <= 2.0 ** -20 * N * M * K
     h.set_precision(3)
     phi3b, gh3b, gl3b = h.energy_grad(th, tl)
     import torch
     assert phi3b == phi3 and torch.equal(gh3b, gh3) and torch.equal(gl3b, gl3)
-    with pytest.raises(shd.ShdError):
-        h.set_precision(4)
+    for bad in (0, 4):
+        with pytest.raises(shd.ShdError):
+            h.set_precision(bad)
     h.close()
