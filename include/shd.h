@@ -55,6 +55,16 @@ int shd_create(int d, long N, double L, double K, const double* v, shd_ctx** out
 /* Same, with the integer shell cutoff n.n <= m_star given directly (no FP compare, D:R8). */
 int shd_create_shell(int d, long N, double L, long m_star, const double* v, shd_ctx** out);
 
+/*
+ * The same with the caller's own wavevector set ("anisotropic exclusion regions"; SURVEY.md 8(f)
+ * NEXT-4): n (HOST, M*d ints, row-major (k,a)) lists M distinct non-zero integer vectors, each in the half
+ * space of D:R7 (first non-zero component positive); k = 2 pi n / L.  The given order is the canonical
+ * order of this handle (v, shd_get_k, shd_get_rho, argmax).  Limits: |n_a| <= 2000 for d >= 2 (|n_1| <= 128
+ * for d = 3), n <= 2e6 for d = 1.  Errors: SHD_EINVAL (bad argument, vector outside the half space,
+ * duplicate), SHD_ENOMEM, SHD_ECUDA.
+ */
+int shd_create_table(int d, long N, double L, long M, const int* n, const double* v, shd_ctx** out);
+
 void shd_destroy(shd_ctx* h);
 
 /* Use CUDA stream `cuda_stream` (a cudaStream_t) for all later work; default is stream 0. */

@@ -10,6 +10,7 @@
 #include <functional>
 #include <map>
 #include <new>
+#include <utility>
 
 namespace {
 
@@ -78,7 +79,7 @@ int build(shd_ctx* h, const double* v) {
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
         return fail(h, SHD_ECUDA, "no CUDA device: libshd has no CPU fallback");
-    enumerate_Q(d, m_star, h->nvec);
+    if (h->nvec.empty()) enumerate_Q(d, m_star, h->nvec);      // else: the caller's table (shd_create_table)
     h->M = (long)h->nvec.size() / d;
     if (h->M < 1) return fail(h, SHD_EINVAL, "empty Q");
     if (v) {
@@ -86,13 +87,23 @@ int build(shd_ctx* h, const double* v) {
         for (double x : h->v)
             if (!(x > 0.0) || !std::isfinite(x)) return fail(h, SHD_EINVAL, "v(k) must be positive and finite");
     }
-    const long R = isqrt_floor(m_star);
-    // ---- outer-product decomposition
+    // ---- outer-product decomposition, derived from the set itself (so that any half-space table works)
     std::map<std::vector<int>, int> index;
-    for (long k = 0; k < h->M; k++)
-        index[std::vector<int>(h->nvec.begin() + k * d, h->nvec.begin() + (k + 1) * d)] = (int)k;
+    long R0 = 0, Rlast = 0;
+    for (long k = 0; k < h->M; k++) {
+        std::vector<int> n(h->nvec.begin() + k * d, h->nvec.begin() + (k + 1) * d);
+        int first = 0;
+        for (int a = 0; a < d && first == 0; a++) first = n[a];
+        if (first <= 0) return fail(h, SHD_EINVAL, "wavevector table: every n must be non-zero with its first non-zero component positive (half space, D:R7)");
+        if (!index.emplace(n, (int)k).second) return fail(h, SHD_EINVAL, "wavevector table: duplicate n");
+        R0 = std::max<long>(R0, n[0]);
+        Rlast = std::max<long>(Rlast, std::abs(n[d - 1]));
+        for (int a = 0; a < d; a++)
+            if (std::abs((long)n[a]) > (d == 1 ? 2000000L : 2000L)) return fail(h, SHD_EINVAL, "wavevector table: |n_a| too large");
+    }
     std::vector<std::vector<int>> wT(3);
     if (d == 1) {
+        const long R = R0;
         int S = 2;
         while ((double)S * S < 2.0 * (double)R) S *= 2;
         h->S1d = S;
@@ -100,17 +111,20 @@ int build(shd_ctx* h, const double* v) {
         h->P = (int)((R + S / 2 - 1) / S) + 1;
         for (int p = 0; p < h->P; p++) { h->pn0.push_back(p); h->pn1.push_back(0); }
     } else if (d == 2) {
-        h->P = (int)R + 1;
-        h->Qn = (int)R + 1;
+        h->P = (int)R0 + 1;
+        h->Qn = (int)Rlast + 1;
         for (int p = 0; p < h->P; p++) { h->pn0.push_back(p); h->pn1.push_back(0); }
     } else {
-        if (R > 128) return fail(h, SHD_EINVAL, "d = 3 supports |n_a| <= 128");
-        for (long a = 0; a <= R; a++) {
-            long r1 = isqrt_floor(m_star - a * a);
-            for (long b = (a == 0 ? 0 : -r1); b <= r1; b++) { h->pn0.push_back((int)a); h->pn1.push_back((int)b); }
+        // A entries = the distinct prefixes (n0, n1) of the set, lexicographic (n0 ascending: k_tables walks
+        // the powers of z0 forward)
+        std::map<std::pair<int, int>, int> prefixes;
+        for (long k = 0; k < h->M; k++) prefixes.emplace(std::make_pair(h->nvec[k * 3], h->nvec[k * 3 + 1]), 0);
+        for (auto& pr : prefixes) {
+            if (std::abs(pr.first.second) > 128) return fail(h, SHD_EINVAL, "d = 3 supports |n_1| <= 128");
+            h->pn0.push_back(pr.first.first); h->pn1.push_back(pr.first.second);
         }
         h->P = (int)h->pn0.size();
-        h->Qn = (int)R + 1;
+        h->Qn = (int)Rlast + 1;
     }
     h->npb = (h->P + 31) / 32;
     h->nqb = (h->Qn + 31) / 32;
@@ -279,15 +293,31 @@ int build(shd_ctx* h, const double* v) {
     return SHD_OK;
 }
 
-int create_common(int d, long N, double L, long m_star, const double* v, shd_ctx** out) {
+// table != nullptr: the caller's half-space set (M vectors, row-major) instead of the shell n.n <= m_star
+int create_common(int d, long N, double L, long m_star, const double* v, shd_ctx** out,
+                  const int* table = nullptr, long M = 0) {
     if (!out) return SHD_EINVAL;
     *out = nullptr;
-    if (d < 1 || d > 3 || N < 1 || !(L > 0.0) || !std::isfinite(L) || m_star < 1) return SHD_EINVAL;
-    if (d == 1 && m_star > (long)4e12) return SHD_EINVAL;
-    if (d >= 2 && m_star > (long)4e6) return SHD_EINVAL;
+    if (d < 1 || d > 3 || N < 1 || !(L > 0.0) || !std::isfinite(L)) return SHD_EINVAL;
+    if (table) {
+        if (M < 1 || M > 50000000L) return SHD_EINVAL;
+    } else {
+        if (m_star < 1) return SHD_EINVAL;
+        if (d == 1 && m_star > (long)4e12) return SHD_EINVAL;
+        if (d >= 2 && m_star > (long)4e6) return SHD_EINVAL;
+    }
     shd_ctx* h = new (std::nothrow) shd_ctx();
     if (!h) return SHD_ENOMEM;
     h->d = d; h->N = N; h->L = L; h->m_star = m_star;
+    if (table) {
+        h->nvec.assign(table, table + M * d);
+        h->m_star = 0;
+        for (long k = 0; k < M; k++) {
+            long nn = 0;
+            for (int a = 0; a < d; a++) nn += (long)table[k * d + a] * table[k * d + a];
+            h->m_star = std::max(h->m_star, nn);       // largest |n|^2 (k_max of the FIRE default time step)
+        }
+    }
     int rc;
     try {
         rc = build(h, v);
@@ -344,6 +374,11 @@ extern "C" {
 
 int shd_create_shell(int d, long N, double L, long m_star, const double* v, shd_ctx** out) {
     return create_common(d, N, L, m_star, v, out);
+}
+
+int shd_create_table(int d, long N, double L, long M, const int* n, const double* v, shd_ctx** out) {
+    if (!n) { if (out) *out = nullptr; return SHD_EINVAL; }
+    return create_common(d, N, L, 0, v, out, n, M);
 }
 
 int shd_create(int d, long N, double L, double K, const double* v, shd_ctx** out) {

@@ -15,7 +15,7 @@ _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libshd.so"
 
 SHD_OK, SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA, SHD_ENAN, SHD_ESTALL, SHD_EMAXEVAL = 0, -1, -2, -3, -4, -5, -6
-EXPORTS = ["shd_create", "shd_create_shell", "shd_destroy", "shd_set_stream", "shd_num_k", "shd_get_k",
+EXPORTS = ["shd_create", "shd_create_shell", "shd_create_table", "shd_destroy", "shd_set_stream", "shd_num_k", "shd_get_k",
            "shd_energy_grad", "shd_energy_grad_host", "shd_set_timing", "shd_smax", "shd_last_smax", "shd_get_rho", "shd_minimize",
            "shd_last_error", "shd_stat", "shd_fp64_peak", "shd_structure_factor", "shd_set_precision"]
 
@@ -45,6 +45,7 @@ def _load():
     vp, dp = C.c_void_p, C.POINTER(C.c_double)
     lib.shd_create.argtypes = [C.c_int, C.c_long, C.c_double, C.c_double, dp, C.POINTER(vp)]
     lib.shd_create_shell.argtypes = [C.c_int, C.c_long, C.c_double, C.c_long, dp, C.POINTER(vp)]
+    lib.shd_create_table.argtypes = [C.c_int, C.c_long, C.c_double, C.c_long, C.POINTER(C.c_int), dp, C.POINTER(vp)]
     lib.shd_destroy.argtypes = [vp]
     lib.shd_destroy.restype = None
     lib.shd_set_stream.argtypes = [vp, vp]
@@ -81,14 +82,18 @@ def _torch():
 class Shd:
     """One handle (shd_ctx).  Tensors are CUDA float64, axis-major ``x[a*N + j]``."""
 
-    def __init__(self, d, N, L, K=None, v=None, m_star=None):
+    def __init__(self, d, N, L, K=None, v=None, m_star=None, table=None):
         self.d, self.N, self.L = int(d), int(N), float(L)
         self._h = C.c_void_p()
         pv = None
         if v is not None:
             self._v = np.ascontiguousarray(v, dtype=np.float64)
             pv = self._v.ctypes.data_as(C.POINTER(C.c_double))
-        if m_star is not None:
+        if table is not None:
+            self._table = np.ascontiguousarray(table, dtype=np.int32).reshape(-1, self.d)
+            rc = lib.shd_create_table(self.d, self.N, self.L, len(self._table),
+                                      self._table.ctypes.data_as(C.POINTER(C.c_int)), pv, C.byref(self._h))
+        elif m_star is not None:
             rc = lib.shd_create_shell(self.d, self.N, self.L, int(m_star), pv, C.byref(self._h))
         else:
             rc = lib.shd_create(self.d, self.N, self.L, float(K), pv, C.byref(self._h))

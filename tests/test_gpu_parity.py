@@ -255,3 +255,55 @@ def test_fast_precision_two_limbs(shd, oracle):
         with pytest.raises(shd.ShdError):
             h.set_precision(bad)
     h.close()
+
+
+@pytest.mark.parametrize("d", [1, 2, 3])
+def test_anisotropic_table(shd, oracle, d):
+    """shd_create_table ("anisotropic exclusion regions"): an elliptical /
+    ellipsoidal exclusion region (d >= 2) or a set with gaps (d = 1), in a scrambled order, against the
+    oracle on the very same table; then the same quench outcome test as for the isotropic sets."""
+    rng = np.random.default_rng(40 + d)
+    if d == 1:
+        N, L = 300, 300.0
+        n = np.array([[m] for m in range(1, 90) if m % 7 != 3], dtype=np.int32)
+    elif d == 2:
+        N, L = 400, 20.0
+        g = np.array([(a, b) for a in range(0, 25) for b in range(-12, 13)
+                      if (a / 18.0) ** 2 + (b / 7.0) ** 2 <= 1.0 and (a > 0 or b > 0)], dtype=np.int32)
+        n = g
+    else:
+        N, L = 216, 6.0
+        g = np.array([(a, b, c) for a in range(0, 4) for b in range(-3, 4) for c in range(-2, 3)
+                      if (a / 3.2) ** 2 + (b / 2.1) ** 2 + (c / 1.4) ** 2 <= 1.0
+                      and (a > 0 or b > 0 or (b == 0 and c > 0))], dtype=np.int32)
+        n = g
+    n = n[rng.permutation(len(n))]
+    v = 0.5 + rng.random(len(n))
+    hi, lo = inputs.uniform_positions_raw(d, N, L, 77)
+    lo = inputs.jitter_lo(hi, 78)
+    h = shd.Shd(d, N, L, table=n, v=v)
+    assert h.M == len(n) and np.array_equal(h.k(), n)
+    th, tl = shd.from_host(hi, lo)
+    phi, gh, gl = h.energy_grad(th, tl)
+    rho = [t.cpu().numpy() for t in h.rho()]
+    o = oracle.energy_grad(d, N, L, hi, lo, n, v=v)
+    M = len(n)
+    K = 2 * np.pi / L * np.sqrt((n.astype(np.int64) ** 2).sum(axis=1).max())
+    assert oracle.cabsdiff_dd(o["rho_re"], o["rho_im"], *rho).max() <= 1e-28 * N
+    assert oracle.absdiff_dd(o["phi"], [phi[0]], [phi[1]])[0] <= 1e-28 * N * N * M * v.max()
+    assert oracle.absdiff_dd(o["grad"], gh.cpu().numpy(), gl.cpu().numpy()).max() <= 1e-27 * N * M * K * v.max()
+    smax, arg = h.last_smax()
+    assert arg == o["argmax"]
+    chi = M / (d * (N - 1))
+    assert chi < (1 / 3 if d == 1 else 1 / 2)
+    rep = h.minimize(th, tl, smax_tol=1e-30, max_evals=20000, poll_every=16)
+    assert rep["status"] == shd.SHD_OK, rep
+    re, im = oracle.rho(d, N, L, th.cpu().numpy(), tl.cpu().numpy(), n)
+    _, s_or, _, _ = oracle.energy(N, re, im, v)
+    assert oracle.to_float(s_or)[0] < 1e-30
+    h.close()
+    # invalid tables
+    for bad in ([[0] * d], [[-1] + [0] * (d - 1)], np.concatenate([n[:3], n[:1]])):
+        with pytest.raises(shd.ShdError) as e:
+            shd.Shd(d, N, L, table=np.array(bad, dtype=np.int32))
+        assert e.value.code == shd.SHD_EINVAL
