@@ -400,6 +400,8 @@ void shd_destroy(shd_ctx* h) {
     cudaFree(h->d_hpos); cudaFree(h->d_hgrad);
     for (int i = 0; i <= SHD_NKERN; i++) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     if (h->h_scal) cudaFreeHost(h->h_scal);
+    if (h->gevent) cudaEventDestroy(h->gevent);
+    if (h->gstream) cudaStreamDestroy(h->gstream);
     delete h;
 }
 

@@ -13,6 +13,7 @@
 #include "../../include/shd.h"
 #include "dd.cuh"
 #include "shd_internal.h"
+#include "slots.cuh"
 
 #include <cmath>
 #include <cstring>
@@ -229,24 +230,22 @@ int shd_fire_run(shd_ctx* h, double* pos_hi, double* pos_lo, const shd_min_opts*
     CUF(cudaMemcpyAsync(s->d_ctrl, c, sizeof(shd_firectrl), cudaMemcpyHostToDevice, st));
     h->d_skip = &s->d_ctrl->done;
     const unsigned ublk = (unsigned)((n + FIRE_THREADS - 1) / FIRE_THREADS);
-    for (;;) {
-        for (int k = 0; k < opts->poll_every; k++) {
-            h->last_launches = 0;
-            CUF(shd_launch_tables(h, pos_hi, pos_lo, true));
-            CUF(shd_launch_rho(h));
-            CUF(shd_launch_finish(h));
-            CUF(shd_launch_ctable(h));
-            CUF(shd_launch_grad(h, s->g, s->g + n));
-            k_fire_dots<<<s->nblk, FIRE_THREADS, 0, st>>>(n, s->d_ctrl, s->g, s->v, s->partial);
-            k_fire_control<<<1, 32, 0, st>>>(s->nblk, s->d_ctrl, h->d_scal, s->partial);
-            k_fire_update<<<ublk, FIRE_THREADS, 0, st>>>(n, s->d_ctrl, pos_hi, pos_lo, s->g, s->v);
-            h->last_launches += 3;
-            CUF(cudaGetLastError());
-        }
-        CUF(cudaMemcpyAsync(c, s->d_ctrl, sizeof(shd_firectrl), cudaMemcpyDeviceToHost, st));
-        CUF(cudaStreamSynchronize(st));
-        if (c->done) break;
-    }
+    auto slot = [&]() -> cudaError_t {
+        cudaError_t e;
+        cudaStream_t q = h->stream;          // the capture stream while shd_run_slots is recording
+        h->last_launches = 0;
+        if ((e = shd_launch_tables(h, pos_hi, pos_lo, true)) != cudaSuccess) return e;
+        if ((e = shd_launch_rho(h)) != cudaSuccess) return e;
+        if ((e = shd_launch_finish(h)) != cudaSuccess) return e;
+        if ((e = shd_launch_ctable(h)) != cudaSuccess) return e;
+        if ((e = shd_launch_grad(h, s->g, s->g + n)) != cudaSuccess) return e;
+        k_fire_dots<<<s->nblk, FIRE_THREADS, 0, q>>>(n, s->d_ctrl, s->g, s->v, s->partial);
+        k_fire_control<<<1, 32, 0, q>>>(s->nblk, s->d_ctrl, h->d_scal, s->partial);
+        k_fire_update<<<ublk, FIRE_THREADS, 0, q>>>(n, s->d_ctrl, pos_hi, pos_lo, s->g, s->v);
+        h->last_launches += 3;
+        return cudaGetLastError();
+    };
+    CUF(shd_run_slots(h, opts->poll_every, slot, c, s->d_ctrl, sizeof(shd_firectrl), &c->done));
     h->d_skip = nullptr;
     report->iters = (long)c->steps;
     report->evals = (long)c->evals;

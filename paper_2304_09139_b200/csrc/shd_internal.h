@@ -115,6 +115,8 @@ struct shd_ctx {
     shd_scalars *h_scal = nullptr;  // pinned
     size_t workspace_bytes = 0;
     cudaStream_t stream = 0;
+    cudaStream_t gstream = nullptr;   // the minimizers' own (capturable) stream, slots.cuh
+    cudaEvent_t gevent = nullptr;
     const int* d_skip = nullptr;    // device flag: when non-NULL and *d_skip != 0 every kernel of the
                                     // evaluation path returns at once (set by the minimizer when done)
     shd_minstate *min = nullptr;

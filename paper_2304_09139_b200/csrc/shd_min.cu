@@ -14,6 +14,7 @@
 #include "../../include/shd.h"
 #include "dd.cuh"
 #include "shd_internal.h"
+#include "slots.cuh"
 
 #include <cstring>
 
@@ -410,26 +411,24 @@ extern "C" int shd_minimize(shd_ctx* h, double* pos_hi, double* pos_lo, const sh
     CUM(cudaMemcpyAsync(s->d_ctrl, s->h_ctrl, sizeof(shd_minctrl), cudaMemcpyHostToDevice, st));
     h->d_skip = &s->d_ctrl->done;
     const unsigned ublk = (unsigned)((n + MIN_THREADS - 1) / MIN_THREADS);
-    for (;;) {
-        for (int k = 0; k < opts->poll_every; k++) {
-            h->last_launches = 0;
-            CUM(shd_launch_tables(h, pos_hi, pos_lo, true));
-            CUM(shd_launch_rho(h));
-            CUM(shd_launch_finish(h));
-            CUM(shd_launch_ctable(h));
-            CUM(shd_launch_grad(h, s->gt, s->gt + n));
-            k_min_dots<<<s->nblk, MIN_THREADS, 0, st>>>(n, m, s->d_ctrl, pos_hi, pos_lo, s->x, s->gt, s->g,
-                                                        s->S, s->Y, s->partial);
-            k_min_control<<<1, MIN_THREADS, 0, st>>>(s->nblk, s->d_ctrl, h->d_scal, s->partial, s->G);
-            k_min_update<<<ublk, MIN_THREADS, 0, st>>>(n, m, s->d_ctrl, pos_hi, pos_lo, s->x, s->gt, s->g,
-                                                       s->p, s->S, s->Y);
-            h->last_launches += 3;
-            CUM(cudaGetLastError());
-        }
-        CUM(cudaMemcpyAsync(s->h_ctrl, s->d_ctrl, sizeof(shd_minctrl), cudaMemcpyDeviceToHost, st));
-        CUM(cudaStreamSynchronize(st));
-        if (s->h_ctrl->done) break;
-    }
+    auto slot = [&]() -> cudaError_t {
+        cudaError_t e;
+        cudaStream_t q = h->stream;          // the capture stream while shd_run_slots is recording
+        h->last_launches = 0;
+        if ((e = shd_launch_tables(h, pos_hi, pos_lo, true)) != cudaSuccess) return e;
+        if ((e = shd_launch_rho(h)) != cudaSuccess) return e;
+        if ((e = shd_launch_finish(h)) != cudaSuccess) return e;
+        if ((e = shd_launch_ctable(h)) != cudaSuccess) return e;
+        if ((e = shd_launch_grad(h, s->gt, s->gt + n)) != cudaSuccess) return e;
+        k_min_dots<<<s->nblk, MIN_THREADS, 0, q>>>(n, m, s->d_ctrl, pos_hi, pos_lo, s->x, s->gt, s->g,
+                                                   s->S, s->Y, s->partial);
+        k_min_control<<<1, MIN_THREADS, 0, q>>>(s->nblk, s->d_ctrl, h->d_scal, s->partial, s->G);
+        k_min_update<<<ublk, MIN_THREADS, 0, q>>>(n, m, s->d_ctrl, pos_hi, pos_lo, s->x, s->gt, s->g,
+                                                  s->p, s->S, s->Y);
+        h->last_launches += 3;
+        return cudaGetLastError();
+    };
+    CUM(shd_run_slots(h, opts->poll_every, slot, s->h_ctrl, s->d_ctrl, sizeof(shd_minctrl), &s->h_ctrl->done));
     h->d_skip = nullptr;
     const shd_minctrl* c = s->h_ctrl;
     report->iters = (long)c->iters;
