@@ -37,8 +37,8 @@ UNIT = "pair-terms/s"
 # DMMA.8x8x4, 256 FMAs per warp instruction).
 ALG_DFMA_RHO, ALG_DFMA_GRAD = 12.0, 24.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/r1c_summary.md), bytes; known for the headline workload only, otherwise null
-NCU_TRAFFIC = {("cfg4", "k_grad"): 12.80e9, ("cfg4", "k_rho"): 2.94e9}
+# (profiles/r1d_summary.md), bytes; known for the headline workload only, otherwise null
+NCU_TRAFFIC = {("cfg4", "k_grad"): 12.77e9, ("cfg4", "k_rho"): 3.63e9}
 
 
 def dist_env():
@@ -269,7 +269,7 @@ def run_gpu(args, cfg):
     roofline = {
         "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
         "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((cfg.name, dom)),
-        "traffic_source": "profiles/r1c_summary.md (one ncu --set full capture of this kernel at this workload)"
+        "traffic_source": "profiles/r1d_summary.md (one ncu --set full capture of this kernel at this workload)"
                           if (cfg.name, dom) in NCU_TRAFFIC else None,
         "peak_source": "measured live: shd_fp64_peak, max of dependent-DFMA chains and DMMA.8x8x4 chains "
                        "(one FP64 pipe), sustained over 1 s (of measured)",
