@@ -44,7 +44,8 @@ extern "C" {
 typedef struct shd_ctx shd_ctx;
 
 /*
- * Create a handle for dimension d in {1,2,3}, N >= 1 particles, box edge L > 0, cutoff K > 0:
+ * Create a handle for dimension d in {1,2,3,4} (d = 4: m_star <= 1024), N >= 1 particles, box edge
+ * L > 0, cutoff K > 0:
  *   m_star = floor( (K L / 2 pi)^2 (1 + 2^-40) ),  Q as above  (integer compare, D:R8).
  * v: HOST pointer to |Q| strictly positive weights v(k) in canonical order, or NULL
  * for v == 1.  The handle owns all device workspaces (phasor tables, rho, partial sums, minimizer
@@ -60,7 +61,7 @@ int shd_create_shell(int d, long N, double L, long m_star, const double* v, shd_
  * NEXT-4): n (HOST, M*d ints, row-major (k,a)) lists M distinct non-zero integer vectors, each in the half
  * space of D:R7 (first non-zero component positive); k = 2 pi n / L.  The given order is the canonical
  * order of this handle (v, shd_get_k, shd_get_rho, argmax).  Limits: |n_a| <= 2000 for d >= 2 (|n_1| <= 128
- * for d = 3), n <= 2e6 for d = 1.  Errors: SHD_EINVAL (bad argument, vector outside the half space,
+ * for d >= 3, |n_2| <= 32 for d = 4), n <= 2e6 for d = 1.  Errors: SHD_EINVAL (bad argument, vector outside the half space,
  * duplicate), SHD_ENOMEM, SHD_ECUDA.
  */
 int shd_create_table(int d, long N, double L, long M, const int* n, const double* v, shd_ctx** out);

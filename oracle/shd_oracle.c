@@ -131,24 +131,26 @@ static int in_half_space(int d, const int *n)
  */
 long shdo_enumerate(int d, long m_star, int *n_out)
 {
-    if (d < 1 || d > 3 || m_star < 1) return -1;
+    if (d < 1 || d > 4 || m_star < 1) return -1;
     int R = (int)floor(sqrt((double)m_star));
     while ((long)(R + 1) * (R + 1) <= m_star) R++;
     while ((long)R * R > m_star) R--;
     long M = 0;
-    int n[3] = {0, 0, 0};
+    int n[4] = {0, 0, 0, 0};
     int lo1 = (d >= 2) ? -R : 0, hi1 = (d >= 2) ? R : 0;
     int lo2 = (d >= 3) ? -R : 0, hi2 = (d >= 3) ? R : 0;
+    int lo3 = (d >= 4) ? -R : 0, hi3 = (d >= 4) ? R : 0;
     for (int n0 = -R; n0 <= R; n0++)
         for (int n1 = lo1; n1 <= hi1; n1++)
-            for (int n2 = lo2; n2 <= hi2; n2++) {
-                n[0] = n0; n[1] = n1; n[2] = n2;
-                long nn = (long)n0 * n0 + (long)n1 * n1 + (long)n2 * n2;
-                if (nn == 0 || nn > m_star) continue;
-                if (!in_half_space(d, n)) continue;
-                if (n_out) for (int a = 0; a < d; a++) n_out[M * d + a] = n[a];
-                M++;
-            }
+            for (int n2 = lo2; n2 <= hi2; n2++)
+                for (int n3 = lo3; n3 <= hi3; n3++) {
+                    n[0] = n0; n[1] = n1; n[2] = n2; n[3] = n3;
+                    long nn = (long)n0 * n0 + (long)n1 * n1 + (long)n2 * n2 + (long)n3 * n3;
+                    if (nn == 0 || nn > m_star) continue;
+                    if (!in_half_space(d, n)) continue;
+                    if (n_out) for (int a = 0; a < d; a++) n_out[M * d + a] = n[a];
+                    M++;
+                }
     return M;
 }
 

@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
     for (int t = 0; t < 2; t++)
 #pragma unroll
         for (int x = 0; x < 4; x++) acc3_zero(acc[t][x]);
-    dd g0{0.0, 0.0}, g1{0.0, 0.0}, g2{0.0, 0.0};
+    dd g0{0.0, 0.0}, g1{0.0, 0.0}, g2{0.0, 0.0}, g3{0.0, 0.0};
 
     // deferred p-contraction state (warp-uniform): quarter pk = (t, e) of block ppb is pending
     bool pend = false;
@@ -160,11 +160,11 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
             dd R = dd_dot2(ar, T[2], ai, T[3], 1.0);      // Re[conj(A) T'']
 #define GACC(AX)                                                                              \
     if (AX < d) {                                                                             \
-        const int wgt = wT[AX * Ppad + p];                                                    \
+        const int wgt = AX < 3 ? wT[(AX < 3 ? AX : 0) * Ppad + p] : 0;                        \
         if (wgt != 0) g##AX = dd_add(g##AX, dd_mul_d(I, (double)wgt));                        \
         if (AX == d - 1) g##AX = dd_add(g##AX, dd_scale2(R, qs));                             \
     }
-            GACC(0) GACC(1) GACC(2)
+            GACC(0) GACC(1) GACC(2) GACC(3)
 #undef GACC
         }
     };
@@ -277,6 +277,7 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
     gred[(0 * 64 + jl) * 4 + (lane & 3)] = make_double2(g0.h, g0.l);
     gred[(1 * 64 + jl) * 4 + (lane & 3)] = make_double2(g1.h, g1.l);
     gred[(2 * 64 + jl) * 4 + (lane & 3)] = make_double2(g2.h, g2.l);
+    gred[(3 * 64 + jl) * 4 + (lane & 3)] = make_double2(g3.h, g3.l);
     __syncthreads();
     if (tid < 64 * d) {
         const int a = tid / 64, jr = tid % 64;

@@ -64,7 +64,8 @@ __device__ __forceinline__ limbs split_limbs(dd x) {
     return r;
 }
 
-constexpr int R3MAX = 128;   // d == 3: max |n_1| supported by the local power table
+constexpr int R3MAX = 128;   // d >= 3: max |n_1| supported by the local power table
+constexpr int R4MAX = 32;    // d == 4: max |n_2|
 constexpr int TB = 64;       // particles (threads) per block
 constexpr int TG = 8;        // table entries staged per flush: 8 x 16 B = one 128-byte row per limb plane
 constexpr int TABLES_SMEM = TB * 3 * TG * 16;
@@ -131,7 +132,7 @@ struct Stager {
 // which = 0: A table.  which = 1: B table (+ the same limbs in the gradient layout Bg).
 __global__ void __launch_bounds__(TB) k_tables(
     int d, long N, double L, long Npad, int P, int Qn, int S1d, int qscale_log2,
-    const int* __restrict__ pn0, const int* __restrict__ pn1, int Qpad,
+    const int* __restrict__ pn0, const int* __restrict__ pn1, const int* __restrict__ pn2, int Qpad,
     const double* __restrict__ pos_hi, const double* __restrict__ pos_lo,
     double* __restrict__ A, double* __restrict__ B, double* __restrict__ Bg, int with_grad,
     const int* __restrict__ skip)
@@ -169,6 +170,14 @@ __global__ void __launch_bounds__(TB) k_tables(
             for (int p = 0; p < P; p++) { int a = abs(pn1[p]); r1max = a > r1max ? a : r1max; }
             pw1[0] = one;
             for (int m = 1; m <= r1max; m++) pw1[m] = cdd_mul(pw1[m - 1], z1);
+            cdd pw2[R4MAX + 1];                      // d == 4: powers of the third axis' base phasor
+            if (d == 4) {
+                cdd z2 = expi_turns(frac_turns(pos_hi[2 * N + jc], pos_lo[2 * N + jc], L, 1.0));
+                int r2max = 0;
+                for (int p = 0; p < P; p++) { int a = abs(pn2[p]); r2max = a > r2max ? a : r2max; }
+                pw2[0] = one;
+                for (int m = 1; m <= r2max; m++) pw2[m] = cdd_mul(pw2[m - 1], z2);
+            }
             cdd cur0 = one;
             int n0cur = 0;
             for (int p0 = 0; p0 < P; p0 += TG) {
@@ -177,6 +186,10 @@ __global__ void __launch_bounds__(TB) k_tables(
                     const int n0 = pn0[p0 + s], n1 = pn1[p0 + s];
                     while (n0cur < n0) { cur0 = cdd_mul(cur0, base); n0cur++; }
                     cdd f = n1 >= 0 ? pw1[n1] : cdd_conj(pw1[-n1]);
+                    if (d == 4) {
+                        const int n2 = pn2[p0 + s];
+                        f = cdd_mul(f, n2 >= 0 ? pw2[n2] : cdd_conj(pw2[-n2]));
+                    }
                     st.put(0, s, cdd_mul(cur0, f));
                 }
                 st.flush(p0, cnt);
@@ -209,7 +222,7 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
 {
     dim3 grid((unsigned)((h->N + TB - 1) / TB), 2);
     k_tables<<<grid, TB, TABLES_SMEM, h->stream>>>(h->d, h->N, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2,
-                                         h->d_pn0, h->d_pn1, h->Qpad, pos_hi, pos_lo,
+                                         h->d_pn0, h->d_pn1, h->d_pn2, h->Qpad, pos_hi, pos_lo,
                                          h->d_A, h->d_B, h->d_Bg, with_grad_tables ? 1 : 0, h->d_skip);
     h->last_launches += 1;
     return cudaGetLastError();

@@ -57,6 +57,21 @@ void enumerate_Q(int d, long m_star, std::vector<int>& out) {
     }
 }
 
+// d = 4 ("d = 1-4"): same order (lexicographic, n0 slowest), by filtering the cube
+void enumerate_Q4(long m_star, std::vector<int>& out) {
+    const long R = isqrt_floor(m_star);
+    out.clear();
+    for (long a = 0; a <= R; a++)
+        for (long b = -R; b <= R; b++)
+            for (long c = -R; c <= R; c++)
+                for (long e = -R; e <= R; e++) {
+                    if (a * a + b * b + c * c + e * e > m_star) continue;
+                    const long first = a != 0 ? a : (b != 0 ? b : (c != 0 ? c : e));
+                    if (first <= 0) continue;
+                    out.push_back((int)a); out.push_back((int)b); out.push_back((int)c); out.push_back((int)e);
+                }
+}
+
 template <class T>
 int upload(shd_ctx* h, T** dst, const std::vector<T>& src) {
     size_t bytes = std::max<size_t>(src.size(), 1) * sizeof(T);
@@ -79,7 +94,9 @@ int build(shd_ctx* h, const double* v) {
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
         return fail(h, SHD_ECUDA, "no CUDA device: libshd has no CPU fallback");
-    if (h->nvec.empty()) enumerate_Q(d, m_star, h->nvec);      // else: the caller's table (shd_create_table)
+    if (h->nvec.empty()) {                                     // else: the caller's table (shd_create_table)
+        if (d == 4) enumerate_Q4(m_star, h->nvec); else enumerate_Q(d, m_star, h->nvec);
+    }
     h->M = (long)h->nvec.size() / d;
     if (h->M < 1) return fail(h, SHD_EINVAL, "empty Q");
     if (v) {
@@ -117,11 +134,15 @@ int build(shd_ctx* h, const double* v) {
     } else {
         // A entries = the distinct prefixes (n0, n1) of the set, lexicographic (n0 ascending: k_tables walks
         // the powers of z0 forward)
-        std::map<std::pair<int, int>, int> prefixes;
-        for (long k = 0; k < h->M; k++) prefixes.emplace(std::make_pair(h->nvec[k * 3], h->nvec[k * 3 + 1]), 0);
+        // (d = 4: prefixes (n0, n1, n2))
+        std::map<std::vector<int>, int> prefixes;
+        for (long k = 0; k < h->M; k++)
+            prefixes.emplace(std::vector<int>(h->nvec.begin() + k * d, h->nvec.begin() + k * d + d - 1), 0);
         for (auto& pr : prefixes) {
-            if (std::abs(pr.first.second) > 128) return fail(h, SHD_EINVAL, "d = 3 supports |n_1| <= 128");
-            h->pn0.push_back(pr.first.first); h->pn1.push_back(pr.first.second);
+            if (std::abs(pr.first[1]) > 128) return fail(h, SHD_EINVAL, "d >= 3 supports |n_1| <= 128");
+            if (d == 4 && std::abs(pr.first[2]) > 32) return fail(h, SHD_EINVAL, "d = 4 supports |n_2| <= 32");
+            h->pn0.push_back(pr.first[0]); h->pn1.push_back(pr.first[1]);
+            h->pn2.push_back(d == 4 ? pr.first[2] : 0);
         }
         h->P = (int)h->pn0.size();
         h->Qn = (int)Rlast + 1;
@@ -136,7 +157,7 @@ int build(shd_ctx* h, const double* v) {
     for (int p = 0; p < h->P; p++) {
         if (d == 1) wT[0][p] = h->S1d * p;
         else if (d == 2) wT[0][p] = h->pn0[p];
-        else { wT[0][p] = h->pn0[p]; wT[1][p] = h->pn1[p]; }
+        else { wT[0][p] = h->pn0[p]; wT[1][p] = h->pn1[p]; if (d == 4) wT[2][p] = h->pn2[p]; }
     }
     std::vector<int> kp((size_t)Ppad * h->Qpad, -1), km((size_t)Ppad * h->Qpad, -1);
     long found = 0;
@@ -147,7 +168,8 @@ int build(shd_ctx* h, const double* v) {
                 std::vector<int> n(d);
                 if (d == 1) n[0] = h->S1d * p + sg * q;
                 else if (d == 2) { n[0] = h->pn0[p]; n[1] = sg * q; }
-                else { n[0] = h->pn0[p]; n[1] = h->pn1[p]; n[2] = sg * q; }
+                else if (d == 3) { n[0] = h->pn0[p]; n[1] = h->pn1[p]; n[2] = sg * q; }
+                else { n[0] = h->pn0[p]; n[1] = h->pn1[p]; n[2] = h->pn2[p]; n[3] = sg * q; }
                 if (d == 1 && q == h->S1d / 2 && sg < 0) continue;   // S p - S/2 is (p-1, +S/2)
                 auto it = index.find(n);
                 if (it == index.end()) continue;
@@ -264,6 +286,7 @@ int build(shd_ctx* h, const double* v) {
     int rc;
     if ((rc = upload(h, &h->d_pn0, h->pn0))) return rc;
     if ((rc = upload(h, &h->d_pn1, h->pn1))) return rc;
+    if ((rc = upload(h, &h->d_pn2, h->pn2))) return rc;
     std::vector<int> wflat;
     for (int a = 0; a < 3; a++) wflat.insert(wflat.end(), wT[a].begin(), wT[a].end());
     if ((rc = upload(h, &h->d_wT, wflat))) return rc;
@@ -298,13 +321,14 @@ int create_common(int d, long N, double L, long m_star, const double* v, shd_ctx
                   const int* table = nullptr, long M = 0) {
     if (!out) return SHD_EINVAL;
     *out = nullptr;
-    if (d < 1 || d > 3 || N < 1 || !(L > 0.0) || !std::isfinite(L)) return SHD_EINVAL;
+    if (d < 1 || d > 4 || N < 1 || !(L > 0.0) || !std::isfinite(L)) return SHD_EINVAL;
     if (table) {
         if (M < 1 || M > 50000000L) return SHD_EINVAL;
     } else {
         if (m_star < 1) return SHD_EINVAL;
         if (d == 1 && m_star > (long)4e12) return SHD_EINVAL;
         if (d >= 2 && m_star > (long)4e6) return SHD_EINVAL;
+        if (d == 4 && m_star > 32 * 32) return SHD_EINVAL;
     }
     shd_ctx* h = new (std::nothrow) shd_ctx();
     if (!h) return SHD_ENOMEM;
@@ -393,7 +417,7 @@ void shd_destroy(shd_ctx* h) {
     if (!h) return;
     shd_min_free(h);
     shd_fire_free(h);
-    cudaFree(h->d_pn0); cudaFree(h->d_pn1); cudaFree(h->d_wT); cudaFree(h->d_cell_kp); cudaFree(h->d_cell_km);
+    cudaFree(h->d_pn0); cudaFree(h->d_pn1); cudaFree(h->d_pn2); cudaFree(h->d_wT); cudaFree(h->d_cell_kp); cudaFree(h->d_cell_km);
     cudaFree(h->d_tile_pb); cudaFree(h->d_tile_qb); cudaFree(h->d_tile_wmap); cudaFree(h->d_steps); cudaFree(h->d_v); cudaFree(h->d_gpart);
     cudaFree(h->d_A); cudaFree(h->d_B); cudaFree(h->d_Bg); cudaFree(h->d_C); cudaFree(h->d_part);
     cudaFree(h->d_rho); cudaFree(h->d_blockred); cudaFree(h->d_scal);

@@ -7,6 +7,7 @@
 //   d=1: n = S p + sigma q,          A[p] = (z^S)^p,          B[q] = z^q       (q <= S/2)
 //   d=2: n = (p, sigma q),           A[p] = z0^p,             B[q] = z1^q
 //   d=3: n = (n0(p), n1(p), sigma q) A[p] = z0^n0 z1^n1,      B[q] = z2^q
+//   d=4: n = (n0, n1, n2, sigma q)(p) A[p] = z0^n0 z1^n1 z2^n2, B[q] = z3^q
 // so that rho(+/-)[p,q] = sum_j A_j[p] B_j[q]^(+/-) is a contraction over particles (rho pass) and
 // the gradient is a contraction over q followed by one over p (gradient pass).
 //
@@ -90,9 +91,9 @@ struct shd_ctx {
     // host copies
     std::vector<int> nvec;     // M * d
     std::vector<double> v;     // M (empty = all ones)
-    std::vector<int> pn0, pn1; // exponent of z0 (and z1 for d=3) of A entry p
+    std::vector<int> pn0, pn1, pn2; // exponent of z0 (and z1 for d>=3, z2 for d=4) of A entry p
     // device: setup tables
-    int *d_pn0 = nullptr, *d_pn1 = nullptr;
+    int *d_pn0 = nullptr, *d_pn1 = nullptr, *d_pn2 = nullptr;
     int *d_wT = nullptr;       // [3][P padded]: integer weight of Im(conj(A) T) for axis a
     int *d_cell_kp = nullptr, *d_cell_km = nullptr;   // [npb*32][Qpad] -> k or -1
     int *d_tile_pb = nullptr, *d_tile_qb = nullptr;   // [ntiles]

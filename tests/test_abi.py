@@ -43,7 +43,8 @@ def test_no_device_fails_loudly():
 def test_bad_arguments():
     from paper_2304_09139_b200 import shd
     h = ctypes.c_void_p()
-    assert shd.lib.shd_create_shell(4, 16, 4.0, 4, None, ctypes.byref(h)) == shd.SHD_EINVAL   # d = 4 (D:R14)
+    assert shd.lib.shd_create_shell(5, 16, 4.0, 4, None, ctypes.byref(h)) == shd.SHD_EINVAL   # d = 5 (D:R14)
+    assert shd.lib.shd_create_shell(0, 16, 4.0, 4, None, ctypes.byref(h)) == shd.SHD_EINVAL
     assert shd.lib.shd_create_shell(2, 0, 4.0, 4, None, ctypes.byref(h)) == shd.SHD_EINVAL
     assert shd.lib.shd_create_shell(2, 16, -1.0, 4, None, ctypes.byref(h)) == shd.SHD_EINVAL
     assert shd.lib.shd_create(2, 16, 4.0, float("nan"), None, ctypes.byref(h)) == shd.SHD_EINVAL

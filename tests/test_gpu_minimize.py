@@ -91,7 +91,8 @@ def test_max_evals_and_reentry(shd, oracle):
     h.close()
 
 
-@pytest.mark.parametrize("d,N,L,m_star,hist", [(1, 300, 300.0, 40 * 40, 5), (3, 216, 6.0, 14, 10), (2, 400, 20.0, 200, 32)])
+@pytest.mark.parametrize("d,N,L,m_star,hist", [(1, 300, 300.0, 40 * 40, 5), (3, 216, 6.0, 14, 10), (2, 400, 20.0, 200, 32),
+                                               (4, 256, 4.0, 5, 10)])
 def test_quench_other_dimensions(shd, oracle, d, N, L, m_star, hist):
     hi, lo = inputs.uniform_positions_raw(d, N, L, 11)
     h = shd.Shd(d, N, L, m_star=m_star)

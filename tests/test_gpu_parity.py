@@ -91,6 +91,7 @@ def test_cfg1_full(shd, oracle):
     (2, 63, 8.0, 15 * 15, 9), (2, 65, 8.0, 16 * 16, 10), (2, 129, 11.0, 17 * 17, 11),   # ragged 64-particle blocks, P = 16, 17, 18
     (2, 96, 300.0, 265 * 265, 12),                                    # q-range > 256: gradient blocks cut after 64 steps
     (1, 50, 50.0, 1100 * 1100, 13),                                   # d = 1, Qn > 256 as well
+    (4, 1, 2.0, 2, 14), (4, 81, 3.0, 3, 15), (4, 200, 3.8, 6, 16),    # d = 4
 ])
 def test_small_cases(shd, oracle, d, N, L, m_star, seed):
     hi, lo = inputs.uniform_positions_raw(d, N, L, seed)

@@ -34,7 +34,7 @@ def mp_rho(d, L, pos, nvec):
 
 
 # --------------------------------------------------------------------------- a0: Q
-@pytest.mark.parametrize("d,m_star", [(1, 49), (2, 2), (2, 49), (2, 5090), (3, 27), (3, 321)])
+@pytest.mark.parametrize("d,m_star", [(1, 49), (2, 2), (2, 49), (2, 5090), (3, 27), (3, 321), (4, 3), (4, 10)])
 def test_enumeration_count_order_halfspace(oracle, d, m_star):
     """of the 2M non-zero lattice vectors with n.n <= m*, M are independent."""
     n = oracle.enumerate_Q(d, m_star)
@@ -431,3 +431,33 @@ def test_structure_factor_closed_forms(oracle):
         S, dev2 = oracle.structure_factor(N, re, im)
         vals.append(oracle.to_float(dev2)[0] / M)
     assert 0.8 < np.mean(vals) < 1.2, vals
+
+
+def test_four_dimensions_direct_mode(oracle):
+    """d = 4 ("dimensions d = 1-4"): the direct-mode oracle is dimension-generic; pin it with the
+    single-site closed form, translation invariance of the gradient, a central finite difference of Phi
+    and the brute-force pair sum Phi = sum_k sum_{l,m} cos(k.(r_l - r_m))."""
+    d, N, L, m_star = 4, 6, 2.5, 3
+    n = oracle.enumerate_Q(d, m_star)
+    assert len(n) == 32                                   # (65 - 1) / 2 lattice points of the 4-ball
+    hi, lo = inputs.single_site(d, N, [0.3, 1.1, 2.2, 0.7])
+    r = oracle.energy_grad(d, N, L, hi, lo, n)
+    assert abs(oracle.to_float(r["phi"])[0] - N * N * len(n)) < 1e-9
+    assert np.abs(oracle.to_float(r["grad"])).max() < 1e-25
+    hi, lo = inputs.uniform_positions_raw(d, N, L, 9)
+    r = oracle.energy_grad(d, N, L, hi, lo, n)
+    g = oracle.to_float(r["grad"]).reshape(d, N)
+    assert np.abs(g.sum(axis=1)).max() < 1e-12
+    x = hi.reshape(d, N)
+    brute = 0.0
+    for k in n:
+        ph = 2 * np.pi * (k[:, None] * x).sum(axis=0) / L
+        brute += np.cos(ph[:, None] - ph[None, :]).sum()
+    assert abs(oracle.to_float(r["phi"])[0] - brute) < 1e-9 * brute
+    h = 1e-6
+    for (a, j) in ((0, 0), (3, 4), (2, 5)):
+        xp, xm = hi.copy(), hi.copy()
+        xp[a * N + j] += h; xm[a * N + j] -= h
+        fp = oracle.to_float(oracle.energy_grad(d, N, L, xp, lo, n, want_grad=False)["phi"])[0]
+        fm = oracle.to_float(oracle.energy_grad(d, N, L, xm, lo, n, want_grad=False)["phi"])[0]
+        assert abs((fp - fm) / (2 * h) - g[a, j]) < 1e-5 * (1 + abs(g[a, j]))
