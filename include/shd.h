@@ -190,6 +190,15 @@ double shd_stat(const shd_ctx* h, int what);
  */
 int shd_fp64_peak(int kind, double seconds, double instr_per_s[2]);
 
+/*
+ * INT8 tensor-core probe (an exact digit-sliced contraction on tcgen05.mma.kind::i8 would
+ * replace the FP64 limb FMAs).  HOST out: *mismatches = wrong entries of a 128 x 64 x 128 s8 x s8 -> s32 product
+ * computed by the 5th-generation tensor core (operands in shared memory, accumulator in TMEM) against the
+ * integer product on the host (0 = exact); *tops = measured issue rate of M=128, N=256, K=32 instructions on
+ * all SMs in tera-operations per second (2 per multiply-accumulate).  Needs no handle.
+ */
+int shd_i8_probe(double* tops, long* mismatches);
+
 #ifdef __cplusplus
 }
 #endif

@@ -5,6 +5,8 @@
 // 8 per thread); the result is thread-level FP64 instructions (FMAs) per second over the whole GPU.
 #include "../../include/shd.h"
 #include <cuda_runtime.h>
+#include <cstdint>
+#include <vector>
 
 namespace {
 
@@ -84,4 +86,145 @@ extern "C" int shd_fp64_peak(int kind, double seconds, double* instr_per_s)
     instr_per_s[0] = best;
     instr_per_s[1] = spent > 0.0 ? work / spent : 0.0;
     return SHD_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// INT8 tensor-core probe (exact digit-sliced contraction on tcgen05.mma.kind::i8).
+// (1) exactness: D(128 x 64, s32) = A(128 x 128, s8) B(64 x 128, s8)^T through UTCIMMA with the operands
+//     in shared memory (no swizzle, K-major core matrices), accumulator in TMEM, read back with
+//     tcgen05.ld and compared with the integer product on the host;
+// (2) rate: one CTA per SM issues M=128, N=256, K=32 instructions back to back from one thread.
+namespace {
+
+__device__ __forceinline__ uint32_t p_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+// shared-memory matrix descriptor: K-major, SWIZZLE_NONE; core matrix = 8 rows x 16 bytes (128 B contiguous),
+// K-adjacent core matrices 128 B apart (LBO), 8-row groups 256 B apart (SBO); version 1 (sm_100)
+__device__ __forceinline__ uint64_t p_desc(uint32_t addr) {
+    return (uint64_t)((addr >> 4) & 0x3FFF) | ((uint64_t)(128 >> 4) << 16) | ((uint64_t)(256 >> 4) << 32) | ((uint64_t)1 << 46);
+}
+// instruction descriptor of kind::i8: D = s32, A = B = s8, both K-major, N >> 3 at bit 17, M >> 4 at bit 24
+__device__ __forceinline__ uint32_t p_idesc(int m, int n) {
+    return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(m >> 4) << 24);
+}
+__device__ __forceinline__ void p_mma_i8(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+    uint32_t z = 0;
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %5, %5, %5}, p;\n\t}"
+                 ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate), "r"(z) : "memory");
+}
+__device__ __forceinline__ void p_wait(uint32_t bar) {
+    uint32_t ok = 0;
+    while (!ok)
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(bar) : "memory");
+}
+
+// MODE 0: exactness (KB = 4 K-blocks, N = 64, result to D); MODE 1: rate (iters x 4 instructions, N = 256)
+template <int MODE>
+__global__ void __launch_bounds__(128) k_i8_probe(const signed char* A, const signed char* B, int* D, int iters)
+{
+    constexpr int NN = MODE == 0 ? 64 : 256, KB = MODE == 0 ? 4 : 2, COLS = MODE == 0 ? 64 : 512;
+    __shared__ __align__(1024) signed char sA[KB][128 * 32];
+    __shared__ __align__(1024) signed char sB[KB][NN * 32];
+    __shared__ __align__(8) unsigned long long bar;
+    __shared__ uint32_t tmem_base;
+    const int tid = threadIdx.x, warp = tid >> 5;
+    if (MODE == 0) {
+        const int K = 32 * KB;
+        for (int i = tid; i < 128 * K; i += 128) {
+            int r = i / K, kk = i % K;
+            sA[kk / 32][(r / 8) * 256 + ((kk % 32) / 16) * 128 + (r % 8) * 16 + kk % 16] = A[i];
+        }
+        for (int i = tid; i < NN * K; i += 128) {
+            int r = i / K, kk = i % K;
+            sB[kk / 32][(r / 8) * 256 + ((kk % 32) / 16) * 128 + (r % 8) * 16 + kk % 16] = B[i];
+        }
+    } else {
+        for (int i = tid; i < KB * 128 * 32; i += 128) (&sA[0][0])[i] = (signed char)(i % 7 - 3);
+        for (int i = tid; i < KB * NN * 32; i += 128) (&sB[0][0])[i] = (signed char)(i % 5 - 2);
+    }
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(p_smem_u32(&bar)));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(p_smem_u32(&tmem_base)), "n"(COLS));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic-proxy smem writes -> UMMA reads
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const uint32_t tb = tmem_base;
+    if (tid == 0) {
+        const uint32_t idesc = p_idesc(128, NN);
+        for (int it = 0; it < (MODE == 0 ? 1 : iters); it++)
+#pragma unroll
+            for (int kb = 0; kb < (MODE == 0 ? KB : 4); kb++)
+                p_mma_i8(tb + (MODE == 1 && (it & 1) ? (uint32_t)NN : 0u), p_desc(p_smem_u32(&sA[kb % KB][0])),
+                         p_desc(p_smem_u32(&sB[kb % KB][0])), idesc, (it | kb) ? 1u : 0u);
+        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(p_smem_u32(&bar)) : "memory");
+    }
+    p_wait(p_smem_u32(&bar));
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    for (int c0 = 0; c0 < (MODE == 0 ? NN : 8); c0 += 8) {
+        uint32_t v[8];
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                     : "r"(tb + ((uint32_t)(warp * 32) << 16) + c0));
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        if (MODE == 0)
+            for (int i = 0; i < 8; i++) D[tid * NN + c0 + i] = (int)v[i];
+        else if (v[0] == 0x12345678u) D[0] = (int)v[1];
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tb), "n"(COLS));
+}
+
+}  // namespace
+
+extern "C" int shd_i8_probe(double* tops, long* mismatches)
+{
+    if (!tops || !mismatches) return SHD_EINVAL;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return SHD_ECUDA;
+    constexpr int M = 128, N = 64, K = 128;
+    std::vector<signed char> hA(M * K), hB(N * K);
+    unsigned s = 12345u;
+    for (auto& x : hA) { s = s * 1664525u + 1013904223u; x = (signed char)((s >> 24) & 0xff); }
+    for (auto& x : hB) { s = s * 1664525u + 1013904223u; x = (signed char)((s >> 24) & 0xff); }
+    signed char *dA = nullptr, *dB = nullptr;
+    int* dD = nullptr;
+    if (cudaMalloc((void**)&dA, M * K) != cudaSuccess || cudaMalloc((void**)&dB, N * K) != cudaSuccess ||
+        cudaMalloc((void**)&dD, M * N * sizeof(int)) != cudaSuccess) { cudaFree(dA); cudaFree(dB); cudaFree(dD); return SHD_ENOMEM; }
+    cudaMemcpy(dA, hA.data(), M * K, cudaMemcpyHostToDevice);
+    cudaMemcpy(dB, hB.data(), N * K, cudaMemcpyHostToDevice);
+    cudaMemset(dD, 0xff, M * N * sizeof(int));
+    k_i8_probe<0><<<1, 128>>>(dA, dB, dD, 1);
+    std::vector<int> hD(M * N);
+    cudaError_t e = cudaMemcpy(hD.data(), dD, M * N * sizeof(int), cudaMemcpyDeviceToHost);
+    long bad = 0;
+    for (int i = 0; i < M; i++)
+        for (int j = 0; j < N; j++) {
+            int ref = 0;
+            for (int k = 0; k < K; k++) ref += (int)hA[i * K + k] * (int)hB[j * K + k];
+            bad += ref != hD[i * N + j];
+        }
+    *mismatches = bad;
+    const int iters = 20000;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    k_i8_probe<1><<<prop.multiProcessorCount, 128>>>(dA, dB, dD, iters);
+    cudaEventRecord(e0, 0);
+    k_i8_probe<1><<<prop.multiProcessorCount, 128>>>(dA, dB, dD, iters);
+    cudaEventRecord(e1, 0);
+    if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    *tops = 2.0 * (double)prop.multiProcessorCount * iters * 4.0 * 128.0 * 256.0 * 32.0 / (ms * 1e-3) / 1e12;
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(dA); cudaFree(dB); cudaFree(dD);
+    return e == cudaSuccess ? SHD_OK : SHD_ECUDA;
 }

@@ -17,7 +17,7 @@ LIB_PATH = _HERE / "libshd.so"
 SHD_OK, SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA, SHD_ENAN, SHD_ESTALL, SHD_EMAXEVAL = 0, -1, -2, -3, -4, -5, -6
 EXPORTS = ["shd_create", "shd_create_shell", "shd_create_table", "shd_destroy", "shd_set_stream", "shd_num_k", "shd_get_k",
            "shd_energy_grad", "shd_energy_grad_host", "shd_set_timing", "shd_smax", "shd_last_smax", "shd_get_rho", "shd_minimize",
-           "shd_last_error", "shd_stat", "shd_fp64_peak", "shd_structure_factor", "shd_set_precision"]
+           "shd_last_error", "shd_stat", "shd_fp64_peak", "shd_structure_factor", "shd_set_precision", "shd_i8_probe"]
 
 
 class ShdError(RuntimeError):
@@ -66,6 +66,7 @@ def _load():
     lib.shd_fp64_peak.argtypes = [C.c_int, C.c_double, dp]
     lib.shd_structure_factor.argtypes = [vp, vp, dp]
     lib.shd_set_precision.argtypes = [vp, C.c_int]
+    lib.shd_i8_probe.argtypes = [dp, C.POINTER(C.c_long)]
     return lib
 
 
@@ -232,6 +233,16 @@ def fp64_peak(kind: int = 0, seconds: float = 1.0):
     if rc != SHD_OK:
         raise ShdError(rc, "shd_fp64_peak failed")
     return out[0], out[1]
+
+
+def i8_probe():
+    """shd_i8_probe: (measured INT8 tensor-core TOPS, number of wrong entries of the exactness check)."""
+    _torch()
+    tops, bad = C.c_double(0.0), C.c_long(-1)
+    rc = lib.shd_i8_probe(C.byref(tops), C.byref(bad))
+    if rc != SHD_OK:
+        raise ShdError(rc, "shd_i8_probe failed")
+    return tops.value, bad.value
 
 
 def from_host(hi: np.ndarray, lo: np.ndarray):

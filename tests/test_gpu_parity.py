@@ -308,3 +308,12 @@ def test_anisotropic_table(shd, oracle, d):
         with pytest.raises(shd.ShdError) as e:
             shd.Shd(d, N, L, table=np.array(bad, dtype=np.int32))
         assert e.value.code == shd.SHD_EINVAL
+
+
+def test_int8_tensor_core_probe(shd):
+    """shd_i8_probe: the 5th-generation tensor core multiplies s8 x s8 -> s32 exactly (the building block of
+    the digit-sliced contraction listed under DESIGN.md "next") and its measured rate is in the PFLOP range."""
+    tops, bad = shd.i8_probe()
+    print("INT8 UMMA:", tops, "TOPS, mismatches", bad)
+    assert bad == 0
+    assert tops > 1000.0
