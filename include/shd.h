@@ -121,6 +121,16 @@ int shd_get_rho(shd_ctx* h, double* re_hi, double* re_lo, double* im_hi, double*
 int shd_set_precision(shd_ctx* h, int limbs);
 
 /*
+ * Engine of the rho pass (step a2).  0 (default): exact FP64 limb contraction on the FP64 matrix instruction
+ * (k_rho.cu).  1: exact digit-sliced contraction on the INT8 tensor cores (tcgen05.mma.kind::i8, k_rho8.cu):
+ * operands as 13 balanced base-256 digits of trunc(x 2^102), the 91 digit pairs with i + l >= 12, s32
+ * accumulators in tensor memory (at most 8192 particles per CTA, so they are exact), the same double-double
+ * result within the same tolerances.  Applies to 3-limb evaluations (shd_set_precision 3); allocates the digit
+ * tables on first use.  Errors: SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA.
+ */
+int shd_set_engine(shd_ctx* h, int rho_engine);
+
+/*
  * Structure factor of the LAST evaluation on this handle (Eq. 3): S(k) = |rho(k)|^2 / N for every k
  * of the handle's Q, canonical order, into S_out (DEVICE, |Q| doubles; may be NULL), and
  * dev2 (HOST, (hi, lo)) = sum_{k in Q} (S(k) - 1)^2 in double-double, the lattice sum behind the order

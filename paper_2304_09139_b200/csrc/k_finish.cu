@@ -56,9 +56,9 @@ __device__ __forceinline__ void account(red& r, dd re, dd im, double v, long lon
 
 // one thread per (tile, cell)
 __global__ void __launch_bounds__(256) k_finish1(
-    const double* __restrict__ part, int nsplit, int ntiles, const int* __restrict__ tile_pb,
+    const double* __restrict__ part, int nsplit, int ntiles, int tp, int tq, const int* __restrict__ tile_pb,
     const int* __restrict__ tile_qb, const int* __restrict__ cell_kp, const int* __restrict__ cell_km,
-    int Qpad, long M, const double* __restrict__ v, double* __restrict__ rho, double* __restrict__ blockred,
+    int Ppad, int Qpad, long M, const double* __restrict__ v, double* __restrict__ rho, double* __restrict__ blockred,
     const int* __restrict__ skip)
 {
     if (skip && *skip) return;
@@ -66,8 +66,10 @@ __global__ void __launch_bounds__(256) k_finish1(
     red r; r.phi = dd{0, 0}; r.smax = dd{-1, 0}; r.arg = -1; r.maxvs = 0;
     if (idx < (long)ntiles * 1024) {
         int tile = (int)(idx >> 10), cell = (int)(idx & 1023);
-        int p = tile_pb[tile] * 32 + (cell >> 5), q = tile_qb[tile] * 32 + (cell & 31);
-        int kp = cell_kp[(size_t)p * Qpad + q], km = cell_km[(size_t)p * Qpad + q];
+        // tiles are tp x tq = 1024 cells: 32 x 32 (k_rho) or 64 x 16 (k_rho8)
+        int p = tile_pb[tile] * tp + cell / tq, q = tile_qb[tile] * tq + cell % tq;
+        const bool inside = p < Ppad && q < Qpad;
+        int kp = inside ? cell_kp[(size_t)p * Qpad + q] : -1, km = inside ? cell_km[(size_t)p * Qpad + q] : -1;
         if (kp >= 0 || km >= 0) {
             const double2* src = reinterpret_cast<const double2*>(part);
             dd X[4];
@@ -227,10 +229,13 @@ cudaError_t shd_launch_sfactor(shd_ctx* h, double* S_out, double* scratch, doubl
 
 cudaError_t shd_launch_finish(shd_ctx* h)
 {
-    int nb = h->nfinish_blocks;
-    k_finish1<<<nb, 256, 0, h->stream>>>(h->d_part, h->nsplit, h->ntiles, h->d_tile_pb, h->d_tile_qb,
-                                         h->d_cell_kp, h->d_cell_km, h->Qpad, h->M, h->d_v, h->d_rho,
-                                         h->d_blockred, h->d_skip);
+    const bool i8 = h->rho_engine == 1 && h->nlimb >= 3;
+    const int ntiles = i8 ? h->ntiles8 : h->ntiles;
+    const int nb = (int)(((long)ntiles * 1024 + 255) / 256);
+    k_finish1<<<nb, 256, 0, h->stream>>>(h->d_part, i8 ? h->nsplit8 : h->nsplit, ntiles, i8 ? SHD_I8_PT : 32,
+                                         i8 ? SHD_I8_QT : 32, i8 ? h->d_tile8_pb : h->d_tile_pb,
+                                         i8 ? h->d_tile8_qb : h->d_tile_qb, h->d_cell_kp, h->d_cell_km,
+                                         h->npb * 32, h->Qpad, h->M, h->d_v, h->d_rho, h->d_blockred, h->d_skip);
     k_finish2<<<1, 1024, 0, h->stream>>>(h->d_blockred, nb, h->N, h->d_scal, h->d_skip);
     h->last_launches += 2;
     return cudaGetLastError();

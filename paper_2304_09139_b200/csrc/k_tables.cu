@@ -52,6 +52,25 @@ __device__ cdd expi_turns(dd t) {
 
 struct limbs { double x0, x1, x2; };
 
+// trunc(x 2^102) of a double as a 128-bit integer (|x| <= 2), integer pipe only
+__device__ __forceinline__ __int128 fix102(double x) {
+    const long long b = __double_as_longlong(x);
+    const int e = (int)((b >> 52) & 0x7ff);
+    if (e == 0) return 0;
+    const unsigned long long m = ((unsigned long long)b & 0xfffffffffffffULL) | (1ULL << 52);
+    const int sh = e - 1075 + 102;                       // x = m 2^(e - 1075)
+    __int128 v = sh >= 0 ? ((__int128)m << sh) : (sh > -64 ? (__int128)(m >> (-sh)) : (__int128)0);
+    return b < 0 ? -v : v;
+}
+// the 13 balanced base-256 digits d_i in [-128, 127] of X = trunc(hi 2^102) + trunc(lo 2^102): bytes of
+// X + sum_i 128 256^i, minus 128 (no carries); sum_i d_i 256^i = X exactly
+__device__ __forceinline__ void digits13(dd x, signed char* d) {
+    const __int128 off = ((__int128)0x0000008080808080ULL << 64) | (__int128)0x8080808080808080ULL;
+    const unsigned __int128 y = (unsigned __int128)(fix102(x.h) + fix102(x.l) + off);
+#pragma unroll
+    for (int i = 0; i < SHD_I8_DIGITS; i++) d[i] = (signed char)((int)((y >> (8 * i)) & 0xff) - 128);
+}
+
 // |x| <= 1 (normalised dd) -> limbs (shd_internal.h)
 __device__ __forceinline__ limbs split_limbs(dd x) {
     const double C0 = 1.5 * 4503599627370496.0 / (double)(1 << SHD_W0);                 // 1.5 * 2^(52-W0)
@@ -83,6 +102,27 @@ struct Stager {
     double* Bg;           // gradient layout (or nullptr)
     long Npad, j0, N;
     int Qpad;
+    signed char* dig;     // digit table of the INT8 rho pass (or nullptr)
+    long nk8;             // K-steps (32 particles) per block of that table
+    int rows8;            // entries per block: 64 (A) or 16 (B)
+    // s8 digits of entry e of this thread's particle: row r = 2 (e % rows8) + re/im of block e / rows8,
+    // K index = particle % 32, in the K-major core-matrix layout the tensor core reads (8 rows x 16 bytes
+    // per core matrix, K-adjacent core matrices 128 B apart, 8-row groups 256 B apart)
+    __device__ __forceinline__ void put8(int e, cdd z, bool live) {
+        if (dig == nullptr || !live) return;
+        const long j = j0 + threadIdx.x;
+        const int k = (int)(j & 31);
+        const size_t slab = (size_t)rows8 * 2 * 32;                    // bytes of one digit of one (block, K-step)
+        signed char* base = dig + (((size_t)(e / rows8) * nk8 + (size_t)(j >> 5)) * SHD_I8_DIGITS) * slab;
+        signed char dr[SHD_I8_DIGITS], di[SHD_I8_DIGITS];
+        digits13(z.re, dr);
+        digits13(z.im, di);
+        const int r0 = 2 * (e % rows8), r1 = r0 + 1;
+        const int o0 = (r0 >> 3) * 256 + (k >> 4) * 128 + (r0 & 7) * 16 + (k & 15);
+        const int o1 = (r1 >> 3) * 256 + (k >> 4) * 128 + (r1 & 7) * 16 + (k & 15);
+#pragma unroll
+        for (int i = 0; i < SHD_I8_DIGITS; i++) { base[(size_t)i * slab + o0] = dr[i]; base[(size_t)i * slab + o1] = di[i]; }
+    }
     __device__ __forceinline__ static int swz(int r) { return ((r & 1) << 2) | (r & 2) | ((r >> 2) & 1); }
     __device__ __forceinline__ void put(int plane0, int slot, cdd z) {
         limbs a = split_limbs(z.re), b = split_limbs(z.im);
@@ -135,6 +175,7 @@ __global__ void __launch_bounds__(TB) k_tables(
     const int* __restrict__ pn0, const int* __restrict__ pn1, const int* __restrict__ pn2, int Qpad,
     const double* __restrict__ pos_hi, const double* __restrict__ pos_lo,
     double* __restrict__ A, double* __restrict__ B, double* __restrict__ Bg, int with_grad,
+    signed char* __restrict__ A8, signed char* __restrict__ B8, long nk8,
     const int* __restrict__ skip)
 {
     if (skip && *skip) return;
@@ -147,7 +188,8 @@ __global__ void __launch_bounds__(TB) k_tables(
     const long jc = live ? j : N - 1;            // dead threads shadow the last particle (keeps barriers uniform)
     const cdd one{dd{1.0, 0.0}, dd{0.0, 0.0}};
     const bool gradB = which == 1 && with_grad != 0;
-    Stager st{tile, 3, which == 0 ? A : B, gradB ? Bg : nullptr, Npad, j0, N, Qpad};
+    Stager st{tile, 3, which == 0 ? A : B, gradB ? Bg : nullptr, Npad, j0, N, Qpad,
+              which == 0 ? A8 : B8, nk8, which == 0 ? SHD_I8_PT : SHD_I8_QT};
     if (which == 0) {
         // ---- A table
         cdd base;
@@ -159,6 +201,7 @@ __global__ void __launch_bounds__(TB) k_tables(
                 const int cnt = min(TG, P - p0);
                 for (int s = 0; s < cnt; s++) {
                     st.put(0, s, cur);
+                    st.put8(p0 + s, cur, live);
                     cur = cdd_mul(cur, base);
                 }
                 st.flush(p0, cnt);
@@ -190,7 +233,9 @@ __global__ void __launch_bounds__(TB) k_tables(
                         const int n2 = pn2[p0 + s];
                         f = cdd_mul(f, n2 >= 0 ? pw2[n2] : cdd_conj(pw2[-n2]));
                     }
-                    st.put(0, s, cdd_mul(cur0, f));
+                    const cdd az = cdd_mul(cur0, f);
+                    st.put(0, s, az);
+                    st.put8(p0 + s, az, live);
                 }
                 st.flush(p0, cnt);
             }
@@ -204,6 +249,7 @@ __global__ void __launch_bounds__(TB) k_tables(
             const int cnt = min(TG, Qn - q0);
             for (int s = 0; s < cnt; s++) {
                 st.put(0, s, cur);
+                st.put8(q0 + s, cur, live);
                 cur = cdd_mul(cur, base);
             }
             st.flush(q0, cnt);
@@ -223,7 +269,9 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
     dim3 grid((unsigned)((h->N + TB - 1) / TB), 2);
     k_tables<<<grid, TB, TABLES_SMEM, h->stream>>>(h->d, h->N, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2,
                                          h->d_pn0, h->d_pn1, h->d_pn2, h->Qpad, pos_hi, pos_lo,
-                                         h->d_A, h->d_B, h->d_Bg, with_grad_tables ? 1 : 0, h->d_skip);
+                                         h->d_A, h->d_B, h->d_Bg, with_grad_tables ? 1 : 0,
+                                         h->rho_engine == 1 && h->nlimb >= 3 ? h->d_A8 : nullptr,
+                                         h->rho_engine == 1 && h->nlimb >= 3 ? h->d_B8 : nullptr, h->nk8, h->d_skip);
     h->last_launches += 1;
     return cudaGetLastError();
 }

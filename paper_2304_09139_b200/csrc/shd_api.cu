@@ -302,7 +302,8 @@ int build(shd_ctx* h, const double* v) {
     if ((rc = dalloc_zero(h, &h->d_Bg, (size_t)(2 * h->njb64) * (h->Qpad / 4) * SHD_GROUP_DOUBLES))) return rc;
     if ((rc = dalloc_zero(h, &h->d_C, (size_t)h->npb16 * (h->Qpad / 4) * (16 * SHD_PG * 4 * 2)))) return rc;
     if ((rc = dalloc_zero(h, &h->d_gpart, (size_t)h->nseg * h->d * h->N * 2))) return rc;
-    if ((rc = dalloc_zero(h, &h->d_part, (size_t)h->nsplit * h->ntiles * 4 * 1024 * 2))) return rc;
+    h->part_doubles = (size_t)h->nsplit * h->ntiles * 4 * 1024 * 2;
+    if ((rc = dalloc_zero(h, &h->d_part, h->part_doubles))) return rc;
     if ((rc = dalloc_zero(h, &h->d_rho, (size_t)4 * h->M))) return rc;
     h->nfinish_blocks = (int)(((long)h->ntiles * 1024 + 255) / 256);
     if ((rc = dalloc_zero(h, &h->d_blockred, (size_t)h->nfinish_blocks * 8))) return rc;
@@ -380,7 +381,7 @@ int run_rho(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool with_gr
     if ((rc = mark(h, 0))) return rc;
     CU(shd_launch_tables(h, pos_hi, pos_lo, with_grad));
     if ((rc = mark(h, 1))) return rc;
-    CU(shd_launch_rho(h));
+    if (h->rho_engine == 1 && h->nlimb >= 3) CU(shd_launch_rho8(h)); else CU(shd_launch_rho(h));
     if ((rc = mark(h, 2))) return rc;
     CU(shd_launch_finish(h));
     if ((rc = mark(h, 3))) return rc;
@@ -422,6 +423,7 @@ void shd_destroy(shd_ctx* h) {
     cudaFree(h->d_A); cudaFree(h->d_B); cudaFree(h->d_Bg); cudaFree(h->d_C); cudaFree(h->d_part);
     cudaFree(h->d_rho); cudaFree(h->d_blockred); cudaFree(h->d_scal);
     cudaFree(h->d_hpos); cudaFree(h->d_hgrad);
+    cudaFree(h->d_A8); cudaFree(h->d_B8); cudaFree(h->d_tile8_pb); cudaFree(h->d_tile8_qb);
     for (int i = 0; i <= SHD_NKERN; i++) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     if (h->h_scal) cudaFreeHost(h->h_scal);
     if (h->gevent) cudaEventDestroy(h->gevent);
@@ -541,6 +543,71 @@ int shd_set_precision(shd_ctx* h, int limbs) {
     return SHD_OK;
 }
 
+// engine 1: build the tile list, the particle splits and the digit tables of the INT8 rho pass (k_rho8.cu)
+int shd_set_engine(shd_ctx* h, int rho_engine) {
+    if (!h) return SHD_EINVAL;
+    if (rho_engine != 0 && rho_engine != 1) return fail(h, SHD_EINVAL, "shd_set_engine: rho_engine must be 0 or 1");
+    if (rho_engine == 1 && !h->d_A8) {
+        h->npb64 = (h->P + SHD_I8_PT - 1) / SHD_I8_PT;
+        h->nqb16 = (h->Qn + SHD_I8_QT - 1) / SHD_I8_QT;
+        std::vector<int> kp((size_t)h->npb * 32 * h->Qpad), km(kp.size());
+        CU(cudaMemcpy(kp.data(), h->d_cell_kp, kp.size() * sizeof(int), cudaMemcpyDeviceToHost));
+        CU(cudaMemcpy(km.data(), h->d_cell_km, km.size() * sizeof(int), cudaMemcpyDeviceToHost));
+        std::vector<int> tpb, tqb;
+        for (int pb = 0; pb < h->npb64; pb++)
+            for (int qb = 0; qb < h->nqb16; qb++) {
+                bool any = false;
+                for (int pi = 0; pi < SHD_I8_PT && !any; pi++)
+                    for (int qi = 0; qi < SHD_I8_QT && !any; qi++) {
+                        const int p = pb * SHD_I8_PT + pi, q = qb * SHD_I8_QT + qi;
+                        if (p < h->npb * 32 && q < h->Qpad) any = kp[(size_t)p * h->Qpad + q] >= 0 || km[(size_t)p * h->Qpad + q] >= 0;
+                    }
+                if (any) { tpb.push_back(pb); tqb.push_back(qb); }
+            }
+        h->ntiles8 = (int)tpb.size();
+        // particle splits: at most SHD_I8_MAXN particles per CTA (exact s32 sums); minimise waves x (K-steps + epilogue)
+        cudaDeviceProp prop;
+        int dev = 0;
+        cudaGetDevice(&dev);
+        CU(cudaGetDeviceProperties(&prop, dev));
+        const long sms = prop.multiProcessorCount, nk = (h->N + 31) / 32;
+        double best = -1.0;
+        for (long ns = (h->N + SHD_I8_MAXN - 1) / SHD_I8_MAXN; ns <= std::min<long>(512, nk); ns++) {
+            const long per = (nk + ns - 1) / ns, waves = ((long)h->ntiles8 * ns + sms - 1) / sms;
+            const double cost = (double)waves * ((double)per + 8.0) + 0.004 * (double)ns * h->ntiles8;
+            if (best < 0.0 || cost < best) { best = cost; h->nsplit8 = (int)ns; h->ksteps8 = (int)per; }
+        }
+        h->nk8 = (long)h->nsplit8 * h->ksteps8;
+        const size_t a8 = (size_t)h->npb64 * h->nk8 * SHD_I8_DIGITS * (SHD_I8_PT * 2 * 32);
+        const size_t b8 = (size_t)h->nqb16 * h->nk8 * SHD_I8_DIGITS * (SHD_I8_QT * 2 * 32);
+        CU(cudaMalloc((void**)&h->d_A8, a8));
+        CU(cudaMalloc((void**)&h->d_B8, b8));
+        CU(cudaMemset(h->d_A8, 0, a8));
+        CU(cudaMemset(h->d_B8, 0, b8));
+        h->workspace_bytes += a8 + b8;
+        int rc;
+        if ((rc = upload(h, &h->d_tile8_pb, tpb))) return rc;
+        if ((rc = upload(h, &h->d_tile8_qb, tqb))) return rc;
+        const size_t need = (size_t)h->nsplit8 * h->ntiles8 * 4 * 1024 * 2;
+        if (need > h->part_doubles) {
+            cudaFree(h->d_part);
+            h->d_part = nullptr;
+            if ((rc = dalloc_zero(h, &h->d_part, need))) return rc;
+            h->part_doubles = need;
+        }
+        const int nb = (int)(((long)std::max(h->ntiles, h->ntiles8) * 1024 + 255) / 256);
+        if (nb > h->nfinish_blocks) {
+            cudaFree(h->d_blockred);
+            h->d_blockred = nullptr;
+            if ((rc = dalloc_zero(h, &h->d_blockred, (size_t)nb * 8))) return rc;
+            h->nfinish_blocks = nb;
+        }
+        CU(shd_rho8_configure());
+    }
+    h->rho_engine = rho_engine;
+    return SHD_OK;
+}
+
 int shd_structure_factor(shd_ctx* h, double* S_out, double dev2[2]) {
     if (!h) return SHD_EINVAL;
     if (!dev2) return fail(h, SHD_EINVAL, "NULL pointer");
@@ -575,6 +642,9 @@ double shd_stat(const shd_ctx* h, int what) {
         case 10: return (double)h->njb;
         case 11: return (double)h->grad_qsteps;
         case 13: return (double)h->nseg;
+        case 14: return (double)h->ntiles8;
+        case 15: return (double)h->nsplit8;
+        case 16: return (double)h->rho_engine;
         case 20: case 21: case 22: case 23: case 24: return (double)h->kern_ms[what - 20];
         default: return 0.0;
     }

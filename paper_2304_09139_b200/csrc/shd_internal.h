@@ -45,6 +45,10 @@ constexpr int SHD_PG = 16;          // p per gradient-pass block
 constexpr int SHD_W0 = 22;          // limb widths (bits)
 constexpr int SHD_W1 = 22;
 constexpr int SHD_NLIMB = 3;
+constexpr int SHD_I8_DIGITS = 13;   // balanced base-256 digits of trunc(x 2^102) (INT8 tensor-core rho pass, k_rho8.cu)
+constexpr int SHD_I8_PT = 64;       // p per tile of that pass
+constexpr int SHD_I8_QT = 16;       // q per tile
+constexpr int SHD_I8_MAXN = 8192;   // particles per CTA: 13 pairs x 8192 x 2^14 < 2^31 keeps the s32 sums exact
 constexpr int SHD_GROUP_DOUBLES = SHD_NLIMB * 32 * 4 * 2;   // one (block, group of 4) slab of A / B: 6 KB
 constexpr int SHD_GGROUP_DOUBLES = 2 * SHD_GROUP_DOUBLES;   // gradient operands: 6 planes (Bg: b, q b; C: C1, C2)
 
@@ -71,6 +75,7 @@ struct shd_ctx {
     double L = 0;
     long m_star = 0;
     long M = 0;
+    int rho_engine = 0;        // 0: FP64 limbs on DMMA (k_rho.cu); 1: s8 digits on tcgen05 (k_rho8.cu); shd_set_engine
     int nlimb = 3;             // 3: double-double products; 2: "fast" 44-bit operands (shd_set_precision)
     // decomposition
     int P = 0, Qn = 0, npb = 0, nqb = 0;
@@ -108,6 +113,13 @@ struct shd_ctx {
     double *d_Bg = nullptr;    // [2 njb64][Qpad/4][3 limbs of b][32 j][4 q][2]
     double *d_C = nullptr;     // [npb16][Qpad/4][16 planes: C1, C2, D1 = q C2, D2 = -q C1, each limbs + (x1+x2)][16 p][4 q][2]
     double *d_gpart = nullptr; // [nseg][d][N] (hi, lo): partial gradients of the segments
+    // INT8 rho pass (allocated by shd_set_engine(h, 1))
+    signed char *d_A8 = nullptr;   // [npb64][nk8][13 digits][128 rows (p, re/im) x 32 particles, core-matrix layout]
+    signed char *d_B8 = nullptr;   // [nqb16][nk8][13 digits][ 32 rows (q, re/im) x 32 particles]
+    int *d_tile8_pb = nullptr, *d_tile8_qb = nullptr;
+    int ntiles8 = 0, nsplit8 = 0, ksteps8 = 0, npb64 = 0, nqb16 = 0;
+    long nk8 = 0;                  // nsplit8 * ksteps8: K-steps (32 particles) in the digit tables
+    size_t part_doubles = 0;       // capacity of d_part
     double *d_part = nullptr;  // [nsplit][ntiles][4][1024][2]
     double *d_rho = nullptr;   // [4][M]: re_hi, re_lo, im_hi, im_lo
     double *d_blockred = nullptr;   // per-block partials of the finish kernel
@@ -136,6 +148,8 @@ struct shd_ctx {
 // kernels / launchers (each returns the cudaError of its launches)
 cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool with_grad_tables);
 cudaError_t shd_launch_rho(shd_ctx* h);
+cudaError_t shd_launch_rho8(shd_ctx* h);
+cudaError_t shd_rho8_configure();
 cudaError_t shd_launch_finish(shd_ctx* h);
 cudaError_t shd_launch_ctable(shd_ctx* h);
 cudaError_t shd_launch_sfactor(shd_ctx* h, double* S_out, double* scratch, double* tau2);

@@ -17,7 +17,7 @@ LIB_PATH = _HERE / "libshd.so"
 SHD_OK, SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA, SHD_ENAN, SHD_ESTALL, SHD_EMAXEVAL = 0, -1, -2, -3, -4, -5, -6
 EXPORTS = ["shd_create", "shd_create_shell", "shd_create_table", "shd_destroy", "shd_set_stream", "shd_num_k", "shd_get_k",
            "shd_energy_grad", "shd_energy_grad_host", "shd_set_timing", "shd_smax", "shd_last_smax", "shd_get_rho", "shd_minimize",
-           "shd_last_error", "shd_stat", "shd_fp64_peak", "shd_structure_factor", "shd_set_precision", "shd_i8_probe"]
+           "shd_last_error", "shd_stat", "shd_fp64_peak", "shd_structure_factor", "shd_set_precision", "shd_i8_probe", "shd_set_engine"]
 
 
 class ShdError(RuntimeError):
@@ -67,6 +67,7 @@ def _load():
     lib.shd_structure_factor.argtypes = [vp, vp, dp]
     lib.shd_set_precision.argtypes = [vp, C.c_int]
     lib.shd_i8_probe.argtypes = [dp, C.POINTER(C.c_long)]
+    lib.shd_set_engine.argtypes = [vp, C.c_int]
     return lib
 
 
@@ -193,6 +194,10 @@ class Shd:
     def set_precision(self, limbs: int):
         """shd_set_precision: 3 = double-double products (default), 2 = 44-bit operands, 1 = 22-bit operands."""
         self._check(lib.shd_set_precision(self._h, int(limbs)))
+
+    def set_engine(self, rho_engine: int):
+        """shd_set_engine: 0 = FP64 DMMA rho pass, 1 = INT8 tensor-core rho pass (tcgen05)."""
+        self._check(lib.shd_set_engine(self._h, int(rho_engine)))
 
     def structure_factor(self, want_S=True):
         """shd_structure_factor on the last evaluation: (S device tensor or None, (hi, lo) of

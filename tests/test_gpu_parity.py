@@ -317,3 +317,56 @@ def test_int8_tensor_core_probe(shd):
     print("INT8 UMMA:", tops, "TOPS, mismatches", bad)
     assert bad == 0
     assert tops > 1000.0
+
+
+@pytest.mark.parametrize("d,N,L,m_star,seed", [
+    (2, 128, 128 ** 0.5, 49, 0), (2, 500, 22.0, 1300, 6), (2, 65, 8.0, 16 * 16, 10), (2, 96, 300.0, 265 * 265, 12),
+    (1, 300, 300.0, 700 * 700, 4), (3, 130, 5.1, 50, 7), (4, 81, 3.0, 3, 15), (2, 1, 3.0, 9, 1),
+])
+def test_int8_engine_small_cases(shd, oracle, d, N, L, m_star, seed):
+    """shd_set_engine(h, 1): the rho pass as an exact digit-sliced contraction on the INT8 tensor cores
+    (tcgen05.mma.kind::i8, s32 sums in tensor memory) against the oracle, same tolerances as the FP64 engine."""
+    hi, lo = inputs.uniform_positions_raw(d, N, L, seed)
+    lo = inputs.jitter_lo(hi, seed + 100)
+    h = shd.Shd(d, N, L, m_star=m_star)
+    h.set_engine(1)
+    th, tl = shd.from_host(hi, lo)
+    phi, gh, gl = h.energy_grad(th, tl)
+    rho = [t.cpu().numpy() for t in h.rho()]
+    smax, arg = h.last_smax()
+    g = dict(phi=phi, grad_hi=gh.cpu().numpy(), grad_lo=gl.cpu().numpy(), rho=rho, smax=smax, argmax=arg, k=h.k(), M=h.M)
+    print(compare(oracle, d, N, L, m_star, hi, lo, g))
+    h.close()
+
+
+def test_int8_engine_full_size_and_determinism(shd, oracle):
+    """BASELINE.json configs[3] on the INT8 engine: sampled rho against the direct-mode oracle, agreement
+    with the FP64 engine at the double-double level, 30 bit-identical repeats."""
+    import torch
+    cfg = inputs.CONFIGS["cfg4"]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    lo = inputs.jitter_lo(hi, 7)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    th, tl = shd.from_host(hi, lo)
+    gh, gl = torch.empty_like(th), torch.empty_like(th)
+    phi0, _, _ = h.energy_grad(th, tl, gh, gl)
+    rho0 = [x.cpu().numpy() for x in h.rho()]
+    h.set_engine(1)
+    phi1, _, _ = h.energy_grad(th, tl, gh, gl)
+    ref = [gh.clone(), gl.clone()] + [x.clone() for x in h.rho()]
+    rho1 = [x.cpu().numpy() for x in ref[2:]]
+    e = oracle.cabsdiff_dd(oracle.from_dd(rho0[0], rho0[1]), oracle.from_dd(rho0[2], rho0[3]), *rho1)
+    assert e.max() <= RHO_TIGHT * np.sqrt(cfg.N) * (1 + 239 / 64)
+    assert abs(phi1[0] - phi0[0]) <= 1e-15 * abs(phi0[0])
+    n = oracle.enumerate_Q(cfg.d, cfg.m_star)
+    ks = np.unique(np.linspace(0, cfg.M - 1, 48).astype(np.int64))
+    re, im = oracle.rho(cfg.d, cfg.N, cfg.L, hi, lo, n[ks])
+    eo = oracle.cabsdiff_dd(re, im, *[x[ks] for x in rho1])
+    print("int8 engine cfg4: vs FP64 engine", e.max(), "vs oracle", eo.max())
+    assert eo.max() <= 1e-28 * cfg.N and eo.max() <= RHO_TIGHT * np.sqrt(cfg.N) * (1 + 239 / 64)
+    for rep in range(30):
+        phi, _, _ = h.energy_grad(th, tl, gh, gl)
+        assert phi == phi1
+        for x, y in zip(ref, [gh, gl] + list(h.rho())):
+            assert torch.equal(x, y), rep
+    h.close()
