@@ -14,7 +14,7 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libshd.so"
-SOURCES = ["shd_api.cu", "k_tables.cu", "k_rho.cu", "k_rho8.cu", "k_finish.cu", "k_grad.cu", "shd_min.cu", "shd_fire.cu", "k_probe.cu"]
+SOURCES = ["shd_api.cu", "k_tables.cu", "k_rho.cu", "k_rho8.cu", "k_finish.cu", "k_grad.cu", "k_grad8.cu", "shd_min.cu", "shd_fire.cu", "k_probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--fmad=false", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 

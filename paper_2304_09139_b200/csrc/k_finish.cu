@@ -188,6 +188,70 @@ __global__ void __launch_bounds__(256) k_ctable(
     }
 }
 
+// Shared operand of the INT8 gradient pass (k_grad8.cu): W[(p, out), (q, c)] with out = T re, T im, T'' re,
+// T'' im and c = re, im of b:  (C1r, C2r), (C1i, C2i), (D1r, D2r), (D1i, D2i), as 13 s8 digits of
+// trunc(x 2^102), layout [pb8][q/16][digit][32 rows (4 p%8 + out) x 32 K (2 (q%16) + c)] in the tensor
+// core's K-major core-matrix layout.  One thread per (p, q).
+__device__ __forceinline__ __int128 f_fix102(double x) {
+    const long long b = __double_as_longlong(x);
+    const int e = (int)((b >> 52) & 0x7ff);
+    if (e == 0) return 0;
+    const unsigned long long m = ((unsigned long long)b & 0xfffffffffffffULL) | (1ULL << 52);
+    const int sh = e - 1075 + 102;
+    __int128 v = sh >= 0 ? ((__int128)m << sh) : (sh > -64 ? (__int128)(m >> (-sh)) : (__int128)0);
+    return b < 0 ? -v : v;
+}
+__global__ void __launch_bounds__(256) k_wtable8(
+    int npb8, int Ppad, int Qpad, int qscale_log2, const int* __restrict__ cell_kp, const int* __restrict__ cell_km,
+    long M, const double* __restrict__ v, const double* __restrict__ rho, const shd_scalars* __restrict__ scal,
+    signed char* __restrict__ W8, const int* __restrict__ skip)
+{
+    if (skip && *skip) return;
+    const long idx = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int nkq = Qpad / 16;
+    if (idx >= (long)npb8 * 8 * Qpad) return;
+    // idx enumerates (pb8, q/16, p%8, q%16), q%16 fastest
+    const int ql = (int)(idx & 15), pl = (int)((idx >> 4) & 7);
+    const long t = idx >> 7;
+    const int kq = (int)(t % nkq), pb = (int)(t / nkq);
+    const int p = pb * 8 + pl, q = kq * 16 + ql;
+    int kp = -1, km = -1;
+    if (p < Ppad) { kp = cell_kp[(size_t)p * Qpad + q]; km = cell_km[(size_t)p * Qpad + q]; }
+    const double sc = scal->cscale;
+    dd wpr{0, 0}, wpi{0, 0}, wmr{0, 0}, wmi{0, 0};
+    if (kp >= 0) {
+        double vv = v ? v[kp] : 1.0;
+        wpr = dd_scale2(dd_mul_d(dd{rho[kp], rho[M + kp]}, vv), sc);
+        wpi = dd_scale2(dd_mul_d(dd{rho[2 * M + kp], rho[3 * M + kp]}, vv), sc);
+    }
+    if (km >= 0) {
+        double vv = v ? v[km] : 1.0;
+        wmr = dd_scale2(dd_mul_d(dd{rho[km], rho[M + km]}, vv), sc);
+        wmi = dd_scale2(dd_mul_d(dd{rho[2 * M + km], rho[3 * M + km]}, vv), sc);
+    }
+    dd op[4][2];
+    op[0][0] = dd_add(wpr, wmr); op[0][1] = dd_add(wpi, wmi);                 // C1
+    const dd dr = dd_sub(wpr, wmr), di = dd_sub(wpi, wmi);
+    op[1][0] = di; op[1][1] = dd_neg(dr);                                     // C2
+    const double qw = ldexp((double)q, -qscale_log2);
+    op[2][0] = dd_mul_d(op[1][0], qw); op[2][1] = dd_mul_d(op[1][1], qw);     // D1 =  q C2
+    op[3][0] = dd_mul_d(op[0][0], -qw); op[3][1] = dd_mul_d(op[0][1], -qw);   // D2 = -q C1
+    // rows: out 0 = T re: (C1r, C2r); 1 = T im: (C1i, C2i); 2 = T'' re: (D1r, D2r); 3 = T'' im: (D1i, D2i)
+    signed char* base = W8 + ((size_t)pb * nkq + kq) * (SHD_I8_DIGITS * 1024);
+    const __int128 off = ((__int128)0x0000008080808080ULL << 64) | (__int128)0x8080808080808080ULL;
+#pragma unroll
+    for (int out = 0; out < 4; out++)
+#pragma unroll
+        for (int c = 0; c < 2; c++) {
+            const dd x = op[2 * (out >> 1) + c][out & 1];
+            const unsigned __int128 y = (unsigned __int128)(f_fix102(x.h) + f_fix102(x.l) + off);
+            const int row = 4 * pl + out, k = 2 * ql + c;
+            const int o = (row >> 3) * 256 + (k >> 4) * 128 + (row & 7) * 16 + (k & 15);
+#pragma unroll
+            for (int i = 0; i < SHD_I8_DIGITS; i++) base[i * 1024 + o] = (signed char)((int)((y >> (8 * i)) & 0xff) - 128);
+        }
+}
+
 // NEXT-3 (Eq. 7, Eq. 3): S(k) = |rho(k)|^2 / N for every k of the handle's Q, and the
 // sum over Q of (S(k) - 1)^2 that the order metric tau integrates, in double-double, fixed tree.
 __global__ void __launch_bounds__(256) k_sfactor1(long M, long N, const double* __restrict__ rho,
@@ -229,7 +293,7 @@ cudaError_t shd_launch_sfactor(shd_ctx* h, double* S_out, double* scratch, doubl
 
 cudaError_t shd_launch_finish(shd_ctx* h)
 {
-    const bool i8 = h->rho_engine == 1 && h->nlimb >= 3;
+    const bool i8 = h->rho_engine >= 1 && h->nlimb >= 3;
     const int ntiles = i8 ? h->ntiles8 : h->ntiles;
     const int nb = (int)(((long)ntiles * 1024 + 255) / 256);
     k_finish1<<<nb, 256, 0, h->stream>>>(h->d_part, i8 ? h->nsplit8 : h->nsplit, ntiles, i8 ? SHD_I8_PT : 32,
@@ -241,8 +305,20 @@ cudaError_t shd_launch_finish(shd_ctx* h)
     return cudaGetLastError();
 }
 
+cudaError_t shd_launch_wtable8(shd_ctx* h);
+cudaError_t shd_launch_wtable8(shd_ctx* h)
+{
+    const long n = (long)h->npb8 * 8 * h->Qpad;
+    k_wtable8<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(
+        h->npb8, h->npb * 32, h->Qpad, h->qscale_log2, h->d_cell_kp, h->d_cell_km, h->M, h->d_v, h->d_rho, h->d_scal,
+        h->d_W8, h->d_skip);
+    h->last_launches += 1;
+    return cudaGetLastError();
+}
+
 cudaError_t shd_launch_ctable(shd_ctx* h)
 {
+    if (h->rho_engine == 2 && h->nlimb >= 3) return shd_launch_wtable8(h);   // the INT8 gradient pass reads W8 instead
     long ncell = (long)h->npb16 * 16 * h->Qpad;
     k_ctable<<<(unsigned)((ncell + 255) / 256), 256, 0, h->stream>>>(
         h->npb16, h->Qpad, h->qscale_log2, h->d_cell_kp, h->d_cell_km, h->M, h->d_v, h->d_rho, h->d_scal, h->d_C, h->d_skip);

@@ -325,6 +325,15 @@ cudaError_t shd_grad_configure()
 
 cudaError_t shd_launch_grad(shd_ctx* h, double* grad_hi, double* grad_lo)
 {
+    if (h->rho_engine == 2 && h->nlimb >= 3) {          // INT8 tensor-core gradient pass (k_grad8.cu)
+        cudaError_t e = shd_launch_grad8_main(h);
+        if (e != cudaSuccess) return e;
+        const long n8 = (long)h->d * h->N;
+        k_gradsum<<<(unsigned)((n8 + 255) / 256), 256, 0, h->stream>>>(
+            n8, h->nseg8, h->L, h->d_gpart, h->d_scal, grad_hi, grad_lo, h->d_skip);
+        h->last_launches += 1;
+        return cudaGetLastError();
+    }
 #define LAUNCH_GRAD(NLV)                                                                                 \
     k_grad<NLV><<<(unsigned)(h->njb64 * h->nseg), NW * 32 + 128, GSMEM, h->stream>>>(                      \
         h->d, h->N, h->Npad, h->njb64, h->Qpad, h->npb * 32, h->qscale_log2,                               \

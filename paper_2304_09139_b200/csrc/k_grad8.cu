@@ -1,0 +1,221 @@
+// k_grad8.cu -- step a4 on the INT8 tensor cores (see k_grad.cu for the mathematics and k_rho8.cu for the
+// digit-sliced exact integer contraction).  The q-contraction
+//   T_j[p] = sum_q (C1 br + C2 bi),   T''_j[p] = sum_q (D1 br + D2 bi)
+// is the matrix product  T[j, (p, out)] = sum_{(q, c)} b_j[(q, c)] W[(p, out), (q, c)]  with out in
+// {T re, T im, T'' re, T'' im}, c in {re, im} and W built from C1, C2, D1, D2 by k_wtable8 (k_finish.cu).
+// One CTA owns 128 particles (the M = 128 rows) and a segment of the step list; a step is 16 q (K = 32) of
+// a block of 8 p (N side: 13 digit blocks of 8 p x 4 out = 32 columns, digits ascending, so one
+// tcgen05.mma.kind::i8 per particle-side digit lands all its digit pairs in the tensor-memory columns of
+// their digit sums; 18 instructions per step).  The s32 sums are exact (<= 2 Qn products per pair, Qn <= 5000).
+// At the end of a block (or of the segment) the four epilogue warps read tensor memory, thread = particle:
+// the 13 digit sums of each of its 32 outputs are combined in 128-bit integers, converted to
+// double-double, and contracted with the particle's own A_j[p] exactly as in k_grad.cu; the per-axis sums
+// stay in registers across blocks.  Warp 4: TMA producer, warp 5: MMA issuer.
+#include "pipe.cuh"
+#include "shd_internal.h"
+
+namespace {
+
+constexpr int G8_ND = SHD_I8_DIGITS;
+constexpr int G8_ASLAB = 128 * 32;                   // one digit of the particle operand of a step
+constexpr int G8_WSLAB = 32 * 32;                    // one digit of the shared operand W
+constexpr int G8_A = G8_ND * G8_ASLAB;               // 53248
+constexpr int G8_W = G8_ND * G8_WSLAB;               // 13312
+constexpr int G8_STAGE = G8_A + G8_W;
+constexpr int G8_NST = 3;
+constexpr int G8_SMEM = G8_NST * G8_STAGE;
+
+__device__ __forceinline__ uint64_t g8_desc(uint32_t addr) {
+    return (uint64_t)((addr >> 4) & 0x3FFF) | ((uint64_t)(128 >> 4) << 16) | ((uint64_t)(256 >> 4) << 32) | ((uint64_t)1 << 46);
+}
+__device__ __forceinline__ uint32_t g8_idesc(int n) {
+    return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+}
+__device__ __forceinline__ void g8_mma(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+    uint32_t z = 0;
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %5, %5, %5}, p;\n\t}"
+                 ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate), "r"(z) : "memory");
+}
+__device__ __forceinline__ void g8_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+// exact double-double of a 128-bit integer of magnitude < 2^92
+__device__ __forceinline__ dd i128_to_dd(__int128 x) {
+    const long long a = (long long)(x >> 40);                           // floor(x / 2^40), |a| < 2^52
+    const long long b = (long long)((unsigned long long)x & ((1ULL << 40) - 1));
+    return fast_two_sum(__dmul_rn((double)a, 1099511627776.0), (double)b);
+}
+__device__ __forceinline__ dd limbs_to_dd8(double x0, double x1, double x2) {
+    return fast_two_sum(__dadd_rn(x0, x1), x2);
+}
+
+__global__ void __launch_bounds__(192, 1) k_grad8(
+    int d, long N, long Npad, long njb128, int Ppad, int qscale_log2, int nkq,
+    const int2* __restrict__ steps, int nsteps, int nseg, const int* __restrict__ wT,
+    const double* __restrict__ A, const signed char* __restrict__ Bg8, const signed char* __restrict__ W8,
+    double* __restrict__ gpart, const int* __restrict__ skip)
+{
+    if (skip && *skip) return;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    __shared__ __align__(8) unsigned long long full_bar[G8_NST], empty_bar[G8_NST], tfull_bar, tempty_bar;
+    __shared__ uint32_t tmem_base;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const long jb = blockIdx.x % njb128;
+    const int seg = (int)(blockIdx.x / njb128);
+    const int c_begin = (int)((long)nsteps * seg / nseg), c_end = (int)((long)nsteps * (seg + 1) / nseg);
+    const int total = c_end - c_begin;
+    const uint32_t s0 = smem_u32(smem);
+    if (tid == 0) {
+        for (int s = 0; s < G8_NST; s++) { mbar_init(smem_u32(&full_bar[s]), 1); mbar_init(smem_u32(&empty_bar[s]), 1); }
+        mbar_init(smem_u32(&tfull_bar), 1);
+        mbar_init(smem_u32(&tempty_bar), 128);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(&tmem_base)));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const uint32_t tb = tmem_base;
+
+    if (warp == 4) {
+        if (lane == 0) {
+            const signed char* gA = Bg8 + (size_t)jb * nkq * G8_A;
+            for (int i = 0; i < total; i++) {
+                const int s = i % G8_NST;
+                if (i >= G8_NST) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((i / G8_NST - 1) & 1));
+                const uint32_t bar = smem_u32(&full_bar[s]);
+                const int2 st = steps[c_begin + i];           // x: pb8 * nkq + kstep,  y: kstep | end << 16
+                mbar_expect_tx(bar, G8_STAGE);
+                tma_load_1d(s0 + s * G8_STAGE, gA + (size_t)(st.y & 0xffff) * G8_A, G8_A, bar);
+                tma_load_1d(s0 + s * G8_STAGE + G8_A, W8 + (size_t)st.x * G8_W, G8_W, bar);
+            }
+        }
+    } else if (warp == 5) {
+        if (lane == 0) {
+            int nblock = 0;
+            bool fresh = true;                                 // next step starts a new accumulation
+            for (int i = 0; i < total; i++) {
+                const int s = i % G8_NST;
+                const int2 st = steps[c_begin + i];
+                if (fresh && nblock > 0) {                     // tensor memory must have been drained by the epilogue
+                    mbar_wait(smem_u32(&tempty_bar), (uint32_t)((nblock - 1) & 1));
+                    asm volatile("tcgen05.fence::after_thread_sync;");
+                }
+                mbar_wait(smem_u32(&full_bar[s]), (uint32_t)((i / G8_NST) & 1));
+                asm volatile("tcgen05.fence::after_thread_sync;");
+                const uint32_t sA = s0 + s * G8_STAGE, sW = sA + G8_A;
+                for (int ii = G8_ND - 1; ii >= 0; ii--) {
+                    const int n = (ii + 1) * 32, l0 = G8_ND - 1 - ii;
+                    const uint64_t da = g8_desc(sA + ii * G8_ASLAB);
+                    const uint32_t acc = (!fresh || ii < G8_ND - 1) ? 1u : 0u;
+                    if (n <= 256) {
+                        g8_mma(tb, da, g8_desc(sW + l0 * G8_WSLAB), g8_idesc(n), acc);
+                    } else {
+                        g8_mma(tb, da, g8_desc(sW + l0 * G8_WSLAB), g8_idesc(256), acc);
+                        g8_mma(tb + 256, da, g8_desc(sW + (l0 + 8) * G8_WSLAB), g8_idesc(n - 256), acc);
+                    }
+                }
+                g8_commit(smem_u32(&empty_bar[s]));
+                fresh = false;
+                if ((st.y >> 16) || i == total - 1) {          // block (or segment) end: hand the sums to the epilogue
+                    g8_commit(smem_u32(&tfull_bar));
+                    nblock++;
+                    fresh = true;
+                }
+            }
+        }
+    } else {
+        // ---- epilogue warps: thread = particle (TMEM lane), columns 32 sidx + 4 p_local + out
+        const long j = jb * 128 + tid;
+        const double qs = ldexp(1.0, qscale_log2);
+        const double2* Aj = reinterpret_cast<const double2*>(A) + (size_t)(j >> 2) * 3 * 32 * 4 + (j & 3);
+        dd g0{0.0, 0.0}, g1{0.0, 0.0}, g2{0.0, 0.0}, g3{0.0, 0.0};
+        int nblock = 0;
+        for (int i = 0; i < total; i++) {
+            const int2 st = steps[c_begin + i];
+            if (!((st.y >> 16) || i == total - 1)) continue;
+            const int pb8 = st.x / nkq;
+            mbar_wait(smem_u32(&tfull_bar), (uint32_t)(nblock & 1));
+            asm volatile("tcgen05.fence::after_thread_sync;");
+            for (int c0 = 0; c0 < 32; c0 += 8) {               // 8 columns = 2 p x 4 out
+                __int128 lo[8], hi[8];
+#pragma unroll
+                for (int e = 0; e < 8; e++) { lo[e] = 0; hi[e] = 0; }
+#pragma unroll
+                for (int sidx = 0; sidx < G8_ND; sidx++) {
+                    uint32_t v[8];
+                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                                 : "r"(tb + ((uint32_t)(warp * 32) << 16) + sidx * 32 + c0));
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                    for (int e = 0; e < 8; e++) {
+                        if (sidx < 7) lo[e] += (__int128)(int)v[e] << (8 * sidx);
+                        else hi[e] += (__int128)(int)v[e] << (8 * (sidx - 7));
+                    }
+                }
+                // value = 2^-204 (256^12 lo + 256^19 hi) = 2^-108 lo + 2^-52 hi
+                dd T[8];
+#pragma unroll
+                for (int e = 0; e < 8; e++) {
+                    const dd a = dd_scale2(i128_to_dd(lo[e]), 0x1p-108), b = dd_scale2(i128_to_dd(hi[e]), 0x1p-52);
+                    T[e] = dd_add(a, b);
+                }
+#pragma unroll
+                for (int pp = 0; pp < 2; pp++) {
+                    const int p = pb8 * 8 + (c0 >> 2) + pp;
+                    if (j < N && p < Ppad) {
+                        const double2* ap = Aj + ((size_t)(p >> 5) * (Npad / 4) * 3 * 32 + (p & 31)) * 4;
+                        const double2 a0 = ap[0], a1 = ap[128], a2 = ap[256];
+                        const dd ar = limbs_to_dd8(a0.x, a1.x, a2.x), ai = limbs_to_dd8(a0.y, a1.y, a2.y);
+                        const dd I = dd_dot2(ar, T[pp * 4 + 1], ai, T[pp * 4 + 0], -1.0);     // Im[conj(A) T]
+                        const dd R = dd_dot2(ar, T[pp * 4 + 2], ai, T[pp * 4 + 3], 1.0);      // Re[conj(A) T'']
+#define GACC8(AX)                                                                             \
+    if (AX < d) {                                                                             \
+        const int wgt = AX < 3 ? wT[(AX < 3 ? AX : 0) * Ppad + p] : 0;                        \
+        if (wgt != 0) g##AX = dd_add(g##AX, dd_mul_d(I, (double)wgt));                        \
+        if (AX == d - 1) g##AX = dd_add(g##AX, dd_scale2(R, qs));                             \
+    }
+                        GACC8(0) GACC8(1) GACC8(2) GACC8(3)
+#undef GACC8
+                    }
+                }
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;");
+            mbar_arrive(smem_u32(&tempty_bar));                // this thread has read its lane: 128 arrivals free TMEM
+            nblock++;
+        }
+        if (j < N) {
+            double2* o = reinterpret_cast<double2*>(gpart);
+            if (d > 0) o[((size_t)seg * d + 0) * N + j] = make_double2(g0.h, g0.l);
+            if (d > 1) o[((size_t)seg * d + 1) * N + j] = make_double2(g1.h, g1.l);
+            if (d > 2) o[((size_t)seg * d + 2) * N + j] = make_double2(g2.h, g2.l);
+            if (d > 3) o[((size_t)seg * d + 3) * N + j] = make_double2(g3.h, g3.l);
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tb));
+}
+
+}  // namespace
+
+cudaError_t shd_grad8_configure()
+{
+    return cudaFuncSetAttribute(k_grad8, cudaFuncAttributeMaxDynamicSharedMemorySize, G8_SMEM);
+}
+
+// k_gradsum (k_grad.cu) adds the segments' partial gradients and applies 4 pi / L / cscale
+cudaError_t shd_launch_grad8_main(shd_ctx* h)
+{
+    k_grad8<<<(unsigned)(h->njb128 * h->nseg8), 192, G8_SMEM, h->stream>>>(
+        h->d, h->N, h->Npad, h->njb128, h->npb * 32, h->qscale_log2, h->nkq8,
+        reinterpret_cast<const int2*>(h->d_steps8), h->nsteps8, h->nseg8, h->d_wT,
+        h->d_A, h->d_Bg8, h->d_W8, h->d_gpart, h->d_skip);
+    h->last_launches += 1;
+    return cudaGetLastError();
+}

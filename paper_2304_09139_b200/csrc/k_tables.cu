@@ -102,6 +102,23 @@ struct Stager {
     double* Bg;           // gradient layout (or nullptr)
     long Npad, j0, N;
     int Qpad;
+    signed char* gdig;    // particle-operand digit table of the INT8 gradient pass (B thread only, or nullptr)
+    int nkq;              // its K-steps (16 q) per particle block
+    // row = particle % 128 of block particle / 128, K index = 2 (q % 16) + re/im of K-step q / 16
+    __device__ __forceinline__ void putg8(int q, cdd z, bool live) {
+        if (gdig == nullptr || !live) return;
+        const long j = j0 + threadIdx.x;
+        const int row = (int)(j & 127);
+        signed char* base = gdig + (((size_t)(j >> 7) * nkq + (size_t)(q >> 4)) * SHD_I8_DIGITS) * 4096;
+        signed char dr[SHD_I8_DIGITS], di[SHD_I8_DIGITS];
+        digits13(z.re, dr);
+        digits13(z.im, di);
+        const int k0 = 2 * (q & 15), k1 = k0 + 1;
+        const int o0 = (row >> 3) * 256 + (k0 >> 4) * 128 + (row & 7) * 16 + (k0 & 15);
+        const int o1 = (row >> 3) * 256 + (k1 >> 4) * 128 + (row & 7) * 16 + (k1 & 15);
+#pragma unroll
+        for (int i = 0; i < SHD_I8_DIGITS; i++) { base[(size_t)i * 4096 + o0] = dr[i]; base[(size_t)i * 4096 + o1] = di[i]; }
+    }
     signed char* dig;     // digit table of the INT8 rho pass (or nullptr)
     long nk8;             // K-steps (32 particles) per block of that table
     int rows8;            // entries per block: 64 (A) or 16 (B)
@@ -175,7 +192,7 @@ __global__ void __launch_bounds__(TB) k_tables(
     const int* __restrict__ pn0, const int* __restrict__ pn1, const int* __restrict__ pn2, int Qpad,
     const double* __restrict__ pos_hi, const double* __restrict__ pos_lo,
     double* __restrict__ A, double* __restrict__ B, double* __restrict__ Bg, int with_grad,
-    signed char* __restrict__ A8, signed char* __restrict__ B8, long nk8,
+    signed char* __restrict__ A8, signed char* __restrict__ B8, long nk8, signed char* __restrict__ Bg8, int nkq8,
     const int* __restrict__ skip)
 {
     if (skip && *skip) return;
@@ -189,6 +206,7 @@ __global__ void __launch_bounds__(TB) k_tables(
     const cdd one{dd{1.0, 0.0}, dd{0.0, 0.0}};
     const bool gradB = which == 1 && with_grad != 0;
     Stager st{tile, 3, which == 0 ? A : B, gradB ? Bg : nullptr, Npad, j0, N, Qpad,
+              gradB ? Bg8 : nullptr, nkq8,
               which == 0 ? A8 : B8, nk8, which == 0 ? SHD_I8_PT : SHD_I8_QT};
     if (which == 0) {
         // ---- A table
@@ -250,6 +268,7 @@ __global__ void __launch_bounds__(TB) k_tables(
             for (int s = 0; s < cnt; s++) {
                 st.put(0, s, cur);
                 st.put8(q0 + s, cur, live);
+                st.putg8(q0 + s, cur, live);
                 cur = cdd_mul(cur, base);
             }
             st.flush(q0, cnt);
@@ -270,8 +289,9 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
     k_tables<<<grid, TB, TABLES_SMEM, h->stream>>>(h->d, h->N, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2,
                                          h->d_pn0, h->d_pn1, h->d_pn2, h->Qpad, pos_hi, pos_lo,
                                          h->d_A, h->d_B, h->d_Bg, with_grad_tables ? 1 : 0,
-                                         h->rho_engine == 1 && h->nlimb >= 3 ? h->d_A8 : nullptr,
-                                         h->rho_engine == 1 && h->nlimb >= 3 ? h->d_B8 : nullptr, h->nk8, h->d_skip);
+                                         h->rho_engine >= 1 && h->nlimb >= 3 ? h->d_A8 : nullptr,
+                                         h->rho_engine >= 1 && h->nlimb >= 3 ? h->d_B8 : nullptr, h->nk8,
+                                         h->rho_engine == 2 && h->nlimb >= 3 ? h->d_Bg8 : nullptr, h->nkq8, h->d_skip);
     h->last_launches += 1;
     return cudaGetLastError();
 }

@@ -301,7 +301,8 @@ int build(shd_ctx* h, const double* v) {
     if ((rc = dalloc_zero(h, &h->d_B, (size_t)h->nqb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
     if ((rc = dalloc_zero(h, &h->d_Bg, (size_t)(2 * h->njb64) * (h->Qpad / 4) * SHD_GROUP_DOUBLES))) return rc;
     if ((rc = dalloc_zero(h, &h->d_C, (size_t)h->npb16 * (h->Qpad / 4) * (16 * SHD_PG * 4 * 2)))) return rc;
-    if ((rc = dalloc_zero(h, &h->d_gpart, (size_t)h->nseg * h->d * h->N * 2))) return rc;
+    h->gpart_doubles = (size_t)h->nseg * h->d * h->N * 2;
+    if ((rc = dalloc_zero(h, &h->d_gpart, h->gpart_doubles))) return rc;
     h->part_doubles = (size_t)h->nsplit * h->ntiles * 4 * 1024 * 2;
     if ((rc = dalloc_zero(h, &h->d_part, h->part_doubles))) return rc;
     if ((rc = dalloc_zero(h, &h->d_rho, (size_t)4 * h->M))) return rc;
@@ -381,7 +382,7 @@ int run_rho(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool with_gr
     if ((rc = mark(h, 0))) return rc;
     CU(shd_launch_tables(h, pos_hi, pos_lo, with_grad));
     if ((rc = mark(h, 1))) return rc;
-    if (h->rho_engine == 1 && h->nlimb >= 3) CU(shd_launch_rho8(h)); else CU(shd_launch_rho(h));
+    if (h->rho_engine >= 1 && h->nlimb >= 3) CU(shd_launch_rho8(h)); else CU(shd_launch_rho(h));
     if ((rc = mark(h, 2))) return rc;
     CU(shd_launch_finish(h));
     if ((rc = mark(h, 3))) return rc;
@@ -424,6 +425,7 @@ void shd_destroy(shd_ctx* h) {
     cudaFree(h->d_rho); cudaFree(h->d_blockred); cudaFree(h->d_scal);
     cudaFree(h->d_hpos); cudaFree(h->d_hgrad);
     cudaFree(h->d_A8); cudaFree(h->d_B8); cudaFree(h->d_tile8_pb); cudaFree(h->d_tile8_qb);
+    cudaFree(h->d_Bg8); cudaFree(h->d_W8); cudaFree(h->d_steps8);
     for (int i = 0; i <= SHD_NKERN; i++) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     if (h->h_scal) cudaFreeHost(h->h_scal);
     if (h->gevent) cudaEventDestroy(h->gevent);
@@ -546,8 +548,61 @@ int shd_set_precision(shd_ctx* h, int limbs) {
 // engine 1: build the tile list, the particle splits and the digit tables of the INT8 rho pass (k_rho8.cu)
 int shd_set_engine(shd_ctx* h, int rho_engine) {
     if (!h) return SHD_EINVAL;
-    if (rho_engine != 0 && rho_engine != 1) return fail(h, SHD_EINVAL, "shd_set_engine: rho_engine must be 0 or 1");
-    if (rho_engine == 1 && !h->d_A8) {
+    if (rho_engine < 0 || rho_engine > 2) return fail(h, SHD_EINVAL, "shd_set_engine: engine must be 0, 1 or 2");
+    if (rho_engine == 2 && !h->d_Bg8) {
+        // ---- INT8 gradient pass: step list over blocks of 8 p (K-steps of 16 q up to the block's last valid cell)
+        h->npb8 = (h->P + 7) / 8;
+        h->nkq8 = h->Qpad / 16;
+        h->njb128 = (h->N + 127) / 128;
+        std::vector<int> kp((size_t)h->npb * 32 * h->Qpad), km(kp.size());
+        CU(cudaMemcpy(kp.data(), h->d_cell_kp, kp.size() * sizeof(int), cudaMemcpyDeviceToHost));
+        CU(cudaMemcpy(km.data(), h->d_cell_km, km.size() * sizeof(int), cudaMemcpyDeviceToHost));
+        std::vector<int> steps;
+        for (int pb = 0; pb < h->npb8; pb++) {
+            int nk = 0;
+            for (int pi = 0; pi < 8; pi++) {
+                const int p = pb * 8 + pi;
+                if (p >= h->npb * 32) continue;
+                for (int q = 0; q < h->Qpad; q++)
+                    if (kp[(size_t)p * h->Qpad + q] >= 0 || km[(size_t)p * h->Qpad + q] >= 0) nk = std::max(nk, q / 16 + 1);
+            }
+            for (int k = 0; k < nk; k++) {
+                steps.push_back(pb * h->nkq8 + k);
+                steps.push_back(k | ((k == nk - 1 ? 1 : 0) << 16));
+            }
+        }
+        h->nsteps8 = (int)steps.size() / 2;
+        cudaDeviceProp prop;
+        int dev = 0;
+        cudaGetDevice(&dev);
+        CU(cudaGetDeviceProperties(&prop, dev));
+        const long sms = prop.multiProcessorCount;
+        double best = -1.0;
+        h->nseg8 = 1;
+        for (int ns = 1; ns <= std::min(32, h->nsteps8); ns++) {
+            const long waves = (h->njb128 * ns + sms - 1) / sms;
+            const double cost = (double)waves * ((double)((h->nsteps8 + ns - 1) / ns) + 6.0);
+            if (best < 0.0 || cost < best) { best = cost; h->nseg8 = ns; }
+        }
+        const size_t g8 = (size_t)h->njb128 * h->nkq8 * SHD_I8_DIGITS * 4096;
+        const size_t w8 = (size_t)h->npb8 * h->nkq8 * SHD_I8_DIGITS * 1024;
+        CU(cudaMalloc((void**)&h->d_Bg8, g8));
+        CU(cudaMemset(h->d_Bg8, 0, g8));
+        CU(cudaMalloc((void**)&h->d_W8, w8));
+        CU(cudaMemset(h->d_W8, 0, w8));
+        h->workspace_bytes += g8 + w8;
+        int rc;
+        if ((rc = upload(h, &h->d_steps8, steps))) return rc;
+        const size_t need = (size_t)h->nseg8 * h->d * h->N * 2;
+        if (need > h->gpart_doubles) {
+            cudaFree(h->d_gpart);
+            h->d_gpart = nullptr;
+            if ((rc = dalloc_zero(h, &h->d_gpart, need))) return rc;
+            h->gpart_doubles = need;
+        }
+        CU(shd_grad8_configure());
+    }
+    if (rho_engine >= 1 && !h->d_A8) {
         h->npb64 = (h->P + SHD_I8_PT - 1) / SHD_I8_PT;
         h->nqb16 = (h->Qn + SHD_I8_QT - 1) / SHD_I8_QT;
         std::vector<int> kp((size_t)h->npb * 32 * h->Qpad), km(kp.size());
@@ -645,6 +700,8 @@ double shd_stat(const shd_ctx* h, int what) {
         case 14: return (double)h->ntiles8;
         case 15: return (double)h->nsplit8;
         case 16: return (double)h->rho_engine;
+        case 17: return (double)h->nseg8;
+        case 18: return (double)h->nsteps8;
         case 20: case 21: case 22: case 23: case 24: return (double)h->kern_ms[what - 20];
         default: return 0.0;
     }

@@ -120,6 +120,13 @@ struct shd_ctx {
     int ntiles8 = 0, nsplit8 = 0, ksteps8 = 0, npb64 = 0, nqb16 = 0;
     long nk8 = 0;                  // nsplit8 * ksteps8: K-steps (32 particles) in the digit tables
     size_t part_doubles = 0;       // capacity of d_part
+    // INT8 gradient pass (shd_set_engine(h, 2))
+    signed char *d_Bg8 = nullptr;  // [njb128][nkq8][13][128 rows (particle) x 32 K (q%16, re/im)]
+    signed char *d_W8 = nullptr;   // [npb8][nkq8][13][32 rows (p%8, out) x 32 K]
+    int *d_steps8 = nullptr;       // int2: x = pb8 * nkq8 + kstep, y = kstep | block-end << 16
+    int nsteps8 = 0, nseg8 = 0, npb8 = 0, nkq8 = 0;
+    long njb128 = 0;
+    size_t gpart_doubles = 0;      // capacity of d_gpart
     double *d_part = nullptr;  // [nsplit][ntiles][4][1024][2]
     double *d_rho = nullptr;   // [4][M]: re_hi, re_lo, im_hi, im_lo
     double *d_blockred = nullptr;   // per-block partials of the finish kernel
@@ -150,6 +157,8 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
 cudaError_t shd_launch_rho(shd_ctx* h);
 cudaError_t shd_launch_rho8(shd_ctx* h);
 cudaError_t shd_rho8_configure();
+cudaError_t shd_grad8_configure();
+cudaError_t shd_launch_grad8_main(shd_ctx* h);
 cudaError_t shd_launch_finish(shd_ctx* h);
 cudaError_t shd_launch_ctable(shd_ctx* h);
 cudaError_t shd_launch_sfactor(shd_ctx* h, double* S_out, double* scratch, double* tau2);
