@@ -8,6 +8,7 @@
 // entry split into limbs and written in the tile-major layouts the rho / gradient kernels stream
 // with TMA bulk copies.
 #include "dd.cuh"
+#include <cstdint>
 #include "shd_internal.h"
 #include "sincos_table.inc"
 
@@ -87,7 +88,8 @@ constexpr int R3MAX = 128;   // d >= 3: max |n_1| supported by the local power t
 constexpr int R4MAX = 32;    // d == 4: max |n_2|
 constexpr int TB = 64;       // particles (threads) per block
 constexpr int TG = 8;        // table entries staged per flush: 8 x 16 B = one 128-byte row per limb plane
-constexpr int TABLES_SMEM = TB * 3 * TG * 16;
+constexpr int TABLES_LIMB_SMEM = TB * 3 * TG * 16;
+constexpr int TABLES_SMEM = TABLES_LIMB_SMEM + TG * 2 * SHD_I8_DIGITS * TB;   // + digit transpose tile
 
 // Staging tile: a thread owns one particle, so its 16-byte stores would land far apart in global
 // memory.  They go to shared memory instead (tile[particle][plane][TG entries], 16-byte chunks
@@ -102,46 +104,89 @@ struct Stager {
     double* Bg;           // gradient layout (or nullptr)
     long Npad, j0, N;
     int Qpad;
-    signed char* gdig;    // particle-operand digit table of the INT8 gradient pass (B thread only, or nullptr)
-    int nkq;              // its K-steps (16 q) per particle block
-    // row = particle % 128 of block particle / 128, K index = 2 (q % 16) + re/im of K-step q / 16
-    __device__ __forceinline__ void putg8(int q, cdd z, bool live) {
-        if (gdig == nullptr || !live) return;
-        const long j = j0 + threadIdx.x;
-        const int row = (int)(j & 127);
-        signed char* base = gdig + (((size_t)(j >> 7) * nkq + (size_t)(q >> 4)) * SHD_I8_DIGITS) * 4096;
+    // ---- s8 digit tables of the INT8 passes (k_rho8.cu, k_grad8.cu); all in the tensor core's K-major
+    // core-matrix layout: 8 rows x 16 bytes per core matrix (128 B contiguous), K-adjacent core matrices
+    // 128 B apart, 8-row groups 256 B apart.
+    signed char* gdig;    // gradient pass, particle operand (B thread only, or nullptr): row = particle % 128 of
+    int nkq;              //   block particle / 128, K index = 2 (q % 16) + re/im of K-step q / 16 (nkq per block)
+    uint32_t gacc[SHD_I8_DIGITS][4];   // this particle's 16 bytes per digit for the 8 entries of a flush group
+    __device__ __forceinline__ void putg8(int slot, cdd z) {
+        if (gdig == nullptr) return;
         signed char dr[SHD_I8_DIGITS], di[SHD_I8_DIGITS];
         digits13(z.re, dr);
         digits13(z.im, di);
-        const int k0 = 2 * (q & 15), k1 = k0 + 1;
-        const int o0 = (row >> 3) * 256 + (k0 >> 4) * 128 + (row & 7) * 16 + (k0 & 15);
-        const int o1 = (row >> 3) * 256 + (k1 >> 4) * 128 + (row & 7) * 16 + (k1 & 15);
+        const int w = slot >> 1, sh = (slot & 1) * 16;             // bytes 2 slot (re) and 2 slot + 1 (im)
 #pragma unroll
-        for (int i = 0; i < SHD_I8_DIGITS; i++) { base[(size_t)i * 4096 + o0] = dr[i]; base[(size_t)i * 4096 + o1] = di[i]; }
+        for (int i = 0; i < SHD_I8_DIGITS; i++) {
+            const uint32_t v = ((uint32_t)(uint8_t)dr[i] | ((uint32_t)(uint8_t)di[i] << 8)) << sh;
+#pragma unroll
+            for (int ww = 0; ww < 4; ww++)
+                if (ww == w) gacc[i][ww] = (sh == 0 ? 0u : gacc[i][ww]) | v;
+        }
     }
-    signed char* dig;     // digit table of the INT8 rho pass (or nullptr)
-    long nk8;             // K-steps (32 particles) per block of that table
-    int rows8;            // entries per block: 64 (A) or 16 (B)
-    // s8 digits of entry e of this thread's particle: row r = 2 (e % rows8) + re/im of block e / rows8,
-    // K index = particle % 32, in the K-major core-matrix layout the tensor core reads (8 rows x 16 bytes
-    // per core matrix, K-adjacent core matrices 128 B apart, 8-row groups 256 B apart)
-    __device__ __forceinline__ void put8(int e, cdd z, bool live) {
-        if (dig == nullptr || !live) return;
+    // q0 = first entry of the group (multiple of 8): one 16-byte store per digit, 8 particles = one 128-byte line
+    __device__ __forceinline__ void flushg8(int q0, int count, bool live) {
+        if (gdig == nullptr) return;
         const long j = j0 + threadIdx.x;
-        const int k = (int)(j & 31);
-        const size_t slab = (size_t)rows8 * 2 * 32;                    // bytes of one digit of one (block, K-step)
-        signed char* base = dig + (((size_t)(e / rows8) * nk8 + (size_t)(j >> 5)) * SHD_I8_DIGITS) * slab;
+        if (live) {
+            const int row = (int)(j & 127);
+            signed char* base = gdig + (((size_t)(j >> 7) * nkq + (size_t)(q0 >> 4)) * SHD_I8_DIGITS) * 4096 +
+                                (row >> 3) * 256 + ((q0 >> 3) & 1) * 128 + (row & 7) * 16;
+#pragma unroll
+            for (int i = 0; i < SHD_I8_DIGITS; i++) {
+                uint4 v = make_uint4(gacc[i][0], gacc[i][1], gacc[i][2], gacc[i][3]);
+                if (count < 8) {                                    // ragged tail: entries >= count are zero digits
+                    uint32_t* pv = &v.x;
+#pragma unroll
+                    for (int ww = 0; ww < 4; ww++) {
+                        if (2 * ww >= count) pv[ww] = 0u;
+                        else if (2 * ww + 1 >= count) pv[ww] &= 0xffffu;
+                    }
+                }
+                *reinterpret_cast<uint4*>(base + (size_t)i * 4096) = v;
+            }
+        }
+    }
+    signed char* dig;     // rho pass (or nullptr): row = 2 (entry % rows8) + re/im of block entry / rows8,
+    long nk8;             //   K index = particle % 32 of K-step particle / 32 (nk8 K-steps per block)
+    int rows8;            // entries per block: 64 (A) or 16 (B)
+    signed char* dtile;   // shared-memory transpose tile [TG entries][2][13 digits][TB particles]
+    __device__ __forceinline__ void put8(int slot, cdd z, bool live) {
+        if (dig == nullptr) return;
         signed char dr[SHD_I8_DIGITS], di[SHD_I8_DIGITS];
         digits13(z.re, dr);
         digits13(z.im, di);
-        const int r0 = 2 * (e % rows8), r1 = r0 + 1;
-        const int o0 = (r0 >> 3) * 256 + (k >> 4) * 128 + (r0 & 7) * 16 + (k & 15);
-        const int o1 = (r1 >> 3) * 256 + (k >> 4) * 128 + (r1 & 7) * 16 + (k & 15);
+        signed char* t = dtile + (size_t)(slot * 2) * SHD_I8_DIGITS * TB + threadIdx.x;
 #pragma unroll
-        for (int i = 0; i < SHD_I8_DIGITS; i++) { base[(size_t)i * slab + o0] = dr[i]; base[(size_t)i * slab + o1] = di[i]; }
+        for (int i = 0; i < SHD_I8_DIGITS; i++) {
+            t[(size_t)i * TB] = live ? dr[i] : (signed char)0;                       // particles beyond N: zero digits
+            t[(size_t)(SHD_I8_DIGITS + i) * TB] = live ? di[i] : (signed char)0;
+        }
+    }
+    // after the block-wide barrier of flush(): 16-byte chunks (16 particles of one row of one digit), consecutive
+    // threads write consecutive chunks of a 128-byte line (8 rows)
+    __device__ __forceinline__ void flush8(int e0, int count) {
+        if (dig == nullptr) return;
+        const size_t slab = (size_t)rows8 * 2 * 32;
+        const int nrow = 2 * count;                                                 // rows of this group
+        signed char* base = dig + ((size_t)(e0 / rows8) * nk8 + (size_t)(j0 >> 5)) * SHD_I8_DIGITS * slab;
+        const int r_first = 2 * (e0 % rows8);
+        for (int c = threadIdx.x; c < SHD_I8_DIGITS * (TB / 16) * 2 * TG; c += TB) {
+            const int rl = c % (2 * TG);                                            // row within the group (fastest)
+            const int kh = (c / (2 * TG)) % (TB / 16);                              // 16-particle chunk of the block
+            const int dg = c / (2 * TG * (TB / 16));
+            if (rl < nrow && (j0 >> 5) + (kh >> 1) < nk8) {        // (the last block may reach past the table's K-steps)
+                const uint4 v = *reinterpret_cast<const uint4*>(dtile + ((size_t)rl * SHD_I8_DIGITS + dg) * TB + kh * 16);
+                const int r = r_first + rl;
+                signed char* dst = base + ((size_t)(kh >> 1) * SHD_I8_DIGITS + dg) * slab +
+                                   (r >> 3) * 256 + (kh & 1) * 128 + (r & 7) * 16;
+                *reinterpret_cast<uint4*>(dst) = v;
+            }
+        }
     }
     __device__ __forceinline__ static int swz(int r) { return ((r & 1) << 2) | (r & 2) | ((r >> 2) & 1); }
     __device__ __forceinline__ void put(int plane0, int slot, cdd z) {
+        if (table == nullptr && Bg == nullptr) return;
         limbs a = split_limbs(z.re), b = split_limbs(z.im);
         const int t = threadIdx.x, c = slot ^ swz(t);
         double2* row = tile + (t * planes + plane0) * TG;
@@ -150,11 +195,13 @@ struct Stager {
         row[2 * TG + c] = make_double2(a.x2, b.x2);
     }
     // entries e0 .. e0+count-1 (e0 a multiple of TG) of every particle of the block
-    __device__ __forceinline__ void flush(int e0, int count) {
+    __device__ __forceinline__ void flush(int e0, int count, bool live) {
         __syncthreads();
+        flush8(e0, count);
+        flushg8(e0, count, live);
         const int blk = e0 >> 5, off = e0 & 31;
         // rho layout: piece -> (group, limb, entry, j%4), j%4 fastest
-        for (int piece = threadIdx.x; piece < (TB / 4) * 3 * TG * 4; piece += TB) {
+        for (int piece = threadIdx.x; table != nullptr && piece < (TB / 4) * 3 * TG * 4; piece += TB) {
             const int jj = piece & 3, c = (piece >> 2) & 7, l = (piece >> 5) % 3, jg = piece / 96;
             const int row = jg * 4 + jj;
             const long j = j0 + row;
@@ -205,9 +252,14 @@ __global__ void __launch_bounds__(TB) k_tables(
     const long jc = live ? j : N - 1;            // dead threads shadow the last particle (keeps barriers uniform)
     const cdd one{dd{1.0, 0.0}, dd{0.0, 0.0}};
     const bool gradB = which == 1 && with_grad != 0;
-    Stager st{tile, 3, which == 0 ? A : B, gradB ? Bg : nullptr, Npad, j0, N, Qpad,
-              gradB ? Bg8 : nullptr, nkq8,
-              which == 0 ? A8 : B8, nk8, which == 0 ? SHD_I8_PT : SHD_I8_QT};
+    Stager st;
+    st.tile = tile; st.planes = 3;
+    st.table = which == 0 ? A : B;                      // may be nullptr: the INT8 rho pass does not read B limbs
+    st.Bg = gradB ? Bg : nullptr;                       // nullptr too when the gradient pass runs on INT8
+    st.Npad = Npad; st.j0 = j0; st.N = N; st.Qpad = Qpad;
+    st.gdig = gradB ? Bg8 : nullptr; st.nkq = nkq8;
+    st.dig = which == 0 ? A8 : B8; st.nk8 = nk8; st.rows8 = which == 0 ? SHD_I8_PT : SHD_I8_QT;
+    st.dtile = reinterpret_cast<signed char*>(tables_smem) + TABLES_LIMB_SMEM;
     if (which == 0) {
         // ---- A table
         cdd base;
@@ -219,10 +271,10 @@ __global__ void __launch_bounds__(TB) k_tables(
                 const int cnt = min(TG, P - p0);
                 for (int s = 0; s < cnt; s++) {
                     st.put(0, s, cur);
-                    st.put8(p0 + s, cur, live);
+                    st.put8(s, cur, live);
                     cur = cdd_mul(cur, base);
                 }
-                st.flush(p0, cnt);
+                st.flush(p0, cnt, live);
             }
         } else {
             cdd z1 = expi_turns(frac_turns(pos_hi[N + jc], pos_lo[N + jc], L, 1.0));
@@ -253,9 +305,9 @@ __global__ void __launch_bounds__(TB) k_tables(
                     }
                     const cdd az = cdd_mul(cur0, f);
                     st.put(0, s, az);
-                    st.put8(p0 + s, az, live);
+                    st.put8(s, az, live);
                 }
-                st.flush(p0, cnt);
+                st.flush(p0, cnt, live);
             }
         }
     } else {
@@ -267,11 +319,11 @@ __global__ void __launch_bounds__(TB) k_tables(
             const int cnt = min(TG, Qn - q0);
             for (int s = 0; s < cnt; s++) {
                 st.put(0, s, cur);
-                st.put8(q0 + s, cur, live);
-                st.putg8(q0 + s, cur, live);
+                st.put8(s, cur, live);
+                st.putg8(s, cur);
                 cur = cdd_mul(cur, base);
             }
-            st.flush(q0, cnt);
+            st.flush(q0, cnt, live);
         }
     }
 }
@@ -288,7 +340,8 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
     dim3 grid((unsigned)((h->N + TB - 1) / TB), 2);
     k_tables<<<grid, TB, TABLES_SMEM, h->stream>>>(h->d, h->N, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2,
                                          h->d_pn0, h->d_pn1, h->d_pn2, h->Qpad, pos_hi, pos_lo,
-                                         h->d_A, h->d_B, h->d_Bg, with_grad_tables ? 1 : 0,
+                                         h->d_A, h->rho_engine >= 1 && h->nlimb >= 3 ? nullptr : h->d_B,
+                                         h->rho_engine == 2 && h->nlimb >= 3 ? nullptr : h->d_Bg, with_grad_tables ? 1 : 0,
                                          h->rho_engine >= 1 && h->nlimb >= 3 ? h->d_A8 : nullptr,
                                          h->rho_engine >= 1 && h->nlimb >= 3 ? h->d_B8 : nullptr, h->nk8,
                                          h->rho_engine == 2 && h->nlimb >= 3 ? h->d_Bg8 : nullptr, h->nkq8, h->d_skip);

@@ -382,7 +382,7 @@ int run_rho(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool with_gr
     if ((rc = mark(h, 0))) return rc;
     CU(shd_launch_tables(h, pos_hi, pos_lo, with_grad));
     if ((rc = mark(h, 1))) return rc;
-    if (h->rho_engine >= 1 && h->nlimb >= 3) CU(shd_launch_rho8(h)); else CU(shd_launch_rho(h));
+    CU(shd_launch_rho(h));
     if ((rc = mark(h, 2))) return rc;
     CU(shd_launch_finish(h));
     if ((rc = mark(h, 3))) return rc;

@@ -322,14 +322,17 @@ def test_int8_tensor_core_probe(shd):
 @pytest.mark.parametrize("d,N,L,m_star,seed", [
     (2, 128, 128 ** 0.5, 49, 0), (2, 500, 22.0, 1300, 6), (2, 65, 8.0, 16 * 16, 10), (2, 96, 300.0, 265 * 265, 12),
     (1, 300, 300.0, 700 * 700, 4), (3, 130, 5.1, 50, 7), (4, 81, 3.0, 3, 15), (2, 1, 3.0, 9, 1),
+    (2, 129, 11.0, 17 * 17, 11), (2, 300, 40.0, 9, 17), (1, 50, 50.0, 1100 * 1100, 13),
 ])
-def test_int8_engine_small_cases(shd, oracle, d, N, L, m_star, seed):
-    """shd_set_engine(h, 1): the rho pass as an exact digit-sliced contraction on the INT8 tensor cores
-    (tcgen05.mma.kind::i8, s32 sums in tensor memory) against the oracle, same tolerances as the FP64 engine."""
+@pytest.mark.parametrize("engine", [1, 2])
+def test_int8_engine_small_cases(shd, oracle, d, N, L, m_star, seed, engine):
+    """shd_set_engine(h, 1 | 2): the rho pass (1) and the gradient pass too (2) as exact digit-sliced
+    contractions on the INT8 tensor cores (tcgen05.mma.kind::i8, s32 sums in tensor memory) against the
+    oracle, same tolerances as the FP64 engine."""
     hi, lo = inputs.uniform_positions_raw(d, N, L, seed)
     lo = inputs.jitter_lo(hi, seed + 100)
     h = shd.Shd(d, N, L, m_star=m_star)
-    h.set_engine(1)
+    h.set_engine(engine)
     th, tl = shd.from_host(hi, lo)
     phi, gh, gl = h.energy_grad(th, tl)
     rho = [t.cpu().numpy() for t in h.rho()]
@@ -339,9 +342,41 @@ def test_int8_engine_small_cases(shd, oracle, d, N, L, m_star, seed):
     h.close()
 
 
+def test_int8_engines_weights_and_quench(shd, oracle):
+    """Weights v(k) and the on-device minimizers on the INT8 engines: parity with the oracle, and the
+    quench of BASELINE.json configs[0] and [1] reaches S_max < 1e-30 (oracle-evaluated)."""
+    d, N, L, m_star = 2, 200, 14.0, 400
+    hi, lo = inputs.uniform_positions_raw(d, N, L, 12)
+    M = len(oracle.enumerate_Q(d, m_star))
+    v = 0.25 + np.random.default_rng(3).random(M) * 4
+    h = shd.Shd(d, N, L, m_star=m_star, v=v)
+    h.set_engine(2)
+    th, tl = shd.from_host(hi, lo)
+    phi, gh, gl = h.energy_grad(th, tl)
+    smax, arg = h.last_smax()
+    g = dict(phi=phi, grad_hi=gh.cpu().numpy(), grad_lo=gl.cpu().numpy(), rho=[t.cpu().numpy() for t in h.rho()],
+             smax=smax, argmax=arg, k=h.k(), M=h.M)
+    print(compare(oracle, d, N, L, m_star, hi, lo, g, v=v))
+    h.close()
+    for name, kind in (("cfg1", 0), ("cfg1", 1), ("cfg2", 0)):
+        cfg = inputs.CONFIGS[name]
+        hi, lo = inputs.uniform_positions(cfg, 0)
+        h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+        h.set_engine(2)
+        th, tl = shd.from_host(hi, lo)
+        rep = h.minimize(th, tl, kind=kind, smax_tol=1e-30, max_evals=20000, poll_every=16)
+        assert rep["status"] == shd.SHD_OK, rep
+        n = oracle.enumerate_Q(cfg.d, cfg.m_star)
+        re, im = oracle.rho(cfg.d, cfg.N, cfg.L, th.cpu().numpy(), tl.cpu().numpy(), n, mode="factored")
+        _, s_or, _, _ = oracle.energy(cfg.N, re, im)
+        print(name, kind, rep, oracle.to_float(s_or)[0])
+        assert oracle.to_float(s_or)[0] < 1e-30
+        h.close()
+
+
 def test_int8_engine_full_size_and_determinism(shd, oracle):
-    """BASELINE.json configs[3] on the INT8 engine: sampled rho against the direct-mode oracle, agreement
-    with the FP64 engine at the double-double level, 30 bit-identical repeats."""
+    """BASELINE.json configs[3] on the INT8 engines: sampled rho and gradient against the direct-mode oracle,
+    agreement with the FP64 engine at the double-double level, 30 bit-identical repeats."""
     import torch
     cfg = inputs.CONFIGS["cfg4"]
     hi, lo = inputs.uniform_positions(cfg, 0)
@@ -351,9 +386,21 @@ def test_int8_engine_full_size_and_determinism(shd, oracle):
     gh, gl = torch.empty_like(th), torch.empty_like(th)
     phi0, _, _ = h.energy_grad(th, tl, gh, gl)
     rho0 = [x.cpu().numpy() for x in h.rho()]
-    h.set_engine(1)
+    g64 = oracle.from_dd(gh.cpu().numpy(), gl.cpu().numpy())
+    h.set_engine(2)
     phi1, _, _ = h.energy_grad(th, tl, gh, gl)
     ref = [gh.clone(), gl.clone()] + [x.clone() for x in h.rho()]
+    eg = oracle.absdiff_dd(g64, gh.cpu().numpy(), gl.cpu().numpy())
+    gscale = float(gh.abs().max())
+    assert eg.max() <= GRAD_TIGHT * gscale * 16, eg.max()
+    js = np.unique(np.linspace(0, cfg.N - 1, 24).astype(np.int64))
+    n_all = oracle.enumerate_Q(cfg.d, cfg.m_star)
+    rq = [x.cpu().numpy() for x in h.rho()]
+    go = oracle.grad(cfg.d, cfg.N, cfg.L, hi, lo, n_all, oracle.from_dd(rq[0], rq[1]), oracle.from_dd(rq[2], rq[3]), jlist=js)
+    sel = np.concatenate([a * cfg.N + js for a in range(cfg.d)])
+    ego = oracle.absdiff_dd(go, gh.cpu().numpy()[sel], gl.cpu().numpy()[sel])
+    print("int8 gradient cfg4: vs FP64 engine", eg.max(), "vs oracle", ego.max())
+    assert ego.max() <= 1e-27 * cfg.N * cfg.M * cfg.K and ego.max() <= GRAD_TIGHT * gscale * 16
     rho1 = [x.cpu().numpy() for x in ref[2:]]
     e = oracle.cabsdiff_dd(oracle.from_dd(rho0[0], rho0[1]), oracle.from_dd(rho0[2], rho0[3]), *rho1)
     assert e.max() <= RHO_TIGHT * np.sqrt(cfg.N) * (1 + 239 / 64)
