@@ -10,7 +10,8 @@
 // At the end of a block (or of the segment) the four epilogue warps read tensor memory, thread = particle:
 // the 13 digit sums of each of its 32 outputs are combined in 128-bit integers, converted to
 // double-double, and contracted with the particle's own A_j[p] exactly as in k_grad.cu; the per-axis sums
-// stay in registers across blocks.  Warp 4: TMA producer, warp 5: MMA issuer.
+// stay in registers across blocks (two threads per particle, one per half of the block's 8 p).  Warp 8: TMA
+// producer, warp 9: MMA issuer.
 #include "pipe.cuh"
 #include "shd_internal.h"
 
@@ -50,7 +51,7 @@ __device__ __forceinline__ dd limbs_to_dd8(double x0, double x1, double x2) {
     return fast_two_sum(__dadd_rn(x0, x1), x2);
 }
 
-__global__ void __launch_bounds__(192, 1) k_grad8(
+__global__ void __launch_bounds__(320, 1) k_grad8(
     int d, long N, long Npad, long njb128, int Ppad, int qscale_log2, int nkq,
     const int2* __restrict__ steps, int nsteps, int nseg, const int* __restrict__ wT,
     const double* __restrict__ A, const signed char* __restrict__ Bg8, const signed char* __restrict__ W8,
@@ -61,15 +62,16 @@ __global__ void __launch_bounds__(192, 1) k_grad8(
     __shared__ __align__(8) unsigned long long full_bar[G8_NST], empty_bar[G8_NST], tfull_bar, tempty_bar;
     __shared__ uint32_t tmem_base;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const long jb = blockIdx.x % njb128;
-    const int seg = (int)(blockIdx.x / njb128);
+    // segment fastest: the CTAs of one particle block run side by side and share its digit slabs in L2
+    const int seg = (int)(blockIdx.x % nseg);
+    const long jb = blockIdx.x / nseg;
     const int c_begin = (int)((long)nsteps * seg / nseg), c_end = (int)((long)nsteps * (seg + 1) / nseg);
     const int total = c_end - c_begin;
     const uint32_t s0 = smem_u32(smem);
     if (tid == 0) {
         for (int s = 0; s < G8_NST; s++) { mbar_init(smem_u32(&full_bar[s]), 1); mbar_init(smem_u32(&empty_bar[s]), 1); }
         mbar_init(smem_u32(&tfull_bar), 1);
-        mbar_init(smem_u32(&tempty_bar), 128);
+        mbar_init(smem_u32(&tempty_bar), 256);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 0) {
@@ -81,7 +83,7 @@ __global__ void __launch_bounds__(192, 1) k_grad8(
     asm volatile("tcgen05.fence::after_thread_sync;");
     const uint32_t tb = tmem_base;
 
-    if (warp == 4) {
+    if (warp == 8) {
         if (lane == 0) {
             const signed char* gA = Bg8 + (size_t)jb * nkq * G8_A;
             for (int i = 0; i < total; i++) {
@@ -94,7 +96,7 @@ __global__ void __launch_bounds__(192, 1) k_grad8(
                 tma_load_1d(s0 + s * G8_STAGE + G8_A, W8 + (size_t)st.x * G8_W, G8_W, bar);
             }
         }
-    } else if (warp == 5) {
+    } else if (warp == 9) {
         if (lane == 0) {
             int nblock = 0;
             bool fresh = true;                                 // next step starts a new accumulation
@@ -129,8 +131,9 @@ __global__ void __launch_bounds__(192, 1) k_grad8(
             }
         }
     } else {
-        // ---- epilogue warps: thread = particle (TMEM lane), columns 32 sidx + 4 p_local + out
-        const long j = jb * 128 + tid;
+        // ---- 8 epilogue warps: thread = (particle = TMEM lane, half of the block's 8 p); columns 32 sidx + 4 p_local + out
+        const int half = warp >> 2, row = tid & 127;
+        const long j = jb * 128 + row;
         const double qs = ldexp(1.0, qscale_log2);
         const double2* Aj = reinterpret_cast<const double2*>(A) + (size_t)(j >> 2) * 3 * 32 * 4 + (j & 3);
         dd g0{0.0, 0.0}, g1{0.0, 0.0}, g2{0.0, 0.0}, g3{0.0, 0.0};
@@ -139,50 +142,71 @@ __global__ void __launch_bounds__(192, 1) k_grad8(
             const int2 st = steps[c_begin + i];
             if (!((st.y >> 16) || i == total - 1)) continue;
             const int pb8 = st.x / nkq;
+            // this block's eight A_j[p] (limbs -> double-double), loaded while the tensor core still works on it
+            double2 araw[4][3];
+#pragma unroll
+            for (int pp = 0; pp < 4; pp++) {
+                const int p = pb8 * 8 + half * 4 + pp;
+                araw[pp][0] = araw[pp][1] = araw[pp][2] = make_double2(0.0, 0.0);
+                if (j < N && p < Ppad) {
+                    const double2* ap = Aj + ((size_t)(p >> 5) * (Npad / 4) * 3 * 32 + (p & 31)) * 4;
+                    asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(araw[pp][0].x), "=d"(araw[pp][0].y) : "l"(ap));
+                    asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(araw[pp][1].x), "=d"(araw[pp][1].y) : "l"(ap + 128));
+                    asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(araw[pp][2].x), "=d"(araw[pp][2].y) : "l"(ap + 256));
+                }
+            }
             mbar_wait(smem_u32(&tfull_bar), (uint32_t)(nblock & 1));
             asm volatile("tcgen05.fence::after_thread_sync;");
-            for (int c0 = 0; c0 < 32; c0 += 8) {               // 8 columns = 2 p x 4 out
-                __int128 lo[8], hi[8];
+            dd ar[4], ai[4];
 #pragma unroll
-                for (int e = 0; e < 8; e++) { lo[e] = 0; hi[e] = 0; }
+            for (int pp = 0; pp < 4; pp++) {
+                ar[pp] = limbs_to_dd8(araw[pp][0].x, araw[pp][1].x, araw[pp][2].x);
+                ai[pp] = limbs_to_dd8(araw[pp][0].y, araw[pp][1].y, araw[pp][2].y);
+            }
 #pragma unroll
-                for (int sidx = 0; sidx < G8_ND; sidx++) {
-                    uint32_t v[8];
-                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
-                                 : "r"(tb + ((uint32_t)(warp * 32) << 16) + sidx * 32 + c0));
-                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+            for (int pp = 0; pp < 4; pp++) {                   // 4 columns = the four outputs of one p
+                const uint32_t taddr = tb + ((uint32_t)((warp & 3) * 32) << 16) + 4 * (half * 4 + pp);
+                uint32_t v[7][4];
+                __int128 lo[4], hi[4];
 #pragma unroll
-                    for (int e = 0; e < 8; e++) {
-                        if (sidx < 7) lo[e] += (__int128)(int)v[e] << (8 * sidx);
-                        else hi[e] += (__int128)(int)v[e] << (8 * (sidx - 7));
-                    }
+                for (int sidx = 0; sidx < 7; sidx++)
+                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+                                 : "=r"(v[sidx][0]), "=r"(v[sidx][1]), "=r"(v[sidx][2]), "=r"(v[sidx][3]) : "r"(taddr + sidx * 32));
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                for (int e = 0; e < 4; e++) {
+                    lo[e] = 0;
+#pragma unroll
+                    for (int sidx = 0; sidx < 7; sidx++) lo[e] += (__int128)(int)v[sidx][e] << (8 * sidx);
+                }
+#pragma unroll
+                for (int sidx = 0; sidx < 6; sidx++)
+                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+                                 : "=r"(v[sidx][0]), "=r"(v[sidx][1]), "=r"(v[sidx][2]), "=r"(v[sidx][3]) : "r"(taddr + (7 + sidx) * 32));
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                for (int e = 0; e < 4; e++) {
+                    hi[e] = 0;
+#pragma unroll
+                    for (int sidx = 0; sidx < 6; sidx++) hi[e] += (__int128)(int)v[sidx][e] << (8 * sidx);
                 }
                 // value = 2^-204 (256^12 lo + 256^19 hi) = 2^-108 lo + 2^-52 hi
-                dd T[8];
+                dd T[4];
 #pragma unroll
-                for (int e = 0; e < 8; e++) {
-                    const dd a = dd_scale2(i128_to_dd(lo[e]), 0x1p-108), b = dd_scale2(i128_to_dd(hi[e]), 0x1p-52);
-                    T[e] = dd_add(a, b);
-                }
-#pragma unroll
-                for (int pp = 0; pp < 2; pp++) {
-                    const int p = pb8 * 8 + (c0 >> 2) + pp;
-                    if (j < N && p < Ppad) {
-                        const double2* ap = Aj + ((size_t)(p >> 5) * (Npad / 4) * 3 * 32 + (p & 31)) * 4;
-                        const double2 a0 = ap[0], a1 = ap[128], a2 = ap[256];
-                        const dd ar = limbs_to_dd8(a0.x, a1.x, a2.x), ai = limbs_to_dd8(a0.y, a1.y, a2.y);
-                        const dd I = dd_dot2(ar, T[pp * 4 + 1], ai, T[pp * 4 + 0], -1.0);     // Im[conj(A) T]
-                        const dd R = dd_dot2(ar, T[pp * 4 + 2], ai, T[pp * 4 + 3], 1.0);      // Re[conj(A) T'']
+                for (int e = 0; e < 4; e++)
+                    T[e] = dd_add(dd_scale2(i128_to_dd(lo[e]), 0x1p-108), dd_scale2(i128_to_dd(hi[e]), 0x1p-52));
+                const int p = pb8 * 8 + half * 4 + pp;
+                if (j < N && p < Ppad) {
+                    const dd I = dd_dot2(ar[pp], T[1], ai[pp], T[0], -1.0);     // Im[conj(A) T]
+                    const dd R = dd_dot2(ar[pp], T[2], ai[pp], T[3], 1.0);      // Re[conj(A) T'']
 #define GACC8(AX)                                                                             \
     if (AX < d) {                                                                             \
         const int wgt = AX < 3 ? wT[(AX < 3 ? AX : 0) * Ppad + p] : 0;                        \
         if (wgt != 0) g##AX = dd_add(g##AX, dd_mul_d(I, (double)wgt));                        \
         if (AX == d - 1) g##AX = dd_add(g##AX, dd_scale2(R, qs));                             \
     }
-                        GACC8(0) GACC8(1) GACC8(2) GACC8(3)
+                    GACC8(0) GACC8(1) GACC8(2) GACC8(3)
 #undef GACC8
-                    }
                 }
             }
             asm volatile("tcgen05.fence::before_thread_sync;");
@@ -191,10 +215,11 @@ __global__ void __launch_bounds__(192, 1) k_grad8(
         }
         if (j < N) {
             double2* o = reinterpret_cast<double2*>(gpart);
-            if (d > 0) o[((size_t)seg * d + 0) * N + j] = make_double2(g0.h, g0.l);
-            if (d > 1) o[((size_t)seg * d + 1) * N + j] = make_double2(g1.h, g1.l);
-            if (d > 2) o[((size_t)seg * d + 2) * N + j] = make_double2(g2.h, g2.l);
-            if (d > 3) o[((size_t)seg * d + 3) * N + j] = make_double2(g3.h, g3.l);
+            const size_t slot = (size_t)(seg * 2 + half) * d;          // two partials per segment (the p halves)
+            if (d > 0) o[(slot + 0) * N + j] = make_double2(g0.h, g0.l);
+            if (d > 1) o[(slot + 1) * N + j] = make_double2(g1.h, g1.l);
+            if (d > 2) o[(slot + 2) * N + j] = make_double2(g2.h, g2.l);
+            if (d > 3) o[(slot + 3) * N + j] = make_double2(g3.h, g3.l);
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;");
@@ -212,7 +237,7 @@ cudaError_t shd_grad8_configure()
 // k_gradsum (k_grad.cu) adds the segments' partial gradients and applies 4 pi / L / cscale
 cudaError_t shd_launch_grad8_main(shd_ctx* h)
 {
-    k_grad8<<<(unsigned)(h->njb128 * h->nseg8), 192, G8_SMEM, h->stream>>>(
+    k_grad8<<<(unsigned)(h->njb128 * h->nseg8), 320, G8_SMEM, h->stream>>>(
         h->d, h->N, h->Npad, h->njb128, h->npb * 32, h->qscale_log2, h->nkq8,
         reinterpret_cast<const int2*>(h->d_steps8), h->nsteps8, h->nseg8, h->d_wT,
         h->d_A, h->d_Bg8, h->d_W8, h->d_gpart, h->d_skip);

@@ -110,11 +110,8 @@ struct Stager {
     signed char* gdig;    // gradient pass, particle operand (B thread only, or nullptr): row = particle % 128 of
     int nkq;              //   block particle / 128, K index = 2 (q % 16) + re/im of K-step q / 16 (nkq per block)
     uint32_t gacc[SHD_I8_DIGITS][4];   // this particle's 16 bytes per digit for the 8 entries of a flush group
-    __device__ __forceinline__ void putg8(int slot, cdd z) {
+    __device__ __forceinline__ void putg8(int slot, const signed char* dr, const signed char* di) {
         if (gdig == nullptr) return;
-        signed char dr[SHD_I8_DIGITS], di[SHD_I8_DIGITS];
-        digits13(z.re, dr);
-        digits13(z.im, di);
         const int w = slot >> 1, sh = (slot & 1) * 16;             // bytes 2 slot (re) and 2 slot + 1 (im)
 #pragma unroll
         for (int i = 0; i < SHD_I8_DIGITS; i++) {
@@ -151,11 +148,17 @@ struct Stager {
     long nk8;             //   K index = particle % 32 of K-step particle / 32 (nk8 K-steps per block)
     int rows8;            // entries per block: 64 (A) or 16 (B)
     signed char* dtile;   // shared-memory transpose tile [TG entries][2][13 digits][TB particles]
-    __device__ __forceinline__ void put8(int slot, cdd z, bool live) {
-        if (dig == nullptr) return;
+    // digits of one table entry for both INT8 tables (computed once)
+    __device__ __forceinline__ void put_digits(int slot, cdd z, bool live) {
+        if (dig == nullptr && gdig == nullptr) return;
         signed char dr[SHD_I8_DIGITS], di[SHD_I8_DIGITS];
         digits13(z.re, dr);
         digits13(z.im, di);
+        put8(slot, dr, di, live);
+        putg8(slot, dr, di);
+    }
+    __device__ __forceinline__ void put8(int slot, const signed char* dr, const signed char* di, bool live) {
+        if (dig == nullptr) return;
         signed char* t = dtile + (size_t)(slot * 2) * SHD_I8_DIGITS * TB + threadIdx.x;
 #pragma unroll
         for (int i = 0; i < SHD_I8_DIGITS; i++) {
@@ -271,7 +274,7 @@ __global__ void __launch_bounds__(TB) k_tables(
                 const int cnt = min(TG, P - p0);
                 for (int s = 0; s < cnt; s++) {
                     st.put(0, s, cur);
-                    st.put8(s, cur, live);
+                    st.put_digits(s, cur, live);
                     cur = cdd_mul(cur, base);
                 }
                 st.flush(p0, cnt, live);
@@ -305,7 +308,7 @@ __global__ void __launch_bounds__(TB) k_tables(
                     }
                     const cdd az = cdd_mul(cur0, f);
                     st.put(0, s, az);
-                    st.put8(s, az, live);
+                    st.put_digits(s, az, live);
                 }
                 st.flush(p0, cnt, live);
             }
@@ -319,8 +322,7 @@ __global__ void __launch_bounds__(TB) k_tables(
             const int cnt = min(TG, Qn - q0);
             for (int s = 0; s < cnt; s++) {
                 st.put(0, s, cur);
-                st.put8(s, cur, live);
-                st.putg8(s, cur);
+                st.put_digits(s, cur, live);
                 cur = cdd_mul(cur, base);
             }
             st.flush(q0, cnt, live);
