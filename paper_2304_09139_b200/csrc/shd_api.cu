@@ -579,7 +579,8 @@ int shd_set_engine(shd_ctx* h, int rho_engine) {
         const long sms = prop.multiProcessorCount;
         double best = -1.0;
         h->nseg8 = 1;
-        for (int ns = 1; ns <= std::min(32, h->nsteps8); ns++) {
+        // at least two segments: the CTAs of one particle block then stream the same digit slabs side by side (L2)
+        for (int ns = std::min(2, h->nsteps8); ns <= std::min(32, h->nsteps8); ns++) {
             const long waves = (h->njb128 * ns + sms - 1) / sms;
             const double cost = (double)waves * ((double)((h->nsteps8 + ns - 1) / ns) + 6.0);
             if (best < 0.0 || cost < best) { best = cost; h->nseg8 = ns; }
