@@ -39,6 +39,9 @@ ALG_DFMA_RHO, ALG_DFMA_GRAD = 12.0, 24.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/r1d_summary.md), bytes; known for the headline workload only, otherwise null
 NCU_TRAFFIC = {("cfg4", "k_grad"): 12.77e9, ("cfg4", "k_rho"): 3.63e9}
+# INT8 tensor-core engines (k_rho8.cu, k_grad8.cu): 91 digit pairs per real product; 4 real products per (p,q)
+# cell = 2 wavevectors in the rho pass, 8 in the gradient pass; 2 operations per multiply-accumulate
+ALG_MAC_RHO8, ALG_MAC_GRAD8 = 182.0, 364.0
 
 
 def dist_env():
@@ -207,29 +210,37 @@ def run_gpu(args, cfg):
             dist.barrier()
         torch.cuda.synchronize()
 
+    # engine of the two O(N M) passes: 2 = INT8 tensor cores (tcgen05), 0 = FP64 limbs on DMMA (the reference
+    # engine).  auto: the tensor-core engine where its digit tables pay off and fit beside the limb tables
+    engine = {"auto": 2 if (cfg.pairs >= 5e7 and cfg.d <= 2 and cfg.N <= 500_000) else 0}.get(args.engine, None)
+    engine = int(args.engine) if engine is None else engine
+
+    def timed_steps(steps, warmup, sample_clocks):
+        """`steps` evaluations timed with CUDA events on the handle's stream (L2 flushed before each)."""
+        h.set_timing(True)
+        for _ in range(warmup):
+            h.energy_grad(pos_hi, pos_lo, grad_hi, grad_lo)
+        barrier()
+        clocks = ClockSampler(local_rank) if (rank == 0 and sample_clocks) else None
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        kms = {k: 0.0 for k in ("tables", "rho", "finish", "ctable", "grad")}
+        launches, phi = 0, None
+        for i in range(steps):
+            flush.zero_()
+            ev[i][0].record(stream)
+            phi, _, _ = h.energy_grad(pos_hi, pos_lo, grad_hi, grad_lo)
+            ev[i][1].record(stream)
+            for k, v in h.kernel_ms().items():
+                kms[k] += v
+            launches += int(h.stat(1))
+        barrier()
+        clk = clocks.stop() if clocks else None
+        h.set_timing(False)
+        return float(sum(a.elapsed_time(b) for a, b in ev)), kms, launches, phi, clk
+
     # ---- device-resident leg (value)
-    h.set_timing(True)
-    for _ in range(args.warmup):
-        h.energy_grad(pos_hi, pos_lo, grad_hi, grad_lo)
-    barrier()
-    clocks = ClockSampler(local_rank) if rank == 0 else None
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    kms = {k: 0.0 for k in ("tables", "rho", "finish", "ctable", "grad")}
-    launches = 0
-    phi = None
-    for i in range(args.steps):
-        flush.zero_()
-        ev[i][0].record(stream)
-        phi, _, _ = h.energy_grad(pos_hi, pos_lo, grad_hi, grad_lo)
-        ev[i][1].record(stream)
-        for k, v in h.kernel_ms().items():
-            kms[k] += v
-        launches += int(h.stat(1))
-    barrier()
-    clk = clocks.stop() if clocks else None
-    step_ms = [a.elapsed_time(b) for a, b in ev]
-    total_ms = float(sum(step_ms))
-    h.set_timing(False)
+    h.set_engine(engine)
+    total_ms, kms, launches, phi, clk = timed_steps(args.steps, args.warmup, True)
 
     # ---- end-to-end leg: host (pinned) buffers through shd_energy_grad_host
     ph = torch.from_numpy(hi).pin_memory(); pl = torch.from_numpy(lo).pin_memory()
@@ -254,34 +265,75 @@ def run_gpu(args, cfg):
     e2e_value = whole_job_value(pairs, args.steps, world, e2e_ms)
     nbytes = 2 * cfg.d * cfg.N * 8
 
-    # ---- roofline of the dominant kernel (ALU-bound on the FP64 pipe)
+    # ---- rooflines of the dominant kernel
     dfma_best, dfma_sus = shd.fp64_peak(0, 0.5)
     dadd_best, dadd_sus = shd.fp64_peak(1, 0.5)
     dmma_best, dmma_sus = shd.fp64_peak(2, 1.0)      # the instruction k_rho / k_grad issue (same FP64 pipe)
     pipe_sus = max(dfma_sus, dmma_sus)
-    grad_ms, rho_ms = kms["grad"] / args.steps, kms["rho"] / args.steps
-    dom = "k_grad" if grad_ms >= rho_ms else "k_rho"
-    dom_ms = max(grad_ms, rho_ms)
-    alg = ALG_DFMA_GRAD if dom == "k_grad" else ALG_DFMA_RHO
-    achieved = pairs * alg * 2.0 / (dom_ms * 1e-3) / 1e12             # TFLOP/s, DFMA = 2 FLOP
-    peak = pipe_sus * 2.0 / 1e12
-    launched = h.stat(12) if dom == "k_grad" else h.stat(0)
-    roofline = {
-        "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-        "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((cfg.name, dom)),
-        "traffic_source": "profiles/r1d_summary.md (one ncu --set full capture of this kernel at this workload)"
-                          if (cfg.name, dom) in NCU_TRAFFIC else None,
-        "peak_source": "measured live: shd_fp64_peak, max of dependent-DFMA chains and DMMA.8x8x4 chains "
-                       "(one FP64 pipe), sustained over 1 s (of measured)",
-        "peak_burst": max(dfma_best, dmma_best) * 2.0 / 1e12, "dfma_peak_tfma": dfma_sus / 1e12,
-        "dmma_peak_tfma": dmma_sus / 1e12, "dadd_peak_tinstr": dadd_sus / 1e12,
-        "nominal_peak": 148 * 64 * 2 * 1.965e9 / 1e12,
-        "kernel_ms": dom_ms, "algorithmic_dfma_per_pair": alg,
-        "launched_dfma_per_pair": launched / pairs,
-        "issue_frac_launched": launched / (dom_ms * 1e-3) / pipe_sus,
-        "whole_eval_frac": pairs * (ALG_DFMA_RHO + ALG_DFMA_GRAD) / (total_ms / args.steps * 1e-3) / pipe_sus,
-        "kernel_ms_all": {k: v / args.steps for k, v in kms.items()},
-    }
+
+    def fp64_roofline(kms_, total_ms_, steps_):
+        """FP64 limb engine: ALU-bound on the FP64 pipe, peak measured live."""
+        grad_ms, rho_ms = kms_["grad"] / steps_, kms_["rho"] / steps_
+        dom = "k_grad" if grad_ms >= rho_ms else "k_rho"
+        dom_ms = max(grad_ms, rho_ms)
+        alg = ALG_DFMA_GRAD if dom == "k_grad" else ALG_DFMA_RHO
+        achieved = pairs * alg * 2.0 / (dom_ms * 1e-3) / 1e12          # TFLOP/s, DFMA = 2 FLOP
+        peak = pipe_sus * 2.0 / 1e12
+        launched = h.stat(12) if dom == "k_grad" else h.stat(0)
+        return {
+            "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+            "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((cfg.name, dom)),
+            "traffic_source": "profiles/r1d_summary.md (one ncu --set full capture of this kernel at this workload)"
+                              if (cfg.name, dom) in NCU_TRAFFIC else None,
+            "peak_source": "measured live: shd_fp64_peak, max of dependent-DFMA chains and DMMA.8x8x4 chains "
+                           "(one FP64 pipe), sustained over 1 s (of measured)",
+            "peak_burst": max(dfma_best, dmma_best) * 2.0 / 1e12, "dfma_peak_tfma": dfma_sus / 1e12,
+            "dmma_peak_tfma": dmma_sus / 1e12, "dadd_peak_tinstr": dadd_sus / 1e12,
+            "nominal_peak": 148 * 64 * 2 * 1.965e9 / 1e12,
+            "kernel_ms": dom_ms, "algorithmic_dfma_per_pair": alg,
+            "launched_dfma_per_pair": launched / pairs,
+            "issue_frac_launched": launched / (dom_ms * 1e-3) / pipe_sus,
+            "whole_eval_frac": pairs * (ALG_DFMA_RHO + ALG_DFMA_GRAD) / (total_ms_ / steps_ * 1e-3) / pipe_sus,
+            "kernel_ms_all": {k: v / steps_ for k, v in kms_.items()},
+        }
+
+    fp64_engine = None
+    if engine == 0:
+        roofline = fp64_roofline(kms, total_ms, args.steps)
+    else:
+        # INT8 tensor-core engines: bound by the tensor pipe; peak = the issue rate of tcgen05.mma.kind::i8
+        # measured live by shd_i8_probe (which also re-checks that the integer products are exact)
+        i8_tops, i8_bad = shd.i8_probe()
+        grad_ms, rho_ms = kms["grad"] / args.steps, kms["rho"] / args.steps
+        grad8 = engine == 2
+        dom = "k_grad8" if (grad8 and grad_ms >= rho_ms) else ("k_rho8" if rho_ms >= grad_ms or not grad8 else "k_grad8")
+        if not grad8 and grad_ms >= rho_ms:
+            roofline = fp64_roofline(kms, total_ms, args.steps)         # FP64 gradient pass still dominates
+        else:
+            dom_ms = grad_ms if dom == "k_grad8" else rho_ms
+            mac = ALG_MAC_GRAD8 if dom == "k_grad8" else ALG_MAC_RHO8
+            achieved = pairs * mac * 2.0 / (dom_ms * 1e-3) / 1e12       # TOP/s, 2 per multiply-accumulate
+            roofline = {
+                "bound": "tensor", "kernel": dom, "achieved": achieved, "peak": i8_tops, "unit": "TFLOP/s",
+                "frac": achieved / i8_tops, "traffic": NCU_TRAFFIC.get((cfg.name, dom)),
+                "traffic_source": "profiles/r1e_summary.md" if (cfg.name, dom) in NCU_TRAFFIC else None,
+                "dtype": "s8 x s8 -> s32 (exact digit-sliced contraction; counted in integer operations)",
+                "peak_source": "measured live: shd_i8_probe, tcgen05.mma.kind::i8 M=128 N=256 K=32 issued back to "
+                               "back on all SMs; MEASURED_PEAKS.json bf16 x 2 (nominal int8 : bf16) for comparison",
+                "peak_from_measured_bf16_x2": 2.0 * float(json.load(open(ROOT / "MEASURED_PEAKS.json"))["bf16_tflops"])
+                                              if (ROOT / "MEASURED_PEAKS.json").exists() else None,
+                "i8_products_exact": i8_bad == 0,
+                "kernel_ms": dom_ms, "algorithmic_mac_per_pair": mac,
+                "whole_eval_frac": pairs * (ALG_MAC_RHO8 + ALG_MAC_GRAD8) * 2.0 / (total_ms / args.steps * 1e-3) / 1e12 / i8_tops,
+                "kernel_ms_all": {k: v / args.steps for k, v in kms.items()},
+            }
+        # the FP64 limb engine (the reference engine of this library) on the same inputs, for comparison
+        h.set_engine(0)
+        n64 = max(3, min(args.steps, 5))
+        t64, k64, _, _, _ = timed_steps(n64, 3, False)
+        fp64_engine = {"ms_per_step": t64 / n64, "value": pairs * n64 / (t64 * 1e-3), "roofline": fp64_roofline(k64, t64, n64)}
+        h.set_engine(engine)
+        h.energy_grad(pos_hi, pos_lo, grad_hi, grad_lo)                 # rho() below belongs to the timed engine
 
     # ---- oracle on the host cores, same run, bounded sample; doubles as a live parity sample
     from oracle import shd_oracle as O
@@ -304,7 +356,10 @@ def run_gpu(args, cfg):
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / args.steps,
                 "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes + 64},
         "gpu_launches": launches,
+        "engine": {0: "fp64 limbs on DMMA.8x8x4", 1: "rho pass on INT8 tensor cores (tcgen05), gradient pass on FP64 limbs",
+                   2: "both O(N M) passes on INT8 tensor cores (tcgen05.mma.kind::i8, exact digit slices)"}[engine],
         "roofline": roofline,
+        "fp64_engine": fp64_engine,
         "cpu_baseline": {"value": s["value"], "unit": UNIT, "cores": s["cores"], "kind": "oracle",
                          "sample": s["sample"], "seconds": s["seconds"]},
         "parity_sample": {"rho_max_abs_err": float(e_rho.max()), "rho_tol": tol_rho,
@@ -320,10 +375,12 @@ def run_gpu(args, cfg):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=40)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="cfg4", choices=sorted(inputs.CONFIGS))
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--engine", default="auto", choices=["auto", "0", "1", "2"],
+                    help="engine of the two O(N M) passes: 0 FP64 limbs (DMMA), 1 rho on INT8 tensor cores, 2 both")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
     cfg = inputs.CONFIGS[args.config]

@@ -36,6 +36,8 @@ def main(argv=None):
                          "(P:50: any positive v has the same ground states; S_max does not depend on v; "
                          "SURVEY.md 8(f) NEXT-1: it removes the k^2 ill-conditioning, decisive in d = 1)")
     ap.add_argument("--fire-dt0", type=float, default=0.0)
+    ap.add_argument("--engine", type=int, default=0, choices=[0, 1, 2],
+                    help="engine of the O(N M) passes (shd_set_engine): 0 FP64 limbs, 1 rho on the INT8 tensor cores, 2 both")
     ap.add_argument("--ladder", type=float, default=0.0,
                     help="precision ladder (P:77 'tunable precision'; SURVEY.md 8(f) NEXT-1): evaluate with two "
                          "limbs (shd_set_precision 2) until S_max < this value, e.g. 1e-18, then with three")
@@ -56,6 +58,7 @@ def main(argv=None):
         n = h.k().astype(np.float64)
         h.close()
         h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star, v=1.0 / (n * n).sum(axis=1))
+    h.set_engine(args.engine)
     pos_hi, pos_lo = shd.from_host(hi, lo)
     phi0, _, _ = h.energy_grad(pos_hi, pos_lo, want_grad=False)
     smax0, _ = h.last_smax()
@@ -96,7 +99,7 @@ def main(argv=None):
     smax, arg = h.smax(pos_hi, pos_lo)
     n = h.k()
     line = {"config": cfg.name, "d": cfg.d, "N": cfg.N, "M": cfg.M, "chi_realised": cfg.M / (cfg.d * (cfg.N - 1)),
-            "seed": args.seed, "kind": "lbfgs" if args.kind == 0 else "fire", "weight": args.weight, "history": args.history,
+            "seed": args.seed, "kind": "lbfgs" if args.kind == 0 else "fire", "weight": args.weight, "engine": args.engine, "history": args.history,
             "tol": args.tol, "ladder": args.ladder, "ladder1": args.ladder1, "status": status, "evals": evals, "iters": iters, "seconds": seconds,
             "ms_per_eval": 1e3 * seconds / max(evals, 1), "phi_start": phi0[0], "smax_start": smax0[0],
             "phi_final": trace[-1]["phi"], "smax_final": smax[0], "argmax_n": n[arg].tolist(), "trace": trace}
