@@ -38,7 +38,8 @@ UNIT = "pair-terms/s"
 ALG_DFMA_RHO, ALG_DFMA_GRAD = 12.0, 24.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/r1d_summary.md), bytes; known for the headline workload only, otherwise null
-NCU_TRAFFIC = {("cfg4", "k_grad"): 12.77e9, ("cfg4", "k_rho"): 3.63e9}
+NCU_TRAFFIC = {("cfg4", "k_grad"): 12.77e9, ("cfg4", "k_rho"): 3.63e9,           # profiles/r1d_summary.md
+               ("cfg4", "k_grad8"): 1.90e9, ("cfg4", "k_rho8"): 1.55e9}          # profiles/r1e_summary.md
 # INT8 tensor-core engines (k_rho8.cu, k_grad8.cu): 91 digit pairs per real product; 4 real products per (p,q)
 # cell = 2 wavevectors in the rho pass, 8 in the gradient pass; 2 operations per multiply-accumulate
 ALG_MAC_RHO8, ALG_MAC_GRAD8 = 182.0, 364.0
