@@ -23,6 +23,7 @@ int fail(shd_ctx* h, int code, const std::string& msg) {
         cudaError_t e_ = (call);                                                         \
         if (e_ != cudaSuccess) {                                                         \
             h->err = std::string(#call) + ": " + cudaGetErrorString(e_);                 \
+            (void)cudaGetLastError();   /* a failed cudaMalloc must not poison the next launch check */ \
             return e_ == cudaErrorMemoryAllocation ? SHD_ENOMEM : SHD_ECUDA;             \
         }                                                                                \
     } while (0)
@@ -298,8 +299,7 @@ int build(shd_ctx* h, const double* v) {
     if ((rc = upload(h, &h->d_steps, steps))) return rc;
     if (!h->v.empty()) { if ((rc = upload(h, &h->d_v, h->v))) return rc; }
     if ((rc = dalloc_zero(h, &h->d_A, (size_t)h->npb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
-    if ((rc = dalloc_zero(h, &h->d_B, (size_t)h->nqb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
-    if ((rc = dalloc_zero(h, &h->d_Bg, (size_t)(2 * h->njb64) * (h->Qpad / 4) * SHD_GROUP_DOUBLES))) return rc;
+    // (the B limb tables of the FP64 passes are allocated on first use: shd_prepare_tables)
     if ((rc = dalloc_zero(h, &h->d_C, (size_t)h->npb16 * (h->Qpad / 4) * (16 * SHD_PG * 4 * 2)))) return rc;
     h->gpart_doubles = (size_t)h->nseg * h->d * h->N * 2;
     if ((rc = dalloc_zero(h, &h->d_gpart, h->gpart_doubles))) return rc;
@@ -319,6 +319,23 @@ int build(shd_ctx* h, const double* v) {
 }
 
 // table != nullptr: the caller's half-space set (M vectors, row-major) instead of the shell n.n <= m_star
+}  // namespace
+
+// Limb tables of the FP64 engine that the current (engine, precision) setting reads, allocated on first use so
+// that a handle driven on the INT8 engines only never holds them (at the paper's N they are 49 GB each).
+// Called outside any stream capture.
+int shd_prepare_tables(shd_ctx* h, bool with_grad) {
+    const bool i8 = h->nlimb >= 3;
+    int rc;
+    if (!(i8 && h->rho_engine >= 1) && !h->d_B)
+        if ((rc = dalloc_zero(h, &h->d_B, (size_t)h->nqb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
+    if (with_grad && !(i8 && h->rho_engine == 2) && !h->d_Bg)
+        if ((rc = dalloc_zero(h, &h->d_Bg, (size_t)(2 * h->njb64) * (h->Qpad / 4) * SHD_GROUP_DOUBLES))) return rc;
+    return SHD_OK;
+}
+
+namespace {
+
 int create_common(int d, long N, double L, long m_star, const double* v, shd_ctx** out,
                   const int* table = nullptr, long M = 0) {
     if (!out) return SHD_EINVAL;
@@ -376,6 +393,8 @@ int collect_timing(shd_ctx* h) {      // after the stream has been synchronised
 }
 // rho pass + reduction (steps a1-a3); optionally the gradient tables too
 int run_rho(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool with_grad) {
+    int prc = shd_prepare_tables(h, with_grad);
+    if (prc) return prc;
     h->last_launches = 0;
     for (int i = 0; i <= SHD_NKERN; i++) h->ev_used[i] = false;
     int rc;

@@ -205,6 +205,7 @@ int shd_fire_run(shd_ctx* h, double* pos_hi, double* pos_lo, const shd_min_opts*
     const bool cont = opts->resume != 0 && h->fire && h->fire->h_ctrl->dt[0] > 0.0;
     int rc = fire_alloc(h);
     if (rc) return rc;
+    if ((rc = shd_prepare_tables(h, true))) return rc;
     shd_firestate* s = h->fire;
     const long n = s->n;
     cudaStream_t st = h->stream;

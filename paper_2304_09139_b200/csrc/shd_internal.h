@@ -167,6 +167,7 @@ cudaError_t shd_tables_configure();
 cudaError_t shd_rho_configure();
 cudaError_t shd_grad_configure();
 
+int shd_prepare_tables(shd_ctx* h, bool with_grad);   // shd_api.cu
 // minimizers (shd_min.cu, shd_fire.cu)
 void shd_min_free(shd_ctx* h);
 void shd_fire_free(shd_ctx* h);

@@ -392,6 +392,7 @@ extern "C" int shd_minimize(shd_ctx* h, double* pos_hi, double* pos_lo, const sh
         return min_fail(h, SHD_EINVAL, "bad smax_tol / max_evals / poll_every");
     int rc = min_alloc(h, m);
     if (rc) return rc;
+    if ((rc = shd_prepare_tables(h, true))) return rc;
     shd_minstate* s = h->min;
     const long n = s->n;
     const size_t v = (size_t)2 * n * sizeof(double);
