@@ -8,7 +8,7 @@
 // tcgen05.mma.kind::i8 per particle-side digit lands all its digit pairs in the tensor-memory columns of
 // their digit sums; 18 instructions per step).  The s32 sums are exact (<= 2 Qn products per pair, Qn <= 5000).
 // At the end of a block (or of the segment) the four epilogue warps read tensor memory, thread = particle:
-// the 13 digit sums of each of its 32 outputs are combined in 128-bit integers, converted to
+// the 13 digit sums of each of its outputs are combined exactly in groups of three per double, added in
 // double-double, and contracted with the particle's own A_j[p] exactly as in k_grad.cu; the per-axis sums
 // stay in registers across blocks (two threads per particle, one per half of the block's 8 p).  Warp 8: TMA
 // producer, warp 9: MMA issuer.
@@ -40,12 +40,6 @@ __device__ __forceinline__ void g8_mma(uint32_t tmem_d, uint64_t da, uint64_t db
 }
 __device__ __forceinline__ void g8_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
-// exact double-double of a 128-bit integer of magnitude < 2^92
-__device__ __forceinline__ dd i128_to_dd(__int128 x) {
-    const long long a = (long long)(x >> 40);                           // floor(x / 2^40), |a| < 2^52
-    const long long b = (long long)((unsigned long long)x & ((1ULL << 40) - 1));
-    return fast_two_sum(__dmul_rn((double)a, 1099511627776.0), (double)b);
 }
 __device__ __forceinline__ dd limbs_to_dd8(double x0, double x1, double x2) {
     return fast_two_sum(__dadd_rn(x0, x1), x2);
@@ -166,8 +160,10 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
 #pragma unroll
             for (int pp = 0; pp < 4; pp++) {                   // 4 columns = the four outputs of one p
                 const uint32_t taddr = tb + ((uint32_t)((warp & 3) * 32) << 16) + 4 * (half * 4 + pp);
+                // the 13 digit sums S_12..S_24 of each of the 4 outputs: groups of three combine EXACTLY in one
+                // double (|S| < 2^31: S_a + 2^8 S_b + 2^16 S_c < 2^48), the five group values are added in double-double
                 uint32_t v[7][4];
-                __int128 lo[4], hi[4];
+                double grp[5][4];
 #pragma unroll
                 for (int sidx = 0; sidx < 7; sidx++)
                     asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
@@ -175,26 +171,28 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
                 for (int e = 0; e < 4; e++) {
-                    lo[e] = 0;
-#pragma unroll
-                    for (int sidx = 0; sidx < 7; sidx++) lo[e] += (__int128)(int)v[sidx][e] << (8 * sidx);
+                    grp[0][e] = __fma_rn((double)(int)v[2][e], 65536.0, __fma_rn((double)(int)v[1][e], 256.0, (double)(int)v[0][e]));
+                    grp[1][e] = __fma_rn((double)(int)v[5][e], 65536.0, __fma_rn((double)(int)v[4][e], 256.0, (double)(int)v[3][e]));
+                    grp[2][e] = (double)(int)v[6][e];
                 }
 #pragma unroll
                 for (int sidx = 0; sidx < 6; sidx++)
                     asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
                                  : "=r"(v[sidx][0]), "=r"(v[sidx][1]), "=r"(v[sidx][2]), "=r"(v[sidx][3]) : "r"(taddr + (7 + sidx) * 32));
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-                for (int e = 0; e < 4; e++) {
-                    hi[e] = 0;
-#pragma unroll
-                    for (int sidx = 0; sidx < 6; sidx++) hi[e] += (__int128)(int)v[sidx][e] << (8 * sidx);
-                }
-                // value = 2^-204 (256^12 lo + 256^19 hi) = 2^-108 lo + 2^-52 hi
                 dd T[4];
 #pragma unroll
-                for (int e = 0; e < 4; e++)
-                    T[e] = dd_add(dd_scale2(i128_to_dd(lo[e]), 0x1p-108), dd_scale2(i128_to_dd(hi[e]), 0x1p-52));
+                for (int e = 0; e < 4; e++) {
+                    grp[2][e] = __fma_rn((double)(int)v[1][e], 65536.0, __fma_rn((double)(int)v[0][e], 256.0, grp[2][e]));   // S_18..S_20
+                    grp[3][e] = __fma_rn((double)(int)v[4][e], 65536.0, __fma_rn((double)(int)v[3][e], 256.0, (double)(int)v[2][e]));
+                    grp[4][e] = (double)(int)v[5][e];
+                    // value = 2^-204 sum_g 256^(12 + 3 g) grp[g] = sum_g 2^(-108 + 24 g) grp[g], smallest first
+                    dd t = dd{__dmul_rn(grp[0][e], 0x1p-108), 0.0};
+                    t = dd_add_d(t, __dmul_rn(grp[1][e], 0x1p-84));
+                    t = dd_add_d(t, __dmul_rn(grp[2][e], 0x1p-60));
+                    t = dd_add_d(t, __dmul_rn(grp[3][e], 0x1p-36));
+                    T[e] = dd_add_d(t, __dmul_rn(grp[4][e], 0x1p-12));
+                }
                 const int p = pb8 * 8 + half * 4 + pp;
                 if (j < N && p < Ppad) {
                     const dd I = dd_dot2(ar[pp], T[1], ai[pp], T[0], -1.0);     // Im[conj(A) T]
