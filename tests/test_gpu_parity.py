@@ -146,8 +146,9 @@ def test_determinism(shd):
     assert np.array_equal(a["grad_hi"], b["grad_hi"]) and np.array_equal(a["grad_lo"], b["grad_lo"])
 
 
+@pytest.mark.parametrize("engine", [0, 2])
 @pytest.mark.parametrize("name,reps", [("cfg2", 200), ("cfg4", 60), ("cfg5", 20), ("cfg3", 100)])
-def test_determinism_stress(shd, name, reps):
+def test_determinism_stress(shd, name, reps, engine):
     """Many repeats of the same evaluation must be bit-identical in EVERY output word.  A stage of the
     TMA ring released before all its LDS were consumed once gave one warp in ~10^5 a stale limb in
     about one evaluation in five: a single repeat does not catch that."""
@@ -155,6 +156,7 @@ def test_determinism_stress(shd, name, reps):
     cfg = inputs.CONFIGS[name]
     hi, lo = inputs.uniform_positions(cfg, 0)
     h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    h.set_engine(engine)
     th, tl = shd.from_host(hi, lo)
     gh, gl = torch.empty_like(th), torch.empty_like(th)
     phi0, _, _ = h.energy_grad(th, tl, gh, gl)
