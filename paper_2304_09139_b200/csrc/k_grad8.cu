@@ -157,6 +157,7 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
                 ar[pp] = limbs_to_dd8(araw[pp][0].x, araw[pp][1].x, araw[pp][2].x);
                 ai[pp] = limbs_to_dd8(araw[pp][0].y, araw[pp][1].y, araw[pp][2].y);
             }
+            dd Tall[4][4];
 #pragma unroll
             for (int pp = 0; pp < 4; pp++) {                   // 4 columns = the four outputs of one p
                 const uint32_t taddr = tb + ((uint32_t)((warp & 3) * 32) << 16) + 4 * (half * 4 + pp);
@@ -180,7 +181,6 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
                     asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
                                  : "=r"(v[sidx][0]), "=r"(v[sidx][1]), "=r"(v[sidx][2]), "=r"(v[sidx][3]) : "r"(taddr + (7 + sidx) * 32));
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                dd T[4];
 #pragma unroll
                 for (int e = 0; e < 4; e++) {
                     grp[2][e] = __fma_rn((double)(int)v[1][e], 65536.0, __fma_rn((double)(int)v[0][e], 256.0, grp[2][e]));   // S_18..S_20
@@ -191,8 +191,15 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
                     t = dd_add_d(t, __dmul_rn(grp[1][e], 0x1p-84));
                     t = dd_add_d(t, __dmul_rn(grp[2][e], 0x1p-60));
                     t = dd_add_d(t, __dmul_rn(grp[3][e], 0x1p-36));
-                    T[e] = dd_add_d(t, __dmul_rn(grp[4][e], 0x1p-12));
+                    Tall[pp][e] = dd_add_d(t, __dmul_rn(grp[4][e], 0x1p-12));
                 }
+            }
+            // tensor memory is drained: the next block's instructions may start while the contractions below run
+            asm volatile("tcgen05.fence::before_thread_sync;");
+            mbar_arrive(smem_u32(&tempty_bar));
+#pragma unroll
+            for (int pp = 0; pp < 4; pp++) {
+                const dd* T = Tall[pp];
                 const int p = pb8 * 8 + half * 4 + pp;
                 if (j < N && p < Ppad) {
                     const dd I = dd_dot2(ar[pp], T[1], ai[pp], T[0], -1.0);     // Im[conj(A) T]
@@ -207,8 +214,6 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
 #undef GACC8
                 }
             }
-            asm volatile("tcgen05.fence::before_thread_sync;");
-            mbar_arrive(smem_u32(&tempty_bar));                // this thread has read its lane: 128 arrivals free TMEM
             nblock++;
         }
         if (j < N) {
