@@ -53,23 +53,23 @@ __device__ cdd expi_turns(dd t) {
 
 struct limbs { double x0, x1, x2; };
 
-// trunc(x 2^102) of a double as a 128-bit integer (|x| <= 2), integer pipe only
-__device__ __forceinline__ __int128 fix102(double x) {
-    const long long b = __double_as_longlong(x);
-    const int e = (int)((b >> 52) & 0x7ff);
-    if (e == 0) return 0;
-    const unsigned long long m = ((unsigned long long)b & 0xfffffffffffffULL) | (1ULL << 52);
-    const int sh = e - 1075 + 102;                       // x = m 2^(e - 1075)
-    __int128 v = sh >= 0 ? ((__int128)m << sh) : (sh > -64 ? (__int128)(m >> (-sh)) : (__int128)0);
-    return b < 0 ? -v : v;
-}
-// the 13 balanced base-256 digits d_i in [-128, 127] of X = trunc(hi 2^102) + trunc(lo 2^102): bytes of
-// X + sum_i 128 256^i, minus 128 (no carries); sum_i d_i 256^i = X exactly
+// The 13 balanced base-256 digits d_i in [-128, 127] of X = trunc(x 2^102), x = hi + lo, |x| <= 1 (a few ulps more
+// are fine): the bytes of X + sum_i 128 256^i, minus 128 (no carries); sum_i d_i 256^i = X.  X is assembled in two
+// 64-bit words split at 2^56: hi 2^46 = H + r (H integer, 0 <= r < 1, both exact), so
+// X = H 2^56 + trunc(r 2^56) + trunc(lo 2^102); the last two terms are below 2^57 in magnitude.
 __device__ __forceinline__ void digits13(dd x, signed char* d) {
-    const __int128 off = ((__int128)0x0000008080808080ULL << 64) | (__int128)0x8080808080808080ULL;
-    const unsigned __int128 y = (unsigned __int128)(fix102(x.h) + fix102(x.l) + off);
+    const double t = __dmul_rn(x.h, 0x1p46);                       // exact
+    const double H = floor(t);
+    const double r = __dadd_rn(t, -H);                             // exact, in [0, 1)
+    long long xlo = __double2ll_rz(__dmul_rn(r, 0x1p56)) + __double2ll_rz(__dmul_rn(x.l, 0x1p102));
+    long long xhi = __double2ll_rz(H);
+    xlo += 0x80808080808080LL;                                     // digits 0..6 of the offset
+    xhi += 0x808080808080LL + (xlo >> 56);                         // digits 7..12, carry (arithmetic shift: may be -1)
+    const unsigned long long ylo = (unsigned long long)xlo & 0xffffffffffffffULL, yhi = (unsigned long long)xhi;
 #pragma unroll
-    for (int i = 0; i < SHD_I8_DIGITS; i++) d[i] = (signed char)((int)((y >> (8 * i)) & 0xff) - 128);
+    for (int i = 0; i < 7; i++) d[i] = (signed char)((int)((ylo >> (8 * i)) & 0xff) - 128);
+#pragma unroll
+    for (int i = 0; i < 6; i++) d[7 + i] = (signed char)((int)((yhi >> (8 * i)) & 0xff) - 128);
 }
 
 // |x| <= 1 (normalised dd) -> limbs (shd_internal.h)
