@@ -104,15 +104,18 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
                 mbar_wait(smem_u32(&full_bar[s]), (uint32_t)((i / G8_NST) & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;");
                 const uint32_t sA = s0 + s * G8_STAGE, sW = sA + G8_A;
+                // descriptors differ only in the 14-bit address field: one base per operand, compile-time offsets
+                const uint64_t dA0 = g8_desc(sA), dW0 = g8_desc(sW);
+#pragma unroll
                 for (int ii = G8_ND - 1; ii >= 0; ii--) {
                     const int n = (ii + 1) * 32, l0 = G8_ND - 1 - ii;
-                    const uint64_t da = g8_desc(sA + ii * G8_ASLAB);
+                    const uint64_t da = dA0 + (uint64_t)((ii * G8_ASLAB) >> 4);
                     const uint32_t acc = (!fresh || ii < G8_ND - 1) ? 1u : 0u;
                     if (n <= 256) {
-                        g8_mma(tb, da, g8_desc(sW + l0 * G8_WSLAB), g8_idesc(n), acc);
+                        g8_mma(tb, da, dW0 + (uint64_t)((l0 * G8_WSLAB) >> 4), g8_idesc(n), acc);
                     } else {
-                        g8_mma(tb, da, g8_desc(sW + l0 * G8_WSLAB), g8_idesc(256), acc);
-                        g8_mma(tb + 256, da, g8_desc(sW + (l0 + 8) * G8_WSLAB), g8_idesc(n - 256), acc);
+                        g8_mma(tb, da, dW0 + (uint64_t)((l0 * G8_WSLAB) >> 4), g8_idesc(256), acc);
+                        g8_mma(tb + 256, da, dW0 + (uint64_t)(((l0 + 8) * G8_WSLAB) >> 4), g8_idesc(n - 256), acc);
                     }
                 }
                 g8_commit(smem_u32(&empty_bar[s]));

@@ -99,15 +99,18 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
                 const uint32_t sA = s0 + s * R8_STAGE, sB = sA + R8_A;
                 // A digit 12 first: its partners are all 13 B digits = all 416 columns, so on the first
                 // K-step it initialises every accumulator (accumulate = 0), everything else accumulates
+                // descriptors differ only in the 14-bit address field: one base per operand, compile-time offsets
+                const uint64_t dA0 = umma_desc(sA), dB0 = umma_desc(sB);
+#pragma unroll
                 for (int ii = R8_ND - 1; ii >= 0; ii--) {
                     const int n = (ii + 1) * 32, l0 = R8_ND - 1 - ii;
-                    const uint64_t da = umma_desc(sA + ii * R8_ASLAB);
+                    const uint64_t da = dA0 + (uint64_t)((ii * R8_ASLAB) >> 4);
                     const uint32_t acc = (i > 0 || ii < R8_ND - 1) ? 1u : 0u;
                     if (n <= 256) {
-                        umma_i8(tb, da, umma_desc(sB + l0 * R8_BSLAB), umma_idesc_i8(n), acc);
+                        umma_i8(tb, da, dB0 + (uint64_t)((l0 * R8_BSLAB) >> 4), umma_idesc_i8(n), acc);
                     } else {
-                        umma_i8(tb, da, umma_desc(sB + l0 * R8_BSLAB), umma_idesc_i8(256), acc);
-                        umma_i8(tb + 256, da, umma_desc(sB + (l0 + 8) * R8_BSLAB), umma_idesc_i8(n - 256), acc);
+                        umma_i8(tb, da, dB0 + (uint64_t)((l0 * R8_BSLAB) >> 4), umma_idesc_i8(256), acc);
+                        umma_i8(tb + 256, da, dB0 + (uint64_t)(((l0 + 8) * R8_BSLAB) >> 4), umma_idesc_i8(n - 256), acc);
                     }
                 }
                 umma_commit(smem_u32(&empty_bar[s]));          // arrives when the tensor core is done with stage s
