@@ -419,3 +419,26 @@ def test_int8_engine_full_size_and_determinism(shd, oracle):
         for x, y in zip(ref, [gh, gl] + list(h.rho())):
             assert torch.equal(x, y), rep
     h.close()
+
+
+def test_int8_engine_worst_case_sums(shd, oracle):
+    """All particles on one site: every digit product of a (p, q) cell has the same value for all particles, so
+    the s32 digit sums in tensor memory take their largest possible magnitude per particle count (the
+    overflow bound of k_rho8 is 13 pairs x 8224 particles x 2^14 < 2^31).  Closed form: rho(k) = N exp(i k.r0),
+    |rho|^2 = N^2, gradient = 0; sites chosen so that the digits are large (coordinates near L/2 give phasors
+    near -1, i.e. digits near -128)."""
+    d, N, L, m_star = 2, 32768, 64.0, 25          # N a power of two: rho / N below is exact
+    for r0 in ([31.99999, 32.00001], [1.3125, 4.75], [63.999999, 0.000001]):
+        hi, lo = inputs.single_site(d, N, r0)
+        h = shd.Shd(d, N, L, m_star=m_star)
+        h.set_engine(2)
+        th, tl = shd.from_host(hi, lo)
+        phi, gh, gl = h.energy_grad(th, tl)
+        rho = [t.cpu().numpy() for t in h.rho()]
+        n = oracle.enumerate_Q(d, m_star)
+        ref_re, ref_im = oracle.rho(d, 1, L, np.array(r0), np.zeros(2), n)       # one particle, times N
+        e = oracle.cabsdiff_dd(ref_re, ref_im, rho[0] / N, rho[1] / N, rho[2] / N, rho[3] / N)
+        assert e.max() <= 1e-28, e.max()
+        assert abs(phi[0] - float(N) ** 2 * len(n)) <= 1e-12 * float(N) ** 2 * len(n)
+        assert float(gh.abs().max()) <= 1e-27 * N * len(n) * 10.0 * N
+        h.close()
