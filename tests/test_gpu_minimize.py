@@ -123,13 +123,15 @@ def test_minimize_argument_errors(shd):
 
 
 # --------------------------------------------------------------------------- FIRE (kind = 1)
-def test_fire_trajectory_matches_oracle(shd, oracle):
+@pytest.mark.parametrize("engine", [0, 2])
+def test_fire_trajectory_matches_oracle(shd, oracle, engine):
     """FIRE has no line search, only the sign test P > 0: the device FIRE (dd) and the binary128 FIRE
     follow the same trajectory, so here the STEP itself is compared, not just the outcome: positions
     after 1, 10, 40 and 200 moves from BASELINE.json configs[0]'s seeded start."""
     cfg = inputs.CONFIGS["cfg1"]
     hi, lo = inputs.uniform_positions(cfg, 0)
     h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    h.set_engine(engine)                 # 2: both O(N M) passes on the INT8 tensor cores
     n = h.k()
     for K, tol in ((2, 1e-30), (11, 1e-29), (41, 1e-27), (201, 1e-26)):
         th, tl = shd.from_host(hi, lo)
@@ -186,8 +188,9 @@ def test_fire_resume_is_a_continuation(shd):
     h.close()
 
 
+@pytest.mark.parametrize("engine", [0, 2])
 @pytest.mark.parametrize("name,floor", [("cfg1", 1e-50), ("cfg2", 1e-48)])
-def test_quench_to_the_precision_floor(shd, oracle, name, floor):
+def test_quench_to_the_precision_floor(shd, oracle, name, floor, engine):
     """the paper quenches "until Phi is at the minimum value attainable within machine precision" and
     reports S_max ~ 1e-51 (Fig. 2a).  With smax_tol = 0 the device L-BFGS runs until its line search
     finds no further decrease (SHD_ESTALL); the ORACLE's S_max on the final positions must then be at the
@@ -195,6 +198,7 @@ def test_quench_to_the_precision_floor(shd, oracle, name, floor):
     cfg = inputs.CONFIGS[name]
     hi, lo = inputs.uniform_positions(cfg, 0)
     h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    h.set_engine(engine)
     th, tl = shd.from_host(hi, lo)
     rep = h.minimize(th, tl, smax_tol=0.0, max_evals=20000, poll_every=32)
     assert rep["status"] == shd.SHD_ESTALL, rep
