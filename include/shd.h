@@ -115,8 +115,9 @@ int shd_get_rho(shd_ctx* h, double* re_hi, double* re_lo, double* im_hi, double*
  * (two exact limbs), half the FMAs; per-term error ~2^-45, i.e. |rho| to ~3e-14 sqrt(N), enough to drive
  * S_max to ~1e-22.  limbs = 1: operands at 22 bits (one exact limb), one sixth of the FMAs, per-term error
  * ~2^-23: the first decades of a quench (S_max down to ~1e-10).  Everything else (phasor tables, reductions,
- * minimizer algebra) stays double-double.  Applies to every later call on the handle.
- * Errors: SHD_EINVAL (limbs not 1, 2 or 3).
+ * minimizer algebra) stays double-double.  On the INT8 engines (shd_set_engine) the same three levels select
+ * the 13, 7 or 4 most significant base-256 digits of the operands (102, 54, 30 bits; 91, 28, 10 digit pairs).
+ * Applies to every later call on the handle.  Errors: SHD_EINVAL (limbs not 1, 2 or 3).
  */
 int shd_set_precision(shd_ctx* h, int limbs);
 
@@ -125,8 +126,8 @@ int shd_set_precision(shd_ctx* h, int limbs);
  * (k_rho.cu).  1: exact digit-sliced contraction on the INT8 tensor cores (tcgen05.mma.kind::i8, k_rho8.cu):
  * operands as 13 balanced base-256 digits of trunc(x 2^102), the 91 digit pairs with i + l >= 12, s32
  * accumulators in tensor memory (at most 8192 particles per CTA, so they are exact), the same double-double
- * result within the same tolerances.  Applies to 3-limb evaluations (shd_set_precision 3); allocates the digit
- * tables on first use.  Errors: SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA.
+ * result within the same tolerances.  2: the gradient pass too (k_grad8.cu).  shd_set_precision selects the
+ * number of digits on these engines.  Allocates the digit tables on first use.  Errors: SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA.
  */
 int shd_set_engine(shd_ctx* h, int rho_engine);
 

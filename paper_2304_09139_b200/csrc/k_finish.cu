@@ -293,7 +293,7 @@ cudaError_t shd_launch_sfactor(shd_ctx* h, double* S_out, double* scratch, doubl
 
 cudaError_t shd_launch_finish(shd_ctx* h)
 {
-    const bool i8 = h->rho_engine >= 1 && h->nlimb >= 3;
+    const bool i8 = h->rho_engine >= 1;
     const int ntiles = i8 ? h->ntiles8 : h->ntiles;
     const int nb = (int)(((long)ntiles * 1024 + 255) / 256);
     k_finish1<<<nb, 256, 0, h->stream>>>(h->d_part, i8 ? h->nsplit8 : h->nsplit, ntiles, i8 ? SHD_I8_PT : 32,
@@ -318,7 +318,7 @@ cudaError_t shd_launch_wtable8(shd_ctx* h)
 
 cudaError_t shd_launch_ctable(shd_ctx* h)
 {
-    if (h->rho_engine == 2 && h->nlimb >= 3) return shd_launch_wtable8(h);   // the INT8 gradient pass reads W8 instead
+    if (h->rho_engine == 2) return shd_launch_wtable8(h);   // the INT8 gradient pass reads W8 instead
     long ncell = (long)h->npb16 * 16 * h->Qpad;
     k_ctable<<<(unsigned)((ncell + 255) / 256), 256, 0, h->stream>>>(
         h->npb16, h->Qpad, h->qscale_log2, h->d_cell_kp, h->d_cell_km, h->M, h->d_v, h->d_rho, h->d_scal, h->d_C, h->d_skip);

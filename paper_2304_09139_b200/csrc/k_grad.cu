@@ -325,7 +325,7 @@ cudaError_t shd_grad_configure()
 
 cudaError_t shd_launch_grad(shd_ctx* h, double* grad_hi, double* grad_lo)
 {
-    if (h->rho_engine == 2 && h->nlimb >= 3) {          // INT8 tensor-core gradient pass (k_grad8.cu)
+    if (h->rho_engine == 2) {          // INT8 tensor-core gradient pass (k_grad8.cu)
         cudaError_t e = shd_launch_grad8_main(h);
         if (e != cudaSuccess) return e;
         const long n8 = (long)h->d * h->N;

@@ -45,6 +45,8 @@ __device__ __forceinline__ dd limbs_to_dd8(double x0, double x1, double x2) {
     return fast_two_sum(__dadd_rn(x0, x1), x2);
 }
 
+// ND = 13: full precision; 7 / 4: the most significant digits only (shd_set_precision 2 / 1; see k_rho8.cu)
+template <int ND>
 __global__ void __launch_bounds__(320, 1) k_grad8(
     int d, long N, long Npad, long njb128, int Ppad, int qscale_log2, int nkq,
     const int2* __restrict__ steps, int nsteps, int nseg, const int* __restrict__ wT,
@@ -76,6 +78,7 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;");
     const uint32_t tb = tmem_base;
+    constexpr int OFF = G8_ND - ND;                  // first (least significant) digit used
 
     if (warp == 8) {
         if (lane == 0) {
@@ -85,9 +88,9 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
                 if (i >= G8_NST) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((i / G8_NST - 1) & 1));
                 const uint32_t bar = smem_u32(&full_bar[s]);
                 const int2 st = steps[c_begin + i];           // x: pb8 * nkq + kstep,  y: kstep | end << 16
-                mbar_expect_tx(bar, G8_STAGE);
-                tma_load_1d(s0 + s * G8_STAGE, gA + (size_t)(st.y & 0xffff) * G8_A, G8_A, bar);
-                tma_load_1d(s0 + s * G8_STAGE + G8_A, W8 + (size_t)st.x * G8_W, G8_W, bar);
+                mbar_expect_tx(bar, ND * (G8_ASLAB + G8_WSLAB));
+                tma_load_1d(s0 + s * G8_STAGE + OFF * G8_ASLAB, gA + (size_t)(st.y & 0xffff) * G8_A + OFF * G8_ASLAB, ND * G8_ASLAB, bar);
+                tma_load_1d(s0 + s * G8_STAGE + G8_A + OFF * G8_WSLAB, W8 + (size_t)st.x * G8_W + OFF * G8_WSLAB, ND * G8_WSLAB, bar);
             }
         }
     } else if (warp == 9) {
@@ -107,10 +110,10 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
                 // descriptors differ only in the 14-bit address field: one base per operand, compile-time offsets
                 const uint64_t dA0 = g8_desc(sA), dW0 = g8_desc(sW);
 #pragma unroll
-                for (int ii = G8_ND - 1; ii >= 0; ii--) {
-                    const int n = (ii + 1) * 32, l0 = G8_ND - 1 - ii;
-                    const uint64_t da = dA0 + (uint64_t)((ii * G8_ASLAB) >> 4);
-                    const uint32_t acc = (!fresh || ii < G8_ND - 1) ? 1u : 0u;
+                for (int ii = ND - 1; ii >= 0; ii--) {              // relative digit i' (absolute OFF + i')
+                    const int n = (ii + 1) * 32, l0 = OFF + ND - 1 - ii;
+                    const uint64_t da = dA0 + (uint64_t)(((OFF + ii) * G8_ASLAB) >> 4);
+                    const uint32_t acc = (!fresh || ii < ND - 1) ? 1u : 0u;
                     if (n <= 256) {
                         g8_mma(tb, da, dW0 + (uint64_t)((l0 * G8_WSLAB) >> 4), g8_idesc(n), acc);
                     } else {
@@ -164,37 +167,47 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
 #pragma unroll
             for (int pp = 0; pp < 4; pp++) {                   // 4 columns = the four outputs of one p
                 const uint32_t taddr = tb + ((uint32_t)((warp & 3) * 32) << 16) + 4 * (half * 4 + pp);
-                // the 13 digit sums S_12..S_24 of each of the 4 outputs: groups of three combine EXACTLY in one
-                // double (|S| < 2^31: S_a + 2^8 S_b + 2^16 S_c < 2^48), the five group values are added in double-double
-                uint32_t v[7][4];
-                double grp[5][4];
+                // the ND digit sums of each of the 4 outputs: groups of three combine EXACTLY in one double
+                // (|S| < 2^31: S_a + 2^8 S_b + 2^16 S_c < 2^48), the group values are added in double-double.
+                // Column c holds the absolute digit sum s = ND - 1 + 2 OFF + c, weight 2^(8 s - 204).
+                constexpr int NB1 = ND < 7 ? ND : 7, NG = (ND + 2) / 3;
+                uint32_t v[NB1][4];
+                double grp[NG][4];
 #pragma unroll
-                for (int sidx = 0; sidx < 7; sidx++)
+                for (int g = 0; g < NG; g++)
+#pragma unroll
+                    for (int e = 0; e < 4; e++) grp[g][e] = 0.0;
+#pragma unroll
+                for (int c = 0; c < NB1; c++)
                     asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
-                                 : "=r"(v[sidx][0]), "=r"(v[sidx][1]), "=r"(v[sidx][2]), "=r"(v[sidx][3]) : "r"(taddr + sidx * 32));
+                                 : "=r"(v[c][0]), "=r"(v[c][1]), "=r"(v[c][2]), "=r"(v[c][3]) : "r"(taddr + c * 32));
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-                for (int e = 0; e < 4; e++) {
-                    grp[0][e] = __fma_rn((double)(int)v[2][e], 65536.0, __fma_rn((double)(int)v[1][e], 256.0, (double)(int)v[0][e]));
-                    grp[1][e] = __fma_rn((double)(int)v[5][e], 65536.0, __fma_rn((double)(int)v[4][e], 256.0, (double)(int)v[3][e]));
-                    grp[2][e] = (double)(int)v[6][e];
+                for (int c = 0; c < NB1; c++)
+#pragma unroll
+                    for (int e = 0; e < 4; e++)
+                        grp[c / 3][e] = __fma_rn((double)(int)v[c][e], (double)(1 << (8 * (c % 3))), grp[c / 3][e]);
+                if (ND > 7) {
+#pragma unroll
+                    for (int c = 7; c < ND; c++)
+                        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+                                     : "=r"(v[c - 7][0]), "=r"(v[c - 7][1]), "=r"(v[c - 7][2]), "=r"(v[c - 7][3]) : "r"(taddr + c * 32));
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                    for (int c = 7; c < ND; c++)
+#pragma unroll
+                        for (int e = 0; e < 4; e++)
+                            grp[c / 3][e] = __fma_rn((double)(int)v[c - 7][e], (double)(1 << (8 * (c % 3))), grp[c / 3][e]);
                 }
 #pragma unroll
-                for (int sidx = 0; sidx < 6; sidx++)
-                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
-                                 : "=r"(v[sidx][0]), "=r"(v[sidx][1]), "=r"(v[sidx][2]), "=r"(v[sidx][3]) : "r"(taddr + (7 + sidx) * 32));
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
                 for (int e = 0; e < 4; e++) {
-                    grp[2][e] = __fma_rn((double)(int)v[1][e], 65536.0, __fma_rn((double)(int)v[0][e], 256.0, grp[2][e]));   // S_18..S_20
-                    grp[3][e] = __fma_rn((double)(int)v[4][e], 65536.0, __fma_rn((double)(int)v[3][e], 256.0, (double)(int)v[2][e]));
-                    grp[4][e] = (double)(int)v[5][e];
-                    // value = 2^-204 sum_g 256^(12 + 3 g) grp[g] = sum_g 2^(-108 + 24 g) grp[g], smallest first
-                    dd t = dd{__dmul_rn(grp[0][e], 0x1p-108), 0.0};
-                    t = dd_add_d(t, __dmul_rn(grp[1][e], 0x1p-84));
-                    t = dd_add_d(t, __dmul_rn(grp[2][e], 0x1p-60));
-                    t = dd_add_d(t, __dmul_rn(grp[3][e], 0x1p-36));
-                    Tall[pp][e] = dd_add_d(t, __dmul_rn(grp[4][e], 0x1p-12));
+                    dd t{0.0, 0.0};
+#pragma unroll
+                    for (int g = 0; g < NG; g++) {                  // smallest weight first
+                        const double w = __longlong_as_double((long long)(1023 + 8 * (ND - 1 + 2 * OFF + 3 * g) - 204) << 52);
+                        t = dd_add_d(t, __dmul_rn(grp[g][e], w));
+                    }
+                    Tall[pp][e] = t;
                 }
             }
             // tensor memory is drained: the next block's instructions may start while the contractions below run
@@ -237,16 +250,24 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
 
 cudaError_t shd_grad8_configure()
 {
-    return cudaFuncSetAttribute(k_grad8, cudaFuncAttributeMaxDynamicSharedMemorySize, G8_SMEM);
+    cudaError_t e = cudaFuncSetAttribute(k_grad8<13>, cudaFuncAttributeMaxDynamicSharedMemorySize, G8_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad8<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, G8_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad8<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, G8_SMEM);
+    return e;
 }
 
 // k_gradsum (k_grad.cu) adds the segments' partial gradients and applies 4 pi / L / cscale
 cudaError_t shd_launch_grad8_main(shd_ctx* h)
 {
-    k_grad8<<<(unsigned)(h->njb128 * h->nseg8), 320, G8_SMEM, h->stream>>>(
-        h->d, h->N, h->Npad, h->njb128, h->npb * 32, h->qscale_log2, h->nkq8,
-        reinterpret_cast<const int2*>(h->d_steps8), h->nsteps8, h->nseg8, h->d_wT,
-        h->d_A, h->d_Bg8, h->d_W8, h->d_gpart, h->d_skip);
+#define LAUNCH_GRAD8(NDV)                                                                            \
+    k_grad8<NDV><<<(unsigned)(h->njb128 * h->nseg8), 320, G8_SMEM, h->stream>>>(                      \
+        h->d, h->N, h->Npad, h->njb128, h->npb * 32, h->qscale_log2, h->nkq8,                          \
+        reinterpret_cast<const int2*>(h->d_steps8), h->nsteps8, h->nseg8, h->d_wT,                     \
+        h->d_A, h->d_Bg8, h->d_W8, h->d_gpart, h->d_skip)
+    if (h->nlimb >= 3) LAUNCH_GRAD8(13);
+    else if (h->nlimb == 2) LAUNCH_GRAD8(7);
+    else LAUNCH_GRAD8(4);
+#undef LAUNCH_GRAD8
     h->last_launches += 1;
     return cudaGetLastError();
 }

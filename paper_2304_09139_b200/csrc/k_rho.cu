@@ -208,7 +208,7 @@ cudaError_t shd_rho_configure()
 
 cudaError_t shd_launch_rho(shd_ctx* h)
 {
-    if (h->rho_engine >= 1 && h->nlimb >= 3) return shd_launch_rho8(h);      // INT8 tensor-core engine (k_rho8.cu)
+    if (h->rho_engine >= 1) return shd_launch_rho8(h);      // INT8 tensor-core engine (k_rho8.cu)
     unsigned grid = (unsigned)(h->ntiles * h->nsplit);
 #define LAUNCH_RHO(NLV)                                                                                   \
     k_rho<NLV><<<grid, NW * 32 + 128, RHO_SMEM, h->stream>>>(h->d_A, h->d_B, h->d_tile_pb, h->d_tile_qb,    \

@@ -47,6 +47,10 @@ __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
 
+// ND = 13: full precision.  ND = 7 / 4: the "fast" precisions of shd_set_precision(h, 2 / 1) on this engine: only the
+// ND most significant digits of both operands (54 / 30 bits) and the digit pairs with i' + l' >= ND - 1
+// (28 / 10 instead of 91), in 32 ND tensor-memory columns.
+template <int ND>
 __global__ void __launch_bounds__(192, 1) k_rho8(
     const signed char* __restrict__ A8, const signed char* __restrict__ B8,
     const int* __restrict__ tile_pb, const int* __restrict__ tile_qb, int ntiles,
@@ -76,6 +80,7 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;");
     const uint32_t tb = tmem_base;
+    constexpr int OFF = R8_ND - ND;                  // first (least significant) digit used
 
     if (warp == 4) {
         if (lane == 0) {
@@ -85,9 +90,9 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
                 const int s = i % R8_NST;
                 if (i >= R8_NST) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((i / R8_NST - 1) & 1));
                 const uint32_t bar = smem_u32(&full_bar[s]);
-                mbar_expect_tx(bar, R8_STAGE);
-                tma_load_1d(s0 + s * R8_STAGE, gA + (size_t)i * R8_A, R8_A, bar);
-                tma_load_1d(s0 + s * R8_STAGE + R8_A, gB + (size_t)i * R8_B, R8_B, bar);
+                mbar_expect_tx(bar, ND * (R8_ASLAB + R8_BSLAB));
+                tma_load_1d(s0 + s * R8_STAGE + OFF * R8_ASLAB, gA + (size_t)i * R8_A + OFF * R8_ASLAB, ND * R8_ASLAB, bar);
+                tma_load_1d(s0 + s * R8_STAGE + R8_A + OFF * R8_BSLAB, gB + (size_t)i * R8_B + OFF * R8_BSLAB, ND * R8_BSLAB, bar);
             }
         }
     } else if (warp == 5) {
@@ -97,15 +102,15 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
                 mbar_wait(smem_u32(&full_bar[s]), (uint32_t)((i / R8_NST) & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;");
                 const uint32_t sA = s0 + s * R8_STAGE, sB = sA + R8_A;
-                // A digit 12 first: its partners are all 13 B digits = all 416 columns, so on the first
-                // K-step it initialises every accumulator (accumulate = 0), everything else accumulates
-                // descriptors differ only in the 14-bit address field: one base per operand, compile-time offsets
+                // the most significant A digit first: its partners are all ND B digits = all 32 ND columns, so on the
+                // first K-step it initialises every accumulator (accumulate = 0), everything else accumulates.
+                // Descriptors differ only in the 14-bit address field: one base per operand, compile-time offsets.
                 const uint64_t dA0 = umma_desc(sA), dB0 = umma_desc(sB);
 #pragma unroll
-                for (int ii = R8_ND - 1; ii >= 0; ii--) {
-                    const int n = (ii + 1) * 32, l0 = R8_ND - 1 - ii;
-                    const uint64_t da = dA0 + (uint64_t)((ii * R8_ASLAB) >> 4);
-                    const uint32_t acc = (i > 0 || ii < R8_ND - 1) ? 1u : 0u;
+                for (int ii = ND - 1; ii >= 0; ii--) {              // relative digit i' (absolute OFF + i')
+                    const int n = (ii + 1) * 32, l0 = OFF + ND - 1 - ii;
+                    const uint64_t da = dA0 + (uint64_t)(((OFF + ii) * R8_ASLAB) >> 4);
+                    const uint32_t acc = (i > 0 || ii < ND - 1) ? 1u : 0u;
                     if (n <= 256) {
                         umma_i8(tb, da, dB0 + (uint64_t)((l0 * R8_BSLAB) >> 4), umma_idesc_i8(n), acc);
                     } else {
@@ -128,13 +133,13 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
 #pragma unroll
             for (int e = 0; e < 8; e++) sum[e] = dd{0.0, 0.0};
 #pragma unroll
-            for (int sidx = 0; sidx < R8_ND; sidx++) {          // digit sum s = 12 + sidx, weight 2^(8 s - 204), small first
+            for (int sidx = 0; sidx < ND; sidx++) {             // absolute digit sum s = ND - 1 + 2 OFF + sidx, weight 2^(8 s - 204)
                 uint32_t v[8];
                 asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                              : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
                              : "r"(tb + ((uint32_t)(warp * 32) << 16) + sidx * 32 + c0));
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                const double w = __longlong_as_double((long long)(1023 + 8 * (12 + sidx) - 204) << 52);
+                const double w = __longlong_as_double((long long)(1023 + 8 * (ND - 1 + 2 * OFF + sidx) - 204) << 52);
 #pragma unroll
                 for (int e = 0; e < 8; e++) sum[e] = dd_add_d(sum[e], __dmul_rn((double)(int)v[e], w));
             }
@@ -155,14 +160,22 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
 
 cudaError_t shd_rho8_configure()
 {
-    return cudaFuncSetAttribute(k_rho8, cudaFuncAttributeMaxDynamicSharedMemorySize, R8_SMEM);
+    cudaError_t e = cudaFuncSetAttribute(k_rho8<13>, cudaFuncAttributeMaxDynamicSharedMemorySize, R8_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rho8<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, R8_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_rho8<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, R8_SMEM);
+    return e;
 }
 
 cudaError_t shd_launch_rho8(shd_ctx* h)
 {
     const unsigned grid = (unsigned)(h->ntiles8 * h->nsplit8);
-    k_rho8<<<grid, 192, R8_SMEM, h->stream>>>(h->d_A8, h->d_B8, h->d_tile8_pb, h->d_tile8_qb, h->ntiles8,
-                                              h->nk8, h->ksteps8, h->d_part, h->d_skip);
+#define LAUNCH_RHO8(NDV)                                                                              \
+    k_rho8<NDV><<<grid, 192, R8_SMEM, h->stream>>>(h->d_A8, h->d_B8, h->d_tile8_pb, h->d_tile8_qb, h->ntiles8, \
+                                                   h->nk8, h->ksteps8, h->d_part, h->d_skip)
+    if (h->nlimb >= 3) LAUNCH_RHO8(13);
+    else if (h->nlimb == 2) LAUNCH_RHO8(7);
+    else LAUNCH_RHO8(4);
+#undef LAUNCH_RHO8
     h->last_launches += 1;
     return cudaGetLastError();
 }

@@ -342,11 +342,11 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
     dim3 grid((unsigned)((h->N + TB - 1) / TB), 2);
     k_tables<<<grid, TB, TABLES_SMEM, h->stream>>>(h->d, h->N, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2,
                                          h->d_pn0, h->d_pn1, h->d_pn2, h->Qpad, pos_hi, pos_lo,
-                                         h->d_A, h->rho_engine >= 1 && h->nlimb >= 3 ? nullptr : h->d_B,
-                                         h->rho_engine == 2 && h->nlimb >= 3 ? nullptr : h->d_Bg, with_grad_tables ? 1 : 0,
-                                         h->rho_engine >= 1 && h->nlimb >= 3 ? h->d_A8 : nullptr,
-                                         h->rho_engine >= 1 && h->nlimb >= 3 ? h->d_B8 : nullptr, h->nk8,
-                                         h->rho_engine == 2 && h->nlimb >= 3 ? h->d_Bg8 : nullptr, h->nkq8, h->d_skip);
+                                         h->d_A, h->rho_engine >= 1 ? nullptr : h->d_B,
+                                         h->rho_engine == 2 ? nullptr : h->d_Bg, with_grad_tables ? 1 : 0,
+                                         h->rho_engine >= 1 ? h->d_A8 : nullptr,
+                                         h->rho_engine >= 1 ? h->d_B8 : nullptr, h->nk8,
+                                         h->rho_engine == 2 ? h->d_Bg8 : nullptr, h->nkq8, h->d_skip);
     h->last_launches += 1;
     return cudaGetLastError();
 }

@@ -325,7 +325,7 @@ int build(shd_ctx* h, const double* v) {
 // that a handle driven on the INT8 engines only never holds them (at the paper's N they are 49 GB each).
 // Called outside any stream capture.
 int shd_prepare_tables(shd_ctx* h, bool with_grad) {
-    const bool i8 = h->nlimb >= 3;
+    const bool i8 = true;          // the engines apply to every precision (fewer digits on the fast rungs)
     int rc;
     if (!(i8 && h->rho_engine >= 1) && !h->d_B)
         if ((rc = dalloc_zero(h, &h->d_B, (size_t)h->nqb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;

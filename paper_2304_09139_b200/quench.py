@@ -68,10 +68,9 @@ def main(argv=None):
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     # rungs: (limbs, stop below this S_max); the last rung is always 3 limbs down to --tol
-    # (the fast rungs are FP64-limb modes; the INT8 engines at full precision are faster than either, so
-    # --engine 1/2 ignores the ladder)
-    rungs = [(1, args.ladder1)] if (args.ladder1 > max(args.ladder, args.tol) and args.engine == 0) else []
-    if args.ladder > args.tol and args.engine == 0:
+    # (on the INT8 engines the rungs are digit counts: 4, 7 and 13 base-256 digits)
+    rungs = [(1, args.ladder1)] if args.ladder1 > max(args.ladder, args.tol) else []
+    if args.ladder > args.tol:
         rungs.append((2, args.ladder))
     rungs.append((3, args.tol))
     rung = 0

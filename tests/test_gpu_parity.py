@@ -442,3 +442,33 @@ def test_int8_engine_worst_case_sums(shd, oracle):
         assert abs(phi[0] - float(N) ** 2 * len(n)) <= 1e-12 * float(N) ** 2 * len(n)
         assert float(gh.abs().max()) <= 1e-27 * N * len(n) * 10.0 * N
         h.close()
+
+
+def test_int8_engine_fast_precisions(shd, oracle):
+    """shd_set_precision on the INT8 engines: 2 -> the 7 most significant digits (54-bit operands, 28 digit
+    pairs), 1 -> 4 digits (30-bit operands, 10 pairs); errors against the 13-digit result as predicted by the
+    truncation, the mode really active, and full precision restored bit for bit afterwards."""
+    import torch
+    cfg = inputs.CONFIGS["cfg2"]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    h.set_engine(2)
+    th, tl = shd.from_host(hi, lo)
+    phi3, gh3, gl3 = h.energy_grad(th, tl)
+    rho3 = [x.cpu().numpy() for x in h.rho()]
+    g3 = oracle.from_dd(gh3.cpu().numpy(), gl3.cpu().numpy())
+    gmax = float(gh3.abs().max())
+    N = cfg.N
+    for limbs, bits in ((2, 52), (1, 28)):
+        h.set_precision(limbs)
+        phi, gh, gl = h.energy_grad(th, tl)
+        rho = [x.cpu().numpy() for x in h.rho()]
+        e = oracle.cabsdiff_dd(oracle.from_dd(rho3[0], rho3[1]), oracle.from_dd(rho3[2], rho3[3]), *rho)
+        eg = oracle.absdiff_dd(g3, gh.cpu().numpy(), gl.cpu().numpy())
+        print("int8 digits", limbs, e.max(), eg.max() / gmax)
+        assert 2.0 ** -(bits + 12) * np.sqrt(N) < e.max() <= 2.0 ** -bits * np.sqrt(N) * 16
+        assert eg.max() <= 2.0 ** -bits * gmax * 64
+    h.set_precision(3)
+    phi3b, gh3b, gl3b = h.energy_grad(th, tl)
+    assert phi3b == phi3 and torch.equal(gh3b, gh3) and torch.equal(gl3b, gl3)
+    h.close()
