@@ -330,7 +330,7 @@ cudaError_t shd_launch_grad(shd_ctx* h, double* grad_hi, double* grad_lo)
         if (e != cudaSuccess) return e;
         const long n8 = (long)h->d * h->N;
         k_gradsum<<<(unsigned)((n8 + 255) / 256), 256, 0, h->stream>>>(
-            n8, 2 * h->nseg8, h->L, h->d_gpart, h->d_scal, grad_hi, grad_lo, h->d_skip);
+            n8, 4 * h->nseg8, h->L, h->d_gpart, h->d_scal, grad_hi, grad_lo, h->d_skip);
         h->last_launches += 1;
         return cudaGetLastError();
     }

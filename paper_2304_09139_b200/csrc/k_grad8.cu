@@ -7,11 +7,11 @@
 // a block of 8 p (N side: 13 digit blocks of 8 p x 4 out = 32 columns, digits ascending, so one
 // tcgen05.mma.kind::i8 per particle-side digit lands all its digit pairs in the tensor-memory columns of
 // their digit sums; 18 instructions per step).  The s32 sums are exact (<= 2 Qn products per pair, Qn <= 5000).
-// At the end of a block (or of the segment) the four epilogue warps read tensor memory, thread = particle:
-// the 13 digit sums of each of its outputs are combined exactly in groups of three per double, added in
-// double-double, and contracted with the particle's own A_j[p] exactly as in k_grad.cu; the per-axis sums
-// stay in registers across blocks (two threads per particle, one per half of the block's 8 p).  Warp 8: TMA
-// producer, warp 9: MMA issuer.
+// At the end of a block (or of the segment) the sixteen epilogue warps read tensor memory, four threads per
+// particle (one per quarter of the block's 8 p): the 13 digit sums of each output are combined exactly into three
+// 64-bit integers on the integer pipe, tensor memory is released, and only then the (128-bit) integer becomes a
+// double-double that is contracted with the particle's own A_j[p] exactly as in k_grad.cu; the per-axis sums
+// stay in registers across blocks.  Warp 16: TMA producer, warp 17: MMA issuer.
 #include "pipe.cuh"
 #include "shd_internal.h"
 
@@ -25,6 +25,8 @@ constexpr int G8_W = G8_ND * G8_WSLAB;               // 13312
 constexpr int G8_STAGE = G8_A + G8_W;
 constexpr int G8_NST = 3;
 constexpr int G8_SMEM = G8_NST * G8_STAGE;
+constexpr int G8_EPI_WARPS = 16;                    // epilogue warps: four threads per particle, 2 p of the block's 8 each
+constexpr int G8_THREADS = (G8_EPI_WARPS + 2) * 32;
 
 __device__ __forceinline__ uint64_t g8_desc(uint32_t addr) {
     return (uint64_t)((addr >> 4) & 0x3FFF) | ((uint64_t)(128 >> 4) << 16) | ((uint64_t)(256 >> 4) << 32) | ((uint64_t)1 << 46);
@@ -44,10 +46,29 @@ __device__ __forceinline__ void g8_commit(uint32_t bar) {
 __device__ __forceinline__ dd limbs_to_dd8(double x0, double x1, double x2) {
     return fast_two_sum(__dadd_rn(x0, x1), x2);
 }
+// T 2^e as a double-double (relative error <= 2^-105; |T| < 2^127).  Sign and magnitude first, so that the four
+// 32-bit words of the magnitude are non-overlapping terms of one sign (no cancellation); every word becomes a
+// double through the 2^52 trick with its scale in the exponent field ((2^52 + u) 2^k - 2^52 2^k = u 2^k, one
+// exact addition), and two exact pair sums are merged.  15 additions instead of three conversions and two
+// double-double sums: the epilogue warps are bound by the FP64 pipe.
+__device__ __forceinline__ dd s128_scaled_to_dd(__int128 T, int e) {
+    const bool neg = T < 0;
+    const unsigned __int128 M = neg ? (unsigned __int128)(-T) : (unsigned __int128)T;
+    const unsigned long long mh = (unsigned long long)(M >> 64), ml = (unsigned long long)M;
+    const int e0 = 0x43300000 + (e << 20);
+    const double x0 = __dadd_rn(__hiloint2double(e0, (int)(unsigned)ml), -__hiloint2double(e0, 0));
+    const double x1 = __dadd_rn(__hiloint2double(e0 + (32 << 20), (int)(unsigned)(ml >> 32)), -__hiloint2double(e0 + (32 << 20), 0));
+    const double x2 = __dadd_rn(__hiloint2double(e0 + (64 << 20), (int)(unsigned)mh), -__hiloint2double(e0 + (64 << 20), 0));
+    const double x3 = __dadd_rn(__hiloint2double(e0 + (96 << 20), (int)(unsigned)(mh >> 32)), -__hiloint2double(e0 + (96 << 20), 0));
+    const dd hi = fast_two_sum(x3, x2), lo = fast_two_sum(x1, x0);   // exact: |x3| >= |x2| or x3 = 0, same below
+    dd r = fast_two_sum(hi.h, __dadd_rn(hi.l, lo.h));
+    r.l = __dadd_rn(r.l, lo.l);
+    return neg ? dd{-r.h, -r.l} : r;
+}
 
 // ND = 13: full precision; 7 / 4: the most significant digits only (shd_set_precision 2 / 1; see k_rho8.cu)
 template <int ND>
-__global__ void __launch_bounds__(320, 1) k_grad8(
+__global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
     int d, long N, long Npad, long njb128, int Ppad, int qscale_log2, int nkq,
     const int2* __restrict__ steps, int nsteps, int nseg, const int* __restrict__ wT,
     const double* __restrict__ A, const signed char* __restrict__ Bg8, const signed char* __restrict__ W8,
@@ -55,7 +76,9 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
 {
     if (skip && *skip) return;
     extern __shared__ __align__(1024) unsigned char smem[];
-    __shared__ __align__(8) unsigned long long full_bar[G8_NST], empty_bar[G8_NST], tfull_bar, tempty_bar;
+    // a stage holds the ND digit slabs in use of both operands; the fewer digits, the deeper the ring
+    constexpr int STG = ND * (G8_ASLAB + G8_WSLAB), NST = G8_SMEM / STG < 8 ? G8_SMEM / STG : 8;
+    __shared__ __align__(8) unsigned long long full_bar[8], empty_bar[8], tfull_bar, tempty_bar;
     __shared__ uint32_t tmem_base;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     // segment fastest: the CTAs of one particle block run side by side and share its digit slabs in L2
@@ -65,9 +88,9 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
     const int total = c_end - c_begin;
     const uint32_t s0 = smem_u32(smem);
     if (tid == 0) {
-        for (int s = 0; s < G8_NST; s++) { mbar_init(smem_u32(&full_bar[s]), 1); mbar_init(smem_u32(&empty_bar[s]), 1); }
+        for (int s = 0; s < NST; s++) { mbar_init(smem_u32(&full_bar[s]), 1); mbar_init(smem_u32(&empty_bar[s]), 1); }
         mbar_init(smem_u32(&tfull_bar), 1);
-        mbar_init(smem_u32(&tempty_bar), 256);
+        mbar_init(smem_u32(&tempty_bar), G8_EPI_WARPS * 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 0) {
@@ -80,39 +103,39 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
     const uint32_t tb = tmem_base;
     constexpr int OFF = G8_ND - ND;                  // first (least significant) digit used
 
-    if (warp == 8) {
+    if (warp == G8_EPI_WARPS) {
         if (lane == 0) {
             const signed char* gA = Bg8 + (size_t)jb * nkq * G8_A;
             for (int i = 0; i < total; i++) {
-                const int s = i % G8_NST;
-                if (i >= G8_NST) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((i / G8_NST - 1) & 1));
+                const int s = i % NST;
+                if (i >= NST) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((i / NST - 1) & 1));
                 const uint32_t bar = smem_u32(&full_bar[s]);
                 const int2 st = steps[c_begin + i];           // x: pb8 * nkq + kstep,  y: kstep | end << 16
                 mbar_expect_tx(bar, ND * (G8_ASLAB + G8_WSLAB));
-                tma_load_1d(s0 + s * G8_STAGE + OFF * G8_ASLAB, gA + (size_t)(st.y & 0xffff) * G8_A + OFF * G8_ASLAB, ND * G8_ASLAB, bar);
-                tma_load_1d(s0 + s * G8_STAGE + G8_A + OFF * G8_WSLAB, W8 + (size_t)st.x * G8_W + OFF * G8_WSLAB, ND * G8_WSLAB, bar);
+                tma_load_1d(s0 + s * STG, gA + (size_t)(st.y & 0xffff) * G8_A + OFF * G8_ASLAB, ND * G8_ASLAB, bar);
+                tma_load_1d(s0 + s * STG + ND * G8_ASLAB, W8 + (size_t)st.x * G8_W + OFF * G8_WSLAB, ND * G8_WSLAB, bar);
             }
         }
-    } else if (warp == 9) {
+    } else if (warp == G8_EPI_WARPS + 1) {
         if (lane == 0) {
             int nblock = 0;
             bool fresh = true;                                 // next step starts a new accumulation
             for (int i = 0; i < total; i++) {
-                const int s = i % G8_NST;
+                const int s = i % NST;
                 const int2 st = steps[c_begin + i];
                 if (fresh && nblock > 0) {                     // tensor memory must have been drained by the epilogue
                     mbar_wait(smem_u32(&tempty_bar), (uint32_t)((nblock - 1) & 1));
                     asm volatile("tcgen05.fence::after_thread_sync;");
                 }
-                mbar_wait(smem_u32(&full_bar[s]), (uint32_t)((i / G8_NST) & 1));
+                mbar_wait(smem_u32(&full_bar[s]), (uint32_t)((i / NST) & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;");
-                const uint32_t sA = s0 + s * G8_STAGE, sW = sA + G8_A;
+                const uint32_t sA = s0 + s * STG, sW = sA + ND * G8_ASLAB;
                 // descriptors differ only in the 14-bit address field: one base per operand, compile-time offsets
                 const uint64_t dA0 = g8_desc(sA), dW0 = g8_desc(sW);
 #pragma unroll
                 for (int ii = ND - 1; ii >= 0; ii--) {              // relative digit i' (absolute OFF + i')
-                    const int n = (ii + 1) * 32, l0 = OFF + ND - 1 - ii;
-                    const uint64_t da = dA0 + (uint64_t)(((OFF + ii) * G8_ASLAB) >> 4);
+                    const int n = (ii + 1) * 32, l0 = ND - 1 - ii;          // its partners: relative digits l0 .. ND - 1
+                    const uint64_t da = dA0 + (uint64_t)((ii * G8_ASLAB) >> 4);
                     const uint32_t acc = (!fresh || ii < ND - 1) ? 1u : 0u;
                     if (n <= 256) {
                         g8_mma(tb, da, dW0 + (uint64_t)((l0 * G8_WSLAB) >> 4), g8_idesc(n), acc);
@@ -131,22 +154,70 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
             }
         }
     } else {
-        // ---- 8 epilogue warps: thread = (particle = TMEM lane, half of the block's 8 p); columns 32 sidx + 4 p_local + out
-        const int half = warp >> 2, row = tid & 127;
+        // ---- 16 epilogue warps: thread = (particle = TMEM lane, quarter of the block's 8 p); columns 32 c + 4 p_local + out
+        const int quarter = warp >> 2, row = tid & 127;
         const long j = jb * 128 + row;
         const double qs = ldexp(1.0, qscale_log2);
         const double2* Aj = reinterpret_cast<const double2*>(A) + (size_t)(j >> 2) * 3 * 32 * 4 + (j & 3);
         dd g0{0.0, 0.0}, g1{0.0, 0.0}, g2{0.0, 0.0}, g3{0.0, 0.0};
         int nblock = 0;
-        for (int i = 0; i < total; i++) {
-            const int2 st = steps[c_begin + i];
-            if (!((st.y >> 16) || i == total - 1)) continue;
+        // next block (or segment) end at or after step i: 32 steps per look, one load latency per block
+        auto next_end = [&](int& i, int2& st) {
+            for (;;) {
+                const int ii = i + lane < total - 1 ? i + lane : total - 1;
+                const int2 sl = steps[c_begin + ii];
+                const unsigned m = __ballot_sync(0xffffffffu, (sl.y >> 16) || ii == total - 1);
+                if (m) {
+                    const int f = __ffs(m) - 1;
+                    st.x = __shfl_sync(0xffffffffu, sl.x, f);
+                    st.y = __shfl_sync(0xffffffffu, sl.y, f);
+                    i += f;
+                    return;
+                }
+                i += 32;
+            }
+        };
+        int i = 0;
+        int2 st;
+        if (total > 0) next_end(i, st);
+        while (i < total) {
             const int pb8 = st.x / nkq;
-            // this block's eight A_j[p] (limbs -> double-double), loaded while the tensor core still works on it
-            double2 araw[4][3];
+            mbar_wait(smem_u32(&tfull_bar), (uint32_t)(nblock & 1));
+            asm volatile("tcgen05.fence::after_thread_sync;");
+            // Drain: the thread's 16 columns (4 p x 4 outputs) of each of the ND digit sums, combined EXACTLY on the
+            // integer pipe into NG 64-bit group values G_g = sum_c 2^(8 (c - 4 g)) S_c (four sums per group, the top
+            // group takes a fifth).  Column block c holds the absolute digit sum s = ND - 1 + 2 OFF + c, a sum
+            // of ND - c digit pairs of <= 2 Qn <= 10^4 products each: |S_c| <= (ND - c) 10^4 2^14, which bounds
+            // the groups by 2^54.6, 2^53.9 and (top five, 5 + 4 2^8 + 3 2^16 + 2 2^24 + 2^32 pairs-weights) 2^59.3.
+            // Nothing else happens before the release, so the tensor core idles only for these loads.
+            constexpr int NG = (ND + 2) / 4;
+            long long G[NG][8];
+            const uint32_t taddr = tb + ((uint32_t)((warp & 3) * 32) << 16) + 8 * quarter;
 #pragma unroll
-            for (int pp = 0; pp < 4; pp++) {
-                const int p = pb8 * 8 + half * 4 + pp;
+            for (int c = 0; c < ND; c++) {
+                uint32_t v[8];
+                asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                             : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                             : "r"(taddr + c * 32));
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                const int g = (c / 4 < NG - 1) ? c / 4 : NG - 1, sh = 8 * (c - 4 * g);
+#pragma unroll
+                for (int e = 0; e < 8; e++) {
+                    const long long x = (long long)(int)v[e];
+                    G[g][e] = sh == 0 ? x : G[g][e] + x * (1ll << sh);
+                }
+            }
+            // tensor memory is drained: the next block's instructions start while the rest of the epilogue runs
+            asm volatile("tcgen05.fence::before_thread_sync;");
+            mbar_arrive(smem_u32(&tempty_bar));
+            int inext = i + 1;                                 // the block after this one
+            int2 stn = st;
+            if (inext < total) next_end(inext, stn);
+            // this block's A_j[p] (limbs -> double-double); the loads fly while the group values are converted
+            double2 araw[2][3];
+#pragma unroll
+            for (int pp = 0; pp < 2; pp++) {
+                const int p = pb8 * 8 + quarter * 2 + pp;
                 araw[pp][0] = araw[pp][1] = araw[pp][2] = make_double2(0.0, 0.0);
                 if (j < N && p < Ppad) {
                     const double2* ap = Aj + ((size_t)(p >> 5) * (Npad / 4) * 3 * 32 + (p & 31)) * 4;
@@ -155,68 +226,25 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
                     asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(araw[pp][2].x), "=d"(araw[pp][2].y) : "l"(ap + 256));
                 }
             }
-            mbar_wait(smem_u32(&tfull_bar), (uint32_t)(nblock & 1));
-            asm volatile("tcgen05.fence::after_thread_sync;");
-            dd ar[4], ai[4];
+            dd Tall[2][4];
 #pragma unroll
-            for (int pp = 0; pp < 4; pp++) {
+            for (int e = 0; e < 8; e++) {
+                __int128 T = (__int128)G[0][e];                         // sum_c 2^(8 c) S_c, exact
+#pragma unroll
+                for (int g = 1; g < NG; g++) T += (__int128)G[g][e] << (32 * g);
+                const dd t = s128_scaled_to_dd(T, 8 * (ND - 1 + 2 * OFF) - 204);
+                Tall[e >> 2][e & 3] = t;
+            }
+            dd ar[2], ai[2];
+#pragma unroll
+            for (int pp = 0; pp < 2; pp++) {
                 ar[pp] = limbs_to_dd8(araw[pp][0].x, araw[pp][1].x, araw[pp][2].x);
                 ai[pp] = limbs_to_dd8(araw[pp][0].y, araw[pp][1].y, araw[pp][2].y);
             }
-            dd Tall[4][4];
 #pragma unroll
-            for (int pp = 0; pp < 4; pp++) {                   // 4 columns = the four outputs of one p
-                const uint32_t taddr = tb + ((uint32_t)((warp & 3) * 32) << 16) + 4 * (half * 4 + pp);
-                // the ND digit sums of each of the 4 outputs: groups of three combine EXACTLY in one double
-                // (|S| < 2^31: S_a + 2^8 S_b + 2^16 S_c < 2^48), the group values are added in double-double.
-                // Column c holds the absolute digit sum s = ND - 1 + 2 OFF + c, weight 2^(8 s - 204).
-                constexpr int NB1 = ND < 7 ? ND : 7, NG = (ND + 2) / 3;
-                uint32_t v[NB1][4];
-                double grp[NG][4];
-#pragma unroll
-                for (int g = 0; g < NG; g++)
-#pragma unroll
-                    for (int e = 0; e < 4; e++) grp[g][e] = 0.0;
-#pragma unroll
-                for (int c = 0; c < NB1; c++)
-                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
-                                 : "=r"(v[c][0]), "=r"(v[c][1]), "=r"(v[c][2]), "=r"(v[c][3]) : "r"(taddr + c * 32));
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-                for (int c = 0; c < NB1; c++)
-#pragma unroll
-                    for (int e = 0; e < 4; e++)
-                        grp[c / 3][e] = __fma_rn((double)(int)v[c][e], (double)(1 << (8 * (c % 3))), grp[c / 3][e]);
-                if (ND > 7) {
-#pragma unroll
-                    for (int c = 7; c < ND; c++)
-                        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
-                                     : "=r"(v[c - 7][0]), "=r"(v[c - 7][1]), "=r"(v[c - 7][2]), "=r"(v[c - 7][3]) : "r"(taddr + c * 32));
-                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-                    for (int c = 7; c < ND; c++)
-#pragma unroll
-                        for (int e = 0; e < 4; e++)
-                            grp[c / 3][e] = __fma_rn((double)(int)v[c - 7][e], (double)(1 << (8 * (c % 3))), grp[c / 3][e]);
-                }
-#pragma unroll
-                for (int e = 0; e < 4; e++) {
-                    dd t{0.0, 0.0};
-#pragma unroll
-                    for (int g = 0; g < NG; g++) {                  // smallest weight first
-                        const double w = __longlong_as_double((long long)(1023 + 8 * (ND - 1 + 2 * OFF + 3 * g) - 204) << 52);
-                        t = dd_add_d(t, __dmul_rn(grp[g][e], w));
-                    }
-                    Tall[pp][e] = t;
-                }
-            }
-            // tensor memory is drained: the next block's instructions may start while the contractions below run
-            asm volatile("tcgen05.fence::before_thread_sync;");
-            mbar_arrive(smem_u32(&tempty_bar));
-#pragma unroll
-            for (int pp = 0; pp < 4; pp++) {
+            for (int pp = 0; pp < 2; pp++) {
                 const dd* T = Tall[pp];
-                const int p = pb8 * 8 + half * 4 + pp;
+                const int p = pb8 * 8 + quarter * 2 + pp;
                 if (j < N && p < Ppad) {
                     const dd I = dd_dot2(ar[pp], T[1], ai[pp], T[0], -1.0);     // Im[conj(A) T]
                     const dd R = dd_dot2(ar[pp], T[2], ai[pp], T[3], 1.0);      // Re[conj(A) T'']
@@ -231,10 +259,12 @@ __global__ void __launch_bounds__(320, 1) k_grad8(
                 }
             }
             nblock++;
+            i = inext;
+            st = stn;
         }
         if (j < N) {
             double2* o = reinterpret_cast<double2*>(gpart);
-            const size_t slot = (size_t)(seg * 2 + half) * d;          // two partials per segment (the p halves)
+            const size_t slot = (size_t)(seg * 4 + quarter) * d;       // four partials per segment (the p quarters)
             if (d > 0) o[(slot + 0) * N + j] = make_double2(g0.h, g0.l);
             if (d > 1) o[(slot + 1) * N + j] = make_double2(g1.h, g1.l);
             if (d > 2) o[(slot + 2) * N + j] = make_double2(g2.h, g2.l);
@@ -260,7 +290,7 @@ cudaError_t shd_grad8_configure()
 cudaError_t shd_launch_grad8_main(shd_ctx* h)
 {
 #define LAUNCH_GRAD8(NDV)                                                                            \
-    k_grad8<NDV><<<(unsigned)(h->njb128 * h->nseg8), 320, G8_SMEM, h->stream>>>(                      \
+    k_grad8<NDV><<<(unsigned)(h->njb128 * h->nseg8), G8_THREADS, G8_SMEM, h->stream>>>(                      \
         h->d, h->N, h->Npad, h->njb128, h->npb * 32, h->qscale_log2, h->nkq8,                          \
         reinterpret_cast<const int2*>(h->d_steps8), h->nsteps8, h->nseg8, h->d_wT,                     \
         h->d_A, h->d_Bg8, h->d_W8, h->d_gpart, h->d_skip)

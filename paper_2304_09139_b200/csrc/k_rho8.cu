@@ -13,7 +13,7 @@
 // multiplies it with all its partners l = 12-i .. 12 and lands every pair in the TMEM columns of its digit sum:
 // column 32 (i + l - 12) + (q, re/im).  18 instructions (N = 32 .. 256) per 32 particles cover the 91 pairs
 // and all four real products of the complex multiply.  13 x 32 = 416 of the 512 TMEM columns are used.
-// Warp 4: TMA producer (cp.async.bulk, 65 KB per stage, 3 stages).  Warp 5: MMA issuer (one thread);
+// Warp 4: TMA producer (cp.async.bulk, 65 KB per stage, 3 stages; 5 / 8 stages with 7 / 4 digits).  Warp 5: MMA issuer (one thread);
 // tcgen05.commit releases a stage when the tensor core has read it.  Warps 0-3: epilogue: tcgen05.ld, the 13
 // integer sums of every cell scaled by exact powers of two and added in double-double, partials written in
 // the layout k_finish1 sums over the particle splits.
@@ -58,7 +58,9 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
 {
     if (skip && *skip) return;
     extern __shared__ __align__(1024) unsigned char smem[];
-    __shared__ __align__(8) unsigned long long full_bar[R8_NST], empty_bar[R8_NST], done_bar;
+    // a stage holds the ND digit slabs in use of both operands; the fewer digits, the deeper the ring
+    constexpr int STG = ND * (R8_ASLAB + R8_BSLAB), NST = R8_SMEM / STG < 8 ? R8_SMEM / STG : 8;
+    __shared__ __align__(8) unsigned long long full_bar[8], empty_bar[8], done_bar;
     __shared__ uint32_t tmem_base;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int tile = blockIdx.x % ntiles;
@@ -68,7 +70,7 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
     const int nk = ksteps_per_split;
     const uint32_t s0 = smem_u32(smem);
     if (tid == 0) {
-        for (int s = 0; s < R8_NST; s++) { mbar_init(smem_u32(&full_bar[s]), 1); mbar_init(smem_u32(&empty_bar[s]), 1); }
+        for (int s = 0; s < NST; s++) { mbar_init(smem_u32(&full_bar[s]), 1); mbar_init(smem_u32(&empty_bar[s]), 1); }
         mbar_init(smem_u32(&done_bar), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -87,29 +89,29 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
             const signed char* gA = A8 + ((size_t)pb * nk_total + k0) * R8_A;
             const signed char* gB = B8 + ((size_t)qb * nk_total + k0) * R8_B;
             for (int i = 0; i < nk; i++) {
-                const int s = i % R8_NST;
-                if (i >= R8_NST) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((i / R8_NST - 1) & 1));
+                const int s = i % NST;
+                if (i >= NST) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((i / NST - 1) & 1));
                 const uint32_t bar = smem_u32(&full_bar[s]);
                 mbar_expect_tx(bar, ND * (R8_ASLAB + R8_BSLAB));
-                tma_load_1d(s0 + s * R8_STAGE + OFF * R8_ASLAB, gA + (size_t)i * R8_A + OFF * R8_ASLAB, ND * R8_ASLAB, bar);
-                tma_load_1d(s0 + s * R8_STAGE + R8_A + OFF * R8_BSLAB, gB + (size_t)i * R8_B + OFF * R8_BSLAB, ND * R8_BSLAB, bar);
+                tma_load_1d(s0 + s * STG, gA + (size_t)i * R8_A + OFF * R8_ASLAB, ND * R8_ASLAB, bar);
+                tma_load_1d(s0 + s * STG + ND * R8_ASLAB, gB + (size_t)i * R8_B + OFF * R8_BSLAB, ND * R8_BSLAB, bar);
             }
         }
     } else if (warp == 5) {
         if (lane == 0) {
             for (int i = 0; i < nk; i++) {
-                const int s = i % R8_NST;
-                mbar_wait(smem_u32(&full_bar[s]), (uint32_t)((i / R8_NST) & 1));
+                const int s = i % NST;
+                mbar_wait(smem_u32(&full_bar[s]), (uint32_t)((i / NST) & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;");
-                const uint32_t sA = s0 + s * R8_STAGE, sB = sA + R8_A;
+                const uint32_t sA = s0 + s * STG, sB = sA + ND * R8_ASLAB;
                 // the most significant A digit first: its partners are all ND B digits = all 32 ND columns, so on the
                 // first K-step it initialises every accumulator (accumulate = 0), everything else accumulates.
                 // Descriptors differ only in the 14-bit address field: one base per operand, compile-time offsets.
                 const uint64_t dA0 = umma_desc(sA), dB0 = umma_desc(sB);
 #pragma unroll
                 for (int ii = ND - 1; ii >= 0; ii--) {              // relative digit i' (absolute OFF + i')
-                    const int n = (ii + 1) * 32, l0 = OFF + ND - 1 - ii;
-                    const uint64_t da = dA0 + (uint64_t)(((OFF + ii) * R8_ASLAB) >> 4);
+                    const int n = (ii + 1) * 32, l0 = ND - 1 - ii;          // its partners: relative digits l0 .. ND - 1
+                    const uint64_t da = dA0 + (uint64_t)((ii * R8_ASLAB) >> 4);
                     const uint32_t acc = (i > 0 || ii < ND - 1) ? 1u : 0u;
                     if (n <= 256) {
                         umma_i8(tb, da, dB0 + (uint64_t)((l0 * R8_BSLAB) >> 4), umma_idesc_i8(n), acc);

@@ -613,7 +613,7 @@ int shd_set_engine(shd_ctx* h, int rho_engine) {
         h->workspace_bytes += g8 + w8;
         int rc;
         if ((rc = upload(h, &h->d_steps8, steps))) return rc;
-        const size_t need = (size_t)2 * h->nseg8 * h->d * h->N * 2;      // two partials per segment (k_grad8.cu)
+        const size_t need = (size_t)4 * h->nseg8 * h->d * h->N * 2;      // four partials per segment (k_grad8.cu)
         if (need > h->gpart_doubles) {
             cudaFree(h->d_gpart);
             h->d_gpart = nullptr;
