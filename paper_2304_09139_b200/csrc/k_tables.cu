@@ -272,10 +272,21 @@ __global__ void __launch_bounds__(TB) k_tables(
             cdd cur = one;
             for (int p0 = 0; p0 < P; p0 += TG) {
                 const int cnt = min(TG, P - p0);
-                for (int s = 0; s < cnt; s++) {
-                    st.put(0, s, cur);
-                    st.put_digits(s, cur, live);
-                    cur = cdd_mul(cur, base);
+                if (cnt == TG) {
+                    // full group: slots known at compile time (no selects in the byte staging), and the integer
+                    // work of one entry overlaps the serial double-double recurrence of the next
+#pragma unroll
+                    for (int s = 0; s < TG; s++) {
+                        st.put(0, s, cur);
+                        st.put_digits(s, cur, live);
+                        cur = cdd_mul(cur, base);
+                    }
+                } else {
+                    for (int s = 0; s < cnt; s++) {
+                        st.put(0, s, cur);
+                        st.put_digits(s, cur, live);
+                        cur = cdd_mul(cur, base);
+                    }
                 }
                 st.flush(p0, cnt, live);
             }
@@ -320,10 +331,19 @@ __global__ void __launch_bounds__(TB) k_tables(
         cdd cur = one;
         for (int q0 = 0; q0 < Qn; q0 += TG) {
             const int cnt = min(TG, Qn - q0);
-            for (int s = 0; s < cnt; s++) {
-                st.put(0, s, cur);
-                st.put_digits(s, cur, live);
-                cur = cdd_mul(cur, base);
+            if (cnt == TG) {
+#pragma unroll
+                for (int s = 0; s < TG; s++) {
+                    st.put(0, s, cur);
+                    st.put_digits(s, cur, live);
+                    cur = cdd_mul(cur, base);
+                }
+            } else {
+                for (int s = 0; s < cnt; s++) {
+                    st.put(0, s, cur);
+                    st.put_digits(s, cur, live);
+                    cur = cdd_mul(cur, base);
+                }
             }
             st.flush(q0, cnt, live);
         }
