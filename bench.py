@@ -39,7 +39,7 @@ ALG_DFMA_RHO, ALG_DFMA_GRAD = 12.0, 24.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
 # (profiles/r1d_summary.md), bytes; known for the headline workload only, otherwise null
 NCU_TRAFFIC = {("cfg4", "k_grad"): 12.77e9, ("cfg4", "k_rho"): 3.63e9,           # profiles/r1d_summary.md
-               ("cfg4", "k_grad8"): 1.90e9, ("cfg4", "k_rho8"): 1.55e9}          # profiles/r1e_summary.md
+               ("cfg4", "k_grad8"): 2.09e9, ("cfg4", "k_rho8"): 1.55e9}          # profiles/r1f_summary.md
 # INT8 tensor-core engines (k_rho8.cu, k_grad8.cu): 91 digit pairs per real product; 4 real products per (p,q)
 # cell = 2 wavevectors in the rho pass, 8 in the gradient pass; 2 operations per multiply-accumulate
 ALG_MAC_RHO8, ALG_MAC_GRAD8 = 182.0, 364.0
@@ -317,7 +317,7 @@ def run_gpu(args, cfg):
             roofline = {
                 "bound": "tensor", "kernel": dom, "achieved": achieved, "peak": i8_tops, "unit": "TFLOP/s",
                 "frac": achieved / i8_tops, "traffic": NCU_TRAFFIC.get((cfg.name, dom)),
-                "traffic_source": "profiles/r1e_summary.md" if (cfg.name, dom) in NCU_TRAFFIC else None,
+                "traffic_source": "profiles/r1f_summary.md" if (cfg.name, dom) in NCU_TRAFFIC else None,
                 "dtype": "s8 x s8 -> s32 (exact digit-sliced contraction; counted in integer operations)",
                 "peak_source": "measured live: shd_i8_probe, tcgen05.mma.kind::i8 M=128 N=256 K=32 issued back to "
                                "back on all SMs; MEASURED_PEAKS.json bf16 x 2 (nominal int8 : bf16) for comparison",
