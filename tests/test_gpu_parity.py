@@ -260,8 +260,9 @@ def test_fast_precision_two_limbs(shd, oracle):
     h.close()
 
 
+@pytest.mark.parametrize("engine", [0, 2])
 @pytest.mark.parametrize("d", [1, 2, 3])
-def test_anisotropic_table(shd, oracle, d):
+def test_anisotropic_table(shd, oracle, d, engine):
     """shd_create_table ("anisotropic exclusion regions"): an elliptical /
     ellipsoidal exclusion region (d >= 2) or a set with gaps (d = 1), in a scrambled order, against the
     oracle on the very same table; then the same quench outcome test as for the isotropic sets."""
@@ -285,6 +286,7 @@ def test_anisotropic_table(shd, oracle, d):
     hi, lo = inputs.uniform_positions_raw(d, N, L, 77)
     lo = inputs.jitter_lo(hi, 78)
     h = shd.Shd(d, N, L, table=n, v=v)
+    h.set_engine(engine)                 # 2: the same table on the INT8 tensor-core engines
     assert h.M == len(n) and np.array_equal(h.k(), n)
     th, tl = shd.from_host(hi, lo)
     phi, gh, gl = h.energy_grad(th, tl)
