@@ -127,7 +127,9 @@ int shd_set_precision(shd_ctx* h, int limbs);
  * operands as 13 balanced base-256 digits of trunc(x 2^102), the 91 digit pairs with i + l >= 12, s32
  * accumulators in tensor memory (at most 8192 particles per CTA, so they are exact), the same double-double
  * result within the same tolerances.  2: the gradient pass too (k_grad8.cu).  shd_set_precision selects the
- * number of digits on these engines.  Allocates the digit tables on first use.  Errors: SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA.
+ * number of digits on these engines.  Allocates the digit tables on first use.  Errors: SHD_EINVAL (engine not
+ * 0, 1 or 2; engine 2 with more than 5024 entries in the last-axis table: its s32 sums would not be exact),
+ * SHD_ENOMEM, SHD_ECUDA.
  */
 int shd_set_engine(shd_ctx* h, int rho_engine);
 

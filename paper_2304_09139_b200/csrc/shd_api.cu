@@ -568,6 +568,9 @@ int shd_set_precision(shd_ctx* h, int limbs) {
 int shd_set_engine(shd_ctx* h, int rho_engine) {
     if (!h) return SHD_EINVAL;
     if (rho_engine < 0 || rho_engine > 2) return fail(h, SHD_EINVAL, "shd_set_engine: engine must be 0, 1 or 2");
+    // exactness of the s32 digit sums of the gradient pass: 13 pairs x 2 Qpad products x 2^14 must stay below 2^31
+    if (rho_engine == 2 && (long)h->Qpad * 2 * SHD_I8_DIGITS * 16384 >= (1L << 31))
+        return fail(h, SHD_EINVAL, "shd_set_engine: last-axis table too long for the INT8 gradient pass (Qn <= 5024)");
     if (rho_engine == 2 && !h->d_Bg8) {
         // ---- INT8 gradient pass: step list over blocks of 8 p (K-steps of 16 q up to the block's last valid cell)
         h->npb8 = (h->P + 7) / 8;
