@@ -28,13 +28,15 @@ def shd():
     return m
 
 
+@pytest.mark.parametrize("engine", [0, 2])       # 0: FP64 limb engine; 2: both passes on the INT8 tensor cores
 @pytest.mark.parametrize("name,nk,nj,jitter", [("cfg3", 120, 100, True), ("cfg4", 60, 50, True), ("cfg5", 40, 120, False)])
-def test_fullsize_sampled(shd, oracle, name, nk, nj, jitter):
+def test_fullsize_sampled(shd, oracle, name, nk, nj, jitter, engine):
     cfg = inputs.CONFIGS[name]
     hi, lo = inputs.uniform_positions(cfg, 0)
     if jitter:
         lo = inputs.jitter_lo(hi, 7)            # non-zero lo words
     h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    h.set_engine(engine)
     assert h.M == cfg.M
     n = oracle.enumerate_Q(cfg.d, cfg.m_star)
     assert np.array_equal(h.k(), n), "canonical order of Q (bit-exact integer work)"
@@ -85,5 +87,5 @@ def test_fullsize_sampled(shd, oracle, name, nk, nj, jitter):
     assert np.array_equal(gh2.cpu().numpy(), g_hi) and np.array_equal(gl2.cpu().numpy(), g_lo)
     for x, y in zip(rho, h.rho()):
         assert np.array_equal(x, y.cpu().numpy())
-    print(name, dict(e_rho=e_rho.max(), e_phi=e_phi, e_g=e_g.max(), sum_grad=tot))
+    print(name, "engine", engine, dict(e_rho=e_rho.max(), e_phi=e_phi, e_g=e_g.max(), sum_grad=tot))
     h.close()
