@@ -182,6 +182,28 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
         if (total > 0) next_end(i, st);
         while (i < total) {
             const int pb8 = st.x / nkq;
+            // this block's A_j[p] (three limbs each) and axis weights.  With fewer digits the epilogue's own latencies
+            // bound the kernel and registers are free: the loads go out before the wait for the tensor core
+            double2 araw[2][3];
+            int wg[2][3];
+            auto load_A = [&]() {
+#pragma unroll
+                for (int pp = 0; pp < 2; pp++) {
+                    const int p = pb8 * 8 + quarter * 2 + pp;
+                    araw[pp][0] = araw[pp][1] = araw[pp][2] = make_double2(0.0, 0.0);
+                    wg[pp][0] = wg[pp][1] = wg[pp][2] = 0;
+                    if (j < N && p < Ppad) {
+                        const double2* ap = Aj + ((size_t)(p >> 5) * (Npad / 4) * 3 * 32 + (p & 31)) * 4;
+                        asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(araw[pp][0].x), "=d"(araw[pp][0].y) : "l"(ap));
+                        asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(araw[pp][1].x), "=d"(araw[pp][1].y) : "l"(ap + 128));
+                        asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(araw[pp][2].x), "=d"(araw[pp][2].y) : "l"(ap + 256));
+#pragma unroll
+                        for (int ax = 0; ax < 3; ax++)
+                            if (ax < d) wg[pp][ax] = wT[ax * Ppad + p];
+                    }
+                }
+            };
+            if constexpr (ND < G8_ND) load_A();
             mbar_wait(smem_u32(&tfull_bar), (uint32_t)(nblock & 1));
             asm volatile("tcgen05.fence::after_thread_sync;");
             // Drain: the thread's 16 columns (4 p x 4 outputs) of each of the ND digit sums, combined EXACTLY on the
@@ -213,49 +235,66 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
             int inext = i + 1;                                 // the block after this one
             int2 stn = st;
             if (inext < total) next_end(inext, stn);
-            // this block's A_j[p] (limbs -> double-double); the loads fly while the group values are converted
-            double2 araw[2][3];
+            if constexpr (ND == G8_ND) load_A();               // (13 digits: after the release, the registers are needed above)
+            if constexpr (ND < G8_ND) {
+                // Fewer digits (operands of 54 or 30 bits): the sums are worth no more than a double, so the
+                // contraction with A_j[p] runs in plain FP64 (products rounded once, ~2^-53 relative, below the
+                // operand truncation); only the running per-axis sums stay double-double.  A tenth of the FP64
+                // instructions of the full path: at these digit counts the epilogue, not the tensor core, is
+                // what bounds the kernel.
+                const double w0 = __longlong_as_double((long long)(1023 + 8 * (ND - 1 + 2 * OFF) - 204) << 52);
 #pragma unroll
-            for (int pp = 0; pp < 2; pp++) {
-                const int p = pb8 * 8 + quarter * 2 + pp;
-                araw[pp][0] = araw[pp][1] = araw[pp][2] = make_double2(0.0, 0.0);
-                if (j < N && p < Ppad) {
-                    const double2* ap = Aj + ((size_t)(p >> 5) * (Npad / 4) * 3 * 32 + (p & 31)) * 4;
-                    asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(araw[pp][0].x), "=d"(araw[pp][0].y) : "l"(ap));
-                    asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(araw[pp][1].x), "=d"(araw[pp][1].y) : "l"(ap + 128));
-                    asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(araw[pp][2].x), "=d"(araw[pp][2].y) : "l"(ap + 256));
+                for (int pp = 0; pp < 2; pp++) {
+                    double T[4];
+#pragma unroll
+                    for (int o4 = 0; o4 < 4; o4++) {
+                        double t = (double)G[0][4 * pp + o4];
+                        if (NG > 1) t = __fma_rn((double)G[NG - 1][4 * pp + o4], 4294967296.0, t);
+                        T[o4] = __dmul_rn(t, w0);
+                    }
+                    const double ar = __dadd_rn(__dadd_rn(araw[pp][0].x, araw[pp][1].x), araw[pp][2].x);
+                    const double ai = __dadd_rn(__dadd_rn(araw[pp][0].y, araw[pp][1].y), araw[pp][2].y);
+                    const int p = pb8 * 8 + quarter * 2 + pp;
+                    if (j < N && p < Ppad) {
+                        const double I = __fma_rn(ar, T[1], -__dmul_rn(ai, T[0]));      // Im[conj(A) T]
+                        const double R = __fma_rn(ar, T[2], __dmul_rn(ai, T[3]));       // Re[conj(A) T'']
+#define GACC8F(AX)                                                                            \
+    if (AX < d) {                                                                             \
+        const int wgt = AX < 3 ? wg[pp][AX < 3 ? AX : 0] : 0;                                 \
+        if (wgt != 0) g##AX = dd_add_d(g##AX, __dmul_rn(I, (double)wgt));                     \
+        if (AX == d - 1) g##AX = dd_add_d(g##AX, __dmul_rn(R, qs));                           \
+    }
+                        GACC8F(0) GACC8F(1) GACC8F(2) GACC8F(3)
+#undef GACC8F
+                    }
                 }
-            }
-            dd Tall[2][4];
+            } else {
+                dd Tall[2][4];
 #pragma unroll
-            for (int e = 0; e < 8; e++) {
-                __int128 T = (__int128)G[0][e];                         // sum_c 2^(8 c) S_c, exact
+                for (int e = 0; e < 8; e++) {
+                    __int128 T = (__int128)G[0][e];                     // sum_c 2^(8 c) S_c, exact
 #pragma unroll
-                for (int g = 1; g < NG; g++) T += (__int128)G[g][e] << (32 * g);
-                const dd t = s128_scaled_to_dd(T, 8 * (ND - 1 + 2 * OFF) - 204);
-                Tall[e >> 2][e & 3] = t;
-            }
-            dd ar[2], ai[2];
+                    for (int g = 1; g < NG; g++) T += (__int128)G[g][e] << (32 * g);
+                    Tall[e >> 2][e & 3] = s128_scaled_to_dd(T, 8 * (ND - 1 + 2 * OFF) - 204);
+                }
 #pragma unroll
-            for (int pp = 0; pp < 2; pp++) {
-                ar[pp] = limbs_to_dd8(araw[pp][0].x, araw[pp][1].x, araw[pp][2].x);
-                ai[pp] = limbs_to_dd8(araw[pp][0].y, araw[pp][1].y, araw[pp][2].y);
-            }
-#pragma unroll
-            for (int pp = 0; pp < 2; pp++) {
-                const dd* T = Tall[pp];
-                const int p = pb8 * 8 + quarter * 2 + pp;
-                if (j < N && p < Ppad) {
-                    const dd I = dd_dot2(ar[pp], T[1], ai[pp], T[0], -1.0);     // Im[conj(A) T]
-                    const dd R = dd_dot2(ar[pp], T[2], ai[pp], T[3], 1.0);      // Re[conj(A) T'']
+                for (int pp = 0; pp < 2; pp++) {
+                    const dd* T = Tall[pp];
+                    const dd ar = limbs_to_dd8(araw[pp][0].x, araw[pp][1].x, araw[pp][2].x);
+                    const dd ai = limbs_to_dd8(araw[pp][0].y, araw[pp][1].y, araw[pp][2].y);
+                    const int p = pb8 * 8 + quarter * 2 + pp;
+                    if (j < N && p < Ppad) {
+                        const dd I = dd_dot2(ar, T[1], ai, T[0], -1.0);         // Im[conj(A) T]
+                        const dd R = dd_dot2(ar, T[2], ai, T[3], 1.0);          // Re[conj(A) T'']
 #define GACC8(AX)                                                                             \
     if (AX < d) {                                                                             \
-        const int wgt = AX < 3 ? wT[(AX < 3 ? AX : 0) * Ppad + p] : 0;                        \
+        const int wgt = AX < 3 ? wg[pp][AX < 3 ? AX : 0] : 0;                                 \
         if (wgt != 0) g##AX = dd_add(g##AX, dd_mul_d(I, (double)wgt));                        \
         if (AX == d - 1) g##AX = dd_add(g##AX, dd_scale2(R, qs));                             \
     }
-                    GACC8(0) GACC8(1) GACC8(2) GACC8(3)
+                        GACC8(0) GACC8(1) GACC8(2) GACC8(3)
 #undef GACC8
+                    }
                 }
             }
             nblock++;
