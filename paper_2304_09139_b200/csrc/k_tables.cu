@@ -97,6 +97,8 @@ constexpr int TABLES_SMEM = TABLES_LIMB_SMEM + TG * 2 * SHD_I8_DIGITS * TB;   //
 // patterns below) and the block then writes runs of 512 contiguous bytes:
 //   rho layout       T[block][j/4][limb 3][32 entries][j%4][re,im]            (A and B)
 //   gradient layout  Bg[j/32][q/4][limb 3][j%32][q%4][re,im]
+// DLO = first digit in use (0, 6 or 9 for 13, 7 or 4 digits, shd_set_precision): lower digit slabs are not written
+template <int DLO>
 struct Stager {
     double2* tile;        // [TB][planes][TG]
     int planes;           // 3 limbs
@@ -114,7 +116,7 @@ struct Stager {
         if (gdig == nullptr) return;
         const int w = slot >> 1, sh = (slot & 1) * 16;             // bytes 2 slot (re) and 2 slot + 1 (im)
 #pragma unroll
-        for (int i = 0; i < SHD_I8_DIGITS; i++) {
+        for (int i = DLO; i < SHD_I8_DIGITS; i++) {
             const uint32_t v = ((uint32_t)(uint8_t)dr[i] | ((uint32_t)(uint8_t)di[i] << 8)) << sh;
 #pragma unroll
             for (int ww = 0; ww < 4; ww++)
@@ -130,7 +132,7 @@ struct Stager {
             signed char* base = gdig + (((size_t)(j >> 7) * nkq + (size_t)(q0 >> 4)) * SHD_I8_DIGITS) * 4096 +
                                 (row >> 3) * 256 + ((q0 >> 3) & 1) * 128 + (row & 7) * 16;
 #pragma unroll
-            for (int i = 0; i < SHD_I8_DIGITS; i++) {
+            for (int i = DLO; i < SHD_I8_DIGITS; i++) {
                 uint4 v = make_uint4(gacc[i][0], gacc[i][1], gacc[i][2], gacc[i][3]);
                 if (count < 8) {                                    // ragged tail: entries >= count are zero digits
                     uint32_t* pv = &v.x;
@@ -161,7 +163,7 @@ struct Stager {
         if (dig == nullptr) return;
         signed char* t = dtile + (size_t)(slot * 2) * SHD_I8_DIGITS * TB + threadIdx.x;
 #pragma unroll
-        for (int i = 0; i < SHD_I8_DIGITS; i++) {
+        for (int i = DLO; i < SHD_I8_DIGITS; i++) {
             t[(size_t)i * TB] = live ? dr[i] : (signed char)0;                       // particles beyond N: zero digits
             t[(size_t)(SHD_I8_DIGITS + i) * TB] = live ? di[i] : (signed char)0;
         }
@@ -174,7 +176,7 @@ struct Stager {
         const int nrow = 2 * count;                                                 // rows of this group
         signed char* base = dig + ((size_t)(e0 / rows8) * nk8 + (size_t)(j0 >> 5)) * SHD_I8_DIGITS * slab;
         const int r_first = 2 * (e0 % rows8);
-        for (int c = threadIdx.x; c < SHD_I8_DIGITS * (TB / 16) * 2 * TG; c += TB) {
+        for (int c = threadIdx.x + DLO * (TB / 16) * 2 * TG; c < SHD_I8_DIGITS * (TB / 16) * 2 * TG; c += TB) {
             const int rl = c % (2 * TG);                                            // row within the group (fastest)
             const int kh = (c / (2 * TG)) % (TB / 16);                              // 16-particle chunk of the block
             const int dg = c / (2 * TG * (TB / 16));
@@ -237,6 +239,7 @@ struct Stager {
 };
 
 // which = 0: A table.  which = 1: B table (+ the same limbs in the gradient layout Bg).
+template <int DLO>
 __global__ void __launch_bounds__(TB) k_tables(
     int d, long N, double L, long Npad, int P, int Qn, int S1d, int qscale_log2,
     const int* __restrict__ pn0, const int* __restrict__ pn1, const int* __restrict__ pn2, int Qpad,
@@ -255,7 +258,7 @@ __global__ void __launch_bounds__(TB) k_tables(
     const long jc = live ? j : N - 1;            // dead threads shadow the last particle (keeps barriers uniform)
     const cdd one{dd{1.0, 0.0}, dd{0.0, 0.0}};
     const bool gradB = which == 1 && with_grad != 0;
-    Stager st;
+    Stager<DLO> st;
     st.tile = tile; st.planes = 3;
     st.table = which == 0 ? A : B;                      // may be nullptr: the INT8 rho pass does not read B limbs
     st.Bg = gradB ? Bg : nullptr;                       // nullptr too when the gradient pass runs on INT8
@@ -354,19 +357,28 @@ __global__ void __launch_bounds__(TB) k_tables(
 
 cudaError_t shd_tables_configure()
 {
-    return cudaFuncSetAttribute(k_tables, cudaFuncAttributeMaxDynamicSharedMemorySize, TABLES_SMEM);
+    cudaError_t e = cudaFuncSetAttribute(k_tables<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TABLES_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tables<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, TABLES_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tables<9>, cudaFuncAttributeMaxDynamicSharedMemorySize, TABLES_SMEM);
+    return e;
 }
 
 cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool with_grad_tables)
 {
     dim3 grid((unsigned)((h->N + TB - 1) / TB), 2);
-    k_tables<<<grid, TB, TABLES_SMEM, h->stream>>>(h->d, h->N, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2,
-                                         h->d_pn0, h->d_pn1, h->d_pn2, h->Qpad, pos_hi, pos_lo,
-                                         h->d_A, h->rho_engine >= 1 ? nullptr : h->d_B,
-                                         h->rho_engine == 2 ? nullptr : h->d_Bg, with_grad_tables ? 1 : 0,
-                                         h->rho_engine >= 1 ? h->d_A8 : nullptr,
-                                         h->rho_engine >= 1 ? h->d_B8 : nullptr, h->nk8,
-                                         h->rho_engine == 2 ? h->d_Bg8 : nullptr, h->nkq8, h->d_skip);
+#define LAUNCH_TABLES(DLOV)                                                                                       \
+    k_tables<DLOV><<<grid, TB, TABLES_SMEM, h->stream>>>(h->d, h->N, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2, \
+                                         h->d_pn0, h->d_pn1, h->d_pn2, h->Qpad, pos_hi, pos_lo,                    \
+                                         h->d_A, h->rho_engine >= 1 ? nullptr : h->d_B,                            \
+                                         h->rho_engine == 2 ? nullptr : h->d_Bg, with_grad_tables ? 1 : 0,         \
+                                         h->rho_engine >= 1 ? h->d_A8 : nullptr,                                   \
+                                         h->rho_engine >= 1 ? h->d_B8 : nullptr, h->nk8,                           \
+                                         h->rho_engine == 2 ? h->d_Bg8 : nullptr, h->nkq8, h->d_skip)
+    // the INT8 engines read only the 13, 7 or 4 most significant digits (shd_set_precision): the rest is not written
+    if (h->rho_engine == 0 || h->nlimb >= 3) LAUNCH_TABLES(0);
+    else if (h->nlimb == 2) LAUNCH_TABLES(6);
+    else LAUNCH_TABLES(9);
+#undef LAUNCH_TABLES
     h->last_launches += 1;
     return cudaGetLastError();
 }
