@@ -132,17 +132,26 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
                 const uint32_t sA = s0 + s * STG, sW = sA + ND * G8_ASLAB;
                 // descriptors differ only in the 14-bit address field: one base per operand, compile-time offsets
                 const uint64_t dA0 = g8_desc(sA), dW0 = g8_desc(sW);
-#pragma unroll
-                for (int ii = ND - 1; ii >= 0; ii--) {              // relative digit i' (absolute OFF + i')
+                auto issue = [&](int ii, uint32_t acc) {            // relative digit i' (absolute OFF + i')
                     const int n = (ii + 1) * 32, l0 = ND - 1 - ii;          // its partners: relative digits l0 .. ND - 1
                     const uint64_t da = dA0 + (uint64_t)((ii * G8_ASLAB) >> 4);
-                    const uint32_t acc = (!fresh || ii < ND - 1) ? 1u : 0u;
                     if (n <= 256) {
                         g8_mma(tb, da, dW0 + (uint64_t)((l0 * G8_WSLAB) >> 4), g8_idesc(n), acc);
                     } else {
                         g8_mma(tb, da, dW0 + (uint64_t)((l0 * G8_WSLAB) >> 4), g8_idesc(256), acc);
                         g8_mma(tb + 256, da, dW0 + (uint64_t)(((l0 + 8) * G8_WSLAB) >> 4), g8_idesc(n - 256), acc);
                     }
+                };
+                // A block's first step runs from the most significant digit down (its first instruction covers all
+                // columns and initialises them); the other steps run upwards, short instructions first and long ones
+                // last, so that the tensor core's queue holds long instructions while this thread crosses the step
+                // boundary (k_rho8.cu).
+                if (fresh || ND < G8_ND) {
+#pragma unroll
+                    for (int ii = ND - 1; ii >= 0; ii--) issue(ii, (!fresh || ii < ND - 1) ? 1u : 0u);
+                } else {
+#pragma unroll
+                    for (int ii = 0; ii < ND; ii++) issue(ii, 1u);
                 }
                 g8_commit(smem_u32(&empty_bar[s]));
                 fresh = false;

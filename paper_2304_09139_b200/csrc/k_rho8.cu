@@ -99,28 +99,44 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
         }
     } else if (warp == 5) {
         if (lane == 0) {
-            for (int i = 0; i < nk; i++) {
-                const int s = i % NST;
-                mbar_wait(smem_u32(&full_bar[s]), (uint32_t)((i / NST) & 1));
+            // the ring position is a compile-time constant inside the unrolled inner loop: shared-memory addresses
+            // and descriptors of a step are constants off one base, the step boundary costs a few instructions
+            const uint64_t dbase = umma_desc(s0);
+            for (int i0 = 0; i0 < nk; i0 += NST) {
+                const uint32_t par = (uint32_t)((i0 / NST) & 1);
+#pragma unroll
+              for (int s = 0; s < NST; s++) {
+                const int i = i0 + s;
+                if (i >= nk) break;
+                mbar_wait(smem_u32(&full_bar[s]), par);
                 asm volatile("tcgen05.fence::after_thread_sync;");
-                const uint32_t sA = s0 + s * STG, sB = sA + ND * R8_ASLAB;
                 // the most significant A digit first: its partners are all ND B digits = all 32 ND columns, so on the
                 // first K-step it initialises every accumulator (accumulate = 0), everything else accumulates.
                 // Descriptors differ only in the 14-bit address field: one base per operand, compile-time offsets.
-                const uint64_t dA0 = umma_desc(sA), dB0 = umma_desc(sB);
-#pragma unroll
-                for (int ii = ND - 1; ii >= 0; ii--) {              // relative digit i' (absolute OFF + i')
+                const uint64_t dA0 = dbase + (uint64_t)((s * STG) >> 4), dB0 = dA0 + (uint64_t)((ND * R8_ASLAB) >> 4);
+                // Order inside a K-step: ascending digits, i.e. the short instructions (N = 32, 64, ...) first and the
+                // long ones last, so that the tensor core's queue holds long instructions while this thread crosses
+                // the step boundary (commit, barrier wait, descriptors): 4 % at 13 digits.  The very first step runs
+                // descending: its first instruction covers all columns and initialises them.
+                auto issue = [&](int ii, uint32_t acc) {            // relative digit i' (absolute OFF + i')
                     const int n = (ii + 1) * 32, l0 = ND - 1 - ii;          // its partners: relative digits l0 .. ND - 1
                     const uint64_t da = dA0 + (uint64_t)((ii * R8_ASLAB) >> 4);
-                    const uint32_t acc = (i > 0 || ii < ND - 1) ? 1u : 0u;
                     if (n <= 256) {
                         umma_i8(tb, da, dB0 + (uint64_t)((l0 * R8_BSLAB) >> 4), umma_idesc_i8(n), acc);
                     } else {
                         umma_i8(tb, da, dB0 + (uint64_t)((l0 * R8_BSLAB) >> 4), umma_idesc_i8(256), acc);
                         umma_i8(tb + 256, da, dB0 + (uint64_t)(((l0 + 8) * R8_BSLAB) >> 4), umma_idesc_i8(n - 256), acc);
                     }
+                };
+                if (i == 0 || ND < R8_ND) {                         // (with fewer digits the order makes no difference)
+#pragma unroll
+                    for (int ii = ND - 1; ii >= 0; ii--) issue(ii, (i > 0 || ii < ND - 1) ? 1u : 0u);
+                } else {
+#pragma unroll
+                    for (int ii = 0; ii < ND; ii++) issue(ii, 1u);
                 }
                 umma_commit(smem_u32(&empty_bar[s]));          // arrives when the tensor core is done with stage s
+              }
             }
             umma_commit(smem_u32(&done_bar));
         }
