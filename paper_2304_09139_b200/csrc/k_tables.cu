@@ -57,7 +57,10 @@ struct limbs { double x0, x1, x2; };
 // are fine): the bytes of X + sum_i 128 256^i, minus 128 (no carries); sum_i d_i 256^i = X.  X is assembled in two
 // 64-bit words split at 2^56: hi 2^46 = H + r (H integer, 0 <= r < 1, both exact), so
 // X = H 2^56 + trunc(r 2^56) + trunc(lo 2^102); the last two terms are below 2^57 in magnitude.
-__device__ __forceinline__ void digits13(dd x, signed char* d) {
+// Returned packed: byte i of lo = digit i (i = 0..6), byte i of hi = digit 7 + i (i = 0..5), as s8 bit patterns
+// (offset byte - 128 = offset byte ^ 0x80, applied to all bytes of a word at once).
+struct digits13_t { unsigned long long lo, hi; };
+__device__ __forceinline__ digits13_t digits13(dd x) {
     const double t = __dmul_rn(x.h, 0x1p46);                       // exact
     const double H = floor(t);
     const double r = __dadd_rn(t, -H);                             // exact, in [0, 1)
@@ -65,11 +68,13 @@ __device__ __forceinline__ void digits13(dd x, signed char* d) {
     long long xhi = __double2ll_rz(H);
     xlo += 0x80808080808080LL;                                     // digits 0..6 of the offset
     xhi += 0x808080808080LL + (xlo >> 56);                         // digits 7..12, carry (arithmetic shift: may be -1)
-    const unsigned long long ylo = (unsigned long long)xlo & 0xffffffffffffffULL, yhi = (unsigned long long)xhi;
-#pragma unroll
-    for (int i = 0; i < 7; i++) d[i] = (signed char)((int)((ylo >> (8 * i)) & 0xff) - 128);
-#pragma unroll
-    for (int i = 0; i < 6; i++) d[7 + i] = (signed char)((int)((yhi >> (8 * i)) & 0xff) - 128);
+    digits13_t d;
+    d.lo = ((unsigned long long)xlo & 0xffffffffffffffULL) ^ 0x80808080808080ULL;
+    d.hi = ((unsigned long long)xhi & 0xffffffffffffULL) ^ 0x808080808080ULL;
+    return d;
+}
+__device__ __forceinline__ uint32_t digit_byte(const digits13_t& d, int i) {       // i compile-time after unrolling
+    return i < 7 ? (uint32_t)(d.lo >> (8 * i)) & 0xffu : (uint32_t)(d.hi >> (8 * (i - 7))) & 0xffu;
 }
 
 // |x| <= 1 (normalised dd) -> limbs (shd_internal.h)
@@ -112,12 +117,12 @@ struct Stager {
     signed char* gdig;    // gradient pass, particle operand (B thread only, or nullptr): row = particle % 128 of
     int nkq;              //   block particle / 128, K index = 2 (q % 16) + re/im of K-step q / 16 (nkq per block)
     uint32_t gacc[SHD_I8_DIGITS][4];   // this particle's 16 bytes per digit for the 8 entries of a flush group
-    __device__ __forceinline__ void putg8(int slot, const signed char* dr, const signed char* di) {
+    __device__ __forceinline__ void putg8(int slot, const digits13_t& dr, const digits13_t& di) {
         if (gdig == nullptr) return;
         const int w = slot >> 1, sh = (slot & 1) * 16;             // bytes 2 slot (re) and 2 slot + 1 (im)
 #pragma unroll
         for (int i = DLO; i < SHD_I8_DIGITS; i++) {
-            const uint32_t v = ((uint32_t)(uint8_t)dr[i] | ((uint32_t)(uint8_t)di[i] << 8)) << sh;
+            const uint32_t v = (digit_byte(dr, i) | (digit_byte(di, i) << 8)) << sh;
 #pragma unroll
             for (int ww = 0; ww < 4; ww++)
                 if (ww == w) gacc[i][ww] = (sh == 0 ? 0u : gacc[i][ww]) | v;
@@ -153,19 +158,18 @@ struct Stager {
     // digits of one table entry for both INT8 tables (computed once)
     __device__ __forceinline__ void put_digits(int slot, cdd z, bool live) {
         if (dig == nullptr && gdig == nullptr) return;
-        signed char dr[SHD_I8_DIGITS], di[SHD_I8_DIGITS];
-        digits13(z.re, dr);
-        digits13(z.im, di);
-        put8(slot, dr, di, live);
+        digits13_t dr = digits13(z.re), di = digits13(z.im);
+        if (!live) dr.lo = dr.hi = di.lo = di.hi = 0ULL;                            // particles beyond N: zero digits
+        put8(slot, dr, di);
         putg8(slot, dr, di);
     }
-    __device__ __forceinline__ void put8(int slot, const signed char* dr, const signed char* di, bool live) {
+    __device__ __forceinline__ void put8(int slot, const digits13_t& dr, const digits13_t& di) {
         if (dig == nullptr) return;
         signed char* t = dtile + (size_t)(slot * 2) * SHD_I8_DIGITS * TB + threadIdx.x;
 #pragma unroll
         for (int i = DLO; i < SHD_I8_DIGITS; i++) {
-            t[(size_t)i * TB] = live ? dr[i] : (signed char)0;                       // particles beyond N: zero digits
-            t[(size_t)(SHD_I8_DIGITS + i) * TB] = live ? di[i] : (signed char)0;
+            t[(size_t)i * TB] = (signed char)digit_byte(dr, i);
+            t[(size_t)(SHD_I8_DIGITS + i) * TB] = (signed char)digit_byte(di, i);
         }
     }
     // after the block-wide barrier of flush(): 16-byte chunks (16 particles of one row of one digit), consecutive
