@@ -209,34 +209,49 @@ struct Stager {
         flush8(e0, count);
         flushg8(e0, count, live);
         const int blk = e0 >> 5, off = e0 & 31;
-        // rho layout: piece -> (group, limb, entry, j%4), j%4 fastest
-        for (int piece = threadIdx.x; table != nullptr && piece < (TB / 4) * 3 * TG * 4; piece += TB) {
-            const int jj = piece & 3, c = (piece >> 2) & 7, l = (piece >> 5) % 3, jg = piece / 96;
-            const int row = jg * 4 + jj;
-            const long j = j0 + row;
-            if (c < count && j < N) {
-                double2 v = tile[(row * planes + l) * TG + (c ^ swz(row))];
-                double2* dst = reinterpret_cast<double2*>(table) +
-                               ((((size_t)blk * (Npad / 4) + (j >> 2)) * 3 + l) * 32 + off + c) * 4 + jj;
-                *dst = v;
+        // rho layout: (j/4, limb, entry, j%4), j%4 fastest.  Thread = (half of the block's 8-particle rows, entry c,
+        // j%4); it walks the 8 row groups and 3 limbs with compile-time strides on both sides (a warp writes 512
+        // contiguous bytes per store), so an iteration is one shared load, one global store and a predicate.
+        if (table != nullptr) {
+            const int t = threadIdx.x, half = t >> 5, jj = t & 3, c = (t >> 2) & 7, r0 = 4 * half + jj;
+            const double2* src = tile + r0 * planes * TG + (c ^ swz(r0));
+            double2* dst = reinterpret_cast<double2*>(table) +
+                           ((((size_t)blk * (Npad / 4) + (j0 >> 2) + half) * 3) * 32 + off + c) * 4 + jj;
+            const bool cok = c < count;
+#pragma unroll
+            for (int a = 0; a < TB / 8; a++) {
+                const bool ok = cok && j0 + 8 * a + r0 < N;
+#pragma unroll
+                for (int l = 0; l < 3; l++)
+                    if (ok) dst[(size_t)(6 * a + l) * 128] = src[(a * 8 * 3 + l) * TG];
             }
         }
         if (Bg != nullptr) {
-            // gradient layout: piece -> (j/32, q-group, plane, j%32, q%4), q%4 fastest
-            for (int piece = threadIdx.x; piece < TB * 3 * TG; piece += TB) {
-                const int q4 = piece & 3, jl = (piece >> 2) & 31;
-                int rest = piece >> 7;
-                const int pl = rest % 3; rest /= 3;
-                const int qg = rest & 1, jbl = rest >> 1;
-                const int row = jbl * 32 + jl, c = qg * 4 + q4;
-                const long j = j0 + row;
-                if (c < count && j < N) {
-                    double2 v = tile[(row * planes + pl) * TG + (c ^ swz(row))];
-                    double2* dst = reinterpret_cast<double2*>(Bg) +
-                                   ((((size_t)(j >> 5) * (Qpad / 4) + ((e0 + c) >> 2)) * 3 + pl) * 32 + jl) * 4 + q4;
-                    *dst = v;
+            // gradient layout: (j/32, q-group, plane, j%32, q%4), q%4 fastest.  Thread = (j%16, q%4); the walk over
+            // (j/32, q-group, plane, upper half of j%32) has compile-time strides on the shared-memory side and
+            // loop-invariant ones on the global side
+            const int t = threadIdx.x, q4 = t & 3, jl0 = t >> 2;
+            const size_t qstride = (size_t)(Qpad / 4) * 3 * 128;          // double2 per 32-particle block
+            double2* dstB = reinterpret_cast<double2*>(Bg) + (size_t)(j0 >> 5) * qstride + (size_t)(e0 >> 2) * 3 * 128 +
+                            (size_t)jl0 * 4 + q4;
+#pragma unroll
+            for (int jbl = 0; jbl < TB / 32; jbl++)
+#pragma unroll
+                for (int u = 0; u < 2; u++) {
+                    const int row = jbl * 32 + 16 * u + jl0;
+                    const double2* srcB = tile + row * 3 * TG;
+                    const int sw = swz(row);
+                    const bool jok = j0 + row < N;
+#pragma unroll
+                    for (int qg = 0; qg < 2; qg++) {
+                        const int c = qg * 4 + q4;
+                        if (jok && c < count) {
+#pragma unroll
+                            for (int pl = 0; pl < 3; pl++)
+                                dstB[(size_t)jbl * qstride + (size_t)((qg * 3 + pl) * 128 + 64 * u)] = srcB[pl * TG + (c ^ sw)];
+                        }
+                    }
                 }
-            }
         }
         __syncthreads();
     }
