@@ -180,17 +180,16 @@ struct Stager {
         const int nrow = 2 * count;                                                 // rows of this group
         signed char* base = dig + ((size_t)(e0 / rows8) * nk8 + (size_t)(j0 >> 5)) * SHD_I8_DIGITS * slab;
         const int r_first = 2 * (e0 % rows8);
-        for (int c = threadIdx.x + DLO * (TB / 16) * 2 * TG; c < SHD_I8_DIGITS * (TB / 16) * 2 * TG; c += TB) {
-            const int rl = c % (2 * TG);                                            // row within the group (fastest)
-            const int kh = (c / (2 * TG)) % (TB / 16);                              // 16-particle chunk of the block
-            const int dg = c / (2 * TG * (TB / 16));
-            if (rl < nrow && (j0 >> 5) + (kh >> 1) < nk8) {        // (the last block may reach past the table's K-steps)
-                const uint4 v = *reinterpret_cast<const uint4*>(dtile + ((size_t)rl * SHD_I8_DIGITS + dg) * TB + kh * 16);
-                const int r = r_first + rl;
-                signed char* dst = base + ((size_t)(kh >> 1) * SHD_I8_DIGITS + dg) * slab +
-                                   (r >> 3) * 256 + (kh & 1) * 128 + (r & 7) * 16;
-                *reinterpret_cast<uint4*>(dst) = v;
-            }
+        // thread = (row of the group, 16-particle chunk of the block): both fixed while it walks the digits
+        static_assert(TB == 2 * TG * (TB / 16), "one pass of the block covers one digit");
+        const int rl = threadIdx.x % (2 * TG), kh = threadIdx.x / (2 * TG);
+        if (rl < nrow && (j0 >> 5) + (kh >> 1) < nk8) {            // (the last block may reach past the table's K-steps)
+            const int r = r_first + rl;
+            const signed char* src = dtile + (size_t)rl * SHD_I8_DIGITS * TB + kh * 16;
+            signed char* dst = base + (size_t)(kh >> 1) * SHD_I8_DIGITS * slab + (r >> 3) * 256 + (kh & 1) * 128 + (r & 7) * 16;
+#pragma unroll
+            for (int dg = DLO; dg < SHD_I8_DIGITS; dg++)
+                *reinterpret_cast<uint4*>(dst + (size_t)dg * slab) = *reinterpret_cast<const uint4*>(src + dg * TB);
         }
     }
     __device__ __forceinline__ static int swz(int r) { return ((r & 1) << 2) | (r & 2) | ((r >> 2) & 1); }
