@@ -88,13 +88,21 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
         if (lane == 0) {
             const signed char* gA = A8 + ((size_t)pb * nk_total + k0) * R8_A;
             const signed char* gB = B8 + ((size_t)qb * nk_total + k0) * R8_B;
-            for (int i = 0; i < nk; i++) {
-                const int s = i % NST;
-                if (i >= NST) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((i / NST - 1) & 1));
+            gA += OFF * R8_ASLAB;
+            gB += OFF * R8_BSLAB;
+            for (int i0 = 0; i0 < nk; i0 += NST) {                 // unrolled over the ring positions (as below)
+                const uint32_t par = (uint32_t)((i0 / NST - 1) & 1);
+#pragma unroll
+              for (int s = 0; s < NST; s++) {
+                if (i0 + s >= nk) break;
+                if (i0 > 0) mbar_wait(smem_u32(&empty_bar[s]), par);
                 const uint32_t bar = smem_u32(&full_bar[s]);
                 mbar_expect_tx(bar, ND * (R8_ASLAB + R8_BSLAB));
-                tma_load_1d(s0 + s * STG, gA + (size_t)i * R8_A + OFF * R8_ASLAB, ND * R8_ASLAB, bar);
-                tma_load_1d(s0 + s * STG + ND * R8_ASLAB, gB + (size_t)i * R8_B + OFF * R8_BSLAB, ND * R8_BSLAB, bar);
+                tma_load_1d(s0 + s * STG, gA, ND * R8_ASLAB, bar);
+                tma_load_1d(s0 + s * STG + ND * R8_ASLAB, gB, ND * R8_BSLAB, bar);
+                gA += R8_A;
+                gB += R8_B;
+              }
             }
         }
     } else if (warp == 5) {
