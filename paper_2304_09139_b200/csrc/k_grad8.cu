@@ -9,9 +9,15 @@
 // their digit sums; 18 instructions per step).  The s32 sums are exact (<= 2 Qn products per pair, Qn <= 5000).
 // At the end of a block (or of the segment) the sixteen epilogue warps read tensor memory, four threads per
 // particle (one per quarter of the block's 8 p): the 13 digit sums of each output are combined exactly into three
-// 64-bit integers on the integer pipe, tensor memory is released, and only then the (128-bit) integer becomes a
-// double-double that is contracted with the particle's own A_j[p] exactly as in k_grad.cu; the per-axis sums
-// stay in registers across blocks.  Warp 16: TMA producer, warp 17: MMA issuer.
+// 64-bit integers on the integer pipe, tensor memory is released, and the exact (128-bit) integer T is contracted
+// with the particle's own A_j[p] -- the integer trunc(a 2^102) k_tables stores in sign-magnitude form -- in
+// INTEGER arithmetic: (|T| |A|) >> 96 by 64-bit multiplies, signed 192-bit per-axis accumulators in registers across
+// blocks, one conversion to double-double per CTA.  Measured on B200 (profiles/r2a_summary.md): FP64 instructions all
+// but stall while tcgen05.mma.kind::i8 streams on the same SM (DADD chains of 16 warps make no progress during a
+// back-to-back N = 256 stream, IMAD chains are unaffected), so the double-double epilogue of round 1 (332 FP64
+// instructions per thread and block) took 11.7 us per block against 9.9 us of tensor work and slowed the issue.
+// Warp 16: TMA producer (one lane); warp 17: MMA issuer, all 32 lanes in the loop (descriptors stay in uniform
+// registers, no per-instruction election loop), one elected lane issues.
 #include "pipe.cuh"
 #include "shd_internal.h"
 
@@ -34,35 +40,69 @@ __device__ __forceinline__ uint64_t g8_desc(uint32_t addr) {
 __device__ __forceinline__ uint32_t g8_idesc(int n) {
     return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
 }
-__device__ __forceinline__ void g8_mma(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+// issued by the elected lane of a converged warp (elected = 1 in one lane)
+__device__ __forceinline__ void g8_mma(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate, uint32_t elected) {
     uint32_t z = 0;
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                 "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %5, %5, %5}, p;\n\t}"
-                 ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate), "r"(z) : "memory");
+    asm volatile("{\n\t.reg .pred p, q;\n\tsetp.ne.b32 p, %4, 0;\n\tsetp.ne.b32 q, %6, 0;\n\t"
+                 "@q tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %5, %5, %5}, p;\n\t}"
+                 ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate), "r"(z), "r"(elected) : "memory");
 }
-__device__ __forceinline__ void g8_commit(uint32_t bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+__device__ __forceinline__ void g8_commit(uint32_t bar, uint32_t elected) {
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %1, 0;\n\t"
+                 "@q tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}" ::"r"(bar), "r"(elected) : "memory");
 }
-__device__ __forceinline__ dd limbs_to_dd8(double x0, double x1, double x2) {
-    return fast_two_sum(__dadd_rn(x0, x1), x2);
+typedef unsigned long long ull;
+// signed 192-bit integer (two's complement), the per-axis gradient accumulator of a thread
+struct acc192 { ull w0, w1, w2; };
+// a += neg ? -r : r   (r = 192-bit magnitude)
+__device__ __forceinline__ void acc_addsub(acc192& a, ull r0, ull r1, ull r2, bool neg) {
+    const ull m = neg ? ~0ull : 0ull;
+    unsigned __int128 s = (unsigned __int128)a.w0 + (r0 ^ m) + (neg ? 1u : 0u);
+    a.w0 = (ull)s;
+    s = (unsigned __int128)a.w1 + (r1 ^ m) + (ull)(s >> 64);
+    a.w1 = (ull)s;
+    a.w2 = a.w2 + (r2 ^ m) + (ull)(s >> 64);
 }
-// T 2^e as a double-double (relative error <= 2^-105; |T| < 2^127).  Sign and magnitude first, so that the four
-// 32-bit words of the magnitude are non-overlapping terms of one sign (no cancellation); every word becomes a
-// double through the 2^52 trick with its scale in the exponent field ((2^52 + u) 2^k - 2^52 2^k = u 2^k, one
-// exact addition), and two exact pair sums are merged.  15 additions instead of three conversions and two
-// double-double sums: the epilogue warps are bound by the FP64 pipe.
-__device__ __forceinline__ dd s128_scaled_to_dd(__int128 T, int e) {
-    const bool neg = T < 0;
-    const unsigned __int128 M = neg ? (unsigned __int128)(-T) : (unsigned __int128)T;
-    const unsigned long long mh = (unsigned long long)(M >> 64), ml = (unsigned long long)M;
-    const int e0 = 0x43300000 + (e << 20);
-    const double x0 = __dadd_rn(__hiloint2double(e0, (int)(unsigned)ml), -__hiloint2double(e0, 0));
-    const double x1 = __dadd_rn(__hiloint2double(e0 + (32 << 20), (int)(unsigned)(ml >> 32)), -__hiloint2double(e0 + (32 << 20), 0));
-    const double x2 = __dadd_rn(__hiloint2double(e0 + (64 << 20), (int)(unsigned)mh), -__hiloint2double(e0 + (64 << 20), 0));
-    const double x3 = __dadd_rn(__hiloint2double(e0 + (96 << 20), (int)(unsigned)(mh >> 32)), -__hiloint2double(e0 + (96 << 20), 0));
-    const dd hi = fast_two_sum(x3, x2), lo = fast_two_sum(x1, x0);   // exact: |x3| >= |x2| or x3 = 0, same below
-    dd r = fast_two_sum(hi.h, __dadd_rn(hi.l, lo.h));
-    r.l = __dadd_rn(r.l, lo.l);
+// g += v w  (mod 2^192; v two's complement, 0 <= w < 2^32)
+__device__ __forceinline__ void acc_mac(acc192& g, const acc192& v, uint32_t w) {
+    unsigned __int128 c = (unsigned __int128)v.w0 * w + g.w0;
+    g.w0 = (ull)c;
+    c = (unsigned __int128)v.w1 * w + g.w1 + (ull)(c >> 64);
+    g.w1 = (ull)c;
+    g.w2 = v.w2 * w + g.w2 + (ull)(c >> 64);
+}
+// (|T| |A|) >> 96 with |T| = (t1 : t0) < 2^127 and |A| = (a1 : a0) <= 2^102 (+ a few units): the product is below 2^230,
+// the result below 2^134.  HI = false: t1 = 0 (the 4-digit precision, |T| < 2^56).
+template <bool HI>
+__device__ __forceinline__ void mul_shr96(ull t0, ull t1, ull a0, ull a1, ull& r0, ull& r1, ull& r2) {
+    const unsigned __int128 p00 = (unsigned __int128)t0 * a0, p01 = (unsigned __int128)t0 * a1;
+    unsigned __int128 mid = (p00 >> 64) + (ull)p01, up = p01 >> 64;
+    if (HI) {
+        const unsigned __int128 p10 = (unsigned __int128)t1 * a0, p11 = (unsigned __int128)t1 * a1;
+        mid += (ull)p10;
+        up += (p10 >> 64) + p11;
+    }
+    up += mid >> 64;
+    const ull l1 = (ull)mid, l2 = (ull)up, l3 = (ull)(up >> 64);
+    r0 = (l1 >> 32) | (l2 << 32);
+    r1 = (l2 >> 32) | (l3 << 32);
+    r2 = l3 >> 32;
+}
+// g 2^e as a double-double (relative error <= 2^-104): sign and magnitude, the six 32-bit words of the magnitude
+// become doubles through the 2^52 trick with their scale in the exponent field ((2^52 + u) 2^k - 2^52 2^k = u 2^k,
+// exact) and are summed from the top.  Once per CTA and axis.
+__device__ __forceinline__ dd acc192_to_dd(acc192 g, int e) {
+    const bool neg = (long long)g.w2 < 0;
+    if (neg) { acc192 z{0, 0, 0}; acc_addsub(z, g.w0, g.w1, g.w2, true); g = z; }
+    const uint32_t w[6] = {(uint32_t)g.w0, (uint32_t)(g.w0 >> 32), (uint32_t)g.w1, (uint32_t)(g.w1 >> 32),
+                           (uint32_t)g.w2, (uint32_t)(g.w2 >> 32)};
+    dd r{0.0, 0.0};
+#pragma unroll
+    for (int k = 5; k >= 0; k--) {
+        const int e0 = 0x43300000 + ((e + 32 * k) << 20);
+        const double x = __dadd_rn(__hiloint2double(e0, (int)w[k]), -__hiloint2double(e0, 0));
+        r = dd_add_d(r, x);
+    }
     return neg ? dd{-r.h, -r.l} : r;
 }
 
@@ -71,7 +111,7 @@ template <int ND>
 __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
     int d, long N, long Npad, long njb128, int Ppad, int qscale_log2, int nkq,
     const int2* __restrict__ steps, int nsteps, int nseg, const int* __restrict__ wT,
-    const double* __restrict__ A, const signed char* __restrict__ Bg8, const signed char* __restrict__ W8,
+    const ulonglong2* __restrict__ Afix, const signed char* __restrict__ Bg8, const signed char* __restrict__ W8,
     double* __restrict__ gpart, const int* __restrict__ skip)
 {
     if (skip && *skip) return;
@@ -117,7 +157,9 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
             }
         }
     } else if (warp == G8_EPI_WARPS + 1) {
-        if (lane == 0) {
+        {
+            uint32_t elected;
+            asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(elected));
             int nblock = 0;
             bool fresh = true;                                 // next step starts a new accumulation
             for (int i = 0; i < total; i++) {
@@ -136,10 +178,10 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
                     const int n = (ii + 1) * 32, l0 = ND - 1 - ii;          // its partners: relative digits l0 .. ND - 1
                     const uint64_t da = dA0 + (uint64_t)((ii * G8_ASLAB) >> 4);
                     if (n <= 256) {
-                        g8_mma(tb, da, dW0 + (uint64_t)((l0 * G8_WSLAB) >> 4), g8_idesc(n), acc);
+                        g8_mma(tb, da, dW0 + (uint64_t)((l0 * G8_WSLAB) >> 4), g8_idesc(n), acc, elected);
                     } else {
-                        g8_mma(tb, da, dW0 + (uint64_t)((l0 * G8_WSLAB) >> 4), g8_idesc(256), acc);
-                        g8_mma(tb + 256, da, dW0 + (uint64_t)(((l0 + 8) * G8_WSLAB) >> 4), g8_idesc(n - 256), acc);
+                        g8_mma(tb, da, dW0 + (uint64_t)((l0 * G8_WSLAB) >> 4), g8_idesc(256), acc, elected);
+                        g8_mma(tb + 256, da, dW0 + (uint64_t)(((l0 + 8) * G8_WSLAB) >> 4), g8_idesc(n - 256), acc, elected);
                     }
                 };
                 // A block's first step runs from the most significant digit down (its first instruction covers all
@@ -153,10 +195,10 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
 #pragma unroll
                     for (int ii = 0; ii < ND; ii++) issue(ii, 1u);
                 }
-                g8_commit(smem_u32(&empty_bar[s]));
+                g8_commit(smem_u32(&empty_bar[s]), elected);
                 fresh = false;
                 if ((st.y >> 16) || i == total - 1) {          // block (or segment) end: hand the sums to the epilogue
-                    g8_commit(smem_u32(&tfull_bar));
+                    g8_commit(smem_u32(&tfull_bar), elected);
                     nblock++;
                     fresh = true;
                 }
@@ -166,9 +208,9 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
         // ---- 16 epilogue warps: thread = (particle = TMEM lane, quarter of the block's 8 p); columns 32 c + 4 p_local + out
         const int quarter = warp >> 2, row = tid & 127;
         const long j = jb * 128 + row;
-        const double qs = ldexp(1.0, qscale_log2);
-        const double2* Aj = reinterpret_cast<const double2*>(A) + (size_t)(j >> 2) * 3 * 32 * 4 + (j & 3);
-        dd g0{0.0, 0.0}, g1{0.0, 0.0}, g2{0.0, 0.0}, g3{0.0, 0.0};
+        const long NpadA = njb128 * 128;
+        const ulonglong2* Aj = Afix + (size_t)j * 2;
+        acc192 g[4] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
         int nblock = 0;
         // next block (or segment) end at or after step i: 32 steps per look, one load latency per block
         auto next_end = [&](int& i, int2& st) {
@@ -191,51 +233,52 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
         if (total > 0) next_end(i, st);
         while (i < total) {
             const int pb8 = st.x / nkq;
-            // this block's A_j[p] (three limbs each) and axis weights.  With fewer digits the epilogue's own latencies
-            // bound the kernel and registers are free: the loads go out before the wait for the tensor core
-            double2 araw[2][3];
+            // this block's A_j[p] (sign-magnitude integers trunc(a 2^102), k_tables) and axis weights, requested before
+            // the wait for the tensor core
+            ulonglong2 ar[2], ai[2];
             int wg[2][3];
-            auto load_A = [&]() {
 #pragma unroll
-                for (int pp = 0; pp < 2; pp++) {
-                    const int p = pb8 * 8 + quarter * 2 + pp;
-                    araw[pp][0] = araw[pp][1] = araw[pp][2] = make_double2(0.0, 0.0);
-                    wg[pp][0] = wg[pp][1] = wg[pp][2] = 0;
-                    if (j < N && p < Ppad) {
-                        const double2* ap = Aj + ((size_t)(p >> 5) * (Npad / 4) * 3 * 32 + (p & 31)) * 4;
-                        asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(araw[pp][0].x), "=d"(araw[pp][0].y) : "l"(ap));
-                        asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(araw[pp][1].x), "=d"(araw[pp][1].y) : "l"(ap + 128));
-                        asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(araw[pp][2].x), "=d"(araw[pp][2].y) : "l"(ap + 256));
+            for (int pp = 0; pp < 2; pp++) {
+                const int p = pb8 * 8 + quarter * 2 + pp;             // < Ppad8 (the table is allocated and zeroed up to there)
+                const ulonglong2* ap = Aj + (size_t)p * NpadA * 2;
+                asm volatile("ld.global.nc.v2.u64 {%0,%1}, [%2];" : "=l"(ar[pp].x), "=l"(ar[pp].y) : "l"(ap));
+                asm volatile("ld.global.nc.v2.u64 {%0,%1}, [%2];" : "=l"(ai[pp].x), "=l"(ai[pp].y) : "l"(ap + 1));
 #pragma unroll
-                        for (int ax = 0; ax < 3; ax++)
-                            if (ax < d) wg[pp][ax] = wT[ax * Ppad + p];
-                    }
-                }
-            };
-            if constexpr (ND < G8_ND) load_A();
+                for (int ax = 0; ax < 3; ax++) wg[pp][ax] = (ax < d && p < Ppad) ? wT[ax * Ppad + p] : 0;
+            }
             mbar_wait(smem_u32(&tfull_bar), (uint32_t)(nblock & 1));
             asm volatile("tcgen05.fence::after_thread_sync;");
-            // Drain: the thread's 16 columns (4 p x 4 outputs) of each of the ND digit sums, combined EXACTLY on the
+            // Drain: the thread's 8 columns (2 p x 4 outputs) of each of the ND digit sums, combined EXACTLY on the
             // integer pipe into NG 64-bit group values G_g = sum_c 2^(8 (c - 4 g)) S_c (four sums per group, the top
             // group takes a fifth).  Column block c holds the absolute digit sum s = ND - 1 + 2 OFF + c, a sum
             // of ND - c digit pairs of <= 2 Qn <= 10^4 products each: |S_c| <= (ND - c) 10^4 2^14, which bounds
             // the groups by 2^54.6, 2^53.9 and (top five, 5 + 4 2^8 + 3 2^16 + 2 2^24 + 2^32 pairs-weights) 2^59.3.
-            // Nothing else happens before the release, so the tensor core idles only for these loads.
+            // The loads go out four at a time (one wait per four); nothing else happens before the release.
             constexpr int NG = (ND + 2) / 4;
             long long G[NG][8];
             const uint32_t taddr = tb + ((uint32_t)((warp & 3) * 32) << 16) + 8 * quarter;
 #pragma unroll
-            for (int c = 0; c < ND; c++) {
-                uint32_t v[8];
-                asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-                             : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
-                             : "r"(taddr + c * 32));
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                const int g = (c / 4 < NG - 1) ? c / 4 : NG - 1, sh = 8 * (c - 4 * g);
+            for (int c0 = 0; c0 < ND; c0 += 4) {
+                uint32_t v[4][8];
 #pragma unroll
-                for (int e = 0; e < 8; e++) {
-                    const long long x = (long long)(int)v[e];
-                    G[g][e] = sh == 0 ? x : G[g][e] + x * (1ll << sh);
+                for (int cc = 0; cc < 4; cc++)
+                    if (c0 + cc < ND)
+                        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                                     : "=r"(v[cc][0]), "=r"(v[cc][1]), "=r"(v[cc][2]), "=r"(v[cc][3]), "=r"(v[cc][4]), "=r"(v[cc][5]),
+                                       "=r"(v[cc][6]), "=r"(v[cc][7])
+                                     : "r"(taddr + (c0 + cc) * 32));
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                for (int cc = 0; cc < 4; cc++) {
+                    const int c = c0 + cc;
+                    if (c < ND) {
+                        const int gq = (c / 4 < NG - 1) ? c / 4 : NG - 1, sh = 8 * (c - 4 * gq);
+#pragma unroll
+                        for (int e = 0; e < 8; e++) {
+                            const long long x = (long long)(int)v[cc][e];
+                            G[gq][e] = sh == 0 ? x : G[gq][e] + x * (1ll << sh);
+                        }
+                    }
                 }
             }
             // tensor memory is drained: the next block's instructions start while the rest of the epilogue runs
@@ -244,79 +287,61 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
             int inext = i + 1;                                 // the block after this one
             int2 stn = st;
             if (inext < total) next_end(inext, stn);
-            if constexpr (ND == G8_ND) load_A();               // (13 digits: after the release, the registers are needed above)
-            if constexpr (ND < G8_ND) {
-                // Fewer digits (operands of 54 or 30 bits): the sums are worth no more than a double, so the
-                // contraction with A_j[p] runs in plain FP64 (products rounded once, ~2^-53 relative, below the
-                // operand truncation); only the running per-axis sums stay double-double.  A tenth of the FP64
-                // instructions of the full path: at these digit counts the epilogue, not the tensor core, is
-                // what bounds the kernel.
-                const double w0 = __longlong_as_double((long long)(1023 + 8 * (ND - 1 + 2 * OFF) - 204) << 52);
+            // T = sum_g G_g 2^(32 g) (exact, |T| < 2^127), as sign and magnitude
+            ull t0[8], t1[8];
+            bool tn[8];
 #pragma unroll
-                for (int pp = 0; pp < 2; pp++) {
-                    double T[4];
+            for (int e = 0; e < 8; e++) {
+                __int128 T = (__int128)G[0][e];
 #pragma unroll
-                    for (int o4 = 0; o4 < 4; o4++) {
-                        double t = (double)G[0][4 * pp + o4];
-                        if (NG > 1) t = __fma_rn((double)G[NG - 1][4 * pp + o4], 4294967296.0, t);
-                        T[o4] = __dmul_rn(t, w0);
-                    }
-                    const double ar = __dadd_rn(__dadd_rn(araw[pp][0].x, araw[pp][1].x), araw[pp][2].x);
-                    const double ai = __dadd_rn(__dadd_rn(araw[pp][0].y, araw[pp][1].y), araw[pp][2].y);
-                    const int p = pb8 * 8 + quarter * 2 + pp;
-                    if (j < N && p < Ppad) {
-                        const double I = __fma_rn(ar, T[1], -__dmul_rn(ai, T[0]));      // Im[conj(A) T]
-                        const double R = __fma_rn(ar, T[2], __dmul_rn(ai, T[3]));       // Re[conj(A) T'']
-#define GACC8F(AX)                                                                            \
-    if (AX < d) {                                                                             \
-        const int wgt = AX < 3 ? wg[pp][AX < 3 ? AX : 0] : 0;                                 \
-        if (wgt != 0) g##AX = dd_add_d(g##AX, __dmul_rn(I, (double)wgt));                     \
-        if (AX == d - 1) g##AX = dd_add_d(g##AX, __dmul_rn(R, qs));                           \
-    }
-                        GACC8F(0) GACC8F(1) GACC8F(2) GACC8F(3)
-#undef GACC8F
-                    }
-                }
-            } else {
-                dd Tall[2][4];
+                for (int gq = 1; gq < NG; gq++) T += (__int128)G[gq][e] << (32 * gq);
+                tn[e] = T < 0;
+                const unsigned __int128 M = tn[e] ? (unsigned __int128)(-T) : (unsigned __int128)T;
+                t0[e] = (ull)M;
+                t1[e] = (ull)(M >> 64);
+            }
 #pragma unroll
-                for (int e = 0; e < 8; e++) {
-                    __int128 T = (__int128)G[0][e];                     // sum_c 2^(8 c) S_c, exact
+            for (int pp = 0; pp < 2; pp++) {
+                const ull ar0 = ar[pp].x, ar1 = ar[pp].y & 0x7fffffffffffffffULL, ai0 = ai[pp].x, ai1 = ai[pp].y & 0x7fffffffffffffffULL;
+                const bool arn = (long long)ar[pp].y < 0, ain = (long long)ai[pp].y < 0;
+                const ull* T0 = t0 + 4 * pp;
+                const ull* T1 = t1 + 4 * pp;
+                const bool* TN = tn + 4 * pp;
+                constexpr bool HI = ND > 4;
+                ull r0, r1, r2;
+                // I = Im[conj(A) T] = ar T_im - ai T_re,   R = Re[conj(A) T''] = ar T''_re + ai T''_im   (units 2^(e0) below)
+                acc192 I{0, 0, 0}, R{0, 0, 0};
+                mul_shr96<HI>(T0[1], T1[1], ar0, ar1, r0, r1, r2); acc_addsub(I, r0, r1, r2, arn != TN[1]);
+                mul_shr96<HI>(T0[0], T1[0], ai0, ai1, r0, r1, r2); acc_addsub(I, r0, r1, r2, ain == TN[0]);
+                mul_shr96<HI>(T0[2], T1[2], ar0, ar1, r0, r1, r2); acc_addsub(R, r0, r1, r2, arn != TN[2]);
+                mul_shr96<HI>(T0[3], T1[3], ai0, ai1, r0, r1, r2); acc_addsub(R, r0, r1, r2, ain != TN[3]);
 #pragma unroll
-                    for (int g = 1; g < NG; g++) T += (__int128)G[g][e] << (32 * g);
-                    Tall[e >> 2][e & 3] = s128_scaled_to_dd(T, 8 * (ND - 1 + 2 * OFF) - 204);
-                }
-#pragma unroll
-                for (int pp = 0; pp < 2; pp++) {
-                    const dd* T = Tall[pp];
-                    const dd ar = limbs_to_dd8(araw[pp][0].x, araw[pp][1].x, araw[pp][2].x);
-                    const dd ai = limbs_to_dd8(araw[pp][0].y, araw[pp][1].y, araw[pp][2].y);
-                    const int p = pb8 * 8 + quarter * 2 + pp;
-                    if (j < N && p < Ppad) {
-                        const dd I = dd_dot2(ar, T[1], ai, T[0], -1.0);         // Im[conj(A) T]
-                        const dd R = dd_dot2(ar, T[2], ai, T[3], 1.0);          // Re[conj(A) T'']
-#define GACC8(AX)                                                                             \
-    if (AX < d) {                                                                             \
-        const int wgt = AX < 3 ? wg[pp][AX < 3 ? AX : 0] : 0;                                 \
-        if (wgt != 0) g##AX = dd_add(g##AX, dd_mul_d(I, (double)wgt));                        \
-        if (AX == d - 1) g##AX = dd_add(g##AX, dd_scale2(R, qs));                             \
-    }
-                        GACC8(0) GACC8(1) GACC8(2) GACC8(3)
-#undef GACC8
+                for (int ax = 0; ax < 3; ax++) {
+                    const int wgt = wg[pp][ax];
+                    if (wgt != 0) {
+                        acc192 v = I;
+                        if (wgt < 0) { v = acc192{0, 0, 0}; acc_addsub(v, I.w0, I.w1, I.w2, true); }
+                        acc_mac(g[ax], v, (uint32_t)(wgt < 0 ? -wgt : wgt));
                     }
                 }
+#pragma unroll
+                for (int ax = 0; ax < 4; ax++)
+                    if (ax == d - 1) acc_mac(g[ax], R, 1u << qscale_log2);
             }
             nblock++;
             i = inext;
             st = stn;
         }
         if (j < N) {
+            constexpr int E0 = 8 * (ND - 1 + 2 * OFF) - 210;      // units of the accumulators: 2^(8 s0 - 204 - 102 + 96)
             double2* o = reinterpret_cast<double2*>(gpart);
             const size_t slot = (size_t)(seg * 4 + quarter) * d;       // four partials per segment (the p quarters)
-            if (d > 0) o[(slot + 0) * N + j] = make_double2(g0.h, g0.l);
-            if (d > 1) o[(slot + 1) * N + j] = make_double2(g1.h, g1.l);
-            if (d > 2) o[(slot + 2) * N + j] = make_double2(g2.h, g2.l);
-            if (d > 3) o[(slot + 3) * N + j] = make_double2(g3.h, g3.l);
+#pragma unroll
+            for (int ax = 0; ax < 4; ax++)
+                if (ax < d) {
+                    const dd r = acc192_to_dd(g[ax], E0);
+                    o[(slot + ax) * N + j] = make_double2(r.h, r.l);
+                }
         }
     }
     asm volatile("tcgen05.fence::before_thread_sync;");
@@ -341,7 +366,7 @@ cudaError_t shd_launch_grad8_main(shd_ctx* h)
     k_grad8<NDV><<<(unsigned)(h->njb128 * h->nseg8), G8_THREADS, G8_SMEM, h->stream>>>(                      \
         h->d, h->N, h->Npad, h->njb128, h->npb * 32, h->qscale_log2, h->nkq8,                          \
         reinterpret_cast<const int2*>(h->d_steps8), h->nsteps8, h->nseg8, h->d_wT,                     \
-        h->d_A, h->d_Bg8, h->d_W8, h->d_gpart, h->d_skip)
+        reinterpret_cast<const ulonglong2*>(h->d_Afix), h->d_Bg8, h->d_W8, h->d_gpart, h->d_skip)
     if (h->nlimb >= 3) LAUNCH_GRAD8(13);
     else if (h->nlimb == 2) LAUNCH_GRAD8(7);
     else LAUNCH_GRAD8(4);

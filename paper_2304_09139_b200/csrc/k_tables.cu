@@ -60,18 +60,33 @@ struct limbs { double x0, x1, x2; };
 // Returned packed: byte i of lo = digit i (i = 0..6), byte i of hi = digit 7 + i (i = 0..5), as s8 bit patterns
 // (offset byte - 128 = offset byte ^ 0x80, applied to all bytes of a word at once).
 struct digits13_t { unsigned long long lo, hi; };
-__device__ __forceinline__ digits13_t digits13(dd x) {
+struct fix102_t { long long lo, hi; };                               // X = hi 2^56 + lo, |lo| < 2^57
+__device__ __forceinline__ fix102_t fix102(dd x) {
     const double t = __dmul_rn(x.h, 0x1p46);                       // exact
     const double H = floor(t);
     const double r = __dadd_rn(t, -H);                             // exact, in [0, 1)
-    long long xlo = __double2ll_rz(__dmul_rn(r, 0x1p56)) + __double2ll_rz(__dmul_rn(x.l, 0x1p102));
-    long long xhi = __double2ll_rz(H);
+    fix102_t f;
+    f.lo = __double2ll_rz(__dmul_rn(r, 0x1p56)) + __double2ll_rz(__dmul_rn(x.l, 0x1p102));
+    f.hi = __double2ll_rz(H);
+    return f;
+}
+__device__ __forceinline__ digits13_t digits13(fix102_t f) {
+    long long xlo = f.lo, xhi = f.hi;
     xlo += 0x80808080808080LL;                                     // digits 0..6 of the offset
     xhi += 0x808080808080LL + (xlo >> 56);                         // digits 7..12, carry (arithmetic shift: may be -1)
     digits13_t d;
     d.lo = ((unsigned long long)xlo & 0xffffffffffffffULL) ^ 0x80808080808080ULL;
     d.hi = ((unsigned long long)xhi & 0xffffffffffffULL) ^ 0x808080808080ULL;
     return d;
+}
+__device__ __forceinline__ digits13_t digits13(dd x) { return digits13(fix102(x)); }
+// The same integer X as sign and magnitude in 128 bits (the INT8 gradient pass contracts its exact integer sums
+// with A_j[p] in integer arithmetic, k_grad8.cu): x = |X| low 64 bits, y = |X| high bits | sign << 63.
+__device__ __forceinline__ ulonglong2 signmag102(fix102_t f) {
+    const __int128 X = ((__int128)f.hi << 56) + (__int128)f.lo;
+    const bool neg = X < 0;
+    const unsigned __int128 M = neg ? (unsigned __int128)(-X) : (unsigned __int128)X;
+    return make_ulonglong2((unsigned long long)M, (unsigned long long)(M >> 64) | (neg ? 0x8000000000000000ULL : 0ULL));
 }
 __device__ __forceinline__ uint32_t digit_byte(const digits13_t& d, int i) {       // i compile-time after unrolling
     return i < 7 ? (uint32_t)(d.lo >> (8 * i)) & 0xffu : (uint32_t)(d.hi >> (8 * (i - 7))) & 0xffu;
@@ -151,14 +166,25 @@ struct Stager {
             }
         }
     }
+    ulonglong2* afix;     // A table of the INT8 gradient pass (or nullptr): [p][NpadA][re, im] sign-magnitude 128-bit integers
+    long NpadA;
+    __device__ __forceinline__ void put_fix(int p, const fix102_t& fr, const fix102_t& fi, bool live) {
+        if (afix == nullptr || !live) return;
+        ulonglong2* dst = afix + ((size_t)p * NpadA + j0 + threadIdx.x) * 2;     // a warp writes 1 KB contiguous
+        dst[0] = signmag102(fr);
+        dst[1] = signmag102(fi);
+    }
     signed char* dig;     // rho pass (or nullptr): row = 2 (entry % rows8) + re/im of block entry / rows8,
     long nk8;             //   K index = particle % 32 of K-step particle / 32 (nk8 K-steps per block)
     int rows8;            // entries per block: 64 (A) or 16 (B)
     signed char* dtile;   // shared-memory transpose tile [TG entries][2][13 digits][TB particles]
     // digits of one table entry for both INT8 tables (computed once)
-    __device__ __forceinline__ void put_digits(int slot, cdd z, bool live) {
+    __device__ __forceinline__ void put_digits(int slot, cdd z, bool live, int entry = -1) {
+        if (dig == nullptr && gdig == nullptr && afix == nullptr) return;
+        const fix102_t fr = fix102(z.re), fi = fix102(z.im);
+        if (entry >= 0) put_fix(entry, fr, fi, live);
         if (dig == nullptr && gdig == nullptr) return;
-        digits13_t dr = digits13(z.re), di = digits13(z.im);
+        digits13_t dr = digits13(fr), di = digits13(fi);
         if (!live) dr.lo = dr.hi = di.lo = di.hi = 0ULL;                            // particles beyond N: zero digits
         put8(slot, dr, di);
         putg8(slot, dr, di);
@@ -264,7 +290,7 @@ __global__ void __launch_bounds__(TB) k_tables(
     const double* __restrict__ pos_hi, const double* __restrict__ pos_lo,
     double* __restrict__ A, double* __restrict__ B, double* __restrict__ Bg, int with_grad,
     signed char* __restrict__ A8, signed char* __restrict__ B8, long nk8, signed char* __restrict__ Bg8, int nkq8,
-    const int* __restrict__ skip)
+    ulonglong2* __restrict__ Afix, long NpadA, const int* __restrict__ skip)
 {
     if (skip && *skip) return;
     extern __shared__ __align__(16) unsigned char tables_smem[];
@@ -284,6 +310,7 @@ __global__ void __launch_bounds__(TB) k_tables(
     st.gdig = gradB ? Bg8 : nullptr; st.nkq = nkq8;
     st.dig = which == 0 ? A8 : B8; st.nk8 = nk8; st.rows8 = which == 0 ? SHD_I8_PT : SHD_I8_QT;
     st.dtile = reinterpret_cast<signed char*>(tables_smem) + TABLES_LIMB_SMEM;
+    st.afix = (which == 0 && with_grad != 0) ? Afix : nullptr; st.NpadA = NpadA;
     if (which == 0) {
         // ---- A table
         cdd base;
@@ -299,13 +326,13 @@ __global__ void __launch_bounds__(TB) k_tables(
 #pragma unroll
                     for (int s = 0; s < TG; s++) {
                         st.put(0, s, cur);
-                        st.put_digits(s, cur, live);
+                        st.put_digits(s, cur, live, p0 + s);
                         cur = cdd_mul(cur, base);
                     }
                 } else {
                     for (int s = 0; s < cnt; s++) {
                         st.put(0, s, cur);
-                        st.put_digits(s, cur, live);
+                        st.put_digits(s, cur, live, p0 + s);
                         cur = cdd_mul(cur, base);
                     }
                 }
@@ -340,7 +367,7 @@ __global__ void __launch_bounds__(TB) k_tables(
                     }
                     const cdd az = cdd_mul(cur0, f);
                     st.put(0, s, az);
-                    st.put_digits(s, az, live);
+                    st.put_digits(s, az, live, p0 + s);
                 }
                 st.flush(p0, cnt, live);
             }
@@ -387,11 +414,13 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
 #define LAUNCH_TABLES(DLOV)                                                                                       \
     k_tables<DLOV><<<grid, TB, TABLES_SMEM, h->stream>>>(h->d, h->N, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2, \
                                          h->d_pn0, h->d_pn1, h->d_pn2, h->Qpad, pos_hi, pos_lo,                    \
-                                         h->d_A, h->rho_engine >= 1 ? nullptr : h->d_B,                            \
+                                         h->rho_engine == 2 ? nullptr : h->d_A, h->rho_engine >= 1 ? nullptr : h->d_B, \
                                          h->rho_engine == 2 ? nullptr : h->d_Bg, with_grad_tables ? 1 : 0,         \
                                          h->rho_engine >= 1 ? h->d_A8 : nullptr,                                   \
                                          h->rho_engine >= 1 ? h->d_B8 : nullptr, h->nk8,                           \
-                                         h->rho_engine == 2 ? h->d_Bg8 : nullptr, h->nkq8, h->d_skip)
+                                         h->rho_engine == 2 ? h->d_Bg8 : nullptr, h->nkq8,                         \
+                                         h->rho_engine == 2 ? reinterpret_cast<ulonglong2*>(h->d_Afix) : nullptr,  \
+                                         h->njb128 * 128, h->d_skip)
     // the INT8 engines read only the 13, 7 or 4 most significant digits (shd_set_precision): the rest is not written
     if (h->rho_engine == 0 || h->nlimb >= 3) LAUNCH_TABLES(0);
     else if (h->nlimb == 2) LAUNCH_TABLES(6);

@@ -298,8 +298,7 @@ int build(shd_ctx* h, const double* v) {
     if ((rc = upload(h, &h->d_tile_wmap, tile_wmap))) return rc;
     if ((rc = upload(h, &h->d_steps, steps))) return rc;
     if (!h->v.empty()) { if ((rc = upload(h, &h->d_v, h->v))) return rc; }
-    if ((rc = dalloc_zero(h, &h->d_A, (size_t)h->npb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
-    // (the B limb tables of the FP64 passes are allocated on first use: shd_prepare_tables)
+    // (the limb tables of the FP64 passes are allocated on first use: shd_prepare_tables)
     if ((rc = dalloc_zero(h, &h->d_C, (size_t)h->npb16 * (h->Qpad / 4) * (16 * SHD_PG * 4 * 2)))) return rc;
     h->gpart_doubles = (size_t)h->nseg * h->d * h->N * 2;
     if ((rc = dalloc_zero(h, &h->d_gpart, h->gpart_doubles))) return rc;
@@ -327,6 +326,8 @@ int build(shd_ctx* h, const double* v) {
 int shd_prepare_tables(shd_ctx* h, bool with_grad) {
     const bool i8 = true;          // the engines apply to every precision (fewer digits on the fast rungs)
     int rc;
+    if (h->rho_engine != 2 && !h->d_A)       // A limbs: both FP64 passes; the INT8 gradient pass reads d_Afix instead
+        if ((rc = dalloc_zero(h, &h->d_A, (size_t)h->npb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
     if (!(i8 && h->rho_engine >= 1) && !h->d_B)
         if ((rc = dalloc_zero(h, &h->d_B, (size_t)h->nqb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
     if (with_grad && !(i8 && h->rho_engine == 2) && !h->d_Bg)
@@ -444,7 +445,7 @@ void shd_destroy(shd_ctx* h) {
     cudaFree(h->d_rho); cudaFree(h->d_blockred); cudaFree(h->d_scal);
     cudaFree(h->d_hpos); cudaFree(h->d_hgrad);
     cudaFree(h->d_A8); cudaFree(h->d_B8); cudaFree(h->d_tile8_pb); cudaFree(h->d_tile8_qb);
-    cudaFree(h->d_Bg8); cudaFree(h->d_W8); cudaFree(h->d_steps8);
+    cudaFree(h->d_Bg8); cudaFree(h->d_W8); cudaFree(h->d_steps8); cudaFree(h->d_Afix);
     for (int i = 0; i <= SHD_NKERN; i++) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     if (h->h_scal) cudaFreeHost(h->h_scal);
     if (h->gevent) cudaEventDestroy(h->gevent);
@@ -609,6 +610,10 @@ int shd_set_engine(shd_ctx* h, int rho_engine) {
         }
         const size_t g8 = (size_t)h->njb128 * h->nkq8 * SHD_I8_DIGITS * 4096;
         const size_t w8 = (size_t)h->npb8 * h->nkq8 * SHD_I8_DIGITS * 1024;
+        const size_t af = (size_t)h->npb8 * 8 * (size_t)h->njb128 * 128 * 32;
+        CU(cudaMalloc(&h->d_Afix, af));
+        CU(cudaMemset(h->d_Afix, 0, af));
+        h->workspace_bytes += af;
         CU(cudaMalloc((void**)&h->d_Bg8, g8));
         CU(cudaMemset(h->d_Bg8, 0, g8));
         CU(cudaMalloc((void**)&h->d_W8, w8));

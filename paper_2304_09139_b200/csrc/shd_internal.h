@@ -123,6 +123,7 @@ struct shd_ctx {
     // INT8 gradient pass (shd_set_engine(h, 2))
     signed char *d_Bg8 = nullptr;  // [njb128][nkq8][13][128 rows (particle) x 32 K (q%16, re/im)]
     signed char *d_W8 = nullptr;   // [npb8][nkq8][13][32 rows (p%8, out) x 32 K]
+    void *d_Afix = nullptr;        // [npb8 * 8][njb128 * 128][re, im]: trunc(a 2^102) as sign-magnitude 128-bit integers
     int *d_steps8 = nullptr;       // int2: x = pb8 * nkq8 + kstep, y = kstep | block-end << 16
     int nsteps8 = 0, nseg8 = 0, npb8 = 0, nkq8 = 0;
     long njb128 = 0;
