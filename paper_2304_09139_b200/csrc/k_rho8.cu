@@ -37,14 +37,17 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t addr) {      // K-major, 
 __device__ __forceinline__ uint32_t umma_idesc_i8(int n) {          // D = s32, A = B = s8, M = 128
     return (2u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
 }
-__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+// issued by the elected lane of a converged warp (elected = 1 in one lane): the whole warp runs the issue loop, so
+// the descriptors stay in uniform registers and there is no per-instruction election loop (k_grad8.cu)
+__device__ __forceinline__ void umma_i8(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate, uint32_t elected) {
     uint32_t z = 0;
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                 "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %5, %5, %5}, p;\n\t}"
-                 ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate), "r"(z) : "memory");
+    asm volatile("{\n\t.reg .pred p, q;\n\tsetp.ne.b32 p, %4, 0;\n\tsetp.ne.b32 q, %6, 0;\n\t"
+                 "@q tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, {%5, %5, %5, %5}, p;\n\t}"
+                 ::"r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate), "r"(z), "r"(elected) : "memory");
 }
-__device__ __forceinline__ void umma_commit(uint32_t bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+__device__ __forceinline__ void umma_commit(uint32_t bar, uint32_t elected) {
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %1, 0;\n\t"
+                 "@q tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}" ::"r"(bar), "r"(elected) : "memory");
 }
 
 // ND = 13: full precision.  ND = 7 / 4: the "fast" precisions of shd_set_precision(h, 2 / 1) on this engine: only the
@@ -106,7 +109,9 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
             }
         }
     } else if (warp == 5) {
-        if (lane == 0) {
+        {
+            uint32_t elected;
+            asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(elected));
             // the ring position is a compile-time constant inside the unrolled inner loop: shared-memory addresses
             // and descriptors of a step are constants off one base, the step boundary costs a few instructions
             const uint64_t dbase = umma_desc(s0);
@@ -130,10 +135,10 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
                     const int n = (ii + 1) * 32, l0 = ND - 1 - ii;          // its partners: relative digits l0 .. ND - 1
                     const uint64_t da = dA0 + (uint64_t)((ii * R8_ASLAB) >> 4);
                     if (n <= 256) {
-                        umma_i8(tb, da, dB0 + (uint64_t)((l0 * R8_BSLAB) >> 4), umma_idesc_i8(n), acc);
+                        umma_i8(tb, da, dB0 + (uint64_t)((l0 * R8_BSLAB) >> 4), umma_idesc_i8(n), acc, elected);
                     } else {
-                        umma_i8(tb, da, dB0 + (uint64_t)((l0 * R8_BSLAB) >> 4), umma_idesc_i8(256), acc);
-                        umma_i8(tb + 256, da, dB0 + (uint64_t)(((l0 + 8) * R8_BSLAB) >> 4), umma_idesc_i8(n - 256), acc);
+                        umma_i8(tb, da, dB0 + (uint64_t)((l0 * R8_BSLAB) >> 4), umma_idesc_i8(256), acc, elected);
+                        umma_i8(tb + 256, da, dB0 + (uint64_t)(((l0 + 8) * R8_BSLAB) >> 4), umma_idesc_i8(n - 256), acc, elected);
                     }
                 };
                 if (i == 0 || ND < R8_ND) {                         // (with fewer digits the order makes no difference)
@@ -143,10 +148,10 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
 #pragma unroll
                     for (int ii = 0; ii < ND; ii++) issue(ii, 1u);
                 }
-                umma_commit(smem_u32(&empty_bar[s]));          // arrives when the tensor core is done with stage s
+                umma_commit(smem_u32(&empty_bar[s]), elected); // arrives when the tensor core is done with stage s
               }
             }
-            umma_commit(smem_u32(&done_bar));
+            umma_commit(smem_u32(&done_bar), elected);
         }
     } else {
         // ---- epilogue warps 0..3: warp w reads TMEM lanes 32 w .. 32 w + 31 (rows r = 2 p_local + c)
