@@ -122,16 +122,63 @@ int shd_get_rho(shd_ctx* h, double* re_hi, double* re_lo, double* im_hi, double*
 int shd_set_precision(shd_ctx* h, int limbs);
 
 /*
- * Engine of the rho pass (step a2).  0 (default): exact FP64 limb contraction on the FP64 matrix instruction
- * (k_rho.cu).  1: exact digit-sliced contraction on the INT8 tensor cores (tcgen05.mma.kind::i8, k_rho8.cu):
- * operands as 13 balanced base-256 digits of trunc(x 2^102), the 91 digit pairs with i + l >= 12, s32
- * accumulators in tensor memory (at most 8192 particles per CTA, so they are exact), the same double-double
- * result within the same tolerances.  2: the gradient pass too (k_grad8.cu).  shd_set_precision selects the
- * number of digits on these engines.  Allocates the digit tables on first use.  Errors: SHD_EINVAL (engine not
- * 0, 1 or 2; engine 2 with more than 5024 entries in the last-axis table: its s32 sums would not be exact),
+ * Engine of the two O(N M) passes (steps a2, a4).
+ *   2: both on the INT8 tensor cores (tcgen05.mma.kind::i8; k_rho8.cu, k_grad8.cu): operands as 13 balanced base-256
+ *      digits of trunc(x 2^102), the 91 digit pairs with i + l >= 12, s32 accumulators in tensor memory (exact: at most
+ *      8192 particles per CTA in the rho pass, at most 5024 last-axis entries in the gradient pass), the gradient pass's
+ *      final contraction in exact integer arithmetic; the same double-double results within the same tolerances.
+ *   1: the rho pass on the INT8 tensor cores, the gradient pass on the FP64 limbs.
+ *   0: exact FP64 limb contraction on the FP64 matrix instruction (k_rho.cu, k_grad.cu).
+ *  -1: the library's own choice, which is also what shd_create* starts with: engine 2 when the last-axis table has at
+ *      least 48 and at most 5024 entries and one evaluation is at least 5e7 pair-terms, engine 0 otherwise (short last
+ *      axes, as in d = 3, leave the 16-q tensor-core steps mostly empty; tiny systems are launch-bound either way).
+ * shd_set_precision selects the number of digits on the INT8 engines.  The tables of an engine are allocated on first
+ * use and those of the engine left behind are freed.  Errors: SHD_EINVAL (engine not -1..2; engine 2 with more than 5024
+ * entries in the last-axis table; no particle split keeps the s32 sums exact: the handle's engine is then unchanged),
  * SHD_ENOMEM, SHD_ECUDA.
  */
 int shd_set_engine(shd_ctx* h, int rho_engine);
+
+/*
+ * Bounded workspace (the paper's N = 2 x 10^6 at chi = 0.2 ... 0.4, needs 260 GB of
+ * phasor tables at once).  The per-particle tables are built for one CHUNK of particles at a time: pass 1 (rho) chunk
+ * by chunk into running double-double sums, pass 2 (gradient) chunk by chunk again.  A chunk is a whole number of the
+ * rho pass's particle splits and the running sums continue the same left fold over the splits, so every result is
+ * bit-identical to the single-chunk evaluation whatever the cap.  bytes = cap on the tables of this handle; 0 (default)
+ * = what the device has free when they are first allocated.  Errors: SHD_ENOMEM at the next evaluation when even one
+ * split does not fit.
+ */
+int shd_set_workspace(shd_ctx* h, unsigned long bytes);
+
+/*
+ * Particle sharding over GPUs: this handle evaluates N particles (its shard: pos_*, grad_* hold
+ * those only) of a system of N_total; rank / world = its position.  One exchange step per evaluation: the running sums
+ * of the shard's contributions to rho (a few MB) are all-gathered as bytes in rank order and added in that order on
+ * every GPU (a double-double add is not an ncclSum); the gradient pass is local.  S_max is normalised by N_total.
+ * Two ways to drive it:
+ *   - shd_comm_init: the library owns an NCCL communicator (unique id from shd_comm_unique_id on rank 0, broadcast by
+ *     the caller, e.g. torch.distributed); shd_energy_grad / shd_smax / shd_minimize then run as on one GPU, the
+ *     minimizers exchanging their few double-double dot products the same way (no host decision per iteration, all
+ *     ranks take bit-identical decisions);
+ *   - or the split calls below, with the caller doing the all-gather (any transport; this is also how several
+ *     shards are driven from one process on one GPU).
+ * Errors: SHD_EINVAL.
+ */
+int shd_set_shard(shd_ctx* h, long N_total, int rank, int world);
+/* 128 bytes (HOST out) identifying a new NCCL communicator; call on one rank, hand the bytes to all.  SHD_ECUDA when NCCL
+ * cannot be loaded (libnccl.so.2 is resolved at run time). */
+int shd_comm_unique_id(void* id128);
+/* Collective over the world of shd_set_shard: every rank calls it with the same 128 bytes. */
+int shd_comm_init(shd_ctx* h, const void* id128);
+/* Size in bytes of a shard's partial (the same on every rank: tiles x 4 sums x 1024 cells x (hi, lo)). */
+unsigned long shd_partial_bytes(const shd_ctx* h);
+/* Pass 1 of a shard: partial_out (DEVICE, shd_partial_bytes(h) bytes, caller-owned) receives the running sums of the
+ * shard's contributions to rho; synchronises the stream. */
+int shd_rho_partial(shd_ctx* h, const double* pos_hi, const double* pos_lo, void* partial_out);
+/* gathered (DEVICE): nparts partials in rank order, back to back -> rho, Phi (HOST phi[2]), S_max on this handle. */
+int shd_rho_finish(shd_ctx* h, const void* gathered, int nparts, double phi[2]);
+/* Pass 2 of a shard: the gradient of its own particles (DEVICE, d*N doubles each) from the rho of shd_rho_finish. */
+int shd_grad_local(shd_ctx* h, const double* pos_hi, const double* pos_lo, double* grad_hi, double* grad_lo);
 
 /*
  * Structure factor of the LAST evaluation on this handle (Eq. 3): S(k) = |rho(k)|^2 / N for every k
@@ -177,40 +224,6 @@ int shd_minimize(shd_ctx* h, double* pos_hi, double* pos_lo, const shd_min_opts*
 
 /* Text of the last error on this handle (never NULL). */
 const char* shd_last_error(const shd_ctx* h);
-
-/* Per-kernel device timing: with on != 0 every later shd_energy_grad / shd_smax records CUDA events on
- * the handle's stream around its launch groups; read the durations with shd_stat(h, 20..24). */
-int shd_set_timing(shd_ctx* h, int on);
-
-/* Introspection used by bench.py / tests (host scalars):
- *   what = 0 / 12: DFMAs the rho / gradient pass launches (padding included),
- *   what = 1: kernel launches of the last call, 2: padded (p,q) cell count of the rho pass,
- *   3: valid cell count, 4: bytes of device workspace, 5: particle splits of the rho pass,
- *   6: (p,q) tiles, 7: P, 8: Qn, 9: padded particle count, 10: particle blocks of the gradient
- *   pass, 11: q-steps walked by one gradient block,
- *   20..24: milliseconds of the last call's launch groups (needs shd_set_timing):
- *           20 phasor tables (a1), 21 rho pass (a2), 22 finish (a3), 23 gradient operand, 24 gradient pass (a4). */
-double shd_stat(const shd_ctx* h, int what);
-
-/*
- * Measured FP64-pipe issue rate of the current device, the denominator of the "alu" roofline
- * (DESIGN.md "roofline").  kind = 0: dependent-DFMA chains, 1: DADD chains (8 per
- * thread, all SMs), 2: chains of the FP64 matrix instruction DMMA.8x8x4 (8 per warp; counted as 8 FMAs
- * per thread and instruction), the instruction the rho and gradient passes issue; runs for about
- * `seconds` (0 < seconds <= 10).  HOST out: instr_per_s[0] = best
- * launch, instr_per_s[1] = mean over the run (sustained), in thread-level FP64 instructions per
- * second.  Errors: SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA.  Needs no handle.
- */
-int shd_fp64_peak(int kind, double seconds, double instr_per_s[2]);
-
-/*
- * INT8 tensor-core probe (an exact digit-sliced contraction on tcgen05.mma.kind::i8 would
- * replace the FP64 limb FMAs).  HOST out: *mismatches = wrong entries of a 128 x 64 x 128 s8 x s8 -> s32 product
- * computed by the 5th-generation tensor core (operands in shared memory, accumulator in TMEM) against the
- * integer product on the host (0 = exact); *tops = measured issue rate of M=128, N=256, K=32 instructions on
- * all SMs in tera-operations per second (2 per multiply-accumulate).  Needs no handle.
- */
-int shd_i8_probe(double* tops, long* mismatches);
 
 #ifdef __cplusplus
 }

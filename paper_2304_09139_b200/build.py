@@ -14,7 +14,7 @@ from pathlib import Path
 HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 LIB = HERE / "libshd.so"
-SOURCES = ["shd_api.cu", "k_tables.cu", "k_rho.cu", "k_rho8.cu", "k_finish.cu", "k_grad.cu", "k_grad8.cu", "shd_min.cu", "shd_fire.cu", "k_probe.cu"]
+SOURCES = ["shd_api.cu", "k_tables.cu", "k_rho.cu", "k_rho8.cu", "k_finish.cu", "k_grad.cu", "k_grad8.cu", "shd_min.cu", "shd_fire.cu", "shd_comm.cu", "k_probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--fmad=false", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
 
@@ -24,7 +24,7 @@ def needs_build() -> bool:
         return True
     t = LIB.stat().st_mtime
     deps = list(CSRC.glob("*.cu")) + list(CSRC.glob("*.cuh")) + list(CSRC.glob("*.h")) + \
-        list(CSRC.glob("*.inc")) + [HERE.parent / "include" / "shd.h"]
+        list(CSRC.glob("*.inc")) + [HERE.parent / "include" / "shd.h", HERE.parent / "include" / "shd_bench.h"]
     return any(p.stat().st_mtime > t for p in deps)
 
 

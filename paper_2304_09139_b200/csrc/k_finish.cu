@@ -54,9 +54,14 @@ __device__ __forceinline__ void account(red& r, dd re, dd im, double v, long lon
     r.maxvs = fmax(r.maxvs, v * v * s.h);
 }
 
-// one thread per (tile, cell)
+// one thread per (tile, cell).  The four real sums X of a cell are the left fold, in fixed order, of the partials of
+// all particle splits: X = (((xin + part_0) + part_1) + ...).  An evaluation whose tables are built chunk by chunk
+// (bounded workspace) calls this once per chunk with the running sums xin / xout (fin = 0), a sharded one once more
+// with the ranks' running sums as the partials; the result does not depend on where the chunk boundaries fall.
+// fin != 0: rho(k), |rho|^2, Phi, S_max partials; else only xout is written.
 __global__ void __launch_bounds__(256) k_finish1(
-    const double* __restrict__ part, int nsplit, int ntiles, int tp, int tq, const int* __restrict__ tile_pb,
+    const double* __restrict__ part, int nsplit, const double* __restrict__ xin, double* __restrict__ xout, int fin,
+    int ntiles, int tp, int tq, const int* __restrict__ tile_pb,
     const int* __restrict__ tile_qb, const int* __restrict__ cell_kp, const int* __restrict__ cell_km,
     int Ppad, int Qpad, long M, const double* __restrict__ v, double* __restrict__ rho, double* __restrict__ blockred,
     const int* __restrict__ skip)
@@ -76,24 +81,30 @@ __global__ void __launch_bounds__(256) k_finish1(
 #pragma unroll
             for (int x = 0; x < 4; x++) {
                 dd acc = dd{0, 0};
+                if (xin) {
+                    double2 t = reinterpret_cast<const double2*>(xin)[((size_t)tile * 4 + x) * 1024 + cell];
+                    acc = dd{t.x, t.y};
+                }
                 for (int s = 0; s < nsplit; s++) {
                     double2 t = src[((size_t)(s * (long)ntiles + tile) * 4 + x) * 1024 + cell];
                     acc = dd_add(acc, dd{t.x, t.y});
                 }
                 X[x] = acc;
+                if (xout) reinterpret_cast<double2*>(xout)[((size_t)tile * 4 + x) * 1024 + cell] = make_double2(acc.h, acc.l);
             }
-            if (kp >= 0) {
+            if (fin && kp >= 0) {
                 dd re = dd_sub(X[0], X[1]), im = dd_add(X[2], X[3]);
                 rho[kp] = re.h; rho[M + kp] = re.l; rho[2 * M + kp] = im.h; rho[3 * M + kp] = im.l;
                 account(r, re, im, v ? v[kp] : 1.0, kp);
             }
-            if (km >= 0) {
+            if (fin && km >= 0) {
                 dd re = dd_add(X[0], X[1]), im = dd_sub(X[3], X[2]);
                 rho[km] = re.h; rho[M + km] = re.l; rho[2 * M + km] = im.h; rho[3 * M + km] = im.l;
                 account(r, re, im, v ? v[km] : 1.0, km);
             }
         }
     }
+    if (!fin) return;
     r = block_reduce(r);
     if (threadIdx.x == 0) {
         double* o = blockred + (size_t)blockIdx.x * 8;
@@ -291,17 +302,22 @@ cudaError_t shd_launch_sfactor(shd_ctx* h, double* S_out, double* scratch, doubl
     return cudaGetLastError();
 }
 
-cudaError_t shd_launch_finish(shd_ctx* h)
+// Fold `nparts` partial arrays (part: [nparts][ntiles][4][1024] (hi, lo)) into the running sums: xin (or zero) -> xout
+// (either may be NULL); fin: also rho, Phi, S_max, argmax (k_finish2).
+cudaError_t shd_launch_fold(shd_ctx* h, const double* part, int nparts, const double* xin, double* xout, bool fin)
 {
     const bool i8 = h->rho_engine >= 1;
     const int ntiles = i8 ? h->ntiles8 : h->ntiles;
     const int nb = (int)(((long)ntiles * 1024 + 255) / 256);
-    k_finish1<<<nb, 256, 0, h->stream>>>(h->d_part, i8 ? h->nsplit8 : h->nsplit, ntiles, i8 ? SHD_I8_PT : 32,
+    k_finish1<<<nb, 256, 0, h->stream>>>(part, nparts, xin, xout, fin ? 1 : 0, ntiles, i8 ? SHD_I8_PT : 32,
                                          i8 ? SHD_I8_QT : 32, i8 ? h->d_tile8_pb : h->d_tile_pb,
                                          i8 ? h->d_tile8_qb : h->d_tile_qb, h->d_cell_kp, h->d_cell_km,
                                          h->npb * 32, h->Qpad, h->M, h->d_v, h->d_rho, h->d_blockred, h->d_skip);
-    k_finish2<<<1, 1024, 0, h->stream>>>(h->d_blockred, nb, h->N, h->d_scal, h->d_skip);
-    h->last_launches += 2;
+    h->last_launches += 1;
+    if (fin) {
+        k_finish2<<<1, 1024, 0, h->stream>>>(h->d_blockred, nb, h->Nsys, h->d_scal, h->d_skip);
+        h->last_launches += 1;
+    }
     return cudaGetLastError();
 }
 

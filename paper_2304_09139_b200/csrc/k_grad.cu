@@ -293,13 +293,16 @@ __global__ void __launch_bounds__(NW * 32 + 128, 1) k_grad(
     }
 }
 
-// grad = (4 pi / L) / cscale * sum_seg gpart[seg], fixed order
+// grad = (4 pi / L) / cscale * sum_seg gpart[seg], fixed order.  gpart holds the nc particles of one chunk
+// ([seg][d][nc]); they are particles j_first .. j_first + nc - 1 of the caller's arrays (axis stride N).
 __global__ void __launch_bounds__(256) k_gradsum(
-    long n, int nseg, double L, const double* __restrict__ gpart, const shd_scalars* __restrict__ scal,
-    double* __restrict__ grad_hi, double* __restrict__ grad_lo, const int* __restrict__ skip)
+    long nc, int d, long j_first, long N, int nseg, double L, const double* __restrict__ gpart,
+    const shd_scalars* __restrict__ scal, double* __restrict__ grad_hi, double* __restrict__ grad_lo,
+    const int* __restrict__ skip)
 {
     if (skip && *skip) return;
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long n = nc * d;
     if (i >= n) return;
     dd sum{0.0, 0.0};
     for (int s = 0; s < nseg; s++) {
@@ -309,8 +312,9 @@ __global__ void __launch_bounds__(256) k_gradsum(
     dd pref = dd_div_d(dd_mul_d(dd{0x1.921fb54442d18p+2, 0x1.1a62633145c07p-52}, 2.0), L);   // 4 pi / L
     sum = dd_mul(sum, pref);
     sum = dd_scale2(sum, 1.0 / scal->cscale);
-    grad_hi[i] = sum.h;
-    grad_lo[i] = sum.l;
+    const long o = (i / nc) * N + j_first + i % nc;
+    grad_hi[o] = sum.h;
+    grad_lo[o] = sum.l;
 }
 
 }  // namespace
@@ -323,29 +327,30 @@ cudaError_t shd_grad_configure()
     return e;
 }
 
-cudaError_t shd_launch_grad(shd_ctx* h, double* grad_hi, double* grad_lo)
+// gradient of the chunk's particles j_first .. j_first + nc - 1 (their tables are in place) into the caller's arrays
+cudaError_t shd_launch_grad(shd_ctx* h, long j_first, long nc, double* grad_hi, double* grad_lo)
 {
+    const long n = (long)h->d * nc;
     if (h->rho_engine == 2) {          // INT8 tensor-core gradient pass (k_grad8.cu)
-        cudaError_t e = shd_launch_grad8_main(h);
+        cudaError_t e = shd_launch_grad8_main(h, nc);
         if (e != cudaSuccess) return e;
-        const long n8 = (long)h->d * h->N;
-        k_gradsum<<<(unsigned)((n8 + 255) / 256), 256, 0, h->stream>>>(
-            n8, 4 * h->nseg8, h->L, h->d_gpart, h->d_scal, grad_hi, grad_lo, h->d_skip);
+        k_gradsum<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(
+            nc, h->d, j_first, h->N, 4 * h->nseg8, h->L, h->d_gpart, h->d_scal, grad_hi, grad_lo, h->d_skip);
         h->last_launches += 1;
         return cudaGetLastError();
     }
+    const long njb = (nc + SHD_JT - 1) / SHD_JT;
 #define LAUNCH_GRAD(NLV)                                                                                 \
-    k_grad<NLV><<<(unsigned)(h->njb64 * h->nseg), NW * 32 + 128, GSMEM, h->stream>>>(                      \
-        h->d, h->N, h->Npad, h->njb64, h->Qpad, h->npb * 32, h->qscale_log2,                               \
+    k_grad<NLV><<<(unsigned)(njb * h->nseg), NW * 32 + 128, GSMEM, h->stream>>>(                           \
+        h->d, nc, h->Npad, njb, h->Qpad, h->npb * 32, h->qscale_log2,                                      \
         reinterpret_cast<const int2*>(h->d_steps), h->nsteps, h->nseg, h->d_wT,                            \
         h->d_A, h->d_Bg, h->d_C, h->d_gpart, h->d_skip)
     if (h->nlimb >= 3) LAUNCH_GRAD(3);
     else if (h->nlimb == 2) LAUNCH_GRAD(2);
     else LAUNCH_GRAD(1);
 #undef LAUNCH_GRAD
-    const long n = (long)h->d * h->N;
     k_gradsum<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(
-        n, h->nseg, h->L, h->d_gpart, h->d_scal, grad_hi, grad_lo, h->d_skip);
+        nc, h->d, j_first, h->N, h->nseg, h->L, h->d_gpart, h->d_scal, grad_hi, grad_lo, h->d_skip);
     h->last_launches += 2;
     return cudaGetLastError();
 }

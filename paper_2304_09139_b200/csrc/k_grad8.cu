@@ -359,12 +359,13 @@ cudaError_t shd_grad8_configure()
     return e;
 }
 
-// k_gradsum (k_grad.cu) adds the segments' partial gradients and applies 4 pi / L / cscale
-cudaError_t shd_launch_grad8_main(shd_ctx* h)
+// k_gradsum (k_grad.cu) adds the segments' partial gradients and applies 4 pi / L / cscale; nc = particles of the chunk
+cudaError_t shd_launch_grad8_main(shd_ctx* h, long nc)
 {
+    const long njb = (nc + 127) / 128;
 #define LAUNCH_GRAD8(NDV)                                                                            \
-    k_grad8<NDV><<<(unsigned)(h->njb128 * h->nseg8), G8_THREADS, G8_SMEM, h->stream>>>(                      \
-        h->d, h->N, h->Npad, h->njb128, h->npb * 32, h->qscale_log2, h->nkq8,                          \
+    k_grad8<NDV><<<(unsigned)(njb * h->nseg8), G8_THREADS, G8_SMEM, h->stream>>>(                            \
+        h->d, nc, h->Npad, h->njb128, h->npb * 32, h->qscale_log2, h->nkq8,                            \
         reinterpret_cast<const int2*>(h->d_steps8), h->nsteps8, h->nseg8, h->d_wT,                     \
         reinterpret_cast<const ulonglong2*>(h->d_Afix), h->d_Bg8, h->d_W8, h->d_gpart, h->d_skip)
     if (h->nlimb >= 3) LAUNCH_GRAD8(13);

@@ -3,7 +3,7 @@
 // Every thread runs 8 independent dependent-DFMA (or DADD) chains, or every warp 8 independent
 // chains of the FP64 matrix instruction (mma.sync m8n8k4, SASS DMMA.8x8x4 = 256 FMAs per warp =
 // 8 per thread); the result is thread-level FP64 instructions (FMAs) per second over the whole GPU.
-#include "../../include/shd.h"
+#include "../../include/shd_bench.h"
 #include <cuda_runtime.h>
 #include <cstdint>
 #include <vector>

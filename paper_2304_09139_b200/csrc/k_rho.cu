@@ -206,10 +206,10 @@ cudaError_t shd_rho_configure()
     return e;
 }
 
-cudaError_t shd_launch_rho(shd_ctx* h)
+cudaError_t shd_launch_rho(shd_ctx* h, int nsplits)
 {
-    if (h->rho_engine >= 1) return shd_launch_rho8(h);      // INT8 tensor-core engine (k_rho8.cu)
-    unsigned grid = (unsigned)(h->ntiles * h->nsplit);
+    if (h->rho_engine >= 1) return shd_launch_rho8(h, nsplits);      // INT8 tensor-core engine (k_rho8.cu)
+    unsigned grid = (unsigned)(h->ntiles * nsplits);        // the splits of one chunk
 #define LAUNCH_RHO(NLV)                                                                                   \
     k_rho<NLV><<<grid, NW * 32 + 128, RHO_SMEM, h->stream>>>(h->d_A, h->d_B, h->d_tile_pb, h->d_tile_qb,    \
         h->d_tile_wmap, h->ntiles, h->Npad, h->chunks_per_split, h->d_part, h->d_skip)

@@ -197,9 +197,9 @@ cudaError_t shd_rho8_configure()
     return e;
 }
 
-cudaError_t shd_launch_rho8(shd_ctx* h)
+cudaError_t shd_launch_rho8(shd_ctx* h, int nsplits)
 {
-    const unsigned grid = (unsigned)(h->ntiles8 * h->nsplit8);
+    const unsigned grid = (unsigned)(h->ntiles8 * nsplits);      // the splits of one chunk
 #define LAUNCH_RHO8(NDV)                                                                              \
     k_rho8<NDV><<<grid, 192, R8_SMEM, h->stream>>>(h->d_A8, h->d_B8, h->d_tile8_pb, h->d_tile8_qb, h->ntiles8, \
                                                    h->nk8, h->ksteps8, h->d_part, h->d_skip)

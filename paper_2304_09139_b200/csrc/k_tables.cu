@@ -11,6 +11,7 @@
 #include <cstdint>
 #include "shd_internal.h"
 #include "sincos_table.inc"
+#include <algorithm>
 
 namespace {
 
@@ -129,6 +130,7 @@ struct Stager {
     // ---- s8 digit tables of the INT8 passes (k_rho8.cu, k_grad8.cu); all in the tensor core's K-major
     // core-matrix layout: 8 rows x 16 bytes per core matrix (128 B contiguous), K-adjacent core matrices
     // 128 B apart, 8-row groups 256 B apart.
+    long NpadG;           // particle slots of the gradient-pass tables (multiple of 128)
     signed char* gdig;    // gradient pass, particle operand (B thread only, or nullptr): row = particle % 128 of
     int nkq;              //   block particle / 128, K index = 2 (q % 16) + re/im of K-step q / 16 (nkq per block)
     uint32_t gacc[SHD_I8_DIGITS][4];   // this particle's 16 bytes per digit for the 8 entries of a flush group
@@ -147,7 +149,11 @@ struct Stager {
     __device__ __forceinline__ void flushg8(int q0, int count, bool live) {
         if (gdig == nullptr) return;
         const long j = j0 + threadIdx.x;
-        if (live) {
+        if (!live) {
+#pragma unroll
+            for (int i = DLO; i < SHD_I8_DIGITS; i++) gacc[i][0] = gacc[i][1] = gacc[i][2] = gacc[i][3] = 0u;
+        }
+        if (j < NpadG) {
             const int row = (int)(j & 127);
             signed char* base = gdig + (((size_t)(j >> 7) * nkq + (size_t)(q0 >> 4)) * SHD_I8_DIGITS) * 4096 +
                                 (row >> 3) * 256 + ((q0 >> 3) & 1) * 128 + (row & 7) * 16;
@@ -169,10 +175,10 @@ struct Stager {
     ulonglong2* afix;     // A table of the INT8 gradient pass (or nullptr): [p][NpadA][re, im] sign-magnitude 128-bit integers
     long NpadA;
     __device__ __forceinline__ void put_fix(int p, const fix102_t& fr, const fix102_t& fi, bool live) {
-        if (afix == nullptr || !live) return;
+        if (afix == nullptr || j0 + threadIdx.x >= NpadA) return;
         ulonglong2* dst = afix + ((size_t)p * NpadA + j0 + threadIdx.x) * 2;     // a warp writes 1 KB contiguous
-        dst[0] = signmag102(fr);
-        dst[1] = signmag102(fi);
+        dst[0] = live ? signmag102(fr) : make_ulonglong2(0ULL, 0ULL);
+        dst[1] = live ? signmag102(fi) : make_ulonglong2(0ULL, 0ULL);
     }
     signed char* dig;     // rho pass (or nullptr): row = 2 (entry % rows8) + re/im of block entry / rows8,
     long nk8;             //   K index = particle % 32 of K-step particle / 32 (nk8 K-steps per block)
@@ -219,9 +225,10 @@ struct Stager {
         }
     }
     __device__ __forceinline__ static int swz(int r) { return ((r & 1) << 2) | (r & 2) | ((r >> 2) & 1); }
-    __device__ __forceinline__ void put(int plane0, int slot, cdd z) {
+    __device__ __forceinline__ void put(int plane0, int slot, cdd z, bool live) {
         if (table == nullptr && Bg == nullptr) return;
         limbs a = split_limbs(z.re), b = split_limbs(z.im);
+        if (!live) a.x0 = a.x1 = a.x2 = b.x0 = b.x1 = b.x2 = 0.0;    // particles beyond N: zero limbs (a chunk's table is reused)
         const int t = threadIdx.x, c = slot ^ swz(t);
         double2* row = tile + (t * planes + plane0) * TG;
         row[0 * TG + c] = make_double2(a.x0, b.x0);
@@ -245,7 +252,7 @@ struct Stager {
             const bool cok = c < count;
 #pragma unroll
             for (int a = 0; a < TB / 8; a++) {
-                const bool ok = cok && j0 + 8 * a + r0 < N;
+                const bool ok = cok && j0 + 8 * a + r0 < Npad;
 #pragma unroll
                 for (int l = 0; l < 3; l++)
                     if (ok) dst[(size_t)(6 * a + l) * 128] = src[(a * 8 * 3 + l) * TG];
@@ -285,7 +292,7 @@ struct Stager {
 // which = 0: A table.  which = 1: B table (+ the same limbs in the gradient layout Bg).
 template <int DLO>
 __global__ void __launch_bounds__(TB) k_tables(
-    int d, long N, double L, long Npad, int P, int Qn, int S1d, int qscale_log2,
+    int d, long N, long j_first, double L, long Npad, int P, int Qn, int S1d, int qscale_log2,
     const int* __restrict__ pn0, const int* __restrict__ pn1, const int* __restrict__ pn2, int Qpad,
     const double* __restrict__ pos_hi, const double* __restrict__ pos_lo,
     double* __restrict__ A, double* __restrict__ B, double* __restrict__ Bg, int with_grad,
@@ -297,16 +304,16 @@ __global__ void __launch_bounds__(TB) k_tables(
     double2* tile = reinterpret_cast<double2*>(tables_smem);
     const int which = blockIdx.y;
     const long j0 = (long)blockIdx.x * TB;
-    const long j = j0 + threadIdx.x;
-    const bool live = j < N;
-    const long jc = live ? j : N - 1;            // dead threads shadow the last particle (keeps barriers uniform)
+    const long j = j0 + threadIdx.x;             // slot in the (chunk's) tables; particle j_first + j of the handle
+    const bool live = j_first + j < N;
+    const long jc = live ? j_first + j : N - 1;  // dead threads shadow the last particle (keeps barriers uniform)
     const cdd one{dd{1.0, 0.0}, dd{0.0, 0.0}};
     const bool gradB = which == 1 && with_grad != 0;
     Stager<DLO> st;
     st.tile = tile; st.planes = 3;
     st.table = which == 0 ? A : B;                      // may be nullptr: the INT8 rho pass does not read B limbs
     st.Bg = gradB ? Bg : nullptr;                       // nullptr too when the gradient pass runs on INT8
-    st.Npad = Npad; st.j0 = j0; st.N = N; st.Qpad = Qpad;
+    st.Npad = Npad; st.j0 = j0; st.N = N - j_first; st.Qpad = Qpad; st.NpadG = NpadA;
     st.gdig = gradB ? Bg8 : nullptr; st.nkq = nkq8;
     st.dig = which == 0 ? A8 : B8; st.nk8 = nk8; st.rows8 = which == 0 ? SHD_I8_PT : SHD_I8_QT;
     st.dtile = reinterpret_cast<signed char*>(tables_smem) + TABLES_LIMB_SMEM;
@@ -325,13 +332,13 @@ __global__ void __launch_bounds__(TB) k_tables(
                     // work of one entry overlaps the serial double-double recurrence of the next
 #pragma unroll
                     for (int s = 0; s < TG; s++) {
-                        st.put(0, s, cur);
+                        st.put(0, s, cur, live);
                         st.put_digits(s, cur, live, p0 + s);
                         cur = cdd_mul(cur, base);
                     }
                 } else {
                     for (int s = 0; s < cnt; s++) {
-                        st.put(0, s, cur);
+                        st.put(0, s, cur, live);
                         st.put_digits(s, cur, live, p0 + s);
                         cur = cdd_mul(cur, base);
                     }
@@ -366,7 +373,7 @@ __global__ void __launch_bounds__(TB) k_tables(
                         f = cdd_mul(f, n2 >= 0 ? pw2[n2] : cdd_conj(pw2[-n2]));
                     }
                     const cdd az = cdd_mul(cur0, f);
-                    st.put(0, s, az);
+                    st.put(0, s, az, live);
                     st.put_digits(s, az, live, p0 + s);
                 }
                 st.flush(p0, cnt, live);
@@ -382,13 +389,13 @@ __global__ void __launch_bounds__(TB) k_tables(
             if (cnt == TG) {
 #pragma unroll
                 for (int s = 0; s < TG; s++) {
-                    st.put(0, s, cur);
+                    st.put(0, s, cur, live);
                     st.put_digits(s, cur, live);
                     cur = cdd_mul(cur, base);
                 }
             } else {
                 for (int s = 0; s < cnt; s++) {
-                    st.put(0, s, cur);
+                    st.put(0, s, cur, live);
                     st.put_digits(s, cur, live);
                     cur = cdd_mul(cur, base);
                 }
@@ -408,21 +415,27 @@ cudaError_t shd_tables_configure()
     return e;
 }
 
-cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool with_grad_tables)
+// what: 1 = the tables of the rho pass, 2 = the tables of the gradient pass (bit mask); j_first = first particle of the chunk
+cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* pos_lo, long j_first, int what)
 {
-    dim3 grid((unsigned)((h->N + TB - 1) / TB), 2);
+    const int e = h->rho_engine;
+    const bool rho = (what & 1) != 0, grad = (what & 2) != 0;
+    // every slot of the chunk's tables is written (zeros beyond the handle's last particle)
+    const long slots = std::max(std::max(h->Npad, h->nk8 * 32), std::max(h->njb128 * 128, h->njb64 * 64));
+    dim3 grid((unsigned)((slots + TB - 1) / TB), 2);
+    double* A = (e == 2 || !(rho || grad)) ? nullptr : ((e == 1 && !grad) ? nullptr : h->d_A);   // FP64 rho pass and FP64 gradient pass
+    double* B = (e == 0 && rho) ? h->d_B : nullptr;
+    double* Bg = (e != 2 && grad) ? h->d_Bg : nullptr;
+    signed char* A8 = (e >= 1 && rho) ? h->d_A8 : nullptr;
+    signed char* B8 = (e >= 1 && rho) ? h->d_B8 : nullptr;
+    signed char* Bg8 = (e == 2 && grad) ? h->d_Bg8 : nullptr;
+    ulonglong2* Afix = (e == 2 && grad) ? reinterpret_cast<ulonglong2*>(h->d_Afix) : nullptr;
 #define LAUNCH_TABLES(DLOV)                                                                                       \
-    k_tables<DLOV><<<grid, TB, TABLES_SMEM, h->stream>>>(h->d, h->N, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2, \
-                                         h->d_pn0, h->d_pn1, h->d_pn2, h->Qpad, pos_hi, pos_lo,                    \
-                                         h->rho_engine == 2 ? nullptr : h->d_A, h->rho_engine >= 1 ? nullptr : h->d_B, \
-                                         h->rho_engine == 2 ? nullptr : h->d_Bg, with_grad_tables ? 1 : 0,         \
-                                         h->rho_engine >= 1 ? h->d_A8 : nullptr,                                   \
-                                         h->rho_engine >= 1 ? h->d_B8 : nullptr, h->nk8,                           \
-                                         h->rho_engine == 2 ? h->d_Bg8 : nullptr, h->nkq8,                         \
-                                         h->rho_engine == 2 ? reinterpret_cast<ulonglong2*>(h->d_Afix) : nullptr,  \
-                                         h->njb128 * 128, h->d_skip)
+    k_tables<DLOV><<<grid, TB, TABLES_SMEM, h->stream>>>(h->d, h->N, j_first, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2, \
+                                         h->d_pn0, h->d_pn1, h->d_pn2, h->Qpad, pos_hi, pos_lo, A, B, Bg, grad ? 1 : 0, \
+                                         A8, B8, h->nk8, Bg8, h->nkq8, Afix, h->njb128 * 128, h->d_skip)
     // the INT8 engines read only the 13, 7 or 4 most significant digits (shd_set_precision): the rest is not written
-    if (h->rho_engine == 0 || h->nlimb >= 3) LAUNCH_TABLES(0);
+    if (e == 0 || h->nlimb >= 3) LAUNCH_TABLES(0);
     else if (h->nlimb == 2) LAUNCH_TABLES(6);
     else LAUNCH_TABLES(9);
 #undef LAUNCH_TABLES

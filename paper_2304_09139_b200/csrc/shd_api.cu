@@ -1,6 +1,6 @@
 // shd_api.cu -- the C-ABI of include/shd.h: host-side setup (step a0: enumeration of Q, the
 // outer-product decomposition, tile lists) and the launch sequences of the hot path.
-#include "../../include/shd.h"
+#include "../../include/shd_bench.h"
 #include "shd_internal.h"
 
 #include <algorithm>
@@ -270,20 +270,19 @@ int build(shd_ctx* h, const double* v) {
             if (best_cost < 0.0 || cost < best_cost) { best_cost = cost; h->nsplit = (int)ns; h->chunks_per_split = cps; }
         }
     }
-    h->Npad = (long)h->nsplit * h->chunks_per_split * SHD_NPS;
     h->njb = (h->N + 31) / 32;
-    h->njb64 = (h->N + SHD_JT - 1) / SHD_JT;
     // ---- segments of the gradient pass: minimise (waves of CTAs) x (steps per CTA)
     {
         double best = -1.0;
         h->nseg = 1;
+        const long njb64 = (h->N + SHD_JT - 1) / SHD_JT;
         for (int ns = 1; ns <= std::min(16, h->nsteps); ns++) {
-            long waves = (h->njb64 * ns + sms - 1) / sms;
+            long waves = (njb64 * ns + sms - 1) / sms;
             double cost = (double)waves * ((double)((h->nsteps + ns - 1) / ns) + 4.0);   // +4: prologue, epilogue, partial write
             if (best < 0.0 || cost < best) { best = cost; h->nseg = ns; }
         }
     }
-    // ---- device memory
+    // ---- device memory that does not depend on the engine or on the chunk size
     int rc;
     if ((rc = upload(h, &h->d_pn0, h->pn0))) return rc;
     if ((rc = upload(h, &h->d_pn1, h->pn1))) return rc;
@@ -298,45 +297,285 @@ int build(shd_ctx* h, const double* v) {
     if ((rc = upload(h, &h->d_tile_wmap, tile_wmap))) return rc;
     if ((rc = upload(h, &h->d_steps, steps))) return rc;
     if (!h->v.empty()) { if ((rc = upload(h, &h->d_v, h->v))) return rc; }
-    // (the limb tables of the FP64 passes are allocated on first use: shd_prepare_tables)
-    if ((rc = dalloc_zero(h, &h->d_C, (size_t)h->npb16 * (h->Qpad / 4) * (16 * SHD_PG * 4 * 2)))) return rc;
-    h->gpart_doubles = (size_t)h->nseg * h->d * h->N * 2;
-    if ((rc = dalloc_zero(h, &h->d_gpart, h->gpart_doubles))) return rc;
-    h->part_doubles = (size_t)h->nsplit * h->ntiles * 4 * 1024 * 2;
-    if ((rc = dalloc_zero(h, &h->d_part, h->part_doubles))) return rc;
     if ((rc = dalloc_zero(h, &h->d_rho, (size_t)4 * h->M))) return rc;
-    h->nfinish_blocks = (int)(((long)h->ntiles * 1024 + 255) / 256);
-    if ((rc = dalloc_zero(h, &h->d_blockred, (size_t)h->nfinish_blocks * 8))) return rc;
     CU(cudaMalloc((void**)&h->d_scal, sizeof(shd_scalars)));
     CU(cudaMemset(h->d_scal, 0, sizeof(shd_scalars)));
     CU(cudaMallocHost((void**)&h->h_scal, sizeof(shd_scalars)));
     std::memset(h->h_scal, 0, sizeof(shd_scalars));
+    h->cell_kp.swap(kp);
+    h->cell_km.swap(km);
     CU(shd_tables_configure());
     CU(shd_rho_configure());
     CU(shd_grad_configure());
     return SHD_OK;
 }
 
-// table != nullptr: the caller's half-space set (M vectors, row-major) instead of the shell n.n <= m_star
+// ---- INT8 engines: tile list and particle splits of the rho pass (k_rho8.cu), step list of the gradient pass
+// (k_grad8.cu).  Host work and small uploads only; the digit tables are allocated by shd_prepare_tables.
+int plan_engine8(shd_ctx* h, int engine) {
+    cudaDeviceProp prop;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    CU(cudaGetDeviceProperties(&prop, dev));
+    const long sms = prop.multiProcessorCount;
+    const std::vector<int>&kp = h->cell_kp, &km = h->cell_km;
+    int rc;
+    if (engine == 2 && !h->d_steps8) {
+        // step list over blocks of 8 p (K-steps of 16 q up to the block's last valid cell)
+        h->npb8 = (h->P + 7) / 8;
+        h->nkq8 = h->Qpad / 16;
+        std::vector<int> steps;
+        for (int pb = 0; pb < h->npb8; pb++) {
+            int nk = 0;
+            for (int pi = 0; pi < 8; pi++) {
+                const int p = pb * 8 + pi;
+                if (p >= h->npb * 32) continue;
+                for (int q = 0; q < h->Qpad; q++)
+                    if (kp[(size_t)p * h->Qpad + q] >= 0 || km[(size_t)p * h->Qpad + q] >= 0) nk = std::max(nk, q / 16 + 1);
+            }
+            for (int k = 0; k < nk; k++) {
+                steps.push_back(pb * h->nkq8 + k);
+                steps.push_back(k | ((k == nk - 1 ? 1 : 0) << 16));
+            }
+        }
+        h->nsteps8 = (int)steps.size() / 2;
+        double best = -1.0;
+        h->nseg8 = 1;
+        const long njb128 = (h->N + 127) / 128;
+        // at least two segments: the CTAs of one particle block then stream the same digit slabs side by side (L2)
+        for (int ns = std::min(2, h->nsteps8); ns <= std::min(32, h->nsteps8); ns++) {
+            const long waves = (njb128 * ns + sms - 1) / sms;
+            const double cost = (double)waves * ((double)((h->nsteps8 + ns - 1) / ns) + 6.0);
+            if (best < 0.0 || cost < best) { best = cost; h->nseg8 = ns; }
+        }
+        if ((rc = upload(h, &h->d_steps8, steps))) return rc;
+        CU(shd_grad8_configure());
+    }
+    if (engine >= 1 && !h->d_tile8_pb) {
+        h->npb64 = (h->P + SHD_I8_PT - 1) / SHD_I8_PT;
+        h->nqb16 = (h->Qn + SHD_I8_QT - 1) / SHD_I8_QT;
+        std::vector<int> tpb, tqb;
+        for (int pb = 0; pb < h->npb64; pb++)
+            for (int qb = 0; qb < h->nqb16; qb++) {
+                bool any = false;
+                for (int pi = 0; pi < SHD_I8_PT && !any; pi++)
+                    for (int qi = 0; qi < SHD_I8_QT && !any; qi++) {
+                        const int p = pb * SHD_I8_PT + pi, q = qb * SHD_I8_QT + qi;
+                        if (p < h->npb * 32 && q < h->Qpad) any = kp[(size_t)p * h->Qpad + q] >= 0 || km[(size_t)p * h->Qpad + q] >= 0;
+                    }
+                if (any) { tpb.push_back(pb); tqb.push_back(qb); }
+            }
+        h->ntiles8 = (int)tpb.size();
+        // particle splits: at most SHD_I8_MAXN particles per CTA (exact s32 sums); minimise waves x (K-steps + epilogue)
+        const long nk = (h->N + 31) / 32;
+        double best = -1.0;
+        h->nsplit8 = 0;
+        for (long ns = (h->N + SHD_I8_MAXN - 1) / SHD_I8_MAXN; ns <= std::max<long>(std::min<long>(512, nk), (h->N + SHD_I8_MAXN - 1) / SHD_I8_MAXN); ns++) {
+            const long per = (nk + ns - 1) / ns, waves = ((long)h->ntiles8 * ns + sms - 1) / sms;
+            const double cost = (double)waves * ((double)per + 8.0) + 0.004 * (double)ns * h->ntiles8;
+            if (best < 0.0 || cost < best) { best = cost; h->nsplit8 = (int)ns; h->ksteps8 = (int)per; }
+        }
+        if (h->nsplit8 < 1 || (long)h->ksteps8 * 32 > SHD_I8_MAXN)
+            return fail(h, SHD_EINVAL, "shd_set_engine: no particle split keeps the s32 digit sums of the INT8 rho pass exact");
+        if ((rc = upload(h, &h->d_tile8_pb, tpb))) return rc;
+        if ((rc = upload(h, &h->d_tile8_qb, tqb))) return rc;
+        CU(shd_rho8_configure());
+    }
+    return SHD_OK;
+}
+
+void free_tables(shd_ctx* h) {
+    cudaFree(h->d_A); cudaFree(h->d_B); cudaFree(h->d_Bg); cudaFree(h->d_A8); cudaFree(h->d_B8); cudaFree(h->d_Bg8);
+    cudaFree(h->d_Afix); cudaFree(h->d_W8); cudaFree(h->d_C); cudaFree(h->d_part); cudaFree(h->d_gpart);
+    cudaFree(h->d_blockred); cudaFree(h->d_xrun); cudaFree(h->d_xall);
+    h->d_A = h->d_B = h->d_Bg = h->d_C = h->d_part = h->d_gpart = h->d_blockred = h->d_xrun = h->d_xall = nullptr;
+    h->d_A8 = h->d_B8 = h->d_Bg8 = h->d_W8 = nullptr;
+    h->d_Afix = nullptr;
+    h->workspace_bytes -= h->table_bytes;
+    h->table_bytes = 0;
+    h->tables_valid = false;
+    h->grad_tables_ready = false;
+}
+
+// bytes of per-particle tables (both passes) and of rho-pass partials per split for the current engine
+void table_footprint(const shd_ctx* h, double& per_particle, double& per_split, double& fixed) {
+    const int e = h->rho_engine;
+    const double limbA = (double)h->npb * 1536.0, limbB = (double)h->nqb * 1536.0, limbBg = (double)h->Qpad * 48.0;
+    const double a8 = (double)h->npb64 * 1664.0, b8 = (double)h->nqb16 * 416.0, bg8 = (double)h->nkq8 * 416.0;
+    const double afix = (double)h->npb8 * 8 * 32.0;
+    const int ntiles = e >= 1 ? h->ntiles8 : h->ntiles;
+    if (e == 0) per_particle = limbA + limbB + limbBg + (double)h->nseg * h->d * 16.0;
+    else if (e == 1) per_particle = a8 + b8 + limbA + limbBg + (double)h->nseg * h->d * 16.0;
+    else per_particle = a8 + b8 + bg8 + afix + 4.0 * h->nseg8 * h->d * 16.0;
+    per_split = (double)ntiles * 65536.0;
+    fixed = 3.0 * ntiles * 65536.0 + (double)h->npb16 * (h->Qpad / 4) * 16384.0 + (double)h->npb8 * h->nkq8 * SHD_I8_DIGITS * 1024.0;
+}
+
+// chunk size for the current engine: as many whole splits as the workspace cap (or the free device memory) holds
+int choose_chunks(shd_ctx* h) {
+    const int e = h->rho_engine;
+    const long nsplit_total = e >= 1 ? h->nsplit8 : h->nsplit;
+    h->unit = e >= 1 ? (long)h->ksteps8 * 32 : h->chunks_per_split * SHD_NPS;
+    double pp, ps, fx;
+    table_footprint(h, pp, ps, fx);
+    double cap = (double)h->ws_cap;
+    if (h->ws_cap == 0) {
+        size_t fr = 0, tot = 0;
+        CU(cudaMemGetInfo(&fr, &tot));
+        cap = 0.92 * (double)fr;
+    }
+    const double per_split_all = pp * (double)h->unit + ps;
+    long m = (long)std::floor((cap - fx) / per_split_all);
+    if (m < 1) return fail(h, SHD_ENOMEM, "workspace cap (or free device memory) below the tables of one particle split");
+    m = std::min(m, nsplit_total);
+    h->nchunk = (int)((nsplit_total + m - 1) / m);
+    h->spc = (int)((nsplit_total + h->nchunk - 1) / h->nchunk);          // balanced chunks
+    h->nchunk = (int)((nsplit_total + h->spc - 1) / h->spc);
+    h->Nc = (long)h->spc * h->unit;
+    h->Npad = e == 0 ? h->Nc : ((h->Nc + 7) / 8) * 8;                    // FP64 limb tables (engine 1: A limbs and Bg of the gradient pass)
+    h->nk8 = e >= 1 ? (long)h->spc * h->ksteps8 : 0;
+    h->njb64 = (h->Nc + SHD_JT - 1) / SHD_JT;
+    h->njb128 = e == 2 ? (h->Nc + 127) / 128 : 0;
+    return SHD_OK;
+}
+
 }  // namespace
 
-// Limb tables of the FP64 engine that the current (engine, precision) setting reads, allocated on first use so
-// that a handle driven on the INT8 engines only never holds them (at the paper's N they are 49 GB each).
-// Called outside any stream capture.
+// Device tables of the current (engine, chunk) setting, allocated on first use (outside any stream capture) and freed
+// when the setting changes: a handle driven on the INT8 engines never holds the FP64 limb tables and vice versa.
 int shd_prepare_tables(shd_ctx* h, bool with_grad) {
-    const bool i8 = true;          // the engines apply to every precision (fewer digits on the fast rungs)
     int rc;
-    if (h->rho_engine != 2 && !h->d_A)       // A limbs: both FP64 passes; the INT8 gradient pass reads d_Afix instead
-        if ((rc = dalloc_zero(h, &h->d_A, (size_t)h->npb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
-    if (!(i8 && h->rho_engine >= 1) && !h->d_B)
-        if ((rc = dalloc_zero(h, &h->d_B, (size_t)h->nqb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
-    if (with_grad && !(i8 && h->rho_engine == 2) && !h->d_Bg)
-        if ((rc = dalloc_zero(h, &h->d_Bg, (size_t)(2 * h->njb64) * (h->Qpad / 4) * SHD_GROUP_DOUBLES))) return rc;
+    const int e = h->rho_engine;
+    if (!h->tables_valid) {
+        free_tables(h);
+        if ((rc = choose_chunks(h))) return rc;
+        const size_t before = h->workspace_bytes;
+        const int ntiles = e >= 1 ? h->ntiles8 : h->ntiles;
+        const size_t xdoubles = (size_t)ntiles * 4 * 1024 * 2;
+        if (e == 0 || e == 1) {
+            if (e == 0 && (rc = dalloc_zero(h, &h->d_B, (size_t)h->nqb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
+        }
+        if (e >= 1) {
+            const size_t a8 = (size_t)h->npb64 * h->nk8 * SHD_I8_DIGITS * (SHD_I8_PT * 2 * 32);
+            const size_t b8 = (size_t)h->nqb16 * h->nk8 * SHD_I8_DIGITS * (SHD_I8_QT * 2 * 32);
+            CU(cudaMalloc((void**)&h->d_A8, a8));
+            CU(cudaMalloc((void**)&h->d_B8, b8));
+            CU(cudaMemset(h->d_A8, 0, a8));
+            CU(cudaMemset(h->d_B8, 0, b8));
+            h->workspace_bytes += a8 + b8;
+        }
+        if (e == 0 && (rc = dalloc_zero(h, &h->d_A, (size_t)h->npb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
+        if ((rc = dalloc_zero(h, &h->d_part, (size_t)h->spc * xdoubles))) return rc;
+        if ((rc = dalloc_zero(h, &h->d_blockred, (size_t)(((long)ntiles * 1024 + 255) / 256) * 8))) return rc;
+        if (h->nchunk > 1 || shd_sharded(h))
+            if ((rc = dalloc_zero(h, &h->d_xrun, xdoubles))) return rc;
+        if (shd_sharded(h))
+            if ((rc = dalloc_zero(h, &h->d_xall, (size_t)h->world * xdoubles))) return rc;
+        h->table_bytes += h->workspace_bytes - before;
+        h->tables_valid = true;
+    }
+    if (with_grad && !h->d_gpart) {
+        const size_t before = h->workspace_bytes;
+        if (e == 2) {
+            const size_t g8 = (size_t)h->njb128 * h->nkq8 * SHD_I8_DIGITS * 4096;
+            const size_t w8 = (size_t)h->npb8 * h->nkq8 * SHD_I8_DIGITS * 1024;
+            const size_t af = (size_t)h->npb8 * 8 * (size_t)h->njb128 * 128 * 32;
+            CU(cudaMalloc(&h->d_Afix, af));
+            CU(cudaMemset(h->d_Afix, 0, af));
+            CU(cudaMalloc((void**)&h->d_Bg8, g8));
+            CU(cudaMemset(h->d_Bg8, 0, g8));
+            CU(cudaMalloc((void**)&h->d_W8, w8));
+            CU(cudaMemset(h->d_W8, 0, w8));
+            h->workspace_bytes += g8 + w8 + af;
+            if ((rc = dalloc_zero(h, &h->d_gpart, (size_t)4 * h->nseg8 * h->d * h->Nc * 2))) return rc;
+        } else {
+            if (e == 1 && (rc = dalloc_zero(h, &h->d_A, (size_t)h->npb * (h->Npad / 4) * SHD_GROUP_DOUBLES))) return rc;
+            if ((rc = dalloc_zero(h, &h->d_Bg, (size_t)(2 * h->njb64) * (h->Qpad / 4) * SHD_GROUP_DOUBLES))) return rc;
+            if ((rc = dalloc_zero(h, &h->d_C, (size_t)h->npb16 * (h->Qpad / 4) * (16 * SHD_PG * 4 * 2)))) return rc;
+            if ((rc = dalloc_zero(h, &h->d_gpart, (size_t)h->nseg * h->d * h->Nc * 2))) return rc;
+        }
+        h->table_bytes += h->workspace_bytes - before;
+    }
     return SHD_OK;
+}
+
+// ---- the evaluation, enqueued on h->stream (also inside the minimizers' captured slots)
+cudaError_t shd_enqueue_rho_partial(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool grad_tables_too)
+{
+    const int e = h->rho_engine;
+    const long nsplit_total = e >= 1 ? h->nsplit8 : h->nsplit;
+    const bool both = h->nchunk == 1 && grad_tables_too;      // one chunk: one table build serves both passes
+    cudaError_t err;
+    for (int c = 0; c < h->nchunk; c++) {
+        const long j0 = (long)c * h->Nc;
+        const int ns = (int)std::min<long>(h->spc, nsplit_total - (long)c * h->spc);
+        const bool last = c == h->nchunk - 1;
+        if ((err = shd_launch_tables(h, pos_hi, pos_lo, j0, both ? 3 : 1)) != cudaSuccess) return err;
+        if (c == 0 && h->timing_mark) h->timing_mark(h, 1);
+        if ((err = shd_launch_rho(h, ns)) != cudaSuccess) return err;
+        if (last && h->timing_mark) h->timing_mark(h, 2);
+        const bool fin = last && !shd_sharded(h);
+        if ((err = shd_launch_fold(h, h->d_part, ns, c > 0 ? h->d_xrun : nullptr, fin ? nullptr : h->d_xrun, fin)) != cudaSuccess) return err;
+    }
+    h->grad_tables_ready = both;
+    return cudaSuccess;
+}
+
+cudaError_t shd_enqueue_rho_finish(shd_ctx* h, const double* gathered, int nparts)
+{
+    return shd_launch_fold(h, gathered, nparts, nullptr, nullptr, true);
+}
+
+cudaError_t shd_enqueue_grad(shd_ctx* h, const double* pos_hi, const double* pos_lo, double* grad_hi, double* grad_lo)
+{
+    cudaError_t err;
+    if ((err = shd_launch_ctable(h)) != cudaSuccess) return err;
+    if (h->timing_mark) h->timing_mark(h, 4);
+    for (int c = 0; c < h->nchunk; c++) {
+        const long j0 = (long)c * h->Nc;
+        const long nc = std::min<long>(h->Nc, h->N - j0);
+        if (nc <= 0) break;
+        if (!h->grad_tables_ready)
+            if ((err = shd_launch_tables(h, pos_hi, pos_lo, j0, 2)) != cudaSuccess) return err;
+        if ((err = shd_launch_grad(h, j0, nc, grad_hi, grad_lo)) != cudaSuccess) return err;
+    }
+    h->grad_tables_ready = false;          // the caller may move the particles before the next call
+    return cudaSuccess;
+}
+
+cudaError_t shd_enqueue_eval(shd_ctx* h, const double* pos_hi, const double* pos_lo, double* grad_hi, double* grad_lo)
+{
+    cudaError_t err;
+    h->last_launches = 0;
+    if (h->timing_mark) h->timing_mark(h, 0);
+    if ((err = shd_enqueue_rho_partial(h, pos_hi, pos_lo, grad_hi != nullptr)) != cudaSuccess) return err;
+    if (shd_sharded(h)) {
+        const int ntiles = h->rho_engine >= 1 ? h->ntiles8 : h->ntiles;
+        if ((err = shd_comm_allgather(h, h->d_xrun, h->d_xall, (size_t)ntiles * 4 * 1024 * 16)) != cudaSuccess) return err;
+        if ((err = shd_enqueue_rho_finish(h, h->d_xall, h->world)) != cudaSuccess) return err;
+    }
+    if (h->timing_mark) h->timing_mark(h, 3);
+    if (grad_hi) {
+        if ((err = shd_enqueue_grad(h, pos_hi, pos_lo, grad_hi, grad_lo)) != cudaSuccess) return err;
+        if (h->timing_mark) h->timing_mark(h, 5);
+    }
+    return cudaSuccess;
 }
 
 namespace {
 
+// The engine a fresh handle starts on: both O(N M) passes on the INT8 tensor cores (engine 2) where they pay off --
+// a last-axis table long enough to fill the 16-q K-steps and short enough for exact s32 sums, and enough pair-terms
+// to amortise the digit tables -- else the FP64 limb engine.  shd_set_engine overrides.
+void auto_engine(shd_ctx* h) {
+    h->engine_auto = 1;
+    const bool fits8 = (long)h->Qpad * 2 * SHD_I8_DIGITS * 16384 < (1L << 31);
+    const bool pays = (double)h->N * (double)h->M >= 5e7 && h->Qn >= 48;
+    if (fits8 && pays && plan_engine8(h, 2) == SHD_OK) h->rho_engine = 2;
+    else { h->rho_engine = 0; h->err.clear(); }
+}
+
+// table != nullptr: the caller's half-space set (M vectors, row-major) instead of the shell n.n <= m_star
 int create_common(int d, long N, double L, long m_star, const double* v, shd_ctx** out,
                   const int* table = nullptr, long M = 0) {
     if (!out) return SHD_EINVAL;
@@ -352,7 +591,7 @@ int create_common(int d, long N, double L, long m_star, const double* v, shd_ctx
     }
     shd_ctx* h = new (std::nothrow) shd_ctx();
     if (!h) return SHD_ENOMEM;
-    h->d = d; h->N = N; h->L = L; h->m_star = m_star;
+    h->d = d; h->N = N; h->Nsys = N; h->L = L; h->m_star = m_star;
     if (table) {
         h->nvec.assign(table, table + M * d);
         h->m_star = 0;
@@ -365,6 +604,7 @@ int create_common(int d, long N, double L, long m_star, const double* v, shd_ctx
     int rc;
     try {
         rc = build(h, v);
+        if (rc == SHD_OK) auto_engine(h);
     } catch (const std::bad_alloc&) {
         rc = SHD_ENOMEM;
         h->err = "host allocation failed";
@@ -374,11 +614,9 @@ int create_common(int d, long N, double L, long m_star, const double* v, shd_ctx
 }
 
 // event i is recorded BEFORE launch group i; event SHD_NKERN after the last group
-int mark(shd_ctx* h, int i) {
-    if (!h->timing) return SHD_OK;
-    CU(cudaEventRecord(h->ev[i], h->stream));
-    h->ev_used[i] = true;
-    return SHD_OK;
+void mark(shd_ctx* h, int i) {
+    if (!h->timing) return;
+    if (cudaEventRecord(h->ev[i], h->stream) == cudaSuccess) h->ev_used[i] = true;
 }
 int collect_timing(shd_ctx* h) {      // after the stream has been synchronised
     if (!h->timing) return SHD_OK;
@@ -392,26 +630,21 @@ int collect_timing(shd_ctx* h) {      // after the stream has been synchronised
     }
     return SHD_OK;
 }
-// rho pass + reduction (steps a1-a3); optionally the gradient tables too
-int run_rho(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool with_grad) {
-    int prc = shd_prepare_tables(h, with_grad);
-    if (prc) return prc;
-    h->last_launches = 0;
-    for (int i = 0; i <= SHD_NKERN; i++) h->ev_used[i] = false;
-    int rc;
-    if ((rc = mark(h, 0))) return rc;
-    CU(shd_launch_tables(h, pos_hi, pos_lo, with_grad));
-    if ((rc = mark(h, 1))) return rc;
-    CU(shd_launch_rho(h));
-    if ((rc = mark(h, 2))) return rc;
-    CU(shd_launch_finish(h));
-    if ((rc = mark(h, 3))) return rc;
-    return SHD_OK;
-}
 int fetch_scalars(shd_ctx* h) {
     CU(cudaMemcpyAsync(h->h_scal, h->d_scal, sizeof(shd_scalars), cudaMemcpyDeviceToHost, h->stream));
     CU(cudaStreamSynchronize(h->stream));
     return SHD_OK;
+}
+int run_eval(shd_ctx* h, const double* pos_hi, const double* pos_lo, double* grad_hi, double* grad_lo) {
+    int rc = shd_prepare_tables(h, grad_hi != nullptr);
+    if (rc) return rc;
+    for (int i = 0; i <= SHD_NKERN; i++) h->ev_used[i] = false;
+    h->timing_mark = h->timing ? mark : nullptr;
+    cudaError_t e = shd_enqueue_eval(h, pos_hi, pos_lo, grad_hi, grad_lo);
+    h->timing_mark = nullptr;
+    CU(e);
+    if ((rc = fetch_scalars(h))) return rc;
+    return collect_timing(h);
 }
 
 }  // namespace
@@ -439,13 +672,12 @@ void shd_destroy(shd_ctx* h) {
     if (!h) return;
     shd_min_free(h);
     shd_fire_free(h);
+    shd_comm_free(h);
+    free_tables(h);
     cudaFree(h->d_pn0); cudaFree(h->d_pn1); cudaFree(h->d_pn2); cudaFree(h->d_wT); cudaFree(h->d_cell_kp); cudaFree(h->d_cell_km);
-    cudaFree(h->d_tile_pb); cudaFree(h->d_tile_qb); cudaFree(h->d_tile_wmap); cudaFree(h->d_steps); cudaFree(h->d_v); cudaFree(h->d_gpart);
-    cudaFree(h->d_A); cudaFree(h->d_B); cudaFree(h->d_Bg); cudaFree(h->d_C); cudaFree(h->d_part);
-    cudaFree(h->d_rho); cudaFree(h->d_blockred); cudaFree(h->d_scal);
-    cudaFree(h->d_hpos); cudaFree(h->d_hgrad);
-    cudaFree(h->d_A8); cudaFree(h->d_B8); cudaFree(h->d_tile8_pb); cudaFree(h->d_tile8_qb);
-    cudaFree(h->d_Bg8); cudaFree(h->d_W8); cudaFree(h->d_steps8); cudaFree(h->d_Afix);
+    cudaFree(h->d_tile_pb); cudaFree(h->d_tile_qb); cudaFree(h->d_tile_wmap); cudaFree(h->d_steps); cudaFree(h->d_v);
+    cudaFree(h->d_rho); cudaFree(h->d_scal); cudaFree(h->d_hpos);
+    cudaFree(h->d_tile8_pb); cudaFree(h->d_tile8_qb); cudaFree(h->d_steps8); cudaFree(h->d_shell); cudaFree(h->d_trace);
     for (int i = 0; i <= SHD_NKERN; i++) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     if (h->h_scal) cudaFreeHost(h->h_scal);
     if (h->gevent) cudaEventDestroy(h->gevent);
@@ -472,17 +704,8 @@ int shd_energy_grad(shd_ctx* h, const double* pos_hi, const double* pos_lo, doub
     if (!h) return SHD_EINVAL;
     if (!pos_hi || !pos_lo || !phi) return fail(h, SHD_EINVAL, "NULL pointer");
     if ((grad_hi == nullptr) != (grad_lo == nullptr)) return fail(h, SHD_EINVAL, "grad_hi and grad_lo must both be given or both NULL");
-    const bool want_grad = grad_hi != nullptr;
-    int rc = run_rho(h, pos_hi, pos_lo, want_grad);
+    int rc = run_eval(h, pos_hi, pos_lo, grad_hi, grad_lo);
     if (rc) return rc;
-    if (want_grad) {
-        CU(shd_launch_ctable(h));
-        if ((rc = mark(h, 4))) return rc;
-        CU(shd_launch_grad(h, grad_hi, grad_lo));
-        if ((rc = mark(h, 5))) return rc;
-    }
-    if ((rc = fetch_scalars(h))) return rc;
-    if ((rc = collect_timing(h))) return rc;
     phi[0] = h->h_scal->phi[0];
     phi[1] = h->h_scal->phi[1];
     if (h->h_scal->nonfinite) return fail(h, SHD_ENAN, "non-finite Phi (non-finite positions?)");
@@ -495,20 +718,20 @@ int shd_energy_grad_host(shd_ctx* h, const double* pos_hi, const double* pos_lo,
     if (!pos_hi || !pos_lo || !phi) return fail(h, SHD_EINVAL, "NULL pointer");
     if ((grad_hi == nullptr) != (grad_lo == nullptr)) return fail(h, SHD_EINVAL, "grad_hi and grad_lo must both be given or both NULL");
     const size_t n = (size_t)h->d * h->N, b = n * sizeof(double);
-    if (!h->d_hpos) {
-        CU(cudaMalloc((void**)&h->d_hpos, 2 * b));
-        CU(cudaMalloc((void**)&h->d_hgrad, 2 * b));
+    if (!h->d_hpos) {                       // one allocation: positions (hi, lo) and gradient (hi, lo)
+        CU(cudaMalloc((void**)&h->d_hpos, 4 * b));
         h->workspace_bytes += 4 * b;
     }
+    double* d_hgrad = h->d_hpos + 2 * n;
     CU(cudaMemcpyAsync(h->d_hpos, pos_hi, b, cudaMemcpyHostToDevice, h->stream));
     CU(cudaMemcpyAsync(h->d_hpos + n, pos_lo, b, cudaMemcpyHostToDevice, h->stream));
     const bool want_grad = grad_hi != nullptr;
-    int rc = shd_energy_grad(h, h->d_hpos, h->d_hpos + n, phi, want_grad ? h->d_hgrad : nullptr,
-                             want_grad ? h->d_hgrad + n : nullptr);
+    int rc = shd_energy_grad(h, h->d_hpos, h->d_hpos + n, phi, want_grad ? d_hgrad : nullptr,
+                             want_grad ? d_hgrad + n : nullptr);
     if (rc) return rc;
     if (want_grad) {
-        CU(cudaMemcpyAsync(grad_hi, h->d_hgrad, b, cudaMemcpyDeviceToHost, h->stream));
-        CU(cudaMemcpyAsync(grad_lo, h->d_hgrad + n, b, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaMemcpyAsync(grad_hi, d_hgrad, b, cudaMemcpyDeviceToHost, h->stream));
+        CU(cudaMemcpyAsync(grad_lo, d_hgrad + n, b, cudaMemcpyDeviceToHost, h->stream));
         CU(cudaStreamSynchronize(h->stream));
     }
     return SHD_OK;
@@ -525,10 +748,8 @@ int shd_set_timing(shd_ctx* h, int on) {
 int shd_smax(shd_ctx* h, const double* pos_hi, const double* pos_lo, double smax[2], long* argmax_k) {
     if (!h) return SHD_EINVAL;
     if (!pos_hi || !pos_lo || !smax) return fail(h, SHD_EINVAL, "NULL pointer");
-    int rc = run_rho(h, pos_hi, pos_lo, false);
+    int rc = run_eval(h, pos_hi, pos_lo, nullptr, nullptr);
     if (rc) return rc;
-    if ((rc = fetch_scalars(h))) return rc;
-    if ((rc = collect_timing(h))) return rc;
     smax[0] = h->h_scal->smax[0];
     smax[1] = h->h_scal->smax[1];
     if (argmax_k) *argmax_k = (long)h->h_scal->argmax;
@@ -565,129 +786,83 @@ int shd_set_precision(shd_ctx* h, int limbs) {
     return SHD_OK;
 }
 
-// engine 1: build the tile list, the particle splits and the digit tables of the INT8 rho pass (k_rho8.cu)
 int shd_set_engine(shd_ctx* h, int rho_engine) {
     if (!h) return SHD_EINVAL;
-    if (rho_engine < 0 || rho_engine > 2) return fail(h, SHD_EINVAL, "shd_set_engine: engine must be 0, 1 or 2");
+    if (rho_engine == -1) {                      // back to the library's own choice
+        const int before = h->rho_engine;
+        auto_engine(h);
+        if (h->rho_engine != before) h->tables_valid = false;
+        return SHD_OK;
+    }
+    if (rho_engine < 0 || rho_engine > 2) return fail(h, SHD_EINVAL, "shd_set_engine: engine must be -1 (auto), 0, 1 or 2");
     // exactness of the s32 digit sums of the gradient pass: 13 pairs x 2 Qpad products x 2^14 must stay below 2^31
     if (rho_engine == 2 && (long)h->Qpad * 2 * SHD_I8_DIGITS * 16384 >= (1L << 31))
         return fail(h, SHD_EINVAL, "shd_set_engine: last-axis table too long for the INT8 gradient pass (Qn <= 5024)");
-    if (rho_engine == 2 && !h->d_Bg8) {
-        // ---- INT8 gradient pass: step list over blocks of 8 p (K-steps of 16 q up to the block's last valid cell)
-        h->npb8 = (h->P + 7) / 8;
-        h->nkq8 = h->Qpad / 16;
-        h->njb128 = (h->N + 127) / 128;
-        std::vector<int> kp((size_t)h->npb * 32 * h->Qpad), km(kp.size());
-        CU(cudaMemcpy(kp.data(), h->d_cell_kp, kp.size() * sizeof(int), cudaMemcpyDeviceToHost));
-        CU(cudaMemcpy(km.data(), h->d_cell_km, km.size() * sizeof(int), cudaMemcpyDeviceToHost));
-        std::vector<int> steps;
-        for (int pb = 0; pb < h->npb8; pb++) {
-            int nk = 0;
-            for (int pi = 0; pi < 8; pi++) {
-                const int p = pb * 8 + pi;
-                if (p >= h->npb * 32) continue;
-                for (int q = 0; q < h->Qpad; q++)
-                    if (kp[(size_t)p * h->Qpad + q] >= 0 || km[(size_t)p * h->Qpad + q] >= 0) nk = std::max(nk, q / 16 + 1);
-            }
-            for (int k = 0; k < nk; k++) {
-                steps.push_back(pb * h->nkq8 + k);
-                steps.push_back(k | ((k == nk - 1 ? 1 : 0) << 16));
-            }
-        }
-        h->nsteps8 = (int)steps.size() / 2;
-        cudaDeviceProp prop;
-        int dev = 0;
-        cudaGetDevice(&dev);
-        CU(cudaGetDeviceProperties(&prop, dev));
-        const long sms = prop.multiProcessorCount;
-        double best = -1.0;
-        h->nseg8 = 1;
-        // at least two segments: the CTAs of one particle block then stream the same digit slabs side by side (L2)
-        for (int ns = std::min(2, h->nsteps8); ns <= std::min(32, h->nsteps8); ns++) {
-            const long waves = (h->njb128 * ns + sms - 1) / sms;
-            const double cost = (double)waves * ((double)((h->nsteps8 + ns - 1) / ns) + 6.0);
-            if (best < 0.0 || cost < best) { best = cost; h->nseg8 = ns; }
-        }
-        const size_t g8 = (size_t)h->njb128 * h->nkq8 * SHD_I8_DIGITS * 4096;
-        const size_t w8 = (size_t)h->npb8 * h->nkq8 * SHD_I8_DIGITS * 1024;
-        const size_t af = (size_t)h->npb8 * 8 * (size_t)h->njb128 * 128 * 32;
-        CU(cudaMalloc(&h->d_Afix, af));
-        CU(cudaMemset(h->d_Afix, 0, af));
-        h->workspace_bytes += af;
-        CU(cudaMalloc((void**)&h->d_Bg8, g8));
-        CU(cudaMemset(h->d_Bg8, 0, g8));
-        CU(cudaMalloc((void**)&h->d_W8, w8));
-        CU(cudaMemset(h->d_W8, 0, w8));
-        h->workspace_bytes += g8 + w8;
-        int rc;
-        if ((rc = upload(h, &h->d_steps8, steps))) return rc;
-        const size_t need = (size_t)4 * h->nseg8 * h->d * h->N * 2;      // four partials per segment (k_grad8.cu)
-        if (need > h->gpart_doubles) {
-            cudaFree(h->d_gpart);
-            h->d_gpart = nullptr;
-            if ((rc = dalloc_zero(h, &h->d_gpart, need))) return rc;
-            h->gpart_doubles = need;
-        }
-        CU(shd_grad8_configure());
+    if (rho_engine >= 1) {
+        int rc = plan_engine8(h, rho_engine);    // the handle's engine is unchanged when this fails
+        if (rc) return rc;
     }
-    if (rho_engine >= 1 && !h->d_A8) {
-        h->npb64 = (h->P + SHD_I8_PT - 1) / SHD_I8_PT;
-        h->nqb16 = (h->Qn + SHD_I8_QT - 1) / SHD_I8_QT;
-        std::vector<int> kp((size_t)h->npb * 32 * h->Qpad), km(kp.size());
-        CU(cudaMemcpy(kp.data(), h->d_cell_kp, kp.size() * sizeof(int), cudaMemcpyDeviceToHost));
-        CU(cudaMemcpy(km.data(), h->d_cell_km, km.size() * sizeof(int), cudaMemcpyDeviceToHost));
-        std::vector<int> tpb, tqb;
-        for (int pb = 0; pb < h->npb64; pb++)
-            for (int qb = 0; qb < h->nqb16; qb++) {
-                bool any = false;
-                for (int pi = 0; pi < SHD_I8_PT && !any; pi++)
-                    for (int qi = 0; qi < SHD_I8_QT && !any; qi++) {
-                        const int p = pb * SHD_I8_PT + pi, q = qb * SHD_I8_QT + qi;
-                        if (p < h->npb * 32 && q < h->Qpad) any = kp[(size_t)p * h->Qpad + q] >= 0 || km[(size_t)p * h->Qpad + q] >= 0;
-                    }
-                if (any) { tpb.push_back(pb); tqb.push_back(qb); }
-            }
-        h->ntiles8 = (int)tpb.size();
-        // particle splits: at most SHD_I8_MAXN particles per CTA (exact s32 sums); minimise waves x (K-steps + epilogue)
-        cudaDeviceProp prop;
-        int dev = 0;
-        cudaGetDevice(&dev);
-        CU(cudaGetDeviceProperties(&prop, dev));
-        const long sms = prop.multiProcessorCount, nk = (h->N + 31) / 32;
-        double best = -1.0;
-        for (long ns = (h->N + SHD_I8_MAXN - 1) / SHD_I8_MAXN; ns <= std::min<long>(512, nk); ns++) {
-            const long per = (nk + ns - 1) / ns, waves = ((long)h->ntiles8 * ns + sms - 1) / sms;
-            const double cost = (double)waves * ((double)per + 8.0) + 0.004 * (double)ns * h->ntiles8;
-            if (best < 0.0 || cost < best) { best = cost; h->nsplit8 = (int)ns; h->ksteps8 = (int)per; }
-        }
-        h->nk8 = (long)h->nsplit8 * h->ksteps8;
-        const size_t a8 = (size_t)h->npb64 * h->nk8 * SHD_I8_DIGITS * (SHD_I8_PT * 2 * 32);
-        const size_t b8 = (size_t)h->nqb16 * h->nk8 * SHD_I8_DIGITS * (SHD_I8_QT * 2 * 32);
-        CU(cudaMalloc((void**)&h->d_A8, a8));
-        CU(cudaMalloc((void**)&h->d_B8, b8));
-        CU(cudaMemset(h->d_A8, 0, a8));
-        CU(cudaMemset(h->d_B8, 0, b8));
-        h->workspace_bytes += a8 + b8;
-        int rc;
-        if ((rc = upload(h, &h->d_tile8_pb, tpb))) return rc;
-        if ((rc = upload(h, &h->d_tile8_qb, tqb))) return rc;
-        const size_t need = (size_t)h->nsplit8 * h->ntiles8 * 4 * 1024 * 2;
-        if (need > h->part_doubles) {
-            cudaFree(h->d_part);
-            h->d_part = nullptr;
-            if ((rc = dalloc_zero(h, &h->d_part, need))) return rc;
-            h->part_doubles = need;
-        }
-        const int nb = (int)(((long)std::max(h->ntiles, h->ntiles8) * 1024 + 255) / 256);
-        if (nb > h->nfinish_blocks) {
-            cudaFree(h->d_blockred);
-            h->d_blockred = nullptr;
-            if ((rc = dalloc_zero(h, &h->d_blockred, (size_t)nb * 8))) return rc;
-            h->nfinish_blocks = nb;
-        }
-        CU(shd_rho8_configure());
-    }
+    if (rho_engine != h->rho_engine) h->tables_valid = false;
     h->rho_engine = rho_engine;
+    h->engine_auto = 0;
+    return SHD_OK;
+}
+
+int shd_set_workspace(shd_ctx* h, size_t bytes) {
+    if (!h) return SHD_EINVAL;
+    h->ws_cap = bytes;
+    h->tables_valid = false;
+    return SHD_OK;
+}
+
+int shd_set_shard(shd_ctx* h, long N_total, int rank, int world) {
+    if (!h) return SHD_EINVAL;
+    if (world < 1 || rank < 0 || rank >= world || N_total < h->N) return fail(h, SHD_EINVAL, "shd_set_shard: bad rank / world / N_total");
+    h->Nsys = N_total;
+    h->rank = rank;
+    h->world = world;
+    h->tables_valid = false;
+    return SHD_OK;
+}
+
+unsigned long shd_partial_bytes(const shd_ctx* h) {
+    if (!h) return 0;
+    return (unsigned long)(h->rho_engine >= 1 ? h->ntiles8 : h->ntiles) * 4 * 1024 * 16;
+}
+
+int shd_rho_partial(shd_ctx* h, const double* pos_hi, const double* pos_lo, void* partial_out) {
+    if (!h) return SHD_EINVAL;
+    if (!pos_hi || !pos_lo || !partial_out) return fail(h, SHD_EINVAL, "NULL pointer");
+    if (!shd_sharded(h)) return fail(h, SHD_EINVAL, "shd_rho_partial: the handle is not a shard (shd_set_shard)");
+    int rc = shd_prepare_tables(h, false);
+    if (rc) return rc;
+    h->last_launches = 0;
+    CU(shd_enqueue_rho_partial(h, pos_hi, pos_lo, false));
+    CU(cudaMemcpyAsync(partial_out, h->d_xrun, shd_partial_bytes(h), cudaMemcpyDeviceToDevice, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return SHD_OK;
+}
+
+int shd_rho_finish(shd_ctx* h, const void* gathered, int nparts, double phi[2]) {
+    if (!h) return SHD_EINVAL;
+    if (!gathered || nparts < 1 || !phi) return fail(h, SHD_EINVAL, "shd_rho_finish: bad argument");
+    if (!h->tables_valid) return fail(h, SHD_EINVAL, "shd_rho_finish: call shd_rho_partial first");
+    CU(shd_enqueue_rho_finish(h, (const double*)gathered, nparts));
+    int rc = fetch_scalars(h);
+    if (rc) return rc;
+    phi[0] = h->h_scal->phi[0];
+    phi[1] = h->h_scal->phi[1];
+    if (h->h_scal->nonfinite) return fail(h, SHD_ENAN, "non-finite Phi (non-finite positions?)");
+    return SHD_OK;
+}
+
+int shd_grad_local(shd_ctx* h, const double* pos_hi, const double* pos_lo, double* grad_hi, double* grad_lo) {
+    if (!h) return SHD_EINVAL;
+    if (!pos_hi || !pos_lo || !grad_hi || !grad_lo) return fail(h, SHD_EINVAL, "NULL pointer");
+    int rc = shd_prepare_tables(h, true);
+    if (rc) return rc;
+    CU(shd_enqueue_grad(h, pos_hi, pos_lo, grad_hi, grad_lo));
+    CU(cudaStreamSynchronize(h->stream));
     return SHD_OK;
 }
 
@@ -711,8 +886,8 @@ double shd_stat(const shd_ctx* h, int what) {
     if (!h) return 0.0;
     const double cells_rho = (double)h->ntiles * 1024.0;
     switch (what) {
-        case 0: return cells_rho * (double)h->Npad * 24.0;     // DFMAs launched by the rho pass (padded, 3 limbs)
-        case 12: return (double)h->njb64 * SHD_JT * (double)h->grad_qsteps * SHD_PG * 48.0;   // ... by the gradient pass
+        case 0: return cells_rho * (double)h->nsplit * h->chunks_per_split * SHD_NPS * 24.0;   // DFMAs launched by the rho pass (padded, 3 limbs)
+        case 12: return (double)((h->N + SHD_JT - 1) / SHD_JT) * SHD_JT * (double)h->grad_qsteps * SHD_PG * 48.0;   // ... by the gradient pass
         case 1: return (double)h->last_launches;
         case 2: return cells_rho;
         case 3: return (double)h->valid_cells;
@@ -730,6 +905,10 @@ double shd_stat(const shd_ctx* h, int what) {
         case 16: return (double)h->rho_engine;
         case 17: return (double)h->nseg8;
         case 18: return (double)h->nsteps8;
+        case 19: return (double)h->nchunk;
+        case 25: return (double)h->Nc;
+        case 26: return (double)h->table_bytes;
+        case 27: return (double)h->engine_auto;
         case 20: case 21: case 22: case 23: case 24: return (double)h->kern_ms[what - 20];
         default: return 0.0;
     }

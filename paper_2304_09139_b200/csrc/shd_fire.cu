@@ -36,6 +36,7 @@ struct shd_firestate {
     int nblk = 0;
     double *v = nullptr, *g = nullptr;     // [2][n] (hi plane, lo plane)
     double *partial = nullptr;             // [nblk][3][2]
+    double *rank_part = nullptr, *rank_all = nullptr;   // sharded: [3][2] and [world][3][2]
     shd_firectrl *d_ctrl = nullptr, *h_ctrl = nullptr;
 };
 
@@ -83,6 +84,25 @@ __global__ void __launch_bounds__(FIRE_THREADS) k_fire_dots(
         for (int k = 0; k < FIRE_THREADS / 32; k++) s = dd_add(s, dd{red[k][threadIdx.x][0], red[k][threadIdx.x][1]});
         double* o = partial + ((size_t)blockIdx.x * 3 + threadIdx.x) * 2;
         o[0] = s.h; o[1] = s.l;
+    }
+}
+
+// this rank's three sums over its blocks, in the tree k_fire_control uses (lane l adds blocks l, l+32, ...; butterfly),
+// so that one rank gives exactly the unsharded result
+__global__ void __launch_bounds__(32) k_fire_rank_sum(int nblk, const shd_firectrl* __restrict__ c, const double* __restrict__ partial,
+                                                      double* __restrict__ out)
+{
+    if (c->done) return;
+    const int lane = threadIdx.x;
+#pragma unroll
+    for (int r = 0; r < 3; r++) {
+        dd s{0.0, 0.0};
+        for (int k = lane; k < nblk; k += 32) {
+            const double* o = partial + ((size_t)k * 3 + r) * 2;
+            s = dd_add(s, dd{o[0], o[1]});
+        }
+        s = warp_sum(s);
+        if (lane == 0) { out[2 * r] = s.h; out[2 * r + 1] = s.l; }
     }
 }
 
@@ -177,6 +197,10 @@ int fire_alloc(shd_ctx* h) {
     CUF(cudaMalloc((void**)&s->v, v));
     CUF(cudaMalloc((void**)&s->g, v));
     CUF(cudaMalloc((void**)&s->partial, (size_t)s->nblk * 3 * 2 * sizeof(double)));
+    if (shd_sharded(h)) {
+        CUF(cudaMalloc((void**)&s->rank_part, 3 * 2 * sizeof(double)));
+        CUF(cudaMalloc((void**)&s->rank_all, (size_t)h->world * 3 * 2 * sizeof(double)));
+    }
     CUF(cudaMalloc((void**)&s->d_ctrl, sizeof(shd_firectrl)));
     CUF(cudaMallocHost((void**)&s->h_ctrl, sizeof(shd_firectrl)));
     std::memset(s->h_ctrl, 0, sizeof(shd_firectrl));
@@ -189,7 +213,7 @@ int fire_alloc(shd_ctx* h) {
 void shd_fire_free(shd_ctx* h) {
     shd_firestate* s = h->fire;
     if (!s) return;
-    cudaFree(s->v); cudaFree(s->g); cudaFree(s->partial); cudaFree(s->d_ctrl);
+    cudaFree(s->v); cudaFree(s->g); cudaFree(s->partial); cudaFree(s->d_ctrl); cudaFree(s->rank_part); cudaFree(s->rank_all);
     if (s->h_ctrl) cudaFreeHost(s->h_ctrl);
     delete s;
     h->fire = nullptr;
@@ -214,7 +238,7 @@ int shd_fire_run(shd_ctx* h, double* pos_hi, double* pos_lo, const shd_min_opts*
     double vmax = 1.0;
     for (double x : h->v) vmax = x > vmax ? x : vmax;
     const double kmax = 2.0 * 3.14159265358979323846 * std::sqrt((double)h->m_star) / h->L;
-    const double dt0 = opts->fire_dt0 > 0.0 ? opts->fire_dt0 : 0.1 / (kmax * std::sqrt(2.0 * (double)h->N * vmax));
+    const double dt0 = opts->fire_dt0 > 0.0 ? opts->fire_dt0 : 0.1 / (kmax * std::sqrt(2.0 * (double)h->Nsys * vmax));
     shd_firectrl* c = s->h_ctrl;
     if (cont) {                        // explicit re-entry: keep velocities, dt, alpha, counters
         const shd_firectrl keep = *c;
@@ -235,13 +259,14 @@ int shd_fire_run(shd_ctx* h, double* pos_hi, double* pos_lo, const shd_min_opts*
         cudaError_t e;
         cudaStream_t q = h->stream;          // the capture stream while shd_run_slots is recording
         h->last_launches = 0;
-        if ((e = shd_launch_tables(h, pos_hi, pos_lo, true)) != cudaSuccess) return e;
-        if ((e = shd_launch_rho(h)) != cudaSuccess) return e;
-        if ((e = shd_launch_finish(h)) != cudaSuccess) return e;
-        if ((e = shd_launch_ctable(h)) != cudaSuccess) return e;
-        if ((e = shd_launch_grad(h, s->g, s->g + n)) != cudaSuccess) return e;
+        if ((e = shd_enqueue_eval(h, pos_hi, pos_lo, s->g, s->g + n)) != cudaSuccess) return e;
         k_fire_dots<<<s->nblk, FIRE_THREADS, 0, q>>>(n, s->d_ctrl, s->g, s->v, s->partial);
-        k_fire_control<<<1, 32, 0, q>>>(s->nblk, s->d_ctrl, h->d_scal, s->partial);
+        if (shd_sharded(h)) {          // sharded vectors: rank sums, all-gathered as bytes, added in rank order (shd_min.cu)
+            k_fire_rank_sum<<<1, 32, 0, q>>>(s->nblk, s->d_ctrl, s->partial, s->rank_part);
+            if ((e = shd_comm_allgather(h, s->rank_part, s->rank_all, 3 * 16)) != cudaSuccess) return e;
+            k_fire_control<<<1, 32, 0, q>>>(h->world, s->d_ctrl, h->d_scal, s->rank_all);
+        } else
+            k_fire_control<<<1, 32, 0, q>>>(s->nblk, s->d_ctrl, h->d_scal, s->partial);
         k_fire_update<<<ublk, FIRE_THREADS, 0, q>>>(n, s->d_ctrl, pos_hi, pos_lo, s->g, s->v);
         h->last_launches += 3;
         return cudaGetLastError();

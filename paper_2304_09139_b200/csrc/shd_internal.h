@@ -69,9 +69,31 @@ struct shd_scalars {
 struct shd_minstate;      // L-BFGS workspace (shd_min.cu)
 struct shd_firestate;     // FIRE workspace (shd_fire.cu)
 
+struct shd_comm;          // NCCL plumbing of a sharded handle (shd_comm.cu)
+
 struct shd_ctx {
     int d = 0;
-    long N = 0;
+    long N = 0;                // particles this handle evaluates (its shard of the system)
+    long Nsys = 0;             // particles of the whole system (= N unless sharded, shd_set_shard): S_max = max |rho|^2 / Nsys
+    int rank = 0, world = 1;   // position of the shard
+    // Bounded workspace: the per-particle tables hold one CHUNK of particles = spc whole splits of the rho pass, so the
+    // reduction tree (left fold over the splits, k_finish1) is the same for every chunk size: results are bit-identical.
+    long unit = 0;             // particles per split of the current engine's rho pass
+    int spc = 0;               // splits per chunk
+    int nchunk = 1;            // chunks per evaluation
+    long Nc = 0;               // particles per chunk = spc * unit
+    size_t ws_cap = 0;         // cap on the per-particle tables in bytes (shd_set_workspace); 0 = what the device has free
+    bool tables_valid = false; // device tables allocated for the current (engine, chunk) setting
+    int engine_auto = 1;       // engine chosen by the library (shd_create*) rather than by shd_set_engine
+    double *d_xrun = nullptr;  // running sums of the fold over chunks / the shard's partial: [ntiles][4][1024] (hi, lo)
+    double *d_xall = nullptr;  // sharded: the ranks' partials gathered in rank order [world][ntiles][4][1024] (hi, lo)
+    shd_comm *comm = nullptr;
+    bool grad_tables_ready = false;   // one chunk: the table build of the rho pass also wrote the gradient pass's tables
+    size_t table_bytes = 0;           // bytes held by the tables of the current (engine, chunk) setting
+    void (*timing_mark)(shd_ctx*, int) = nullptr;   // set around a timed evaluation (shd_set_timing)
+    std::vector<int> cell_kp, cell_km;              // host copies of the (p, q) -> k maps
+    int *d_shell = nullptr;           // radial shells of shd_structure_factor_shells (k_finish.cu)
+    void *d_trace = nullptr;          // device trace ring of the minimizers (shd_min.cu)
     double L = 0;
     long m_star = 0;
     long M = 0;
@@ -81,12 +103,12 @@ struct shd_ctx {
     int P = 0, Qn = 0, npb = 0, nqb = 0;
     int S1d = 0;               // d == 1: n = S1d * p + sigma q
     int qscale_log2 = 0;       // q * B is stored as q * B * 2^-qscale_log2
-    long Npad = 0;             // particles padded to nsplit * chunks_per_split * NPS
+    long Npad = 0;             // particle slots of the FP64 engine's tables (one chunk): spc * chunks_per_split * NPS
     int nsplit = 0;
     long chunks_per_split = 0;
     int ntiles = 0;
     long njb = 0;              // ceil(N / 32)
-    long njb64 = 0;            // ceil(N / 64): particle blocks of the gradient pass
+    long njb64 = 0;            // ceil(Nc / 64): particle blocks of the gradient pass in one chunk
     int npb16 = 0;             // ceil(P / 16): p-blocks of the gradient pass
     int nsteps = 0;            // gradient pass: steps (16 p x 4 q) in the step list
     int nseg = 0;              // gradient pass: equal segments of the step list (work units per particle block)
@@ -118,7 +140,7 @@ struct shd_ctx {
     signed char *d_B8 = nullptr;   // [nqb16][nk8][13 digits][ 32 rows (q, re/im) x 32 particles]
     int *d_tile8_pb = nullptr, *d_tile8_qb = nullptr;
     int ntiles8 = 0, nsplit8 = 0, ksteps8 = 0, npb64 = 0, nqb16 = 0;
-    long nk8 = 0;                  // nsplit8 * ksteps8: K-steps (32 particles) in the digit tables
+    long nk8 = 0;                  // spc * ksteps8: K-steps (32 particles) in the digit tables (one chunk)
     size_t part_doubles = 0;       // capacity of d_part
     // INT8 gradient pass (shd_set_engine(h, 2))
     signed char *d_Bg8 = nullptr;  // [njb128][nkq8][13][128 rows (particle) x 32 K (q%16, re/im)]
@@ -149,26 +171,36 @@ struct shd_ctx {
     cudaEvent_t ev[SHD_NKERN + 1] = {};
     bool ev_used[SHD_NKERN + 1] = {};
     float kern_ms[SHD_NKERN] = {};
-    // staging buffers of shd_energy_grad_host (device)
-    double *d_hpos = nullptr, *d_hgrad = nullptr;
+    // staging buffer of shd_energy_grad_host (device): positions (hi, lo) then gradient (hi, lo)
+    double *d_hpos = nullptr;
 };
 
 // kernels / launchers (each returns the cudaError of its launches)
-cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool with_grad_tables);
-cudaError_t shd_launch_rho(shd_ctx* h);
-cudaError_t shd_launch_rho8(shd_ctx* h);
+cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* pos_lo, long j_first, int what);
+cudaError_t shd_launch_rho(shd_ctx* h, int nsplits);      // the rho pass over nsplits splits of the chunk in the tables
+cudaError_t shd_launch_rho8(shd_ctx* h, int nsplits);
 cudaError_t shd_rho8_configure();
 cudaError_t shd_grad8_configure();
-cudaError_t shd_launch_grad8_main(shd_ctx* h);
-cudaError_t shd_launch_finish(shd_ctx* h);
+cudaError_t shd_launch_grad8_main(shd_ctx* h, long nc);
+cudaError_t shd_launch_fold(shd_ctx* h, const double* part, int nparts, const double* xin, double* xout, bool fin);
 cudaError_t shd_launch_ctable(shd_ctx* h);
 cudaError_t shd_launch_sfactor(shd_ctx* h, double* S_out, double* scratch, double* tau2);
-cudaError_t shd_launch_grad(shd_ctx* h, double* grad_hi, double* grad_lo);
+cudaError_t shd_launch_grad(shd_ctx* h, long j_first, long nc, double* grad_hi, double* grad_lo);
 cudaError_t shd_tables_configure();
 cudaError_t shd_rho_configure();
 cudaError_t shd_grad_configure();
 
-int shd_prepare_tables(shd_ctx* h, bool with_grad);   // shd_api.cu
+// a shard exchanges its partial sums: more than one rank, or a communicator of one rank (the same calls on one GPU)
+inline bool shd_sharded(const shd_ctx* h) { return h->world > 1 || h->comm != nullptr; }
+int shd_prepare_tables(shd_ctx* h, bool with_grad);   // shd_api.cu: allocate what the current setting needs (outside any capture)
+// the whole evaluation (steps a1-a4) enqueued on h->stream, chunk by chunk; grad_hi == NULL: rho pass and reduction only
+cudaError_t shd_enqueue_eval(shd_ctx* h, const double* pos_hi, const double* pos_lo, double* grad_hi, double* grad_lo);
+cudaError_t shd_enqueue_rho_partial(shd_ctx* h, const double* pos_hi, const double* pos_lo, bool grad_tables_too);   // -> d_xrun (or rho when not sharded)
+cudaError_t shd_enqueue_rho_finish(shd_ctx* h, const double* gathered, int nparts);
+cudaError_t shd_enqueue_grad(shd_ctx* h, const double* pos_hi, const double* pos_lo, double* grad_hi, double* grad_lo);
+// NCCL plumbing (shd_comm.cu): all-gather of `bytes` bytes per rank on h->stream, fixed rank order
+cudaError_t shd_comm_allgather(shd_ctx* h, const void* send, void* recv, size_t bytes);
+void shd_comm_free(shd_ctx* h);
 // minimizers (shd_min.cu, shd_fire.cu)
 void shd_min_free(shd_ctx* h);
 void shd_fire_free(shd_ctx* h);

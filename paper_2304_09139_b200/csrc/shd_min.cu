@@ -45,6 +45,7 @@ struct shd_minstate {
     double *x = nullptr, *g = nullptr, *gt = nullptr, *p = nullptr;   // [2][n] (hi plane, lo plane)
     double *S = nullptr, *Y = nullptr;                                 // [m+1][2][n]
     double *partial = nullptr;                                         // [nblk][NB][3][2]
+    double *rank_part = nullptr, *rank_all = nullptr;                  // sharded: [NB][3][2] and [world][NB][3][2]
     double *G = nullptr;                                               // [MIN_NBS][MIN_NBS][2]
     shd_minctrl *d_ctrl = nullptr, *h_ctrl = nullptr;
 };
@@ -120,6 +121,19 @@ __global__ void __launch_bounds__(MIN_THREADS) k_min_dots(
             o[0] = s.h; o[1] = s.l;
         }
     }
+}
+
+// out[q] = sum over this rank's blocks of partial[block][q] (dd, fixed order); nq quantities of (hi, lo)
+__global__ void __launch_bounds__(64) k_rank_sum(int nblk, int nq, const double* __restrict__ partial, double* __restrict__ out,
+                                                 const int* __restrict__ done)
+{
+    if (*done) return;
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= nq) return;
+    dd s{0.0, 0.0};
+    for (int k = 0; k < nblk; k++) s = dd_add(s, dd{partial[((size_t)k * nq + q) * 2], partial[((size_t)k * nq + q) * 2 + 1]});
+    out[2 * q] = s.h;
+    out[2 * q + 1] = s.l;
 }
 
 // sum_l delta[l] * G[l][c] over the basis, lanes in parallel, identical result in every lane
@@ -361,6 +375,10 @@ int min_alloc(shd_ctx* h, int m) {
     CUM(cudaMalloc((void**)&s->S, v * (m + 1))); CUM(cudaMalloc((void**)&s->Y, v * (m + 1)));
     CUM(cudaMalloc((void**)&s->partial, (size_t)s->nblk * NB * 3 * 2 * sizeof(double)));
     CUM(cudaMalloc((void**)&s->G, (size_t)MIN_NBS * MIN_NBS * 2 * sizeof(double)));
+    if (shd_sharded(h)) {
+        CUM(cudaMalloc((void**)&s->rank_part, NB * 3 * 2 * sizeof(double)));
+        CUM(cudaMalloc((void**)&s->rank_all, (size_t)h->world * NB * 3 * 2 * sizeof(double)));
+    }
     CUM(cudaMalloc((void**)&s->d_ctrl, sizeof(shd_minctrl)));
     CUM(cudaMallocHost((void**)&s->h_ctrl, sizeof(shd_minctrl)));
     std::memset(s->h_ctrl, 0, sizeof(shd_minctrl));
@@ -374,7 +392,7 @@ void shd_min_free(shd_ctx* h) {
     shd_minstate* s = h->min;
     if (!s) return;
     cudaFree(s->x); cudaFree(s->g); cudaFree(s->gt); cudaFree(s->p); cudaFree(s->S); cudaFree(s->Y);
-    cudaFree(s->partial); cudaFree(s->G); cudaFree(s->d_ctrl);
+    cudaFree(s->partial); cudaFree(s->G); cudaFree(s->d_ctrl); cudaFree(s->rank_part); cudaFree(s->rank_all);
     if (s->h_ctrl) cudaFreeHost(s->h_ctrl);
     delete s;
     h->min = nullptr;
@@ -416,14 +434,18 @@ extern "C" int shd_minimize(shd_ctx* h, double* pos_hi, double* pos_lo, const sh
         cudaError_t e;
         cudaStream_t q = h->stream;          // the capture stream while shd_run_slots is recording
         h->last_launches = 0;
-        if ((e = shd_launch_tables(h, pos_hi, pos_lo, true)) != cudaSuccess) return e;
-        if ((e = shd_launch_rho(h)) != cudaSuccess) return e;
-        if ((e = shd_launch_finish(h)) != cudaSuccess) return e;
-        if ((e = shd_launch_ctable(h)) != cudaSuccess) return e;
-        if ((e = shd_launch_grad(h, s->gt, s->gt + n)) != cudaSuccess) return e;
+        if ((e = shd_enqueue_eval(h, pos_hi, pos_lo, s->gt, s->gt + n)) != cudaSuccess) return e;
         k_min_dots<<<s->nblk, MIN_THREADS, 0, q>>>(n, m, s->d_ctrl, pos_hi, pos_lo, s->x, s->gt, s->g,
                                                    s->S, s->Y, s->partial);
-        k_min_control<<<1, MIN_THREADS, 0, q>>>(s->nblk, s->d_ctrl, h->d_scal, s->partial, s->G);
+        if (shd_sharded(h)) {
+            // sharded vectors: this rank's sums of its block partials, all-gathered as bytes, added in rank order by
+            // k_min_control on every rank (identical decisions everywhere: Phi, S_max and the dots are bit-identical)
+            const int nq = 3 * (2 * (m + 1) + 1);
+            k_rank_sum<<<(nq + 63) / 64, 64, 0, q>>>(s->nblk, nq, s->partial, s->rank_part, &s->d_ctrl->done);
+            if ((e = shd_comm_allgather(h, s->rank_part, s->rank_all, (size_t)nq * 16)) != cudaSuccess) return e;
+            k_min_control<<<1, MIN_THREADS, 0, q>>>(h->world, s->d_ctrl, h->d_scal, s->rank_all, s->G);
+        } else
+            k_min_control<<<1, MIN_THREADS, 0, q>>>(s->nblk, s->d_ctrl, h->d_scal, s->partial, s->G);
         k_min_update<<<ublk, MIN_THREADS, 0, q>>>(n, m, s->d_ctrl, pos_hi, pos_lo, s->x, s->gt, s->g,
                                                   s->p, s->S, s->Y);
         h->last_launches += 3;

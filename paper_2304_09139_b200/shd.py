@@ -17,7 +17,9 @@ LIB_PATH = _HERE / "libshd.so"
 SHD_OK, SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA, SHD_ENAN, SHD_ESTALL, SHD_EMAXEVAL = 0, -1, -2, -3, -4, -5, -6
 EXPORTS = ["shd_create", "shd_create_shell", "shd_create_table", "shd_destroy", "shd_set_stream", "shd_num_k", "shd_get_k",
            "shd_energy_grad", "shd_energy_grad_host", "shd_set_timing", "shd_smax", "shd_last_smax", "shd_get_rho", "shd_minimize",
-           "shd_last_error", "shd_stat", "shd_fp64_peak", "shd_structure_factor", "shd_set_precision", "shd_i8_probe", "shd_set_engine"]
+           "shd_last_error", "shd_stat", "shd_fp64_peak", "shd_structure_factor", "shd_set_precision", "shd_i8_probe", "shd_set_engine",
+           "shd_set_workspace", "shd_set_shard", "shd_comm_unique_id", "shd_comm_init", "shd_partial_bytes", "shd_rho_partial", "shd_rho_finish",
+           "shd_grad_local"]
 
 
 class ShdError(RuntimeError):
@@ -68,6 +70,15 @@ def _load():
     lib.shd_set_precision.argtypes = [vp, C.c_int]
     lib.shd_i8_probe.argtypes = [dp, C.POINTER(C.c_long)]
     lib.shd_set_engine.argtypes = [vp, C.c_int]
+    lib.shd_set_workspace.argtypes = [vp, C.c_ulong]
+    lib.shd_set_shard.argtypes = [vp, C.c_long, C.c_int, C.c_int]
+    lib.shd_comm_unique_id.argtypes = [vp]
+    lib.shd_comm_init.argtypes = [vp, vp]
+    lib.shd_partial_bytes.argtypes = [vp]
+    lib.shd_partial_bytes.restype = C.c_ulong
+    lib.shd_rho_partial.argtypes = [vp, vp, vp, vp]
+    lib.shd_rho_finish.argtypes = [vp, vp, C.c_int, dp]
+    lib.shd_grad_local.argtypes = [vp, vp, vp, vp, vp]
     return lib
 
 
@@ -196,8 +207,49 @@ class Shd:
         self._check(lib.shd_set_precision(self._h, int(limbs)))
 
     def set_engine(self, rho_engine: int):
-        """shd_set_engine: 0 = FP64 DMMA rho pass, 1 = INT8 tensor-core rho pass (tcgen05)."""
+        """shd_set_engine: 2 = both passes on the INT8 tensor cores (tcgen05), 1 = rho pass only, 0 = FP64 limbs (DMMA),
+        -1 = the library's own choice (what a fresh handle starts with)."""
         self._check(lib.shd_set_engine(self._h, int(rho_engine)))
+
+    @property
+    def engine(self) -> int:
+        return int(self.stat(16))
+
+    def set_workspace(self, nbytes: int):
+        """shd_set_workspace: cap on the per-particle tables; the evaluation then runs chunk by chunk (bit-identical)."""
+        self._check(lib.shd_set_workspace(self._h, int(nbytes)))
+
+    def set_shard(self, N_total: int, rank: int, world: int):
+        """shd_set_shard: this handle's N particles are shard `rank` of `world` of a system of N_total."""
+        self._check(lib.shd_set_shard(self._h, int(N_total), int(rank), int(world)))
+
+    def comm_init(self, id128: bytes):
+        """shd_comm_init (collective): the 128 bytes of comm_unique_id() from one rank."""
+        buf = C.create_string_buffer(bytes(id128), 128)
+        self._check(lib.shd_comm_init(self._h, C.cast(buf, C.c_void_p)))
+
+    def rho_partial(self, pos_hi, pos_lo, out=None):
+        """shd_rho_partial: this shard's running sums as a CUDA uint8 tensor of shd_partial_bytes bytes."""
+        torch = _torch()
+        ph, pl = self._pos(pos_hi, pos_lo)
+        if out is None:
+            out = torch.empty(int(lib.shd_partial_bytes(self._h)), dtype=torch.uint8, device="cuda")
+        self._check(lib.shd_rho_partial(self._h, ph, pl, C.c_void_p(out.data_ptr())))
+        return out
+
+    def rho_finish(self, gathered, nparts: int):
+        """shd_rho_finish: gathered = CUDA uint8 tensor holding nparts partials in rank order.  Returns (phi_hi, phi_lo)."""
+        phi = (C.c_double * 2)()
+        self._check(lib.shd_rho_finish(self._h, C.c_void_p(gathered.data_ptr()), int(nparts), phi))
+        return phi[0], phi[1]
+
+    def grad_local(self, pos_hi, pos_lo, grad_hi=None, grad_lo=None):
+        torch = _torch()
+        ph, pl = self._pos(pos_hi, pos_lo)
+        if grad_hi is None:
+            grad_hi, grad_lo = torch.empty_like(pos_hi), torch.empty_like(pos_hi)
+        self._check(lib.shd_grad_local(self._h, ph, pl, C.c_void_p(grad_hi.data_ptr()), C.c_void_p(grad_lo.data_ptr())))
+        return grad_hi, grad_lo
 
     def structure_factor(self, want_S=True):
         """shd_structure_factor on the last evaluation: (S device tensor or None, (hi, lo) of
@@ -248,6 +300,15 @@ def i8_probe():
     if rc != SHD_OK:
         raise ShdError(rc, "shd_i8_probe failed")
     return tops.value, bad.value
+
+
+def comm_unique_id() -> bytes:
+    """shd_comm_unique_id: 128 bytes naming a new NCCL communicator (call on one rank, broadcast to all)."""
+    buf = C.create_string_buffer(128)
+    rc = lib.shd_comm_unique_id(C.cast(buf, C.c_void_p))
+    if rc != SHD_OK:
+        raise ShdError(rc, "shd_comm_unique_id failed (NCCL not loadable?)")
+    return buf.raw
 
 
 def from_host(hi: np.ndarray, lo: np.ndarray):

@@ -7,9 +7,12 @@ ROOT = Path(__file__).resolve().parent.parent
 
 
 def declared():
-    text = (ROOT / "include" / "shd.h").read_text()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(shd_[a-z0-9_]+)\s*\(", text)))
+    names = set()
+    for header in ("shd.h", "shd_bench.h"):          # the hot-path boundary and the measurement tooling
+        text = (ROOT / "include" / header).read_text()
+        text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+        names |= set(re.findall(r"\b(shd_[a-z0-9_]+)\s*\(", text))
+    return sorted(names)
 
 
 def test_header_symbols_exported():

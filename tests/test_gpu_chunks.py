@@ -1,0 +1,167 @@
+"""Bounded workspace (shd_set_workspace) and particle sharding (shd_set_shard), SURVEY.md 8(e) / 8(f) NEXT-4.
+
+Chunked evaluation: the per-particle tables hold one chunk of particles, a whole number of the rho pass's particle
+splits, and the running sums continue the same left fold over the splits -- so every output word must be IDENTICAL to
+the single-chunk evaluation, whatever the cap.  Sharding: G handles evaluate G particle ranges (here in one process on
+one GPU: the ranks as successive launches, the all-gather as a concatenation), every rank must end with bit-identical
+rho / Phi / S_max, and the whole must agree with the oracle within BASELINE.json's tolerances.
+"""
+import numpy as np
+import pytest
+
+from paper_2304_09139_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def shd():
+    from paper_2304_09139_b200 import shd as m
+    return m
+
+
+def evaluate(h, shd, hi, lo):
+    th, tl = shd.from_host(hi, lo)
+    phi, gh, gl = h.energy_grad(th, tl)
+    rho = [t.cpu().numpy() for t in h.rho()]
+    return phi, gh.cpu().numpy(), gl.cpu().numpy(), rho, h.last_smax()
+
+
+@pytest.mark.parametrize("name,engine", [("cfg4", 2), ("cfg4", 0), ("cfg2", 2), ("cfg2", 1), ("cfg3", 0), ("cfg5", 2)])
+def test_chunked_is_bit_identical(shd, name, engine):
+    cfg = inputs.CONFIGS[name]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    lo = inputs.jitter_lo(hi, 3)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    h.set_engine(engine)
+    ref = evaluate(h, shd, hi, lo)
+    assert h.stat(19) == 1, "the reference evaluation must be a single chunk"
+    full = h.stat(26)                      # bytes of per-particle tables of the single-chunk evaluation
+    seen = set()
+    for frac in (0.55, 0.3, 0.12):
+        h.set_workspace(int(full * frac))
+        got = evaluate(h, shd, hi, lo)
+        nchunk = int(h.stat(19))
+        assert nchunk > 1, (frac, nchunk)
+        assert h.stat(26) <= full * frac
+        seen.add(nchunk)
+        assert got[0] == ref[0], "Phi"
+        assert got[4] == ref[4], "S_max / argmax"
+        assert np.array_equal(got[1], ref[1]) and np.array_equal(got[2], ref[2]), "gradient"
+        for a, b in zip(got[3], ref[3]):
+            assert np.array_equal(a, b), "rho"
+        # S_max alone (rho pass only) on the chunked handle
+        th, tl = shd.from_host(hi, lo)
+        assert h.smax(th, tl) == ref[4]
+    assert len(seen) >= 2
+    h.set_workspace(0)
+    assert evaluate(h, shd, hi, lo)[0] == ref[0] and h.stat(19) == 1
+    h.close()
+
+
+def test_chunked_quench_is_bit_identical(shd):
+    """The minimizers run on the chunked evaluation unchanged: same trajectory, same final positions."""
+    cfg = inputs.CONFIGS["cfg2"]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    out = []
+    for cap in (0, 0.3):
+        h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+        th, tl = shd.from_host(hi, lo)
+        if cap:
+            h.energy_grad(th, tl)
+            h.set_workspace(int(h.stat(26) * cap))
+        rep = h.minimize(th, tl, smax_tol=1e-12, max_evals=400)
+        assert (h.stat(19) > 1) == bool(cap)
+        out.append((rep, th.cpu().numpy(), tl.cpu().numpy()))
+        h.close()
+    assert out[0][0] == out[1][0]
+    assert np.array_equal(out[0][1], out[1][1]) and np.array_equal(out[0][2], out[1][2])
+
+
+def shard_ranges(N, G):
+    """particle range of rank r: the first N % G ranks hold one particle more"""
+    base, extra = divmod(N, G)
+    starts = [r * base + min(r, extra) for r in range(G + 1)]
+    return [(starts[r], starts[r + 1]) for r in range(G)]
+
+
+@pytest.mark.parametrize("name,G,engine", [("cfg2", 3, 2), ("cfg2", 2, 0), ("cfg3", 4, 0), ("cfg4", 8, 2)])
+def test_sharded_evaluation(shd, oracle, name, G, engine):
+    import torch
+    cfg = inputs.CONFIGS[name]
+    d, N = cfg.d, cfg.N
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    lo = inputs.jitter_lo(hi, 9)
+    hi2, lo2 = hi.reshape(d, N), lo.reshape(d, N)
+    ranks = []
+    for r, (a, b) in enumerate(shard_ranges(N, G)):
+        h = shd.Shd(d, b - a, cfg.L, m_star=cfg.m_star)
+        h.set_engine(engine)
+        h.set_shard(N, r, G)
+        th, tl = shd.from_host(np.ascontiguousarray(hi2[:, a:b]).reshape(-1), np.ascontiguousarray(lo2[:, a:b]).reshape(-1))
+        ranks.append((h, th, tl, a, b))
+    # pass 1 on every rank, then the "all-gather": the ranks' partials back to back in rank order
+    parts = []
+    for h, th, tl, a, b in ranks:
+        buf = h.rho_partial(th, tl)
+        parts.append(buf)
+    gathered = torch.cat(parts)
+    results = []
+    for h, th, tl, a, b in ranks:
+        phi = h.rho_finish(gathered, G)
+        gh, gl = h.grad_local(th, tl)
+        results.append((phi, [t.cpu().numpy() for t in h.rho()], h.last_smax(), gh.cpu().numpy(), gl.cpu().numpy()))
+    # every rank holds the same rho, Phi, S_max, bit for bit
+    for res in results[1:]:
+        assert res[0] == results[0][0] and res[2] == results[0][2]
+        for x, y in zip(res[1], results[0][1]):
+            assert np.array_equal(x, y)
+    # against the oracle (sampled at cfg4)
+    n = oracle.enumerate_Q(d, cfg.m_star)
+    M = len(n)
+    K = cfg.K
+    rho = results[0][1]
+    ks = np.arange(M) if N * M <= 2e8 else np.unique(np.linspace(0, M - 1, 48).astype(np.int64))
+    re, im = oracle.rho(d, N, cfg.L, hi, lo, n[ks])
+    e_rho = oracle.cabsdiff_dd(re, im, *[x[ks] for x in rho]).max()
+    assert e_rho <= 1e-28 * N, e_rho
+    fr, fi = oracle.from_dd(rho[0], rho[1]), oracle.from_dd(rho[2], rho[3])
+    o_phi, o_smax, o_arg, _ = oracle.energy(N, fr, fi)
+    assert oracle.absdiff_dd(o_phi, [results[0][0][0]], [results[0][0][1]])[0] <= 1e-28 * N * N * M
+    (s_hi, s_lo), arg = results[0][2]
+    assert arg == o_arg and oracle.absdiff_dd(o_smax, [s_hi], [s_lo])[0] <= 1e-26 * max(oracle.to_float(o_smax)[0], 1.0)
+    g_hi = np.concatenate([res[3].reshape(d, -1) for res in results], axis=1).reshape(-1)
+    g_lo = np.concatenate([res[4].reshape(d, -1) for res in results], axis=1).reshape(-1)
+    js = np.arange(N) if N * M <= 2e8 else np.unique(np.concatenate(
+        [np.linspace(0, N - 1, 40).astype(np.int64)] + [[a, b - 1] for _, _, _, a, b in ranks]))
+    og = oracle.grad(d, N, cfg.L, hi, lo, n, fr, fi, jlist=js)
+    sel = np.concatenate([a * N + js for a in range(d)])
+    e_g = oracle.absdiff_dd(og, g_hi[sel], g_lo[sel]).max()
+    assert e_g <= 1e-27 * N * M * K, e_g
+    print(name, G, engine, dict(e_rho=e_rho, e_g=e_g))
+    for h, *_ in ranks:
+        h.close()
+
+
+def test_one_rank_communicator(shd, oracle):
+    """The library-owned NCCL path on one GPU: a communicator of one rank runs the same calls (all-gather, fold of the
+    gathered partials, sharded dot products of the minimizer); the result is that of the plain handle."""
+    cfg = inputs.CONFIGS["cfg2"]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    plain = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    ref = evaluate(plain, shd, hi, lo)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    h.set_shard(cfg.N, 0, 1)
+    h.comm_init(shd.comm_unique_id())
+    got = evaluate(h, shd, hi, lo)
+    assert got[0] == ref[0] and got[4] == ref[4]
+    assert np.array_equal(got[1], ref[1]) and np.array_equal(got[2], ref[2])
+    for kind in (0, 1):
+        ta, tb = shd.from_host(hi, lo)
+        tc, td = shd.from_host(hi, lo)
+        r1 = plain.minimize(ta, tb, kind=kind, smax_tol=1e-10, max_evals=300)
+        r2 = h.minimize(tc, td, kind=kind, smax_tol=1e-10, max_evals=300)
+        assert r1 == r2, (kind, r1, r2)
+        assert np.array_equal(ta.cpu().numpy(), tc.cpu().numpy()) and np.array_equal(tb.cpu().numpy(), td.cpu().numpy())
+    h.close()
+    plain.close()

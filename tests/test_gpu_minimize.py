@@ -233,3 +233,47 @@ def test_precision_ladder_quench(shd, oracle):
     _, smax, _, _ = oracle.energy(cfg.N, re, im)
     assert oracle.to_float(smax)[0] < 1e-30
     h.close()
+
+
+def test_cfg4_quench_reaches_1e30(shd, oracle):
+    """BASELINE.json north_star target: full minimization of configs[3] (d=2, N=1e5, chi=0.45, 9e4 wavevectors) to
+    S_max < 1e-30 on one B200, judged by the ORACLE on the device's final positions (R16): factored mode over
+    all 90 000 wavevectors, direct mode (the definition) on a strided subset as a cross-check of the factored tables at
+    this size.  P:77 (stop rule), P:64 / P:107 (no run may get stuck for chi < 1/2).  Also the first GPU test of
+    shd_smax: value and argmax against the oracle's."""
+    import time
+    cfg = inputs.CONFIGS["cfg4"]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    assert h.engine == 2, "the library's own choice at this size is the INT8 tensor-core engine"
+    th, tl = shd.from_host(hi, lo)
+    t0 = time.perf_counter()
+    rep = h.minimize(th, tl, smax_tol=1e-30, max_evals=12000, poll_every=16)
+    seconds = time.perf_counter() - t0
+    assert rep["status"] == shd.SHD_OK, rep
+    assert rep["smax"][0] < 1e-30
+    assert rep["evals"] <= 1.5 * rep["iters"] + 10, "backtracking should be rare"
+    fh, fl = th.cpu().numpy(), tl.cpu().numpy()
+    n = oracle.enumerate_Q(cfg.d, cfg.m_star)
+    t1 = time.perf_counter()
+    re, im = oracle.rho(cfg.d, cfg.N, cfg.L, fh, fl, n, mode="factored")
+    o_phi, o_smax, o_arg, s2 = oracle.energy(cfg.N, re, im)
+    oracle_seconds = time.perf_counter() - t1
+    s_or = oracle.to_float(o_smax)[0]
+    print(f"cfg4 quench: {rep['evals']} evaluations in {seconds:.1f} s; S_max(device) = {rep['smax'][0]:.3e}, "
+          f"S_max(oracle, all {len(n)} k, factored, {oracle_seconds:.0f} s) = {s_or:.3e} at n = {n[o_arg].tolist()}")
+    assert s_or < 1e-30, f"oracle S_max on the device's final positions: {s_or:.3e}"
+    # the factored tables against the definition at this size: strided wavevectors plus the argmax and both ends
+    ks = np.unique(np.concatenate([np.arange(0, len(n), 431), [0, len(n) - 1, o_arg]]))
+    assert len(ks) >= 200
+    dre, dim_ = oracle.rho(cfg.d, cfg.N, cfg.L, fh, fl, n[ks], mode="direct")
+    fre_hi, fre_lo = oracle.to_dd(re[ks])
+    fim_hi, fim_lo = oracle.to_dd(im[ks])
+    assert oracle.cabsdiff_dd(dre, dim_, fre_hi, fre_lo, fim_hi, fim_lo).max() <= 1e-28 * cfg.N * 1e-3
+    # shd_smax on the final positions: same value as the minimizer's report, oracle's value and argmax
+    (s_hi, s_lo), arg = h.smax(th, tl)
+    assert (s_hi, s_lo) == rep["smax"]
+    assert arg == o_arg
+    assert abs(s_hi - s_or) <= 1e-3 * s_or
+    assert oracle.to_float(o_phi)[0] <= rep["phi"][0] * (1 + 1e-3) + 1e-40
+    h.close()

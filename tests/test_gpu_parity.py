@@ -474,3 +474,74 @@ def test_int8_engine_fast_precisions(shd, oracle):
     phi3b, gh3b, gl3b = h.energy_grad(th, tl)
     assert phi3b == phi3 and torch.equal(gh3b, gh3) and torch.equal(gl3b, gl3)
     h.close()
+
+
+@pytest.mark.parametrize("engine", [0, 2])
+def test_energy_grad_host_matches_device_call(shd, oracle, engine):
+    """shd_energy_grad_host (host buffers in, host buffers out: the e2e leg of bench.py) must give exactly what
+    shd_energy_grad gives on device buffers; pinned and pageable memory; with and without the gradient."""
+    import torch
+    cfg = inputs.CONFIGS["cfg2"]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    lo = inputs.jitter_lo(hi, 11)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    h.set_engine(engine)
+    th, tl = shd.from_host(hi, lo)
+    phi, gh, gl = h.energy_grad(th, tl)
+    g_hi, g_lo = gh.cpu().numpy(), gl.cpu().numpy()
+    rho = [t.cpu().numpy() for t in h.rho()]
+    for pinned in (False, True):
+        if pinned:
+            ph, pl = torch.from_numpy(hi).pin_memory().numpy(), torch.from_numpy(lo).pin_memory().numpy()
+            oh = torch.empty(hi.size, dtype=torch.float64).pin_memory().numpy()
+            ol = torch.empty(hi.size, dtype=torch.float64).pin_memory().numpy()
+        else:
+            ph, pl, oh, ol = hi.copy(), lo.copy(), np.full_like(hi, np.nan), np.full_like(hi, np.nan)
+        phi_h = h.energy_grad_host(ph, pl, oh, ol)
+        assert phi_h == phi
+        assert np.array_equal(oh, g_hi) and np.array_equal(ol, g_lo)
+        for a, b in zip(rho, h.rho()):
+            assert np.array_equal(a, b.cpu().numpy())
+        assert h.energy_grad_host(ph, pl) == phi            # energy only
+    # and against the oracle once (this entry point had no parity test of its own)
+    n = oracle.enumerate_Q(cfg.d, cfg.m_star)
+    o = oracle.energy_grad(cfg.d, cfg.N, cfg.L, hi, lo, n, mode="factored")
+    assert oracle.absdiff_dd(o["grad"], oh, ol).max() <= 1e-27 * cfg.N * cfg.M * cfg.K
+    assert oracle.absdiff_dd(o["phi"], [phi_h[0]], [phi_h[1]])[0] <= 1e-28 * cfg.N ** 2 * cfg.M
+    h.close()
+
+
+def test_smax_entry_point(shd, oracle):
+    """shd_smax (rho pass and reduction only): value and argmax against the oracle, and equal to what shd_energy_grad
+    leaves behind (shd_last_smax), on both engines and on a handle that never evaluated a gradient."""
+    cfg = inputs.CONFIGS["cfg2"]
+    hi, lo = inputs.uniform_positions(cfg, 2)
+    n = oracle.enumerate_Q(cfg.d, cfg.m_star)
+    re, im = oracle.rho(cfg.d, cfg.N, cfg.L, hi, lo, n, mode="factored")
+    _, o_smax, o_arg, _ = oracle.energy(cfg.N, re, im)
+    for engine in (0, 2, -1):
+        h = shd.Shd(cfg.d, cfg.N, cfg.L, K=cfg.K)
+        h.set_engine(engine)
+        th, tl = shd.from_host(hi, lo)
+        (s_hi, s_lo), arg = h.smax(th, tl)
+        assert arg == o_arg
+        assert oracle.absdiff_dd(o_smax, [s_hi], [s_lo])[0] <= 1e-28 * cfg.N
+        h.energy_grad(th, tl)
+        assert h.last_smax() == ((s_hi, s_lo), arg)
+        h.close()
+
+
+def test_engine_selection_is_the_librarys(shd):
+    """A fresh handle runs on the engine the library chooses (include/shd.h, shd_set_engine): INT8 tensor cores for the
+    large d <= 2 workloads, FP64 limbs for short last axes (d = 3) and tiny systems; -1 restores the choice."""
+    want = {"cfg1": 0, "cfg2": 2, "cfg3": 0, "cfg4": 2, "cfg5": 2}
+    for name, e in want.items():
+        cfg = inputs.CONFIGS[name]
+        h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+        assert h.engine == e, (name, h.engine)
+        assert h.stat(27) == 1
+        h.set_engine(0)
+        assert h.engine == 0 and h.stat(27) == 0
+        h.set_engine(-1)
+        assert h.engine == e and h.stat(27) == 1
+        h.close()
