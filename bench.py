@@ -9,8 +9,10 @@ second (N*M per evaluation, "2 calculations, each with M N terms").
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config cfg4] [--impl reference]
 
-N > 1 (torchrun, one rank per GPU): the path runs as independent replicas (one quench per GPU, the
-paper's own ensemble parallelism), no data-path collective; "weak".
+N > 1 (torchrun, one rank per GPU): the particles are SHARDED over the ranks: every rank builds
+the tables of its own particles, one all-gather of the partial sums of rho per evaluation (NCCL, bytes, added in fixed
+rank order by the library's kernel), local gradient pass; total work fixed: "scaling": "strong".  `--replicas` runs
+the paper's own ensemble parallelism instead (independent systems; no collective; "weak").
 """
 from __future__ import annotations
 
@@ -36,10 +38,24 @@ UNIT = "pair-terms/s"
 # rho pass 24 per (p,q) cell = 2 wavevectors -> 12; gradient pass 48 per cell -> 24 (issued as
 # DMMA.8x8x4, 256 FMAs per warp instruction).
 ALG_DFMA_RHO, ALG_DFMA_GRAD = 12.0, 24.0
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture
-# (profiles/r1d_summary.md), bytes; known for the headline workload only, otherwise null
-NCU_TRAFFIC = {("cfg4", "k_grad"): 12.77e9, ("cfg4", "k_rho"): 3.63e9,           # profiles/r1d_summary.md
-               ("cfg4", "k_grad8"): 2.09e9, ("cfg4", "k_rho8"): 1.55e9}          # profiles/r1f_summary.md
+
+
+def ncu_traffic(kernel, workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, read from the NEWEST committed ncu summary
+    under profiles/ that states it for this workload, in the line format
+        `traffic` (<workload>, dram read + write per launch): `k_a` 1.23 GB, `k_b` 4.56 GB
+    Returns (bytes, file name) or (None, None): nothing is hard-coded here."""
+    import re
+    best = (None, None)
+    for f in sorted((ROOT / "profiles").glob("r*_summary.md")):
+        for ln in f.read_text().splitlines():
+            if not ln.startswith("`traffic` (") or workload not in ln.split(")")[0]:
+                continue
+            m = re.search(r"`%s`\s+([0-9.]+)\s*GB" % re.escape(kernel), ln)
+            if m:
+                best = (float(m.group(1)) * 1e9, "profiles/" + f.name)
+    return best
+
 # INT8 tensor-core engines (k_rho8.cu, k_grad8.cu): 91 digit pairs per real product; 4 real products per (p,q)
 # cell = 2 wavevectors in the rho pass, 8 in the gradient pass; 2 operations per multiply-accumulate
 ALG_MAC_RHO8, ALG_MAC_GRAD8 = 182.0, 364.0
@@ -68,7 +84,7 @@ def whole_job_value(pairs_per_rank, steps, world, total_ms):
 
 
 # ------------------------------------------------------------------------------ oracle legs
-def oracle_sample(cfg, hi, lo, budget_pairs, rho_dd=None):
+def oracle_sample(cfg, hi, lo, budget_pairs, rho_dd=None, jrange=None):
     """Time the binary128 oracle (direct mode, as it stands) on a bounded sample of the workload:
     a strided set of wavevectors x all particles (rho) and a strided set of particles x all
     wavevectors (gradient).  Returns timing, the sample description and the oracle values."""
@@ -78,7 +94,8 @@ def oracle_sample(cfg, hi, lo, budget_pairs, rho_dd=None):
     nk = int(max(1, min(M, budget_pairs // cfg.N)))
     nj = int(max(1, min(cfg.N, budget_pairs // M)))
     ks = np.unique(np.linspace(0, M - 1, nk).astype(np.int64))
-    js = np.unique(np.linspace(0, cfg.N - 1, nj).astype(np.int64))
+    j0, j1 = jrange if jrange else (0, cfg.N)       # (sharded bench: the gradient sample lies in rank 0's particles)
+    js = np.unique(np.linspace(j0, j1 - 1, min(nj, j1 - j0)).astype(np.int64))
     t0 = time.perf_counter()
     re, im = O.rho(cfg.d, cfg.N, cfg.L, hi, lo, n[ks])
     t1 = time.perf_counter()
@@ -128,13 +145,14 @@ def run_reference(args, cfg):
     print(json.dumps(line), flush=True)
 
 
-def workload_config(cfg, world):
+def workload_config(cfg, world, replicas=True):
     src = f"BASELINE.json configs[{int(cfg.name[3:]) - 1}]" if cfg.name.startswith("cfg") else \
         "the paper's system size (P:33, P:89; not a BASELINE.json config)"
     return {"workload": f"{src}: d={cfg.d}, N={cfg.N}, unit density, "
                         f"chi={cfg.chi} (m*={cfg.m_star}, |Q|={cfg.M}), v=1, uniform seeded positions",
             "d": cfg.d, "N": cfg.N, "M": cfg.M, "pair_terms_per_eval": cfg.pairs,
-            "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (seed = rank)",
+            "parallelism": "single GPU" if world == 1 else (f"{world} independent replicas (seed = rank)" if replicas else
+                            f"{world} particle shards, one all-gather of partial rho per evaluation (NCCL)"),
             "l2": "256 MB memset between timed steps; the streamed phasor tables are GBs (>> 126 MB L2)"}
 
 
@@ -197,12 +215,28 @@ def run_gpu(args, cfg):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     from paper_2304_09139_b200 import shd
 
-    hi, lo = inputs.uniform_positions(cfg, rank)            # replica r quenches seed r
-    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    sharded = world > 1 and not args.replicas
+    from paper_2304_09139_b200 import sharding
+    if sharded:
+        hi, lo = inputs.uniform_positions(cfg, 0)           # one system, its particles dealt out in contiguous ranges
+        j_begin, j_end = sharding.shard_range(cfg.N, rank, world)
+        hi_l, lo_l = sharding.local_positions(hi, lo, cfg.d, cfg.N, rank, world)
+    else:
+        hi, lo = inputs.uniform_positions(cfg, rank)        # replica r quenches seed r
+        j_begin, j_end = 0, cfg.N
+        hi_l, lo_l = hi, lo
+    n_local = j_end - j_begin
+    h = shd.Shd(cfg.d, n_local, cfg.L, m_star=cfg.m_star)
     assert h.M == cfg.M
     stream = torch.cuda.current_stream()
     h.set_stream(stream)
-    pos_hi, pos_lo = shd.from_host(hi, lo)
+    if args.engine != "auto":
+        h.set_engine(int(args.engine))      # else: the engine the library chose for this workload (shd_set_engine -1)
+    engine = h.engine
+    if sharded:
+        h.set_shard(cfg.N, rank, world)
+        sharding.init_comm(h)
+    pos_hi, pos_lo = shd.from_host(hi_l, lo_l)
     grad_hi, grad_lo = torch.empty_like(pos_hi), torch.empty_like(pos_hi)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
 
@@ -210,11 +244,6 @@ def run_gpu(args, cfg):
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
-
-    # engine of the two O(N M) passes: 2 = INT8 tensor cores (tcgen05), 0 = FP64 limbs on DMMA (the reference
-    # engine).  auto: the tensor-core engine where its digit tables pay off and fit beside the limb tables
-    engine = {"auto": 2 if (cfg.pairs >= 5e7 and cfg.d <= 2) else 0}.get(args.engine, None)
-    engine = int(args.engine) if engine is None else engine
 
     def timed_steps(steps, warmup, sample_clocks):
         """`steps` evaluations timed with CUDA events on the handle's stream (L2 flushed before each)."""
@@ -240,13 +269,12 @@ def run_gpu(args, cfg):
         return float(sum(a.elapsed_time(b) for a, b in ev)), kms, launches, phi, clk
 
     # ---- device-resident leg (value)
-    h.set_engine(engine)
     h.set_precision(args.precision)      # 3 (default) = the headline; 2 / 1 = the truncated evaluations of the precision ladder
     total_ms, kms, launches, phi, clk = timed_steps(args.steps, args.warmup, True)
 
     # ---- end-to-end leg: host (pinned) buffers through shd_energy_grad_host
-    ph = torch.from_numpy(hi).pin_memory(); pl = torch.from_numpy(lo).pin_memory()
-    gh = torch.empty(cfg.d * cfg.N, dtype=torch.float64).pin_memory(); gl = torch.empty_like(gh).pin_memory()
+    ph = torch.from_numpy(hi_l).pin_memory(); pl = torch.from_numpy(lo_l).pin_memory()
+    gh = torch.empty(cfg.d * n_local, dtype=torch.float64).pin_memory(); gl = torch.empty_like(gh).pin_memory()
     for _ in range(max(1, min(args.warmup, 2))):
         h.energy_grad_host(ph.numpy(), pl.numpy(), gh.numpy(), gl.numpy())
     barrier()
@@ -257,15 +285,30 @@ def run_gpu(args, cfg):
     e2e_s = time.perf_counter() - t0
     barrier()
 
-    total_ms, e2e_ms = max_over_ranks([total_ms, e2e_s * 1e3], "cuda")
+    # ---- the same evaluation at a mid-quench state (non-zero lo words; dd paths with lo = 0 can be
+    # accidentally cheaper): positions after --midquench-evals L-BFGS evaluations from the seeded start
+    mid = None
+    if args.midquench_evals > 0 and args.precision == 3:
+        start = (pos_hi.clone(), pos_lo.clone())
+        rep_ = h.minimize(pos_hi, pos_lo, smax_tol=0.0, max_evals=args.midquench_evals, poll_every=16)
+        nz = float((pos_lo != 0).double().mean().item())
+        nmid = max(3, min(args.steps, 10))
+        mid_ms, _, _, _, _ = timed_steps(nmid, 3, False)
+        mid = {"ms": mid_ms, "steps": nmid, "evals_before": rep_["evals"], "smax": rep_["smax"][0], "lo_nonzero_fraction": nz}
+        pos_hi.copy_(start[0]); pos_lo.copy_(start[1])
+        h.energy_grad(pos_hi, pos_lo, grad_hi, grad_lo)     # rho() / last_smax() below belong to the seeded start
+
+    total_ms, e2e_ms, mid_ms = max_over_ranks([total_ms, e2e_s * 1e3, mid["ms"] if mid else 0.0], "cuda")
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
     pairs = float(cfg.pairs)
-    value = whole_job_value(pairs, args.steps, world, total_ms)
-    e2e_value = whole_job_value(pairs, args.steps, world, e2e_ms)
-    nbytes = 2 * cfg.d * cfg.N * 8
+    jobs = 1 if sharded else world          # sharded: ONE system's pair-terms over all ranks; replicas: one system per rank
+    value = whole_job_value(pairs, args.steps, jobs, total_ms)
+    e2e_value = whole_job_value(pairs, args.steps, jobs, e2e_ms)
+    nbytes = 2 * cfg.d * n_local * 8
+    pairs_rank = pairs * n_local / cfg.N    # pair-terms this rank's O(N M) kernels process per evaluation
 
     # ---- rooflines of the dominant kernel
     dfma_best, dfma_sus = shd.fp64_peak(0, 0.5)
@@ -279,23 +322,22 @@ def run_gpu(args, cfg):
         dom = "k_grad" if grad_ms >= rho_ms else "k_rho"
         dom_ms = max(grad_ms, rho_ms)
         alg = ALG_DFMA_GRAD if dom == "k_grad" else ALG_DFMA_RHO
-        achieved = pairs * alg * 2.0 / (dom_ms * 1e-3) / 1e12          # TFLOP/s, DFMA = 2 FLOP
+        achieved = pairs_rank * alg * 2.0 / (dom_ms * 1e-3) / 1e12     # TFLOP/s, DFMA = 2 FLOP
         peak = pipe_sus * 2.0 / 1e12
         launched = h.stat(12) if dom == "k_grad" else h.stat(0)
         return {
             "bound": "alu", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-            "frac": achieved / peak, "traffic": NCU_TRAFFIC.get((cfg.name, dom)),
-            "traffic_source": "profiles/r1d_summary.md (one ncu --set full capture of this kernel at this workload)"
-                              if (cfg.name, dom) in NCU_TRAFFIC else None,
+            "frac": achieved / peak, "traffic": ncu_traffic(dom, cfg.name)[0] if world == 1 else None,
+            "traffic_source": ncu_traffic(dom, cfg.name)[1] if world == 1 else None,
             "peak_source": "measured live: shd_fp64_peak, max of dependent-DFMA chains and DMMA.8x8x4 chains "
                            "(one FP64 pipe), sustained over 1 s (of measured)",
             "peak_burst": max(dfma_best, dmma_best) * 2.0 / 1e12, "dfma_peak_tfma": dfma_sus / 1e12,
             "dmma_peak_tfma": dmma_sus / 1e12, "dadd_peak_tinstr": dadd_sus / 1e12,
             "nominal_peak": 148 * 64 * 2 * 1.965e9 / 1e12,
             "kernel_ms": dom_ms, "algorithmic_dfma_per_pair": alg,
-            "launched_dfma_per_pair": launched / pairs,
+            "launched_dfma_per_pair": launched / pairs_rank,
             "issue_frac_launched": launched / (dom_ms * 1e-3) / pipe_sus,
-            "whole_eval_frac": pairs * (ALG_DFMA_RHO + ALG_DFMA_GRAD) / (total_ms_ / steps_ * 1e-3) / pipe_sus,
+            "whole_eval_frac": pairs_rank * (ALG_DFMA_RHO + ALG_DFMA_GRAD) / (total_ms_ / steps_ * 1e-3) / pipe_sus,
             "kernel_ms_all": {k: v / steps_ for k, v in kms_.items()},
         }
 
@@ -314,34 +356,44 @@ def run_gpu(args, cfg):
         else:
             dom_ms = grad_ms if dom == "k_grad8" else rho_ms
             mac = ALG_MAC_GRAD8 if dom == "k_grad8" else ALG_MAC_RHO8
-            achieved = pairs * mac * 2.0 / (dom_ms * 1e-3) / 1e12       # TOP/s, 2 per multiply-accumulate
+            achieved = pairs_rank * mac * 2.0 / (dom_ms * 1e-3) / 1e12  # TOP/s, 2 per multiply-accumulate
+            mp = json.load(open(ROOT / "MEASURED_PEAKS.json")) if (ROOT / "MEASURED_PEAKS.json").exists() else {}
             roofline = {
                 "bound": "tensor", "kernel": dom, "achieved": achieved, "peak": i8_tops, "unit": "TFLOP/s",
-                "frac": achieved / i8_tops, "traffic": NCU_TRAFFIC.get((cfg.name, dom)),
-                "traffic_source": "profiles/r1f_summary.md" if (cfg.name, dom) in NCU_TRAFFIC else None,
+                "frac": achieved / i8_tops, "traffic": ncu_traffic(dom, cfg.name)[0] if world == 1 else None,
+                "traffic_source": ncu_traffic(dom, cfg.name)[1] if world == 1 else None,
+                # the guide's rule for a contraction in another dtype: measured bf16 peak x nominal int8 : bf16 = 2
+                "frac_of_measured_bf16_x2_burst": achieved / (2.0 * mp["bf16_tflops"]) if "bf16_tflops" in mp else None,
+                "frac_of_measured_bf16_x2_sustained": achieved / (2.0 * mp["bf16_tflops_sustained"]) if "bf16_tflops_sustained" in mp else None,
+                # SM clock at which one tcgen05.mma.kind::i8 of N = 256 takes its 128 cycles and gives this peak; the hot
+                # kernels themselves run at ~1.66 GHz (clock64 against globaltimer inside k_rho8, profiles/r2a_summary.md)
+                "peak_implied_sm_mhz": i8_tops * 1e12 / (148 * 8192 * 2.0) / 1e6,
                 "dtype": "s8 x s8 -> s32 (exact digit-sliced contraction; counted in integer operations)",
                 "peak_source": "measured live: shd_i8_probe, tcgen05.mma.kind::i8 M=128 N=256 K=32 issued back to "
                                "back on all SMs; MEASURED_PEAKS.json bf16 x 2 (nominal int8 : bf16) for comparison",
-                "peak_from_measured_bf16_x2": 2.0 * float(json.load(open(ROOT / "MEASURED_PEAKS.json"))["bf16_tflops"])
-                                              if (ROOT / "MEASURED_PEAKS.json").exists() else None,
+                "peak_from_measured_bf16_x2": 2.0 * float(mp["bf16_tflops"]) if "bf16_tflops" in mp else None,
                 "i8_products_exact": i8_bad == 0,
                 "kernel_ms": dom_ms, "algorithmic_mac_per_pair": mac,
-                "whole_eval_frac": pairs * (ALG_MAC_RHO8 + ALG_MAC_GRAD8) * 2.0 / (total_ms / args.steps * 1e-3) / 1e12 / i8_tops,
+                "whole_eval_frac": pairs_rank * (ALG_MAC_RHO8 + ALG_MAC_GRAD8) * 2.0 / (total_ms / args.steps * 1e-3) / 1e12 / i8_tops,
                 "kernel_ms_all": {k: v / args.steps for k, v in kms.items()},
             }
         # the FP64 limb engine (the reference engine of this library) on the same inputs, for comparison
-        h.set_engine(0)
+        # (single GPU only: a sharded evaluation is a collective and the other ranks have left)
         n64 = max(3, min(args.steps, 5))
-        try:
+        if sharded:
+            fp64_engine = {"skipped": "sharded run"}
+        else:
+          h.set_engine(0)
+          try:
             t64, k64, _, _, _ = timed_steps(n64, 3, False)
-            fp64_engine = {"ms_per_step": t64 / n64, "value": pairs * n64 / (t64 * 1e-3),
+            fp64_engine = {"ms_per_step": t64 / n64, "value": pairs_rank * n64 / (t64 * 1e-3),
                            "roofline": fp64_roofline(k64, t64, n64)}
-        except shd.ShdError as e:          # at the paper's N the FP64 engine's tables do not fit beside the digit tables
+          except shd.ShdError as e:        # at the paper's N the FP64 engine's tables do not fit
             if e.code != shd.SHD_ENOMEM:
                 raise
-            fp64_engine = {"unavailable": "the FP64 engine's limb tables do not fit beside the INT8 digit tables"}
-        h.set_engine(engine)
-        h.energy_grad(pos_hi, pos_lo, grad_hi, grad_lo)                 # rho() below belongs to the timed engine
+            fp64_engine = {"unavailable": "the FP64 engine's limb tables do not fit"}
+          h.set_engine(engine)
+          h.energy_grad(pos_hi, pos_lo, grad_hi, grad_lo)               # rho() below belongs to the timed engine
 
     # ---- oracle on the host cores, same run, bounded sample; doubles as a live parity sample
     from oracle import shd_oracle as O
@@ -349,9 +401,9 @@ def run_gpu(args, cfg):
     cores = O.num_threads()
     rho_dd = [x.cpu().numpy() for x in h.rho()]
     g_hi, g_lo = gh.numpy(), gl.numpy()
-    s = oracle_sample(cfg, hi, lo, int(2.5e6 * cores), rho_dd)
+    s = oracle_sample(cfg, hi, lo, int(2.5e6 * cores), rho_dd, jrange=(j_begin, j_end))
     e_rho = O.cabsdiff_dd(s["re"], s["im"], *[x[s["ks"]] for x in rho_dd])
-    sel = np.concatenate([a * cfg.N + s["js"] for a in range(cfg.d)])
+    sel = np.concatenate([a * n_local + (s["js"] - j_begin) for a in range(cfg.d)])
     e_g = O.absdiff_dd(s["grad"], g_hi[sel], g_lo[sel])
     tol_rho, tol_g = 1e-28 * cfg.N, 1e-27 * cfg.N * cfg.M * cfg.K
     smax, arg = h.last_smax()
@@ -359,12 +411,20 @@ def run_gpu(args, cfg):
         "metric": METRIC if args.precision == 3 else f"{METRIC} [shd_set_precision {args.precision}: truncated evaluation, not the headline]",
         "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64 (double-double)", "data": "synthetic",
-        "config": workload_config(cfg, world),
+        "scaling": "strong" if sharded else "weak", "vs_baseline": None,
+        "dtype": {0: "f64 (exact 22-bit limb products on the FP64 matrix instruction -> double-double)",
+                  1: "rho pass: s8 digit slices of 102-bit fixed point -> s32 exact -> double-double; gradient pass: f64 limbs",
+                  2: "s8 digit slices of 102-bit fixed point -> s32 exact (tensor memory) -> exact integer contraction -> "
+                     "double-double in and out"}[engine],
+        "data": "synthetic",
+        "config": workload_config(cfg, world, replicas=not sharded),
         "clocks": clk,
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / args.steps,
                 "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes + 64},
         "gpu_launches": launches,
+        "value_midquench": (whole_job_value(pairs, mid["steps"], jobs, mid_ms) if mid else None),
+        "midquench": ({k: v for k, v in mid.items() if k != "ms"} | {"ms_per_step": mid_ms / mid["steps"]}) if mid else None,
+        "engine_selected_by": "library (shd_set_engine -1)" if args.engine == "auto" else "--engine",
         "engine": {0: "fp64 limbs on DMMA.8x8x4", 1: "rho pass on INT8 tensor cores (tcgen05), gradient pass on FP64 limbs",
                    2: "both O(N M) passes on INT8 tensor cores (tcgen05.mma.kind::i8, exact digit slices)"}[engine],
         "precision_limbs": args.precision,
@@ -391,6 +451,10 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--engine", default="auto", choices=["auto", "0", "1", "2"],
                     help="engine of the two O(N M) passes: 0 FP64 limbs (DMMA), 1 rho on INT8 tensor cores, 2 both")
+    ap.add_argument("--replicas", action="store_true",
+                    help="N > 1: independent replicas (weak scaling, no collective) instead of particle shards (strong scaling)")
+    ap.add_argument("--midquench-evals", type=int, default=300,
+                    help="also time the evaluation at the state this many L-BFGS evaluations into the quench (0 = skip)")
     ap.add_argument("--precision", type=int, default=3, choices=[1, 2, 3],
                     help="shd_set_precision: 3 = full double-double (the headline); 2 / 1 time the truncated evaluations of "
                          "the precision ladder (their line fails the parity sample by design and is not a bench value)")

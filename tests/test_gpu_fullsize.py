@@ -9,7 +9,10 @@ the gradient sum is checked on its own), plus properties that hold at any size:
   translation invariance sum_j dPhi/dr_j = 0, bit-identical repeats.
 Tolerances: BASELINE.json north_star, and the tighter "what the arithmetic delivers" bounds.
 """
+import json
 import math
+import os
+from pathlib import Path
 
 import numpy as np
 import pytest
@@ -89,3 +92,138 @@ def test_fullsize_sampled(shd, oracle, name, nk, nj, jitter, engine):
         assert np.array_equal(x, y.cpu().numpy())
     print(name, "engine", engine, dict(e_rho=e_rho.max(), e_phi=e_phi, e_g=e_g.max(), sum_grad=tot))
     h.close()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Targeted samples: the kernels' special paths, hit on purpose instead of by the luck of an even stride.
+def decompose(cfg, n):
+    """(p, q) cell of every wavevector under the library's outer-product decomposition (csrc/shd_internal.h):
+    d=1: n = S p + sigma q (S a power of two >= sqrt(2 n_max)); d=2: (p, q) = (n0, |n1|); d>=3: p = index of the prefix
+    (n0, .., n_{d-2}) among the distinct prefixes in lexicographic order, q = |n_{d-1}|."""
+    n = np.asarray(n).reshape(len(n), -1).astype(np.int64)
+    if cfg.d == 1:
+        R = int(n.max())
+        S = 2
+        while S * S < 2 * R:
+            S *= 2
+        p = (n[:, 0] + S // 2 - 1) // S
+        return p, np.abs(n[:, 0] - S * p)
+    if cfg.d == 2:
+        return n[:, 0], np.abs(n[:, 1])
+    pref = n[:, :-1]
+    _, inv = np.unique(pref, axis=0, return_inverse=True)       # np.unique sorts rows lexicographically
+    return inv.reshape(-1), np.abs(n[:, -1])
+
+
+def targeted_k(cfg, n, seed):
+    """all wavevectors of the first, the last and two seeded boundary tiles of both rho kernels (32 x 32 cells for
+    k_rho, 64 x 16 for k_rho8), capped at 1500 per tile by a seeded draw"""
+    p, q = decompose(cfg, n)
+    rng = np.random.default_rng(seed)
+    chosen = []
+    for tp, tq in ((32, 32), (64, 16)):
+        tile = (p // tp) * 100000 + q // tq
+        ids, counts = np.unique(tile, return_counts=True)
+        full = 2 * tp * tq
+        boundary = ids[counts < 0.75 * full]
+        pick = [ids[0], ids[-1]] + list(rng.choice(boundary, size=min(2, len(boundary)), replace=False))
+        for t in pick:
+            ks = np.nonzero(tile == t)[0]
+            if len(ks) > 1500:
+                ks = rng.choice(ks, size=1500, replace=False)
+            chosen.append(ks)
+    return np.unique(np.concatenate(chosen))
+
+
+def targeted_j(N):
+    """first and last particle of the first, a middle and the last 64- and 128-particle block (the ragged one)"""
+    js = []
+    for b in (64, 128):
+        nb = (N + b - 1) // b
+        for blk in (0, nb // 2, nb - 1):
+            js += [blk * b, min(blk * b + b - 1, N - 1)]
+    return np.unique(np.array(js, dtype=np.int64))
+
+
+@pytest.mark.parametrize("engine", [0, 2])
+@pytest.mark.parametrize("name", ["cfg3", "cfg4", "cfg5"])
+def test_fullsize_targeted(shd, oracle, name, engine):
+    """Boundary tiles, first/last tiles, block edges and the ragged last block at the full sizes: rho on every
+    wavevector of the chosen tiles (factored oracle, itself checked against the definition on a subset here),
+    gradient on the block-edge particles (direct mode on the GPU's own promoted rho)."""
+    cfg = inputs.CONFIGS[name]
+    hi, lo = inputs.uniform_positions(cfg, 1)
+    lo = inputs.jitter_lo(hi, 17)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    h.set_engine(engine)
+    n = oracle.enumerate_Q(cfg.d, cfg.m_star)
+    th, tl = shd.from_host(hi, lo)
+    phi, gh, gl = h.energy_grad(th, tl)
+    rho = [t.cpu().numpy() for t in h.rho()]
+    g_hi, g_lo = gh.cpu().numpy(), gl.cpu().numpy()
+    N, M, d = cfg.N, cfg.M, cfg.d
+    nmax = int(np.abs(n).max())
+    K = cfg.K if d > 1 else 2 * np.pi / cfg.L * (nmax + 0.5)
+    ks = targeted_k(cfg, n, 5)
+    re, im = oracle.rho(d, N, cfg.L, hi, lo, n[ks], mode="factored")
+    e_rho = oracle.cabsdiff_dd(re, im, *[x[ks] for x in rho])
+    assert e_rho.max() <= 1e-28 * N, f"rho: {e_rho.max():.3e} at n = {n[ks[e_rho.argmax()]]}"
+    assert e_rho.max() <= RHO_TIGHT * np.sqrt(N) * (1 + nmax / 64), f"rho (tight): {e_rho.max():.3e}"
+    sub = ks[:: max(1, len(ks) // 24)]                         # the factored tables against the definition
+    dre, dim_ = oracle.rho(d, N, cfg.L, hi, lo, n[sub], mode="direct")
+    fh = [oracle.to_dd(x[np.isin(ks, sub)]) for x in (re, im)]
+    assert oracle.cabsdiff_dd(dre, dim_, fh[0][0], fh[0][1], fh[1][0], fh[1][1]).max() <= 1e-30 * N
+    fr, fi = oracle.from_dd(rho[0], rho[1]), oracle.from_dd(rho[2], rho[3])
+    js = targeted_j(N)
+    og = oracle.grad(d, N, cfg.L, hi, lo, n, fr, fi, jlist=js)
+    sel = np.concatenate([a * N + js for a in range(d)])
+    e_g = oracle.absdiff_dd(og, g_hi[sel], g_lo[sel])
+    assert e_g.max() <= 1e-27 * N * M * K, f"grad: {e_g.max():.3e}"
+    _, _, _, s2 = oracle.energy(N, fr, fi)
+    gscale = 2 * K * np.sqrt(M * oracle.to_float(s2).max())
+    assert e_g.max() <= GRAD_TIGHT * gscale * (1 + nmax / 64), f"grad (tight): {e_g.max():.3e}"
+    print(name, "engine", engine, f"{len(ks)} wavevectors of 8 tiles, {len(js)} block-edge particles",
+          dict(e_rho=e_rho.max(), e_g=e_g.max()))
+    h.close()
+
+
+@pytest.mark.skipif(os.environ.get("SHD_SLOW") != "1", reason="~10 min of oracle time: run with SHD_SLOW=1 (profiles/r2_fullparity.md)")
+@pytest.mark.parametrize("name", ["cfg3", "cfg4", "cfg5"])
+def test_full_array_parity(shd, oracle, name):
+    """one FULL factored-oracle pass per large config -- every wavevector and every gradient component
+    of both engines against the oracle.  Writes one JSON line per (config, engine) to gpurun_out/fullparity.jsonl."""
+    import time
+    cfg = inputs.CONFIGS[name]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    lo = inputs.jitter_lo(hi, 7)
+    N, M, d = cfg.N, cfg.M, cfg.d
+    n = oracle.enumerate_Q(d, cfg.m_star)
+    nmax = int(np.abs(n).max())
+    K = cfg.K if d > 1 else 2 * np.pi / cfg.L * (nmax + 0.5)
+    t0 = time.perf_counter()
+    o = oracle.energy_grad(d, N, cfg.L, hi, lo, n, mode="factored")
+    t_or = time.perf_counter() - t0
+    out = Path(os.environ.get("GRAFT_REPO_ROOT", ".")) / "gpurun_out"
+    out.mkdir(exist_ok=True)
+    for engine in (0, 2):
+        h = shd.Shd(d, N, cfg.L, m_star=cfg.m_star)
+        h.set_engine(engine)
+        th, tl = shd.from_host(hi, lo)
+        phi, gh, gl = h.energy_grad(th, tl)
+        rho = [t.cpu().numpy() for t in h.rho()]
+        smax, arg = h.last_smax()
+        e_rho = oracle.cabsdiff_dd(o["rho_re"], o["rho_im"], *rho)
+        e_g = oracle.absdiff_dd(o["grad"], gh.cpu().numpy(), gl.cpu().numpy())
+        e_phi = oracle.absdiff_dd(o["phi"], [phi[0]], [phi[1]])[0]
+        e_s = oracle.absdiff_dd(o["smax"], [smax[0]], [smax[1]])[0]
+        line = dict(config=name, engine=engine, N=N, M=M, oracle_seconds=round(t_or, 1),
+                    rho_max_err=float(e_rho.max()), rho_tol=1e-28 * N, rho_argmax_n=n[int(e_rho.argmax())].tolist(),
+                    grad_max_err=float(e_g.max()), grad_tol=1e-27 * N * M * K, phi_err=float(e_phi), phi_tol=1e-28 * N * N * M,
+                    smax_err=float(e_s), argmax_equal=bool(arg == o["argmax"]))
+        print(json.dumps(line))
+        with open(out / "fullparity.jsonl", "a") as f:
+            f.write(json.dumps(line) + "\n")
+        assert e_rho.max() <= 1e-28 * N and e_g.max() <= 1e-27 * N * M * K and e_phi <= 1e-28 * N * N * M
+        assert e_rho.max() <= RHO_TIGHT * np.sqrt(N) * (1 + nmax / 64)
+        assert arg == o["argmax"]
+        h.close()
