@@ -380,8 +380,8 @@ def run_gpu(args, cfg):
         # the FP64 limb engine (the reference engine of this library) on the same inputs, for comparison
         # (single GPU only: a sharded evaluation is a collective and the other ranks have left)
         n64 = max(3, min(args.steps, 5))
-        if sharded:
-            fp64_engine = {"skipped": "sharded run"}
+        if sharded or args.no_fp64_compare:
+            fp64_engine = {"skipped": "sharded run" if sharded else "--no-fp64-compare"}
         else:
           h.set_engine(0)
           try:
@@ -422,6 +422,7 @@ def run_gpu(args, cfg):
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms / args.steps,
                 "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes + 64},
         "gpu_launches": launches,
+        "chunks_per_evaluation": int(h.stat(19)), "table_bytes": h.stat(26),
         "value_midquench": (whole_job_value(pairs, mid["steps"], jobs, mid_ms) if mid else None),
         "midquench": ({k: v for k, v in mid.items() if k != "ms"} | {"ms_per_step": mid_ms / mid["steps"]}) if mid else None,
         "engine_selected_by": "library (shd_set_engine -1)" if args.engine == "auto" else "--engine",
@@ -451,6 +452,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--engine", default="auto", choices=["auto", "0", "1", "2"],
                     help="engine of the two O(N M) passes: 0 FP64 limbs (DMMA), 1 rho on INT8 tensor cores, 2 both")
+    ap.add_argument("--no-fp64-compare", action="store_true", help="do not time the FP64 limb engine beside the INT8 one")
     ap.add_argument("--replicas", action="store_true",
                     help="N > 1: independent replicas (weak scaling, no collective) instead of particle shards (strong scaling)")
     ap.add_argument("--midquench-evals", type=int, default=300,

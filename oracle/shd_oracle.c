@@ -611,3 +611,25 @@ void shdo_structure_factor(long N, long M, const q128 *rho_re, const q128 *rho_i
     *dev2 = pairwise_sum(t, M);
     free(t);
 }
+
+/*
+ * Radially averaged structure factor (Fig. 2a, Fig. S1a: S(k) against |k|, beyond K too when the wavevector
+ * set reaches there).  |k|^2 = (2 pi / L)^2 n.n, so a radial bin is a range of the INTEGER n.n: bin b collects the
+ * wavevectors with edges[b] <= n.n < edges[b+1] (edges ascending, nbins + 1 of them); count[b] = how many,
+ * S_mean[b] = (sum of S(k) over them) / count[b] (0 for an empty bin).  Only half-space vectors are listed, and
+ * S(-k) = S(k), so the mean over the half shell is the mean over the whole shell.  Plain loops, binary128.
+ */
+void shdo_structure_factor_shells(int d, long N, long M, const int *n, const q128 *rho_re, const q128 *rho_im,
+                                  long nbins, const long *edges, long *count, q128 *S_mean)
+{
+    for (long b = 0; b < nbins; b++) { count[b] = 0; S_mean[b] = 0; }
+    for (long k = 0; k < M; k++) {
+        long nn = 0;
+        for (int a = 0; a < d; a++) nn += (long)n[k * d + a] * (long)n[k * d + a];
+        const q128 S = (rho_re[k] * rho_re[k] + rho_im[k] * rho_im[k]) / (q128)N;
+        for (long b = 0; b < nbins; b++)
+            if (edges[b] <= nn && nn < edges[b + 1]) { count[b]++; S_mean[b] += S; break; }
+    }
+    for (long b = 0; b < nbins; b++)
+        if (count[b] > 0) S_mean[b] /= (q128)count[b];
+}

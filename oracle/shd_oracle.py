@@ -66,6 +66,7 @@ def lib():
                                          C.c_int, C.c_double, C.c_double, C.c_long, lp, vp, vp]
         L.shdo_minimize_fire.restype = C.c_int
         L.shdo_structure_factor.argtypes = [C.c_long, C.c_long, vp, vp, vp, vp]
+        L.shdo_structure_factor_shells.argtypes = [C.c_int, C.c_long, C.c_long, ip, vp, vp, C.c_long, lp, lp, vp]
         _lib = L
     return _lib
 
@@ -290,6 +291,20 @@ def structure_factor(N, rho_re, rho_im):
     S, dev2 = qzeros(M), qzeros(1)
     lib().shdo_structure_factor(int(N), M, _q(rho_re), _q(rho_im), _q(S), _q(dev2))
     return S, dev2
+
+
+def structure_factor_shells(d, N, n, rho_re, rho_im, edges):
+    """Radial average of S(k) (Fig. 2a, Fig. S1a): bin b = wavevectors with edges[b] <= n.n < edges[b+1].
+    Returns (count int64 array, S_mean binary128 array)."""
+    n, pn = _i(n)
+    M = n.size // d
+    e = np.ascontiguousarray(edges, dtype=np.int64)
+    nb = e.size - 1
+    count = np.zeros(nb, dtype=np.int64)
+    S = qzeros(nb)
+    lib().shdo_structure_factor_shells(d, int(N), M, pn, _q(rho_re), _q(rho_im), nb,
+                                       e.ctypes.data_as(C.POINTER(C.c_long)), count.ctypes.data_as(C.POINTER(C.c_long)), _q(S))
+    return count, S
 
 
 def tau(d, N, L, K, dev2) -> float:

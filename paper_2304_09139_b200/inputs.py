@@ -49,6 +49,10 @@ CONFIGS = {
     # the paper's own system size (d = 2, N = 2 x 10^6) at its smallest chi; context, not a
     # BASELINE.json config: one evaluation is 8 x 10^11 pair-terms and needs ~150 GB of phasor tables
     "paper01": Config("paper01", 2, 2_000_000, float.fromhex("0x1.618dab0184066p+10"), 0.10, 254626, 399996),
+    # the paper's other three chi: their phasor tables (up to 225 GB) are built chunk by chunk (shd_set_workspace)
+    "paper02": Config("paper02", 2, 2_000_000, float.fromhex("0x1.618dab0184066p+10"), 0.20, 509290, 800002),
+    "paper03": Config("paper03", 2, 2_000_000, float.fromhex("0x1.618dab0184066p+10"), 0.30, 763940, 1200000),
+    "paper04": Config("paper04", 2, 2_000_000, float.fromhex("0x1.618dab0184066p+10"), 0.40, 1018580, 1599996),
 }
 
 

@@ -461,3 +461,47 @@ def test_four_dimensions_direct_mode(oracle):
         fp = oracle.to_float(oracle.energy_grad(d, N, L, xp, lo, n, want_grad=False)["phi"])[0]
         fm = oracle.to_float(oracle.energy_grad(d, N, L, xm, lo, n, want_grad=False)["phi"])[0]
         assert abs((fp - fm) / (2 * h) - g[a, j]) < 1e-5 * (1 + abs(g[a, j]))
+
+
+def test_structure_factor_shells_pins(oracle):
+    """Radial average of S(k) (Fig. 2a, Fig. S1a), bins = ranges of the integer n.n.
+    Counts: a shell n.n = m of the square lattice holds r2(m) vectors, half of them in the half space (brute-force
+    count over the square here); the bins partition Q.  Values: single site => every mean is N exactly; perfect
+    lattice with its first reciprocal shell beyond the cutoff => every mean is 0; a bin that holds one wavevector
+    returns that wavevector's S(k); the count-weighted mean of the means is the plain mean of S over Q."""
+    d, N, L, m_star = 2, 128, inputs.CONFIGS["cfg1"].L, 49
+    n = oracle.enumerate_Q(d, m_star)
+    nn = (n.astype(np.int64) ** 2).sum(axis=1)
+    shells = np.unique(nn)
+    edges = np.concatenate([shells, [m_star + 1]])
+    hi, lo = inputs.uniform_positions(inputs.CONFIGS["cfg1"], 0)
+    re, im = oracle.rho(d, N, L, hi, lo, n)
+    count, Sm = oracle.structure_factor_shells(d, N, n, re, im, edges)
+    # brute-force r2(m) / 2
+    R = 8
+    g = np.arange(-R, R + 1)
+    a, b = np.meshgrid(g, g, indexing="ij")
+    allnn = (a * a + b * b).reshape(-1)
+    for m, c in zip(shells, count):
+        assert 2 * c == int((allnn == m).sum())
+    assert count.sum() == len(n)
+    S, _ = oracle.structure_factor(N, re, im)
+    Sf, Smf = oracle.to_float(S), oracle.to_float(Sm)
+    for m, c, v in zip(shells, count, Smf):
+        assert abs(v - Sf[nn == m].mean()) <= 1e-14 * max(1.0, v)
+    assert abs((count * Smf).sum() / count.sum() - Sf.mean()) <= 1e-13
+    # coarser bins: [1, 10), [10, 30), [30, 50) and an empty one [50, 60)
+    c2, S2 = oracle.structure_factor_shells(d, N, n, re, im, [1, 10, 30, 50, 60])
+    assert c2.tolist() == [int(((nn >= lo_) & (nn < hi_)).sum()) for lo_, hi_ in ((1, 10), (10, 30), (30, 50), (50, 60))]
+    assert c2[3] == 0 and oracle.to_float(S2)[3] == 0.0
+    assert abs(oracle.to_float(S2)[1] - Sf[(nn >= 10) & (nn < 30)].mean()) <= 1e-14
+    # single site: S(k) = N for every k
+    shi, slo = inputs.single_site(d, N, (1.2345, 7.0))
+    re, im = oracle.rho(d, N, L, shi, slo, n)
+    _, Sm = oracle.structure_factor_shells(d, N, n, re, im, edges)
+    assert oracle.absdiff_dd(Sm, np.full(len(shells), float(N)), np.zeros(len(shells))).max() <= 1e-28 * N
+    # perfect 16 x 8 lattice: rho = 0 on all of Q
+    lhi, llo = inputs.lattice((16, 8), L)
+    re, im = oracle.rho(d, N, L, lhi, llo, n)
+    _, Sm = oracle.structure_factor_shells(d, N, n, re, im, edges)
+    assert np.abs(oracle.to_float(Sm)).max() <= 1e-55
