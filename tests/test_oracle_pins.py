@@ -504,4 +504,4 @@ def test_structure_factor_shells_pins(oracle):
     lhi, llo = inputs.lattice((16, 8), L)
     re, im = oracle.rho(d, N, L, lhi, llo, n)
     _, Sm = oracle.structure_factor_shells(d, N, n, re, im, edges)
-    assert np.abs(oracle.to_float(Sm)).max() <= 1e-55
+    assert np.abs(oracle.to_float(Sm)).max() <= 1e-26      # (the lattice sites k L / 16 are rounded to doubles: |rho| ~ 1e-13)
