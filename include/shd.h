@@ -40,6 +40,7 @@ extern "C" {
 #define SHD_ENAN     -4   /* non-finite position or non-finite Phi                         */
 #define SHD_ESTALL   -5   /* shd_minimize: line search found no decrease (report written)  */
 #define SHD_EMAXEVAL -6   /* shd_minimize: max_evals reached before smax_tol (report written) */
+#define SHD_ESTOPPED -7   /* shd_minimize: stopped by the caller's poll callback (report written)  */
 
 typedef struct shd_ctx shd_ctx;
 
@@ -191,6 +192,34 @@ int shd_grad_local(shd_ctx* h, const double* pos_hi, const double* pos_lo, doubl
  */
 int shd_structure_factor(shd_ctx* h, double* S_out, double dev2[2]);
 
+/*
+ * Radially averaged structure factor of the LAST evaluation (Fig. 2a, Fig. S1a: S against |k|, beyond K when
+ * the handle's cutoff reaches there).  |k|^2 = (2 pi / L)^2 n.n, so a radial bin is a range of the integer n.n: bin b
+ * holds the wavevectors with edges[b] <= n.n < edges[b+1] (HOST, nbins + 1 strictly ascending longs; index work only,
+ * no floating-point compare).  HOST out: count[b] = members of bin b, S_mean (hi, lo)[b] = their mean S(k) in
+ * double-double, 0 for an empty bin (the half shell stands for the whole shell: S(-k) = S(k)).
+ * Errors: SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA.  Synchronises the stream.
+ */
+int shd_structure_factor_shells(shd_ctx* h, long nbins, const long* edges, long* count, double* S_mean_hi, double* S_mean_lo);
+
+/*
+ * Order metric tau of Eq. 7 from the LAST evaluation on this handle with D = 1/K, as the lattice sum over +-Q:
+ * tau = K^d V / N^2 * 2 * sum_{k in Q} (S(k) - 1)^2  (V = L^d), HOST (hi, lo).  The handle's own cutoff must reach far
+ * enough beyond K that S(k) has decayed to 1.  Errors: SHD_EINVAL, SHD_ECUDA.
+ */
+int shd_tau(shd_ctx* h, double K, double tau[2]);
+
+typedef struct {
+    long   iters, evals;
+    double phi[2], smax[2];
+    int    status;      /* SHD_OK, SHD_ESTALL, SHD_EMAXEVAL, SHD_ENAN, SHD_ESTOPPED */
+} shd_min_report;
+
+/* Host callback of shd_minimize, called after every poll (every poll_every iterations; the device is idle): report =
+ * the state so far (status = SHD_OK while running).  Return non-zero to stop (SHD_ESTOPPED).  shd_get_trace and
+ * shd_minimize_snapshot may be called from inside it (periodic log / checkpoint); nothing else on this handle. */
+typedef int (*shd_poll_fn)(const shd_min_report* report, void* user);
+
 typedef struct {
     int    kind;        /* 0 = L-BFGS (D:R12); 1 = FIRE                               */
     int    history;     /* L-BFGS pairs kept (1..32); 0 = default 10                          */
@@ -201,13 +230,26 @@ typedef struct {
                            0.1 / (k_max sqrt(2 N max v)): dt_max is half the explicit stability bound */
     int    resume;      /* FIRE only: 1 = continue the previous call on this handle (same positions
                            buffer content as it left): keep velocities, dt, alpha; 0 = fresh start    */
+    double ladder_tol[2]; /* precision ladder ("tunable precision"): evaluate with ONE limb
+                           (4 digits on the INT8 engines) until S_max < ladder_tol[0], with TWO limbs (7 digits) until
+                           S_max < ladder_tol[1], then at the handle's precision (shd_set_precision) down to smax_tol.
+                           0 = rung not used.  The device decides when a rung ends; the minimizer state (L-BFGS pairs,
+                           FIRE velocities) is kept across rungs, the first evaluation of a rung refreshes Phi and the
+                           gradient at the current point.  A line-search stall on a lower rung moves on to the next. */
+    shd_poll_fn on_poll;  /* optional host callback after every poll (NULL = none) */
+    void*  on_poll_user;
 } shd_min_opts;
 
+/* One record per evaluation of the last shd_minimize call, written by the device-side control kernel into a ring and
+ * collected by the host at every poll. */
 typedef struct {
-    long   iters, evals;
-    double phi[2], smax[2];
-    int    status;      /* SHD_OK, SHD_ESTALL, SHD_EMAXEVAL, SHD_ENAN */
-} shd_min_report;
+    long   iters, evals;   /* accepted iterations / evaluations so far (both cumulative over the call) */
+    double phi, smax;      /* Phi and S_max of THIS evaluation (the trial point) */
+    double gnorm;          /* |grad|_2 of this evaluation */
+    double step;           /* L-BFGS: step length t of the trial; FIRE: dt */
+    int    limbs;          /* precision of the evaluation (shd_set_precision levels; the ladder's rung) */
+    int    accepted;       /* L-BFGS: Armijo accepted; FIRE: P > 0 */
+} shd_trace_rec;
 
 /*
  * Quench: minimise Phi from pos (DEVICE, in/out, d*N doubles each) until S_max < smax_tol.
@@ -217,10 +259,20 @@ typedef struct {
  * kind 0: L-BFGS with Armijo backtracking (D:R12); the caller's buffer ends at the last accepted point.
  * kind 1: FIRE (ref.[37]) with the published default parameters, unit masses, semi-implicit Euler;
  *         report->iters counts MD steps; there is no step rejection, the buffer ends at the last point
- *         evaluated.  Returns report->status.
+ *         evaluated -- except on SHD_ENAN after at least one step, where it is restored to the last point with a
+ *         finite Phi (a too large fire_dt0 must not destroy the caller's state).  Returns report->status.
  */
 int shd_minimize(shd_ctx* h, double* pos_hi, double* pos_lo, const shd_min_opts* opts,
                  shd_min_report* report);
+
+/* Records first .. first + max - 1 of the last shd_minimize call's trace into out (HOST); returns how many were
+ * copied (0 when first is past the end; the trace keeps at most 2^22 records). */
+long shd_get_trace(shd_ctx* h, long first, long max, shd_trace_rec* out);
+
+/* During (from the poll callback) or after shd_minimize: the minimizer's current best point into pos_hi / pos_lo
+ * (DEVICE, d*N doubles each): L-BFGS: the last accepted point; FIRE: the current point.  Errors: SHD_EINVAL when no
+ * minimizer has run on this handle. */
+int shd_minimize_snapshot(shd_ctx* h, double* pos_hi, double* pos_lo);
 
 /* Text of the last error on this handle (never NULL). */
 const char* shd_last_error(const shd_ctx* h);

@@ -290,13 +290,42 @@ __global__ void __launch_bounds__(1024) k_sfactor2(const double* __restrict__ bl
     if (threadIdx.x == 0) { out[0] = r.phi.h; out[1] = r.phi.l; }
 }
 
+// Radially averaged S(k) (Fig. 2a, Fig. S1a): bin b holds the wavevectors order[start[b] .. start[b+1]) (the
+// host sorted them by their integer n.n; ascending k inside a bin).  One warp per bin: lane l adds members l, l+32, ...
+// in double-double, then the butterfly: a fixed tree, bit-reproducible.  mean = sum / count.
+__global__ void __launch_bounds__(128) k_sfactor_shells(long nbins, const long* __restrict__ start, const int* __restrict__ order,
+                                                        long M, long N, const double* __restrict__ rho,
+                                                        double* __restrict__ mean_hi, double* __restrict__ mean_lo)
+{
+    const long b = (long)blockIdx.x * 4 + (threadIdx.x >> 5);
+    if (b >= nbins) return;
+    const int lane = threadIdx.x & 31;
+    const long s0 = start[b], s1 = start[b + 1];
+    dd sum{0.0, 0.0};
+    for (long i = s0 + lane; i < s1; i += 32) {
+        const long k = order[i];
+        dd re{rho[k], rho[M + k]}, im{rho[2 * M + k], rho[3 * M + k]};
+        sum = dd_add(sum, dd_div_d(dd_add(dd_mul(re, re), dd_mul(im, im)), (double)N));
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        dd o{__shfl_xor_sync(0xffffffffu, sum.h, off), __shfl_xor_sync(0xffffffffu, sum.l, off)};
+        sum = dd_add(sum, o);
+    }
+    if (lane == 0) {
+        const dd m = s1 > s0 ? dd_div_d(sum, (double)(s1 - s0)) : dd{0.0, 0.0};
+        mean_hi[b] = m.h;
+        mean_lo[b] = m.l;
+    }
+}
+
 }  // namespace
 
 // S_out (device, M doubles) may be NULL; tau2 (device, 2 doubles) receives sum_k (S(k)-1)^2 as (hi, lo)
 cudaError_t shd_launch_sfactor(shd_ctx* h, double* S_out, double* scratch, double* tau2)
 {
     const int nb = (int)((h->M + 255) / 256);
-    k_sfactor1<<<nb, 256, 0, h->stream>>>(h->M, h->N, h->d_rho, S_out, scratch);
+    k_sfactor1<<<nb, 256, 0, h->stream>>>(h->M, h->Nsys, h->d_rho, S_out, scratch);
     k_sfactor2<<<1, 1024, 0, h->stream>>>(scratch, nb, tau2);
     h->last_launches += 2;
     return cudaGetLastError();
@@ -318,6 +347,13 @@ cudaError_t shd_launch_fold(shd_ctx* h, const double* part, int nparts, const do
         k_finish2<<<1, 1024, 0, h->stream>>>(h->d_blockred, nb, h->Nsys, h->d_scal, h->d_skip);
         h->last_launches += 1;
     }
+    return cudaGetLastError();
+}
+
+cudaError_t shd_launch_sfactor_shells(shd_ctx* h, long nbins, const long* d_start, const int* d_order, double* d_mean_hi, double* d_mean_lo)
+{
+    k_sfactor_shells<<<(unsigned)((nbins + 3) / 4), 128, 0, h->stream>>>(nbins, d_start, d_order, h->M, h->Nsys, h->d_rho, d_mean_hi, d_mean_lo);
+    h->last_launches += 1;
     return cudaGetLastError();
 }
 

@@ -677,7 +677,7 @@ void shd_destroy(shd_ctx* h) {
     cudaFree(h->d_pn0); cudaFree(h->d_pn1); cudaFree(h->d_pn2); cudaFree(h->d_wT); cudaFree(h->d_cell_kp); cudaFree(h->d_cell_km);
     cudaFree(h->d_tile_pb); cudaFree(h->d_tile_qb); cudaFree(h->d_tile_wmap); cudaFree(h->d_steps); cudaFree(h->d_v);
     cudaFree(h->d_rho); cudaFree(h->d_scal); cudaFree(h->d_hpos);
-    cudaFree(h->d_tile8_pb); cudaFree(h->d_tile8_qb); cudaFree(h->d_steps8); cudaFree(h->d_shell); cudaFree(h->d_trace);
+    cudaFree(h->d_tile8_pb); cudaFree(h->d_tile8_qb); cudaFree(h->d_steps8); cudaFree(h->d_trace);
     for (int i = 0; i <= SHD_NKERN; i++) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     if (h->h_scal) cudaFreeHost(h->h_scal);
     if (h->gevent) cudaEventDestroy(h->gevent);
@@ -877,6 +877,60 @@ int shd_structure_factor(shd_ctx* h, double* S_out, double dev2[2]) {
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     cudaFree(scratch);
     CU(e);
+    return SHD_OK;
+}
+
+int shd_structure_factor_shells(shd_ctx* h, long nbins, const long* edges, long* count, double* S_mean_hi, double* S_mean_lo) {
+    if (!h) return SHD_EINVAL;
+    if (nbins < 1 || !edges || !count || !S_mean_hi || !S_mean_lo) return fail(h, SHD_EINVAL, "shd_structure_factor_shells: bad argument");
+    for (long b = 0; b < nbins; b++)
+        if (!(edges[b] < edges[b + 1])) return fail(h, SHD_EINVAL, "shd_structure_factor_shells: edges must be strictly ascending");
+    // index work on the host (exact integers): the wavevectors of each bin, ascending k inside a bin
+    std::vector<long> start((size_t)nbins + 1, 0);
+    std::vector<int> bin((size_t)h->M);
+    for (long k = 0; k < h->M; k++) {
+        long nn = 0;
+        for (int a = 0; a < h->d; a++) nn += (long)h->nvec[k * h->d + a] * h->nvec[k * h->d + a];
+        const long b = (long)(std::upper_bound(edges, edges + nbins + 1, nn) - edges) - 1;      // edges[b] <= nn < edges[b+1]
+        bin[k] = (b >= 0 && b < nbins) ? (int)b : -1;
+        if (bin[k] >= 0) start[(size_t)b + 1]++;
+    }
+    for (long b = 0; b < nbins; b++) { count[b] = start[(size_t)b + 1]; start[(size_t)b + 1] += start[(size_t)b]; }
+    std::vector<int> order((size_t)std::max<long>(start[(size_t)nbins], 1));
+    std::vector<long> fill(start.begin(), start.end() - 1);
+    for (long k = 0; k < h->M; k++)
+        if (bin[k] >= 0) order[(size_t)fill[(size_t)bin[k]]++] = (int)k;
+    long* d_start = nullptr;
+    int* d_order = nullptr;
+    double* d_mean = nullptr;
+    cudaError_t e = cudaMalloc((void**)&d_start, start.size() * sizeof(long));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&d_order, order.size() * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&d_mean, (size_t)2 * nbins * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_start, start.data(), start.size() * sizeof(long), cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_order, order.data(), order.size() * sizeof(int), cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) e = shd_launch_sfactor_shells(h, nbins, d_start, d_order, d_mean, d_mean + nbins);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(S_mean_hi, d_mean, (size_t)nbins * sizeof(double), cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(S_mean_lo, d_mean + nbins, (size_t)nbins * sizeof(double), cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    cudaFree(d_start); cudaFree(d_order); cudaFree(d_mean);
+    CU(e);
+    return SHD_OK;
+}
+
+int shd_tau(shd_ctx* h, double K, double tau[2]) {
+    if (!h) return SHD_EINVAL;
+    if (!tau || !(K > 0.0) || !std::isfinite(K)) return fail(h, SHD_EINVAL, "shd_tau: bad argument");
+    double dev2[2];
+    int rc = shd_structure_factor(h, nullptr, dev2);
+    if (rc) return rc;
+    // tau = K^d V / N^2 * 2 * dev2 (Eq. 7 P:81 as a lattice sum, D = 1/K): prefactor in long double, product error-free
+    long double pref = 2.0L;
+    for (int a = 0; a < h->d; a++) pref *= (long double)K * (long double)h->L;
+    pref /= (long double)h->Nsys * (long double)h->Nsys;
+    const double ph = (double)pref, pl = (double)(pref - (long double)ph);
+    const double p = dev2[0] * ph, e = std::fma(dev2[0], ph, -p) + (dev2[0] * pl + dev2[1] * ph);
+    tau[0] = p + e;
+    tau[1] = e - (tau[0] - p);
     return SHD_OK;
 }
 

@@ -17,6 +17,8 @@
 
 #include <cmath>
 #include <cstring>
+#include <utility>
+#include <vector>
 
 constexpr int FIRE_THREADS = 256;
 constexpr int FIRE_EPT = 4;
@@ -29,6 +31,8 @@ struct shd_firectrl {
     double smax_tol;
     double dt[2], dt_max[2], alpha[2];   // dd: the step control is part of the arithmetic that is compared
     double a[2], b[2];   // this step's mixing: v <- a v - b g   (a = b = 0: v <- 0)
+    long long ring_n;    // trace records written so far
+    int ring_cap, limbs;
 };
 
 struct shd_firestate {
@@ -38,6 +42,10 @@ struct shd_firestate {
     double *partial = nullptr;             // [nblk][3][2]
     double *rank_part = nullptr, *rank_all = nullptr;   // sharded: [3][2] and [world][3][2]
     shd_firectrl *d_ctrl = nullptr, *h_ctrl = nullptr;
+    double *xprev = nullptr;               // [2][n]: the point before the last move (restored on SHD_ENAN)
+    double *pos_hi = nullptr, *pos_lo = nullptr;   // the caller's buffer of the running call (shd_minimize_snapshot)
+    shd_trace_rec *d_ring = nullptr, *h_ring = nullptr;
+    int ring_cap = 0;
 };
 
 namespace {
@@ -107,7 +115,8 @@ __global__ void __launch_bounds__(32) k_fire_rank_sum(int nblk, const shd_firect
 }
 
 __global__ void __launch_bounds__(32) k_fire_control(
-    int nblk, shd_firectrl* __restrict__ c, const shd_scalars* __restrict__ scal, const double* __restrict__ partial)
+    int nblk, shd_firectrl* __restrict__ c, const shd_scalars* __restrict__ scal, const double* __restrict__ partial,
+    shd_trace_rec* __restrict__ ring)
 {
     if (c->done) {
         if (threadIdx.x == 0) c->done = 2;
@@ -153,6 +162,14 @@ __global__ void __launch_bounds__(32) k_fire_control(
         }
         c->steps++;
     }
+    if (ring && c->ring_cap > 0) {               // one trace record per evaluation
+        shd_trace_rec& r = ring[c->ring_n % c->ring_cap];
+        r.iters = (long)c->steps; r.evals = (long)evals;
+        r.phi = scal->phi[0]; r.smax = scal->smax[0];
+        r.gnorm = sqrt(fmax(D[2].h, 0.0));
+        r.step = c->dt[0]; r.limbs = c->limbs; r.accepted = (a.h != 0.0 || b.h != 0.0) ? 1 : 0;
+        c->ring_n++;
+    }
     c->evals = evals;
     c->since = since;
     c->dt[0] = dt.h; c->dt[1] = dt.l; c->alpha[0] = alpha.h; c->alpha[1] = alpha.l;
@@ -163,11 +180,20 @@ __global__ void __launch_bounds__(32) k_fire_control(
 
 __global__ void __launch_bounds__(FIRE_THREADS) k_fire_update(
     long n, const shd_firectrl* __restrict__ c, double* __restrict__ x_hi, double* __restrict__ x_lo,
-    const double* __restrict__ g, double* __restrict__ v)
+    const double* __restrict__ g, double* __restrict__ v, double* __restrict__ xprev)
 {
-    if (c->done) return;
     const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c->done) {
+        // Phi went non-finite after at least one move (a too large time step): the caller gets the last point with a
+        // finite Phi back, at rest, instead of the diverged one
+        if (c->done == 1 && c->status == SHD_ENAN && c->steps > 0 && i < n) {
+            x_hi[i] = xprev[i]; x_lo[i] = xprev[n + i];
+            v[i] = 0.0; v[n + i] = 0.0;
+        }
+        return;
+    }
     if (i >= n) return;
+    xprev[i] = x_hi[i]; xprev[n + i] = x_lo[i];
     const dd gi = ld2(g, n, i);
     dd vi = ld2(v, n, i);
     const dd a{c->a[0], c->a[1]}, b{c->b[0], c->b[1]}, dt{c->dt[0], c->dt[1]};
@@ -196,6 +222,7 @@ int fire_alloc(shd_ctx* h) {
     const size_t v = (size_t)2 * s->n * sizeof(double);
     CUF(cudaMalloc((void**)&s->v, v));
     CUF(cudaMalloc((void**)&s->g, v));
+    CUF(cudaMalloc((void**)&s->xprev, v));
     CUF(cudaMalloc((void**)&s->partial, (size_t)s->nblk * 3 * 2 * sizeof(double)));
     if (shd_sharded(h)) {
         CUF(cudaMalloc((void**)&s->rank_part, 3 * 2 * sizeof(double)));
@@ -204,7 +231,7 @@ int fire_alloc(shd_ctx* h) {
     CUF(cudaMalloc((void**)&s->d_ctrl, sizeof(shd_firectrl)));
     CUF(cudaMallocHost((void**)&s->h_ctrl, sizeof(shd_firectrl)));
     std::memset(s->h_ctrl, 0, sizeof(shd_firectrl));
-    h->workspace_bytes += 2 * v;
+    h->workspace_bytes += 3 * v;
     return SHD_OK;
 }
 
@@ -214,9 +241,26 @@ void shd_fire_free(shd_ctx* h) {
     shd_firestate* s = h->fire;
     if (!s) return;
     cudaFree(s->v); cudaFree(s->g); cudaFree(s->partial); cudaFree(s->d_ctrl); cudaFree(s->rank_part); cudaFree(s->rank_all);
+    cudaFree(s->xprev); cudaFree(s->d_ring);
+    if (s->h_ring) cudaFreeHost(s->h_ring);
     if (s->h_ctrl) cudaFreeHost(s->h_ctrl);
     delete s;
     h->fire = nullptr;
+}
+
+std::vector<std::pair<int, double>> shd_ladder_rungs(const shd_ctx* h, const shd_min_opts* o);      // shd_min.cu
+bool shd_after_poll(shd_ctx* h, const shd_trace_rec* d_ring, shd_trace_rec* h_ring, int ring_cap, long long ring_n,
+                    long long& ring_seen, const shd_min_opts* opts, const shd_min_report& rep);
+
+int shd_fire_snapshot(shd_ctx* h, double* pos_hi, double* pos_lo) {
+    shd_firestate* s = h->fire;
+    if (!s || !s->pos_hi) { h->err = "shd_minimize_snapshot: no minimizer has run on this handle"; return SHD_EINVAL; }
+    const size_t b = (size_t)s->n * sizeof(double);
+    cudaStream_t st = h->gstream ? h->gstream : h->stream;
+    CUF(cudaMemcpyAsync(pos_hi, s->pos_hi, b, cudaMemcpyDeviceToDevice, st));
+    CUF(cudaMemcpyAsync(pos_lo, s->pos_lo, b, cudaMemcpyDeviceToDevice, st));
+    CUF(cudaStreamSynchronize(st));
+    return SHD_OK;
 }
 
 // kind == 1 of shd_minimize (shd_min.cu dispatches here)
@@ -233,6 +277,15 @@ int shd_fire_run(shd_ctx* h, double* pos_hi, double* pos_lo, const shd_min_opts*
     shd_firestate* s = h->fire;
     const long n = s->n;
     cudaStream_t st = h->stream;
+    s->pos_hi = pos_hi; s->pos_lo = pos_lo;
+    if (s->ring_cap < opts->poll_every) {
+        cudaFree(s->d_ring);
+        if (s->h_ring) cudaFreeHost(s->h_ring);
+        s->d_ring = nullptr; s->h_ring = nullptr;
+        s->ring_cap = opts->poll_every;
+        CUF(cudaMalloc((void**)&s->d_ring, sizeof(shd_trace_rec) * s->ring_cap));
+        CUF(cudaMallocHost((void**)&s->h_ring, sizeof(shd_trace_rec) * s->ring_cap));
+    }
     // default time step: the stiffest collective mode of Phi = sum v |rho|^2 has curvature ~ 2 N v k_max^2,
     // explicit integration is stable for dt < 2 / (k_max sqrt(2 N v)); dt_max = 10 dt0 sits at half of it
     double vmax = 1.0;
@@ -251,34 +304,58 @@ int shd_fire_run(shd_ctx* h, double* pos_hi, double* pos_lo, const shd_min_opts*
         c->dt[0] = dt0; c->dt_max[0] = 10.0 * dt0; c->alpha[0] = 0.1;     // 10 dt0 rounded to double, as the oracle
     }
     c->max_evals = opts->max_evals;
-    c->smax_tol = opts->smax_tol;
-    CUF(cudaMemcpyAsync(s->d_ctrl, c, sizeof(shd_firectrl), cudaMemcpyHostToDevice, st));
-    h->d_skip = &s->d_ctrl->done;
+    c->ring_cap = s->ring_cap;
     const unsigned ublk = (unsigned)((n + FIRE_THREADS - 1) / FIRE_THREADS);
     auto slot = [&]() -> cudaError_t {
         cudaError_t e;
         cudaStream_t q = h->stream;          // the capture stream while shd_run_slots is recording
-        h->last_launches = 0;
         if ((e = shd_enqueue_eval(h, pos_hi, pos_lo, s->g, s->g + n)) != cudaSuccess) return e;
         k_fire_dots<<<s->nblk, FIRE_THREADS, 0, q>>>(n, s->d_ctrl, s->g, s->v, s->partial);
-        if (shd_sharded(h)) {          // sharded vectors: rank sums, all-gathered as bytes, added in rank order (shd_min.cu)
+        if (shd_sharded(h)) {        // sharded vectors: rank sums, all-gathered as bytes, added in rank order (shd_min.cu)
             k_fire_rank_sum<<<1, 32, 0, q>>>(s->nblk, s->d_ctrl, s->partial, s->rank_part);
             if ((e = shd_comm_allgather(h, s->rank_part, s->rank_all, 3 * 16)) != cudaSuccess) return e;
-            k_fire_control<<<1, 32, 0, q>>>(h->world, s->d_ctrl, h->d_scal, s->rank_all);
+            k_fire_control<<<1, 32, 0, q>>>(h->world, s->d_ctrl, h->d_scal, s->rank_all, s->d_ring);
         } else
-            k_fire_control<<<1, 32, 0, q>>>(s->nblk, s->d_ctrl, h->d_scal, s->partial);
-        k_fire_update<<<ublk, FIRE_THREADS, 0, q>>>(n, s->d_ctrl, pos_hi, pos_lo, s->g, s->v);
+            k_fire_control<<<1, 32, 0, q>>>(s->nblk, s->d_ctrl, h->d_scal, s->partial, s->d_ring);
+        k_fire_update<<<ublk, FIRE_THREADS, 0, q>>>(n, s->d_ctrl, pos_hi, pos_lo, s->g, s->v, s->xprev);
         h->last_launches += 3;
         return cudaGetLastError();
     };
-    CUF(shd_run_slots(h, opts->poll_every, slot, c, s->d_ctrl, sizeof(shd_firectrl), &c->done));
-    h->d_skip = nullptr;
+    // the rungs of the precision ladder (shd_min.cu): velocities, dt and alpha carry over from rung to rung
+    const std::vector<std::pair<int, double>> rungs = shd_ladder_rungs(h, opts);
+    const int nlimb_user = h->nlimb;
+    long long ring_seen = 0;
+    bool stopped = false;
+    for (size_t r = 0; r < rungs.size(); r++) {
+        h->nlimb = rungs[r].first;
+        c->done = 0; c->status = SHD_OK;
+        c->smax_tol = rungs[r].second;
+        c->limbs = rungs[r].first;
+        cudaError_t ce = cudaMemcpyAsync(s->d_ctrl, c, sizeof(shd_firectrl), cudaMemcpyHostToDevice, st);
+        if (ce == cudaSuccess) {
+            h->d_skip = &s->d_ctrl->done;
+            ce = shd_run_slots(h, opts->poll_every, slot, c, s->d_ctrl, sizeof(shd_firectrl), &c->done, [&]() -> bool {
+                shd_min_report rp;
+                rp.iters = (long)c->steps; rp.evals = (long)c->evals;
+                rp.phi[0] = c->phi[0]; rp.phi[1] = c->phi[1]; rp.smax[0] = c->smax[0]; rp.smax[1] = c->smax[1];
+                rp.status = c->done ? c->status : SHD_OK;
+                stopped = shd_after_poll(h, s->d_ring, s->h_ring, s->ring_cap, c->ring_n, ring_seen, opts, rp) && !c->done;
+                return stopped;
+            });
+            h->d_skip = nullptr;
+        }
+        if (ce != cudaSuccess) { h->nlimb = nlimb_user; CUF(ce); }
+        if (stopped) { c->status = SHD_ESTOPPED; break; }
+        if (r + 1 == rungs.size() || c->status != SHD_OK) break;
+    }
+    h->nlimb = nlimb_user;
     report->iters = (long)c->steps;
     report->evals = (long)c->evals;
     report->phi[0] = c->phi[0]; report->phi[1] = c->phi[1];
     report->smax[0] = c->smax[0]; report->smax[1] = c->smax[1];
     report->status = c->status;
-    if (c->status == SHD_ENAN) h->err = "shd_minimize (FIRE): non-finite Phi";
+    if (c->status == SHD_ENAN) h->err = "shd_minimize (FIRE): non-finite Phi (the buffer holds the last point with a finite Phi)";
     else if (c->status == SHD_EMAXEVAL) h->err = "shd_minimize (FIRE): max_evals reached";
+    else if (c->status == SHD_ESTOPPED) h->err = "shd_minimize (FIRE): stopped by the poll callback";
     return c->status;
 }

@@ -28,6 +28,7 @@
 // inside a group  [limb 3][entry 32][index-in-group 4][re,im]  so that the 32 lanes of a warp
 // (entry = lane/4, index = lane%4) read one contiguous 512-byte run with LDS.128.
 #pragma once
+#include "../../include/shd.h"
 #include <cuda_runtime.h>
 #include <cstddef>
 #include <string>
@@ -92,8 +93,9 @@ struct shd_ctx {
     size_t table_bytes = 0;           // bytes held by the tables of the current (engine, chunk) setting
     void (*timing_mark)(shd_ctx*, int) = nullptr;   // set around a timed evaluation (shd_set_timing)
     std::vector<int> cell_kp, cell_km;              // host copies of the (p, q) -> k maps
-    int *d_shell = nullptr;           // radial shells of shd_structure_factor_shells (k_finish.cu)
-    void *d_trace = nullptr;          // device trace ring of the minimizers (shd_min.cu)
+    void *d_trace = nullptr;
+    std::vector<shd_trace_rec> trace; // trace of the last shd_minimize call, collected at every poll (shd_get_trace)
+    int last_min_kind = -1;           // minimizer of the last shd_minimize call (shd_minimize_snapshot)
     double L = 0;
     long m_star = 0;
     long M = 0;
@@ -185,6 +187,7 @@ cudaError_t shd_launch_grad8_main(shd_ctx* h, long nc);
 cudaError_t shd_launch_fold(shd_ctx* h, const double* part, int nparts, const double* xin, double* xout, bool fin);
 cudaError_t shd_launch_ctable(shd_ctx* h);
 cudaError_t shd_launch_sfactor(shd_ctx* h, double* S_out, double* scratch, double* tau2);
+cudaError_t shd_launch_sfactor_shells(shd_ctx* h, long nbins, const long* d_start, const int* d_order, double* d_mean_hi, double* d_mean_lo);
 cudaError_t shd_launch_grad(shd_ctx* h, long j_first, long nc, double* grad_hi, double* grad_lo);
 cudaError_t shd_tables_configure();
 cudaError_t shd_rho_configure();

@@ -16,9 +16,13 @@
 #include "shd_internal.h"
 #include "slots.cuh"
 
+#include <algorithm>
 #include <cstring>
+#include <utility>
+#include <vector>
 
 int shd_fire_run(shd_ctx* h, double* pos_hi, double* pos_lo, const shd_min_opts* opts, shd_min_report* report);
+std::vector<std::pair<int, double>> shd_ladder_rungs(const shd_ctx* h, const shd_min_opts* o);
 
 constexpr int MIN_MAXHIST = 32;
 constexpr int MIN_NBS = 2 * (MIN_MAXHIST + 1) + 1;   // basis stride of the Gram matrix
@@ -36,6 +40,8 @@ struct shd_minctrl {
     double smax_tol;
     double gamma;        // last H0 scaling s.y / y.y (persists across calls: first step of a continued quench)
     double delta[MIN_NBS][2];
+    long long ring_n;    // trace records written so far (ring index = ring_n % ring_cap)
+    int ring_cap, limbs;
 };
 
 struct shd_minstate {
@@ -48,6 +54,8 @@ struct shd_minstate {
     double *rank_part = nullptr, *rank_all = nullptr;                  // sharded: [NB][3][2] and [world][NB][3][2]
     double *G = nullptr;                                               // [MIN_NBS][MIN_NBS][2]
     shd_minctrl *d_ctrl = nullptr, *h_ctrl = nullptr;
+    shd_trace_rec *d_ring = nullptr, *h_ring = nullptr;                // device trace ring (poll_every records) and its pinned mirror
+    int ring_cap = 0;
 };
 
 namespace {
@@ -153,7 +161,7 @@ __device__ dd gram_dot(const dd* delta, const double* G, int NB, int c) {
 
 __global__ void __launch_bounds__(MIN_THREADS) k_min_control(
     int nblk, shd_minctrl* __restrict__ c, const shd_scalars* __restrict__ scal, const double* __restrict__ partial,
-    double* __restrict__ G)
+    double* __restrict__ G, shd_trace_rec* __restrict__ ring)
 {
     if (c->done) {
         if (threadIdx.x == 0) c->done = 2;
@@ -295,6 +303,14 @@ __global__ void __launch_bounds__(MIN_THREADS) k_min_control(
     if (!done && evals >= c->max_evals) { done = 1; status = SHD_EMAXEVAL; }
     __syncwarp();
     if (lane == 0) {
+        if (ring && c->ring_cap > 0) {           // one trace record per evaluation (collected by the host at every poll)
+            shd_trace_rec& r = ring[c->ring_n % c->ring_cap];
+            r.iters = (long)c->iters; r.evals = (long)evals;
+            r.phi = phi_t.h; r.smax = smax_t.h;
+            r.gnorm = sqrt(fmax(D[2 * MIN_NBS + gidx].h, 0.0));
+            r.step = c->t[0]; r.limbs = c->limbs; r.accepted = accepted;
+            c->ring_n++;
+        }
         c->evals = evals;
         c->first = 0;
         c->accepted = accepted;
@@ -393,16 +409,66 @@ void shd_min_free(shd_ctx* h) {
     if (!s) return;
     cudaFree(s->x); cudaFree(s->g); cudaFree(s->gt); cudaFree(s->p); cudaFree(s->S); cudaFree(s->Y);
     cudaFree(s->partial); cudaFree(s->G); cudaFree(s->d_ctrl); cudaFree(s->rank_part); cudaFree(s->rank_all);
+    cudaFree(s->d_ring);
+    if (s->h_ring) cudaFreeHost(s->h_ring);
     if (s->h_ctrl) cudaFreeHost(s->h_ctrl);
     delete s;
     h->min = nullptr;
+}
+
+// rungs of the precision ladder: (limbs, stop below this S_max); the last rung is the handle's own precision down to tol
+std::vector<std::pair<int, double>> shd_ladder_rungs(const shd_ctx* h, const shd_min_opts* o) {
+    std::vector<std::pair<int, double>> r;
+    const double l0 = o->ladder_tol[0], l1 = o->ladder_tol[1];
+    if (h->nlimb > 1 && l0 > 0.0 && l0 > std::max(l1, o->smax_tol)) r.push_back({1, l0});
+    if (h->nlimb > 2 && l1 > 0.0 && l1 > o->smax_tol) r.push_back({2, l1});
+    r.push_back({h->nlimb, o->smax_tol});
+    return r;
+}
+
+// host side of a poll: new trace records from the device ring into h->trace, then the caller's callback
+bool shd_after_poll(shd_ctx* h, const shd_trace_rec* d_ring, shd_trace_rec* h_ring, int ring_cap, long long ring_n,
+                    long long& ring_seen, const shd_min_opts* opts, const shd_min_report& rep) {
+    if (d_ring && ring_n > ring_seen) {
+        if (cudaMemcpyAsync(h_ring, d_ring, sizeof(shd_trace_rec) * ring_cap, cudaMemcpyDeviceToHost, h->stream) == cudaSuccess &&
+            cudaStreamSynchronize(h->stream) == cudaSuccess) {
+            for (long long i = std::max(ring_seen, ring_n - ring_cap); i < ring_n; i++)
+                if (h->trace.size() < ((size_t)1 << 22)) h->trace.push_back(h_ring[i % ring_cap]);
+        }
+        ring_seen = ring_n;
+    }
+    return opts->on_poll && opts->on_poll(&rep, opts->on_poll_user) != 0;
+}
+
+extern "C" long shd_get_trace(shd_ctx* h, long first, long max, shd_trace_rec* out) {
+    if (!h || !out || first < 0 || max < 1 || (size_t)first >= h->trace.size()) return 0;
+    const long n = (long)std::min<size_t>((size_t)max, h->trace.size() - (size_t)first);
+    std::memcpy(out, h->trace.data() + first, sizeof(shd_trace_rec) * (size_t)n);
+    return n;
+}
+
+int shd_fire_snapshot(shd_ctx* h, double* pos_hi, double* pos_lo);
+
+extern "C" int shd_minimize_snapshot(shd_ctx* h, double* pos_hi, double* pos_lo) {
+    if (!h) return SHD_EINVAL;
+    if (!pos_hi || !pos_lo) return min_fail(h, SHD_EINVAL, "NULL pointer");
+    if (h->last_min_kind == 1) return shd_fire_snapshot(h, pos_hi, pos_lo);
+    if (h->last_min_kind != 0 || !h->min) return min_fail(h, SHD_EINVAL, "shd_minimize_snapshot: no minimizer has run on this handle");
+    const size_t b = (size_t)h->min->n * sizeof(double);
+    cudaStream_t st = h->gstream ? h->gstream : h->stream;      // (from the poll callback: the minimizers' own stream)
+    CUM(cudaMemcpyAsync(pos_hi, h->min->x, b, cudaMemcpyDeviceToDevice, st));
+    CUM(cudaMemcpyAsync(pos_lo, h->min->x + h->min->n, b, cudaMemcpyDeviceToDevice, st));
+    CUM(cudaStreamSynchronize(st));
+    return SHD_OK;
 }
 
 extern "C" int shd_minimize(shd_ctx* h, double* pos_hi, double* pos_lo, const shd_min_opts* opts,
                             shd_min_report* report) {
     if (!h) return SHD_EINVAL;
     if (!pos_hi || !pos_lo || !opts || !report) return min_fail(h, SHD_EINVAL, "NULL pointer");
-    if (opts->kind == 1) return shd_fire_run(h, pos_hi, pos_lo, opts, report);
+    if (!(opts->ladder_tol[0] >= 0.0) || !(opts->ladder_tol[1] >= 0.0)) return min_fail(h, SHD_EINVAL, "bad ladder_tol");
+    h->trace.clear();
+    if (opts->kind == 1) { h->last_min_kind = 1; return shd_fire_run(h, pos_hi, pos_lo, opts, report); }
     if (opts->kind != 0) return min_fail(h, SHD_EINVAL, "shd_minimize: kind must be 0 (L-BFGS) or 1 (FIRE)");
     const int m = opts->history == 0 ? 10 : opts->history;
     if (m < 1 || m > MIN_MAXHIST) return min_fail(h, SHD_EINVAL, "history must be in 1..32");
@@ -411,10 +477,19 @@ extern "C" int shd_minimize(shd_ctx* h, double* pos_hi, double* pos_lo, const sh
     int rc = min_alloc(h, m);
     if (rc) return rc;
     if ((rc = shd_prepare_tables(h, true))) return rc;
+    h->last_min_kind = 0;
     shd_minstate* s = h->min;
     const long n = s->n;
     const size_t v = (size_t)2 * n * sizeof(double);
     cudaStream_t st = h->stream;
+    if (s->ring_cap < opts->poll_every) {
+        cudaFree(s->d_ring);
+        if (s->h_ring) cudaFreeHost(s->h_ring);
+        s->d_ring = nullptr; s->h_ring = nullptr;
+        s->ring_cap = opts->poll_every;
+        CUM(cudaMalloc((void**)&s->d_ring, sizeof(shd_trace_rec) * s->ring_cap));
+        CUM(cudaMallocHost((void**)&s->h_ring, sizeof(shd_trace_rec) * s->ring_cap));
+    }
     CUM(cudaMemsetAsync(s->x, 0, v, st)); CUM(cudaMemsetAsync(s->g, 0, v, st));
     CUM(cudaMemsetAsync(s->p, 0, v, st));
     CUM(cudaMemsetAsync(s->S, 0, v * (m + 1), st)); CUM(cudaMemsetAsync(s->Y, 0, v * (m + 1), st));
@@ -422,18 +497,13 @@ extern "C" int shd_minimize(shd_ctx* h, double* pos_hi, double* pos_lo, const sh
     const double gamma_prev = s->h_ctrl->gamma;      // 0 on a fresh state (min_alloc zeroes it)
     std::memset(s->h_ctrl, 0, sizeof(shd_minctrl));
     s->h_ctrl->gamma = gamma_prev;
-    s->h_ctrl->first = 1;
     s->h_ctrl->m = m;
     s->h_ctrl->max_evals = opts->max_evals;
-    s->h_ctrl->smax_tol = opts->smax_tol;
-    s->h_ctrl->t[0] = 1.0;
-    CUM(cudaMemcpyAsync(s->d_ctrl, s->h_ctrl, sizeof(shd_minctrl), cudaMemcpyHostToDevice, st));
-    h->d_skip = &s->d_ctrl->done;
+    s->h_ctrl->ring_cap = s->ring_cap;
     const unsigned ublk = (unsigned)((n + MIN_THREADS - 1) / MIN_THREADS);
     auto slot = [&]() -> cudaError_t {
         cudaError_t e;
         cudaStream_t q = h->stream;          // the capture stream while shd_run_slots is recording
-        h->last_launches = 0;
         if ((e = shd_enqueue_eval(h, pos_hi, pos_lo, s->gt, s->gt + n)) != cudaSuccess) return e;
         k_min_dots<<<s->nblk, MIN_THREADS, 0, q>>>(n, m, s->d_ctrl, pos_hi, pos_lo, s->x, s->gt, s->g,
                                                    s->S, s->Y, s->partial);
@@ -443,17 +513,53 @@ extern "C" int shd_minimize(shd_ctx* h, double* pos_hi, double* pos_lo, const sh
             const int nq = 3 * (2 * (m + 1) + 1);
             k_rank_sum<<<(nq + 63) / 64, 64, 0, q>>>(s->nblk, nq, s->partial, s->rank_part, &s->d_ctrl->done);
             if ((e = shd_comm_allgather(h, s->rank_part, s->rank_all, (size_t)nq * 16)) != cudaSuccess) return e;
-            k_min_control<<<1, MIN_THREADS, 0, q>>>(h->world, s->d_ctrl, h->d_scal, s->rank_all, s->G);
+            k_min_control<<<1, MIN_THREADS, 0, q>>>(h->world, s->d_ctrl, h->d_scal, s->rank_all, s->G, s->d_ring);
         } else
-            k_min_control<<<1, MIN_THREADS, 0, q>>>(s->nblk, s->d_ctrl, h->d_scal, s->partial, s->G);
+            k_min_control<<<1, MIN_THREADS, 0, q>>>(s->nblk, s->d_ctrl, h->d_scal, s->partial, s->G, s->d_ring);
         k_min_update<<<ublk, MIN_THREADS, 0, q>>>(n, m, s->d_ctrl, pos_hi, pos_lo, s->x, s->gt, s->g,
                                                   s->p, s->S, s->Y);
         h->last_launches += 3;
         return cudaGetLastError();
     };
-    CUM(shd_run_slots(h, opts->poll_every, slot, s->h_ctrl, s->d_ctrl, sizeof(shd_minctrl), &s->h_ctrl->done));
-    h->d_skip = nullptr;
-    const shd_minctrl* c = s->h_ctrl;
+    // ---- the rungs of the precision ladder (one rung when opts->ladder_tol is zero): the device decides when a rung
+    // ends (S_max below its threshold, or the line search stalls at the rung's precision floor); the pairs, the Gram
+    // matrix and the counters carry over, the first slot of a rung re-evaluates Phi and the gradient at the current point
+    const std::vector<std::pair<int, double>> rungs = shd_ladder_rungs(h, opts);
+    const int nlimb_user = h->nlimb;
+    shd_minctrl* c = s->h_ctrl;
+    long long ring_seen = 0;
+    bool stopped = false;
+    for (size_t r = 0; r < rungs.size(); r++) {
+        h->nlimb = rungs[r].first;
+        c->done = 0; c->status = SHD_OK; c->first = 1; c->accepted = 0; c->ls_fails = 0;
+        c->t[0] = 1.0; c->t[1] = 0.0;
+        c->smax_tol = rungs[r].second;
+        c->limbs = rungs[r].first;
+        cudaError_t ce = cudaMemcpyAsync(s->d_ctrl, c, sizeof(shd_minctrl), cudaMemcpyHostToDevice, st);
+        if (ce == cudaSuccess) {
+            h->d_skip = &s->d_ctrl->done;
+            ce = shd_run_slots(h, opts->poll_every, slot, c, s->d_ctrl, sizeof(shd_minctrl), &c->done, [&]() -> bool {
+                shd_min_report rp;
+                rp.iters = (long)c->iters; rp.evals = (long)c->evals;
+                rp.phi[0] = c->phi[0]; rp.phi[1] = c->phi[1]; rp.smax[0] = c->smax[0]; rp.smax[1] = c->smax[1];
+                rp.status = c->done ? c->status : SHD_OK;
+                stopped = shd_after_poll(h, s->d_ring, s->h_ring, s->ring_cap, c->ring_n, ring_seen, opts, rp) && !c->done;
+                return stopped;
+            });
+            h->d_skip = nullptr;
+        }
+        if (ce != cudaSuccess) { h->nlimb = nlimb_user; CUM(ce); }
+        if (stopped) {
+            // the caller's buffer holds a trial point: put the last accepted one back (k_min_update's exit path)
+            c->done = 1; c->status = SHD_ESTOPPED; c->accepted = 0;
+            CUM(cudaMemcpyAsync(s->d_ctrl, c, sizeof(shd_minctrl), cudaMemcpyHostToDevice, st));
+            k_min_update<<<ublk, MIN_THREADS, 0, st>>>(n, m, s->d_ctrl, pos_hi, pos_lo, s->x, s->gt, s->g, s->p, s->S, s->Y);
+            CUM(cudaStreamSynchronize(st));
+            break;
+        }
+        if (r + 1 == rungs.size() || !(c->status == SHD_OK || c->status == SHD_ESTALL)) break;
+    }
+    h->nlimb = nlimb_user;
     report->iters = (long)c->iters;
     report->evals = (long)c->evals;
     report->phi[0] = c->phi[0]; report->phi[1] = c->phi[1];
@@ -462,5 +568,6 @@ extern "C" int shd_minimize(shd_ctx* h, double* pos_hi, double* pos_lo, const sh
     if (c->status == SHD_ENAN) h->err = "shd_minimize: non-finite Phi at the starting point";
     else if (c->status == SHD_ESTALL) h->err = "shd_minimize: line search found no decrease";
     else if (c->status == SHD_EMAXEVAL) h->err = "shd_minimize: max_evals reached";
+    else if (c->status == SHD_ESTOPPED) h->err = "shd_minimize: stopped by the poll callback";
     return c->status;
 }

@@ -9,9 +9,11 @@
 #pragma once
 #include "shd_internal.h"
 
-template <class EnqueueSlot>
+// after_poll(): host hook run after every poll (control block already in h_ctrl, stream idle): fetches the trace ring,
+// calls the caller's callback; returns true to stop replaying.
+template <class EnqueueSlot, class AfterPoll>
 cudaError_t shd_run_slots(shd_ctx* h, int poll_every, EnqueueSlot enqueue_slot, void* h_ctrl, const void* d_ctrl,
-                          size_t ctrl_bytes, const int* h_done)
+                          size_t ctrl_bytes, const int* h_done, AfterPoll after_poll)
 {
     cudaError_t e;
     if (!h->gstream) {
@@ -36,7 +38,8 @@ cudaError_t shd_run_slots(shd_ctx* h, int poll_every, EnqueueSlot enqueue_slot, 
         if ((e = cudaGraphLaunch(exec, gs)) != cudaSuccess) break;
         if ((e = cudaMemcpyAsync(h_ctrl, d_ctrl, ctrl_bytes, cudaMemcpyDeviceToHost, gs)) != cudaSuccess) break;
         if ((e = cudaStreamSynchronize(gs)) != cudaSuccess) break;
-        if (*h_done) break;
+        const bool stop = after_poll();
+        if (*h_done || stop) break;
     }
     if (exec) cudaGraphExecDestroy(exec);
     if (graph) cudaGraphDestroy(graph);

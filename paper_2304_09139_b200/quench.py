@@ -1,13 +1,14 @@
 """Quench one BASELINE.json configuration from its seeded random start to S_max < tol.
 
     python -m paper_2304_09139_b200.quench --config cfg4 [--seed 0] [--tol 1e-30] [--max-evals 20000]
-                                           [--kind 0|1] [--weight one|n2] [--history 10] [--chunk 500]
+                                           [--kind 0|1] [--weight one|n2] [--history 10] [--ladder1 1e-6 --ladder 1e-24]
                                            [--out file.json]
 
-The whole iteration runs on the device (shd_minimize); this script only calls it in chunks of
-``--chunk`` evaluations (shd_minimize is re-entrant) to log the S_max / Phi trajectory, and
-prints one JSON line at the end.  ``--save prefix`` writes the final positions as
-``prefix_hi.npy`` / ``prefix_lo.npy`` (axis-major, x[a*N + j]).
+ONE shd_minimize call: the whole iteration runs on the device, the precision ladder (--ladder1 / --ladder) switches
+rungs inside the library, the device writes a trace record per evaluation (shd_get_trace), and the poll callback of the
+call logs progress and writes periodic checkpoints (shd_minimize_snapshot).  One JSON line at the end.  ``--save prefix``
+writes the final positions as ``prefix_hi.npy`` / ``prefix_lo.npy`` (axis-major, x[a*N + j]); with
+``--checkpoint-every K`` also every K polls while running.
 """
 from __future__ import annotations
 
@@ -29,15 +30,19 @@ def main(argv=None):
     ap.add_argument("--max-evals", type=int, default=20000)
     ap.add_argument("--kind", type=int, default=0, help="0 = L-BFGS, 1 = FIRE")
     ap.add_argument("--history", type=int, default=10)
-    ap.add_argument("--chunk", type=int, default=500)
     ap.add_argument("--poll-every", type=int, default=16)
     ap.add_argument("--weight", default="one", choices=["one", "n2"],
                     help="v(k): 'one' = the step potential of BASELINE.json's configs; 'n2' = 1/|n|^2 "
                          "(P:50: any positive v has the same ground states; S_max does not depend on v; "
                          "SURVEY.md 8(f) NEXT-1: it removes the k^2 ill-conditioning, decisive in d = 1)")
     ap.add_argument("--fire-dt0", type=float, default=0.0)
-    ap.add_argument("--engine", type=int, default=0, choices=[0, 1, 2],
-                    help="engine of the O(N M) passes (shd_set_engine): 0 FP64 limbs, 1 rho on the INT8 tensor cores, 2 both")
+    ap.add_argument("--engine", type=int, default=-1, choices=[-1, 0, 1, 2],
+                    help="engine of the O(N M) passes (shd_set_engine): -1 the library's choice, 0 FP64 limbs, 1 rho on the "
+                         "INT8 tensor cores, 2 both")
+    ap.add_argument("--workspace-gb", type=float, default=0.0, help="cap on the phasor tables (shd_set_workspace); 0 = what fits")
+    ap.add_argument("--log-every", type=int, default=32, help="progress line every this many polls (0 = none)")
+    ap.add_argument("--checkpoint-every", type=int, default=0,
+                    help="with --save: write the minimizer's current best point every this many polls")
     ap.add_argument("--ladder", type=float, default=0.0,
                     help="precision ladder (P:77 'tunable precision'; SURVEY.md 8(f) NEXT-1): evaluate with two "
                          "limbs (shd_set_precision 2) until S_max < this value, e.g. 1e-18, then with three")
@@ -53,57 +58,59 @@ def main(argv=None):
 
     cfg = inputs.CONFIGS[args.config]
     hi, lo = inputs.uniform_positions(cfg, args.seed)
+    v = None
     h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
     if args.weight == "n2":
         n = h.k().astype(np.float64)
         h.close()
-        h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star, v=1.0 / (n * n).sum(axis=1))
-    h.set_engine(args.engine)
+        v = 1.0 / (n * n).sum(axis=1)
+        h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star, v=v)
+    if args.engine >= 0:
+        h.set_engine(args.engine)          # default: the library's own choice
+    if args.workspace_gb > 0:
+        h.set_workspace(int(args.workspace_gb * 2 ** 30))
     pos_hi, pos_lo = shd.from_host(hi, lo)
     phi0, _, _ = h.energy_grad(pos_hi, pos_lo, want_grad=False)
     smax0, _ = h.last_smax()
-    trace = [{"evals": 0, "iters": 0, "phi": phi0[0], "smax": smax0[0], "seconds": 0.0}]
-    evals = iters = 0
-    status = shd.SHD_EMAXEVAL
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    # rungs: (limbs, stop below this S_max); the last rung is always 3 limbs down to --tol
-    # (on the INT8 engines the rungs are digit counts: 4, 7 and 13 base-256 digits)
-    rungs = [(1, args.ladder1)] if args.ladder1 > max(args.ladder, args.tol) else []
-    if args.ladder > args.tol:
-        rungs.append((2, args.ladder))
-    rungs.append((3, args.tol))
-    rung = 0
-    h.set_precision(rungs[0][0])
-    while evals < args.max_evals:
-        fast = rung < len(rungs) - 1
-        rep = h.minimize(pos_hi, pos_lo, kind=args.kind, history=args.history,
-                         smax_tol=rungs[rung][1],
-                         max_evals=min(args.chunk, args.max_evals - evals), poll_every=args.poll_every,
-                         resume=evals > 0, fire_dt0=args.fire_dt0)
-        evals += rep["evals"]
-        iters += rep["iters"]
-        status = rep["status"]
-        trace.append({"evals": evals, "iters": iters, "phi": rep["phi"][0], "smax": rep["smax"][0],
-                      "seconds": time.perf_counter() - t0})
-        print(f"[quench {cfg.name}] evals={evals} iters={iters} Phi={rep['phi'][0]:.6e} "
-              f"S_max={rep['smax'][0]:.6e} t={trace[-1]['seconds']:.1f}s", file=sys.stderr, flush=True)
-        if fast and status in (shd.SHD_OK, shd.SHD_ESTALL):
-            rung += 1                         # next rung: more limbs from here on
-            h.set_precision(rungs[rung][0])
-            trace[-1]["switched_to_limbs"] = rungs[rung][0]
-            status = shd.SHD_EMAXEVAL
-            continue
-        if status != shd.SHD_EMAXEVAL:
-            break
+    polls = [0]
+
+    def on_poll(rep):
+        """host side of a poll: a progress line every --log-every polls, a checkpoint every --checkpoint-every polls"""
+        polls[0] += 1
+        if args.log_every > 0 and polls[0] % args.log_every == 0:
+            print(f"[quench {cfg.name}] evals={rep['evals']} iters={rep['iters']} Phi={rep['phi'][0]:.6e} "
+                  f"S_max={rep['smax'][0]:.6e} t={time.perf_counter() - t0:.1f}s", file=sys.stderr, flush=True)
+        if args.save and args.checkpoint_every > 0 and polls[0] % args.checkpoint_every == 0:
+            sh, sl = h.minimize_snapshot()
+            np.save(args.save + "_hi.npy", sh.cpu().numpy())
+            np.save(args.save + "_lo.npy", sl.cpu().numpy())
+        return False
+
+    rep = h.minimize(pos_hi, pos_lo, kind=args.kind, history=args.history, smax_tol=args.tol,
+                     max_evals=args.max_evals, poll_every=args.poll_every, fire_dt0=args.fire_dt0,
+                     ladder=(args.ladder1, args.ladder), on_poll=on_poll)
+    torch.cuda.synchronize()
     seconds = time.perf_counter() - t0
+    status, evals, iters = rep["status"], rep["evals"], rep["iters"]
+    tr = h.trace()
+    # the trace the device wrote (one record per evaluation), thinned to <= 400 points for the JSON line
+    keep = np.unique(np.concatenate([np.linspace(0, len(tr) - 1, min(len(tr), 400)).astype(np.int64),
+                                     np.nonzero(np.diff(tr["limbs"]))[0] + 1])) if len(tr) else []
+    trace = [{"evals": int(tr["evals"][i]), "iters": int(tr["iters"][i]), "phi": float(tr["phi"][i]),
+              "smax": float(tr["smax"][i]), "gnorm": float(tr["gnorm"][i]), "step": float(tr["step"][i]),
+              "limbs": int(tr["limbs"][i])} for i in keep]
+    by_limbs = {int(l): int((tr["limbs"] == l).sum()) for l in np.unique(tr["limbs"])} if len(tr) else {}
     smax, arg = h.smax(pos_hi, pos_lo)
     n = h.k()
     line = {"config": cfg.name, "d": cfg.d, "N": cfg.N, "M": cfg.M, "chi_realised": cfg.M / (cfg.d * (cfg.N - 1)),
-            "seed": args.seed, "kind": "lbfgs" if args.kind == 0 else "fire", "weight": args.weight, "engine": args.engine, "history": args.history,
-            "tol": args.tol, "ladder": args.ladder, "ladder1": args.ladder1, "status": status, "evals": evals, "iters": iters, "seconds": seconds,
+            "seed": args.seed, "kind": "lbfgs" if args.kind == 0 else "fire", "weight": args.weight, "engine": h.engine,
+            "chunks": int(h.stat(19)), "history": args.history,
+            "tol": args.tol, "ladder": args.ladder, "ladder1": args.ladder1, "status": status, "evals": evals, "iters": iters,
+            "evals_by_limbs": by_limbs, "seconds": seconds,
             "ms_per_eval": 1e3 * seconds / max(evals, 1), "phi_start": phi0[0], "smax_start": smax0[0],
-            "phi_final": trace[-1]["phi"], "smax_final": smax[0], "argmax_n": n[arg].tolist(), "trace": trace}
+            "phi_final": rep["phi"][0], "smax_final": smax[0], "argmax_n": n[arg].tolist(), "trace": trace}
     if args.save:
         np.save(args.save + "_hi.npy", pos_hi.cpu().numpy())
         np.save(args.save + "_lo.npy", pos_lo.cpu().numpy())

@@ -14,12 +14,12 @@ import numpy as np
 _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libshd.so"
 
-SHD_OK, SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA, SHD_ENAN, SHD_ESTALL, SHD_EMAXEVAL = 0, -1, -2, -3, -4, -5, -6
+SHD_OK, SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA, SHD_ENAN, SHD_ESTALL, SHD_EMAXEVAL, SHD_ESTOPPED = 0, -1, -2, -3, -4, -5, -6, -7
 EXPORTS = ["shd_create", "shd_create_shell", "shd_create_table", "shd_destroy", "shd_set_stream", "shd_num_k", "shd_get_k",
            "shd_energy_grad", "shd_energy_grad_host", "shd_set_timing", "shd_smax", "shd_last_smax", "shd_get_rho", "shd_minimize",
            "shd_last_error", "shd_stat", "shd_fp64_peak", "shd_structure_factor", "shd_set_precision", "shd_i8_probe", "shd_set_engine",
            "shd_set_workspace", "shd_set_shard", "shd_comm_unique_id", "shd_comm_init", "shd_partial_bytes", "shd_rho_partial", "shd_rho_finish",
-           "shd_grad_local"]
+           "shd_grad_local", "shd_structure_factor_shells", "shd_tau", "shd_get_trace", "shd_minimize_snapshot"]
 
 
 class ShdError(RuntimeError):
@@ -28,15 +28,24 @@ class ShdError(RuntimeError):
         self.code = code
 
 
-class shd_min_opts(C.Structure):
-    _fields_ = [("kind", C.c_int), ("history", C.c_int), ("smax_tol", C.c_double),
-                ("max_evals", C.c_long), ("poll_every", C.c_int), ("fire_dt0", C.c_double),
-                ("resume", C.c_int)]
-
-
 class shd_min_report(C.Structure):
     _fields_ = [("iters", C.c_long), ("evals", C.c_long), ("phi", C.c_double * 2),
                 ("smax", C.c_double * 2), ("status", C.c_int)]
+
+
+shd_poll_fn = C.CFUNCTYPE(C.c_int, C.POINTER(shd_min_report), C.c_void_p)
+
+
+class shd_min_opts(C.Structure):
+    _fields_ = [("kind", C.c_int), ("history", C.c_int), ("smax_tol", C.c_double),
+                ("max_evals", C.c_long), ("poll_every", C.c_int), ("fire_dt0", C.c_double),
+                ("resume", C.c_int), ("ladder_tol", C.c_double * 2), ("on_poll", shd_poll_fn),
+                ("on_poll_user", C.c_void_p)]
+
+
+class shd_trace_rec(C.Structure):
+    _fields_ = [("iters", C.c_long), ("evals", C.c_long), ("phi", C.c_double), ("smax", C.c_double),
+                ("gnorm", C.c_double), ("step", C.c_double), ("limbs", C.c_int), ("accepted", C.c_int)]
 
 
 def _load():
@@ -79,6 +88,11 @@ def _load():
     lib.shd_rho_partial.argtypes = [vp, vp, vp, vp]
     lib.shd_rho_finish.argtypes = [vp, vp, C.c_int, dp]
     lib.shd_grad_local.argtypes = [vp, vp, vp, vp, vp]
+    lib.shd_structure_factor_shells.argtypes = [vp, C.c_long, C.POINTER(C.c_long), C.POINTER(C.c_long), dp, dp]
+    lib.shd_tau.argtypes = [vp, C.c_double, dp]
+    lib.shd_get_trace.argtypes = [vp, C.c_long, C.c_long, C.POINTER(shd_trace_rec)]
+    lib.shd_get_trace.restype = C.c_long
+    lib.shd_minimize_snapshot.argtypes = [vp, vp, vp]
     return lib
 
 
@@ -261,22 +275,71 @@ class Shd:
         return S, (dev2[0], dev2[1])
 
     def tau(self, K):
-        """Order metric tau of Eq. 7 from the last evaluation on this handle, D = 1/K, as the
-        lattice sum over +-Q:  tau = K^d V / N^2 * 2 sum_{k in Q} (S(k) - 1)^2  (V = L^d).  The handle's
-        own cutoff must reach far enough beyond K that S(k) has decayed to 1."""
-        _, (hi, lo) = self.structure_factor(want_S=False)
-        return float(K) ** self.d * self.L ** self.d / float(self.N) ** 2 * 2.0 * (hi + lo)
+        """shd_tau: order metric tau of Eq. 7 from the last evaluation on this handle, D = 1/K (hi + lo)."""
+        t = (C.c_double * 2)()
+        self._check(lib.shd_tau(self._h, float(K), t))
+        return t[0] + t[1]
+
+    def structure_factor_shells(self, edges=None):
+        """shd_structure_factor_shells on the last evaluation.  edges: ascending integer n.n bin edges (default: one bin
+        per distinct shell of this handle's Q).  Returns (edges, count, S_mean_hi, S_mean_lo) as numpy arrays."""
+        if edges is None:
+            nn = (self.k().astype(np.int64) ** 2).sum(axis=1)
+            sh = np.unique(nn)
+            edges = np.concatenate([sh, [sh[-1] + 1]])
+        e = np.ascontiguousarray(edges, dtype=np.int64)
+        nb = e.size - 1
+        count = np.zeros(nb, dtype=np.int64)
+        hi, lo = np.zeros(nb), np.zeros(nb)
+        lp, dp = C.POINTER(C.c_long), C.POINTER(C.c_double)
+        self._check(lib.shd_structure_factor_shells(self._h, nb, e.ctypes.data_as(lp), count.ctypes.data_as(lp),
+                                                    hi.ctypes.data_as(dp), lo.ctypes.data_as(dp)))
+        return e, count, hi, lo
 
     def minimize(self, pos_hi, pos_lo, kind=0, history=10, smax_tol=1e-30, max_evals=10000, poll_every=8,
-                 fire_dt0=0.0, resume=False):
-        """shd_minimize: kind 0 = L-BFGS, 1 = FIRE (fire_dt0 = 0: the library's default time step)."""
+                 fire_dt0=0.0, resume=False, ladder=(0.0, 0.0), on_poll=None):
+        """shd_minimize: kind 0 = L-BFGS, 1 = FIRE (fire_dt0 = 0: the library's default time step).
+        ladder = (S_max below which one limb / 4 digits is left, S_max below which two limbs / 7 digits are left);
+        on_poll(report dict) -> truthy to stop: host callback after every poll (trace / snapshot may be read in it)."""
         ph, pl = self._pos(pos_hi, pos_lo)
-        opts = shd_min_opts(kind, history, smax_tol, max_evals, poll_every, fire_dt0, 1 if resume else 0)
+        cb = shd_poll_fn()
+        if on_poll is not None:
+            def _cb(rep, _user):
+                r = rep.contents
+                return 1 if on_poll(dict(iters=int(r.iters), evals=int(r.evals), phi=(r.phi[0], r.phi[1]),
+                                         smax=(r.smax[0], r.smax[1]), status=int(r.status))) else 0
+            cb = shd_poll_fn(_cb)
+        opts = shd_min_opts(kind, history, smax_tol, max_evals, poll_every, fire_dt0, 1 if resume else 0,
+                            (C.c_double * 2)(float(ladder[0]), float(ladder[1])), cb, None)
         rep = shd_min_report()
         rc = lib.shd_minimize(self._h, ph, pl, C.byref(opts), C.byref(rep))
-        self._check(rc, ok=(SHD_OK, SHD_ESTALL, SHD_EMAXEVAL))
+        self._check(rc, ok=(SHD_OK, SHD_ESTALL, SHD_EMAXEVAL, SHD_ESTOPPED))
         return dict(status=rc, iters=int(rep.iters), evals=int(rep.evals),
                     phi=(rep.phi[0], rep.phi[1]), smax=(rep.smax[0], rep.smax[1]))
+
+    def trace(self, first=0, max_records=1 << 22):
+        """shd_get_trace: records of the last minimize call as a numpy structured array."""
+        dt = np.dtype([("iters", "i8"), ("evals", "i8"), ("phi", "f8"), ("smax", "f8"), ("gnorm", "f8"), ("step", "f8"),
+                       ("limbs", "i4"), ("accepted", "i4")])
+        assert dt.itemsize == C.sizeof(shd_trace_rec)
+        out, got = [], 0
+        while got < max_records:
+            buf = np.zeros(min(65536, max_records - got), dtype=dt)
+            k = int(lib.shd_get_trace(self._h, first + got, len(buf), buf.ctypes.data_as(C.POINTER(shd_trace_rec))))
+            out.append(buf[:k])
+            got += k
+            if k < len(buf):
+                break
+        return np.concatenate(out) if out else np.zeros(0, dtype=dt)
+
+    def minimize_snapshot(self, pos_hi=None, pos_lo=None):
+        """shd_minimize_snapshot: the minimizer's current best point (device tensors), e.g. from on_poll for a checkpoint."""
+        torch = _torch()
+        if pos_hi is None:
+            pos_hi = torch.empty(self.d * self.N, dtype=torch.float64, device="cuda")
+            pos_lo = torch.empty_like(pos_hi)
+        self._check(lib.shd_minimize_snapshot(self._h, C.c_void_p(pos_hi.data_ptr()), C.c_void_p(pos_lo.data_ptr())))
+        return pos_hi, pos_lo
 
     def stat(self, what: int) -> float:
         return float(lib.shd_stat(self._h, int(what)))

@@ -277,3 +277,98 @@ def test_cfg4_quench_reaches_1e30(shd, oracle):
     assert abs(s_hi - s_or) <= 1e-3 * s_or
     assert oracle.to_float(o_phi)[0] <= rep["phi"][0] * (1 + 1e-3) + 1e-40
     h.close()
+
+
+@pytest.mark.parametrize("kind,engine", [(0, 2), (0, 0), (1, 2)])
+def test_ladder_inside_the_library(shd, oracle, kind, engine):
+    """opts->ladder_tol ("tunable precision"): ONE shd_minimize call walks the rungs
+    4 digits / 1 limb -> 7 digits / 2 limbs -> full precision, the device deciding when a rung ends and the minimizer
+    state carried across; outcome judged by the oracle; the device-written trace shows the rungs in order."""
+    cfg = inputs.CONFIGS["cfg2"]
+    hi, lo = inputs.uniform_positions(cfg, 1)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    h.set_engine(engine)
+    th, tl = shd.from_host(hi, lo)
+    rep = h.minimize(th, tl, kind=kind, smax_tol=1e-30, max_evals=20000, poll_every=16, ladder=(1e-6, 1e-18))
+    assert rep["status"] == shd.SHD_OK, rep
+    tr = h.trace()
+    assert len(tr) == rep["evals"] and np.array_equal(tr["evals"], np.arange(1, rep["evals"] + 1))
+    limbs = tr["limbs"]
+    assert limbs[0] == 1 and limbs[-1] == 3 and np.all(np.diff(limbs) >= 0), "rungs in order"
+    n1, n2, n3 = [(limbs == l).sum() for l in (1, 2, 3)]
+    assert n1 > 10 and n2 > 10 and n3 > 10
+    # a rung ends the first time S_max falls below its threshold (or the line search stalls at its precision floor)
+    assert tr["smax"][limbs == 1][:-1].min() >= 1e-6 or kind == 0
+    s_or, _ = oracle_smax(oracle, cfg.d, cfg.N, cfg.L, cfg.m_star, th.cpu().numpy(), tl.cpu().numpy())
+    print("ladder in library", kind, engine, rep["evals"], (n1, n2, n3), s_or)
+    assert s_or < 1e-30
+    # the handle's own precision setting is untouched by the ladder
+    phi3, _, _ = h.energy_grad(th, tl, want_grad=False)
+    assert phi3[0] == rep["phi"][0] and phi3[1] == rep["phi"][1]
+    h.close()
+
+
+def test_trace_callback_snapshot_stop(shd, oracle):
+    """The device-side trace ring (one record per evaluation, collected at every poll), the host poll callback, the
+    snapshot of the last accepted point from inside it (periodic checkpoint) and stopping from it (SHD_ESTOPPED: the
+    caller's buffer must hold the last accepted point, not a trial point)."""
+    cfg = inputs.CONFIGS["cfg1"]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    check = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    th, tl = shd.from_host(hi, lo)
+    polls, snaps = [], []
+
+    def on_poll(rep):
+        polls.append(rep)
+        if len(polls) in (3, 7):
+            a, b = h.minimize_snapshot()
+            snaps.append((rep, a.clone(), b.clone(), len(h.trace())))
+        return len(polls) >= 9
+
+    rep = h.minimize(th, tl, smax_tol=1e-30, max_evals=5000, poll_every=5, on_poll=on_poll)
+    assert rep["status"] == shd.SHD_ESTOPPED and len(polls) == 9 and rep["evals"] == 45
+    assert [p["evals"] for p in polls] == [5 * (i + 1) for i in range(9)]
+    tr = h.trace()
+    assert len(tr) == 45 and np.array_equal(tr["evals"], np.arange(1, 46))
+    assert np.all(tr["gnorm"] > 0) and np.all(tr["step"] > 0) and set(tr["limbs"]) == {3}
+    # Phi of accepted evaluations never increases
+    acc = tr["phi"][tr["accepted"] == 1]
+    assert np.all(np.diff(acc) <= 0)
+    # snapshots taken inside the callback are the accepted points reported at those polls
+    for r, a, b, ntr in snaps:
+        assert ntr == r["evals"]
+        phi, _, _ = check.energy_grad(a, b, want_grad=False)
+        assert phi == r["phi"]
+    # stopped: the buffer holds the last accepted point
+    phi, _, _ = check.energy_grad(th, tl, want_grad=False)
+    assert phi == rep["phi"] and phi == polls[-1]["phi"]
+    # continuing from there still converges, and FIRE's trace works too
+    rep2 = h.minimize(th, tl, smax_tol=1e-30, max_evals=5000)
+    assert rep2["status"] == shd.SHD_OK
+    assert len(h.trace()) == rep2["evals"]
+    th2, tl2 = shd.from_host(hi, lo)
+    rep3 = h.minimize(th2, tl2, kind=1, smax_tol=1e-12, max_evals=3000, poll_every=50)
+    tr3 = h.trace()
+    assert rep3["status"] == shd.SHD_OK and len(tr3) == rep3["evals"] and tr3["step"][0] > 0
+    h.close(); check.close()
+
+
+def test_fire_nonfinite_restores_the_last_finite_point(shd):
+    """FIRE integrates in place; when a (far too large) time step drives Phi non-finite the caller must get
+    the last point with a finite Phi back, not the diverged one."""
+    cfg = inputs.CONFIGS["cfg1"]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    th, tl = shd.from_host(hi, lo)
+    with pytest.raises(shd.ShdError) as e:
+        h.minimize(th, tl, kind=1, fire_dt0=1e300, max_evals=50)
+    assert e.value.code == shd.SHD_ENAN
+    x = th.cpu().numpy()
+    assert np.all(np.isfinite(x)) and np.all(np.isfinite(tl.cpu().numpy()))
+    phi, _, _ = h.energy_grad(th, tl, want_grad=False)
+    assert np.isfinite(phi[0])
+    # and the state is usable: a sane run from there converges
+    rep = h.minimize(th, tl, kind=1, smax_tol=1e-12, max_evals=5000)
+    assert rep["status"] == shd.SHD_OK
+    h.close()

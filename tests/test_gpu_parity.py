@@ -545,3 +545,42 @@ def test_engine_selection_is_the_librarys(shd):
         h.set_engine(-1)
         assert h.engine == e and h.stat(27) == 1
         h.close()
+
+
+def test_structure_factor_shells(shd, oracle):
+    """Radially averaged S(k) (Fig. 2a, Fig. S1a) on a handle whose cutoff reaches to 2 K: the bin counts are
+    index work (bit-exact against the oracle), the bin means double-double sums (against the binary128 means); one bin
+    per shell (the default) and a handful of coarse bins with an empty one; single-site closed form S = N."""
+    cfg = inputs.CONFIGS["cfg2"]
+    m_big = 4 * cfg.m_star
+    hi, lo = inputs.uniform_positions(cfg, 4)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=m_big)
+    th, tl = shd.from_host(hi, lo)
+    h.energy_grad(th, tl, want_grad=False)
+    n = oracle.enumerate_Q(cfg.d, m_big)
+    rho = [t.cpu().numpy() for t in h.rho()]
+    fr, fi = oracle.from_dd(rho[0], rho[1]), oracle.from_dd(rho[2], rho[3])     # the device's own rho: the binning is what is tested
+    edges, count, s_hi, s_lo = h.structure_factor_shells()
+    o_count, o_S = oracle.structure_factor_shells(cfg.d, cfg.N, n, fr, fi, edges)
+    assert np.array_equal(count, o_count) and count.sum() == len(n) and len(count) > 3000
+    assert oracle.absdiff_dd(o_S, s_hi, s_lo).max() <= 1e-29 * cfg.N
+    coarse = [1, 100, cfg.m_star + 1, 2 * cfg.m_star, m_big + 1, m_big + 50]
+    e2, c2, h2, l2 = h.structure_factor_shells(coarse)
+    oc2, oS2 = oracle.structure_factor_shells(cfg.d, cfg.N, n, fr, fi, coarse)
+    assert np.array_equal(c2, oc2) and c2[-1] == 0 and h2[-1] == 0.0
+    assert oracle.absdiff_dd(oS2, h2, l2).max() <= 1e-29 * cfg.N
+    # ideal-gas start: the mean over a wide bin is close to 1 (P:83)
+    assert abs(h2[3] - 1.0) < 0.05
+    # against the oracle's own rho on one coarse bin (ties the whole chain to the definition)
+    ks = np.nonzero(((n.astype(np.int64) ** 2).sum(axis=1) >= 1) & ((n.astype(np.int64) ** 2).sum(axis=1) < 100))[0]
+    re, im = oracle.rho(cfg.d, cfg.N, cfg.L, hi, lo, n[ks])
+    _, oS = oracle.structure_factor_shells(cfg.d, cfg.N, n[ks], re, im, [1, 100])
+    assert oracle.absdiff_dd(oS, h2[:1], l2[:1])[0] <= 1e-27 * cfg.N
+    with pytest.raises(shd.ShdError):
+        h.structure_factor_shells([5, 5, 9])
+    shi, slo = inputs.single_site(cfg.d, cfg.N, (3.25, 41.0))
+    th, tl = shd.from_host(shi, slo)
+    h.energy_grad(th, tl, want_grad=False)
+    _, _, s_hi, s_lo = h.structure_factor_shells()
+    assert np.abs(s_hi + s_lo - cfg.N).max() <= 1e-24 * cfg.N
+    h.close()
