@@ -131,8 +131,8 @@ int shd_set_precision(shd_ctx* h, int limbs);
  *   1: the rho pass on the INT8 tensor cores, the gradient pass on the FP64 limbs.
  *   0: exact FP64 limb contraction on the FP64 matrix instruction (k_rho.cu, k_grad.cu).
  *  -1: the library's own choice, which is also what shd_create* starts with: engine 2 when the last-axis table has at
- *      least 48 and at most 5024 entries and one evaluation is at least 5e7 pair-terms, engine 0 otherwise (short last
- *      axes, as in d = 3, leave the 16-q tensor-core steps mostly empty; tiny systems are launch-bound either way).
+ *      most 5024 entries and one evaluation is at least 5e7 pair-terms, engine 0 otherwise (tiny systems are
+ *      launch-bound either way).
  * shd_set_precision selects the number of digits on the INT8 engines.  The tables of an engine are allocated on first
  * use and those of the engine left behind are freed.  Errors: SHD_EINVAL (engine not -1..2; engine 2 with more than 5024
  * entries in the last-axis table; no particle split keeps the s32 sums exact: the handle's engine is then unchanged),

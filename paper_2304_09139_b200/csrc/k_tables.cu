@@ -52,6 +52,18 @@ __device__ cdd expi_turns(dd t) {
     return cdd_mul(root, w);
 }
 
+// z^e by binary powering (start of a chunk of a power table: ~2 log2(e) complex dd products; the phase error of the
+// result is e times the base's, as for the recurrence)
+__device__ cdd cdd_pow(cdd z, int e) {
+    cdd r{dd{1.0, 0.0}, dd{0.0, 0.0}};
+    while (e > 0) {
+        if (e & 1) r = cdd_mul(r, z);
+        e >>= 1;
+        if (e) z = cdd_mul(z, z);
+    }
+    return r;
+}
+
 struct limbs { double x0, x1, x2; };
 
 // The 13 balanced base-256 digits d_i in [-128, 127] of X = trunc(x 2^102), x = hi + lo, |x| <= 1 (a few ulps more
@@ -297,9 +309,13 @@ __global__ void __launch_bounds__(TB) k_tables(
     const double* __restrict__ pos_hi, const double* __restrict__ pos_lo,
     double* __restrict__ A, double* __restrict__ B, double* __restrict__ Bg, int with_grad,
     signed char* __restrict__ A8, signed char* __restrict__ B8, long nk8, signed char* __restrict__ Bg8, int nkq8,
-    ulonglong2* __restrict__ Afix, long NpadA, const int* __restrict__ skip)
+    ulonglong2* __restrict__ Afix, long NpadA, int ech, const int* __restrict__ skip)
 {
     if (skip && *skip) return;
+    // blockIdx.z: chunk of `ech` table entries (a multiple of 8).  With few particles one thread per particle walking the
+    // whole table is a long serial recurrence on a mostly idle GPU, so the entries are dealt out over blockIdx.z and every
+    // chunk starts from the base's power (cdd_pow); with many particles ech covers the whole table (one chunk).
+    const int e_begin = blockIdx.z * ech;
     extern __shared__ __align__(16) unsigned char tables_smem[];
     double2* tile = reinterpret_cast<double2*>(tables_smem);
     const int which = blockIdx.y;
@@ -323,10 +339,12 @@ __global__ void __launch_bounds__(TB) k_tables(
         cdd base;
         if (d == 1) base = expi_turns(frac_turns(pos_hi[jc], pos_lo[jc], L, (double)S1d));
         else base = expi_turns(frac_turns(pos_hi[jc], pos_lo[jc], L, 1.0));
+        const int e_end = min(P, e_begin + ech);
+        if (e_begin >= P) return;
         if (d <= 2) {
-            cdd cur = one;
-            for (int p0 = 0; p0 < P; p0 += TG) {
-                const int cnt = min(TG, P - p0);
+            cdd cur = e_begin == 0 ? one : cdd_pow(base, e_begin);
+            for (int p0 = e_begin; p0 < e_end; p0 += TG) {
+                const int cnt = min(TG, e_end - p0);
                 if (cnt == TG) {
                     // full group: slots known at compile time (no selects in the byte staging), and the integer
                     // work of one entry overlaps the serial double-double recurrence of the next
@@ -349,21 +367,21 @@ __global__ void __launch_bounds__(TB) k_tables(
             cdd z1 = expi_turns(frac_turns(pos_hi[N + jc], pos_lo[N + jc], L, 1.0));
             cdd pw1[R3MAX + 1];
             int r1max = 0;
-            for (int p = 0; p < P; p++) { int a = abs(pn1[p]); r1max = a > r1max ? a : r1max; }
+            for (int p = e_begin; p < e_end; p++) { int a = abs(pn1[p]); r1max = a > r1max ? a : r1max; }
             pw1[0] = one;
             for (int m = 1; m <= r1max; m++) pw1[m] = cdd_mul(pw1[m - 1], z1);
             cdd pw2[R4MAX + 1];                      // d == 4: powers of the third axis' base phasor
             if (d == 4) {
                 cdd z2 = expi_turns(frac_turns(pos_hi[2 * N + jc], pos_lo[2 * N + jc], L, 1.0));
                 int r2max = 0;
-                for (int p = 0; p < P; p++) { int a = abs(pn2[p]); r2max = a > r2max ? a : r2max; }
+                for (int p = e_begin; p < e_end; p++) { int a = abs(pn2[p]); r2max = a > r2max ? a : r2max; }
                 pw2[0] = one;
                 for (int m = 1; m <= r2max; m++) pw2[m] = cdd_mul(pw2[m - 1], z2);
             }
-            cdd cur0 = one;
-            int n0cur = 0;
-            for (int p0 = 0; p0 < P; p0 += TG) {
-                const int cnt = min(TG, P - p0);
+            int n0cur = pn0[e_begin];
+            cdd cur0 = n0cur == 0 ? one : cdd_pow(base, n0cur);
+            for (int p0 = e_begin; p0 < e_end; p0 += TG) {
+                const int cnt = min(TG, e_end - p0);
                 for (int s = 0; s < cnt; s++) {
                     const int n0 = pn0[p0 + s], n1 = pn1[p0 + s];
                     while (n0cur < n0) { cur0 = cdd_mul(cur0, base); n0cur++; }
@@ -383,9 +401,11 @@ __global__ void __launch_bounds__(TB) k_tables(
         // ---- B table: powers of the last axis' base phasor
         const int a = d - 1;
         cdd base = expi_turns(frac_turns(pos_hi[(size_t)a * N + jc], pos_lo[(size_t)a * N + jc], L, 1.0));
-        cdd cur = one;
-        for (int q0 = 0; q0 < Qn; q0 += TG) {
-            const int cnt = min(TG, Qn - q0);
+        const int e_end = min(Qn, e_begin + ech);
+        if (e_begin >= Qn) return;
+        cdd cur = e_begin == 0 ? one : cdd_pow(base, e_begin);
+        for (int q0 = e_begin; q0 < e_end; q0 += TG) {
+            const int cnt = min(TG, e_end - q0);
             if (cnt == TG) {
 #pragma unroll
                 for (int s = 0; s < TG; s++) {
@@ -422,7 +442,11 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
     const bool rho = (what & 1) != 0, grad = (what & 2) != 0;
     // every slot of the chunk's tables is written (zeros beyond the handle's last particle)
     const long slots = std::max(std::max(h->Npad, h->nk8 * 32), std::max(h->njb128 * 128, h->njb64 * 64));
-    dim3 grid((unsigned)((slots + TB - 1) / TB), 2);
+    // entries per chunk (blockIdx.z): the whole table when the particles alone fill the GPU, else 32-entry chunks
+    const int emax = std::max(h->P, h->Qn);
+    int ech = ((emax + 7) / 8) * 8;
+    if (slots < 96 * 1024 && emax > 32) ech = slots < 24 * 1024 ? 16 : 32;
+    dim3 grid((unsigned)((slots + TB - 1) / TB), 2, (unsigned)((emax + ech - 1) / ech));
     double* A = (e == 2 || !(rho || grad)) ? nullptr : ((e == 1 && !grad) ? nullptr : h->d_A);   // FP64 rho pass and FP64 gradient pass
     double* B = (e == 0 && rho) ? h->d_B : nullptr;
     double* Bg = (e != 2 && grad) ? h->d_Bg : nullptr;
@@ -433,7 +457,7 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
 #define LAUNCH_TABLES(DLOV)                                                                                       \
     k_tables<DLOV><<<grid, TB, TABLES_SMEM, h->stream>>>(h->d, h->N, j_first, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2, \
                                          h->d_pn0, h->d_pn1, h->d_pn2, h->Qpad, pos_hi, pos_lo, A, B, Bg, grad ? 1 : 0, \
-                                         A8, B8, h->nk8, Bg8, h->nkq8, Afix, h->njb128 * 128, h->d_skip)
+                                         A8, B8, h->nk8, Bg8, h->nkq8, Afix, h->njb128 * 128, ech, h->d_skip)
     // the INT8 engines read only the 13, 7 or 4 most significant digits (shd_set_precision): the rest is not written
     if (e == 0 || h->nlimb >= 3) LAUNCH_TABLES(0);
     else if (h->nlimb == 2) LAUNCH_TABLES(6);

@@ -565,12 +565,13 @@ cudaError_t shd_enqueue_eval(shd_ctx* h, const double* pos_hi, const double* pos
 namespace {
 
 // The engine a fresh handle starts on: both O(N M) passes on the INT8 tensor cores (engine 2) where they pay off --
-// a last-axis table long enough to fill the 16-q K-steps and short enough for exact s32 sums, and enough pair-terms
-// to amortise the digit tables -- else the FP64 limb engine.  shd_set_engine overrides.
+// a last-axis table short enough for exact s32 sums and enough pair-terms to amortise the digit tables (measured on
+// B200: cfg2, 8e7 pair-terms, 0.23 ms against 0.44 ms; cfg3, d = 3 with an 18-entry last axis, 0.61 against 0.95 ms;
+// cfg1, 9e3 pair-terms, is launch-bound either way) -- else the FP64 limb engine.  shd_set_engine overrides.
 void auto_engine(shd_ctx* h) {
     h->engine_auto = 1;
     const bool fits8 = (long)h->Qpad * 2 * SHD_I8_DIGITS * 16384 < (1L << 31);
-    const bool pays = (double)h->N * (double)h->M >= 5e7 && h->Qn >= 48;
+    const bool pays = (double)h->N * (double)h->M >= 5e7;
     if (fits8 && pays && plan_engine8(h, 2) == SHD_OK) h->rho_engine = 2;
     else { h->rho_engine = 0; h->err.clear(); }
 }

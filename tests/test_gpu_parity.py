@@ -533,8 +533,8 @@ def test_smax_entry_point(shd, oracle):
 
 def test_engine_selection_is_the_librarys(shd):
     """A fresh handle runs on the engine the library chooses (include/shd.h, shd_set_engine): INT8 tensor cores for the
-    large d <= 2 workloads, FP64 limbs for short last axes (d = 3) and tiny systems; -1 restores the choice."""
-    want = {"cfg1": 0, "cfg2": 2, "cfg3": 0, "cfg4": 2, "cfg5": 2}
+    workloads of at least 5e7 pair-terms, FP64 limbs for tiny systems; -1 restores the choice."""
+    want = {"cfg1": 0, "cfg2": 2, "cfg3": 2, "cfg4": 2, "cfg5": 2}
     for name, e in want.items():
         cfg = inputs.CONFIGS[name]
         h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
