@@ -373,6 +373,8 @@ def run_gpu(args, cfg):
                                "back on all SMs; MEASURED_PEAKS.json bf16 x 2 (nominal int8 : bf16) for comparison",
                 "peak_from_measured_bf16_x2": 2.0 * float(mp["bf16_tflops"]) if "bf16_tflops" in mp else None,
                 "i8_products_exact": i8_bad == 0,
+                # why k_grad8's epilogue is integer arithmetic: FP64 beside a tcgen05.mma.kind::i8 stream (shd_mix_probe)
+                "alu_beside_mma": shd.mix_probe(),
                 "kernel_ms": dom_ms, "algorithmic_mac_per_pair": mac,
                 "whole_eval_frac": pairs_rank * (ALG_MAC_RHO8 + ALG_MAC_GRAD8) * 2.0 / (total_ms / args.steps * 1e-3) / 1e12 / i8_tops,
                 "kernel_ms_all": {k: v / args.steps for k, v in kms.items()},

@@ -47,6 +47,15 @@ int shd_fp64_peak(int kind, double seconds, double instr_per_s[2]);
  */
 int shd_i8_probe(double* tops, long* mismatches);
 
+/*
+ * FP64 and integer ALU work beside a tcgen05.mma.kind::i8 stream on the same SM (the measurement behind the integer
+ * epilogue of k_grad8).  HOST out[8]: [0] cycles per DADD per warp, 16 warps of dependent chains alone;
+ * [1] the same while a back-to-back M=128 N=256 K=32 stream runs on the SM; [2], [3] the same for IMAD chains;
+ * [4] cycles per N = 256 instruction alone, [5] beside the DADD chains, [6] beside the IMAD chains; [7] SM clock in MHz
+ * during the stream (clock64 against globaltimer).  Needs no handle.
+ */
+int shd_mix_probe(double out[8]);
+
 #ifdef __cplusplus
 }
 #endif

@@ -184,6 +184,118 @@ __global__ void __launch_bounds__(128) k_i8_probe(const signed char* A, const si
 
 }  // namespace
 
+// ---------------------------------------------------------------------------------------------------
+// FP64 under a tcgen05.mma.kind::i8 stream (the measurement behind k_grad8's integer epilogue): one CTA
+// per SM; warp 16 issues M=128 N=256 K=32 instructions back to back, warps 0..15 run dependent chains (4 per thread)
+// of DADD (KIND 0) or IMAD (KIND 1).  The chains are sized to outlast the MMA stream, so the progress they make WHILE
+// it runs follows from the two durations.  Also the SM clock under that load (clock64 against globaltimer).
+namespace {
+template <int KIND>
+__global__ void __launch_bounds__(544) k_mix_probe(int mma_iters, int alu_iters, long long* out, double* sink)
+{
+    __shared__ __align__(1024) signed char sA[2][128 * 32];
+    __shared__ __align__(1024) signed char sB[2][256 * 32];
+    __shared__ __align__(8) unsigned long long bar;
+    __shared__ uint32_t tmem_base;
+    const int tid = threadIdx.x, warp = tid >> 5;
+    for (int i = tid; i < 2 * 128 * 32; i += blockDim.x) (&sA[0][0])[i] = (signed char)(i % 7 - 3);
+    for (int i = tid; i < 2 * 256 * 32; i += blockDim.x) (&sB[0][0])[i] = (signed char)(i % 5 - 2);
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(p_smem_u32(&bar)));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(p_smem_u32(&tmem_base)));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const uint32_t tb = tmem_base;
+    if (warp == 16) {
+        if (tid == 512) {
+            unsigned long long g0, g1;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));
+            const long long t0 = clock64();
+            const uint32_t idesc = p_idesc(128, 256);
+            for (int it = 0; it < mma_iters; it++)
+#pragma unroll
+                for (int kb = 0; kb < 4; kb++)
+                    p_mma_i8(tb + ((it & 1) ? 256u : 0u), p_desc(p_smem_u32(&sA[kb & 1][0])), p_desc(p_smem_u32(&sB[kb & 1][0])),
+                             idesc, (it | kb) ? 1u : 0u);
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(p_smem_u32(&bar)) : "memory");
+            p_wait(p_smem_u32(&bar));
+            const long long t1 = clock64();
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
+            if (blockIdx.x == 0) { out[1] = t1 - t0; out[2] = (long long)(g1 - g0); }
+        }
+    } else {
+        const long long t0 = clock64();
+        if (KIND == 0) {
+            double a0 = tid, a1 = tid + 1, a2 = tid + 2, a3 = tid + 3;
+            for (int it = 0; it < alu_iters; it++)
+#pragma unroll
+                for (int u = 0; u < 16; u++) {
+                    a0 = __dadd_rn(a0, 1e-9); a1 = __dadd_rn(a1, 1e-9); a2 = __dadd_rn(a2, 1e-9); a3 = __dadd_rn(a3, 1e-9);
+                }
+            if (a0 + a1 + a2 + a3 == 1.2345) sink[0] = a0;
+        } else {
+            int a0 = tid, a1 = tid + 1, a2 = tid + 2, a3 = tid + 3;
+            for (int it = 0; it < alu_iters; it++)
+#pragma unroll
+                for (int u = 0; u < 16; u++) { a0 = a0 * 3 + tid; a1 = a1 * 3 + tid; a2 = a2 * 3 + tid; a3 = a3 * 3 + tid; }
+            if (a0 + a1 + a2 + a3 == 12345) sink[0] = a0;
+        }
+        if (tid == 0 && blockIdx.x == 0) out[0] = clock64() - t0;
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tb));
+}
+}  // namespace
+
+// out[0]: cycles per DADD per warp, chains alone (16 warps per SM);  out[1]: the same averaged over the time a back-to-back
+// tcgen05.mma.kind::i8 stream runs on the SM (progress the chains make during the stream / their progress alone = out[0] / out[1]);
+// out[2], out[3]: the same for IMAD chains;  out[4]: cycles per N = 256 instruction alone, out[5]: beside the DADD chains,
+// out[6]: beside the IMAD chains;  out[7]: SM clock in MHz during the MMA stream (clock64 against globaltimer).
+extern "C" int shd_mix_probe(double out[8])
+{
+    if (!out) return SHD_EINVAL;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return SHD_ECUDA;
+    long long* d = nullptr;
+    double* sink = nullptr;
+    if (cudaMalloc((void**)&d, 3 * sizeof(long long)) != cudaSuccess || cudaMalloc((void**)&sink, 8) != cudaSuccess) { cudaFree(d); return SHD_ENOMEM; }
+    const int sms = prop.multiProcessorCount, mma_iters = 4000, alu_iters = 8000;
+    const double per = 16.0 * 4.0;                  // chain instructions per thread and iteration
+    long long h[3];
+    auto run = [&](int kind, int mi, int ai) -> cudaError_t {
+        cudaMemset(d, 0, 3 * sizeof(long long));
+        for (int r = 0; r < 2; r++) {
+            if (kind == 0) k_mix_probe<0><<<sms, 544>>>(mi, ai, d, sink); else k_mix_probe<1><<<sms, 544>>>(mi, ai, d, sink);
+        }
+        cudaError_t e = cudaMemcpy(h, d, sizeof(h), cudaMemcpyDeviceToHost);
+        return e == cudaSuccess ? cudaGetLastError() : e;
+    };
+    cudaError_t e = cudaSuccess;
+    for (int kind = 0; kind < 2 && e == cudaSuccess; kind++) {
+        if ((e = run(kind, 0, alu_iters)) != cudaSuccess) break;
+        const double alone = (double)h[0] / (alu_iters * per);
+        if ((e = run(kind, mma_iters, alu_iters)) != cudaSuccess) break;
+        // the chains ran h[0] cycles in all, h[1] of them beside the MMA stream and the rest alone at `alone` cycles per instruction
+        const double done_alone = ((double)h[0] - (double)h[1]) / alone, done_beside = alu_iters * per - done_alone;
+        out[2 * kind] = alone;
+        out[2 * kind + 1] = done_beside > 0.0 ? (double)h[1] / done_beside : 1e30;
+        out[5 + kind] = (double)h[1] / (mma_iters * 4.0);
+        if (kind == 0) out[7] = (double)h[1] / (double)h[2] * 1e3;
+    }
+    if (e == cudaSuccess && (e = run(0, mma_iters, 1)) == cudaSuccess) out[4] = (double)h[1] / (mma_iters * 4.0);
+    cudaFree(d); cudaFree(sink);
+    return e == cudaSuccess ? SHD_OK : SHD_ECUDA;
+}
+
 extern "C" int shd_i8_probe(double* tops, long* mismatches)
 {
     if (!tops || !mismatches) return SHD_EINVAL;

@@ -454,8 +454,11 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
     signed char* B8 = (e >= 1 && rho) ? h->d_B8 : nullptr;
     signed char* Bg8 = (e == 2 && grad) ? h->d_Bg8 : nullptr;
     ulonglong2* Afix = (e == 2 && grad) ? reinterpret_cast<ulonglong2*>(h->d_Afix) : nullptr;
+    // the staging tiles are used by the limb tables and the rho pass's digit tables only: the INT8 gradient pass's
+    // tables (Afix, Bg8) go out from registers, so that launch needs no shared memory and its CTAs fit beside k_rho8's
+    const size_t smem = (A || B || Bg || A8 || B8) ? TABLES_SMEM : 0;
 #define LAUNCH_TABLES(DLOV)                                                                                       \
-    k_tables<DLOV><<<grid, TB, TABLES_SMEM, h->stream>>>(h->d, h->N, j_first, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2, \
+    k_tables<DLOV><<<grid, TB, smem, h->stream>>>(h->d, h->N, j_first, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2, \
                                          h->d_pn0, h->d_pn1, h->d_pn2, h->Qpad, pos_hi, pos_lo, A, B, Bg, grad ? 1 : 0, \
                                          A8, B8, h->nk8, Bg8, h->nkq8, Afix, h->njb128 * 128, ech, h->d_skip)
     // the INT8 engines read only the 13, 7 or 4 most significant digits (shd_set_precision): the rest is not written

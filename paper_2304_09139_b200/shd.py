@@ -19,7 +19,7 @@ EXPORTS = ["shd_create", "shd_create_shell", "shd_create_table", "shd_destroy", 
            "shd_energy_grad", "shd_energy_grad_host", "shd_set_timing", "shd_smax", "shd_last_smax", "shd_get_rho", "shd_minimize",
            "shd_last_error", "shd_stat", "shd_fp64_peak", "shd_structure_factor", "shd_set_precision", "shd_i8_probe", "shd_set_engine",
            "shd_set_workspace", "shd_set_shard", "shd_comm_unique_id", "shd_comm_init", "shd_partial_bytes", "shd_rho_partial", "shd_rho_finish",
-           "shd_grad_local", "shd_structure_factor_shells", "shd_tau", "shd_get_trace", "shd_minimize_snapshot"]
+           "shd_grad_local", "shd_structure_factor_shells", "shd_tau", "shd_get_trace", "shd_minimize_snapshot", "shd_mix_probe"]
 
 
 class ShdError(RuntimeError):
@@ -93,6 +93,7 @@ def _load():
     lib.shd_get_trace.argtypes = [vp, C.c_long, C.c_long, C.POINTER(shd_trace_rec)]
     lib.shd_get_trace.restype = C.c_long
     lib.shd_minimize_snapshot.argtypes = [vp, vp, vp]
+    lib.shd_mix_probe.argtypes = [dp]
     return lib
 
 
@@ -363,6 +364,18 @@ def i8_probe():
     if rc != SHD_OK:
         raise ShdError(rc, "shd_i8_probe failed")
     return tops.value, bad.value
+
+
+def mix_probe():
+    """shd_mix_probe: FP64 / integer ALU chains beside a tcgen05.mma.kind::i8 stream (see include/shd_bench.h)."""
+    _torch()
+    out = (C.c_double * 8)()
+    rc = lib.shd_mix_probe(out)
+    if rc != SHD_OK:
+        raise ShdError(rc, "shd_mix_probe failed")
+    keys = ["dadd_cycles_alone", "dadd_cycles_beside_mma", "imad_cycles_alone", "imad_cycles_beside_mma",
+            "mma_n256_cycles_alone", "mma_n256_cycles_beside_dadd", "mma_n256_cycles_beside_imad", "sm_mhz_under_mma"]
+    return dict(zip(keys, [float(x) for x in out]))
 
 
 def comm_unique_id() -> bytes:
