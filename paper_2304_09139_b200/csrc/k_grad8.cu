@@ -20,6 +20,7 @@
 // registers, no per-instruction election loop), one elected lane issues.
 #include "pipe.cuh"
 #include "shd_internal.h"
+#include <algorithm>
 
 namespace {
 
@@ -108,11 +109,11 @@ __device__ __forceinline__ dd acc192_to_dd(acc192 g, int e) {
 
 // ND = 13: full precision; 7 / 4: the most significant digits only (shd_set_precision 2 / 1; see k_rho8.cu)
 template <int ND>
-__global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
+__global__ void __maxnreg__(112) k_grad8(
     int d, long N, long Npad, long njb128, int Ppad, int qscale_log2, int nkq,
     const int2* __restrict__ steps, int nsteps, int nseg, const int* __restrict__ wT,
     const ulonglong2* __restrict__ Afix, const signed char* __restrict__ Bg8, const signed char* __restrict__ W8,
-    double* __restrict__ gpart, const int* __restrict__ skip)
+    double* __restrict__ gpart, long nunits, const int* __restrict__ skip)
 {
     if (skip && *skip) return;
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -121,11 +122,11 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
     __shared__ __align__(8) unsigned long long full_bar[8], empty_bar[8], tfull_bar, tempty_bar;
     __shared__ uint32_t tmem_base;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    // segment fastest: the CTAs of one particle block run side by side and share its digit slabs in L2
-    const int seg = (int)(blockIdx.x % nseg);
-    const long jb = blockIdx.x / nseg;
-    const int c_begin = (int)((long)nsteps * seg / nseg), c_end = (int)((long)nsteps * (seg + 1) / nseg);
-    const int total = c_end - c_begin;
+    // PERSISTENT: one CTA per SM walks the work units u = blockIdx.x, blockIdx.x + gridDim.x, ... (unit = particle block x
+    // segment of the step list, all of the same length; segment fastest, so that the CTAs of one particle block run side
+    // by side and share its digit slabs in L2).  The TMA ring and the tensor-memory hand-shake run on across units: the
+    // producer is already loading the next unit while the epilogue of the last block of a unit -- and its conversion and
+    // write-out -- runs beside the next unit's first instructions, and nothing is set up twice.
     const uint32_t s0 = smem_u32(smem);
     if (tid == 0) {
         for (int s = 0; s < NST; s++) { mbar_init(smem_u32(&full_bar[s]), 1); mbar_init(smem_u32(&empty_bar[s]), 1); }
@@ -145,31 +146,40 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
 
     if (warp == G8_EPI_WARPS) {
         if (lane == 0) {
+          long it = 0;                                          // steps issued by this CTA so far (ring position)
+          for (long u = blockIdx.x; u < nunits; u += gridDim.x) {
+            const int seg = (int)(u % nseg);
+            const long jb = u / nseg;
+            const int c_begin = (int)((long)nsteps * seg / nseg), total = (int)((long)nsteps * (seg + 1) / nseg) - c_begin;
             const signed char* gA = Bg8 + (size_t)jb * nkq * G8_A;
-            for (int i = 0; i < total; i++) {
-                const int s = i % NST;
-                if (i >= NST) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((i / NST - 1) & 1));
+            for (int i = 0; i < total; i++, it++) {
+                const int s = (int)(it % NST);
+                if (it >= NST) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((it / NST - 1) & 1));
                 const uint32_t bar = smem_u32(&full_bar[s]);
                 const int2 st = steps[c_begin + i];           // x: pb8 * nkq + kstep,  y: kstep | end << 16
                 mbar_expect_tx(bar, ND * (G8_ASLAB + G8_WSLAB));
                 tma_load_1d(s0 + s * STG, gA + (size_t)(st.y & 0xffff) * G8_A + OFF * G8_ASLAB, ND * G8_ASLAB, bar);
                 tma_load_1d(s0 + s * STG + ND * G8_ASLAB, W8 + (size_t)st.x * G8_W + OFF * G8_WSLAB, ND * G8_WSLAB, bar);
             }
+          }
         }
     } else if (warp == G8_EPI_WARPS + 1) {
         {
             uint32_t elected;
             asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(elected));
-            int nblock = 0;
+            long nblock = 0, it = 0;                           // blocks handed over / steps issued by this CTA so far
             bool fresh = true;                                 // next step starts a new accumulation
-            for (int i = 0; i < total; i++) {
-                const int s = i % NST;
+          for (long u = blockIdx.x; u < nunits; u += gridDim.x) {
+            const int seg = (int)(u % nseg);
+            const int c_begin = (int)((long)nsteps * seg / nseg), total = (int)((long)nsteps * (seg + 1) / nseg) - c_begin;
+            for (int i = 0; i < total; i++, it++) {
+                const int s = (int)(it % NST);
                 const int2 st = steps[c_begin + i];
                 if (fresh && nblock > 0) {                     // tensor memory must have been drained by the epilogue
                     mbar_wait(smem_u32(&tempty_bar), (uint32_t)((nblock - 1) & 1));
                     asm volatile("tcgen05.fence::after_thread_sync;");
                 }
-                mbar_wait(smem_u32(&full_bar[s]), (uint32_t)((i / NST) & 1));
+                mbar_wait(smem_u32(&full_bar[s]), (uint32_t)((it / NST) & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;");
                 const uint32_t sA = s0 + s * STG, sW = sA + ND * G8_ASLAB;
                 // descriptors differ only in the 14-bit address field: one base per operand, compile-time offsets
@@ -203,15 +213,20 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
                     fresh = true;
                 }
             }
+          }
         }
     } else {
         // ---- 16 epilogue warps: thread = (particle = TMEM lane, quarter of the block's 8 p); columns 32 c + 4 p_local + out
         const int quarter = warp >> 2, row = tid & 127;
-        const long j = jb * 128 + row;
         const long NpadA = njb128 * 128;
+        long nblock = 0;                                       // blocks drained by this CTA so far (tensor-memory hand-shake)
+      for (long u = blockIdx.x; u < nunits; u += gridDim.x) {
+        const int seg = (int)(u % nseg);
+        const long jb = u / nseg;
+        const int c_begin = (int)((long)nsteps * seg / nseg), total = (int)((long)nsteps * (seg + 1) / nseg) - c_begin;
+        const long j = jb * 128 + row;
         const ulonglong2* Aj = Afix + (size_t)j * 2;
         acc192 g[4] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
-        int nblock = 0;
         // next block (or segment) end at or after step i: 32 steps per look, one load latency per block
         auto next_end = [&](int& i, int2& st) {
             for (;;) {
@@ -343,6 +358,7 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
                     o[(slot + ax) * N + j] = make_double2(r.h, r.l);
                 }
         }
+      }
     }
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();
@@ -362,12 +378,13 @@ cudaError_t shd_grad8_configure()
 // k_gradsum (k_grad.cu) adds the segments' partial gradients and applies 4 pi / L / cscale; nc = particles of the chunk
 cudaError_t shd_launch_grad8_main(shd_ctx* h, long nc)
 {
-    const long njb = (nc + 127) / 128;
+    const long njb = (nc + 127) / 128, nunits = njb * h->nseg8;
+    const unsigned grid = (unsigned)std::min<long>(nunits, h->sms);        // persistent: one CTA per SM
 #define LAUNCH_GRAD8(NDV)                                                                            \
-    k_grad8<NDV><<<(unsigned)(njb * h->nseg8), G8_THREADS, G8_SMEM, h->stream>>>(                            \
+    k_grad8<NDV><<<grid, G8_THREADS, G8_SMEM, h->stream>>>(                                                  \
         h->d, nc, h->Npad, h->njb128, h->npb * 32, h->qscale_log2, h->nkq8,                            \
         reinterpret_cast<const int2*>(h->d_steps8), h->nsteps8, h->nseg8, h->d_wT,                     \
-        reinterpret_cast<const ulonglong2*>(h->d_Afix), h->d_Bg8, h->d_W8, h->d_gpart, h->d_skip)
+        reinterpret_cast<const ulonglong2*>(h->d_Afix), h->d_Bg8, h->d_W8, h->d_gpart, nunits, h->d_skip)
     if (h->nlimb >= 3) LAUNCH_GRAD8(13);
     else if (h->nlimb == 2) LAUNCH_GRAD8(7);
     else LAUNCH_GRAD8(4);

@@ -245,6 +245,7 @@ int build(shd_ctx* h, const double* v) {
     cudaGetDevice(&dev);
     if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return fail(h, SHD_ECUDA, "cudaGetDeviceProperties failed");
     const long sms = prop.multiProcessorCount;
+    h->sms = (int)sms;
     const long nchunks = (h->N + SHD_NPS - 1) / SHD_NPS;
     // CTAs are dispatched in blockIdx order (split-major, tile-minor) to the first free SM; a tile with
     // <= 4 valid units takes ~0.6 of a full tile's time.  Simulate that list schedule for every split count.

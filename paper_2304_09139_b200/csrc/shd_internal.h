@@ -77,6 +77,7 @@ struct shd_ctx {
     long N = 0;                // particles this handle evaluates (its shard of the system)
     long Nsys = 0;             // particles of the whole system (= N unless sharded, shd_set_shard): S_max = max |rho|^2 / Nsys
     int rank = 0, world = 1;   // position of the shard
+    int sms = 148;             // SMs of the device
     // Bounded workspace: the per-particle tables hold one CHUNK of particles = spc whole splits of the rho pass, so the
     // reduction tree (left fold over the splits, k_finish1) is the same for every chunk size: results are bit-identical.
     long unit = 0;             // particles per split of the current engine's rho pass
