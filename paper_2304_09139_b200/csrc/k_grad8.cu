@@ -21,6 +21,8 @@
 #include "pipe.cuh"
 #include "shd_internal.h"
 #include <algorithm>
+#include <cstdio>
+#include <cstdlib>
 
 namespace {
 
@@ -109,7 +111,7 @@ __device__ __forceinline__ dd acc192_to_dd(acc192 g, int e) {
 
 // ND = 13: full precision; 7 / 4: the most significant digits only (shd_set_precision 2 / 1; see k_rho8.cu)
 template <int ND>
-__global__ void __maxnreg__(112) k_grad8(
+__global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
     int d, long N, long Npad, long njb128, int Ppad, int qscale_log2, int nkq,
     const int2* __restrict__ steps, int nsteps, int nseg, const int* __restrict__ wT,
     const ulonglong2* __restrict__ Afix, const signed char* __restrict__ Bg8, const signed char* __restrict__ W8,
@@ -119,7 +121,9 @@ __global__ void __maxnreg__(112) k_grad8(
     extern __shared__ __align__(1024) unsigned char smem[];
     // a stage holds the ND digit slabs in use of both operands; the fewer digits, the deeper the ring
     constexpr int STG = ND * (G8_ASLAB + G8_WSLAB), NST = G8_SMEM / STG < 8 ? G8_SMEM / STG : 8;
-    __shared__ __align__(8) unsigned long long full_bar[8], empty_bar[8], tfull_bar, tempty_bar;
+    // tempty_bar[g]: column blocks 4 g .. 4 g + 3 of the accumulator set have been read AND zeroed by the epilogue
+    constexpr int NTG = (ND + 3) / 4;
+    __shared__ __align__(8) unsigned long long full_bar[8], empty_bar[8], tfull_bar, tempty_bar[4];
     __shared__ uint32_t tmem_base;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     // PERSISTENT: one CTA per SM walks the work units u = blockIdx.x, blockIdx.x + gridDim.x, ... (unit = particle block x
@@ -127,11 +131,17 @@ __global__ void __maxnreg__(112) k_grad8(
     // by side and share its digit slabs in L2).  The TMA ring and the tensor-memory hand-shake run on across units: the
     // producer is already loading the next unit while the epilogue of the last block of a unit -- and its conversion and
     // write-out -- runs beside the next unit's first instructions, and nothing is set up twice.
+    // HAND-OVER: one accumulator set (32 ND of the 512 columns) is all tensor memory holds, so at a block end the tensor
+    // core waits for the epilogue to read it -- 0.9 us, bound by the tensor-memory read bandwidth.  To hide most of that the
+    // epilogue ZEROES each group of four column blocks right after reading it (tcgen05.st is four times faster than the
+    // read) and releases the group on its own barrier; every instruction accumulates (no initialising instruction), and
+    // the first K-step of the next block runs in ASCENDING digit order -- digit i' touches column blocks 0 .. i' only --
+    // waiting for a group just before the first instruction that needs it.
     const uint32_t s0 = smem_u32(smem);
     if (tid == 0) {
         for (int s = 0; s < NST; s++) { mbar_init(smem_u32(&full_bar[s]), 1); mbar_init(smem_u32(&empty_bar[s]), 1); }
         mbar_init(smem_u32(&tfull_bar), 1);
-        mbar_init(smem_u32(&tempty_bar), G8_EPI_WARPS * 32);
+        for (int g = 0; g < NTG; g++) mbar_init(smem_u32(&tempty_bar[g]), G8_EPI_WARPS * 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 0) {
@@ -175,10 +185,6 @@ __global__ void __maxnreg__(112) k_grad8(
             for (int i = 0; i < total; i++, it++) {
                 const int s = (int)(it % NST);
                 const int2 st = steps[c_begin + i];
-                if (fresh && nblock > 0) {                     // tensor memory must have been drained by the epilogue
-                    mbar_wait(smem_u32(&tempty_bar), (uint32_t)((nblock - 1) & 1));
-                    asm volatile("tcgen05.fence::after_thread_sync;");
-                }
                 mbar_wait(smem_u32(&full_bar[s]), (uint32_t)((it / NST) & 1));
                 asm volatile("tcgen05.fence::after_thread_sync;");
                 const uint32_t sA = s0 + s * STG, sW = sA + ND * G8_ASLAB;
@@ -194,16 +200,17 @@ __global__ void __maxnreg__(112) k_grad8(
                         g8_mma(tb + 256, da, dW0 + (uint64_t)(((l0 + 8) * G8_WSLAB) >> 4), g8_idesc(n - 256), acc, elected);
                     }
                 };
-                // A block's first step runs from the most significant digit down (its first instruction covers all
-                // columns and initialises them); the other steps run upwards, short instructions first and long ones
-                // last, so that the tensor core's queue holds long instructions while this thread crosses the step
-                // boundary (k_rho8.cu).
-                if (fresh || ND < G8_ND) {
+                // Every step runs upwards, short instructions first and long ones last, so that the tensor core's queue
+                // holds long instructions while this thread crosses the step boundary (k_rho8.cu); all accumulate (the
+                // accumulator set is zero at a block's start: zeroed by the epilogue, or at kernel start).  A block's
+                // first step waits for column group g (read and zeroed) before its first instruction that touches it.
 #pragma unroll
-                    for (int ii = ND - 1; ii >= 0; ii--) issue(ii, (!fresh || ii < ND - 1) ? 1u : 0u);
-                } else {
-#pragma unroll
-                    for (int ii = 0; ii < ND; ii++) issue(ii, 1u);
+                for (int ii = 0; ii < ND; ii++) {
+                    if (fresh && (ii & 3) == 0) {
+                        mbar_wait(smem_u32(&tempty_bar[ii >> 2]), (uint32_t)(nblock & 1));
+                        asm volatile("tcgen05.fence::after_thread_sync;");
+                    }
+                    issue(ii, 1u);
                 }
                 g8_commit(smem_u32(&empty_bar[s]), elected);
                 fresh = false;
@@ -220,6 +227,19 @@ __global__ void __maxnreg__(112) k_grad8(
         const int quarter = warp >> 2, row = tid & 127;
         const long NpadA = njb128 * 128;
         long nblock = 0;                                       // blocks drained by this CTA so far (tensor-memory hand-shake)
+        {
+            // the accumulator set starts at zero: every thread clears its own 8 columns of every column block, then
+            // releases all groups (phase 0 of the tempty barriers = "zero at kernel start")
+            const uint32_t taddr0 = tb + ((uint32_t)((warp & 3) * 32) << 16) + 8 * quarter;
+            const uint32_t z = 0;
+#pragma unroll
+            for (int c = 0; c < ND; c++)
+                asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%1,%1,%1,%1,%1,%1,%1};" ::"r"(taddr0 + c * 32), "r"(z) : "memory");
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            asm volatile("tcgen05.fence::before_thread_sync;");
+#pragma unroll
+            for (int g = 0; g < NTG; g++) mbar_arrive(smem_u32(&tempty_bar[g]));
+        }
       for (long u = blockIdx.x; u < nunits; u += gridDim.x) {
         const int seg = (int)(u % nseg);
         const long jb = u / nseg;
@@ -283,6 +303,18 @@ __global__ void __maxnreg__(112) k_grad8(
                                        "=r"(v[cc][6]), "=r"(v[cc][7])
                                      : "r"(taddr + (c0 + cc) * 32));
                 asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                {
+                    // this group of column blocks is in registers: zero it and hand it back to the tensor core
+                    const uint32_t z = 0;
+#pragma unroll
+                    for (int cc = 0; cc < 4; cc++)
+                        if (c0 + cc < ND)
+                            asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%1,%1,%1,%1,%1,%1,%1};"
+                                         ::"r"(taddr + (c0 + cc) * 32), "r"(z) : "memory");
+                    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+                    asm volatile("tcgen05.fence::before_thread_sync;");
+                    mbar_arrive(smem_u32(&tempty_bar[c0 >> 2]));
+                }
 #pragma unroll
                 for (int cc = 0; cc < 4; cc++) {
                     const int c = c0 + cc;
@@ -296,9 +328,7 @@ __global__ void __maxnreg__(112) k_grad8(
                     }
                 }
             }
-            // tensor memory is drained: the next block's instructions start while the rest of the epilogue runs
-            asm volatile("tcgen05.fence::before_thread_sync;");
-            mbar_arrive(smem_u32(&tempty_bar));
+            // tensor memory is drained and zeroed: the next block's instructions run while the rest of the epilogue does
             int inext = i + 1;                                 // the block after this one
             int2 stn = st;
             if (inext < total) next_end(inext, stn);
@@ -369,6 +399,11 @@ __global__ void __maxnreg__(112) k_grad8(
 
 cudaError_t shd_grad8_configure()
 {
+    if (getenv("SHD_DEBUG")) {
+        cudaFuncAttributes a;
+        cudaFuncGetAttributes(&a, k_grad8<13>);
+        fprintf(stderr, "k_grad8<13>: regs %d maxThreadsPerBlock %d static smem %zu local %zu\n", a.numRegs, a.maxThreadsPerBlock, a.sharedSizeBytes, a.localSizeBytes);
+    }
     cudaError_t e = cudaFuncSetAttribute(k_grad8<13>, cudaFuncAttributeMaxDynamicSharedMemorySize, G8_SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad8<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, G8_SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad8<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, G8_SMEM);

@@ -442,10 +442,12 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
     const bool rho = (what & 1) != 0, grad = (what & 2) != 0;
     // every slot of the chunk's tables is written (zeros beyond the handle's last particle)
     const long slots = std::max(std::max(h->Npad, h->nk8 * 32), std::max(h->njb128 * 128, h->njb64 * 64));
-    // entries per chunk (blockIdx.z): the whole table when the particles alone fill the GPU, else 32-entry chunks
+    // entries per chunk (blockIdx.z): the whole table when the particles alone fill the GPU, else 32- or 16-entry
+    // chunks.  Decided from the handle's particle count, not from the size of the tables in use: a chunk start is a
+    // binary power, rounded differently from the recurrence, and results must not depend on the workspace cap.
     const int emax = std::max(h->P, h->Qn);
     int ech = ((emax + 7) / 8) * 8;
-    if (slots < 96 * 1024 && emax > 32) ech = slots < 24 * 1024 ? 16 : 32;
+    if (h->N < 96 * 1024 && emax > 32) ech = h->N < 24 * 1024 ? 16 : 32;
     dim3 grid((unsigned)((slots + TB - 1) / TB), 2, (unsigned)((emax + ech - 1) / ech));
     double* A = (e == 2 || !(rho || grad)) ? nullptr : ((e == 1 && !grad) ? nullptr : h->d_A);   // FP64 rho pass and FP64 gradient pass
     double* B = (e == 0 && rho) ? h->d_B : nullptr;
@@ -455,7 +457,7 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
     signed char* Bg8 = (e == 2 && grad) ? h->d_Bg8 : nullptr;
     ulonglong2* Afix = (e == 2 && grad) ? reinterpret_cast<ulonglong2*>(h->d_Afix) : nullptr;
     // the staging tiles are used by the limb tables and the rho pass's digit tables only: the INT8 gradient pass's
-    // tables (Afix, Bg8) go out from registers, so that launch needs no shared memory and its CTAs fit beside k_rho8's
+    // tables (Afix, Bg8) go out from registers
     const size_t smem = (A || B || Bg || A8 || B8) ? TABLES_SMEM : 0;
 #define LAUNCH_TABLES(DLOV)                                                                                       \
     k_tables<DLOV><<<grid, TB, smem, h->stream>>>(h->d, h->N, j_first, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2, \

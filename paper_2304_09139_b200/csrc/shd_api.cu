@@ -475,13 +475,6 @@ int shd_prepare_tables(shd_ctx* h, bool with_grad) {
         h->table_bytes += h->workspace_bytes - before;
         h->tables_valid = true;
     }
-    if (with_grad && e == 2 && !h->side) {
-        int lo_pri = 0, hi_pri = 0;
-        CU(cudaDeviceGetStreamPriorityRange(&lo_pri, &hi_pri));
-        CU(cudaStreamCreateWithPriority(&h->side, cudaStreamNonBlocking, lo_pri));
-        CU(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
-        CU(cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming));
-    }
     if (with_grad && !h->d_gpart) {
         const size_t before = h->workspace_bytes;
         if (e == 2) {
@@ -513,27 +506,15 @@ cudaError_t shd_enqueue_rho_partial(shd_ctx* h, const double* pos_hi, const doub
     const int e = h->rho_engine;
     const long nsplit_total = e >= 1 ? h->nsplit8 : h->nsplit;
     const bool both = h->nchunk == 1 && grad_tables_too;      // one chunk: one table build serves both passes
-    // INT8 engine: the gradient pass's tables (HBM-write-bound, no shared memory) are built on a low-priority side stream
-    // BESIDE the rho pass (tensor-bound, one CTA per SM by shared memory): forked after the rho tables' launch, joined
-    // before the gradient pass.  Works inside the minimizers' graph capture too (event fork / join).
-    const bool overlap = both && e == 2 && h->side != nullptr;
+    // (Building the gradient pass's tables on a side stream beside k_rho8 was tried and is slower, 4.73 against 4.45 ms at
+    // cfg4: k_tables is bound by its FP64 recurrences, not by its writes -- the rho tables alone take 0.65 of its 0.73 ms --
+    // and FP64 all but stalls beside a tensor stream, so the second launch repeats the recurrences and then waits.)
     cudaError_t err;
     for (int c = 0; c < h->nchunk; c++) {
         const long j0 = (long)c * h->Nc;
         const int ns = (int)std::min<long>(h->spc, nsplit_total - (long)c * h->spc);
         const bool last = c == h->nchunk - 1;
-        if ((err = shd_launch_tables(h, pos_hi, pos_lo, j0, (both && !overlap) ? 3 : 1)) != cudaSuccess) return err;
-        if (overlap) {
-            cudaStream_t main_stream = h->stream;
-            if ((err = cudaEventRecord(h->ev_fork, main_stream)) != cudaSuccess) return err;
-            if ((err = cudaStreamWaitEvent(h->side, h->ev_fork, 0)) != cudaSuccess) return err;
-            h->stream = h->side;
-            err = shd_launch_tables(h, pos_hi, pos_lo, j0, 2);
-            h->stream = main_stream;
-            if (err != cudaSuccess) return err;
-            if ((err = cudaEventRecord(h->ev_join, h->side)) != cudaSuccess) return err;
-            h->join_pending = true;
-        }
+        if ((err = shd_launch_tables(h, pos_hi, pos_lo, j0, both ? 3 : 1)) != cudaSuccess) return err;
         if (c == 0 && h->timing_mark) h->timing_mark(h, 1);
         if ((err = shd_launch_rho(h, ns)) != cudaSuccess) return err;
         if (last && h->timing_mark) h->timing_mark(h, 2);
@@ -553,10 +534,6 @@ cudaError_t shd_enqueue_grad(shd_ctx* h, const double* pos_hi, const double* pos
 {
     cudaError_t err;
     if ((err = shd_launch_ctable(h)) != cudaSuccess) return err;
-    if (h->join_pending) {                       // the gradient pass's tables were built on the side stream
-        if ((err = cudaStreamWaitEvent(h->stream, h->ev_join, 0)) != cudaSuccess) return err;
-        h->join_pending = false;
-    }
     if (h->timing_mark) h->timing_mark(h, 4);
     for (int c = 0; c < h->nchunk; c++) {
         const long j0 = (long)c * h->Nc;
@@ -708,9 +685,6 @@ void shd_destroy(shd_ctx* h) {
     cudaFree(h->d_tile8_pb); cudaFree(h->d_tile8_qb); cudaFree(h->d_steps8); cudaFree(h->d_trace);
     for (int i = 0; i <= SHD_NKERN; i++) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     if (h->h_scal) cudaFreeHost(h->h_scal);
-    if (h->ev_fork) cudaEventDestroy(h->ev_fork);
-    if (h->ev_join) cudaEventDestroy(h->ev_join);
-    if (h->side) cudaStreamDestroy(h->side);
     if (h->gevent) cudaEventDestroy(h->gevent);
     if (h->gstream) cudaStreamDestroy(h->gstream);
     delete h;

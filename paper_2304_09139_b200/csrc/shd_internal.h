@@ -161,9 +161,6 @@ struct shd_ctx {
     shd_scalars *h_scal = nullptr;  // pinned
     size_t workspace_bytes = 0;
     cudaStream_t stream = 0;
-    cudaStream_t side = nullptr;      // low-priority side stream: the gradient pass's tables are built beside the rho pass
-    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
-    bool join_pending = false;        // the side stream's work must be joined before the gradient pass
     cudaStream_t gstream = nullptr;   // the minimizers' own (capturable) stream, slots.cuh
     cudaEvent_t gevent = nullptr;
     const int* d_skip = nullptr;    // device flag: when non-NULL and *d_skip != 0 every kernel of the
