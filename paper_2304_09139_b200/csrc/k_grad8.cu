@@ -156,20 +156,22 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
 
     if (warp == G8_EPI_WARPS) {
         if (lane == 0) {
-          long it = 0;                                          // steps issued by this CTA so far (ring position)
+          int s = 0;                                            // ring position and the parity of its "empty" phase,
+          uint32_t epar = 0u;                                   //   kept incrementally (no division in the loop)
+          bool first_round = true;
           for (long u = blockIdx.x; u < nunits; u += gridDim.x) {
             const int seg = (int)(u % nseg);
             const long jb = u / nseg;
             const int c_begin = (int)((long)nsteps * seg / nseg), total = (int)((long)nsteps * (seg + 1) / nseg) - c_begin;
             const signed char* gA = Bg8 + (size_t)jb * nkq * G8_A;
-            for (int i = 0; i < total; i++, it++) {
-                const int s = (int)(it % NST);
-                if (it >= NST) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((it / NST - 1) & 1));
+            for (int i = 0; i < total; i++) {
+                if (!first_round) mbar_wait(smem_u32(&empty_bar[s]), epar);
                 const uint32_t bar = smem_u32(&full_bar[s]);
                 const int2 st = steps[c_begin + i];           // x: pb8 * nkq + kstep,  y: kstep | end << 16
                 mbar_expect_tx(bar, ND * (G8_ASLAB + G8_WSLAB));
                 tma_load_1d(s0 + s * STG, gA + (size_t)(st.y & 0xffff) * G8_A + OFF * G8_ASLAB, ND * G8_ASLAB, bar);
                 tma_load_1d(s0 + s * STG + ND * G8_ASLAB, W8 + (size_t)st.x * G8_W + OFF * G8_WSLAB, ND * G8_WSLAB, bar);
+                if (++s == NST) { s = 0; if (first_round) first_round = false; else epar ^= 1u; }
             }
           }
         }
@@ -177,15 +179,16 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
         {
             uint32_t elected;
             asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(elected));
-            long nblock = 0, it = 0;                           // blocks handed over / steps issued by this CTA so far
+            uint32_t tpar = 0u;                                // parity of the tensor-memory hand-shake (blocks handed over so far)
+            int s = 0;                                         // ring position and the parity of its "full" phase
+            uint32_t fpar = 0u;
             bool fresh = true;                                 // next step starts a new accumulation
           for (long u = blockIdx.x; u < nunits; u += gridDim.x) {
             const int seg = (int)(u % nseg);
             const int c_begin = (int)((long)nsteps * seg / nseg), total = (int)((long)nsteps * (seg + 1) / nseg) - c_begin;
-            for (int i = 0; i < total; i++, it++) {
-                const int s = (int)(it % NST);
+            for (int i = 0; i < total; i++) {
                 const int2 st = steps[c_begin + i];
-                mbar_wait(smem_u32(&full_bar[s]), (uint32_t)((it / NST) & 1));
+                mbar_wait(smem_u32(&full_bar[s]), fpar);
                 asm volatile("tcgen05.fence::after_thread_sync;");
                 const uint32_t sA = s0 + s * STG, sW = sA + ND * G8_ASLAB;
                 // descriptors differ only in the 14-bit address field: one base per operand, compile-time offsets
@@ -207,7 +210,7 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
 #pragma unroll
                 for (int ii = 0; ii < ND; ii++) {
                     if (fresh && (ii & 3) == 0) {
-                        mbar_wait(smem_u32(&tempty_bar[ii >> 2]), (uint32_t)(nblock & 1));
+                        mbar_wait(smem_u32(&tempty_bar[ii >> 2]), tpar);
                         asm volatile("tcgen05.fence::after_thread_sync;");
                     }
                     issue(ii, 1u);
@@ -216,9 +219,10 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
                 fresh = false;
                 if ((st.y >> 16) || i == total - 1) {          // block (or segment) end: hand the sums to the epilogue
                     g8_commit(smem_u32(&tfull_bar), elected);
-                    nblock++;
+                    tpar ^= 1u;
                     fresh = true;
                 }
+                if (++s == NST) { s = 0; fpar ^= 1u; }
             }
           }
         }
@@ -226,7 +230,7 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
         // ---- 16 epilogue warps: thread = (particle = TMEM lane, quarter of the block's 8 p); columns 32 c + 4 p_local + out
         const int quarter = warp >> 2, row = tid & 127;
         const long NpadA = njb128 * 128;
-        long nblock = 0;                                       // blocks drained by this CTA so far (tensor-memory hand-shake)
+        uint32_t nblock = 0;                                   // blocks drained by this CTA so far (tensor-memory hand-shake)
         {
             // the accumulator set starts at zero: every thread clears its own 8 columns of every column block, then
             // releases all groups (phase 0 of the tempty barriers = "zero at kernel start")
