@@ -368,6 +368,11 @@ def run_gpu(args, cfg):
                 # SM clock at which one tcgen05.mma.kind::i8 of N = 256 takes its 128 cycles and gives this peak; the hot
                 # kernels themselves run at ~1.66 GHz (clock64 against globaltimer inside k_rho8, profiles/r2a_summary.md)
                 "peak_implied_sm_mhz": i8_tops * 1e12 / (148 * 8192 * 2.0) / 1e6,
+                # the SM clock INSIDE the timed tensor kernels (clock64 against globaltimer, last evaluation) and the
+                # roofline at that clock: 148 SMs x 8192 MAC per cycle x 2
+                "sm_mhz_in_kernel": {"k_rho8": h.stat(28), "k_grad8": h.stat(29)},
+                "frac_at_kernel_clock": achieved * 1e12 / (148 * 8192 * 2.0 * 1e6 * (h.stat(29) if dom == "k_grad8" else h.stat(28)))
+                                        if (h.stat(29) if dom == "k_grad8" else h.stat(28)) > 0 else None,
                 "dtype": "s8 x s8 -> s32 (exact digit-sliced contraction; counted in integer operations)",
                 "peak_source": "measured live: shd_i8_probe, tcgen05.mma.kind::i8 M=128 N=256 K=32 issued back to "
                                "back on all SMs; MEASURED_PEAKS.json bf16 x 2 (nominal int8 : bf16) for comparison",

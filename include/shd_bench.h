@@ -23,6 +23,8 @@ int shd_set_timing(shd_ctx* h, int on);
  *   14 / 15: tiles / particle splits of the INT8 rho pass, 16: engine in use, 18: K-steps of the INT8 gradient pass,
  *   19: chunks per evaluation (shd_set_workspace), 25: particles per chunk, 26: bytes of per-particle tables,
  *   27: 1 when the engine is the library's own choice,
+ *   28 / 29: SM clock in MHz INSIDE k_rho8 / k_grad8 during the last evaluation (clock64 against globaltimer in the
+ *            issuing thread of CTA 0; under tensor load it is well below the clock nvidia-smi reports between kernels),
  *   20..24: milliseconds of the last call's launch groups (needs shd_set_timing):
  *           20 phasor tables (a1), 21 rho pass (a2), 22 finish (a3), 23 gradient operand, 24 gradient pass (a4). */
 double shd_stat(const shd_ctx* h, int what);

@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
     int d, long N, long Npad, long njb128, int Ppad, int qscale_log2, int nkq,
     const int2* __restrict__ steps, int nsteps, int nseg, const int* __restrict__ wT,
     const ulonglong2* __restrict__ Afix, const signed char* __restrict__ Bg8, const signed char* __restrict__ W8,
-    double* __restrict__ gpart, long nunits, const int* __restrict__ skip)
+    double* __restrict__ gpart, long nunits, long long* __restrict__ clk, const int* __restrict__ skip)
 {
     if (skip && *skip) return;
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -179,6 +179,9 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
         {
             uint32_t elected;
             asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(elected));
+            unsigned long long g0 = 0;
+            long long c0 = 0;
+            if (blockIdx.x == 0 && clk) { asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0)); c0 = clock64(); }
             uint32_t tpar = 0u;                                // parity of the tensor-memory hand-shake (blocks handed over so far)
             int s = 0;                                         // ring position and the parity of its "full" phase
             uint32_t fpar = 0u;
@@ -224,6 +227,12 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
                 }
                 if (++s == NST) { s = 0; fpar ^= 1u; }
             }
+          }
+          if (blockIdx.x == 0 && clk && elected) {
+              unsigned long long g1;
+              asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
+              clk[0] = clock64() - c0;
+              clk[1] = (long long)(g1 - g0);
           }
         }
     } else {
@@ -423,7 +432,7 @@ cudaError_t shd_launch_grad8_main(shd_ctx* h, long nc)
     k_grad8<NDV><<<grid, G8_THREADS, G8_SMEM, h->stream>>>(                                                  \
         h->d, nc, h->Npad, h->njb128, h->npb * 32, h->qscale_log2, h->nkq8,                            \
         reinterpret_cast<const int2*>(h->d_steps8), h->nsteps8, h->nseg8, h->d_wT,                     \
-        reinterpret_cast<const ulonglong2*>(h->d_Afix), h->d_Bg8, h->d_W8, h->d_gpart, nunits, h->d_skip)
+        reinterpret_cast<const ulonglong2*>(h->d_Afix), h->d_Bg8, h->d_W8, h->d_gpart, nunits, h->d_scal->clk + 2, h->d_skip)
     if (h->nlimb >= 3) LAUNCH_GRAD8(13);
     else if (h->nlimb == 2) LAUNCH_GRAD8(7);
     else LAUNCH_GRAD8(4);

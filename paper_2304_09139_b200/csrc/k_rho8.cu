@@ -57,7 +57,7 @@ template <int ND>
 __global__ void __launch_bounds__(192, 1) k_rho8(
     const signed char* __restrict__ A8, const signed char* __restrict__ B8,
     const int* __restrict__ tile_pb, const int* __restrict__ tile_qb, int ntiles,
-    long nk_total, int ksteps_per_split, double* __restrict__ part, const int* __restrict__ skip)
+    long nk_total, int ksteps_per_split, double* __restrict__ part, long long* __restrict__ clk, const int* __restrict__ skip)
 {
     if (skip && *skip) return;
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -114,6 +114,9 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
             asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(elected));
             // the ring position is a compile-time constant inside the unrolled inner loop: shared-memory addresses
             // and descriptors of a step are constants off one base, the step boundary costs a few instructions
+            unsigned long long g0 = 0;
+            long long c0 = 0;
+            if (blockIdx.x == 0 && clk) { asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0)); c0 = clock64(); }
             const uint64_t dbase = umma_desc(s0);
             for (int i0 = 0; i0 < nk; i0 += NST) {
                 const uint32_t par = (uint32_t)((i0 / NST) & 1);
@@ -152,6 +155,12 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
               }
             }
             umma_commit(smem_u32(&done_bar), elected);
+            if (blockIdx.x == 0 && clk && elected) {
+                unsigned long long g1;
+                asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
+                clk[0] = clock64() - c0;
+                clk[1] = (long long)(g1 - g0);
+            }
         }
     } else {
         // ---- epilogue warps 0..3: warp w reads TMEM lanes 32 w .. 32 w + 31 (rows r = 2 p_local + c)
@@ -202,7 +211,7 @@ cudaError_t shd_launch_rho8(shd_ctx* h, int nsplits)
     const unsigned grid = (unsigned)(h->ntiles8 * nsplits);      // the splits of one chunk
 #define LAUNCH_RHO8(NDV)                                                                              \
     k_rho8<NDV><<<grid, 192, R8_SMEM, h->stream>>>(h->d_A8, h->d_B8, h->d_tile8_pb, h->d_tile8_qb, h->ntiles8, \
-                                                   h->nk8, h->ksteps8, h->d_part, h->d_skip)
+                                                   h->nk8, h->ksteps8, h->d_part, h->d_scal->clk, h->d_skip)
     if (h->nlimb >= 3) LAUNCH_RHO8(13);
     else if (h->nlimb == 2) LAUNCH_RHO8(7);
     else LAUNCH_RHO8(4);

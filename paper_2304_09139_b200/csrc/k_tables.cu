@@ -303,7 +303,7 @@ struct Stager {
 
 // which = 0: A table.  which = 1: B table (+ the same limbs in the gradient layout Bg).
 template <int DLO>
-__global__ void __launch_bounds__(TB) k_tables(
+__global__ void __launch_bounds__(TB, 8) k_tables(
     int d, long N, long j_first, double L, long Npad, int P, int Qn, int S1d, int qscale_log2,
     const int* __restrict__ pn0, const int* __restrict__ pn1, const int* __restrict__ pn2, int Qpad,
     const double* __restrict__ pos_hi, const double* __restrict__ pos_lo,
@@ -332,7 +332,9 @@ __global__ void __launch_bounds__(TB) k_tables(
     st.Npad = Npad; st.j0 = j0; st.N = N - j_first; st.Qpad = Qpad; st.NpadG = NpadA;
     st.gdig = gradB ? Bg8 : nullptr; st.nkq = nkq8;
     st.dig = which == 0 ? A8 : B8; st.nk8 = nk8; st.rows8 = which == 0 ? SHD_I8_PT : SHD_I8_QT;
-    st.dtile = reinterpret_cast<signed char*>(tables_smem) + TABLES_LIMB_SMEM;
+    // (the limb staging tile comes first when a limb table is written; the digit transpose tile follows it)
+    const bool limb_tile = A != nullptr || B != nullptr || Bg != nullptr;
+    st.dtile = reinterpret_cast<signed char*>(tables_smem) + (limb_tile ? TABLES_LIMB_SMEM : 0);
     st.afix = (which == 0 && with_grad != 0) ? Afix : nullptr; st.NpadA = NpadA;
     if (which == 0) {
         // ---- A table
@@ -458,7 +460,8 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
     ulonglong2* Afix = (e == 2 && grad) ? reinterpret_cast<ulonglong2*>(h->d_Afix) : nullptr;
     // the staging tiles are used by the limb tables and the rho pass's digit tables only: the INT8 gradient pass's
     // tables (Afix, Bg8) go out from registers
-    const size_t smem = (A || B || Bg || A8 || B8) ? TABLES_SMEM : 0;
+    // (8 CTAs of 64 threads per SM by registers; without the 24 KB limb tile the shared memory allows them too)
+    const size_t smem = ((A || B || Bg) ? TABLES_LIMB_SMEM : 0) + ((A8 || B8) ? TABLES_SMEM - TABLES_LIMB_SMEM : 0);
 #define LAUNCH_TABLES(DLOV)                                                                                       \
     k_tables<DLOV><<<grid, TB, smem, h->stream>>>(h->d, h->N, j_first, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2, \
                                          h->d_pn0, h->d_pn1, h->d_pn2, h->Qpad, pos_hi, pos_lo, A, B, Bg, grad ? 1 : 0, \

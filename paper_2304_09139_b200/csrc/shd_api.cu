@@ -968,6 +968,9 @@ double shd_stat(const shd_ctx* h, int what) {
         case 25: return (double)h->Nc;
         case 26: return (double)h->table_bytes;
         case 27: return (double)h->engine_auto;
+        // SM clock in MHz inside the tensor kernels of the last evaluation whose scalars were fetched (shd_internal.h)
+        case 28: return h->h_scal && h->h_scal->clk[1] > 0 ? 1e3 * (double)h->h_scal->clk[0] / (double)h->h_scal->clk[1] : 0.0;
+        case 29: return h->h_scal && h->h_scal->clk[3] > 0 ? 1e3 * (double)h->h_scal->clk[2] / (double)h->h_scal->clk[3] : 0.0;
         case 20: case 21: case 22: case 23: case 24: return (double)h->kern_ms[what - 20];
         default: return 0.0;
     }

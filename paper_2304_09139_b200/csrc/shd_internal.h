@@ -65,6 +65,10 @@ struct shd_scalars {
     long long argmax;
     int nonfinite;
     int pad;
+    // SM clock inside the tensor kernels: cycles (clock64) and nanoseconds (globaltimer) of the issuing thread of CTA 0,
+    // [0..1] k_rho8, [2..3] k_grad8 of the last evaluation (the clock under tensor load is well below what nvidia-smi
+    // shows between kernels; bench.py states the roofline at this clock too)
+    long long clk[4];
 };
 
 struct shd_minstate;      // L-BFGS workspace (shd_min.cu)
