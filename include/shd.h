@@ -201,6 +201,10 @@ int shd_structure_factor(shd_ctx* h, double* S_out, double dev2[2]);
  * Errors: SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA.  Synchronises the stream.
  */
 int shd_structure_factor_shells(shd_ctx* h, long nbins, const long* edges, long* count, double* S_mean_hi, double* S_mean_lo);
+/* The distinct values of n.n in the handle's Q, ascending (HOST, shd_num_shells(h) longs): with edges = these values
+ * followed by (the last + 1), shd_structure_factor_shells returns one bin per shell, the finest radial resolution. */
+long shd_num_shells(const shd_ctx* h);
+int shd_get_shells(const shd_ctx* h, long* nn_out);
 
 /*
  * Order metric tau of Eq. 7 from the LAST evaluation on this handle with D = 1/K, as the lattice sum over +-Q:

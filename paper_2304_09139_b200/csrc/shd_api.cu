@@ -885,6 +885,28 @@ int shd_structure_factor(shd_ctx* h, double* S_out, double dev2[2]) {
     return SHD_OK;
 }
 
+// distinct values of n.n in Q, ascending (the finest radial bins: one per shell)
+static std::vector<long> shells_of(const shd_ctx* h) {
+    std::vector<long> nn((size_t)h->M);
+    for (long k = 0; k < h->M; k++) {
+        long v = 0;
+        for (int a = 0; a < h->d; a++) v += (long)h->nvec[k * h->d + a] * h->nvec[k * h->d + a];
+        nn[(size_t)k] = v;
+    }
+    std::sort(nn.begin(), nn.end());
+    nn.erase(std::unique(nn.begin(), nn.end()), nn.end());
+    return nn;
+}
+
+long shd_num_shells(const shd_ctx* h) { return h ? (long)shells_of(h).size() : 0; }
+
+int shd_get_shells(const shd_ctx* h, long* nn_out) {
+    if (!h || !nn_out) return SHD_EINVAL;
+    const std::vector<long> nn = shells_of(h);
+    std::memcpy(nn_out, nn.data(), nn.size() * sizeof(long));
+    return SHD_OK;
+}
+
 int shd_structure_factor_shells(shd_ctx* h, long nbins, const long* edges, long* count, double* S_mean_hi, double* S_mean_lo) {
     if (!h) return SHD_EINVAL;
     if (nbins < 1 || !edges || !count || !S_mean_hi || !S_mean_lo) return fail(h, SHD_EINVAL, "shd_structure_factor_shells: bad argument");

@@ -19,7 +19,7 @@ EXPORTS = ["shd_create", "shd_create_shell", "shd_create_table", "shd_destroy", 
            "shd_energy_grad", "shd_energy_grad_host", "shd_set_timing", "shd_smax", "shd_last_smax", "shd_get_rho", "shd_minimize",
            "shd_last_error", "shd_stat", "shd_fp64_peak", "shd_structure_factor", "shd_set_precision", "shd_i8_probe", "shd_set_engine",
            "shd_set_workspace", "shd_set_shard", "shd_comm_unique_id", "shd_comm_init", "shd_partial_bytes", "shd_rho_partial", "shd_rho_finish",
-           "shd_grad_local", "shd_structure_factor_shells", "shd_tau", "shd_get_trace", "shd_minimize_snapshot", "shd_mix_probe"]
+           "shd_grad_local", "shd_structure_factor_shells", "shd_tau", "shd_get_trace", "shd_minimize_snapshot", "shd_mix_probe", "shd_num_shells", "shd_get_shells"]
 
 
 class ShdError(RuntimeError):
@@ -94,6 +94,9 @@ def _load():
     lib.shd_get_trace.restype = C.c_long
     lib.shd_minimize_snapshot.argtypes = [vp, vp, vp]
     lib.shd_mix_probe.argtypes = [dp]
+    lib.shd_num_shells.argtypes = [vp]
+    lib.shd_num_shells.restype = C.c_long
+    lib.shd_get_shells.argtypes = [vp, C.POINTER(C.c_long)]
     return lib
 
 
@@ -285,8 +288,8 @@ class Shd:
         """shd_structure_factor_shells on the last evaluation.  edges: ascending integer n.n bin edges (default: one bin
         per distinct shell of this handle's Q).  Returns (edges, count, S_mean_hi, S_mean_lo) as numpy arrays."""
         if edges is None:
-            nn = (self.k().astype(np.int64) ** 2).sum(axis=1)
-            sh = np.unique(nn)
+            sh = np.zeros(int(lib.shd_num_shells(self._h)), dtype=np.int64)
+            self._check(lib.shd_get_shells(self._h, sh.ctypes.data_as(C.POINTER(C.c_long))))
             edges = np.concatenate([sh, [sh[-1] + 1]])
         e = np.ascontiguousarray(edges, dtype=np.int64)
         nb = e.size - 1

@@ -51,3 +51,16 @@ def test_bad_arguments():
     assert shd.lib.shd_create_shell(2, 0, 4.0, 4, None, ctypes.byref(h)) == shd.SHD_EINVAL
     assert shd.lib.shd_create_shell(2, 16, -1.0, 4, None, ctypes.byref(h)) == shd.SHD_EINVAL
     assert shd.lib.shd_create(2, 16, 4.0, float("nan"), None, ctypes.byref(h)) == shd.SHD_EINVAL
+
+
+def test_bench_reads_ncu_traffic_from_profiles():
+    """bench.py's roofline.traffic is parsed from the newest committed ncu summary that states it (nothing hard-coded)."""
+    import sys
+    sys.path.insert(0, str(ROOT))
+    import bench
+    b, src = bench.ncu_traffic("k_grad8", "cfg4")
+    assert src and src.startswith("profiles/r") and 1e8 < b < 1e11
+    b2, src2 = bench.ncu_traffic("k_rho8", "cfg4")
+    assert src2 == src and 1e8 < b2 < 1e11
+    assert bench.ncu_traffic("k_grad8", "no_such_workload") == (None, None)
+    assert bench.ncu_traffic("k_no_such_kernel", "cfg4") == (None, None)

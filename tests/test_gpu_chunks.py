@@ -165,3 +165,33 @@ def test_one_rank_communicator(shd, oracle):
         assert np.array_equal(ta.cpu().numpy(), tc.cpu().numpy()) and np.array_equal(tb.cpu().numpy(), td.cpu().numpy())
     h.close()
     plain.close()
+
+
+def test_workspace_and_shard_errors(shd):
+    """Error behaviour of the new calls (include/shd.h): a cap below one particle split is SHD_ENOMEM at the next
+    evaluation (and lifting it recovers); the split calls refuse a handle that is not a shard; a sharded handle without
+    a communicator refuses the fused calls instead of hanging; bad shard arguments are SHD_EINVAL."""
+    cfg = inputs.CONFIGS["cfg2"]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    th, tl = shd.from_host(hi, lo)
+    ref = h.energy_grad(th, tl)[0]
+    h.set_workspace(4096)
+    with pytest.raises(shd.ShdError) as e:
+        h.energy_grad(th, tl)
+    assert e.value.code == shd.SHD_ENOMEM
+    h.set_workspace(0)
+    assert h.energy_grad(th, tl)[0] == ref
+    with pytest.raises(shd.ShdError) as e:
+        h.rho_partial(th, tl)
+    assert e.value.code == shd.SHD_EINVAL
+    for bad in ((cfg.N - 1, 0, 2), (cfg.N, 2, 2), (cfg.N, -1, 2), (cfg.N, 0, 0)):
+        with pytest.raises(shd.ShdError) as e:
+            h.set_shard(*bad)
+        assert e.value.code == shd.SHD_EINVAL
+    h.set_shard(2 * cfg.N, 0, 2)
+    with pytest.raises(shd.ShdError):
+        h.energy_grad(th, tl)            # two ranks, no communicator: refused, not a hang
+    part = h.rho_partial(th, tl)         # ... while the split calls work
+    assert part.numel() == shd.lib.shd_partial_bytes(h._h)
+    h.close()
