@@ -210,12 +210,14 @@ def run_gpu(args, cfg):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (libshd has no CPU fallback)")
     torch.cuda.set_device(local_rank)
-    if world > 1:
+    if world > 1 or args.force_shard:
         import torch.distributed as dist
+        if args.force_shard and world == 1 and "MASTER_ADDR" not in os.environ:
+            os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT="29517", RANK="0", WORLD_SIZE="1")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     from paper_2304_09139_b200 import shd
 
-    sharded = world > 1 and not args.replicas
+    sharded = (world > 1 and not args.replicas) or args.force_shard
     from paper_2304_09139_b200 import sharding
     if sharded:
         hi, lo = inputs.uniform_positions(cfg, 0)           # one system, its particles dealt out in contiguous ranges
@@ -460,6 +462,8 @@ def main():
     ap.add_argument("--engine", default="auto", choices=["auto", "0", "1", "2"],
                     help="engine of the two O(N M) passes: 0 FP64 limbs (DMMA), 1 rho on INT8 tensor cores, 2 both")
     ap.add_argument("--no-fp64-compare", action="store_true", help="do not time the FP64 limb engine beside the INT8 one")
+    ap.add_argument("--force-shard", action="store_true",
+                    help="N = 1: run the sharded code path anyway (one shard, a library-owned NCCL communicator of one rank)")
     ap.add_argument("--replicas", action="store_true",
                     help="N > 1: independent replicas (weak scaling, no collective) instead of particle shards (strong scaling)")
     ap.add_argument("--midquench-evals", type=int, default=300,

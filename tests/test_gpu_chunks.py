@@ -195,3 +195,41 @@ def test_workspace_and_shard_errors(shd):
     part = h.rho_partial(th, tl)         # ... while the split calls work
     assert part.numel() == shd.lib.shd_partial_bytes(h._h)
     h.close()
+
+
+def test_paper_scale_two_chunks_sampled(shd, oracle):
+    """The paper's own system size at its largest chi (d = 2, N = 2 x 10^6, chi = 0.4; 3.2 x 10^12 pair-terms,
+    225 GB of phasor tables) on one GPU: the default workspace cap (92 % of the free memory) makes it two chunks.
+    Sampled parity against the oracle's definition (direct mode): strided wavevectors x all particles, strided particles
+    x all wavevectors, at BASELINE.json's tolerances.  Skipped when the device has less than 150 GB free."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 150 * 2 ** 30:
+        pytest.skip("needs a 180 GB device with 150 GB free")
+    cfg = inputs.CONFIGS["paper04"]
+    hi, lo = inputs.uniform_positions(cfg, 0)
+    h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
+    assert h.M == cfg.M and h.engine == 2
+    th, tl = shd.from_host(hi, lo)
+    phi, gh, gl = h.energy_grad(th, tl)
+    assert h.stat(19) >= 2, "chunked"
+    rho = [t.cpu().numpy() for t in h.rho()]
+    n = h.k()
+    N, M = cfg.N, cfg.M
+    ks = np.unique(np.concatenate([np.linspace(0, M - 1, 14).astype(np.int64), [0, M - 1, h.last_smax()[1]]]))
+    re, im = oracle.rho(cfg.d, N, cfg.L, hi, lo, n[ks])
+    e_rho = oracle.cabsdiff_dd(re, im, *[x[ks] for x in rho]).max()
+    assert e_rho <= 1e-28 * N, e_rho
+    fr, fi = oracle.from_dd(rho[0], rho[1]), oracle.from_dd(rho[2], rho[3])
+    js = np.unique(np.concatenate([np.linspace(0, N - 1, 10).astype(np.int64), [int(h.stat(25)) - 1, int(h.stat(25))]]))   # incl. both sides of the chunk boundary
+    og = oracle.grad(cfg.d, N, cfg.L, hi, lo, n, fr, fi, jlist=js)
+    g_hi, g_lo = gh.cpu().numpy(), gl.cpu().numpy()
+    sel = np.concatenate([a * N + js for a in range(cfg.d)])
+    e_g = oracle.absdiff_dd(og, g_hi[sel], g_lo[sel]).max()
+    assert e_g <= 1e-27 * N * M * cfg.K, e_g
+    o_phi, _, _, _ = oracle.energy(N, fr, fi)
+    assert oracle.absdiff_dd(o_phi, [phi[0]], [phi[1]])[0] <= 1e-28 * N * N * M
+    print("paper04", dict(chunks=int(h.stat(19)), table_gib=h.stat(26) / 2 ** 30, e_rho=e_rho, e_g=e_g))
+    h.close()
+    del th, tl, gh, gl
+    torch.cuda.empty_cache()
