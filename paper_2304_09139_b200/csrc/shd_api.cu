@@ -343,10 +343,13 @@ int plan_engine8(shd_ctx* h, int engine) {
         double best = -1.0;
         h->nseg8 = 1;
         const long njb128 = (h->N + 127) / 128;
-        // at least two segments: the CTAs of one particle block then stream the same digit slabs side by side (L2)
+        // at least two segments: the CTAs of one particle block then stream the same digit slabs side by side (L2).
+        // The kernel is persistent (one CTA per SM walks the units round-robin), so a unit costs its steps plus about one
+        // block's epilogue (1.5 step-times), not a CTA prologue: finer segments balance small systems (cfg3: 79 particle
+        // blocks on 148 SMs) at the price of one more partial gradient per segment for k_gradsum to add (0.05 each).
         for (int ns = std::min(2, h->nsteps8); ns <= std::min(32, h->nsteps8); ns++) {
-            const long waves = (njb128 * ns + sms - 1) / sms;
-            const double cost = (double)waves * ((double)((h->nsteps8 + ns - 1) / ns) + 6.0);
+            const long rounds = (njb128 * ns + sms - 1) / sms;
+            const double cost = (double)rounds * ((double)((h->nsteps8 + ns - 1) / ns) + 1.5) + 0.05 * ns;
             if (best < 0.0 || cost < best) { best = cost; h->nseg8 = ns; }
         }
         if ((rc = upload(h, &h->d_steps8, steps))) return rc;
