@@ -153,7 +153,7 @@ def workload_config(cfg, world, replicas=True):
             "d": cfg.d, "N": cfg.N, "M": cfg.M, "pair_terms_per_eval": cfg.pairs,
             "parallelism": "single GPU" if world == 1 else (f"{world} independent replicas (seed = rank)" if replicas else
                             f"{world} particle shards, one all-gather of partial rho per evaluation (NCCL)"),
-            "l2": "256 MB memset between timed steps; the streamed phasor tables are GBs (>> 126 MB L2)"}
+            "l2": "256 MB memset between timed steps (> 126 MB L2); table_bytes = the phasor tables an evaluation streams"}
 
 
 # ------------------------------------------------------------------------------ clocks
