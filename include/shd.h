@@ -193,6 +193,29 @@ int shd_grad_local(shd_ctx* h, const double* pos_hi, const double* pos_lo, doubl
 int shd_structure_factor(shd_ctx* h, double* S_out, double dev2[2]);
 
 /*
+ * shd_structure_factor for callers that must not allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same two kernels and the same fixed reduction tree, so S_out and dev2 are
+ * bit-identical to shd_structure_factor's, but the per-block partial sums live in a file-scope device array of the
+ * library instead of a cudaMalloc'ed buffer.  The call makes no cudaMalloc / cudaFree and calls no allocating library
+ * routine; it enqueues two kernels on the handle's stream.
+ *   input : the rho(k) of the LAST evaluation on this handle (as shd_structure_factor);
+ *   S_out : DEVICE, |Q| doubles, may be NULL;   dev2 : DEVICE, 2 doubles (hi, lo) -- note: device, not host;
+ *   wait  : nonzero = cudaStreamSynchronize before returning; 0 = return once enqueued (read the outputs after the
+ *           handle's stream has been synchronised).
+ * Limit: |Q| <= SHD_NOALLOC_MAX_Q (the array holds 2 doubles per 256 wavevectors: 256 KiB of device memory that EVERY
+ * GPU which loads libshd.so holds until the process exits).  A handle with more wavevectors gets SHD_EINVAL and a message
+ * naming the limit; use shd_structure_factor there.  The handle's device must be the current device (checked, SHD_EINVAL).
+ * The first call on each device resolves the array's device address (cudaGetSymbolAddress: no allocation by this
+ * library, but the CUDA runtime may load the module then) -- make one call per device before a capture.
+ * ALL calls on a device share the one array.  It keeps the last call's contents; nothing has to start at zero (every
+ * element the second kernel reads was written by the first kernel of the same call).  Two calls whose kernels overlap
+ * on the GPU (different handles = different streams, or two host threads) RACE on it: serialise them.
+ * Errors: SHD_EINVAL, SHD_ECUDA.
+ */
+#define SHD_NOALLOC_MAX_Q 4194304L
+int shd_structure_factor_noalloc(shd_ctx* h, double* S_out, double* dev2, int wait);
+
+/*
  * Radially averaged structure factor of the LAST evaluation (Fig. 2a, Fig. S1a: S against |k|, beyond K when
  * the handle's cutoff reaches there).  |k|^2 = (2 pi / L)^2 n.n, so a radial bin is a range of the integer n.n: bin b
  * holds the wavevectors with edges[b] <= n.n < edges[b+1] (HOST, nbins + 1 strictly ascending longs; index work only,

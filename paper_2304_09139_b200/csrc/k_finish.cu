@@ -5,6 +5,8 @@
 #include "dd.cuh"
 #include "shd_internal.h"
 
+#include <cstdio>
+
 namespace {
 
 struct red { dd phi; dd smax; long long arg; double maxvs; };
@@ -376,4 +378,64 @@ cudaError_t shd_launch_ctable(shd_ctx* h)
         h->npb16, h->Qpad, h->qscale_log2, h->d_cell_kp, h->d_cell_km, h->M, h->d_v, h->d_rho, h->d_scal, h->d_C, h->d_skip);
     h->last_launches += 1;
     return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// shd_structure_factor_noalloc (include/shd.h): k_sfactor1 / k_sfactor2 as above, with the per-block partial sums in a
+// file-scope device array instead of a cudaMalloc'ed buffer, for callers that must not allocate.  2 doubles per block of
+// 256 wavevectors: SHD_NOALLOC_MAX_Q / 256 blocks = 256 KiB, held by every GPU that loads this library until exit.
+// Every call on a device shares the array: calls whose kernels overlap on the GPU race on it (shd.h says so).  Nothing
+// in it has to start at zero: k_sfactor2 reads the 2 nb doubles that the nb blocks of k_sfactor1 of the same call wrote.
+static __device__ __align__(256) double g_sf_scratch[2 * (SHD_NOALLOC_MAX_Q / 256)];
+
+namespace {
+
+// In HOST code the name g_sf_scratch is a stand-in the runtime uses to find the array, not a device address: a kernel
+// handed `g_sf_scratch` from here would fault (or, where the GPU reaches host memory, write somewhere else).  The device
+// address is per device: resolved once for each, with that device current, and kept.
+constexpr int SF_MAX_DEVICES = 64;
+double* g_sf_scratch_addr[SF_MAX_DEVICES];
+
+cudaError_t sf_scratch_address(int dev, double** out)
+{
+    double* p = __atomic_load_n(&g_sf_scratch_addr[dev], __ATOMIC_ACQUIRE);
+    if (!p) {
+        void* sym = nullptr;
+        cudaError_t e = cudaGetSymbolAddress(&sym, g_sf_scratch);     // `dev` is the current device (caller checked)
+        if (e != cudaSuccess) return e;
+        if (!sym) return cudaErrorInvalidSymbol;
+        p = (double*)sym;
+        __atomic_store_n(&g_sf_scratch_addr[dev], p, __ATOMIC_RELEASE);   // two racing first calls store the same value
+    }
+    *out = p;
+    return cudaSuccess;
+}
+
+int sf_fail(shd_ctx* h, int code, const char* msg) { h->err = msg; return code; }
+
+}  // namespace
+
+extern "C" int shd_structure_factor_noalloc(shd_ctx* h, double* S_out, double* dev2, int wait)
+{
+    if (!h) return SHD_EINVAL;
+    if (!dev2) return sf_fail(h, SHD_EINVAL, "shd_structure_factor_noalloc: dev2 is NULL");
+    if (h->M > SHD_NOALLOC_MAX_Q) {
+        char msg[192];
+        snprintf(msg, sizeof msg, "shd_structure_factor_noalloc: |Q| = %ld exceeds SHD_NOALLOC_MAX_Q = %ld (the static scratch "
+                 "array); use shd_structure_factor", h->M, (long)SHD_NOALLOC_MAX_Q);
+        return sf_fail(h, SHD_EINVAL, msg);
+    }
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    cudaPointerAttributes attr;
+    if (e == cudaSuccess) e = cudaPointerGetAttributes(&attr, h->d_rho);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return sf_fail(h, SHD_ECUDA, cudaGetErrorString(e)); }
+    if (dev < 0 || dev >= SF_MAX_DEVICES || attr.type != cudaMemoryTypeDevice || attr.device != dev)
+        return sf_fail(h, SHD_EINVAL, "shd_structure_factor_noalloc: the handle's device is not the current device");
+    double* scratch = nullptr;
+    e = sf_scratch_address(dev, &scratch);
+    if (e == cudaSuccess) e = shd_launch_sfactor(h, S_out, scratch, dev2);
+    if (e == cudaSuccess && wait) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return sf_fail(h, SHD_ECUDA, cudaGetErrorString(e)); }
+    return SHD_OK;
 }

@@ -15,11 +15,13 @@ _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libshd.so"
 
 SHD_OK, SHD_EINVAL, SHD_ENOMEM, SHD_ECUDA, SHD_ENAN, SHD_ESTALL, SHD_EMAXEVAL, SHD_ESTOPPED = 0, -1, -2, -3, -4, -5, -6, -7
+SHD_NOALLOC_MAX_Q = 4194304          # shd.h: the most wavevectors shd_structure_factor_noalloc accepts
 EXPORTS = ["shd_create", "shd_create_shell", "shd_create_table", "shd_destroy", "shd_set_stream", "shd_num_k", "shd_get_k",
            "shd_energy_grad", "shd_energy_grad_host", "shd_set_timing", "shd_smax", "shd_last_smax", "shd_get_rho", "shd_minimize",
            "shd_last_error", "shd_stat", "shd_fp64_peak", "shd_structure_factor", "shd_set_precision", "shd_i8_probe", "shd_set_engine",
            "shd_set_workspace", "shd_set_shard", "shd_comm_unique_id", "shd_comm_init", "shd_partial_bytes", "shd_rho_partial", "shd_rho_finish",
-           "shd_grad_local", "shd_structure_factor_shells", "shd_tau", "shd_get_trace", "shd_minimize_snapshot", "shd_mix_probe", "shd_num_shells", "shd_get_shells"]
+           "shd_grad_local", "shd_structure_factor_shells", "shd_tau", "shd_get_trace", "shd_minimize_snapshot", "shd_mix_probe", "shd_num_shells", "shd_get_shells",
+           "shd_structure_factor_noalloc"]
 
 
 class ShdError(RuntimeError):
@@ -76,6 +78,7 @@ def _load():
     lib.shd_stat.restype = C.c_double
     lib.shd_fp64_peak.argtypes = [C.c_int, C.c_double, dp]
     lib.shd_structure_factor.argtypes = [vp, vp, dp]
+    lib.shd_structure_factor_noalloc.argtypes = [vp, vp, vp, C.c_int]
     lib.shd_set_precision.argtypes = [vp, C.c_int]
     lib.shd_i8_probe.argtypes = [dp, C.POINTER(C.c_long)]
     lib.shd_set_engine.argtypes = [vp, C.c_int]
@@ -277,6 +280,15 @@ class Shd:
         dev2 = (C.c_double * 2)()
         self._check(lib.shd_structure_factor(self._h, C.c_void_p(S.data_ptr()) if want_S else None, dev2))
         return S, (dev2[0], dev2[1])
+
+    def structure_factor_noalloc(self, dev2, S=None, wait=True):
+        """shd_structure_factor_noalloc on the last evaluation: the caller passes the outputs (dev2: CUDA float64 tensor
+        of 2 elements; S: CUDA float64 tensor of |Q| elements or None); nothing is allocated by the call."""
+        for t, n in ((dev2, 2), (S, self.M)):
+            if t is not None and not (t.is_cuda and t.dtype == _torch().float64 and t.is_contiguous() and t.numel() == n):
+                raise ValueError("structure_factor_noalloc: outputs must be contiguous CUDA float64 tensors of 2 and |Q| elements")
+        self._check(lib.shd_structure_factor_noalloc(self._h, C.c_void_p(S.data_ptr()) if S is not None else None,
+                                                     C.c_void_p(dev2.data_ptr()), 1 if wait else 0))
 
     def tau(self, K):
         """shd_tau: order metric tau of Eq. 7 from the last evaluation on this handle, D = 1/K (hi + lo)."""
