@@ -202,8 +202,13 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
                     if (n <= 256) {
                         g8_mma(tb, da, dW0 + (uint64_t)((l0 * G8_WSLAB) >> 4), g8_idesc(n), acc, elected);
                     } else {
-                        g8_mma(tb, da, dW0 + (uint64_t)((l0 * G8_WSLAB) >> 4), g8_idesc(256), acc, elected);
-                        g8_mma(tb + 256, da, dW0 + (uint64_t)(((l0 + 8) * G8_WSLAB) >> 4), g8_idesc(n - 256), acc, elected);
+                        // two instructions of n / 2 columns each, not 256 + the rest: an instruction reads its 4 KB A
+                        // slab and 32 n bytes of the other operand from shared memory, about 32 + n / 4 cycles, against
+                        // n / 2 cycles of arithmetic, so below n = 128 the operand fetch is what it costs (measured:
+                        // the 256 + rest split is 2.5 % slower in k_grad8, 1 % in k_rho8; profiles/r2b_summary.md)
+                        const int n1 = n / 2;                                  // 144 .. 208: a multiple of 16
+                        g8_mma(tb, da, dW0 + (uint64_t)((l0 * G8_WSLAB) >> 4), g8_idesc(n1), acc, elected);
+                        g8_mma(tb + n1, da, dW0 + (uint64_t)((l0 * G8_WSLAB + n1 * 32) >> 4), g8_idesc(n - n1), acc, elected);
                     }
                 };
                 // Every step runs upwards, short instructions first and long ones last, so that the tensor core's queue

@@ -140,8 +140,13 @@ __global__ void __launch_bounds__(192, 1) k_rho8(
                     if (n <= 256) {
                         umma_i8(tb, da, dB0 + (uint64_t)((l0 * R8_BSLAB) >> 4), umma_idesc_i8(n), acc, elected);
                     } else {
-                        umma_i8(tb, da, dB0 + (uint64_t)((l0 * R8_BSLAB) >> 4), umma_idesc_i8(256), acc, elected);
-                        umma_i8(tb + 256, da, dB0 + (uint64_t)(((l0 + 8) * R8_BSLAB) >> 4), umma_idesc_i8(n - 256), acc, elected);
+                        // two instructions of n / 2 columns each, not 256 + the rest: an instruction reads its 4 KB A
+                        // slab and 32 n bytes of the other operand from shared memory, about 32 + n / 4 cycles, against
+                        // n / 2 cycles of arithmetic, so below n = 128 the operand fetch is what it costs (measured:
+                        // the 256 + rest split is 2.5 % slower in k_grad8, 1 % in k_rho8; profiles/r2b_summary.md)
+                        const int n1 = n / 2;                                  // 144 .. 208: a multiple of 16
+                        umma_i8(tb, da, dB0 + (uint64_t)((l0 * R8_BSLAB) >> 4), umma_idesc_i8(n1), acc, elected);
+                        umma_i8(tb + n1, da, dB0 + (uint64_t)((l0 * R8_BSLAB + n1 * 32) >> 4), umma_idesc_i8(n - n1), acc, elected);
                     }
                 };
                 if (i == 0 || ND < R8_ND) {                         // (with fewer digits the order makes no difference)

@@ -49,6 +49,8 @@ def main(argv=None):
     ap.add_argument("--ladder1", type=float, default=0.0,
                     help="optional first rung below that: ONE limb (22-bit operands) until S_max < this value, "
                          "e.g. 1e-8")
+    ap.add_argument("--start", default=None,
+                    help="continue from positions saved by --save (PREFIX_hi.npy, PREFIX_lo.npy) instead of the seeded start")
     ap.add_argument("--out", default=None)
     ap.add_argument("--save", default=None)
     args = ap.parse_args(argv)
@@ -58,6 +60,10 @@ def main(argv=None):
 
     cfg = inputs.CONFIGS[args.config]
     hi, lo = inputs.uniform_positions(cfg, args.seed)
+    if args.start:
+        hi, lo = np.load(args.start + "_hi.npy").reshape(-1), np.load(args.start + "_lo.npy").reshape(-1)
+        if hi.size != cfg.d * cfg.N or lo.size != hi.size:
+            raise SystemExit(f"--start: {args.start}_hi/_lo.npy do not hold d*N = {cfg.d * cfg.N} doubles each")
     v = None
     h = shd.Shd(cfg.d, cfg.N, cfg.L, m_star=cfg.m_star)
     if args.weight == "n2":
@@ -105,7 +111,7 @@ def main(argv=None):
     smax, arg = h.smax(pos_hi, pos_lo)
     n = h.k()
     line = {"config": cfg.name, "d": cfg.d, "N": cfg.N, "M": cfg.M, "chi_realised": cfg.M / (cfg.d * (cfg.N - 1)),
-            "seed": args.seed, "kind": "lbfgs" if args.kind == 0 else "fire", "weight": args.weight, "engine": h.engine,
+            "seed": args.seed, "start": args.start, "kind": "lbfgs" if args.kind == 0 else "fire", "weight": args.weight, "engine": h.engine,
             "chunks": int(h.stat(19)), "history": args.history,
             "tol": args.tol, "ladder": args.ladder, "ladder1": args.ladder1, "status": status, "evals": evals, "iters": iters,
             "evals_by_limbs": by_limbs, "seconds": seconds,
