@@ -131,7 +131,8 @@ constexpr int TABLES_SMEM = TABLES_LIMB_SMEM + TG * 2 * SHD_I8_DIGITS * TB;   //
 //   rho layout       T[block][j/4][limb 3][32 entries][j%4][re,im]            (A and B)
 //   gradient layout  Bg[j/32][q/4][limb 3][j%32][q%4][re,im]
 // DLO = first digit in use (0, 6 or 9 for 13, 7 or 4 digits, shd_set_precision): lower digit slabs are not written
-template <int DLO>
+// LIMBS = false: no FP64 limb table is written (both passes on the INT8 engine): the limb staging is compiled out
+template <int DLO, bool LIMBS>
 struct Stager {
     double2* tile;        // [TB][planes][TG]
     int planes;           // 3 limbs
@@ -238,7 +239,7 @@ struct Stager {
     }
     __device__ __forceinline__ static int swz(int r) { return ((r & 1) << 2) | (r & 2) | ((r >> 2) & 1); }
     __device__ __forceinline__ void put(int plane0, int slot, cdd z, bool live) {
-        if (table == nullptr && Bg == nullptr) return;
+        if (!LIMBS || (table == nullptr && Bg == nullptr)) return;
         limbs a = split_limbs(z.re), b = split_limbs(z.im);
         if (!live) a.x0 = a.x1 = a.x2 = b.x0 = b.x1 = b.x2 = 0.0;    // particles beyond N: zero limbs (a chunk's table is reused)
         const int t = threadIdx.x, c = slot ^ swz(t);
@@ -256,7 +257,7 @@ struct Stager {
         // rho layout: (j/4, limb, entry, j%4), j%4 fastest.  Thread = (half of the block's 8-particle rows, entry c,
         // j%4); it walks the 8 row groups and 3 limbs with compile-time strides on both sides (a warp writes 512
         // contiguous bytes per store), so an iteration is one shared load, one global store and a predicate.
-        if (table != nullptr) {
+        if (LIMBS && table != nullptr) {
             const int t = threadIdx.x, half = t >> 5, jj = t & 3, c = (t >> 2) & 7, r0 = 4 * half + jj;
             const double2* src = tile + r0 * planes * TG + (c ^ swz(r0));
             double2* dst = reinterpret_cast<double2*>(table) +
@@ -270,7 +271,7 @@ struct Stager {
                     if (ok) dst[(size_t)(6 * a + l) * 128] = src[(a * 8 * 3 + l) * TG];
             }
         }
-        if (Bg != nullptr) {
+        if (LIMBS && Bg != nullptr) {
             // gradient layout: (j/32, q-group, plane, j%32, q%4), q%4 fastest.  Thread = (j%16, q%4); the walk over
             // (j/32, q-group, plane, upper half of j%32) has compile-time strides on the shared-memory side and
             // loop-invariant ones on the global side
@@ -302,7 +303,8 @@ struct Stager {
 };
 
 // which = 0: A table.  which = 1: B table (+ the same limbs in the gradient layout Bg).
-template <int DLO>
+// HID = true: d >= 3 (A entries are products of per-axis powers kept in local tables); false: d <= 2 (one recurrence)
+template <int DLO, bool LIMBS, bool HID>
 __global__ void __launch_bounds__(TB, 8) k_tables(
     int d, long N, long j_first, double L, long Npad, int P, int Qn, int S1d, int qscale_log2,
     const int* __restrict__ pn0, const int* __restrict__ pn1, const int* __restrict__ pn2, int Qpad,
@@ -325,7 +327,7 @@ __global__ void __launch_bounds__(TB, 8) k_tables(
     const long jc = live ? j_first + j : N - 1;  // dead threads shadow the last particle (keeps barriers uniform)
     const cdd one{dd{1.0, 0.0}, dd{0.0, 0.0}};
     const bool gradB = which == 1 && with_grad != 0;
-    Stager<DLO> st;
+    Stager<DLO, LIMBS> st;
     st.tile = tile; st.planes = 3;
     st.table = which == 0 ? A : B;                      // may be nullptr: the INT8 rho pass does not read B limbs
     st.Bg = gradB ? Bg : nullptr;                       // nullptr too when the gradient pass runs on INT8
@@ -333,7 +335,7 @@ __global__ void __launch_bounds__(TB, 8) k_tables(
     st.gdig = gradB ? Bg8 : nullptr; st.nkq = nkq8;
     st.dig = which == 0 ? A8 : B8; st.nk8 = nk8; st.rows8 = which == 0 ? SHD_I8_PT : SHD_I8_QT;
     // (the limb staging tile comes first when a limb table is written; the digit transpose tile follows it)
-    const bool limb_tile = A != nullptr || B != nullptr || Bg != nullptr;
+    const bool limb_tile = LIMBS && (A != nullptr || B != nullptr || Bg != nullptr);
     st.dtile = reinterpret_cast<signed char*>(tables_smem) + (limb_tile ? TABLES_LIMB_SMEM : 0);
     st.afix = (which == 0 && with_grad != 0) ? Afix : nullptr; st.NpadA = NpadA;
     if (which == 0) {
@@ -343,7 +345,7 @@ __global__ void __launch_bounds__(TB, 8) k_tables(
         else base = expi_turns(frac_turns(pos_hi[jc], pos_lo[jc], L, 1.0));
         const int e_end = min(P, e_begin + ech);
         if (e_begin >= P) return;
-        if (d <= 2) {
+        if (!HID) {
             cdd cur = e_begin == 0 ? one : cdd_pow(base, e_begin);
             for (int p0 = e_begin; p0 < e_end; p0 += TG) {
                 const int cnt = min(TG, e_end - p0);
@@ -431,9 +433,16 @@ __global__ void __launch_bounds__(TB, 8) k_tables(
 
 cudaError_t shd_tables_configure()
 {
-    cudaError_t e = cudaFuncSetAttribute(k_tables<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, TABLES_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tables<6>, cudaFuncAttributeMaxDynamicSharedMemorySize, TABLES_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tables<9>, cudaFuncAttributeMaxDynamicSharedMemorySize, TABLES_SMEM);
+    cudaError_t e = cudaSuccess;
+#define CONF_TABLES(DLOV)                                                                                                   \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tables<DLOV, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TABLES_SMEM);  \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tables<DLOV, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TABLES_SMEM);   \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tables<DLOV, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, TABLES_SMEM); \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tables<DLOV, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, TABLES_SMEM);
+    CONF_TABLES(0)
+    CONF_TABLES(6)
+    CONF_TABLES(9)
+#undef CONF_TABLES
     return e;
 }
 
@@ -462,15 +471,22 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
     // tables (Afix, Bg8) go out from registers
     // (8 CTAs of 64 threads per SM by registers; without the 24 KB limb tile the shared memory allows them too)
     const size_t smem = ((A || B || Bg) ? TABLES_LIMB_SMEM : 0) + ((A8 || B8) ? TABLES_SMEM - TABLES_LIMB_SMEM : 0);
-#define LAUNCH_TABLES(DLOV)                                                                                       \
-    k_tables<DLOV><<<grid, TB, smem, h->stream>>>(h->d, h->N, j_first, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2, \
+    const bool limbs = A || B || Bg, hid = h->d > 2;
+#define LAUNCH_TABLES_(DLOV, LV, HV)                                                                               \
+    k_tables<DLOV, LV, HV><<<grid, TB, smem, h->stream>>>(h->d, h->N, j_first, h->L, h->Npad, h->P, h->Qn, h->S1d, h->qscale_log2, \
                                          h->d_pn0, h->d_pn1, h->d_pn2, h->Qpad, pos_hi, pos_lo, A, B, Bg, grad ? 1 : 0, \
                                          A8, B8, h->nk8, Bg8, h->nkq8, Afix, h->njb128 * 128, ech, h->d_skip)
+#define LAUNCH_TABLES(DLOV)                                                                                       \
+    do {                                                                                                          \
+        if (limbs) { if (hid) LAUNCH_TABLES_(DLOV, true, true); else LAUNCH_TABLES_(DLOV, true, false); }         \
+        else       { if (hid) LAUNCH_TABLES_(DLOV, false, true); else LAUNCH_TABLES_(DLOV, false, false); }       \
+    } while (0)
     // the INT8 engines read only the 13, 7 or 4 most significant digits (shd_set_precision): the rest is not written
     if (e == 0 || h->nlimb >= 3) LAUNCH_TABLES(0);
     else if (h->nlimb == 2) LAUNCH_TABLES(6);
     else LAUNCH_TABLES(9);
 #undef LAUNCH_TABLES
+#undef LAUNCH_TABLES_
     h->last_launches += 1;
     return cudaGetLastError();
 }
