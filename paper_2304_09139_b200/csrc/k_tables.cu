@@ -458,7 +458,9 @@ cudaError_t shd_launch_tables(shd_ctx* h, const double* pos_hi, const double* po
     // binary power, rounded differently from the recurrence, and results must not depend on the workspace cap.
     const int emax = std::max(h->P, h->Qn);
     int ech = ((emax + 7) / 8) * 8;
-    if (h->N < 96 * 1024 && emax > 32) ech = h->N < 24 * 1024 ? 16 : 32;
+    // (d >= 3: a chunk start also rebuilds the local power tables, so chunks are twice as long; measured at cfg3: 0.189 ms
+    // with 16-entry chunks, 0.178 with 32, 0.176 with 48, 0.203 with 64)
+    if (h->N < 96 * 1024 && emax > 32) ech = (h->N < 24 * 1024 && h->d <= 2) ? 16 : 32;
     dim3 grid((unsigned)((slots + TB - 1) / TB), 2, (unsigned)((emax + ech - 1) / ech));
     double* A = (e == 2 || !(rho || grad)) ? nullptr : ((e == 1 && !grad) ? nullptr : h->d_A);   // FP64 rho pass and FP64 gradient pass
     double* B = (e == 0 && rho) ? h->d_B : nullptr;
