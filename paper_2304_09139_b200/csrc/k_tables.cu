@@ -122,7 +122,10 @@ constexpr int R4MAX = 32;    // d == 4: max |n_2|
 constexpr int TB = 64;       // particles (threads) per block
 constexpr int TG = 8;        // table entries staged per flush: 8 x 16 B = one 128-byte row per limb plane
 constexpr int TABLES_LIMB_SMEM = TB * 3 * TG * 16;
-constexpr int TABLES_SMEM = TABLES_LIMB_SMEM + TG * 2 * SHD_I8_DIGITS * TB;   // + digit transpose tile
+// digit transpose tile: rows of 13 digits x TB particles, padded by 16 bytes so that the 16-byte reads of flush8 (eight
+// rows per shared-memory wavefront) fall into eight different bank groups (832-byte rows: two)
+constexpr int DROW = SHD_I8_DIGITS * TB + 16;
+constexpr int TABLES_SMEM = TABLES_LIMB_SMEM + TG * 2 * DROW;
 
 // Staging tile: a thread owns one particle, so its 16-byte stores would land far apart in global
 // memory.  They go to shared memory instead (tile[particle][plane][TG entries], 16-byte chunks
@@ -196,7 +199,7 @@ struct Stager {
     signed char* dig;     // rho pass (or nullptr): row = 2 (entry % rows8) + re/im of block entry / rows8,
     long nk8;             //   K index = particle % 32 of K-step particle / 32 (nk8 K-steps per block)
     int rows8;            // entries per block: 64 (A) or 16 (B)
-    signed char* dtile;   // shared-memory transpose tile [TG entries][2][13 digits][TB particles]
+    signed char* dtile;   // shared-memory transpose tile [TG entries][2] rows of DROW bytes: [13 digits][TB particles] + pad
     // digits of one table entry for both INT8 tables (computed once)
     __device__ __forceinline__ void put_digits(int slot, cdd z, bool live, int entry = -1) {
         if (dig == nullptr && gdig == nullptr && afix == nullptr) return;
@@ -210,11 +213,11 @@ struct Stager {
     }
     __device__ __forceinline__ void put8(int slot, const digits13_t& dr, const digits13_t& di) {
         if (dig == nullptr) return;
-        signed char* t = dtile + (size_t)(slot * 2) * SHD_I8_DIGITS * TB + threadIdx.x;
+        signed char* t = dtile + (size_t)(slot * 2) * DROW + threadIdx.x;
 #pragma unroll
         for (int i = DLO; i < SHD_I8_DIGITS; i++) {
             t[(size_t)i * TB] = (signed char)digit_byte(dr, i);
-            t[(size_t)(SHD_I8_DIGITS + i) * TB] = (signed char)digit_byte(di, i);
+            t[(size_t)DROW + i * TB] = (signed char)digit_byte(di, i);
         }
     }
     // after the block-wide barrier of flush(): 16-byte chunks (16 particles of one row of one digit), consecutive
@@ -230,7 +233,7 @@ struct Stager {
         const int rl = threadIdx.x % (2 * TG), kh = threadIdx.x / (2 * TG);
         if (rl < nrow && (j0 >> 5) + (kh >> 1) < nk8) {            // (the last block may reach past the table's K-steps)
             const int r = r_first + rl;
-            const signed char* src = dtile + (size_t)rl * SHD_I8_DIGITS * TB + kh * 16;
+            const signed char* src = dtile + (size_t)rl * DROW + kh * 16;
             signed char* dst = base + (size_t)(kh >> 1) * SHD_I8_DIGITS * slab + (r >> 3) * 256 + (kh & 1) * 128 + (r & 7) * 16;
 #pragma unroll
             for (int dg = DLO; dg < SHD_I8_DIGITS; dg++)
