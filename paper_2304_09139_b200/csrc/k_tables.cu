@@ -122,9 +122,9 @@ constexpr int R4MAX = 32;    // d == 4: max |n_2|
 constexpr int TB = 64;       // particles (threads) per block
 constexpr int TG = 8;        // table entries staged per flush: 8 x 16 B = one 128-byte row per limb plane
 constexpr int TABLES_LIMB_SMEM = TB * 3 * TG * 16;
-// digit transpose tile: rows of 13 digits x TB particles, padded by 16 bytes so that the 16-byte reads of flush8 (eight
-// rows per shared-memory wavefront) fall into eight different bank groups (832-byte rows: two)
-constexpr int DROW = SHD_I8_DIGITS * TB + 16;
+// digit transpose tile: rows of 4 packed digit words x TB particles, padded by 16 bytes so that the 16-byte reads of
+// flush8 (eight rows per shared-memory wavefront) fall into eight different bank groups
+constexpr int DROW = 4 * TB * 4 + 16;
 constexpr int TABLES_SMEM = TABLES_LIMB_SMEM + TG * 2 * DROW;
 
 // Staging tile: a thread owns one particle, so its 16-byte stores would land far apart in global
@@ -199,7 +199,7 @@ struct Stager {
     signed char* dig;     // rho pass (or nullptr): row = 2 (entry % rows8) + re/im of block entry / rows8,
     long nk8;             //   K index = particle % 32 of K-step particle / 32 (nk8 K-steps per block)
     int rows8;            // entries per block: 64 (A) or 16 (B)
-    signed char* dtile;   // shared-memory transpose tile [TG entries][2] rows of DROW bytes: [13 digits][TB particles] + pad
+    signed char* dtile;   // shared-memory transpose tile [TG entries][2] rows of DROW bytes: [4 digit words][TB particles] + pad
     // digits of one table entry for both INT8 tables (computed once)
     __device__ __forceinline__ void put_digits(int slot, cdd z, bool live, int entry = -1) {
         if (dig == nullptr && gdig == nullptr && afix == nullptr) return;
@@ -211,33 +211,55 @@ struct Stager {
         put8(slot, dr, di);
         putg8(slot, dr, di);
     }
+    // first 32-bit word of the packed digits in use (words: digits 0-3, 4-6, 7-10, 11-12)
+    static constexpr int W0 = DLO < 4 ? 0 : DLO < 7 ? 1 : DLO < 11 ? 2 : 3;
+    // the packed digit words go to the tile as they are (conflict-free 32-bit stores); flush8 separates the bytes
     __device__ __forceinline__ void put8(int slot, const digits13_t& dr, const digits13_t& di) {
         if (dig == nullptr) return;
-        signed char* t = dtile + (size_t)(slot * 2) * DROW + threadIdx.x;
+        uint32_t* t = reinterpret_cast<uint32_t*>(dtile + (size_t)(slot * 2) * DROW) + threadIdx.x;
+        const uint32_t wr[4] = {(uint32_t)dr.lo, (uint32_t)(dr.lo >> 32), (uint32_t)dr.hi, (uint32_t)(dr.hi >> 32)};
+        const uint32_t wi[4] = {(uint32_t)di.lo, (uint32_t)(di.lo >> 32), (uint32_t)di.hi, (uint32_t)(di.hi >> 32)};
 #pragma unroll
-        for (int i = DLO; i < SHD_I8_DIGITS; i++) {
-            t[(size_t)i * TB] = (signed char)digit_byte(dr, i);
-            t[(size_t)DROW + i * TB] = (signed char)digit_byte(di, i);
+        for (int w = W0; w < 4; w++) {
+            t[w * TB] = wr[w];
+            t[DROW / 4 + w * TB] = wi[w];
         }
     }
-    // after the block-wide barrier of flush(): 16-byte chunks (16 particles of one row of one digit), consecutive
-    // threads write consecutive chunks of a 128-byte line (8 rows)
+    // after the block-wide barrier of flush(): thread = (row of the group, 16 particles of the block).  Per digit word it
+    // reads the 16 particles' words (four 16-byte loads), transposes 4 x 4 bytes by byte permutes (eight per four words) and
+    // writes one 16-byte chunk per digit (16 particles of one row of one digit); consecutive threads write consecutive
+    // chunks of a 128-byte line (8 rows)
     __device__ __forceinline__ void flush8(int e0, int count) {
         if (dig == nullptr) return;
         const size_t slab = (size_t)rows8 * 2 * 32;
         const int nrow = 2 * count;                                                 // rows of this group
         signed char* base = dig + ((size_t)(e0 / rows8) * nk8 + (size_t)(j0 >> 5)) * SHD_I8_DIGITS * slab;
         const int r_first = 2 * (e0 % rows8);
-        // thread = (row of the group, 16-particle chunk of the block): both fixed while it walks the digits
         static_assert(TB == 2 * TG * (TB / 16), "one pass of the block covers one digit");
         const int rl = threadIdx.x % (2 * TG), kh = threadIdx.x / (2 * TG);
         if (rl < nrow && (j0 >> 5) + (kh >> 1) < nk8) {            // (the last block may reach past the table's K-steps)
             const int r = r_first + rl;
-            const signed char* src = dtile + (size_t)rl * DROW + kh * 16;
+            const uint32_t* src = reinterpret_cast<const uint32_t*>(dtile + (size_t)rl * DROW) + kh * 16;
             signed char* dst = base + (size_t)(kh >> 1) * SHD_I8_DIGITS * slab + (r >> 3) * 256 + (kh & 1) * 128 + (r & 7) * 16;
 #pragma unroll
-            for (int dg = DLO; dg < SHD_I8_DIGITS; dg++)
-                *reinterpret_cast<uint4*>(dst + (size_t)dg * slab) = *reinterpret_cast<const uint4*>(src + dg * TB);
+            for (int w = W0; w < 4; w++) {
+                constexpr int first[4] = {0, 4, 7, 11};
+                uint32_t o[4][4];                                   // o[byte of the word = digit][group of four particles]
+#pragma unroll
+                for (int g = 0; g < 4; g++) {
+                    const uint4 a = *reinterpret_cast<const uint4*>(src + w * TB + 4 * g);
+                    const uint32_t t0 = __byte_perm(a.x, a.y, 0x5140), t1 = __byte_perm(a.z, a.w, 0x5140);
+                    const uint32_t t2 = __byte_perm(a.x, a.y, 0x7362), t3 = __byte_perm(a.z, a.w, 0x7362);
+                    o[0][g] = __byte_perm(t0, t1, 0x5410); o[1][g] = __byte_perm(t0, t1, 0x7632);
+                    o[2][g] = __byte_perm(t2, t3, 0x5410); o[3][g] = __byte_perm(t2, t3, 0x7632);
+                }
+#pragma unroll
+                for (int bb = 0; bb < 4; bb++) {
+                    const int dg = first[w] + bb;
+                    if (dg >= DLO && dg < (w < 3 ? first[w + 1 < 4 ? w + 1 : 3] : SHD_I8_DIGITS))
+                        *reinterpret_cast<uint4*>(dst + (size_t)dg * slab) = make_uint4(o[bb][0], o[bb][1], o[bb][2], o[bb][3]);
+                }
+            }
         }
     }
     __device__ __forceinline__ static int swz(int r) { return ((r & 1) << 2) | (r & 2) | ((r >> 2) & 1); }
