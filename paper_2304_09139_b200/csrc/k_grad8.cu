@@ -110,7 +110,10 @@ __device__ __forceinline__ dd acc192_to_dd(acc192 g, int e) {
 }
 
 // ND = 13: full precision; 7 / 4: the most significant digits only (shd_set_precision 2 / 1; see k_rho8.cu)
-template <int ND>
+// D = the dimension d: the epilogue is bound by instruction issue (about 1500 instructions per thread and block), so the
+// per-axis accumulations exist only for the axes there are: axis a < NI takes I w_a[p] (NI = d - 1 prefix axes; d = 1: the one
+// axis, split as n = S p + q), axis d - 1 takes R 2^qscale
+template <int ND, int D>
 __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
     int d, long N, long Npad, long njb128, int Ppad, int qscale_log2, int nkq,
     const int2* __restrict__ steps, int nsteps, int nseg, const int* __restrict__ wT,
@@ -264,7 +267,10 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
         const int c_begin = (int)((long)nsteps * seg / nseg), total = (int)((long)nsteps * (seg + 1) / nseg) - c_begin;
         const long j = jb * 128 + row;
         const ulonglong2* Aj = Afix + (size_t)j * 2;
-        acc192 g[4] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+        constexpr int NI = D == 1 ? 1 : D - 1;
+        acc192 g[D];
+#pragma unroll
+        for (int ax = 0; ax < D; ax++) g[ax] = acc192{0, 0, 0};
         // next block (or segment) end at or after step i: 32 steps per look, one load latency per block
         auto next_end = [&](int& i, int2& st) {
             for (;;) {
@@ -289,7 +295,7 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
             // this block's A_j[p] (sign-magnitude integers trunc(a 2^102), k_tables) and axis weights, requested before
             // the wait for the tensor core
             ulonglong2 ar[2], ai[2];
-            int wg[2][3];
+            int wg[2][NI];
 #pragma unroll
             for (int pp = 0; pp < 2; pp++) {
                 const int p = pb8 * 8 + quarter * 2 + pp;             // < Ppad8 (the table is allocated and zeroed up to there)
@@ -297,7 +303,7 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
                 asm volatile("ld.global.nc.v2.u64 {%0,%1}, [%2];" : "=l"(ar[pp].x), "=l"(ar[pp].y) : "l"(ap));
                 asm volatile("ld.global.nc.v2.u64 {%0,%1}, [%2];" : "=l"(ai[pp].x), "=l"(ai[pp].y) : "l"(ap + 1));
 #pragma unroll
-                for (int ax = 0; ax < 3; ax++) wg[pp][ax] = (ax < d && p < Ppad) ? wT[ax * Ppad + p] : 0;
+                for (int ax = 0; ax < NI; ax++) wg[pp][ax] = p < Ppad ? wT[ax * Ppad + p] : 0;
             }
             mbar_wait(smem_u32(&tfull_bar), (uint32_t)(nblock & 1));
             asm volatile("tcgen05.fence::after_thread_sync;");
@@ -379,7 +385,7 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
                 mul_shr96<HI>(T0[2], T1[2], ar0, ar1, r0, r1, r2); acc_addsub(R, r0, r1, r2, arn != TN[2]);
                 mul_shr96<HI>(T0[3], T1[3], ai0, ai1, r0, r1, r2); acc_addsub(R, r0, r1, r2, ain != TN[3]);
 #pragma unroll
-                for (int ax = 0; ax < 3; ax++) {
+                for (int ax = 0; ax < NI; ax++) {
                     const int wgt = wg[pp][ax];
                     if (wgt != 0) {
                         acc192 v = I;
@@ -387,9 +393,7 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
                         acc_mac(g[ax], v, (uint32_t)(wgt < 0 ? -wgt : wgt));
                     }
                 }
-#pragma unroll
-                for (int ax = 0; ax < 4; ax++)
-                    if (ax == d - 1) acc_mac(g[ax], R, 1u << qscale_log2);
+                acc_mac(g[D - 1], R, 1u << qscale_log2);
             }
             nblock++;
             i = inext;
@@ -398,13 +402,12 @@ __global__ void __launch_bounds__(G8_THREADS, 1) k_grad8(
         if (j < N) {
             constexpr int E0 = 8 * (ND - 1 + 2 * OFF) - 210;      // units of the accumulators: 2^(8 s0 - 204 - 102 + 96)
             double2* o = reinterpret_cast<double2*>(gpart);
-            const size_t slot = (size_t)(seg * 4 + quarter) * d;       // four partials per segment (the p quarters)
+            const size_t slot = (size_t)(seg * 4 + quarter) * D;       // four partials per segment (the p quarters)
 #pragma unroll
-            for (int ax = 0; ax < 4; ax++)
-                if (ax < d) {
-                    const dd r = acc192_to_dd(g[ax], E0);
-                    o[(slot + ax) * N + j] = make_double2(r.h, r.l);
-                }
+            for (int ax = 0; ax < D; ax++) {
+                const dd r = acc192_to_dd(g[ax], E0);
+                o[(slot + ax) * N + j] = make_double2(r.h, r.l);
+            }
         }
       }
     }
@@ -419,12 +422,19 @@ cudaError_t shd_grad8_configure()
 {
     if (getenv("SHD_DEBUG")) {
         cudaFuncAttributes a;
-        cudaFuncGetAttributes(&a, k_grad8<13>);
-        fprintf(stderr, "k_grad8<13>: regs %d maxThreadsPerBlock %d static smem %zu local %zu\n", a.numRegs, a.maxThreadsPerBlock, a.sharedSizeBytes, a.localSizeBytes);
+        cudaFuncGetAttributes(&a, k_grad8<13, 2>);
+        fprintf(stderr, "k_grad8<13, 2>: regs %d maxThreadsPerBlock %d static smem %zu local %zu\n", a.numRegs, a.maxThreadsPerBlock, a.sharedSizeBytes, a.localSizeBytes);
     }
-    cudaError_t e = cudaFuncSetAttribute(k_grad8<13>, cudaFuncAttributeMaxDynamicSharedMemorySize, G8_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad8<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, G8_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad8<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, G8_SMEM);
+    cudaError_t e = cudaSuccess;
+#define CONF_GRAD8(NDV)                                                                                                       \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad8<NDV, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, G8_SMEM);    \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad8<NDV, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, G8_SMEM);    \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad8<NDV, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, G8_SMEM);    \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_grad8<NDV, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, G8_SMEM);
+    CONF_GRAD8(13)
+    CONF_GRAD8(7)
+    CONF_GRAD8(4)
+#undef CONF_GRAD8
     return e;
 }
 
@@ -433,15 +443,23 @@ cudaError_t shd_launch_grad8_main(shd_ctx* h, long nc)
 {
     const long njb = (nc + 127) / 128, nunits = njb * h->nseg8;
     const unsigned grid = (unsigned)std::min<long>(nunits, h->sms);        // persistent: one CTA per SM
-#define LAUNCH_GRAD8(NDV)                                                                            \
-    k_grad8<NDV><<<grid, G8_THREADS, G8_SMEM, h->stream>>>(                                                  \
+#define LAUNCH_GRAD8_(NDV, DV)                                                                       \
+    k_grad8<NDV, DV><<<grid, G8_THREADS, G8_SMEM, h->stream>>>(                                              \
         h->d, nc, h->Npad, h->njb128, h->npb * 32, h->qscale_log2, h->nkq8,                            \
         reinterpret_cast<const int2*>(h->d_steps8), h->nsteps8, h->nseg8, h->d_wT,                     \
         reinterpret_cast<const ulonglong2*>(h->d_Afix), h->d_Bg8, h->d_W8, h->d_gpart, nunits, h->d_scal->clk + 2, h->d_skip)
+#define LAUNCH_GRAD8(NDV)                                                                            \
+    do {                                                                                             \
+        if (h->d == 1) LAUNCH_GRAD8_(NDV, 1);                                                        \
+        else if (h->d == 2) LAUNCH_GRAD8_(NDV, 2);                                                   \
+        else if (h->d == 3) LAUNCH_GRAD8_(NDV, 3);                                                   \
+        else LAUNCH_GRAD8_(NDV, 4);                                                                  \
+    } while (0)
     if (h->nlimb >= 3) LAUNCH_GRAD8(13);
     else if (h->nlimb == 2) LAUNCH_GRAD8(7);
     else LAUNCH_GRAD8(4);
 #undef LAUNCH_GRAD8
+#undef LAUNCH_GRAD8_
     h->last_launches += 1;
     return cudaGetLastError();
 }
