@@ -584,3 +584,30 @@ def test_structure_factor_shells(shd, oracle):
     _, _, s_hi, s_lo = h.structure_factor_shells()
     assert np.abs(s_hi + s_lo - cfg.N).max() <= 1e-24 * cfg.N
     h.close()
+
+
+@pytest.mark.parametrize("d,N,L,m_star,seed", [
+    (2, 3000, 55.0, 40 * 40, 21), (3, 700, 9.0, 12 * 12, 22), (1, 900, 900.0, 300 * 300, 23), (4, 81, 3.0, 3, 24),
+])
+def test_table_specialisations_agree(shd, d, N, L, m_star, seed):
+    """k_tables is a template on (limb tables written?, d >= 3?): engine 1 (INT8 rho pass + FP64 gradient pass) writes
+    limb AND digit tables in one launch, engine 2 only digit tables, and both feed the same k_rho8.  The digits must
+    not depend on the specialisation: rho, Phi and S_max are bit-identical between the two engines (the gradient comes
+    from different kernels and agrees at the double-double level, checked elsewhere)."""
+    import torch
+    hi, lo = inputs.uniform_positions_raw(d, N, L, seed)
+    lo = inputs.jitter_lo(hi, seed + 1)
+    h = shd.Shd(d, N, L, m_star=m_star)
+    th, tl = shd.from_host(hi, lo)
+    h.set_engine(1)
+    phi1, _, _ = h.energy_grad(th, tl)
+    rho1 = [x.clone() for x in h.rho()]
+    s1 = h.last_smax()
+    h.set_engine(2)
+    phi2, _, _ = h.energy_grad(th, tl)
+    rho2 = [x.clone() for x in h.rho()]
+    s2 = h.last_smax()
+    assert phi1 == phi2 and s1 == s2
+    for a, b in zip(rho1, rho2):
+        assert torch.equal(a, b)
+    h.close()
